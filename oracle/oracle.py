@@ -1,0 +1,147 @@
+"""ctypes binding of oracle/hprmat_oracle.c (numpy in, numpy out).  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Every function cites the passage of /root/reference/PAPER.md it follows in hprmat_oracle.c.  Arrays are column-major
+(Fortran order) complex128 unless stated.  V has shape (nb, nch, nch) C-order with V[i, c2, c1] = V_{c1 c2}(r_i).
+"""
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def _L():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.orc_num_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def num_threads() -> int:
+    return int(_L().orc_num_threads())
+
+
+def mesh(nb: int, a: float):
+    """Gauss-Legendre mesh on (0,a).  Returns x (on (0,1), ascending), lam (weights on (0,1)),
+    r = a*x, fa = f_i(a) (the paper's q2(r_i))."""
+    x, lam, r, fa = (np.zeros(nb) for _ in range(4))
+    rc = _L().orc_mesh(C.c_int(nb), C.c_double(a), _p(x), _p(lam), _p(r), _p(fa))
+    if rc:
+        raise ValueError(f"orc_mesh rc={rc}")
+    return x, lam, r, fa
+
+
+def kinetic(nb: int, a: float, x: np.ndarray) -> np.ndarray:
+    """kinetic + Bloch matrix T (nb x nb, units hbar^2/2mu = 1)."""
+    T = np.zeros((nb, nb), order="F")
+    rc = _L().orc_kinetic(C.c_int(nb), C.c_double(a), _p(np.ascontiguousarray(x)), _p(T))
+    if rc:
+        raise ValueError(f"orc_kinetic rc={rc}")
+    return T
+
+
+def _chan(lval, ethr):
+    lv = np.ascontiguousarray(lval, dtype=np.int32)
+    et = np.ascontiguousarray(ethr, dtype=np.float64)
+    return lv, et
+
+
+def assemble(nch, nb, a, h2m, lval, ethr, energy, V) -> np.ndarray:
+    """PAPER.md:87-99 Eqs. (3),(4) with Eq. (1)'s diagonal terms -- C - E*I, N x N column-major."""
+    lv, et = _chan(lval, ethr)
+    V = np.ascontiguousarray(V, dtype=np.complex128)
+    assert V.shape == (nb, nch, nch)
+    N = nch * nb
+    Cm = np.zeros((N, N), dtype=np.complex128, order="F")
+    rc = _L().orc_assemble(C.c_int(nch), C.c_int(nb), C.c_double(a), C.c_double(h2m), _p(lv), _p(et),
+                           C.c_double(energy), _p(V), _p(Cm))
+    if rc:
+        raise ValueError(f"orc_assemble rc={rc}")
+    return Cm
+
+
+def rhs(nch, nb, fa) -> np.ndarray:
+    """B[(c,i), c'] = fa_i delta_cc'."""
+    N = nch * nb
+    B = np.zeros((N, nch), dtype=np.complex128, order="F")
+    _L().orc_rhs(C.c_int(nch), C.c_int(nb), _p(np.ascontiguousarray(fa)), _p(B))
+    return B
+
+
+def solve(A, B, mode: int = 0, nrefine: int = 2, return_ipiv: bool = False):
+    """PAPER.md:125-137 Eq. (5) -- dense A X = B by Crout LU with partial pivoting, accumulated dot products."""
+    A = np.asfortranarray(A, dtype=np.complex128)
+    B = np.asfortranarray(B, dtype=np.complex128)
+    if B.ndim == 1:
+        B = B.reshape(-1, 1, order="F")
+    n, nrhs = A.shape[0], B.shape[1]
+    assert A.shape == (n, n) and B.shape[0] == n
+    X = np.zeros((n, nrhs), dtype=np.complex128, order="F")
+    ipiv = np.zeros(max(n, 1), dtype=np.int32)
+    rc = _L().orc_solve(C.c_int(n), C.c_int(nrhs), _p(A), _p(B), _p(X), _p(ipiv), C.c_int(mode), C.c_int(nrefine))
+    if rc < 0:
+        raise ValueError(f"orc_solve rc={rc}")
+    if rc > 0:
+        raise ZeroDivisionError(f"orc_solve: zero pivot at step {rc}")
+    return (X, ipiv[:n]) if return_ipiv else X
+
+
+def structured_residual(nch, nb, a, h2m, lval, ethr, energy, V, X, B=None) -> np.ndarray:
+    """B - (C - E I) X in long double from the block structure of Eqs. (3),(4)."""
+    lv, et = _chan(lval, ethr)
+    V = np.ascontiguousarray(V, dtype=np.complex128)
+    X = np.asfortranarray(X, dtype=np.complex128)
+    N = nch * nb
+    nrhs = X.shape[1]
+    assert X.shape[0] == N
+    Bp = None
+    if B is not None:
+        B = np.asfortranarray(B, dtype=np.complex128)
+        assert B.shape == X.shape
+        Bp = _p(B)
+    Rr = np.zeros((N, nrhs), dtype=np.complex128, order="F")
+    rc = _L().orc_structured_residual(C.c_int(nch), C.c_int(nb), C.c_double(a), C.c_double(h2m), _p(lv), _p(et),
+                                      C.c_double(energy), _p(V), C.c_int(nrhs), Bp, _p(X), _p(Rr))
+    if rc:
+        raise ValueError(f"orc_structured_residual rc={rc}")
+    return Rr
+
+
+def contract(nch, nb, a, h2m, fa, X) -> np.ndarray:
+    """PAPER.md:137 step 4 (+ BASELINE.json prefactor) -- R = (h2m/a) B^T X."""
+    X = np.asfortranarray(X, dtype=np.complex128)
+    R = np.zeros((nch, nch), dtype=np.complex128, order="F")
+    _L().orc_contract(C.c_int(nch), C.c_int(nb), C.c_double(a), C.c_double(h2m), _p(np.ascontiguousarray(fa)),
+                      _p(X), _p(R))
+    return R
+
+
+def rmatrix(nch, nb, a, h2m, lval, ethr, energy, V, mode: int = 0, nrefine: int = 2, return_x=False,
+            return_seconds=False):
+    """Whole chain: mesh -> T -> C - E I -> LU -> solves -> refinement -> R."""
+    lv, et = _chan(lval, ethr)
+    V = np.ascontiguousarray(V, dtype=np.complex128)
+    assert V.shape == (nb, nch, nch)
+    N = nch * nb
+    R = np.zeros((nch, nch), dtype=np.complex128, order="F")
+    X = np.zeros((N, nch), dtype=np.complex128, order="F")
+    sec = C.c_double(0.0)
+    rc = _L().orc_rmatrix(C.c_int(nch), C.c_int(nb), C.c_double(a), C.c_double(h2m), _p(lv), _p(et),
+                          C.c_double(energy), _p(V), C.c_int(mode), C.c_int(nrefine), _p(R), _p(X), C.byref(sec))
+    if rc < 0:
+        raise ValueError(f"orc_rmatrix rc={rc}")
+    if rc > 0:
+        raise ZeroDivisionError(f"orc_rmatrix: zero pivot at step {rc}")
+    out = [R]
+    if return_x:
+        out.append(X)
+    if return_seconds:
+        out.append(sec.value)
+    return out[0] if len(out) == 1 else tuple(out)

@@ -1,0 +1,404 @@
+"""Pins of the CPU oracle (oracle/) against things OTHER than itself: library quadrature, exact polynomial integrals in
+mpmath, Cramer's rule / Gauss-Jordan on tiny systems, closed-form R-matrices, symmetry and unitarity.
+All CPU-only ("-m 'not gpu'").  Each test names the passage of PAPER.md whose step it pins.
+"""
+import itertools
+
+import mpmath as mp
+import numpy as np
+import pytest
+
+import oracle
+from paper_2512_11590_b200.workloads import H2M, make_workload
+from scatter import R_constant_potential, smatrix
+
+# ---------------------------------------------------------------------------------------------------- mesh
+
+
+@pytest.mark.parametrize("nb", [1, 2, 5, 8, 50, 100])
+def test_mesh_matches_library_gauss_legendre(nb):
+    x, lam, r, fa = oracle.mesh(nb, 7.5)
+    t, w = np.polynomial.legendre.leggauss(nb)
+    assert np.allclose(x, (1 + t) / 2, rtol=0, atol=2e-16 * 4)
+    assert np.allclose(lam, w / 2, rtol=5e-12, atol=0)   # numpy weights are plain double
+    assert np.allclose(r, 7.5 * x, rtol=3e-16, atol=0)
+    assert np.all(np.diff(x) > 0)
+    assert np.allclose(x + x[::-1], 1.0, atol=4e-16)
+
+
+@pytest.mark.parametrize("nb", [3, 10, 50])
+def test_mesh_quadrature_exact_to_degree_2nb_minus_1(nb):
+    x, lam, _, _ = oracle.mesh(nb, 1.0)
+    assert abs(lam.sum() - 1.0) < 5e-16 * nb
+    for k in range(0, 2 * nb, max(1, nb // 5)):
+        assert abs(np.sum(lam * x ** k) - 1.0 / (k + 1)) < 1e-14
+
+
+# ---------------------------------------------------- basis values and kinetic + Bloch table
+
+def _lagrange_functions(nb, a, dps=50):
+    """f_i(r) = (r / r_i) prod_{j != i} (r - r_j)/(r_i - r_j) / sqrt(a lam_i): the polynomial of degree nb that vanishes
+    at r = 0, satisfies the Lagrange property f_i(r_j) = delta_ij / sqrt(lambda_j) (lambda_j = a lam_j on
+    (0,a)).  Coefficients in mpmath from mpmath's OWN Gauss-Legendre nodes (not the oracle's)."""
+    mp.mp.dps = dps
+    nodes = sorted(mp.polyroots([mp.mpf(c) for c in mp.taylor(lambda t: mp.legendre(nb, t), 0, nb)[::-1]],
+                                maxsteps=500, extraprec=400))
+    xs = [(1 + t) / 2 for t in nodes]
+    rs = [mp.mpf(a) * xx for xx in xs]
+    lams = []
+    for t in nodes:
+        dp = mp.diff(lambda s: mp.legendre(nb, s), t)
+        lams.append(1 / ((1 - t * t) * dp * dp))          # weight on (0,1): (2/((1-t^2)P'^2))/2
+    polys = []
+    for i in range(nb):
+        c = [mp.mpf(1)]                                   # ascending coefficients
+        for j in range(nb):
+            if j == i:
+                continue
+            c = [(c[k - 1] if k >= 1 else 0) - rs[j] * (c[k] if k < len(c) else 0) for k in range(len(c) + 1)]
+            den = rs[i] - rs[j]
+            c = [v / den for v in c]
+        c = [mp.mpf(0)] + c                               # multiply by r
+        scale = 1 / (rs[i] * mp.sqrt(mp.mpf(a) * lams[i]))
+        polys.append([v * scale for v in c])
+    return xs, lams, polys
+
+
+def _polyval(c, r):
+    return sum(v * r ** k for k, v in enumerate(c))
+
+
+def _polyder(c):
+    return [k * v for k, v in enumerate(c)][1:]
+
+
+def _polyint(c, lo, hi):
+    return sum(v * (hi ** (k + 1) - lo ** (k + 1)) / (k + 1) for k, v in enumerate(c))
+
+
+def _polymul(p, q):
+    out = [mp.mpf(0)] * (len(p) + len(q) - 1)
+    for i, a_ in enumerate(p):
+        for j, b_ in enumerate(q):
+            out[i + j] += a_ * b_
+    return out
+
+
+@pytest.mark.parametrize("nb,a", [(2, 1.0), (4, 10.0), (7, 3.5), (8, 20.0)])
+def test_surface_values_and_kinetic_bloch_table_from_lagrange_polynomials(nb, a):
+    xs, lams, polys = _lagrange_functions(nb, a)
+    x, lam, r, fa = oracle.mesh(nb, a)
+    T = oracle.kinetic(nb, a, x)
+    assert np.allclose(x, [float(v) for v in xs], atol=4e-16)
+    # q2(r_i) = f_i(a)
+    fa_ref = np.array([float(_polyval(p, mp.mpf(a))) for p in polys])
+    assert np.allclose(fa, fa_ref, rtol=1e-13)
+    # <f_i| -d2/dr2 + delta(r-a) d/dr |f_j> = int_0^a f_i' f_j' dr   (f_i(0) = 0), exact polynomial integral
+    Tref = np.zeros((nb, nb))
+    for i in range(nb):
+        for j in range(nb):
+            Tref[i, j] = float(_polyint(_polymul(_polyder(polys[i]), _polyder(polys[j])), mp.mpf(0), mp.mpf(a)))
+    assert np.allclose(T, Tref, rtol=1e-12, atol=1e-12 * np.abs(Tref).max())
+    assert np.array_equal(T, T.T)
+    # the same matrix element written the other way: -int f_i f_j'' + f_i(a) f_j'(a)
+    i, j = 0, nb - 1
+    d2 = _polyder(_polyder(polys[j]))
+    alt = -_polyint(_polymul(polys[i], d2), mp.mpf(0), mp.mpf(a)) + _polyval(polys[i], mp.mpf(a)) * _polyval(
+        _polyder(polys[j]), mp.mpf(a))
+    assert abs(float(alt) - T[i, j]) < 1e-12 * np.abs(Tref).max()
+
+
+def test_lagrange_property_of_reference_polynomials():
+    """Sanity of the test's own reference: f_i(r_j) = delta_ij / sqrt(a lam_j), orthonormal at Gauss accuracy."""
+    nb, a = 5, 2.0
+    xs, lams, polys = _lagrange_functions(nb, a)
+    for i in range(nb):
+        for j in range(nb):
+            v = _polyval(polys[i], a * xs[j])
+            ref = (1 / mp.sqrt(a * lams[j])) if i == j else 0
+            assert abs(v - ref) < mp.mpf(10) ** -30
+
+
+# ----------------------------------------------------------------- assembly structure (PAPER.md:87-99 Eqs. 3,4; :137)
+
+def _small_system(nch=3, nb=4, seed=5, symmetric=False):
+    rng = np.random.default_rng(seed)
+    a, h2m = 6.0, 11.0
+    lval = np.array([2, 0, 1][:nch], dtype=np.int32)
+    ethr = np.array([0.0, 0.7, 1.9][:nch])
+    V = rng.normal(size=(nb, nch, nch)) + 1j * rng.normal(size=(nb, nch, nch))
+    if symmetric:
+        V = (V + V.transpose(0, 2, 1)) / 2
+    return a, h2m, lval, ethr, V
+
+
+def test_assemble_block_structure_and_index_convention():
+    nch, nb, E = 3, 4, 2.5
+    a, h2m, lval, ethr, V = _small_system(nch, nb)
+    C = oracle.assemble(nch, nb, a, h2m, lval, ethr, E, V)
+    x, lam, r, fa = oracle.mesh(nb, a)
+    T = oracle.kinetic(nb, a, x)
+    for c1, c2 in itertools.product(range(nch), repeat=2):
+        blk = C[c1 * nb:(c1 + 1) * nb, c2 * nb:(c2 + 1) * nb]       # row = i + c*nb (PAPER.md:137 step 4)
+        if c1 != c2:
+            # Eq. (4): D_cc' diagonal with V_cc'(r_i); V[i, c2, c1] = V_{c1 c2}(r_i)
+            assert np.array_equal(blk, np.diag(V[:, c2, c1]))
+        else:
+            off = blk - np.diag(np.diag(blk))
+            assert np.array_equal(off, h2m * (T - np.diag(np.diag(T))))
+            want = h2m * np.diag(T) + h2m * lval[c1] * (lval[c1] + 1) / r ** 2 + (ethr[c1] - E) + V[:, c1, c1]
+            assert np.allclose(np.diag(blk), want, rtol=1e-15)
+    # energy enters as -E on the whole diagonal and nowhere else (C - E I)
+    C0 = oracle.assemble(nch, nb, a, h2m, lval, ethr, 0.0, V)
+    assert np.allclose(C0 - C, E * np.eye(nch * nb), atol=1e-12)
+
+
+def test_rhs_layout():
+    nch, nb = 3, 4
+    _, _, _, fa = oracle.mesh(nb, 6.0)
+    B = oracle.rhs(nch, nb, fa)
+    for c in range(nch):
+        col = np.zeros(nch * nb)
+        col[c * nb:(c + 1) * nb] = fa
+        assert np.array_equal(B[:, c], col)
+
+
+# ----------------------------------------------------------------- LU / solve (Eq. 5)
+
+def _cramer(A, b):
+    mp.mp.dps = 40
+    n = A.shape[0]
+    Am = mp.matrix(n, n)
+    for i in range(n):
+        for j in range(n):
+            Am[i, j] = mp.mpc(A[i, j])
+
+    def det(M):  # cofactor expansion, written out (no LU inside)
+        m = M.rows
+        if m == 1:
+            return M[0, 0]
+        s = mp.mpc(0)
+        for j in range(m):
+            minor = mp.matrix(m - 1, m - 1)
+            for ii in range(1, m):
+                cc = 0
+                for jj in range(m):
+                    if jj == j:
+                        continue
+                    minor[ii - 1, cc] = M[ii, jj]
+                    cc += 1
+            s += (-1) ** j * M[0, j] * det(minor)
+        return s
+
+    d = det(Am)
+    x = []
+    for k in range(n):
+        Ak = Am.copy()
+        for i in range(n):
+            Ak[i, k] = mp.mpc(b[i])
+        x.append(complex(det(Ak) / d))
+    return np.array(x)
+
+
+def _gauss_jordan_inverse(A):
+    mp.mp.dps = 40
+    n = A.shape[0]
+    M = [[mp.mpc(A[i, j]) for j in range(n)] + [mp.mpc(1 if i == j else 0) for j in range(n)] for i in range(n)]
+    for c in range(n):
+        p = max(range(c, n), key=lambda rr: abs(M[rr][c]))
+        M[c], M[p] = M[p], M[c]
+        pv = M[c][c]
+        M[c] = [v / pv for v in M[c]]
+        for rr in range(n):
+            if rr != c:
+                f = M[rr][c]
+                M[rr] = [v - f * w for v, w in zip(M[rr], M[c])]
+    return np.array([[complex(M[i][n + j]) for j in range(n)] for i in range(n)])
+
+
+@pytest.mark.parametrize("n,seed", [(1, 0), (2, 1), (3, 2), (5, 3), (7, 4)])
+@pytest.mark.parametrize("mode,nrefine", [(0, 0), (1, 0), (0, 2)])
+def test_solve_against_cramers_rule(n, seed, mode, nrefine):
+    rng = np.random.default_rng(seed)
+    A = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    A[0, 0] = 0.0                                            # forces a row interchange at step 0 when n > 1
+    if n == 1:
+        A[0, 0] = 0.3 - 2j
+    B = rng.normal(size=(n, 2)) + 1j * rng.normal(size=(n, 2))
+    X = oracle.solve(A, B, mode=mode, nrefine=nrefine)
+    for q in range(2):
+        assert np.allclose(X[:, q], _cramer(A, B[:, q]), rtol=1e-12, atol=1e-13)
+
+
+@pytest.mark.parametrize("n", [4, 8])
+def test_solve_against_explicit_gauss_jordan_inverse(n):
+    rng = np.random.default_rng(100 + n)
+    A = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    B = rng.normal(size=(n, 3)) + 1j * rng.normal(size=(n, 3))
+    X = oracle.solve(A, B, nrefine=0)
+    assert np.allclose(X, _gauss_jordan_inverse(A) @ B, rtol=1e-12, atol=1e-13)
+
+
+def test_solve_pivots_are_valid_and_first_max():
+    rng = np.random.default_rng(9)
+    n = 40
+    A = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    X, ipiv = oracle.solve(A, np.eye(n, dtype=complex), nrefine=0, return_ipiv=True)
+    assert np.all(ipiv >= np.arange(n)) and np.all(ipiv < n)
+    col0 = np.abs(A[:, 0].real) + np.abs(A[:, 0].imag)
+    assert ipiv[0] == int(np.argmax(col0))
+    assert np.allclose(A @ X, np.eye(n), atol=1e-11)
+
+
+def test_solve_singular_matrix_is_reported():
+    A = np.array([[1, 2], [2, 4]], dtype=complex)
+    with pytest.raises(ZeroDivisionError):
+        oracle.solve(A, np.ones((2, 1), dtype=complex))
+
+
+@pytest.mark.parametrize("n", [64, 300])
+def test_manufactured_solution_x_equals_one(n):
+    """PAPER.md:563 (Table 7 caption): x_exact = 1, b = A 1."""
+    rng = np.random.default_rng(n)
+    A = rng.uniform(-1, 1, size=(n, n)) + 1j * rng.uniform(-1, 1, size=(n, n)) + np.sqrt(n) * np.eye(n)
+    b = A @ np.ones((n, 1))
+    for mode in (0, 1):
+        X = oracle.solve(A, b, mode=mode, nrefine=2)
+        assert np.abs(X - 1).max() < 1e-14
+
+
+def test_structured_residual_equals_dense_residual():
+    nch, nb, E = 3, 6, 1.3
+    a, h2m, lval, ethr, V = _small_system(nch, nb, seed=11)
+    C = oracle.assemble(nch, nb, a, h2m, lval, ethr, E, V)
+    rng = np.random.default_rng(0)
+    X = np.asfortranarray(rng.normal(size=(nch * nb, nch)) + 1j * rng.normal(size=(nch * nb, nch)))
+    _, _, _, fa = oracle.mesh(nb, a)
+    B = oracle.rhs(nch, nb, fa)
+    r1 = oracle.structured_residual(nch, nb, a, h2m, lval, ethr, E, V, X)
+    r2 = B - np.asarray(C, dtype=np.clongdouble) @ np.asarray(X, dtype=np.clongdouble)
+    assert np.allclose(r1, r2.astype(complex), rtol=0, atol=1e-13 * np.abs(C).max())
+    Bx = np.asfortranarray(rng.normal(size=X.shape) + 0j)
+    r3 = oracle.structured_residual(nch, nb, a, h2m, lval, ethr, E, V, X, B=Bx)
+    assert np.allclose(r3 - r1, Bx - B, atol=1e-12 * np.abs(C).max())
+
+
+# ----------------------------------------------------------------- whole chain: closed forms
+
+@pytest.mark.parametrize("l", [0, 1, 2, 3])
+def test_free_particle_R_matrix_and_zero_phase_shift(l):
+    """V = 0: R = F_l(ka)/(ka F_l'(ka)), S = 1, phase shift 0."""
+    nb, a, E = 30, 10.0, 10.0
+    k = np.sqrt(E / H2M)
+    V = np.zeros((nb, 1, 1), dtype=complex)
+    R = oracle.rmatrix(1, nb, a, H2M, [l], [0.0], E, V)
+    want = R_constant_potential(l, k, a)
+    assert abs(R[0, 0] - want) < 1e-11 * abs(want)
+    S = smatrix(R, [l], np.array([k]), a)
+    assert abs(S[0, 0] - 1.0) < 1e-10
+    assert abs(0.5 * np.angle(S[0, 0])) < 1e-10
+
+
+def test_square_well_phase_shift_converges_with_nb():
+    """Constant well of depth V0 filling (0,a), l = 0: R = tan(Ka)/(Ka), tan(ka + delta) = (k/K) tan(Ka).
+    Error falls exponentially with nb (Gauss quadrature is exact for the polynomial basis)."""
+    a, E, V0 = 10.0, 10.0, 50.0
+    k, K = np.sqrt(E / H2M), np.sqrt((E + V0) / H2M)
+    Rex = np.tan(K * a) / (K * a)
+    delta_ex = np.arctan((k / K) * np.tan(K * a)) - k * a
+    errs = []
+    for nb in (10, 15, 20, 25):
+        V = np.full((nb, 1, 1), -V0, dtype=complex)
+        R = oracle.rmatrix(1, nb, a, H2M, [0], [0.0], E, V)
+        errs.append(abs(R[0, 0] - Rex) / abs(Rex))
+        S = smatrix(R, [0], np.array([k]), a)
+        d = 0.5 * np.angle(S[0, 0])
+        derr = abs(np.exp(2j * d) - np.exp(2j * delta_ex))
+        if nb >= 20:
+            assert derr < 1e-9
+    assert errs[0] > 1e-3 and errs[1] < errs[0] * 1e-2 and errs[2] < 1e-9 and errs[3] < 1e-10
+
+
+def test_uncoupled_channels_with_thresholds_and_complex_well():
+    """Diagonal V: every channel is an independent constant-potential problem with its own l_c and E - E_c (the
+    threshold enters as +E_c on the diagonal); absorptive (complex) wells and a CLOSED channel included."""
+    nb, a, E = 40, 8.0, 6.0
+    lval = [0, 2, 1, 3]
+    ethr = [0.0, 1.5, 3.0, 9.0]                                 # last channel closed (E < E_c)
+    depth = [30.0 + 5j, 12.0, 0.0, 20.0 + 1j]
+    V = np.zeros((nb, 4, 4), dtype=complex)
+    for c in range(4):
+        V[:, c, c] = -depth[c]
+    R = oracle.rmatrix(4, nb, a, H2M, lval, ethr, E, V)
+    assert np.abs(R - np.diag(np.diag(R))).max() == 0.0
+    for c in range(4):
+        K = np.sqrt(complex((E - ethr[c] + depth[c]) / H2M))
+        want = R_constant_potential(lval[c], K, a)
+        assert abs(R[c, c] - want) < 2e-10 * abs(want), c
+
+
+def test_constant_nonsymmetric_coupling_matrix_pins_channel_index_order():
+    """All channels share l and threshold, V(r) = W constant and NON-symmetric, W = P diag(w) P^-1.  Then the system
+    decouples in the eigenbasis: R = P diag(R_l(K_m)) P^-1 with K_m = sqrt((E - w_m)/h2m).  A transposed V index
+    (c1 <-> c2) would give R^T instead."""
+    nb, a, E, l = 40, 8.0, 6.0, 1
+    rng = np.random.default_rng(3)
+    P = rng.normal(size=(3, 3)) + 2 * np.eye(3)
+    w = np.array([-20.0 - 3j, -5.0, 1.0 - 0.5j])
+    W = P @ np.diag(w) @ np.linalg.inv(P)
+    V = np.empty((nb, 3, 3), dtype=complex)
+    V[:] = W.T[None]                                             # V[i, c2, c1] = W[c1, c2]
+    R = oracle.rmatrix(3, nb, a, H2M, [l] * 3, [0.0] * 3, E, V)
+    Rm = np.array([R_constant_potential(l, np.sqrt(complex((E - wm) / H2M)), a) for wm in w])
+    want = P @ np.diag(Rm) @ np.linalg.inv(P)
+    assert np.abs(R - want).max() < 1e-9 * np.abs(want).max()
+    assert np.abs(R - want.T).max() > 1e-3 * np.abs(want).max()
+
+
+# ----------------------------------------------------------------- whole chain: invariants at config 0
+
+def test_cfg0_R_symmetric_and_S_subunitary_and_big_n_mode_agrees():
+    w = make_workload(0)
+    x, lam, r, fa = oracle.mesh(w.nb, w.a)
+    V = w.potential(r)
+    E = float(w.energies[0])
+    R = oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, V)
+    assert np.abs(R - R.T).max() < 1e-13 * np.abs(R).max()       # C = C^T  =>  R = R^T
+    k = np.sqrt((E - w.ethr) / w.h2m)
+    S = smatrix(R, w.lval, k, w.a)
+    assert np.abs(S - S.T).max() < 1e-11
+    sv = np.linalg.svd(S, compute_uv=False)
+    assert sv.max() < 1.0                                        # W0 > 0: absorption
+    R1 = oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, V, mode=1)
+    assert np.abs(R1 - R).max() < 1e-13 * np.abs(R).max()        # big-N mode validation
+
+
+def test_cfg0_real_potential_gives_unitary_S():
+    w = make_workload(0)
+    w.W0 = 0.0
+    x, lam, r, fa = oracle.mesh(w.nb, w.a)
+    V = w.potential(r)
+    E = float(w.energies[0])
+    R = oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, V)
+    assert np.abs(R.imag).max() < 1e-13 * np.abs(R).max()
+    S = smatrix(R, w.lval, np.sqrt((E - w.ethr) / w.h2m), w.a)
+    assert np.abs(S.conj().T @ S - np.eye(w.nch)).max() < 1e-11
+
+
+def test_rmatrix_equals_definition_via_dense_solve_and_certificate():
+    """R = (h2m/a) B^T (C - E)^-1 B computed the long way (assemble -> dense solve -> contract) equals orc_rmatrix, and
+    the a-posteriori certificate (h2m/a) X^T (B - C X) of SURVEY 8(c) is ~0 for the oracle's own X."""
+    w = make_workload(0, nch=3, nb=20)
+    x, lam, r, fa = oracle.mesh(w.nb, w.a)
+    V = w.potential(r)
+    E = 7.0
+    R, X = oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, V, return_x=True)
+    C = oracle.assemble(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, V)
+    B = oracle.rhs(w.nch, w.nb, fa)
+    X2 = oracle.solve(C, B, nrefine=2)
+    R2 = oracle.contract(w.nch, w.nb, w.a, w.h2m, fa, X2)
+    assert np.abs(R2 - R).max() < 1e-14 * np.abs(R).max()
+    assert np.allclose(R2, (w.h2m / w.a) * B.T @ X2, rtol=1e-13, atol=1e-16)
+    res = oracle.structured_residual(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, V, X)
+    cert = (w.h2m / w.a) * X.T @ res
+    assert np.abs(cert).max() < 1e-13 * np.abs(R).max()
