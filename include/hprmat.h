@@ -1,0 +1,140 @@
+/*
+ * hprmat.h -- C ABI of the B200-native (sm_100a) hot path of the R-matrix method of arxiv 2512.11590 (HPRMAT).
+ *
+ * What the library computes (citations are /root/reference/PAPER.md lines):
+ *   - the dense complex-symmetric Lagrange-Legendre internal-region matrix  C - E*I  of Eqs. (1),(3),(4)
+ *     (PAPER.md:73-99), N = nch*nbasis, row/column index of (channel c, mesh point i) = c*nbasis + i;
+ *   - the solution X of (C - E*I) X = B for the nch right-hand sides B[(c,i),c'] = f_i(a) delta_cc'
+ *      by blocked LU with partial pivoting, M = P L U (Eq. 5), either in
+ *     FP64 (the paper's Type 1) or with low-precision factors plus FP64 iterative refinement (Types 2/4,
+ *     PAPER.md:147-151, 192-230), the low-precision factorisation being applied to the block-diagonally
+ *     preconditioned matrix K_diag^-1 M of the paper's Type 3 (Eqs. 7-9);
+ *   - the R-matrix  R_cc' = (hbar^2/2 mu a) sum_i f_i(a) X[(c,i),c']  (PAPER.md:137 step 4; prefactor from
+ *     BASELINE.json north_star).
+ *
+ * Conventions
+ *   - All matrices are COLUMN-MAJOR.  "complex" is interleaved (re, im) double unless stated.
+ *   - Pointers marked  dev  are CUDA device pointers, those marked  host  are host pointers.  The library never
+ *     allocates device memory inside hprmat_solve / hprmat_zsolve / hprmat_zgetrf / hprmat_zgetrs / hprmat_zgemm.
+ *   - Every call enqueues its kernels on the stream given at setup (or as argument); calls that fill a host
+ *     hprmat_info synchronise that stream before returning, the others do not.
+ *   - Return value: 0 success; -k = argument k (1-based) invalid; >0 = one of the HPRMAT_E* codes below.
+ *   - There is NO CPU fallback: without a CUDA device every compute entry returns HPRMAT_ECUDA.
+ *   - One context per host thread / stream.  The caller owns V, R, A, B, ipiv and the workspace; the context owns
+ *     everything else and is reused across an energy scan.
+ */
+#ifndef HPRMAT_H
+#define HPRMAT_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hprmat_ctx hprmat_ctx; /* opaque */
+
+/* precision modes (PAPER.md:253-269 solver_type; Fig. 3) */
+enum {
+    HPRMAT_FP64 = 1,         /* FP64 LU of C - E*I on FP64 tensor cores (+ refinement with a compensated residual)     */
+    HPRMAT_MIXED = 2,        /* low-precision (complex64 storage, TF32 tensor-core update) LU, NO refinement            */
+    HPRMAT_MIXED_REFINE = 3  /* low-precision LU + FP64 residual / iterative refinement to double accuracy            */
+};
+
+/* status codes */
+enum {
+    HPRMAT_OK = 0,
+    HPRMAT_ESINGULAR = 1,     /* exact zero pivot; info->pivot_index = 1-based column                                  */
+    HPRMAT_ENOTCONVERGED = 2, /* refinement hit max_refine or stagnated; X / R hold the last iterate    */
+    HPRMAT_ENOMEM = 3,        /* device allocation failed at setup, or workspace too small                             */
+    HPRMAT_ECUDA = 4          /* CUDA error (no device, launch failure, ...); see hprmat_last_cuda_error()             */
+};
+
+typedef struct {
+    int status;            /* same as the return value                                                                  */
+    int refine_steps;      /* refinement steps actually taken                                                           */
+    int pivot_index;       /* first zero pivot (1-based) or 0                                                           */
+    int reserved;
+    double resid_max;      /* max_ij |B - A X|_ij of the last residual evaluated (absolute)                             */
+    double backward_err;   /* max_j ||b_j - A x_j||_inf / (||A||_inf ||x_j||_inf + ||b_j||_inf); <0 if not evaluated     */
+    double ms_assemble, ms_lu, ms_solve, ms_refine, ms_contract, ms_total; /* CUDA-event stage times, milliseconds      */
+    double lu_tflops;      /* (8 N^3 / 3) / ms_lu, the paper's flop convention                           */
+} hprmat_info;
+
+/* ---- structured R-matrix path ------------------------------------------------------------------------------------ */
+
+/* Create a context for nch channels and nbasis Lagrange-Legendre functions on (0, a).
+ *   a      channel radius, fm;  h2m = hbar^2/2mu, MeV fm^2 (equal reduced mass in all channels)
+ *   lval   host, int[nch]: orbital momenta l_c;  ethr  host, double[nch]: thresholds E_c, MeV (enter as +E_c on the
+ *          diagonal of Eq. 1)
+ *   max_mode  bitwise OR of (1 << HPRMAT_FP64), (1 << HPRMAT_MIXED), (1 << HPRMAT_MIXED_REFINE): sizes the buffers
+ *          (FP64: 16 N^2 bytes; mixed: 8 N^2 bytes; plus O(N nch)).  0 means all modes.
+ *   cuda_stream  a cudaStream_t (may be NULL = default stream)
+ * Computes the mesh, f_i(a) and the kinetic + Bloch table on the host in long double and uploads them. */
+int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, double h2m, const int *lval, const double *ethr,
+                 int max_mode, void *cuda_stream);
+
+/* Mesh abscissas r_i = a x_i (ascending, fm) and surface values f_i(a) (the paper's q2(r_i)) so the
+ * caller can evaluate V_cc'(r_i).  r, fa: host, double[nbasis]; either may be NULL. */
+int hprmat_mesh(const hprmat_ctx *ctx, double *r, double *fa);
+
+/* One energy point: assemble, factorise, solve, (refine), contract.
+ *   V    dev, complex [nbasis][nch][nch]: V[(i*nch + c2)*nch + c1] = V_{c1 c2}(r_i), MeV (Eq. 4)
+ *   mode one of HPRMAT_FP64 / HPRMAT_MIXED / HPRMAT_MIXED_REFINE (must be inside max_mode)
+ *   max_refine  maximum refinement steps; <0 = default (2 for FP64, 5 for MIXED_REFINE)
+ *   tol  refinement stops when max|r| <= tol * max|B|; <=0 = default 1e-13
+ *   R    dev, complex nch x nch column-major (output)
+ *   info host, may be NULL (then the call does not synchronise) */
+int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int max_refine, double tol, void *R,
+                 hprmat_info *info);
+
+/* Solution block of the last hprmat_solve: X dev, complex N x nch column-major (copy out). */
+int hprmat_get_x(const hprmat_ctx *ctx, void *X);
+
+/* Assembly only (Eqs. 3-4): C dev, complex N x N column-major, ldc = N. */
+int hprmat_get_matrix(hprmat_ctx *ctx, double energy, const void *V, void *C);
+
+int hprmat_destroy(hprmat_ctx *ctx);
+
+/* ---- raw dense complex entries (PAPER.md:119 "take M, b, return c"; :125-137 ZGESV) -------------------------------- */
+
+/* Workspace (bytes) needed by hprmat_zsolve / hprmat_zgetrf / hprmat_zgetrs for an n x n system with nrhs right-hand
+ * sides in the given mode. */
+size_t hprmat_workspace_bytes(int n, int nrhs, int mode);
+
+/* Solve A X = B.  A dev complex n x n (lda >= n); B dev complex n x nrhs (ldb >= n), overwritten by X;
+ * ipiv dev int[n], 1-based LAPACK row interchanges (of the matrix actually factorised: A itself in FP64 mode).
+ * HPRMAT_FP64: A is OVERWRITTEN by its LU factors (unit-lower L and U, LAPACK zgetrf layout).
+ * HPRMAT_MIXED / HPRMAT_MIXED_REFINE: A is preserved; the factors of the row/column-equilibrated complex64 copy live
+ * in the workspace; refinement uses the FP64 residual B - A X.
+ * workspace dev, workspace_bytes >= hprmat_workspace_bytes(n, nrhs, mode). */
+int hprmat_zsolve(void *cuda_stream, int n, int nrhs, void *A, int lda, void *B, int ldb, int *ipiv, int mode,
+                  int max_refine, double tol, void *workspace, size_t workspace_bytes, hprmat_info *info);
+
+/* FP64 LU with partial pivoting in place (Eq. 5): A = P L U.  info_dev: dev int[1], 0 or first zero pivot (1-based). */
+int hprmat_zgetrf(void *cuda_stream, int n, void *A, int lda, int *ipiv, int *info_dev, void *workspace,
+                  size_t workspace_bytes);
+
+/* Triangular solves with the factors of hprmat_zgetrf (same workspace, untouched in between): B <- A^-1 B. */
+int hprmat_zgetrs(void *cuda_stream, int n, int nrhs, const void *A, int lda, const int *ipiv, void *B, int ldb,
+                  void *workspace, size_t workspace_bytes);
+
+/* C <- beta*C + alpha*A*B, complex128 column-major, real alpha and beta; the FP64 tensor-core (DMMA) kernel that
+ * performs the trailing update of the LU.  A m x k, B k x n, C m x n. */
+int hprmat_zgemm(void *cuda_stream, int m, int n, int k, double alpha, const void *A, int lda, const void *B, int ldb,
+                 double beta, void *C, int ldc);
+
+/* Same for split (planar) complex64: separate real and imaginary float planes, TF32 tensor cores, FP32 accumulate;
+ * the trailing-update kernel of the mixed path. */
+int hprmat_cgemm_planar(void *cuda_stream, int m, int n, int k, float alpha, const float *Ar, const float *Ai, int lda,
+                        const float *Br, const float *Bi, int ldb, float beta, float *Cr, float *Ci, int ldc);
+
+const char *hprmat_strerror(int code);
+const char *hprmat_last_cuda_error(void);
+/* number of kernel launches issued by this library since process start (bench.py's gpu_launches) */
+long long hprmat_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HPRMAT_H */

@@ -1,0 +1,107 @@
+// common.cuh -- shared device/host helpers of the HPRMAT B200 path (sm_100a only).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/hprmat.h"
+
+namespace hp {
+
+// ---- error plumbing ------------------------------------------------------------------------------------------------
+extern thread_local char g_cuda_err[256];
+extern long long g_launches;
+
+inline int cuda_fail(cudaError_t e, const char *file, int line) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s (%s:%d)", cudaGetErrorString(e), file, line);
+    return HPRMAT_ECUDA;
+}
+#define HP_CUDA(x)                                                   \
+    do {                                                             \
+        cudaError_t e__ = (x);                                       \
+        if (e__ != cudaSuccess) return hp::cuda_fail(e__, __FILE__, __LINE__); \
+    } while (0)
+#define HP_TRY(x)                 \
+    do {                          \
+        int r__ = (x);            \
+        if (r__ != 0) return r__; \
+    } while (0)
+// after a kernel launch: count it and pick up launch-configuration errors
+#define HP_LAUNCHED()                  \
+    do {                               \
+        ++hp::g_launches;              \
+        HP_CUDA(cudaPeekAtLastError()); \
+    } while (0)
+
+constexpr int kNumSMs = 148;  // B200
+
+inline int ceil_div(long a, long b) { return (int)((a + b - 1) / b); }
+inline long round_up(long a, long b) { return (a + b - 1) / b * b; }
+
+// ---- complex matrix views ------------------------------------------------------------------------------------------
+// The FP64 path stores interleaved complex128 (LAPACK layout; the raw solve factorises the caller's array in place).
+// The mixed path stores SPLIT (planar) complex64 -- one float plane for the real and one for the imaginary part -- so
+// that the trailing update is four real TF32 tensor-core products on operands that can be fed to the MMA unchanged.
+struct ZView {
+    typedef double real_t;
+    typedef double2 elem_t;
+    double2 *p;
+    long ld;
+    __host__ __device__ ZView() : p(nullptr), ld(0) {}
+    __host__ __device__ ZView(double2 *p_, long ld_) : p(p_), ld(ld_) {}
+    __host__ __device__ ZView sub(long i, long j) const { return ZView(p + j * ld + i, ld); }
+    __device__ __forceinline__ double2 get(long i, long j) const { return p[j * ld + i]; }
+    __device__ __forceinline__ void set(long i, long j, double2 v) const { p[j * ld + i] = v; }
+};
+
+struct CView {
+    typedef float real_t;
+    typedef float2 elem_t;
+    float *re, *im;
+    long ld;
+    __host__ __device__ CView() : re(nullptr), im(nullptr), ld(0) {}
+    __host__ __device__ CView(float *r_, float *i_, long ld_) : re(r_), im(i_), ld(ld_) {}
+    __host__ __device__ CView sub(long i, long j) const { return CView(re + j * ld + i, im + j * ld + i, ld); }
+    __device__ __forceinline__ float2 get(long i, long j) const {
+        return make_float2(re[j * ld + i], im[j * ld + i]);
+    }
+    __device__ __forceinline__ void set(long i, long j, float2 v) const {
+        re[j * ld + i] = v.x;
+        im[j * ld + i] = v.y;
+    }
+};
+
+// ---- complex arithmetic on double2 / float2 -------------------------------------------------------------------------
+template <class E> struct real_of;
+template <> struct real_of<double2> { typedef double type; };
+template <> struct real_of<float2> { typedef float type; };
+
+__device__ __forceinline__ double2 mk(double a, double b) { return make_double2(a, b); }
+__device__ __forceinline__ float2 mk(float a, float b) { return make_float2(a, b); }
+
+template <class E> __device__ __forceinline__ E cmul(E a, E b) { return mk(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+template <class E> __device__ __forceinline__ E cadd(E a, E b) { return mk(a.x + b.x, a.y + b.y); }
+template <class E> __device__ __forceinline__ E csub(E a, E b) { return mk(a.x - b.x, a.y - b.y); }
+// a - b*c
+template <class E> __device__ __forceinline__ E cfnma(E a, E b, E c) {
+    typedef typename real_of<E>::type T;
+    T re = a.x - b.x * c.x;
+    re = re + b.y * c.y;
+    T im = a.y - b.x * c.y;
+    im = im - b.y * c.x;
+    return mk(re, im);
+}
+template <class E> __device__ __forceinline__ typename real_of<E>::type cabs1(E a) { return fabs(a.x) + fabs(a.y); }
+// 1/a with scaling against overflow (Smith)
+template <class E> __device__ __forceinline__ E crecip(E a) {
+    typedef typename real_of<E>::type T;
+    if (fabs(a.x) >= fabs(a.y)) {
+        T r = a.y / a.x, d = a.x + a.y * r;
+        return mk((T)1 / d, -r / d);
+    } else {
+        T r = a.x / a.y, d = a.x * r + a.y;
+        return mk(r / d, (T)-1 / d);
+    }
+}
+
+}  // namespace hp

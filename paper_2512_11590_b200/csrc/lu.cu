@@ -1,0 +1,418 @@
+// lu.cu -- recursive blocked LU with partial pivoting, M = P L U (Eq. 5), and the triangular
+// solves for the nch right-hand sides (PAPER.md:127 "forward and backward substitution"; :137 step 3).
+//
+// Structure:
+//   getrf_rec(c0,c1): width <= IB -> panel kernel; else factor the left half, U12 <- L11^-1 A12 (recursive TRSM whose
+//   leaves multiply by inverted IB x IB diagonal blocks), A22 <- A22 - L21 U12 (tensor-core GEMM), factor the right
+//   half.  All O(N^3) work is GEMM with K up to N/2, so the trailing update is compute- not HBM-bound.
+//   Panel: one cooperative kernel, one CTA per SM, each CTA keeps its slice of panel rows in shared memory for all IB
+//   columns; per column one grid barrier: every CTA publishes its local pivot candidate ROW, all CTAs pick the same
+//   winner and read its row, swap and rank-1 update locally.  The multipliers are scaled at write-back.
+//   Row interchanges: right after each panel, its IB swaps are folded into one net permutation of <= 2 IB rows and
+//   applied to ALL other columns of the matrix by a gather/scatter kernel (independent loads, no swap chain).
+#include "lu.cuh"
+
+#include <cooperative_groups.h>
+
+namespace hp {
+
+constexpr int PANEL_NT = 256;
+constexpr int PANEL_MINROWS = 128;
+
+// ------------------------------------------------------------------------------------------------- workspace
+template <class V> static V alloc_view(char *&p, long rows, long cols);
+template <> ZView alloc_view<ZView>(char *&p, long rows, long cols) {
+    ZView v((double2 *)p, rows);
+    p += round_up(rows * cols * sizeof(double2), 256);
+    return v;
+}
+template <> CView alloc_view<CView>(char *&p, long rows, long cols) {
+    float *re = (float *)p;
+    p += round_up(rows * cols * sizeof(float), 256);
+    float *im = (float *)p;
+    p += round_up(rows * cols * sizeof(float), 256);
+    return CView(re, im, rows);
+}
+
+template <class V> size_t LuWork<V>::carve(void *base, int n_) {
+    char *p = (char *)base;
+    n = n_;
+    nblk = ceil_div(n, IB);
+    auto take = [&](size_t bytes) {
+        char *q = p;
+        p += round_up((long)bytes, 256);
+        return q;
+    };
+    dinvL = alloc_view<V>(p, IB, (long)nblk * IB);
+    dinvU = alloc_view<V>(p, IB, (long)nblk * IB);
+    perm = (int *)take(sizeof(int) * (size_t)nblk * PERM_STRIDE);
+    cand_val = (T *)take(sizeof(T) * 2 * MAXG);
+    cand_row = (int *)take(sizeof(int) * 2 * MAXG);
+    cand_data = (E *)take(sizeof(E) * 2 * MAXG * IB);
+    jrow = (E *)take(sizeof(E) * 2 * IB);
+    counter = (unsigned *)take(256);
+    return (size_t)(p - (char *)base);
+}
+template <class V> size_t LuWork<V>::bytes(int n) {
+    LuWork<V> tmp;
+    return tmp.carve((void *)0, n);
+}
+
+// ------------------------------------------------------------------------------------------------- panel kernel
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// all CTAs of the (cooperatively launched, hence co-resident) grid arrive; counter is monotone, target = base + G*k
+__device__ __forceinline__ void grid_barrier(unsigned *counter, unsigned target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(counter, 1u);
+        while ((int)(ld_acquire_u32(counter) - target) < 0) {
+        }
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+template <class T> __device__ __forceinline__ bool better(T v, int i, T bv, int bi) {
+    // larger modulus wins; ties go to the smaller row index (first maximum, LAPACK's izamax)
+    return (v > bv) || (v == bv && i >= 0 && (bi < 0 || i < bi));
+}
+
+template <class E> __device__ __forceinline__ E ldcg_e(const E *p);
+template <> __device__ __forceinline__ double2 ldcg_e<double2>(const double2 *p) { return __ldcg(p); }
+template <> __device__ __forceinline__ float2 ldcg_e<float2>(const float2 *p) { return __ldcg(p); }
+
+template <class V>
+__global__ void __launch_bounds__(PANEL_NT, 1)
+    panel_lu_kernel(V A, int m, int jb, int j0, int rpc, int *ipiv, int *info, typename V::real_t *cand_val,
+                    int *cand_row, typename V::elem_t *cand_data, typename V::elem_t *jrow_g, unsigned *counter,
+                    unsigned bar_base, V dinvL, V dinvU, int *perm) {
+    typedef typename V::elem_t E;
+    typedef typename V::real_t T;
+    extern __shared__ __align__(16) unsigned char smraw[];
+    E *chunk = reinterpret_cast<E *>(smraw);          // [IB][rpc], column-major slice of the panel
+    E *inv_s = chunk + (size_t)IB * rpc;              // [2][IB][IB] scratch for the diagonal-block inverses (CTA 0)
+    __shared__ E prow[IB], jr[IB], invp[IB];
+    __shared__ int piv[IB];
+    __shared__ T red_val[PANEL_NT / 32];
+    __shared__ int red_idx[PANEL_NT / 32];
+    __shared__ T s_bval;
+    __shared__ int s_bli, s_win, s_p;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int cta = blockIdx.x, G = gridDim.x;
+    const int row0 = cta * rpc;
+    const int nloc = max(0, min(rpc, m - row0));
+
+    for (int idx = tid; idx < jb * nloc; idx += PANEL_NT) {
+        int c = idx / nloc, li = idx - c * nloc;
+        chunk[c * rpc + li] = A.get(row0 + li, c);
+    }
+    __syncthreads();
+
+    T myval = (T)-1;
+    int myli = -1;
+    for (int li = tid; li < nloc; li += PANEL_NT) {
+        T v = cabs1(chunk[li]);
+        if (v > myval) { myval = v; myli = li; }
+    }
+
+    for (int j = 0; j < jb; ++j) {
+        const int par = j & 1;
+        // ---- local arg-max of column j over this CTA's rows (global panel row >= j)
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            T ov = __shfl_down_sync(0xffffffffu, myval, off);
+            int oi = __shfl_down_sync(0xffffffffu, myli, off);
+            if (better(ov, oi, myval, myli)) { myval = ov; myli = oi; }
+        }
+        if (lane == 0) { red_val[warp] = myval; red_idx[warp] = myli; }
+        __syncthreads();
+        if (warp == 0) {
+            T v = lane < PANEL_NT / 32 ? red_val[lane] : (T)-1;
+            int i = lane < PANEL_NT / 32 ? red_idx[lane] : -1;
+#pragma unroll
+            for (int off = 4; off > 0; off >>= 1) {
+                T ov = __shfl_down_sync(0xffffffffu, v, off);
+                int oi = __shfl_down_sync(0xffffffffu, i, off);
+                if (better(ov, oi, v, i)) { v = ov; i = oi; }
+            }
+            if (lane == 0) { s_bval = v; s_bli = i; }
+        }
+        __syncthreads();
+        // ---- publish the candidate row (and row j, for the swap) and meet the other CTAs
+        {
+            const int bli = s_bli;
+            if (tid < jb && bli >= 0) cand_data[(size_t)(par * MAXG + cta) * IB + tid] = chunk[tid * rpc + bli];
+            if (tid == 0) {
+                cand_val[par * MAXG + cta] = bli >= 0 ? s_bval : (T)-1;
+                cand_row[par * MAXG + cta] = row0 + bli;
+            }
+            if (j >= row0 && j < row0 + nloc && tid >= 32 && tid < 32 + jb)
+                jrow_g[par * IB + tid - 32] = chunk[(tid - 32) * rpc + j - row0];
+        }
+        grid_barrier(counter, bar_base + (unsigned)G * (unsigned)(j + 1));
+        // ---- every CTA picks the same winner
+        if (warp == 0) {
+            T bv = (T)-1;
+            int br = -1, bg = -1;
+            for (int g = lane; g < G; g += 32) {
+                T v = __ldcg(&cand_val[par * MAXG + g]);
+                int rr = __ldcg(&cand_row[par * MAXG + g]);
+                if (v >= (T)0 && better(v, rr, bv, br)) { bv = v; br = rr; bg = g; }
+            }
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+                T ov = __shfl_down_sync(0xffffffffu, bv, off);
+                int orr = __shfl_down_sync(0xffffffffu, br, off);
+                int og = __shfl_down_sync(0xffffffffu, bg, off);
+                if (og >= 0 && better(ov, orr, bv, br)) { bv = ov; br = orr; bg = og; }
+            }
+            if (lane == 0) { s_win = bg; s_p = bg >= 0 ? br : j; }
+        }
+        __syncthreads();
+        const int p = s_p, win = s_win;
+        const bool ownp = (p >= row0 && p < row0 + nloc), ownj = (j >= row0 && j < row0 + nloc);
+        if (tid < jb) prow[tid] = win >= 0 ? ldcg_e(&cand_data[(size_t)(par * MAXG + win) * IB + tid]) : mk((T)0, (T)0);
+        if (ownp && p != j && tid >= 32 && tid < 32 + jb) jr[tid - 32] = ldcg_e(&jrow_g[par * IB + tid - 32]);
+        if (tid == 0) {
+            piv[j] = p;
+            if (cta == 0) ipiv[j0 + j] = j0 + p + 1;
+        }
+        __syncthreads();
+        if (tid < jb) {
+            if (ownp && p != j) chunk[tid * rpc + p - row0] = jr[tid];
+            if (ownj) chunk[tid * rpc + j - row0] = prow[tid];
+        }
+        const E pv = prow[j];
+        const bool sing = (pv.x == (T)0 && pv.y == (T)0);
+        const E ip = sing ? mk((T)0, (T)0) : crecip(pv);
+        if (tid == 0) {
+            invp[j] = ip;
+            if (sing && cta == 0) atomicCAS(info, 0, j0 + j + 1);
+        }
+        __syncthreads();
+        // ---- rank-1 update of the local rows below the diagonal, fused with the next column's arg-max
+        myval = (T)-1;
+        myli = -1;
+        if (!sing || j + 1 < jb) {
+            for (int li = tid; li < nloc; li += PANEL_NT) {
+                if (row0 + li > j) {
+                    if (!sing) {
+                        const E l = cmul(chunk[j * rpc + li], ip);
+                        for (int c = j + 1; c < jb; ++c) chunk[c * rpc + li] = cfnma(chunk[c * rpc + li], l, prow[c]);
+                    }
+                    if (j + 1 < jb) {
+                        T v = cabs1(chunk[(j + 1) * rpc + li]);
+                        if (v > myval) { myval = v; myli = li; }
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- write back; multipliers are scaled by 1/pivot here
+    for (int idx = tid; idx < jb * nloc; idx += PANEL_NT) {
+        int c = idx / nloc, li = idx - c * nloc;
+        E v = chunk[c * rpc + li];
+        if (row0 + li > c) v = cmul(v, invp[c]);
+        A.set(row0 + li, c, v);
+    }
+
+    if (cta != 0) return;
+    // ---- CTA 0 owns the top jb x jb block: inverses of its unit-lower and upper triangles (leaves of the TRSM
+    //      recursion), and the net row permutation of this swap batch.
+    E *xl = inv_s, *xu = inv_s + IB * IB;  // column-major jb x jb, ld = IB
+    if (tid < jb) {
+        const int cc = tid;  // column cc of inv(L): forward substitution on e_cc
+        for (int i = 0; i < jb; ++i) xl[cc * IB + i] = mk((T)(i == cc ? 1 : 0), (T)0);
+        for (int i = cc + 1; i < jb; ++i) {
+            E s = mk((T)0, (T)0);
+            for (int k = cc; k < i; ++k) s = cadd(s, cmul(cmul(chunk[k * rpc + i], invp[k]), xl[cc * IB + k]));
+            xl[cc * IB + i] = mk(-s.x, -s.y);
+        }
+        for (int i = 0; i < jb; ++i) dinvL.set(i, cc, xl[cc * IB + i]);
+    } else if (tid >= 32 && tid < 32 + jb) {
+        const int cc = tid - 32;  // column cc of inv(U): back substitution on e_cc
+        for (int i = 0; i < jb; ++i) xu[cc * IB + i] = mk((T)0, (T)0);
+        xu[cc * IB + cc] = invp[cc];
+        for (int i = cc - 1; i >= 0; --i) {
+            E s = mk((T)0, (T)0);
+            for (int k = i + 1; k <= cc; ++k) s = cadd(s, cmul(chunk[k * rpc + i], xu[cc * IB + k]));
+            E q = cmul(s, invp[i]);
+            xu[cc * IB + i] = mk(-q.x, -q.y);
+        }
+        for (int i = 0; i < jb; ++i) dinvU.set(i, cc, xu[cc * IB + i]);
+    } else if (warp == 2) {
+        // net permutation: content of every touched row after the jb interchanges (rows are panel-relative here)
+        __shared__ int top[IB], orow[IB], ocont[IB];
+        __shared__ int nout;
+        if (lane == 0) nout = 0;
+        for (int k = lane; k < jb; k += 32) top[k] = k;
+        __syncwarp();
+        for (int k = 0; k < jb; ++k) {
+            const int pk = piv[k];
+            if (pk == k) continue;
+            if (pk < jb) {
+                if (lane == 0) { int t = top[k]; top[k] = top[pk]; top[pk] = t; }
+            } else {
+                const int no = nout;
+                int found = -1;
+                if (lane < no && orow[lane] == pk) found = lane;
+                unsigned bal = __ballot_sync(0xffffffffu, found >= 0);
+                int idx = bal ? (__ffs(bal) - 1) : no;
+                if (lane == 0) {
+                    if (!bal) { orow[idx] = pk; ocont[idx] = pk; nout = no + 1; }
+                    int t = top[k]; top[k] = ocont[idx]; ocont[idx] = t;
+                }
+            }
+            __syncwarp();
+        }
+        if (lane == 0) {
+            int cnt = 0;
+            for (int k = 0; k < jb; ++k)
+                if (top[k] != k) { perm[1 + cnt] = j0 + k; perm[1 + 2 * IB + cnt] = j0 + top[k]; ++cnt; }
+            for (int q = 0; q < nout; ++q)
+                if (ocont[q] != orow[q]) { perm[1 + cnt] = j0 + orow[q]; perm[1 + 2 * IB + cnt] = j0 + ocont[q]; ++cnt; }
+            perm[0] = cnt;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------- row interchanges
+constexpr int SWP_CW = 16;  // columns per CTA
+constexpr int SWP_NT = 256;
+
+// Apply the net permutations of swap batches [b0, b1) in order to the columns [lo1,hi1) U [lo2,hi2) of A.
+template <class V>
+__global__ void __launch_bounds__(SWP_NT) laswp_kernel(V A, int lo1, int hi1, int lo2, int hi2, const int *perm, int b0, int b1) {
+    typedef typename V::elem_t E;
+    const int n1 = hi1 - lo1, ntot = n1 + (hi2 - lo2);
+    const int tid = threadIdx.x;
+    const int q = tid & (2 * IB - 1);          // pair slot 0..63
+    const int cl = tid >> 6;                   // 0..3; columns cl, cl+4, cl+8, cl+12 of this CTA's group
+    long col[SWP_CW / 4];
+    bool cok[SWP_CW / 4];
+#pragma unroll
+    for (int e = 0; e < SWP_CW / 4; ++e) {
+        int v = blockIdx.x * SWP_CW + cl + 4 * e;
+        cok[e] = v < ntot;
+        col[e] = v < n1 ? lo1 + v : lo2 + (v - n1);
+    }
+    for (int b = b0; b < b1; ++b) {
+        const int *pb = perm + (size_t)b * PERM_STRIDE;
+        const int cnt = pb[0];
+        if (cnt == 0) continue;  // uniform across the CTA
+        E val[SWP_CW / 4];
+        int dst = 0;
+        if (q < cnt) {
+            dst = pb[1 + q];
+            const int src = pb[1 + 2 * IB + q];
+#pragma unroll
+            for (int e = 0; e < SWP_CW / 4; ++e)
+                if (cok[e]) val[e] = A.get(src, col[e]);
+        }
+        __syncthreads();
+        if (q < cnt) {
+#pragma unroll
+            for (int e = 0; e < SWP_CW / 4; ++e)
+                if (cok[e]) A.set(dst, col[e], val[e]);
+        }
+        __syncthreads();
+    }
+}
+
+template <class V> static int laswp(cudaStream_t st, V A, int lo1, int hi1, int lo2, int hi2, const int *perm, int b0, int b1) {
+    int ntot = (hi1 - lo1) + (hi2 - lo2);
+    if (ntot <= 0 || b1 <= b0) return 0;
+    laswp_kernel<V><<<ceil_div(ntot, SWP_CW), SWP_NT, 0, st>>>(A, lo1, hi1, lo2, hi2, perm, b0, b1);
+    HP_LAUNCHED();
+    return 0;
+}
+
+// ------------------------------------------------------------------------------------------------- host recursion
+static inline int split(int w) { return (int)round_up((w + 1) / 2, IB); }
+
+template <class V> static int panel(cudaStream_t st, int n, V A, int c0, int w, int *ipiv, int *info_dev, LuWork<V> &wk) {
+    typedef typename V::elem_t E;
+    const int m = n - c0;
+    int rpc = std::max(ceil_div(m, MAXG), PANEL_MINROWS);
+    rpc = (int)round_up(rpc, 2);
+    const int G = ceil_div(m, rpc);
+    const size_t smem = ((size_t)IB * rpc + 2 * IB * IB) * sizeof(E);
+    auto kern = panel_lu_kernel<V>;
+    static size_t configured = 0;
+    if (smem > configured) {
+        HP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    V Asub = A.sub(c0, c0);
+    const int blk = c0 / IB;
+    V dl = wk.dinvL.sub(0, (long)blk * IB), du = wk.dinvU.sub(0, (long)blk * IB);
+    int *perm = wk.perm + (size_t)blk * PERM_STRIDE;
+    int m_ = m, w_ = w, c0_ = c0, rpc_ = rpc;
+    unsigned base = wk.bar_base;
+    void *args[] = {&Asub, &m_, &w_, &c0_, &rpc_, &ipiv, &info_dev, &wk.cand_val, &wk.cand_row, &wk.cand_data,
+                    &wk.jrow, &wk.counter, &base, &dl, &du, &perm};
+    HP_CUDA(cudaLaunchCooperativeKernel((void *)kern, dim3(G), dim3(PANEL_NT), args, smem, st));
+    HP_LAUNCHED();
+    wk.bar_base += (unsigned)G * (unsigned)w;
+    // this batch's interchanges on every other column of the matrix
+    return laswp(st, A, 0, c0, c0 + w, n, wk.perm, blk, blk + 1);
+}
+
+// B <- L^-1 B, L = unit lower triangle of the s x s diagonal block of A at (d0,d0); B is s x ncols
+template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk) {
+    if (s <= 0 || ncols <= 0) return 0;
+    if (s <= IB) return gemm(st, s, ncols, s, 1.0, wk.dinvL.sub(0, (long)(d0 / IB) * IB), B, 0.0, B);
+    const int h = split(s);
+    HP_TRY(trsm_lower(st, A, d0, h, B, ncols, wk));
+    HP_TRY(gemm(st, s - h, ncols, h, -1.0, A.sub(d0 + h, d0), B, 1.0, B.sub(h, 0)));
+    return trsm_lower(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk);
+}
+
+// B <- U^-1 B, U = upper triangle (with diagonal) of the s x s diagonal block of A at (d0,d0)
+template <class V> static int trsm_upper(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk) {
+    if (s <= 0 || ncols <= 0) return 0;
+    if (s <= IB) return gemm(st, s, ncols, s, 1.0, wk.dinvU.sub(0, (long)(d0 / IB) * IB), B, 0.0, B);
+    const int h = split(s);
+    HP_TRY(trsm_upper(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk));
+    HP_TRY(gemm(st, h, ncols, s - h, -1.0, A.sub(d0, d0 + h), B.sub(h, 0), 1.0, B));
+    return trsm_upper(st, A, d0, h, B, ncols, wk);
+}
+
+template <class V> static int getrf_rec(cudaStream_t st, int n, V A, int c0, int c1, int *ipiv, int *info_dev, LuWork<V> &wk) {
+    const int w = c1 - c0;
+    if (w <= IB) return panel(st, n, A, c0, w, ipiv, info_dev, wk);
+    const int h = split(w), mid = c0 + h;
+    HP_TRY(getrf_rec(st, n, A, c0, mid, ipiv, info_dev, wk));
+    HP_TRY(trsm_lower(st, A, c0, h, A.sub(c0, mid), c1 - mid, wk));
+    HP_TRY(gemm(st, n - mid, c1 - mid, h, -1.0, A.sub(mid, c0), A.sub(c0, mid), 1.0, A.sub(mid, mid)));
+    return getrf_rec(st, n, A, mid, c1, ipiv, info_dev, wk);
+}
+
+template <class V> int getrf(cudaStream_t st, int n, V A, int *ipiv, int *info_dev, LuWork<V> &wk) {
+    if (n <= 0) return 0;
+    HP_CUDA(cudaMemsetAsync(wk.counter, 0, sizeof(unsigned), st));
+    wk.bar_base = 0;
+    return getrf_rec(st, n, A, 0, n, ipiv, info_dev, wk);
+}
+
+template <class V> int getrs(cudaStream_t st, int n, int nrhs, V A, V B, LuWork<V> &wk) {
+    if (n <= 0 || nrhs <= 0) return 0;
+    HP_TRY(laswp(st, B, 0, nrhs, 0, 0, wk.perm, 0, wk.nblk));
+    HP_TRY(trsm_lower(st, A, 0, n, B, nrhs, wk));
+    return trsm_upper(st, A, 0, n, B, nrhs, wk);
+}
+
+template struct LuWork<ZView>;
+template int getrf<ZView>(cudaStream_t, int, ZView, int *, int *, LuWork<ZView> &);
+template int getrs<ZView>(cudaStream_t, int, int, ZView, ZView, LuWork<ZView> &);
+
+}  // namespace hp

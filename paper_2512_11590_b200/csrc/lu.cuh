@@ -1,0 +1,42 @@
+// lu.cuh -- blocked recursive LU with partial pivoting and the triangular solves, for both matrix views.
+#pragma once
+#include "common.cuh"
+
+namespace hp {
+
+constexpr int IB = 32;        // panel width = swap batch = inverted diagonal block size
+constexpr int MAXG = kNumSMs; // CTAs of the cooperative panel kernel (one per SM)
+
+// GEMM back-ends (zgemm.cu / cgemm.cu): C <- beta*C + alpha*A*B.  nbatch > 1: operand b lives at view + b*stride
+// elements.  C may alias B when m <= 32 and the whole K extent is one diagonal block (see trsm in lu.cu).
+int gemm(cudaStream_t st, int m, int n, int k, double alpha, ZView A, ZView B, double beta, ZView C);
+int gemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
+int zgemm_batched(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda, long strideA,
+                  const double2 *B, long ldb, long strideB, double beta, double2 *C, long ldc, long strideC, int nbatch);
+
+// Workspace of one factorisation (device memory carved from a caller-provided buffer).
+template <class V> struct LuWork {
+    typedef typename V::elem_t E;
+    typedef typename V::real_t T;
+    int n = 0, nblk = 0;
+    V dinvL, dinvU;      // nblk blocks of IB x IB, block b at column offset b*IB, ld = IB
+    int *perm = nullptr; // nblk x (1 + 4*IB): count, dst rows[2*IB], src rows[2*IB]  (net permutation of each swap batch)
+    T *cand_val = nullptr;
+    int *cand_row = nullptr;
+    E *cand_data = nullptr, *jrow = nullptr;
+    unsigned *counter = nullptr;
+    unsigned bar_base = 0; // host-side running value of the grid-barrier counter
+    static size_t bytes(int n);
+    // carve from p (must be 256-byte aligned); returns bytes used
+    size_t carve(void *p, int n);
+};
+
+constexpr int PERM_STRIDE = 1 + 4 * IB;
+
+// A = P L U in place (Eq. 5).  ipiv: device, 1-based LAPACK interchanges.  info_dev: device int, set to
+// the first zero pivot (1-based) or left 0 (caller zeroes it).
+template <class V> int getrf(cudaStream_t st, int n, V A, int *ipiv, int *info_dev, LuWork<V> &w);
+// B <- A^-1 B with the factors (forward and backward substitution).
+template <class V> int getrs(cudaStream_t st, int n, int nrhs, V A, V B, LuWork<V> &w);
+
+}  // namespace hp

@@ -1,0 +1,203 @@
+// zgemm.cu -- complex128 GEMM on the FP64 tensor cores (DMMA, mma.sync.m8n8k4.f64) for sm_100a.
+//
+//   C <- beta*C + alpha*A*B,   A m x k, B k x n, C m x n, interleaved complex128, column-major.
+//
+// This is the trailing update A22 <- A22 - L21*U12 of the blocked LU (Eq. 5; the O(N^3) part that
+// the paper hands to ZGETRF/CGETRF), and the GEMM inside the blocked triangular solves.  tcgen05.mma has no f64 kind,
+// so FP64 tensor work on sm_100a is warp-level mma.sync.
+//
+// Complex product on a real MMA ("4M" form, 8 real flops per complex multiply-add = the 8N^3/3 convention of
+// PAPER.md:190): view column-major complex C (m x n) as the real 2m x n array C~ (re/im interleaved along rows), B as
+// the real 2k x n array B~, and expand A on the fly into the real 2m x 2k array
+//     A~[2i  ,2p] =  Ar   A~[2i  ,2p+1] = -Ai
+//     A~[2i+1,2p] =  Ai   A~[2i+1,2p+1] =  Ar
+// so that C~ = A~ * B~.  The expansion happens in registers while the A fragment is read from shared memory (each lane
+// picks the real or imaginary word of one complex element and flips its sign bit if needed); B~ and C~ fragments are
+// the natural memory layout.  One m8n8k4 MMA = 4 complex rows x 8 columns x 2 complex k.
+//
+// Tiling: CTA = WM x WN warps, warp tile 32 complex rows x 32 columns (8 x 4 MMAs per 2 complex k, 64 accumulators
+// per lane), CTA tile (32 WM) x (32 WN), k-slab KC, STAGES-deep cp.async ring.  Shared-memory leading dimensions are
+// padded to == 2 (mod 8) complex elements so that every fragment load (LDS.64) is bank-conflict free.
+#include "lu.cuh"
+
+namespace hp {
+
+__device__ __forceinline__ void cp_async16(void *sdst, const void *gsrc, bool valid) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(sdst);
+    int sz = valid ? 16 : 0;  // src-size 0 => 16 bytes of zero fill, nothing is read
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gsrc), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
+}
+
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+template <int WM, int WN, int KC, int STAGES, int MINB>
+__global__ void __launch_bounds__(WM *WN * 32, MINB)
+    zgemm_kernel(int M, int N, int K, double alpha, const double2 *__restrict__ A, long lda,
+                 const double2 *__restrict__ B, long ldb, double beta, double2 *C, long ldc, long strideA,
+                 long strideB, long strideC) {
+    constexpr int BM = WM * 32, BN = WN * 32, NT = WM * WN * 32;
+    constexpr int LDA_S = BM + 2, LDB_S = KC + 2;
+    constexpr int A_STAGE = KC * LDA_S, B_STAGE = BN * LDB_S;
+    static_assert(KC % 8 == 0, "KC must be a multiple of 8");
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2 *sA = reinterpret_cast<double2 *>(smem_raw);
+    double2 *sB = sA + STAGES * A_STAGE;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int wm = warp % WM, wn = warp / WM;
+    const int r = lane >> 2, kk = lane & 3;
+    const long m0 = (long)blockIdx.x * BM, n0 = (long)blockIdx.y * BN;
+    A += (long)blockIdx.z * strideA;
+    B += (long)blockIdx.z * strideB;
+    C += (long)blockIdx.z * strideC;
+
+    auto load_stage = [&](int slot, int k0) {
+        double2 *a = sA + slot * A_STAGE;
+        double2 *b = sB + slot * B_STAGE;
+#pragma unroll
+        for (int idx = tid; idx < BM * KC; idx += NT) {
+            int i = idx % BM, p = idx / BM;
+            bool ok = (m0 + i < M) && (k0 + p < K);
+            const double2 *src = ok ? (A + (long)(k0 + p) * lda + m0 + i) : A;
+            cp_async16(a + p * LDA_S + i, src, ok);
+        }
+#pragma unroll
+        for (int idx = tid; idx < BN * KC; idx += NT) {
+            int p = idx % KC, n = idx / KC;
+            bool ok = (n0 + n < N) && (k0 + p < K);
+            const double2 *src = ok ? (B + (n0 + n) * ldb + k0 + p) : B;
+            cp_async16(b + n * LDB_S + p, src, ok);
+        }
+    };
+
+    double acc[8][4][2];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    const int nk = (K + KC - 1) / KC;
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; ++s) {
+        if (s < nk) load_stage(s, s * KC);
+        cp_async_commit();
+    }
+
+    // per-lane fragment offsets (in doubles) inside a stage
+    const int a_off0 = ((kk >> 1) * LDA_S + wm * 32 + (r >> 1)) * 2 + ((r ^ kk) & 1);
+    const int b_off0 = ((wn * 32 + r) * LDB_S) * 2 + kk;
+    const unsigned sign_hi = (((r & 1) == 0) && ((kk & 1) == 1)) ? 0x80000000u : 0u;
+
+    for (int kt = 0; kt < nk; ++kt) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        {
+            int nxt = kt + STAGES - 1;
+            if (nxt < nk) load_stage(nxt % STAGES, nxt * KC);
+            cp_async_commit();
+        }
+        const int slot = kt % STAGES;
+        const double *a_s = reinterpret_cast<const double *>(sA + slot * A_STAGE) + a_off0;
+        const double *b_s = reinterpret_cast<const double *>(sB + slot * B_STAGE) + b_off0;
+#pragma unroll
+        for (int ks = 0; ks < KC / 2; ++ks) {
+            double af[8], bf[4];
+#pragma unroll
+            for (int ai = 0; ai < 8; ++ai) {
+                double v = a_s[ks * (2 * LDA_S * 2) + ai * 8];
+                int hi = __double2hiint(v) ^ (int)sign_hi;
+                af[ai] = __hiloint2double(hi, __double2loint(v));
+            }
+#pragma unroll
+            for (int bi = 0; bi < 4; ++bi) bf[bi] = b_s[ks * 4 + bi * (8 * LDB_S * 2)];
+#pragma unroll
+            for (int ai = 0; ai < 8; ++ai)
+#pragma unroll
+                for (int bi = 0; bi < 4; ++bi) dmma884(acc[ai][bi][0], acc[ai][bi][1], af[ai], bf[bi]);
+        }
+    }
+    cp_async_wait<0>();
+
+    // epilogue: lane holds C~[real row 8*ai + r][cols 8*bi + 2*kk + {0,1}] of the warp tile
+    double *Cd = reinterpret_cast<double *>(C);
+#pragma unroll
+    for (int ai = 0; ai < 8; ++ai) {
+        long crow = m0 + wm * 32 + ai * 4 + (r >> 1);
+        if (crow >= M) continue;
+#pragma unroll
+        for (int bi = 0; bi < 4; ++bi) {
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                long col = n0 + wn * 32 + bi * 8 + 2 * kk + e;
+                if (col < N) {
+                    double *p = Cd + (col * ldc + crow) * 2 + (r & 1);
+                    double v = alpha * acc[ai][bi][e];
+                    if (beta != 0.0) v += beta * (*p);
+                    *p = v;
+                }
+            }
+        }
+    }
+}
+
+template <int WM, int WN, int KC, int STAGES, int MINB>
+static int launch_zgemm(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda,
+                        const double2 *B, long ldb, double beta, double2 *C, long ldc, long sA = 0, long sB = 0,
+                        long sC = 0, int nbatch = 1) {
+    constexpr int BM = WM * 32, BN = WN * 32;
+    constexpr size_t smem = (size_t)STAGES * (KC * (BM + 2) + BN * (KC + 2)) * sizeof(double2);
+    auto kern = zgemm_kernel<WM, WN, KC, STAGES, MINB>;
+    static bool configured = false;
+    if (!configured) {
+        HP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = true;
+    }
+    dim3 grid(ceil_div(m, BM), ceil_div(n, BN), nbatch);
+    kern<<<grid, WM * WN * 32, smem, st>>>(m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC);
+    HP_LAUNCHED();
+    return 0;
+}
+
+// C <- beta*C + alpha*A*B  (device pointers, column-major)
+int zgemm(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda, const double2 *B, long ldb,
+          double beta, double2 *C, long ldc) {
+    if (m <= 0 || n <= 0) return 0;
+    if (k <= 0 && beta == 1.0) return 0;
+    if (n <= 32) return launch_zgemm<8, 1, 8, 4, 1>(st, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc);
+    return launch_zgemm<4, 2, 16, 4, 1>(st, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc);
+}
+
+int gemm(cudaStream_t st, int m, int n, int k, double alpha, ZView A, ZView B, double beta, ZView C) {
+    return zgemm(st, m, n, k, alpha, A.p, A.ld, B.p, B.ld, beta, C.p, C.ld);
+}
+
+int zgemm_batched(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda, long strideA,
+                  const double2 *B, long ldb, long strideB, double beta, double2 *C, long ldc, long strideC, int nbatch) {
+    if (m <= 0 || n <= 0 || nbatch <= 0) return 0;
+    if (n <= 32)
+        return launch_zgemm<8, 1, 8, 4, 1>(st, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, strideA, strideB, strideC, nbatch);
+    return launch_zgemm<4, 2, 16, 4, 1>(st, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, strideA, strideB, strideC, nbatch);
+}
+
+}  // namespace hp
+
+extern "C" int hprmat_zgemm(void *cuda_stream, int m, int n, int k, double alpha, const void *A, int lda, const void *B,
+                            int ldb, double beta, void *C, int ldc) {
+    if (m < 0) return -2;
+    if (n < 0) return -3;
+    if (k < 0) return -4;
+    if (lda < (m > 1 ? m : 1)) return -7;
+    if (ldb < (k > 1 ? k : 1)) return -9;
+    if (ldc < (m > 1 ? m : 1)) return -12;
+    return hp::zgemm((cudaStream_t)cuda_stream, m, n, k, alpha, (const double2 *)A, lda, (const double2 *)B, ldb, beta,
+                     (double2 *)C, ldc);
+}
