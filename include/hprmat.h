@@ -88,6 +88,12 @@ int hprmat_mesh(const hprmat_ctx *ctx, double *r, double *fa);
 int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int max_refine, double tol, void *R,
                  hprmat_info *info);
 
+/* Same call with HOST buffers (the end-to-end entry): V_host complex [nbasis][nch][nch] and R_host complex nch x nch are
+ * host pointers (pinned memory makes the copies asynchronous); the host->device copy of V, all kernels and the
+ * device->host copy of R are enqueued on the context's stream, which is synchronised before returning. */
+int hprmat_solve_host(hprmat_ctx *ctx, double energy, const void *V_host, int mode, int max_refine, double tol,
+                      void *R_host, hprmat_info *info);
+
 /* Solution block of the last hprmat_solve: X dev, complex N x nch column-major (copy out). */
 int hprmat_get_x(const hprmat_ctx *ctx, void *X);
 
@@ -123,11 +129,6 @@ int hprmat_zgetrs(void *cuda_stream, int n, int nrhs, const void *A, int lda, co
  * performs the trailing update of the LU.  A m x k, B k x n, C m x n. */
 int hprmat_zgemm(void *cuda_stream, int m, int n, int k, double alpha, const void *A, int lda, const void *B, int ldb,
                  double beta, void *C, int ldc);
-
-/* Same for split (planar) complex64: separate real and imaginary float planes, TF32 tensor cores, FP32 accumulate;
- * the trailing-update kernel of the mixed path. */
-int hprmat_cgemm_planar(void *cuda_stream, int m, int n, int k, float alpha, const float *Ar, const float *Ai, int lda,
-                        const float *Br, const float *Bi, int ldb, float beta, float *Cr, float *Ci, int ldc);
 
 const char *hprmat_strerror(int code);
 const char *hprmat_last_cuda_error(void);

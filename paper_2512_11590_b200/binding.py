@@ -1,0 +1,195 @@
+"""Thin ctypes binding of libhprmat.so (include/hprmat.h): argument marshalling only, same names as the C ABI.
+
+Device buffers are torch CUDA tensors (PyTorch is used for device memory and streams only); every arithmetic step
+runs in the library's own sm_100a kernels.  There is no CPU fallback: if the shared library is missing or no CUDA
+device is present the calls raise.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIBPATH = os.path.join(HERE, "libhprmat.so")
+
+HPRMAT_FP64, HPRMAT_MIXED, HPRMAT_MIXED_REFINE = 1, 2, 3
+HPRMAT_OK, HPRMAT_ESINGULAR, HPRMAT_ENOTCONVERGED, HPRMAT_ENOMEM, HPRMAT_ECUDA = 0, 1, 2, 3, 4
+MODES = {"fp64": HPRMAT_FP64, "mixed": HPRMAT_MIXED, "mixed_refine": HPRMAT_MIXED_REFINE}
+
+
+class hprmat_info(C.Structure):
+    _fields_ = [("status", C.c_int), ("refine_steps", C.c_int), ("pivot_index", C.c_int), ("reserved", C.c_int),
+                ("resid_max", C.c_double), ("backward_err", C.c_double),
+                ("ms_assemble", C.c_double), ("ms_lu", C.c_double), ("ms_solve", C.c_double),
+                ("ms_refine", C.c_double), ("ms_contract", C.c_double), ("ms_total", C.c_double),
+                ("lu_tflops", C.c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class HprmatError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        msg = lib().hprmat_strerror(C.c_int(code)).decode()
+        if code == HPRMAT_ECUDA:
+            msg += ": " + lib().hprmat_last_cuda_error().decode()
+        super().__init__(f"{where}: rc={code} ({msg})")
+
+
+_lib = None
+
+
+def lib():
+    """Load libhprmat.so (built in-tree by paper_2512_11590_b200.build); fails loudly if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIBPATH):
+            raise ImportError(f"{LIBPATH} not found: run `python -m paper_2512_11590_b200.build` (no CPU fallback)")
+        L = C.CDLL(LIBPATH)
+        L.hprmat_strerror.restype = C.c_char_p
+        L.hprmat_last_cuda_error.restype = C.c_char_p
+        L.hprmat_launch_count.restype = C.c_longlong
+        L.hprmat_workspace_bytes.restype = C.c_size_t
+        _lib = L
+    return _lib
+
+
+def _dev(t: torch.Tensor):
+    assert t.is_cuda, "device pointer expected"
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _check(rc, where, ok=(HPRMAT_OK,)):
+    if rc not in ok:
+        raise HprmatError(rc, where)
+    return rc
+
+
+def hprmat_launch_count() -> int:
+    return int(lib().hprmat_launch_count())
+
+
+# ---- structured R-matrix path ---------------------------------------------------------------------------------------
+class Context:
+    """Owner of an hprmat_ctx (hprmat_setup ... hprmat_destroy)."""
+
+    def __init__(self, nch, nbasis, a, h2m, lval, ethr, max_mode=0, stream=None):
+        self.nch, self.nb, self.n = int(nch), int(nbasis), int(nch) * int(nbasis)
+        lv = np.ascontiguousarray(lval, dtype=np.int32)
+        et = np.ascontiguousarray(ethr, dtype=np.float64)
+        assert lv.shape == (nch,) and et.shape == (nch,)
+        self._h = C.c_void_p()
+        self._stream = stream
+        rc = lib().hprmat_setup(C.byref(self._h), C.c_int(nch), C.c_int(nbasis), C.c_double(a), C.c_double(h2m),
+                                lv.ctypes.data_as(C.c_void_p), et.ctypes.data_as(C.c_void_p), C.c_int(max_mode),
+                                _stream(stream))
+        _check(rc, "hprmat_setup")
+
+    def mesh(self):
+        r = np.zeros(self.nb)
+        fa = np.zeros(self.nb)
+        _check(lib().hprmat_mesh(self._h, r.ctypes.data_as(C.c_void_p), fa.ctypes.data_as(C.c_void_p)), "hprmat_mesh")
+        return r, fa
+
+    def solve(self, energy, V, mode=HPRMAT_FP64, max_refine=-1, tol=0.0, R=None, want_info=True, allow=(HPRMAT_OK,)):
+        """hprmat_solve: V torch complex128 CUDA [nb, nch, nch]; returns (R [nch, nch] column-major as a torch tensor
+        holding R^T in row-major terms -- use .T for R[c1, c2]), info dict or None)."""
+        assert V.is_cuda and V.dtype == torch.complex128 and V.is_contiguous() and V.numel() == self.nb * self.nch ** 2
+        if R is None:
+            R = torch.empty((self.nch, self.nch), dtype=torch.complex128, device=V.device)
+        info = hprmat_info() if want_info else None
+        rc = lib().hprmat_solve(self._h, C.c_double(energy), _dev(V), C.c_int(mode), C.c_int(max_refine),
+                                C.c_double(tol), _dev(R), C.byref(info) if want_info else None)
+        _check(rc, "hprmat_solve", allow)
+        return R, (info.as_dict() if want_info else None)
+
+    def solve_host(self, energy, V_host, mode=HPRMAT_FP64, max_refine=-1, tol=0.0, R_host=None, allow=(HPRMAT_OK,)):
+        """hprmat_solve_host: V and R are HOST buffers (numpy complex128); copies are inside the call."""
+        V_host = np.ascontiguousarray(V_host, dtype=np.complex128)
+        if R_host is None:
+            R_host = np.empty((self.nch, self.nch), dtype=np.complex128)
+        info = hprmat_info()
+        rc = lib().hprmat_solve_host(self._h, C.c_double(energy), V_host.ctypes.data_as(C.c_void_p), C.c_int(mode),
+                                     C.c_int(max_refine), C.c_double(tol), R_host.ctypes.data_as(C.c_void_p),
+                                     C.byref(info))
+        _check(rc, "hprmat_solve_host", allow)
+        return R_host, info.as_dict()
+
+    def get_x(self, device="cuda"):
+        X = torch.empty((self.nch, self.n), dtype=torch.complex128, device=device)  # column-major N x nch
+        _check(lib().hprmat_get_x(self._h, _dev(X)), "hprmat_get_x")
+        return X
+
+    def get_matrix(self, energy, V):
+        Cm = torch.empty((self.n, self.n), dtype=torch.complex128, device=V.device)  # column-major N x N
+        _check(lib().hprmat_get_matrix(self._h, C.c_double(energy), _dev(V), _dev(Cm)), "hprmat_get_matrix")
+        return Cm
+
+    def destroy(self):
+        if self._h:
+            lib().hprmat_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+# ---- raw dense entries ----------------------------------------------------------------------------------------------
+def hprmat_workspace_bytes(n, nrhs, mode=HPRMAT_FP64) -> int:
+    return int(lib().hprmat_workspace_bytes(C.c_int(n), C.c_int(nrhs), C.c_int(mode)))
+
+
+def _workspace(n, nrhs, mode, device):
+    nbytes = hprmat_workspace_bytes(n, nrhs, mode)
+    return torch.empty(nbytes + 256, dtype=torch.uint8, device=device), nbytes
+
+
+def _aligned(ws):
+    off = (-ws.data_ptr()) % 256
+    return C.c_void_p(ws.data_ptr() + off)
+
+
+def hprmat_zgemm(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, stream=None):
+    rc = lib().hprmat_zgemm(_stream(stream), C.c_int(m), C.c_int(n), C.c_int(k), C.c_double(alpha), _dev(A),
+                            C.c_int(lda), _dev(B), C.c_int(ldb), C.c_double(beta), _dev(Cm), C.c_int(ldc))
+    _check(rc, "hprmat_zgemm")
+
+
+def hprmat_zgetrf(n, A, lda, ipiv, info_dev, ws=None, stream=None):
+    """In-place FP64 LU; A torch complex128 CUDA holding the column-major n x n matrix (lda >= n)."""
+    if ws is None:
+        ws, _ = _workspace(n, 0, HPRMAT_FP64, A.device)
+    rc = lib().hprmat_zgetrf(_stream(stream), C.c_int(n), _dev(A), C.c_int(lda), _dev(ipiv), _dev(info_dev),
+                             _aligned(ws), C.c_size_t(ws.numel() - 256))
+    _check(rc, "hprmat_zgetrf")
+    return ws
+
+
+def hprmat_zgetrs(n, nrhs, A, lda, ipiv, B, ldb, ws, stream=None):
+    rc = lib().hprmat_zgetrs(_stream(stream), C.c_int(n), C.c_int(nrhs), _dev(A), C.c_int(lda), _dev(ipiv), _dev(B),
+                             C.c_int(ldb), _aligned(ws), C.c_size_t(ws.numel() - 256))
+    _check(rc, "hprmat_zgetrs")
+
+
+def hprmat_zsolve(n, nrhs, A, lda, B, ldb, ipiv=None, mode=HPRMAT_FP64, max_refine=-1, tol=0.0, ws=None, stream=None,
+                  allow=(HPRMAT_OK,)):
+    if ipiv is None:
+        ipiv = torch.empty(max(n, 1), dtype=torch.int32, device=A.device)
+    if ws is None:
+        ws, _ = _workspace(n, nrhs, mode, A.device)
+    info = hprmat_info()
+    rc = lib().hprmat_zsolve(_stream(stream), C.c_int(n), C.c_int(nrhs), _dev(A), C.c_int(lda), _dev(B), C.c_int(ldb),
+                             _dev(ipiv), C.c_int(mode), C.c_int(max_refine), C.c_double(tol), _aligned(ws),
+                             C.c_size_t(ws.numel() - 256), C.byref(info))
+    _check(rc, "hprmat_zsolve", allow)
+    return ipiv, info.as_dict()

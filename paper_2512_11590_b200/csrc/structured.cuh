@@ -1,0 +1,33 @@
+// structured.cuh -- device tables of the Lagrange-Legendre problem and the O(N^2) kernels around the LU.
+#pragma once
+#include <algorithm>
+
+#include "common.cuh"
+
+namespace hp {
+
+// Device-resident tables computed once at hprmat_setup.
+struct StructTables {
+    int nch = 0, nb = 0;
+    double a = 0, h2m = 0;
+    const double *hT = nullptr;    // nb x nb column-major: (double)(h2m * T_ij), T = kinetic + Bloch in units h2m = 1
+    const double *dg0 = nullptr;   // [nch*nb]: h2m*T_ii + h2m*l_c(l_c+1)/r_i^2
+    const double *ethr = nullptr;  // [nch]
+    const double *fa = nullptr;    // [nb]: f_i(a)
+};
+
+int assemble_z(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double2 *C, long ldc);
+int build_rhs(cudaStream_t st, const StructTables &t, double2 *B, long ldb);
+// R <- Bx - (C - E I) X (Bx == nullptr: the surface right-hand sides), double-double accumulation; Rlo is scratch of
+// the same shape as R; rmax_dev (may be nullptr) receives max |R_ij|.
+int structured_residual(cudaStream_t st, const StructTables &t, double energy, const double2 *V, int nrhs,
+                        const double2 *Bx, long ldb, const double2 *X, long ldx, double2 *R, double2 *Rlo, long ldr,
+                        double *rmax_dev);
+int axpy_norm(cudaStream_t st, long rows, int cols, double2 *X, long ldx, const double2 *D, long ldd, double *norms_dev);
+int maxabs(cudaStream_t st, long rows, int cols, const double2 *X, long ldx, double *out_dev);
+int backward_error(cudaStream_t st, long rows, int nrhs, const double2 *R, long ldr, const double2 *X, long ldx,
+                   double anorm, double bnorm, double *out_dev);
+int structured_anorm(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double *out_dev);
+int contract(cudaStream_t st, const StructTables &t, const double2 *X, long ldx, double2 *R);
+
+}  // namespace hp

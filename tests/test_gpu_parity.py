@@ -1,0 +1,221 @@
+"""Parity of the CUDA path (through the C ABI, include/hprmat.h) with the CPU oracle, element by element on the same
+seeded inputs.  All tests here need a B200 ("-m gpu").
+
+Tolerances (BASELINE.json north_star; norms per DESIGN.md readings R7/R8):
+  FP64 path: max|R - R_orc| / max|R_orc| <= 1e-10, backward error <= 50 N 2^-53;
+  assembly: every entry within 4 ulp of the oracle's (the two sides evaluate the closed forms independently in long
+  double and round once; the FP64 evaluation order of the diagonal is fixed by reading R4), structural zeros exact;
+  integer/index work (pivots): validity of P A = L U, since ties make the pivot sequence non-unique (reading R6).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2512_11590_b200 import binding as hb
+from paper_2512_11590_b200.workloads import dense_test_matrix, make_workload
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def _dev_colmajor(a: np.ndarray) -> torch.Tensor:
+    """numpy (m, n) -> torch CUDA tensor of shape (n, m) whose memory is the column-major m x n matrix."""
+    return torch.from_numpy(np.ascontiguousarray(a.T)).to(DEV)
+
+
+def _host(t: torch.Tensor) -> np.ndarray:
+    """inverse of _dev_colmajor"""
+    return t.cpu().numpy().T
+
+
+def _ctx(w, max_mode=0):
+    return hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=max_mode)
+
+
+def _relmax(a, b):
+    return np.abs(a - b).max() / np.abs(b).max()
+
+
+# ---------------------------------------------------------------------------------------------------- setup tables
+@pytest.mark.parametrize("nb,a", [(2, 1.0), (5, 3.0), (37, 7.5), (50, 10.0), (100, 20.0), (151, 12.0)])
+def test_mesh_matches_oracle(nb, a):
+    w = make_workload(0, nch=2, nb=nb)
+    ctx = hb.Context(2, nb, a, w.h2m, w.lval[:2], w.ethr[:2], max_mode=1 << hb.HPRMAT_FP64)
+    r, fa = ctx.mesh()
+    _, _, r_o, fa_o = oracle.mesh(nb, a)
+    assert np.all(np.abs(r - r_o) <= 1 * np.spacing(r_o))
+    assert np.all(np.abs(fa - fa_o) <= 1 * np.spacing(np.abs(fa_o)))
+    ctx.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------- assembly
+@pytest.mark.parametrize("cfg,nch,nb", [(0, None, None), (1, 8, 100), (1, 5, 37), (2, 1, 64), (3, 3, 130), (1, 33, 20)])
+def test_assembly_parity(cfg, nch, nb):
+    w = make_workload(cfg, nch=nch, nb=nb)
+    ctx = _ctx(w, 1 << hb.HPRMAT_FP64)
+    r, _ = ctx.mesh()
+    V = w.potential(r)
+    E = float(w.energies[0])
+    Cg = _host(ctx.get_matrix(E, torch.from_numpy(V).to(DEV)))
+    Co = oracle.assemble(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, w.potential(oracle.mesh(w.nb, w.a)[2]))
+    assert Cg.shape == Co.shape == (w.n, w.n)
+    zero = Co == 0
+    assert np.all(Cg[zero] == 0), "structural zeros must be exact"
+    ulp = np.maximum(np.spacing(np.abs(Co.real)), np.spacing(np.abs(Co.imag)))
+    assert np.all(np.abs(Cg.real - Co.real) <= 4 * np.spacing(np.abs(Co.real)) + 0 * ulp)
+    assert np.all(np.abs(Cg.imag - Co.imag) <= 4 * np.spacing(np.abs(Co.imag)))
+    assert np.abs(Cg - Cg.T).max() == 0.0 or _relmax(Cg, Cg.T) < 1e-15   # complex symmetric
+    ctx.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------- raw GEMM / LU
+@pytest.mark.parametrize("m,n,k", [(1, 1, 1), (32, 32, 32), (100, 50, 37), (257, 129, 65), (130, 33, 300), (1000, 333, 200),
+                                   (5, 700, 3)])
+def test_zgemm_matches_definition(m, n, k):
+    rng = np.random.default_rng(m * 1000003 + n * 1009 + k)
+    A = rng.uniform(-1, 1, (m, k)) + 1j * rng.uniform(-1, 1, (m, k))
+    B = rng.uniform(-1, 1, (k, n)) + 1j * rng.uniform(-1, 1, (k, n))
+    C0 = rng.uniform(-1, 1, (m, n)) + 1j * rng.uniform(-1, 1, (m, n))
+    Cd = _dev_colmajor(C0)
+    hb.hprmat_zgemm(m, n, k, -1.0, _dev_colmajor(A), m, _dev_colmajor(B), k, 1.0, Cd, m)
+    ref = C0 - (A.astype(np.clongdouble) @ B.astype(np.clongdouble)).astype(np.complex128)
+    assert np.abs(_host(Cd) - ref).max() <= 4 * (k + 2) * 2.0 ** -53 * 2.0 * max(1.0, np.abs(ref).max())
+
+
+@pytest.mark.parametrize("n,nrhs", [(1, 1), (2, 3), (31, 1), (32, 5), (33, 2), (100, 7), (257, 4), (640, 64), (1500, 3)])
+def test_zsolve_fp64_matches_oracle(n, nrhs):
+    A = dense_test_matrix(n, nrhs, seed=7000 + n)
+    B = np.asfortranarray(A @ np.ones((n, nrhs), dtype=np.complex128))       # x_exact = 1
+    Xo = oracle.solve(A, B, mode=0, nrefine=2)
+    assert np.abs(Xo - 1.0).max() < 1e-12                                    # the oracle itself reproduces x = 1
+    Ad, Bd = _dev_colmajor(A), _dev_colmajor(B)
+    ipiv, info = hb.hprmat_zsolve(n, nrhs, Ad, n, Bd, n)
+    X = _host(Bd)
+    assert info["status"] == 0
+    assert _relmax(X, Xo) <= 1e-10
+    # the factors left in A and the 1-based interchanges are a valid P A = L U (not compared with the oracle's: ties)
+    LU = _host(Ad)
+    L = np.tril(LU, -1) + np.eye(n)
+    U = np.triu(LU)
+    piv = ipiv.cpu().numpy() - 1
+    assert piv.min() >= 0 and piv.max() < n and np.all(piv >= np.arange(n))
+    PA = A.copy()
+    for j in range(n):
+        if piv[j] != j:
+            PA[[j, piv[j]]] = PA[[piv[j], j]]
+    assert np.abs(L @ U - PA).max() <= 50 * n * 2.0 ** -53 * np.abs(A).sum(1).max()
+    assert np.abs(np.tril(LU, -1)).max() <= np.sqrt(2.0) + 1e-12             # partial pivoting on |re|+|im|
+
+
+def test_zsolve_reports_singular():
+    n = 64
+    A = dense_test_matrix(n, 1, seed=99)
+    A[:, 10] = 0.0
+    Ad, Bd = _dev_colmajor(A), _dev_colmajor(np.ones((n, 1), dtype=np.complex128))
+    with pytest.raises(hb.HprmatError) as e:
+        hb.hprmat_zsolve(n, 1, Ad, n, Bd, n)
+    assert e.value.code == hb.HPRMAT_ESINGULAR
+
+
+def test_zsolve_empty():
+    A = torch.zeros(1, dtype=torch.complex128, device=DEV)
+    ipiv, info = hb.hprmat_zsolve(0, 0, A, 1, A, 1)
+    assert info["status"] == 0
+
+
+# ---------------------------------------------------------------------------------------------------- whole path, FP64
+def _oracle_R(w, E, mode=0):
+    r = oracle.mesh(w.nb, w.a)[2]
+    return oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, w.potential(r), mode=mode, nrefine=2,
+                          return_x=True)
+
+
+@pytest.mark.parametrize("cfg,nch,nb", [(0, None, None), (0, 1, 50), (1, 8, 100), (1, 5, 37), (2, 16, 100), (3, 12, 64)])
+def test_rmatrix_fp64_parity(cfg, nch, nb):
+    w = make_workload(cfg, nch=nch, nb=nb)
+    ctx = _ctx(w, 1 << hb.HPRMAT_FP64)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    for E in w.energies[:2]:
+        R, info = ctx.solve(float(E), V, hb.HPRMAT_FP64)
+        Ro, Xo = _oracle_R(w, float(E))
+        Rg = _host(R)
+        assert info["status"] == 0
+        assert _relmax(Rg, Ro) <= 1e-10, (info, _relmax(Rg, Ro))
+        assert 0 <= info["backward_err"] <= 50 * w.n * 2.0 ** -53
+        assert _relmax(_host(ctx.get_x()), Xo) <= 1e-10
+        assert _relmax(Rg, Rg.T) <= 1e-10                                     # R = R^T since C = C^T
+    ctx.destroy()
+
+
+def test_rmatrix_fp64_host_entry_matches_device_entry():
+    w = make_workload(0)
+    ctx = _ctx(w, 1 << hb.HPRMAT_FP64)
+    r, _ = ctx.mesh()
+    Vh = w.potential(r)
+    R1, _ = ctx.solve(10.0, torch.from_numpy(Vh).to(DEV), hb.HPRMAT_FP64)
+    R2, info = ctx.solve_host(10.0, Vh, hb.HPRMAT_FP64)
+    assert np.array_equal(R1.cpu().numpy(), R2)
+    assert info["ms_total"] > 0 and info["lu_tflops"] > 0
+    ctx.destroy()
+
+
+def test_rmatrix_no_info_path_is_asynchronous_and_equal():
+    w = make_workload(1, nch=8, nb=100)
+    ctx = _ctx(w, 1 << hb.HPRMAT_FP64)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    R1, _ = ctx.solve(20.0, V, hb.HPRMAT_FP64, max_refine=1)
+    R2, none = ctx.solve(20.0, V, hb.HPRMAT_FP64, max_refine=1, want_info=False)
+    torch.cuda.synchronize()
+    assert none is None
+    assert _relmax(R2.cpu().numpy(), R1.cpu().numpy()) <= 1e-13
+    ctx.destroy()
+
+
+@pytest.mark.slow
+def test_rmatrix_fp64_cfg1_full_size():
+    """BASELINE.json configs[1] at full size (N = 6400), one energy; oracle in big-N mode (double accumulation in the
+    factorisation, long-double residual refinement), which test_oracle_pins checks against the long-double mode."""
+    w = make_workload(1)
+    ctx = _ctx(w, 1 << hb.HPRMAT_FP64)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    E = float(w.energies[3])
+    R, info = ctx.solve(E, V, hb.HPRMAT_FP64)
+    Ro, Xo = _oracle_R(w, E, mode=1)
+    assert _relmax(_host(R), Ro) <= 1e-10, info
+    assert 0 <= info["backward_err"] <= 50 * w.n * 2.0 ** -53
+    ctx.destroy()
+
+
+def _certificate(w, E, X, R):
+    """A-posteriori certificate: since C = C^T, R_exact - R~ = (h2m/a) X~^T (B - C X~) + O(r^2);
+    the residual is evaluated by the ORACLE in long double with the matrix-free operator."""
+    r = oracle.mesh(w.nb, w.a)[2]
+    res = oracle.structured_residual(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, w.potential(r), X)
+    dR = (w.h2m / w.a) * (X.T @ res)
+    return np.abs(dR).max() / np.abs(R).max(), np.abs(res).max()
+
+
+@pytest.mark.slow
+def test_rmatrix_fp64_cfg3_headline_size_certificate():
+    """BASELINE.json configs[3] (N = 25600) in the launch configuration bench.py times.  The full oracle needs ~10
+    core-hours here, so correctness is certified from the oracle's long-double residual of the GPU solution."""
+    w = make_workload(3)
+    ctx = _ctx(w, 1 << hb.HPRMAT_FP64)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    R, info = ctx.solve(30.0, V, hb.HPRMAT_FP64)
+    X = _host(ctx.get_x())
+    Rg = _host(R)
+    est, rmax = _certificate(w, 30.0, X, Rg)
+    assert est <= 1e-10, (est, rmax, info)
+    assert 0 <= info["backward_err"] <= 50 * w.n * 2.0 ** -53
+    assert _relmax(Rg, Rg.T) <= 1e-10
+    # sampled outputs the oracle can compute one by one: R_c1c2 = (h2m/a) sum_i fa_i X[(c1,i),c2] from the GPU's X
+    fa = oracle.mesh(w.nb, w.a)[3]
+    for (c1, c2) in [(0, 0), (3, 200), (255, 255), (17, 4)]:
+        assert abs(Rg[c1, c2] - (w.h2m / w.a) * np.dot(fa, X[c1 * w.nb:(c1 + 1) * w.nb, c2])) <= 1e-13 * np.abs(Rg).max()
+    ctx.destroy()
