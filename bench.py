@@ -1,0 +1,267 @@
+#!/usr/bin/env python
+"""bench.py -- time-to-R-matrix and complex-LU TFLOP/s (8 N^3 / 3) of the HPRMAT hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--mode fp64|mixed_refine|mixed] [--cfg 3] [--impl reference]
+
+One "step" = one hprmat_solve (assemble C - E I -> blocked LU -> triangular solves -> refinement -> R contraction) of
+BASELINE.json configs[cfg] (default 3: Nc=256, Nb=100, N=25600, the paper's headline size) on seeded synthetic inputs
+(paper_2512_11590_b200/workloads.py).  `value` = (8 N^3 / 3) / time-to-R-matrix summed over ranks, V resident in HBM;
+`e2e` = the same through hprmat_solve_host with V in pinned host memory and R read back to the host every step.
+N > 1 GPUs: the path does not shard (one LU is sequential in its panels) -> independent replicas, one energy point of a
+scan per rank, no data-path collective; torch.distributed only carries the barrier and the max-time.
+
+--impl reference: the CPU oracle (oracle/), as it stands, on the host cores, on a bounded sample of the same workload
+family (reduced channel count), same metric and unit.  That leg and the cpu_baseline object are the only places where
+bench.py executes oracle/.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "time-to-R-matrix and complex LU TFLOP/s (8N^3/3) at N=25600"
+UNIT = "TFLOP/s"
+CPU_SAMPLE_NCH = 64          # oracle sample: the cfg family reduced to 64 channels (N = 6400), long-double mode
+
+
+def lu_flops(n):
+    return 8.0 * n ** 3 / 3.0
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d, "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
+
+
+# FP64 tensor (DMMA) peak: 148 SMs x 128 FP64 flop/clk/SM x 1.965 GHz = 37.2 TFLOP/s; measured on this pool with a
+# register-resident mma.sync.m8n8k4.f64 loop: 37.15 TFLOP/s burst and sustained (profiles/r01_dmma_peak.md).  The ratio
+# to the driver's measured bf16 figure is not used because FP64 DMMA is not power-capped on this part.
+FP64_TENSOR_PEAK_TFLOPS = 37.15
+
+
+def oracle_sample(cfg, steps, warmup):
+    """Time the oracle on the bounded sample.  Returns (TFLOP/s by the 8N^3/3 convention, seconds per step, cores, text)."""
+    import oracle
+    from paper_2512_11590_b200.workloads import make_workload
+    w = make_workload(cfg, nch=CPU_SAMPLE_NCH)
+    r = oracle.mesh(w.nb, w.a)[2]
+    V = w.potential(r)
+    E = float(w.energies[0])
+    secs = []
+    for it in range(warmup + steps):
+        _, sec = oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, V, mode=0, nrefine=2, return_seconds=True)
+        if it >= warmup:
+            secs.append(sec)
+    t = statistics.mean(secs)
+    text = (f"configs[{cfg}] family reduced to Nc={w.nch}, Nb={w.nb} (N={w.n}); oracle long-double mode, factor + solves + 2 "
+            f"long-double-residual refinement steps + contraction; mean of {steps} run(s)")
+    return lu_flops(w.n) / t * 1e-12, t, oracle.num_threads(), text
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    v, t, cores, text = oracle_sample(args.cfg, max(1, args.steps), max(0, min(args.warmup, 1)))
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64 (long-double accumulation)", "data": "synthetic",
+            "config": {"workload": text},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [ln.split(",") for ln in open(self.f.name).read().strip().splitlines() if ln.count(",") >= 6]
+        os.unlink(self.f.name)
+        if not rows:
+            return out
+        sm = []
+        reasons = set()
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                out["sm_max_mhz"] = float(r[1])
+            except ValueError:
+                continue
+            for name, val in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], r[3:7]):
+                if val.strip().lower().startswith("active"):
+                    reasons.add(name)
+        if sm:
+            out["sm_mhz"] = statistics.median(sm)
+            out["samples"] = len(sm)
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--mode", default="fp64", choices=["fp64", "mixed", "mixed_refine"])
+    ap.add_argument("--cfg", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2512_11590_b200 import binding as hb
+    from paper_2512_11590_b200.workloads import make_workload
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = make_workload(args.cfg)
+    mode = hb.MODES[args.mode]
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
+    r, _ = ctx.mesh()
+    V_host = torch.from_numpy(w.potential(r)).pin_memory()
+    V = V_host.to("cuda")
+    R = torch.empty((w.nch, w.nch), dtype=torch.complex128, device="cuda")
+    R_host = torch.empty((w.nch, w.nch), dtype=torch.complex128).pin_memory()
+    # rank k takes the k-th point of an energy scan around the config's energy (replicas; weak scaling)
+    E = float(w.energies[0]) + 0.5 * rank
+    N = w.n
+
+    for _ in range(args.warmup):
+        ctx.solve(E, V, mode, R=R)
+    # ---- timed region: K steps, device-resident inputs
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    infos = []
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = hb.hprmat_launch_count()
+    e0.record()
+    for _ in range(args.steps):
+        _, info = ctx.solve(E, V, mode, R=R)
+        infos.append(info)
+    e1.record()
+    barrier()
+    launches = hb.hprmat_launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    t_dev = e0.elapsed_time(e1) * 1e-3
+    tt = torch.tensor([t_dev], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_max = float(tt.item())
+    sec_per_step = t_max / args.steps
+
+    # ---- end to end: host V in, host R out, through hprmat_solve_host, copies inside the timed region
+    Vh_np, Rh_np = V_host.numpy(), R_host.numpy()
+    ctx.solve_host(E, Vh_np, mode, R_host=Rh_np)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ctx.solve_host(E, Vh_np, mode, R_host=Rh_np)
+    torch.cuda.synchronize()
+    te = time.perf_counter() - t0
+    tt = torch.tensor([te], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    e2e_sec = float(tt.item()) / args.steps
+
+    # ---- roofline leg: one more step with a CUDA-event pair around every GEMM launch (the trailing-update kernel)
+    roof = None
+    if rank == 0:
+        hb.hprmat_profile(True)
+        _, pinfo = ctx.solve(E, V, mode, R=R)
+        hb.hprmat_profile(False)
+        g_ms, g_fl, g_n = hb.hprmat_profile_read()
+        pk, how = peaks()
+        if mode == hb.HPRMAT_FP64:
+            peak, pname = FP64_TENSOR_PEAK_TFLOPS, "FP64 DMMA peak measured on this pool with a register-resident mma.sync loop"
+        else:
+            peak = 0.5 * pk["bf16_tflops_sustained"]
+            pname = f"TF32 dense = 0.5 x bf16 sustained ({how})"
+        ach = g_fl / (g_ms * 1e-3) * 1e-12 if g_ms > 0 else 0.0
+        roof = {"bound": "tensor", "kernel": "zgemm_kernel (trailing update + TRSM GEMMs)" if mode == hb.HPRMAT_FP64 else
+                "cgemm trailing update", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                "traffic": None, "peak_source": pname, "launches": g_n, "kernel_ms_per_step": g_ms,
+                "share_of_step": g_ms / pinfo["ms_total"] if pinfo["ms_total"] else None,
+                "algorithmic_flops_per_step": g_fl}
+
+    if rank == 0:
+        info = infos[-1]
+        value = world * lu_flops(N) / sec_per_step * 1e-12
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64" if mode == hb.HPRMAT_FP64 else "tf32/f32 factors + f64 refinement",
+                "data": "synthetic",
+                "config": {"workload": f"BASELINE.json configs[{args.cfg}]: Nc={w.nch}, Nb={w.nb}, N={N}, a={w.a} fm, "
+                                       f"E={E} MeV, mode={args.mode}", "parallelism": f"replicas x{world}",
+                           "l2": "inputs_larger_than_L2 (matrix 16 N^2 B >> 126 MB)"},
+                "time_to_rmatrix_s": sec_per_step,
+                "lu_tflops": info["lu_tflops"],
+                "stages_ms": {k: info[k] for k in ("ms_assemble", "ms_lu", "ms_solve", "ms_refine", "ms_contract", "ms_total")},
+                "refine_steps": info["refine_steps"], "backward_err": info["backward_err"],
+                "e2e": {"value": world * lu_flops(N) / e2e_sec * 1e-12, "unit": UNIT, "seconds_per_step": e2e_sec,
+                        "h2d_bytes_per_step": int(V_host.numel() * 16), "d2h_bytes_per_step": int(R_host.numel() * 16)},
+                "gpu_launches": int(launches), "clocks": clocks, "roofline": roof,
+                "paper_context": {"rtx3090_fp32_s": 3.554, "rtx3090_hybrid_s": 9.85, "xeon48_zgesv_s": 52.098,
+                                  "legacy_inversion_s": 144.948, "note": "PAPER.md Tables 3-4, N=25600, other hardware"}}
+        if not args.no_cpu_baseline and world == 1:
+            v, t, cores, text = oracle_sample(args.cfg, 1, 0)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text,
+                                    "seconds": t}
+        print(json.dumps(line))
+    ctx.destroy()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

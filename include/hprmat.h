@@ -132,6 +132,12 @@ int hprmat_zgemm(void *cuda_stream, int m, int n, int k, double alpha, const voi
 
 const char *hprmat_strerror(int code);
 const char *hprmat_last_cuda_error(void);
+/* Measurement aid (bench.py's roofline leg): while enabled, every launch of the GEMM kernel inside the LU and the
+ * triangular solves is bracketed by a CUDA-event pair on its stream.  hprmat_profile_read synchronises those events,
+ * returns the summed kernel milliseconds, the summed algorithmic flops (8 m n k per launch) and the launch count, and
+ * resets the record. */
+int hprmat_profile(int enable);
+int hprmat_profile_read(double *ms, double *flops, long long *launches);
 /* number of kernel launches issued by this library since process start (bench.py's gpu_launches) */
 long long hprmat_launch_count(void);
 

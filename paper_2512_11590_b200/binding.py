@@ -76,6 +76,16 @@ def hprmat_launch_count() -> int:
     return int(lib().hprmat_launch_count())
 
 
+def hprmat_profile(enable: bool):
+    _check(lib().hprmat_profile(C.c_int(1 if enable else 0)), "hprmat_profile")
+
+
+def hprmat_profile_read():
+    ms, fl, n = C.c_double(0), C.c_double(0), C.c_longlong(0)
+    _check(lib().hprmat_profile_read(C.byref(ms), C.byref(fl), C.byref(n)), "hprmat_profile_read")
+    return ms.value, fl.value, n.value
+
+
 # ---- structured R-matrix path ---------------------------------------------------------------------------------------
 class Context:
     """Owner of an hprmat_ctx (hprmat_setup ... hprmat_destroy)."""

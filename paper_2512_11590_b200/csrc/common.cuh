@@ -35,6 +35,10 @@ inline int cuda_fail(cudaError_t e, const char *file, int line) {
 
 constexpr int kNumSMs = 148;  // B200
 
+bool prof_enabled();
+void prof_begin(cudaStream_t st, double flops);
+void prof_end(cudaStream_t st);
+
 inline int ceil_div(long a, long b) { return (int)((a + b - 1) / b); }
 inline long round_up(long a, long b) { return (a + b - 1) / b * b; }
 

@@ -1,10 +1,53 @@
 // util.cu -- process-wide state behind the C ABI: error strings and the launch counter.
+#include <vector>
+
 #include "common.cuh"
 
 namespace hp {
 thread_local char g_cuda_err[256] = "";
 long long g_launches = 0;
+
+// ---- optional per-launch timing of the GEMM kernel (bench.py's roofline leg): one CUDA-event pair around every launch
+struct ProfRec { cudaEvent_t a, b; double flops; };
+static bool g_prof_on = false;
+static std::vector<ProfRec> g_prof;
+static std::vector<cudaEvent_t> g_prof_pool;
+static cudaEvent_t prof_event() {
+    cudaEvent_t e = nullptr;
+    if (!g_prof_pool.empty()) { e = g_prof_pool.back(); g_prof_pool.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+}
+bool prof_enabled() { return g_prof_on; }
+void prof_begin(cudaStream_t st, double flops) {
+    ProfRec r{prof_event(), prof_event(), flops};
+    cudaEventRecord(r.a, st);
+    g_prof.push_back(r);
+}
+void prof_end(cudaStream_t st) { cudaEventRecord(g_prof.back().b, st); }
 }  // namespace hp
+
+extern "C" int hprmat_profile(int enable) {
+    hp::g_prof_on = enable != 0;
+    return HPRMAT_OK;
+}
+extern "C" int hprmat_profile_read(double *ms, double *flops, long long *launches) {
+    double t = 0.0, f = 0.0;
+    long long n = 0;
+    for (auto &r : hp::g_prof) {
+        if (cudaEventSynchronize(r.b) != cudaSuccess) return HPRMAT_ECUDA;
+        float m = 0.f;
+        cudaEventElapsedTime(&m, r.a, r.b);
+        t += m; f += r.flops; ++n;
+        hp::g_prof_pool.push_back(r.a);
+        hp::g_prof_pool.push_back(r.b);
+    }
+    hp::g_prof.clear();
+    if (ms) *ms = t;
+    if (flops) *flops = f;
+    if (launches) *launches = n;
+    return HPRMAT_OK;
+}
 
 extern "C" const char *hprmat_strerror(int code) {
     switch (code) {

@@ -177,7 +177,11 @@ int zgemm(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, 
 }
 
 int gemm(cudaStream_t st, int m, int n, int k, double alpha, ZView A, ZView B, double beta, ZView C) {
-    return zgemm(st, m, n, k, alpha, A.p, A.ld, B.p, B.ld, beta, C.p, C.ld);
+    const bool prof = prof_enabled() && m > 0 && n > 0 && k > 0;
+    if (prof) prof_begin(st, 8.0 * m * n * k);
+    const int rc = zgemm(st, m, n, k, alpha, A.p, A.ld, B.p, B.ld, beta, C.p, C.ld);
+    if (prof) prof_end(st);
+    return rc;
 }
 
 int zgemm_batched(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda, long strideA,
