@@ -85,6 +85,39 @@ def run_reference(args):
     return 0
 
 
+def run_probe(args):
+    """Kernel probes (one JSON line each): the GEMM entry alone, or the DMMA ceiling."""
+    import torch
+    from paper_2512_11590_b200 import binding as hb
+    torch.cuda.set_device(0)
+    if args.probe == "dmma":
+        out = []
+        for cps in (1, 2, 4):
+            tf, ms = hb.hprmat_probe_dmma(40000, cps)
+            out.append({"ctas_per_sm": cps, "tflops": tf, "ms": ms})
+        print(json.dumps({"probe": "dmma", "runs": out, "peak_tflops": max(o["tflops"] for o in out)}))
+        return 0
+    m, n, k = args.m, args.n, args.k
+    g = torch.Generator(device="cuda").manual_seed(1)
+    A = torch.randn((k, m), dtype=torch.complex128, device="cuda", generator=g)   # column-major m x k
+    B = torch.randn((n, k), dtype=torch.complex128, device="cuda", generator=g)   # column-major k x n
+    Cm = torch.randn((n, m), dtype=torch.complex128, device="cuda", generator=g)  # column-major m x n
+    for _ in range(args.warmup):
+        hb.hprmat_zgemm(m, n, k, -1.0, A, m, B, k, 1.0, Cm, m)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        hb.hprmat_zgemm(m, n, k, -1.0, A, m, B, k, 1.0, Cm, m)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    tf = 8.0 * m * n * k / (ms * 1e-3) * 1e-12
+    print(json.dumps({"probe": "zgemm", "m": m, "n": n, "k": k, "ms": ms, "tflops": tf,
+                      "frac_of_dmma_peak": tf / FP64_TENSOR_PEAK_TFLOPS}))
+    return 0
+
+
 class ClockSampler:
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
@@ -139,9 +172,17 @@ def main():
     ap.add_argument("--cfg", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--probe", default=None, choices=["zgemm", "dmma"],
+                    help="kernel probes instead of the step: zgemm = hprmat_zgemm alone at --m/--n/--k; dmma = FP64 "
+                         "tensor-core issue-rate ceiling (hprmat_probe_dmma)")
+    ap.add_argument("--m", type=int, default=12800)
+    ap.add_argument("--n", type=int, default=12800)
+    ap.add_argument("--k", type=int, default=1024)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.probe:
+        return run_probe(args)
 
     import torch
     from paper_2512_11590_b200 import binding as hb

@@ -130,6 +130,13 @@ int hprmat_zgetrs(void *cuda_stream, int n, int nrhs, const void *A, int lda, co
 int hprmat_zgemm(void *cuda_stream, int m, int n, int k, double alpha, const void *A, int lda, const void *B, int ldb,
                  double beta, void *C, int ldc);
 
+/* C <- beta*C + alpha*A*B on SPLIT-complex (planar) complex64 operands: every matrix is a pair of column-major float
+ * planes (re, im).  The tcgen05 (kind::tf32, FP32 accumulation in TMEM) kernel that performs the trailing update of the
+ * low-precision LU of the mixed modes.  All pointers dev; plane base addresses 16-byte
+ * aligned; lda, ldb multiples of 4.  Operands are rounded to TF32 (10-bit mantissa) by the tensor core. */
+int hprmat_cgemm_tf32(void *cuda_stream, int m, int n, int k, float alpha, const float *A_re, const float *A_im, int lda,
+                      const float *B_re, const float *B_im, int ldb, float beta, float *C_re, float *C_im, int ldc);
+
 const char *hprmat_strerror(int code);
 const char *hprmat_last_cuda_error(void);
 /* Measurement aid (bench.py's roofline leg): while enabled, every launch of the GEMM kernel inside the LU and the
@@ -138,6 +145,10 @@ const char *hprmat_last_cuda_error(void);
  * resets the record. */
 int hprmat_profile(int enable);
 int hprmat_profile_read(double *ms, double *flops, long long *launches);
+/* Measurement aid: FP64 tensor-core (DMMA, mma.sync.m8n8k4.f64) issue-rate ceiling of the device, measured with a
+ * register-resident loop (no memory traffic) on 148*ctas_per_sm CTAs of 8 warps, `iters` x 8 MMAs per warp.
+ * tflops (host, out): real TFLOP/s; ms (host, out, may be NULL): device time of the timed launch.  Synchronises. */
+int hprmat_probe_dmma(void *cuda_stream, int iters, int ctas_per_sm, double *tflops, double *ms);
 /* number of kernel launches issued by this library since process start (bench.py's gpu_launches) */
 long long hprmat_launch_count(void);
 

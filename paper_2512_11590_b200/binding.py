@@ -86,6 +86,13 @@ def hprmat_profile_read():
     return ms.value, fl.value, n.value
 
 
+def hprmat_probe_dmma(iters=20000, ctas_per_sm=2, stream=None):
+    tf, ms = C.c_double(0), C.c_double(0)
+    _check(lib().hprmat_probe_dmma(_stream(stream), C.c_int(iters), C.c_int(ctas_per_sm), C.byref(tf), C.byref(ms)),
+           "hprmat_probe_dmma")
+    return tf.value, ms.value
+
+
 # ---- structured R-matrix path ---------------------------------------------------------------------------------------
 class Context:
     """Owner of an hprmat_ctx (hprmat_setup ... hprmat_destroy)."""
@@ -173,6 +180,14 @@ def hprmat_zgemm(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, stream=None):
     rc = lib().hprmat_zgemm(_stream(stream), C.c_int(m), C.c_int(n), C.c_int(k), C.c_double(alpha), _dev(A),
                             C.c_int(lda), _dev(B), C.c_int(ldb), C.c_double(beta), _dev(Cm), C.c_int(ldc))
     _check(rc, "hprmat_zgemm")
+
+
+def hprmat_cgemm_tf32(m, n, k, alpha, A_re, A_im, lda, B_re, B_im, ldb, beta, C_re, C_im, ldc, stream=None):
+    """Planar complex64 GEMM on the tcgen05 TF32 tensor cores; all operands torch float32 CUDA tensors (column-major)."""
+    rc = lib().hprmat_cgemm_tf32(_stream(stream), C.c_int(m), C.c_int(n), C.c_int(k), C.c_float(alpha), _dev(A_re),
+                                 _dev(A_im), C.c_int(lda), _dev(B_re), _dev(B_im), C.c_int(ldb), C.c_float(beta),
+                                 _dev(C_re), _dev(C_im), C.c_int(ldc))
+    _check(rc, "hprmat_cgemm_tf32")
 
 
 def hprmat_zgetrf(n, A, lda, ipiv, info_dev, ws=None, stream=None):

@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "lu.cuh"
+#include "precond.cuh"
 #include "structured.cuh"
 
 using namespace hp;
@@ -34,6 +35,12 @@ struct hprmat_ctx {
     double *h_scal = nullptr;                                 // pinned mirror
     int *h_info = nullptr;                                    // pinned
     LuWork<ZView> wz;
+    // mixed modes: split-complex64 system S = K_d^-1 (C - E I), its right-hand sides, the FP64 block inverses
+    float *d_Sre = nullptr, *d_Sim = nullptr, *d_Bre = nullptr, *d_Bim = nullptr;
+    double2 *d_Kinv = nullptr;
+    void *d_workc = nullptr;
+    long ldS = 0;
+    LuWork<CView> wc;
     cudaEvent_t ev[8] = {};
     bool have_x = false;
     StructTables tab;
@@ -80,6 +87,7 @@ int free_ctx(hprmat_ctx *c) {
     if (!c) return 0;
     cudaFree(c->d_hT); cudaFree(c->d_dg0); cudaFree(c->d_ethr); cudaFree(c->d_fa);
     cudaFree(c->d_C); cudaFree(c->d_X); cudaFree(c->d_Rr); cudaFree(c->d_Rlo); cudaFree(c->d_V); cudaFree(c->d_R);
+    cudaFree(c->d_Sre); cudaFree(c->d_Sim); cudaFree(c->d_Bre); cudaFree(c->d_Bim); cudaFree(c->d_Kinv); cudaFree(c->d_workc);
     cudaFree(c->d_work); cudaFree(c->d_ipiv); cudaFree(c->d_info); cudaFree(c->d_scal);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     if (c->h_info) cudaFreeHost(c->h_info);
@@ -176,6 +184,18 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
         const size_t wb = LuWork<ZView>::bytes((int)N);
         HP_ALLOC(c->d_work, wb);
         c->wz.carve(c->d_work, (int)N);
+    }
+    if (max_mode & ((1 << HPRMAT_MIXED) | (1 << HPRMAT_MIXED_REFINE))) {
+        c->ldS = round_up(N, 32);
+        HP_ALLOC(c->d_Sre, sizeof(float) * c->ldS * N);
+        HP_ALLOC(c->d_Sim, sizeof(float) * c->ldS * N);
+        HP_ALLOC(c->d_Bre, sizeof(float) * c->ldS * nch);
+        HP_ALLOC(c->d_Bim, sizeof(float) * c->ldS * nch);
+        HP_ALLOC(c->d_Kinv, sizeof(double2) * (size_t)nch * nb * nb);
+        const size_t wb = LuWork<CView>::bytes((int)N);
+        HP_ALLOC(c->d_workc, wb);
+        if (cudaMemsetAsync(c->d_workc, 0, wb, c->st) != cudaSuccess) { free_ctx(c); return HPRMAT_ECUDA; }
+        c->wc.carve(c->d_workc, (int)N);
     }
     HP_ALLOC(c->d_X, sizeof(double2) * N * nch);
     HP_ALLOC(c->d_Rr, sizeof(double2) * N * nch);
@@ -332,6 +352,99 @@ int solve_fp64(hprmat_ctx *c, double energy, const double2 *V, int max_refine, d
     return status;
 }
 
+// Mixed modes (PAPER.md:147-151 Type 2, :192-230 Type 4; preconditioned per reading R10):
+//   Kinv = K_d^-1 (FP64) -> S = K_d^-1 (C - E I) in split complex64 -> P L U = S (TF32 tensor-core trailing update)
+//   -> X0 = S^-1 (K_d^-1 B)  [HPRMAT_MIXED stops here]
+//   -> repeat: r = B - (C - E I) X (FP64, double-double, matrix-free); z = K_d^-1 r (FP64); d = S^-1 z (complex64
+//      factors); X += d; until the correction is below tol or stagnates.
+int solve_mixed(hprmat_ctx *c, double energy, const double2 *V, bool refine, int max_refine, double tol, double2 *R,
+                hprmat_info *info) {
+    cudaStream_t st = c->st;
+    const int N = c->n, nch = c->nch, nb = c->nb;
+    const bool timed = info != nullptr;
+    CView S(c->d_Sre, c->d_Sim, c->ldS), Bs(c->d_Bre, c->d_Bim, c->ldS);
+    if (max_refine < 0) max_refine = 5;
+    if (!refine) max_refine = 0;
+    if (!(tol > 0.0)) tol = 1e-13;
+    int status = HPRMAT_OK, steps = 0;
+
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[0], st));
+    HP_CUDA(cudaMemsetAsync(c->d_info, 0, 2 * sizeof(int), st));
+    HP_TRY(precond_invert(st, c->tab, energy, V, c->d_Kinv, c->d_info + 1));
+    HP_TRY(precond_assemble(st, c->tab, c->d_Kinv, V, S));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[1], st));
+    HP_TRY(getrf<CView>(st, N, S, c->d_ipiv, c->d_info, c->wc));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[2], st));
+    if (timed) {
+        HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        if (c->h_info[0] != 0 || c->h_info[1] != 0) {
+            info->status = HPRMAT_ESINGULAR;
+            info->pivot_index = c->h_info[0] ? c->h_info[0] : c->h_info[1];
+            return HPRMAT_ESINGULAR;
+        }
+    }
+    HP_TRY(precond_rhs(st, c->tab, c->d_Kinv, Bs));
+    HP_TRY(getrs<CView>(st, N, nch, S, Bs, c->wc));
+    HP_TRY(promote_add(st, N, nch, c->d_X, N, Bs, false, c->d_scal));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[3], st));
+    double dprev = 0.0;
+    if (max_refine > 0) {
+        HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        dprev = c->h_scal[1];
+        status = HPRMAT_ENOTCONVERGED;
+    }
+    for (int k = 0; k < max_refine; ++k) {
+        HP_TRY(structured_residual(st, c->tab, energy, V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, c->d_scal + 3));
+        // z = K_d^-1 r: one nb x nb by nb x nch product per channel (FP64 tensor cores), into Rlo
+        HP_TRY(zgemm_batched(st, nb, nch, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, c->d_Rr, N, nb, 0.0, c->d_Rlo, N, nb, nch));
+        HP_TRY(demote(st, N, nch, c->d_Rlo, N, Bs));
+        HP_TRY(getrs<CView>(st, N, nch, S, Bs, c->wc));
+        HP_TRY(promote_add(st, N, nch, c->d_X, N, Bs, true, c->d_scal));
+        ++steps;
+        HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        const double dn = c->h_scal[0], xn = c->h_scal[1];
+        const int v = refine_verdict(dn, xn, dprev, tol);
+        dprev = dn;
+        if (v == REF_CONVERGED) { status = HPRMAT_OK; break; }
+        if (v == REF_STAGNATED) {
+            // a correction at the FP64 rounding floor of X is convergence, not failure
+            status = (dn <= 64.0 * 2.220446049250313e-16 * xn) ? HPRMAT_OK : HPRMAT_ENOTCONVERGED;
+            break;
+        }
+    }
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[4], st));
+    HP_TRY(contract(st, c->tab, c->d_X, N, R));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[5], st));
+    c->have_x = true;
+    if (timed) {
+        HP_TRY(structured_residual(st, c->tab, energy, V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, c->d_scal + 3));
+        HP_TRY(structured_anorm(st, c->tab, energy, V, c->d_scal + 4));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 3, c->d_scal + 3, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        double bn = 0.0;
+        for (double f : c->fa) bn = std::max(bn, fabs(f));
+        HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        info->status = status;
+        info->refine_steps = steps;
+        info->pivot_index = 0;
+        info->resid_max = c->h_scal[3];
+        info->backward_err = c->h_scal[5];
+        info->ms_assemble = ev_ms(c->ev[0], c->ev[1]);
+        info->ms_lu = ev_ms(c->ev[1], c->ev[2]);
+        info->ms_solve = ev_ms(c->ev[2], c->ev[3]);
+        info->ms_refine = ev_ms(c->ev[3], c->ev[4]);
+        info->ms_contract = ev_ms(c->ev[4], c->ev[5]);
+        info->ms_total = ev_ms(c->ev[0], c->ev[5]);
+        info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)N * N * N / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
+    }
+    return status;
+}
+
 }  // namespace
 
 extern "C" int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int max_refine, double tol, void *R,
@@ -349,7 +462,7 @@ extern "C" int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int m
     if (mode == HPRMAT_FP64) {
         rc = solve_fp64(ctx, energy, (const double2 *)V, max_refine, tol, (double2 *)R, info);
     } else {
-        return -4;  // the mixed path is not built yet
+        rc = solve_mixed(ctx, energy, (const double2 *)V, mode == HPRMAT_MIXED_REFINE, max_refine, tol, (double2 *)R, info);
     }
     if (info) info->status = rc;
     return rc;

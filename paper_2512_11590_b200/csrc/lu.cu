@@ -411,6 +411,9 @@ template <class V> int getrs(cudaStream_t st, int n, int nrhs, V A, V B, LuWork<
     return trsm_upper(st, A, 0, n, B, nrhs, wk);
 }
 
+template struct LuWork<CView>;
+template int getrf<CView>(cudaStream_t, int, CView, int *, int *, LuWork<CView> &);
+template int getrs<CView>(cudaStream_t, int, int, CView, CView, LuWork<CView> &);
 template struct LuWork<ZView>;
 template int getrf<ZView>(cudaStream_t, int, ZView, int *, int *, LuWork<ZView> &);
 template int getrs<ZView>(cudaStream_t, int, int, ZView, ZView, LuWork<ZView> &);

@@ -1,0 +1,272 @@
+// precond.cu -- the FP64 block-diagonal preconditioner of the mixed-precision path and the kernels that move between the
+// FP64 problem and the split-complex64 system the tensor cores factorise (reading R10).
+//
+// With K_d = blockdiag(K_1 .. K_Nc), K_c = the Nb x Nb diagonal block of C - E*I (kinetic + Bloch + centrifugal +
+// threshold + V_cc, Eqs. 1, 3 of PAPER.md:73-97), the paper's Type 3 writes M = K_d (I + K_d^-1 V_coupling)
+// (Eqs. 6-9).  The mixed path factorises  S = K_d^-1 (C - E*I) = I + K_d^-1 V_coupling  in complex64:
+//     S[(c,i),(c',j)] = delta_cc' delta_ij + (1 - delta_cc') Kinv_c[i,j] V_cc'(r_j)
+// and solves  S X = K_d^-1 B;  the FP64 residual of the refinement is always that of the ORIGINAL system
+// (PAPER.md:151, 222), mapped through K_d^-1 before the low-precision correction solve.
+#include "precond.cuh"
+
+namespace hp {
+
+// ---------------------------------------------------------------------------------------------------- K_c^-1
+// One CTA per channel: Gauss-Jordan inversion in place with partial pivoting (first row of maximal |re|+|im|), matrix
+// column-major n x n in shared memory when it fits (n <= 118), else in its global output buffer (L2-resident).
+constexpr int KI_NT = 512;
+
+__global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const double *__restrict__ hT,
+                                                     const double *__restrict__ dg0, const double *__restrict__ ethr,
+                                                     double energy, const double2 *__restrict__ V, double2 *__restrict__ Kinv,
+                                                     int use_smem, int *info) {
+    extern __shared__ __align__(16) unsigned char smraw[];
+    const int c = blockIdx.x, n = nb, tid = threadIdx.x;
+    double2 *out = Kinv + (size_t)c * n * n;
+    double2 *rowk = reinterpret_cast<double2 *>(smraw);  // [n] pivot row
+    double2 *colk = rowk + n;                            // [n] pivot column
+    int *piv = reinterpret_cast<int *>(colk + n);        // [n]
+    double2 *a = use_smem ? reinterpret_cast<double2 *>(piv + ((n + 3) & ~3)) : out;
+    __shared__ double red_v[KI_NT / 32];
+    __shared__ int red_i[KI_NT / 32];
+    __shared__ int s_p;
+
+    for (int idx = tid; idx < n * n; idx += KI_NT) {
+        const int i = idx % n, j = idx / n;
+        double2 v = make_double2(hT[(size_t)j * n + i], 0.0);
+        if (i == j) {
+            const double2 vd = V[((size_t)i * nch + c) * nch + c];
+            const double d2 = __dadd_rn(dg0[(size_t)c * n + i], __dsub_rn(ethr[c], energy));
+            v.x = __dadd_rn(d2, vd.x);
+            v.y = vd.y;
+        }
+        a[idx] = v;
+    }
+    __syncthreads();
+
+    for (int k = 0; k < n; ++k) {
+        // pivot search in column k, rows >= k
+        double bv = -1.0;
+        int bi = -1;
+        for (int i = k + tid; i < n; i += KI_NT) {
+            const double v = cabs1(a[(size_t)k * n + i]);
+            if (v > bv) { bv = v; bi = i; }
+        }
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            const double ov = __shfl_down_sync(0xffffffffu, bv, off);
+            const int oi = __shfl_down_sync(0xffffffffu, bi, off);
+            if (ov > bv || (ov == bv && oi >= 0 && (bi < 0 || oi < bi))) { bv = ov; bi = oi; }
+        }
+        if ((tid & 31) == 0) { red_v[tid >> 5] = bv; red_i[tid >> 5] = bi; }
+        __syncthreads();
+        if (tid == 0) {
+            for (int w = 1; w < KI_NT / 32; ++w)
+                if (red_v[w] > bv || (red_v[w] == bv && red_i[w] >= 0 && (bi < 0 || red_i[w] < bi))) { bv = red_v[w]; bi = red_i[w]; }
+            s_p = bi;
+            piv[k] = bi;
+            if (!(bv > 0.0)) atomicCAS(info, 0, c * n + k + 1);
+        }
+        __syncthreads();
+        const int p = s_p;
+        // swap rows k and p, stage the (swapped) pivot row and pivot column
+        for (int j = tid; j < n; j += KI_NT) {
+            const double2 vk = a[(size_t)j * n + k], vp = a[(size_t)j * n + p];
+            if (p != k) { a[(size_t)j * n + k] = vp; a[(size_t)j * n + p] = vk; }
+            rowk[j] = vp;
+        }
+        __syncthreads();
+        for (int i = tid; i < n; i += KI_NT) colk[i] = a[(size_t)k * n + i];
+        __syncthreads();
+        const double2 pv = rowk[k];
+        const bool sing = (pv.x == 0.0 && pv.y == 0.0);
+        const double2 ip = sing ? make_double2(0.0, 0.0) : crecip(pv);
+        // a[i][j] <- a[i][j] - colk[i] * (rowk[j] * ip)   for i != k;  row k <- rowk * ip;  column k <- -colk*ip, [k][k] = ip
+        for (int idx = tid; idx < n * n; idx += KI_NT) {
+            const int i = idx % n, j = idx / n;
+            double2 v;
+            if (j == k) {
+                v = (i == k) ? ip : cmul(make_double2(-colk[i].x, -colk[i].y), ip);
+            } else {
+                const double2 rj = cmul(rowk[j], ip);
+                v = (i == k) ? rj : cfnma(a[idx], colk[i], rj);
+            }
+            a[idx] = v;
+        }
+        __syncthreads();
+    }
+    // undo the row interchanges: columns of the inverse, in reverse order
+    for (int k = n - 1; k >= 0; --k) {
+        const int p = piv[k];
+        if (p != k) {
+            for (int i = tid; i < n; i += KI_NT) {
+                const double2 t = a[(size_t)k * n + i];
+                a[(size_t)k * n + i] = a[(size_t)p * n + i];
+                a[(size_t)p * n + i] = t;
+            }
+        }
+        __syncthreads();
+    }
+    if (use_smem)
+        for (int idx = tid; idx < n * n; idx += KI_NT) out[idx] = a[idx];
+}
+
+int precond_invert(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double2 *Kinv, int *info_dev) {
+    const int n = t.nb;
+    const size_t small = sizeof(double2) * 2 * n + sizeof(int) * ((n + 3) & ~3);
+    const size_t full = small + sizeof(double2) * (size_t)n * n;
+    const int use_smem = full <= 200 * 1024;
+    const size_t smem = use_smem ? full : small;
+    static size_t configured = 48 * 1024;
+    if (smem > configured) {
+        HP_CUDA(cudaFuncSetAttribute(kinv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    kinv_kernel<<<t.nch, KI_NT, smem, st>>>(t.nch, n, t.hT, t.dg0, t.ethr, energy, V, Kinv, use_smem, info_dev);
+    HP_LAUNCHED();
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------------- assemble S
+// Thread = one row (c,i) x one mesh column j x SA_CC consecutive column channels c': loads Kinv_c[i,j] once and writes
+// SA_CC entries, each store instruction of a warp covering 128 contiguous bytes of a plane.
+constexpr int SA_NT = 256, SA_CC = 8;
+
+__global__ void __launch_bounds__(SA_NT) assemble_s_kernel(int nch, int nb, const double2 *__restrict__ Kinv,
+                                                           const double2 *__restrict__ V, float *__restrict__ Sre,
+                                                           float *__restrict__ Sim, long ld) {
+    const int N = nch * nb;
+    const int row = blockIdx.x * SA_NT + threadIdx.x;
+    if (row >= N) return;
+    const int c = row / nb, i = row - c * nb;
+    const int j = blockIdx.y;
+    const int cc0 = blockIdx.z * SA_CC;
+    const double2 kij = Kinv[((size_t)c * nb + j) * nb + i];
+#pragma unroll
+    for (int e = 0; e < SA_CC; ++e) {
+        const int c2 = cc0 + e;
+        if (c2 >= nch) break;
+        float re, im;
+        if (c2 == c) {
+            re = (i == j) ? 1.f : 0.f;
+            im = 0.f;
+        } else {
+            const double2 v = V[((size_t)j * nch + c2) * nch + c];
+            re = (float)(kij.x * v.x - kij.y * v.y);
+            im = (float)(kij.x * v.y + kij.y * v.x);
+        }
+        const size_t off = (size_t)(c2 * nb + j) * ld + row;
+        Sre[off] = re;
+        Sim[off] = im;
+    }
+}
+
+int precond_assemble(cudaStream_t st, const StructTables &t, const double2 *Kinv, const double2 *V, CView S) {
+    const int N = t.nch * t.nb;
+    dim3 grid(ceil_div(N, SA_NT), t.nb, ceil_div(t.nch, SA_CC));
+    assemble_s_kernel<<<grid, SA_NT, 0, st>>>(t.nch, t.nb, Kinv, V, S.re, S.im, S.ld);
+    HP_LAUNCHED();
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------------- right-hand side
+// (K_d^-1 B)[(c,i),c'] = delta_cc' sum_j Kinv_c[i,j] fa_j, demoted to the split-complex64 right-hand side block.
+__global__ void __launch_bounds__(256) rhs_s_kernel(int nch, int nb, const double2 *__restrict__ Kinv,
+                                                    const double *__restrict__ fa, float *__restrict__ Bre,
+                                                    float *__restrict__ Bim, long ld) {
+    const long N = (long)nch * nb;
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= N * nch) return;
+    const int q = (int)(idx / N);
+    const int row = (int)(idx - (long)q * N);
+    const int c = row / nb, i = row - c * nb;
+    float re = 0.f, im = 0.f;
+    if (c == q) {
+        double sr = 0.0, si = 0.0;
+        const double2 *k = Kinv + (size_t)c * nb * nb + i;
+        for (int j = 0; j < nb; ++j) {
+            const double2 v = k[(size_t)j * nb];
+            sr = fma(v.x, fa[j], sr);
+            si = fma(v.y, fa[j], si);
+        }
+        re = (float)sr;
+        im = (float)si;
+    }
+    Bre[(size_t)q * ld + row] = re;
+    Bim[(size_t)q * ld + row] = im;
+}
+
+int precond_rhs(cudaStream_t st, const StructTables &t, const double2 *Kinv, CView B) {
+    const long tot = (long)t.nch * t.nb * t.nch;
+    rhs_s_kernel<<<ceil_div(tot, 256), 256, 0, st>>>(t.nch, t.nb, Kinv, t.fa, B.re, B.im, B.ld);
+    HP_LAUNCHED();
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------------- precision moves
+// complex128 (interleaved) -> split complex64
+__global__ void __launch_bounds__(256) demote_kernel(long rows, int cols, const double2 *__restrict__ Z, long ldz,
+                                                     float *__restrict__ re, float *__restrict__ im, long ld) {
+    const long tot = rows * cols;
+    for (long idx = (long)blockIdx.x * blockDim.x + threadIdx.x; idx < tot; idx += (long)gridDim.x * blockDim.x) {
+        const long q = idx / rows, r = idx - q * rows;
+        const double2 z = Z[q * ldz + r];
+        re[q * ld + r] = (float)z.x;
+        im[q * ld + r] = (float)z.y;
+    }
+}
+
+int demote(cudaStream_t st, long rows, int cols, const double2 *Z, long ldz, CView D) {
+    const long tot = rows * cols;
+    if (tot <= 0) return 0;
+    const int grid = (int)std::min<long>(ceil_div(tot, 256), 148L * 8);
+    demote_kernel<<<grid, 256, 0, st>>>(rows, cols, Z, ldz, D.re, D.im, D.ld);
+    HP_LAUNCHED();
+    return 0;
+}
+
+// X <- (accumulate ? X : 0) + D with D split complex64 (PAPER.md:220 c2z, :225 add_correction, fused);
+// norms[0] = max|D|, norms[1] = max|X_new| (moduli; pre-zeroed here)
+__global__ void __launch_bounds__(256) promote_add_kernel(long rows, int cols, double2 *__restrict__ X, long ldx,
+                                                          const float *__restrict__ re, const float *__restrict__ im, long ld,
+                                                          int accumulate, double *norms) {
+    __shared__ double shred[32];
+    double md = 0.0, mx = 0.0;
+    const long tot = rows * cols;
+    for (long idx = (long)blockIdx.x * blockDim.x + threadIdx.x; idx < tot; idx += (long)gridDim.x * blockDim.x) {
+        const long q = idx / rows, r = idx - q * rows;
+        const double dr = (double)re[q * ld + r], di = (double)im[q * ld + r];
+        double2 x = accumulate ? X[q * ldx + r] : make_double2(0.0, 0.0);
+        x.x += dr;
+        x.y += di;
+        X[q * ldx + r] = x;
+        md = fmax(md, sqrt(dr * dr + di * di));
+        mx = fmax(mx, sqrt(x.x * x.x + x.y * x.y));
+    }
+    // block maxima (same reduction shape as structured.cu's)
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        md = fmax(md, __shfl_xor_sync(0xffffffffu, md, off));
+        mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, off));
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { shred[warp] = md; shred[8 + warp] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) { md = fmax(md, shred[w]); mx = fmax(mx, shred[8 + w]); }
+        atomicMax(reinterpret_cast<unsigned long long *>(norms), (unsigned long long)__double_as_longlong(md));
+        atomicMax(reinterpret_cast<unsigned long long *>(norms + 1), (unsigned long long)__double_as_longlong(mx));
+    }
+}
+
+int promote_add(cudaStream_t st, long rows, int cols, double2 *X, long ldx, CView D, bool accumulate, double *norms_dev) {
+    HP_CUDA(cudaMemsetAsync(norms_dev, 0, 2 * sizeof(double), st));
+    const long tot = rows * cols;
+    if (tot <= 0) return 0;
+    const int grid = (int)std::min<long>(ceil_div(tot, 256), 148L * 8);
+    promote_add_kernel<<<grid, 256, 0, st>>>(rows, cols, X, ldx, D.re, D.im, D.ld, accumulate ? 1 : 0, norms_dev);
+    HP_LAUNCHED();
+    return 0;
+}
+
+}  // namespace hp

@@ -1,0 +1,19 @@
+// precond.cuh -- FP64 block-diagonal preconditioner and precision moves of the mixed path (precond.cu).
+#pragma once
+#include "structured.cuh"
+
+namespace hp {
+
+// Kinv[c] <- K_c^-1, K_c = diagonal block c of C - E*I (nb x nb complex128, column-major, blocks contiguous).
+// info_dev (pre-zeroed by the caller) receives c*nb + k + 1 if block c has no non-zero pivot at step k.
+int precond_invert(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double2 *Kinv, int *info_dev);
+// S <- K_d^-1 (C - E*I) in split complex64 (identity diagonal blocks, Kinv_c * diag V_cc' elsewhere)
+int precond_assemble(cudaStream_t st, const StructTables &t, const double2 *Kinv, const double2 *V, CView S);
+// B <- K_d^-1 * (surface right-hand sides), split complex64, N x nch
+int precond_rhs(cudaStream_t st, const StructTables &t, const double2 *Kinv, CView B);
+// D <- (complex64) Z
+int demote(cudaStream_t st, long rows, int cols, const double2 *Z, long ldz, CView D);
+// X <- (accumulate ? X : 0) + D;  norms_dev[0] = max|D|, norms_dev[1] = max|X|
+int promote_add(cudaStream_t st, long rows, int cols, double2 *X, long ldx, CView D, bool accumulate, double *norms_dev);
+
+}  // namespace hp

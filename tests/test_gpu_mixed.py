@@ -1,0 +1,165 @@
+"""Parity of the mixed-precision CUDA path (tcgen05 TF32 complex GEMM, complex64 LU, FP64 refinement) with the CPU
+oracle / the plain definitions.  All tests need a B200 ("-m gpu").
+
+Tolerances:
+  hprmat_cgemm_tf32: the tensor core rounds every operand to TF32 (unit roundoff 2^-11, or 2^-10 if it truncates) and
+  accumulates in FP32, so elementwise  |C - C_def| <= (2^-9 + (k + 4) 2^-23) * (|alpha| (|A| |B|)_ij + |beta| |C0|_ij)
+  with |A| = |Re A| + |Im A| -- a rigorous first-order bound, written in the test.
+  mixed R-matrix: north_star -- <= 1e-10 with refinement, <= 1e-3 without.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2512_11590_b200 import binding as hb
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def _planes(a: np.ndarray, ld: int):
+    """complex (m, n) -> two torch float32 CUDA planes holding the column-major matrix with leading dimension ld."""
+    m, n = a.shape
+    out = []
+    for part in (a.real, a.imag):
+        buf = np.zeros((n, ld), dtype=np.float32)
+        buf[:, :m] = part.T
+        out.append(torch.from_numpy(buf).to(DEV))
+    return out
+
+
+def _unplanes(re: torch.Tensor, im: torch.Tensor, m: int):
+    return (re.cpu().numpy()[:, :m].T.astype(np.float64) + 1j * im.cpu().numpy()[:, :m].T.astype(np.float64))
+
+
+def _rup(x, q):
+    return (x + q - 1) // q * q
+
+
+@pytest.mark.parametrize("m,n,k,alpha,beta", [
+    (128, 128, 32, 1.0, 0.0), (128, 128, 64, -1.0, 1.0), (256, 384, 96, -1.0, 1.0), (100, 50, 37, 1.0, 0.0),
+    (257, 129, 65, -1.0, 1.0), (32, 700, 32, 1.0, 0.0), (1000, 333, 200, -1.0, 1.0), (5, 3, 1, 2.0, -0.5),
+    (640, 512, 1024, -1.0, 1.0), (1, 1, 8, 1.0, 1.0)])
+def test_cgemm_tf32_matches_definition(m, n, k, alpha, beta):
+    rng = np.random.default_rng(m * 1000003 + n * 1009 + k)
+    A = (rng.uniform(-1, 1, (m, k)) + 1j * rng.uniform(-1, 1, (m, k))).astype(np.complex64).astype(np.complex128)
+    B = (rng.uniform(-1, 1, (k, n)) + 1j * rng.uniform(-1, 1, (k, n))).astype(np.complex64).astype(np.complex128)
+    C0 = (rng.uniform(-1, 1, (m, n)) + 1j * rng.uniform(-1, 1, (m, n))).astype(np.complex64).astype(np.complex128)
+    lda, ldb, ldc = _rup(m, 4), _rup(k, 4), _rup(m, 4) + 4
+    Ar, Ai = _planes(A, lda)
+    Br, Bi = _planes(B, ldb)
+    Cr, Ci = _planes(C0, ldc)
+    hb.hprmat_cgemm_tf32(m, n, k, alpha, Ar, Ai, lda, Br, Bi, ldb, beta, Cr, Ci, ldc)
+    torch.cuda.synchronize()
+    got = _unplanes(Cr, Ci, m)
+    ref = beta * C0 + alpha * (A @ B)                                         # the definition, in double
+    absA = np.abs(A.real) + np.abs(A.imag)
+    absB = np.abs(B.real) + np.abs(B.imag)
+    bound = (2.0 ** -9 + (k + 4) * 2.0 ** -23) * (abs(alpha) * (absA @ absB) + abs(beta) * (np.abs(C0.real) + np.abs(C0.imag)))
+    err = np.abs(got - ref)
+    assert np.all(err <= bound + 1e-30), (err.max(), bound.max(), np.unravel_index(np.argmax(err - bound), err.shape))
+    # padding rows of C (ldc > m) are not touched
+    assert float(Cr[:, m:].abs().max()) == 0.0 and float(Ci[:, m:].abs().max()) == 0.0
+
+
+def test_cgemm_tf32_is_exact_on_tf32_representable_integers():
+    """Small integers are exact in TF32 and their dot products exact in FP32: the result must equal the definition
+    bit for bit -- pins the operand layouts / descriptors (a transposed or mis-swizzled tile cannot pass)."""
+    m, n, k = 384, 256, 160
+    rng = np.random.default_rng(5)
+    A = rng.integers(-8, 9, (m, k)) + 1j * rng.integers(-8, 9, (m, k))
+    B = rng.integers(-8, 9, (k, n)) + 1j * rng.integers(-8, 9, (k, n))
+    C0 = rng.integers(-100, 101, (m, n)) + 1j * rng.integers(-100, 101, (m, n))
+    Ar, Ai = _planes(A, m)
+    Br, Bi = _planes(B, k)
+    Cr, Ci = _planes(C0, m)
+    hb.hprmat_cgemm_tf32(m, n, k, -1.0, Ar, Ai, m, Br, Bi, k, 1.0, Cr, Ci, m)
+    torch.cuda.synchronize()
+    assert np.array_equal(_unplanes(Cr, Ci, m), C0 - A @ B)
+
+
+# ---------------------------------------------------------------------------------------------------- whole path, mixed
+import oracle  # noqa: E402
+from paper_2512_11590_b200.workloads import make_workload  # noqa: E402
+
+
+def _host(t: torch.Tensor) -> np.ndarray:
+    return t.cpu().numpy().T
+
+
+def _relmax(a, b):
+    return np.abs(a - b).max() / np.abs(b).max()
+
+
+def _oracle_R(w, E, mode=0):
+    r = oracle.mesh(w.nb, w.a)[2]
+    return oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, w.potential(r), mode=mode, nrefine=2, return_x=True)
+
+
+MIXED_CASES = [(0, None, None), (0, 1, 50), (1, 8, 100), (1, 5, 37), (2, 16, 100), (3, 12, 64), (1, 3, 130)]
+
+
+@pytest.mark.parametrize("cfg,nch,nb", MIXED_CASES)
+def test_rmatrix_mixed_refine_parity(cfg, nch, nb):
+    """north_star: mixed path with refinement <= 1e-10 in R against the oracle."""
+    w = make_workload(cfg, nch=nch, nb=nb)
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << hb.HPRMAT_MIXED_REFINE)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    for E in w.energies[:2]:
+        R, info = ctx.solve(float(E), V, hb.HPRMAT_MIXED_REFINE)
+        Ro, Xo = _oracle_R(w, float(E))
+        Rg = _host(R)
+        assert info["status"] == 0, info
+        assert 1 <= info["refine_steps"] <= 5
+        assert _relmax(Rg, Ro) <= 1e-10, (info, _relmax(Rg, Ro))
+        assert _relmax(_host(ctx.get_x()), Xo) <= 1e-10
+        assert 0 <= info["backward_err"] <= 50 * w.n * 2.0 ** -53
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("cfg,nch,nb", MIXED_CASES)
+def test_rmatrix_mixed_norefine_parity(cfg, nch, nb):
+    """north_star: mixed path without refinement <= 1e-3 in R-matrix elements (the paper's cross-section level)."""
+    w = make_workload(cfg, nch=nch, nb=nb)
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << hb.HPRMAT_MIXED)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    E = float(w.energies[0])
+    R, info = ctx.solve(E, V, hb.HPRMAT_MIXED)
+    Ro, _ = _oracle_R(w, E)
+    assert info["status"] == 0 and info["refine_steps"] == 0
+    err = _relmax(_host(R), Ro)
+    assert err <= 1e-3, (err, info)
+    print(f"mixed no-refine {w.name}: R error {err:.2e}")
+    ctx.destroy()
+
+
+def test_mixed_strong_coupling_needs_and_gets_more_refinement():
+    """Couplings 100x stronger than the configs': the TF32 factors are poorer, refinement still reaches 1e-10 or the
+    call reports HPRMAT_ENOTCONVERGED -- never a silent low-precision result."""
+    w = make_workload(1, nch=6, nb=60)
+    w.beta *= 100.0
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << hb.HPRMAT_MIXED_REFINE)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    R, info = ctx.solve(20.0, V, hb.HPRMAT_MIXED_REFINE, max_refine=12, allow=(hb.HPRMAT_OK, hb.HPRMAT_ENOTCONVERGED))
+    Ro, _ = _oracle_R(w, 20.0)
+    if info["status"] == hb.HPRMAT_OK:
+        assert _relmax(_host(R), Ro) <= 1e-10, info
+    else:
+        assert info["status"] == hb.HPRMAT_ENOTCONVERGED
+    ctx.destroy()
+
+
+def test_mixed_matches_fp64_mode_on_the_same_context():
+    w = make_workload(2, nch=10, nb=100)
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=0)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    R1, _ = ctx.solve(16.25, V, hb.HPRMAT_FP64)
+    R1 = R1.clone()
+    R2, info = ctx.solve(16.25, V, hb.HPRMAT_MIXED_REFINE)
+    assert info["status"] == 0
+    assert _relmax(R2.cpu().numpy(), R1.cpu().numpy()) <= 1e-10
+    ctx.destroy()
