@@ -12,8 +12,10 @@
 // accumulating UMMAs on the four planes as they lie in memory -- that is why the mixed path stores split complex.
 //
 // Operand layouts in shared memory (what the column-major planes give without any transposition):
-//   A tile (BM x KC): M is the contiguous dimension  -> "MN-major" canonical layout, swizzle atoms of 32 (M) x 8 (K)
-//                     floats; loaded as BM/32 TMA boxes of 32 (M) x KC (K);  LBO = KC*128 B between 32-row chunks.
+//   A tile (BM x KC): M is the contiguous dimension  -> "MN-major" canonical layout.  For 32-bit operands the only
+//                     MN-major layout the UMMA accepts is SWIZZLE_128B with a 32-byte swizzle base (layout type 1; TMA's
+//                     CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B): atoms of 32 (M) x 4 (K) floats.  Loaded as BM/32 TMA boxes of
+//                     32 (M) x KC (K);  LBO = KC*128 B between 32-row chunks, SBO = 512 B between 4-row K groups.
 //   B tile (KC x BN): K is the contiguous dimension  -> "K-major" canonical layout, rows of KC = 32 floats (128 B),
 //                     swizzle atoms of 8 rows; one TMA box of 32 (K) x BN (N);  SBO = 1024 B between 8-column groups.
 // TMA zero-fills out-of-bounds elements, which takes care of ragged M, N and K edges.
@@ -112,9 +114,10 @@ __global__ void __launch_bounds__(CG_NT, 1)
                 const uint32_t b_re = a_re + 2 * Cfg::A_PLANE, b_im = b_re + Cfg::B_PLANE;
 #pragma unroll
                 for (int ks = 0; ks < CG_KC / 8; ++ks) {
-                    // A: one K-group of 8 rows = 1024 B per k-step; 32-row M chunks CG_KC*128 B apart
-                    const uint64_t dar = smem_desc_sw128(a_re + ks * 1024, CG_KC * 128, 1024);
-                    const uint64_t dai = smem_desc_sw128(a_im + ks * 1024, CG_KC * 128, 1024);
+                    // A: 8 k-rows of 128 B = 1024 B per k-step, as two 4-row (512 B) swizzle atoms; 32-row M chunks
+                    // CG_KC*128 B apart
+                    const uint64_t dar = smem_desc_sw128_base32(a_re + ks * 1024, CG_KC * 128, 512);
+                    const uint64_t dai = smem_desc_sw128_base32(a_im + ks * 1024, CG_KC * 128, 512);
                     // B: 8 floats of K = 32 B per k-step inside the 128-byte row; 8-column groups 1024 B apart
                     const uint64_t dbr = smem_desc_sw128(b_re + ks * 32, 16, 1024);
                     const uint64_t dbi = smem_desc_sw128(b_im + ks * 32, 16, 1024);
@@ -197,7 +200,8 @@ EncodeTiledFn encode_fn() {
 }
 
 // plane: rows x cols floats, column-major with leading dimension ld; box = box_rows x box_cols
-int make_map(CUtensorMap *map, const float *plane, long rows, long cols, long ld, int box_rows, int box_cols) {
+int make_map(CUtensorMap *map, const float *plane, long rows, long cols, long ld, int box_rows, int box_cols,
+             CUtensorMapSwizzle swz) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) {
         snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled entry point not found");
@@ -208,7 +212,7 @@ int make_map(CUtensorMap *map, const float *plane, long rows, long cols, long ld
     cuuint32_t box[2] = {(cuuint32_t)box_rows, (cuuint32_t)box_cols};
     cuuint32_t estr[2] = {1, 1};
     CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)plane, dims, strides, box, estr,
-                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed (%d): rows=%ld cols=%ld ld=%ld ptr=%p", (int)r,
@@ -229,10 +233,10 @@ int launch_cgemm(cudaStream_t st, int m, int n, int k, float alpha, CView A, CVi
     }
     CgMaps maps;
     const int kk = k > 0 ? k : 1;
-    HP_TRY(make_map(&maps.a_re, A.re, m, kk, A.ld, 32, CG_KC));
-    HP_TRY(make_map(&maps.a_im, A.im, m, kk, A.ld, 32, CG_KC));
-    HP_TRY(make_map(&maps.b_re, B.re, kk, n, B.ld, CG_KC, BN));
-    HP_TRY(make_map(&maps.b_im, B.im, kk, n, B.ld, CG_KC, BN));
+    HP_TRY(make_map(&maps.a_re, A.re, m, kk, A.ld, 32, CG_KC, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B));
+    HP_TRY(make_map(&maps.a_im, A.im, m, kk, A.ld, 32, CG_KC, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B));
+    HP_TRY(make_map(&maps.b_re, B.re, kk, n, B.ld, CG_KC, BN, CU_TENSOR_MAP_SWIZZLE_128B));
+    HP_TRY(make_map(&maps.b_im, B.im, kk, n, B.ld, CG_KC, BN, CU_TENSOR_MAP_SWIZZLE_128B));
     dim3 grid(ceil_div(m, CG_BM), ceil_div(n, BN));
     kern<<<grid, CG_NT, Cfg::SMEM, st>>>(maps, m, n, k, alpha, beta, C.re, C.im, C.ld);
     HP_LAUNCHED();

@@ -103,6 +103,17 @@ __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t addr, uint32_t lbo,
     d |= (uint64_t)2 << 61;                          // layout type: SWIZZLE_128B
     return d;
 }
+// Same, layout type SWIZZLE_128B_BASE32B (32-byte swizzle chunks inside the 128-byte span, atoms of 4 rows): the only
+// MN-major layout for 32-bit (tf32) operands.
+__device__ __forceinline__ uint64_t smem_desc_sw128_base32(uint32_t addr, uint32_t lbo, uint32_t sbo) {
+    uint64_t d = 0;
+    d |= (uint64_t)((addr & 0x3FFFF) >> 4);
+    d |= (uint64_t)((lbo >> 4) & 0x3FFF) << 16;
+    d |= (uint64_t)((sbo >> 4) & 0x3FFF) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)1 << 61;                          // layout type: SWIZZLE_128B_BASE32B
+    return d;
+}
 // Instruction descriptor for kind::tf32 with FP32 accumulation; A is MN-major (a_mn = 1) or K-major, likewise B.
 __host__ __device__ constexpr uint32_t idesc_tf32(int M, int N, int a_mn, int b_mn, int neg_a, int neg_b) {
     return (1u << 4) /* D = F32 */ | (2u << 7) /* A = TF32 */ | (2u << 10) /* B = TF32 */ | ((uint32_t)neg_a << 13) |
