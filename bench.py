@@ -260,7 +260,9 @@ def main():
         hb.hprmat_profile(True)
         _, pinfo = ctx.solve(E, V, mode, R=R)
         hb.hprmat_profile(False)
-        g_ms, g_fl, g_n = hb.hprmat_profile_read()
+        hb.hprmat_profile_read()
+        cats = {name: dict(zip(("ms", "flops", "launches"), hb.hprmat_profile_cat(i))) for i, name in enumerate(hb.PROF_CATS)}
+        g_ms, g_fl, g_n = cats["lu_gemm"]["ms"], cats["lu_gemm"]["flops"], cats["lu_gemm"]["launches"]
         pk, how = peaks()
         if mode == hb.HPRMAT_FP64:
             peak, pname = FP64_TENSOR_PEAK_TFLOPS, "FP64 DMMA peak measured on this pool with a register-resident mma.sync loop"
@@ -268,11 +270,13 @@ def main():
             peak = 0.5 * pk["bf16_tflops_sustained"]
             pname = f"TF32 dense = 0.5 x bf16 sustained ({how})"
         ach = g_fl / (g_ms * 1e-3) * 1e-12 if g_ms > 0 else 0.0
-        roof = {"bound": "tensor", "kernel": "zgemm_kernel (trailing update + TRSM GEMMs)" if mode == hb.HPRMAT_FP64 else
-                "cgemm trailing update", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                "traffic": None, "peak_source": pname, "launches": g_n, "kernel_ms_per_step": g_ms,
+        roof = {"bound": "tensor", "kernel": ("zgemm_kernel" if mode == hb.HPRMAT_FP64 else "cgemm_tf32_kernel") +
+                " (trailing update A22 -= L21 U12 of the LU)", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                "frac": ach / peak, "traffic": None, "peak_source": pname, "launches": g_n, "kernel_ms_per_step": g_ms,
                 "share_of_step": g_ms / pinfo["ms_total"] if pinfo["ms_total"] else None,
-                "algorithmic_flops_per_step": g_fl}
+                "algorithmic_flops_per_step": g_fl,
+                "breakdown_ms": {k: round(v["ms"], 3) for k, v in cats.items()},
+                "breakdown_launches": {k: v["launches"] for k, v in cats.items()}}
 
     if rank == 0:
         info = infos[-1]

@@ -145,6 +145,10 @@ const char *hprmat_last_cuda_error(void);
  * resets the record. */
 int hprmat_profile(int enable);
 int hprmat_profile_read(double *ms, double *flops, long long *launches);
+/* Per-category totals of the record consumed by the last hprmat_profile_read: cat 0 = trailing-update GEMMs of the LU,
+ * 1 = GEMMs of the U12 triangular solves inside the LU, 2 = panel factorisations, 3 = row interchanges, 4 = GEMMs of the
+ * right-hand-side triangular solves, 5 = other.  ms/flops/launches host, may be NULL. */
+int hprmat_profile_cat(int cat, double *ms, double *flops, long long *launches);
 /* Measurement aid: FP64 tensor-core (DMMA, mma.sync.m8n8k4.f64) issue-rate ceiling of the device, measured with a
  * register-resident loop (no memory traffic) on 148*ctas_per_sm CTAs of 8 warps, `iters` x 8 MMAs per warp.
  * tflops (host, out): real TFLOP/s; ms (host, out, may be NULL): device time of the timed launch.  Synchronises. */

@@ -86,6 +86,15 @@ def hprmat_profile_read():
     return ms.value, fl.value, n.value
 
 
+PROF_CATS = ("lu_gemm", "lu_trsm", "panel", "laswp", "solve", "other")
+
+
+def hprmat_profile_cat(cat: int):
+    ms, fl, n = C.c_double(0), C.c_double(0), C.c_longlong(0)
+    _check(lib().hprmat_profile_cat(C.c_int(cat), C.byref(ms), C.byref(fl), C.byref(n)), "hprmat_profile_cat")
+    return ms.value, fl.value, n.value
+
+
 def hprmat_probe_dmma(iters=20000, ctas_per_sm=2, stream=None):
     tf, ms = C.c_double(0), C.c_double(0)
     _check(lib().hprmat_probe_dmma(_stream(stream), C.c_int(iters), C.c_int(ctas_per_sm), C.byref(tf), C.byref(ms)),

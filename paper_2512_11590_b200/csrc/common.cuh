@@ -35,6 +35,14 @@ inline int cuda_fail(cudaError_t e, const char *file, int line) {
 
 constexpr int kNumSMs = 148;  // B200
 
+// launch categories of the per-launch timing (hprmat_profile_cat)
+enum { PROF_LU_GEMM = 0, PROF_LU_TRSM = 1, PROF_PANEL = 2, PROF_LASWP = 3, PROF_SOLVE = 4, PROF_OTHER = 5, PROF_NCAT = 6 };
+extern int g_prof_cat;
+struct ProfCat {  // RAII: category of the launches issued in this scope
+    int prev;
+    explicit ProfCat(int c) : prev(g_prof_cat) { g_prof_cat = c; }
+    ~ProfCat() { g_prof_cat = prev; }
+};
 bool prof_enabled();
 void prof_begin(cudaStream_t st, double flops);
 void prof_end(cudaStream_t st);

@@ -43,8 +43,11 @@ template <class V> size_t LuWork<V>::carve(void *base, int n_) {
         p += round_up((long)bytes, 256);
         return q;
     };
-    dinvL = alloc_view<V>(p, IB, (long)nblk * IB);
-    dinvU = alloc_view<V>(p, IB, (long)nblk * IB);
+    for (int lev = 0; lev < NLEV; ++lev) {
+        const long sz = (long)IB << lev;
+        dinvL[lev] = alloc_view<V>(p, sz, (long)ceil_div(n, sz) * sz);
+        dinvU[lev] = alloc_view<V>(p, sz, (long)ceil_div(n, sz) * sz);
+    }
     perm = (int *)take(sizeof(int) * (size_t)nblk * PERM_STRIDE);
     cand_val = (T *)take(sizeof(T) * 2 * MAXG);
     cand_row = (int *)take(sizeof(int) * 2 * MAXG);
@@ -331,13 +334,148 @@ __global__ void __launch_bounds__(SWP_NT) laswp_kernel(V A, int lo1, int hi1, in
 template <class V> static int laswp(cudaStream_t st, V A, int lo1, int hi1, int lo2, int hi2, const int *perm, int b0, int b1) {
     int ntot = (hi1 - lo1) + (hi2 - lo2);
     if (ntot <= 0 || b1 <= b0) return 0;
+    ProfCat pc(PROF_LASWP);
+    const bool prof = prof_enabled();
+    if (prof) prof_begin(st, 0.0);
     laswp_kernel<V><<<ceil_div(ntot, SWP_CW), SWP_NT, 0, st>>>(A, lo1, hi1, lo2, hi2, perm, b0, b1);
+    if (prof) prof_end(st);
     HP_LAUNCHED();
     return 0;
 }
 
+// ------------------------------------------------------------------------------------------------- inverse doubling
+// Inverse of the w x w diagonal block at (c0,c0) from the inverses of its two diagonal sub-blocks a = [0,h), b = [h,w):
+//     inv(L) = [ inv(La)                 0      ]      inv(U) = [ inv(Ua)   -inv(Ua) Uab inv(Ub) ]
+//              [ -inv(Lb) Lba inv(La)   inv(Lb) ]               [   0              inv(Ub)       ]
+// blockIdx.y = 0: L, 1: U.  Each CTA produces INV_RS rows of the w x w result; the off-diagonal part is
+// out[I,:] = -(XL[I,:] * M) * XR with XL p x p, M p x q (the factor block), XR q x q.
+constexpr int INV_RS = 16, INV_NT = 256;
+
+template <class V>
+__global__ void __launch_bounds__(INV_NT) inv_double_kernel(V A, int h, int w, V La, V Lb, V Lout, V Ua, V Ub, V Uout) {
+    typedef typename V::elem_t E;
+    typedef typename V::real_t T;
+    extern __shared__ __align__(16) unsigned char smraw[];
+    const bool isU = blockIdx.y == 1;
+    const int i0 = blockIdx.x * INV_RS;            // first row of this strip inside the w x w block
+    const int nr = min(INV_RS, w - i0);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const V Xa = isU ? Ua : La, Xb = isU ? Ub : Lb, O = isU ? Uout : Lout;
+    const int hb = w - h;
+    const bool top = i0 < h;
+    // rows that are plain copies / zeros
+    if (top != isU) {
+        // L top rows: [inv(La) | 0];  U bottom rows: [0 | inv(Ub)]
+        for (int idx = tid; idx < nr * w; idx += INV_NT) {
+            const int r = idx % nr, c = idx / nr;
+            E v = mk((T)0, (T)0);
+            if (!isU) { if (c < h) v = Xa.get(i0 + r, c); }
+            else      { if (c >= h) v = Xb.get(i0 + r - h, c - h); }
+            O.set(i0 + r, c, v);
+        }
+        return;
+    }
+    // L bottom rows: [-(inv(Lb)[I,:] Lba) inv(La) | inv(Lb)[I,:]];  U top rows: [inv(Ua)[I,:] | -(inv(Ua)[I,:] Uab) inv(Ub)]
+    const int p = isU ? h : hb, q = isU ? hb : h;
+    const V XL = isU ? Xa : Xb, XR = isU ? Xb : Xa;
+    const V M = isU ? A.sub(0, h) : A.sub(h, 0);   // p x q factor block
+    const int li0 = isU ? i0 : i0 - h;             // row offset inside XL
+    const int ocol = isU ? h : 0;                  // column offset of the product inside the output
+    E *xs = reinterpret_cast<E *>(smraw);          // [p][INV_RS]: XL[I, k] at xs[k*INV_RS + r]
+    E *ts = xs + (size_t)(LEAF / 2) * INV_RS;      // [q][INV_RS]: T[r, j] at ts[j*INV_RS + r]
+    for (int idx = tid; idx < INV_RS * p; idx += INV_NT) {
+        const int r = idx % INV_RS, k = idx / INV_RS;
+        xs[idx] = r < nr ? XL.get(li0 + r, k) : mk((T)0, (T)0);
+    }
+    // the diagonal-block copy of this strip
+    for (int idx = tid; idx < nr * p; idx += INV_NT) {
+        const int r = idx % nr, c = idx / nr;
+        O.set(i0 + r, (isU ? 0 : h) + c, XL.get(li0 + r, c));
+    }
+    __syncthreads();
+    // phase 1: T = XL[I,:] * M   (warp per column j of M, lanes over k)
+    for (int j = warp; j < q; j += INV_NT / 32) {
+        E acc[INV_RS];
+#pragma unroll
+        for (int r = 0; r < INV_RS; ++r) acc[r] = mk((T)0, (T)0);
+        for (int k = lane; k < p; k += 32) {
+            const E m = M.get(k, j);
+#pragma unroll
+            for (int r = 0; r < INV_RS; ++r) acc[r] = cfnma(acc[r], mk(-xs[k * INV_RS + r].x, -xs[k * INV_RS + r].y), m);
+        }
+#pragma unroll
+        for (int r = 0; r < INV_RS; ++r) {
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+                acc[r].x += __shfl_xor_sync(0xffffffffu, acc[r].x, off);
+                acc[r].y += __shfl_xor_sync(0xffffffffu, acc[r].y, off);
+            }
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int r = 0; r < INV_RS; ++r) ts[j * INV_RS + r] = acc[r];
+        }
+    }
+    __syncthreads();
+    // phase 2: out = -T * XR   (warp per column c of XR, lanes over j)
+    for (int c = warp; c < q; c += INV_NT / 32) {
+        E acc[INV_RS];
+#pragma unroll
+        for (int r = 0; r < INV_RS; ++r) acc[r] = mk((T)0, (T)0);
+        for (int j = lane; j < q; j += 32) {
+            const E x = XR.get(j, c);
+#pragma unroll
+            for (int r = 0; r < INV_RS; ++r) acc[r] = cfnma(acc[r], ts[j * INV_RS + r], x);
+        }
+#pragma unroll
+        for (int r = 0; r < INV_RS; ++r) {
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+                acc[r].x += __shfl_xor_sync(0xffffffffu, acc[r].x, off);
+                acc[r].y += __shfl_xor_sync(0xffffffffu, acc[r].y, off);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < INV_RS; ++r)
+            if (lane == r && r < nr) O.set(i0 + r, ocol + c, acc[r]);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------- host recursion
-static inline int split(int w) { return (int)round_up((w + 1) / 2, IB); }
+// Column split of a node of width w: below LEAF the tree is binary on power-of-two multiples of IB, so that every left
+// child is a full block of its size class (its inverse is kept, see LuWork); above, splits fall on multiples of LEAF.
+static inline int split(int w) {
+    if (w > LEAF) return (int)round_up((w + 1) / 2, LEAF);
+    int h = IB;
+    while (2 * h < w) h *= 2;
+    return h;
+}
+static inline int level_of(int w) {
+    int lev = 0;
+    while ((IB << lev) < w) ++lev;
+    return lev;
+}
+// inverse of the (unit-lower | upper) triangle of the diagonal block of size s (<= LEAF) at offset d0 (a multiple of its
+// size class)
+template <class V> static V dinv_of(const V *tab, int d0, int s) {
+    const int lev = level_of(s);
+    const long sz = (long)IB << lev;
+    return tab[lev].sub(0, (long)(d0 / sz) * sz);
+}
+
+template <class V> static int inv_double(cudaStream_t st, V A, int c0, int h, int w, LuWork<V> &wk) {
+    typedef typename V::elem_t E;
+    V La = dinv_of(wk.dinvL, c0, h), Lb = dinv_of(wk.dinvL, c0 + h, w - h), Lo = dinv_of(wk.dinvL, c0, w);
+    V Ua = dinv_of(wk.dinvU, c0, h), Ub = dinv_of(wk.dinvU, c0 + h, w - h), Uo = dinv_of(wk.dinvU, c0, w);
+    const size_t smem = 2 * (size_t)(LEAF / 2) * INV_RS * sizeof(E);  // p, q <= LEAF/2
+    ProfCat pc(PROF_OTHER);
+    const bool prof = prof_enabled();
+    if (prof) prof_begin(st, 0.0);
+    inv_double_kernel<V><<<dim3(ceil_div(w, INV_RS), 2), INV_NT, smem, st>>>(A.sub(c0, c0), h, w, La, Lb, Lo, Ua, Ub, Uo);
+    if (prof) prof_end(st);
+    HP_LAUNCHED();
+    return 0;
+}
 
 template <class V> static int panel(cudaStream_t st, int n, V A, int c0, int w, int *ipiv, int *info_dev, LuWork<V> &wk) {
     typedef typename V::elem_t E;
@@ -354,23 +492,30 @@ template <class V> static int panel(cudaStream_t st, int n, V A, int c0, int w, 
     }
     V Asub = A.sub(c0, c0);
     const int blk = c0 / IB;
-    V dl = wk.dinvL.sub(0, (long)blk * IB), du = wk.dinvU.sub(0, (long)blk * IB);
+    V dl = wk.dinvL[0].sub(0, (long)blk * IB), du = wk.dinvU[0].sub(0, (long)blk * IB);
     int *perm = wk.perm + (size_t)blk * PERM_STRIDE;
     int m_ = m, w_ = w, c0_ = c0, rpc_ = rpc;
     unsigned base = wk.bar_base;
     void *args[] = {&Asub, &m_, &w_, &c0_, &rpc_, &ipiv, &info_dev, &wk.cand_val, &wk.cand_row, &wk.cand_data,
                     &wk.jrow, &wk.counter, &base, &dl, &du, &perm};
-    HP_CUDA(cudaLaunchCooperativeKernel((void *)kern, dim3(G), dim3(PANEL_NT), args, smem, st));
+    {
+        ProfCat pc(PROF_PANEL);
+        const bool prof = prof_enabled();
+        if (prof) prof_begin(st, 0.0);
+        HP_CUDA(cudaLaunchCooperativeKernel((void *)kern, dim3(G), dim3(PANEL_NT), args, smem, st));
+        if (prof) prof_end(st);
+    }
     HP_LAUNCHED();
     wk.bar_base += (unsigned)G * (unsigned)w;
     // this batch's interchanges on every other column of the matrix
     return laswp(st, A, 0, c0, c0 + w, n, wk.perm, blk, blk + 1);
 }
 
-// B <- L^-1 B, L = unit lower triangle of the s x s diagonal block of A at (d0,d0); B is s x ncols
+// B <- L^-1 B, L = unit lower triangle of the s x s diagonal block of A at (d0,d0); B is s x ncols.  d0 is a multiple of
+// LEAF, or s <= LEAF is a full block of its size class (or the ragged last block).
 template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk) {
     if (s <= 0 || ncols <= 0) return 0;
-    if (s <= IB) return gemm(st, s, ncols, s, 1.0, wk.dinvL.sub(0, (long)(d0 / IB) * IB), B, 0.0, B);
+    if (s <= LEAF) return gemm(st, s, ncols, s, 1.0, dinv_of(wk.dinvL, d0, s), B, 0.0, B);
     const int h = split(s);
     HP_TRY(trsm_lower(st, A, d0, h, B, ncols, wk));
     HP_TRY(gemm(st, s - h, ncols, h, -1.0, A.sub(d0 + h, d0), B, 1.0, B.sub(h, 0)));
@@ -380,7 +525,7 @@ template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V 
 // B <- U^-1 B, U = upper triangle (with diagonal) of the s x s diagonal block of A at (d0,d0)
 template <class V> static int trsm_upper(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk) {
     if (s <= 0 || ncols <= 0) return 0;
-    if (s <= IB) return gemm(st, s, ncols, s, 1.0, wk.dinvU.sub(0, (long)(d0 / IB) * IB), B, 0.0, B);
+    if (s <= LEAF) return gemm(st, s, ncols, s, 1.0, dinv_of(wk.dinvU, d0, s), B, 0.0, B);
     const int h = split(s);
     HP_TRY(trsm_upper(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk));
     HP_TRY(gemm(st, h, ncols, s - h, -1.0, A.sub(d0, d0 + h), B.sub(h, 0), 1.0, B));
@@ -392,9 +537,18 @@ template <class V> static int getrf_rec(cudaStream_t st, int n, V A, int c0, int
     if (w <= IB) return panel(st, n, A, c0, w, ipiv, info_dev, wk);
     const int h = split(w), mid = c0 + h;
     HP_TRY(getrf_rec(st, n, A, c0, mid, ipiv, info_dev, wk));
-    HP_TRY(trsm_lower(st, A, c0, h, A.sub(c0, mid), c1 - mid, wk));
-    HP_TRY(gemm(st, n - mid, c1 - mid, h, -1.0, A.sub(mid, c0), A.sub(c0, mid), 1.0, A.sub(mid, mid)));
-    return getrf_rec(st, n, A, mid, c1, ipiv, info_dev, wk);
+    {
+        ProfCat pc(PROF_LU_TRSM);
+        HP_TRY(trsm_lower(st, A, c0, h, A.sub(c0, mid), c1 - mid, wk));
+    }
+    {
+        ProfCat pc(PROF_LU_GEMM);
+        HP_TRY(gemm(st, n - mid, c1 - mid, h, -1.0, A.sub(mid, c0), A.sub(c0, mid), 1.0, A.sub(mid, mid)));
+    }
+    HP_TRY(getrf_rec(st, n, A, mid, c1, ipiv, info_dev, wk));
+    // the node's diagonal block is final: keep its inverse for the triangular solves further up / in getrs
+    if (w <= LEAF) HP_TRY(inv_double(st, A, c0, h, w, wk));
+    return 0;
 }
 
 template <class V> int getrf(cudaStream_t st, int n, V A, int *ipiv, int *info_dev, LuWork<V> &wk) {
@@ -406,6 +560,7 @@ template <class V> int getrf(cudaStream_t st, int n, V A, int *ipiv, int *info_d
 
 template <class V> int getrs(cudaStream_t st, int n, int nrhs, V A, V B, LuWork<V> &wk) {
     if (n <= 0 || nrhs <= 0) return 0;
+    ProfCat pc(PROF_SOLVE);
     HP_TRY(laswp(st, B, 0, nrhs, 0, 0, wk.perm, 0, wk.nblk));
     HP_TRY(trsm_lower(st, A, 0, n, B, nrhs, wk));
     return trsm_upper(st, A, 0, n, B, nrhs, wk);

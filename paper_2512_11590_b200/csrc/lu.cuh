@@ -4,7 +4,10 @@
 
 namespace hp {
 
-constexpr int IB = 32;        // panel width = swap batch = inverted diagonal block size
+constexpr int IB = 32;        // panel width = swap batch = smallest inverted diagonal block
+constexpr int LEAF = 128;     // largest inverted diagonal block = leaf of the triangular-solve recursion (one GEMM M tile,
+                              // so that the leaf product B <- inv * B may run in place)
+constexpr int NLEV = 3;       // inverted diagonal blocks are kept at sizes IB << lev, lev = 0 .. NLEV-1
 constexpr int MAXG = kNumSMs; // CTAs of the cooperative panel kernel (one per SM)
 
 // GEMM back-ends (zgemm.cu / cgemm.cu): C <- beta*C + alpha*A*B.  nbatch > 1: operand b lives at view + b*stride
@@ -19,7 +22,8 @@ template <class V> struct LuWork {
     typedef typename V::elem_t E;
     typedef typename V::real_t T;
     int n = 0, nblk = 0;
-    V dinvL, dinvU;      // nblk blocks of IB x IB, block b at column offset b*IB, ld = IB
+    V dinvL[NLEV], dinvU[NLEV];  // level lev: blocks of s x s, s = IB << lev, block b at column offset b*s, ld = s:
+                                 // inverses of the unit-lower / upper triangle of the diagonal block at (b*s, b*s)
     int *perm = nullptr; // nblk x (1 + 4*IB): count, dst rows[2*IB], src rows[2*IB]  (net permutation of each swap batch)
     T *cand_val = nullptr;
     int *cand_row = nullptr;

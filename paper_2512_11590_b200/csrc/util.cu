@@ -8,8 +8,11 @@ thread_local char g_cuda_err[256] = "";
 long long g_launches = 0;
 
 // ---- optional per-launch timing of the GEMM kernel (bench.py's roofline leg): one CUDA-event pair around every launch
-struct ProfRec { cudaEvent_t a, b; double flops; };
+struct ProfRec { cudaEvent_t a, b; double flops; int cat; };
 static bool g_prof_on = false;
+int g_prof_cat = PROF_OTHER;
+static double g_cat_ms[PROF_NCAT], g_cat_flops[PROF_NCAT];
+static long long g_cat_n[PROF_NCAT];
 static std::vector<ProfRec> g_prof;
 static std::vector<cudaEvent_t> g_prof_pool;
 static cudaEvent_t prof_event() {
@@ -20,7 +23,7 @@ static cudaEvent_t prof_event() {
 }
 bool prof_enabled() { return g_prof_on; }
 void prof_begin(cudaStream_t st, double flops) {
-    ProfRec r{prof_event(), prof_event(), flops};
+    ProfRec r{prof_event(), prof_event(), flops, g_prof_cat};
     cudaEventRecord(r.a, st);
     g_prof.push_back(r);
 }
@@ -34,11 +37,13 @@ extern "C" int hprmat_profile(int enable) {
 extern "C" int hprmat_profile_read(double *ms, double *flops, long long *launches) {
     double t = 0.0, f = 0.0;
     long long n = 0;
+    for (int c = 0; c < hp::PROF_NCAT; ++c) { hp::g_cat_ms[c] = hp::g_cat_flops[c] = 0.0; hp::g_cat_n[c] = 0; }
     for (auto &r : hp::g_prof) {
         if (cudaEventSynchronize(r.b) != cudaSuccess) return HPRMAT_ECUDA;
         float m = 0.f;
         cudaEventElapsedTime(&m, r.a, r.b);
-        t += m; f += r.flops; ++n;
+        hp::g_cat_ms[r.cat] += m; hp::g_cat_flops[r.cat] += r.flops; ++hp::g_cat_n[r.cat];
+        if (r.flops > 0.0) { t += m; f += r.flops; ++n; }
         hp::g_prof_pool.push_back(r.a);
         hp::g_prof_pool.push_back(r.b);
     }
@@ -46,6 +51,14 @@ extern "C" int hprmat_profile_read(double *ms, double *flops, long long *launche
     if (ms) *ms = t;
     if (flops) *flops = f;
     if (launches) *launches = n;
+    return HPRMAT_OK;
+}
+
+extern "C" int hprmat_profile_cat(int cat, double *ms, double *flops, long long *launches) {
+    if (cat < 0 || cat >= hp::PROF_NCAT) return -1;
+    if (ms) *ms = hp::g_cat_ms[cat];
+    if (flops) *flops = hp::g_cat_flops[cat];
+    if (launches) *launches = hp::g_cat_n[cat];
     return HPRMAT_OK;
 }
 
