@@ -97,6 +97,15 @@ def run_probe(args):
             out.append({"ctas_per_sm": cps, "tflops": tf, "ms": ms})
         print(json.dumps({"probe": "dmma", "runs": out, "peak_tflops": max(o["tflops"] for o in out)}))
         return 0
+    if args.probe == "panel":
+        for m in (256, 2048, 12800, 25600, 37888):
+            us, ph = hb.hprmat_probe_panel(m, 20)
+            G = sum(1 for r in ph if any(r))
+            names = ("load", "argmax", "publish", "wait_all", "fetch_row", "update")
+            for c in sorted({0, G // 2, G - 1}):
+                print(json.dumps({"probe": "panel", "m": m, "us_per_panel": us, "ctas": G, "cta": c,
+                                  "cycles": dict(zip(names, ph[c]))}))
+        return 0
     m, n, k = args.m, args.n, args.k
     g = torch.Generator(device="cuda").manual_seed(1)
     A = torch.randn((k, m), dtype=torch.complex128, device="cuda", generator=g)   # column-major m x k
@@ -172,7 +181,7 @@ def main():
     ap.add_argument("--cfg", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--probe", default=None, choices=["zgemm", "dmma"],
+    ap.add_argument("--probe", default=None, choices=["zgemm", "dmma", "panel"],
                     help="kernel probes instead of the step: zgemm = hprmat_zgemm alone at --m/--n/--k; dmma = FP64 "
                          "tensor-core issue-rate ceiling (hprmat_probe_dmma)")
     ap.add_argument("--m", type=int, default=12800)

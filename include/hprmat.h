@@ -153,6 +153,13 @@ int hprmat_profile_cat(int cat, double *ms, double *flops, long long *launches);
  * register-resident loop (no memory traffic) on 148*ctas_per_sm CTAs of 8 warps, `iters` x 8 MMAs per warp.
  * tflops (host, out): real TFLOP/s; ms (host, out, may be NULL): device time of the timed launch.  Synchronises. */
 int hprmat_probe_dmma(void *cuda_stream, int iters, int ctas_per_sm, double *tflops, double *ms);
+/* Measurement aid: `reps` back-to-back launches of the register-resident panel-factorisation kernel (complex64 planes) on
+ * the m x 32 panel A (dev, lda >= m, contents destroyed), m <= 148*256.  workspace: dev, hprmat_workspace_bytes(m, 0,
+ * HPRMAT_MIXED) bytes.  us_per_panel (host, out): mean device time per launch.  phase_cycles (host, out, may be NULL):
+ * long long[148*8]; [cta*8 + k] = SM cycles thread 0 of CTA cta spent in phase k of the last launch (0 load, 1 local
+ * arg-max, 2 publish, 3 wait for all candidates, 4 fetch pivot row, 5 interchange + rank-1 update).  Synchronises. */
+int hprmat_probe_panel(void *cuda_stream, int m, int reps, float *A_re, float *A_im, int lda, void *workspace,
+                       double *us_per_panel, long long *phase_cycles);
 /* number of kernel launches issued by this library since process start (bench.py's gpu_launches) */
 long long hprmat_launch_count(void);
 

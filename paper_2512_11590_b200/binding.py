@@ -102,6 +102,23 @@ def hprmat_probe_dmma(iters=20000, ctas_per_sm=2, stream=None):
     return tf.value, ms.value
 
 
+def hprmat_probe_panel(m: int, reps: int = 20, stream=None):
+    """Mean device time (us) of the panel-factorisation kernel on an m x 32 complex64 panel + per-phase cycles."""
+    import torch
+    g = torch.Generator(device="cuda").manual_seed(7)
+    Are = torch.rand((32, m), dtype=torch.float32, device="cuda", generator=g)
+    Aim = torch.rand((32, m), dtype=torch.float32, device="cuda", generator=g)
+    wsb = int(lib().hprmat_workspace_bytes(C.c_int(m), C.c_int(0), C.c_int(HPRMAT_MIXED)))
+    ws = torch.empty(wsb + 256, dtype=torch.uint8, device="cuda")
+    wp = (ws.data_ptr() + 255) // 256 * 256
+    us = C.c_double(0)
+    ph = (C.c_longlong * (148 * 8))()
+    _check(lib().hprmat_probe_panel(_stream(stream), C.c_int(m), C.c_int(reps), C.c_void_p(Are.data_ptr()),
+                                    C.c_void_p(Aim.data_ptr()), C.c_int(m), C.c_void_p(wp), C.byref(us), ph),
+           "hprmat_probe_panel")
+    return us.value, [[int(ph[c * 8 + k]) for k in range(6)] for c in range(148)]
+
+
 # ---- structured R-matrix path ---------------------------------------------------------------------------------------
 class Context:
     """Owner of an hprmat_ctx (hprmat_setup ... hprmat_destroy)."""

@@ -30,6 +30,8 @@ template <class V> struct LuWork {
     E *cand_data = nullptr, *jrow = nullptr;
     unsigned *counter = nullptr;
     unsigned bar_base = 0; // host-side running value of the grid-barrier counter
+    unsigned long long *slots = nullptr; // epoch-tagged exchange words of the register-resident panel kernel (lu.cu)
+    unsigned ep_base = 0;  // host-side running column count (epoch base) of that kernel
     static size_t bytes(int n);
     // carve from p (must be 256-byte aligned); returns bytes used
     size_t carve(void *p, int n);

@@ -55,3 +55,20 @@ extern "C" int hprmat_probe_dmma(void *cuda_stream, int iters, int ctas_per_sm, 
     cudaFree(sink);
     return HPRMAT_OK;
 }
+
+
+namespace hp {
+int probe_panel(cudaStream_t st, int m, int reps, float *A_re, float *A_im, long lda, void *work, double *us_per_panel,
+                long long *phase_cycles_host);
+}
+// Panel-factorisation probe: see hprmat.h.
+extern "C" int hprmat_probe_panel(void *cuda_stream, int m, int reps, float *A_re, float *A_im, int lda, void *workspace,
+                                  double *us_per_panel, long long *phase_cycles) {
+    if (m < 1) return -2;
+    if (reps < 1) return -3;
+    if (!A_re || !A_im) return -4;
+    if (lda < m) return -6;
+    if (!workspace) return -7;
+    if (!us_per_panel) return -8;
+    return hp::probe_panel((cudaStream_t)cuda_stream, m, reps, A_re, A_im, lda, workspace, us_per_panel, phase_cycles);
+}
