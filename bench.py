@@ -107,6 +107,25 @@ def run_probe(args):
                                   "cycles": dict(zip(names, ph[c]))}))
         return 0
     m, n, k = args.m, args.n, args.k
+    if args.probe == "cgemm":
+        g = torch.Generator(device="cuda").manual_seed(1)
+        pl = lambda r, c: torch.randn((c, r), dtype=torch.float32, device="cuda", generator=g)   # column-major r x c
+        Ar, Ai, Br, Bi, Cr, Ci = pl(m, k), pl(m, k), pl(k, n), pl(k, n), pl(m, n), pl(m, n)
+        for _ in range(args.warmup):
+            hb.hprmat_cgemm_tf32(m, n, k, -1.0, Ar, Ai, m, Br, Bi, k, 1.0, Cr, Ci, m)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(args.steps):
+            hb.hprmat_cgemm_tf32(m, n, k, -1.0, Ar, Ai, m, Br, Bi, k, 1.0, Cr, Ci, m)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        tf = 8.0 * m * n * k / (ms * 1e-3) * 1e-12
+        pk, how = peaks()
+        print(json.dumps({"probe": "cgemm_tf32", "m": m, "n": n, "k": k, "ms": ms, "tflops": tf,
+                          "frac_of_tf32_peak": tf / (0.5 * pk["bf16_tflops_sustained"]), "peak_source": how}))
+        return 0
     g = torch.Generator(device="cuda").manual_seed(1)
     A = torch.randn((k, m), dtype=torch.complex128, device="cuda", generator=g)   # column-major m x k
     B = torch.randn((n, k), dtype=torch.complex128, device="cuda", generator=g)   # column-major k x n
@@ -181,7 +200,7 @@ def main():
     ap.add_argument("--cfg", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--probe", default=None, choices=["zgemm", "dmma", "panel"],
+    ap.add_argument("--probe", default=None, choices=["zgemm", "cgemm", "dmma", "panel"],
                     help="kernel probes instead of the step: zgemm = hprmat_zgemm alone at --m/--n/--k; dmma = FP64 "
                          "tensor-core issue-rate ceiling (hprmat_probe_dmma)")
     ap.add_argument("--m", type=int, default=12800)
