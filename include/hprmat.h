@@ -137,6 +137,12 @@ int hprmat_zgemm(void *cuda_stream, int m, int n, int k, double alpha, const voi
 int hprmat_cgemm_tf32(void *cuda_stream, int m, int n, int k, float alpha, const float *A_re, const float *A_im, int lda,
                       const float *B_re, const float *B_im, int ldb, float beta, float *C_re, float *C_im, int ldc);
 
+/* Same operation with FP32-class accuracy ("3xTF32": every operand split in registers into two TF32 terms, three
+ * mma.sync products per real product, FP32 accumulation): the GEMM of the triangular solves of the mixed modes, whose
+ * O(1) right-hand sides must not be rounded to 10 mantissa bits.  Same argument rules. */
+int hprmat_cgemm_3xtf32(void *cuda_stream, int m, int n, int k, float alpha, const float *A_re, const float *A_im, int lda,
+                        const float *B_re, const float *B_im, int ldb, float beta, float *C_re, float *C_im, int ldc);
+
 const char *hprmat_strerror(int code);
 const char *hprmat_last_cuda_error(void);
 /* Measurement aid (bench.py's roofline leg): while enabled, every launch of the GEMM kernel inside the LU and the

@@ -216,6 +216,14 @@ def hprmat_cgemm_tf32(m, n, k, alpha, A_re, A_im, lda, B_re, B_im, ldb, beta, C_
     _check(rc, "hprmat_cgemm_tf32")
 
 
+def hprmat_cgemm_3xtf32(m, n, k, alpha, A_re, A_im, lda, B_re, B_im, ldb, beta, C_re, C_im, ldc, stream=None):
+    """Planar complex64 GEMM with FP32-class accuracy (3xTF32, mma.sync); operands as hprmat_cgemm_tf32."""
+    rc = lib().hprmat_cgemm_3xtf32(_stream(stream), C.c_int(m), C.c_int(n), C.c_int(k), C.c_float(alpha), _dev(A_re),
+                                   _dev(A_im), C.c_int(lda), _dev(B_re), _dev(B_im), C.c_int(ldb), C.c_float(beta),
+                                   _dev(C_re), _dev(C_im), C.c_int(ldc))
+    _check(rc, "hprmat_cgemm_3xtf32")
+
+
 def hprmat_zgetrf(n, A, lda, ipiv, info_dev, ws=None, stream=None):
     """In-place FP64 LU; A torch complex128 CUDA holding the column-major n x n matrix (lda >= n)."""
     if ws is None:

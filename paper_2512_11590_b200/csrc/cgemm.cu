@@ -61,7 +61,9 @@ __global__ void __launch_bounds__(CG_NT, 1)
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tmem_full + 1);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int m0 = blockIdx.x * CG_BM, n0 = blockIdx.y * BN;
+    int tm, tn;
+    raster((int)blockIdx.x, (M + CG_BM - 1) / CG_BM, (N + BN - 1) / BN, 12, tm, tn);
+    const int m0 = tm * CG_BM, n0 = tn * BN;
     const int nk = (K + CG_KC - 1) / CG_KC;
 
     if (warp == 0 && lane == 0) {
@@ -237,7 +239,7 @@ int launch_cgemm(cudaStream_t st, int m, int n, int k, float alpha, CView A, CVi
     HP_TRY(make_map(&maps.a_im, A.im, m, kk, A.ld, 32, CG_KC, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B));
     HP_TRY(make_map(&maps.b_re, B.re, kk, n, B.ld, CG_KC, BN, CU_TENSOR_MAP_SWIZZLE_128B));
     HP_TRY(make_map(&maps.b_im, B.im, kk, n, B.ld, CG_KC, BN, CU_TENSOR_MAP_SWIZZLE_128B));
-    dim3 grid(ceil_div(m, CG_BM), ceil_div(n, BN));
+    dim3 grid(ceil_div(m, CG_BM) * ceil_div(n, BN));
     kern<<<grid, CG_NT, Cfg::SMEM, st>>>(maps, m, n, k, alpha, beta, C.re, C.im, C.ld);
     HP_LAUNCHED();
     return 0;

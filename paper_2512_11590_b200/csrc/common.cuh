@@ -47,6 +47,19 @@ bool prof_enabled();
 void prof_begin(cudaStream_t st, double flops);
 void prof_end(cudaStream_t st);
 
+// Grouped ("super-tile") CTA rasterisation of a tiles_m x tiles_n grid: consecutive CTA ids walk down GROUP tile rows, then
+// step one tile column, so that the ~148 CTAs in flight cover a roughly square block of C and share their A and B panels
+// through L2 instead of streaming the whole of A once per tile column.
+__device__ __forceinline__ void raster(int pid, int tiles_m, int tiles_n, int group, int &tm, int &tn) {
+    const int per_group = group * tiles_n;
+    const int gid = pid / per_group;
+    const int first = gid * group;
+    const int gsz = min(tiles_m - first, group);
+    const int r = pid - gid * per_group;
+    tm = first + r % gsz;
+    tn = r / gsz;
+}
+
 inline int ceil_div(long a, long b) { return (int)((a + b - 1) / b); }
 inline long round_up(long a, long b) { return (a + b - 1) / b * b; }
 

@@ -926,25 +926,36 @@ template <class V> static int panel(cudaStream_t st, int n, V A, int c0, int w, 
     return laswp(st, A, 0, c0, c0 + w, n, wk.perm, blk, blk + 1);
 }
 
+// Leaf product of the triangular solves (inverted diagonal block times the right-hand sides): acc = FP32-class accuracy
+// for the complex64 type (3xTF32).  The diagonal blocks are O(1) (their rounding to 10 mantissa bits would cap the solve
+// at ~1e-3); the off-diagonal updates B2 -= L21 X1 stay single-pass like the trailing update of the factorisation, their
+// error being 2^-11 |L21| |X1| with |L21| the (small) coupling entries.
+static int gemm_sel(bool, cudaStream_t st, int m, int n, int k, double alpha, ZView A, ZView B, double beta, ZView C) {
+    return gemm(st, m, n, k, alpha, A, B, beta, C);
+}
+static int gemm_sel(bool acc, cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C) {
+    return acc ? cgemm3(st, m, n, k, alpha, A, B, beta, C) : gemm(st, m, n, k, alpha, A, B, beta, C);
+}
+
 // B <- L^-1 B, L = unit lower triangle of the s x s diagonal block of A at (d0,d0); B is s x ncols.  d0 is a multiple of
 // LEAF, or s <= LEAF is a full block of its size class (or the ragged last block).
-template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk) {
+template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk, bool acc = false) {
     if (s <= 0 || ncols <= 0) return 0;
-    if (s <= LEAF) return gemm(st, s, ncols, s, 1.0, dinv_of(wk.dinvL, d0, s), B, 0.0, B);
+    if (s <= LEAF) return gemm_sel(acc, st, s, ncols, s, 1.0, dinv_of(wk.dinvL, d0, s), B, 0.0, B);
     const int h = split(s);
-    HP_TRY(trsm_lower(st, A, d0, h, B, ncols, wk));
+    HP_TRY(trsm_lower(st, A, d0, h, B, ncols, wk, acc));
     HP_TRY(gemm(st, s - h, ncols, h, -1.0, A.sub(d0 + h, d0), B, 1.0, B.sub(h, 0)));
-    return trsm_lower(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk);
+    return trsm_lower(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk, acc);
 }
 
 // B <- U^-1 B, U = upper triangle (with diagonal) of the s x s diagonal block of A at (d0,d0)
-template <class V> static int trsm_upper(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk) {
+template <class V> static int trsm_upper(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk, bool acc = false) {
     if (s <= 0 || ncols <= 0) return 0;
-    if (s <= LEAF) return gemm(st, s, ncols, s, 1.0, dinv_of(wk.dinvU, d0, s), B, 0.0, B);
+    if (s <= LEAF) return gemm_sel(acc, st, s, ncols, s, 1.0, dinv_of(wk.dinvU, d0, s), B, 0.0, B);
     const int h = split(s);
-    HP_TRY(trsm_upper(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk));
+    HP_TRY(trsm_upper(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk, acc));
     HP_TRY(gemm(st, h, ncols, s - h, -1.0, A.sub(d0, d0 + h), B.sub(h, 0), 1.0, B));
-    return trsm_upper(st, A, d0, h, B, ncols, wk);
+    return trsm_upper(st, A, d0, h, B, ncols, wk, acc);
 }
 
 template <class V> static int getrf_rec(cudaStream_t st, int n, V A, int c0, int c1, int *ipiv, int *info_dev, LuWork<V> &wk) {
@@ -979,8 +990,9 @@ template <class V> int getrs(cudaStream_t st, int n, int nrhs, V A, V B, LuWork<
     if (n <= 0 || nrhs <= 0) return 0;
     ProfCat pc(PROF_SOLVE);
     HP_TRY(laswp(st, B, 0, nrhs, 0, 0, wk.perm, 0, wk.nblk));
-    HP_TRY(trsm_lower(st, A, 0, n, B, nrhs, wk));
-    return trsm_upper(st, A, 0, n, B, nrhs, wk);
+    // the right-hand sides and the solution are O(1): FP32-class diagonal-block products (3xTF32 for the complex64 type)
+    HP_TRY(trsm_lower(st, A, 0, n, B, nrhs, wk, true));
+    return trsm_upper(st, A, 0, n, B, nrhs, wk, true);
 }
 
 // Measurement aid (hprmat_probe_panel): `reps` back-to-back factorisations of the same m x IB panel (the data are garbage

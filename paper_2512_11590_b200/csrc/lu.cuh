@@ -14,6 +14,8 @@ constexpr int MAXG = kNumSMs; // CTAs of the cooperative panel kernel (one per S
 // elements.  C may alias B when m <= 32 and the whole K extent is one diagonal block (see trsm in lu.cu).
 int gemm(cudaStream_t st, int m, int n, int k, double alpha, ZView A, ZView B, double beta, ZView C);
 int gemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
+// FP32-class accuracy variant for the planar complex64 type (3xTF32, cgemm3.cu); C may alias B when m <= 128, beta == 0
+int cgemm3(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
 int zgemm_batched(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda, long strideA,
                   const double2 *B, long ldb, long strideB, double beta, double2 *C, long ldc, long strideC, int nbatch);
 

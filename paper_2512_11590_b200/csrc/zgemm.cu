@@ -55,7 +55,9 @@ __global__ void __launch_bounds__(WM *WN * 32, MINB)
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int wm = warp % WM, wn = warp / WM;
     const int r = lane >> 2, kk = lane & 3;
-    const long m0 = (long)blockIdx.x * BM, n0 = (long)blockIdx.y * BN;
+    int tm, tn;
+    raster((int)blockIdx.x, (M + BM - 1) / BM, (N + BN - 1) / BN, 8, tm, tn);
+    const long m0 = (long)tm * BM, n0 = (long)tn * BN;
     A += (long)blockIdx.z * strideA;
     B += (long)blockIdx.z * strideB;
     C += (long)blockIdx.z * strideC;
@@ -161,7 +163,7 @@ static int launch_zgemm(cudaStream_t st, int m, int n, int k, double alpha, cons
         HP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured = true;
     }
-    dim3 grid(ceil_div(m, BM), ceil_div(n, BN), nbatch);
+    dim3 grid(ceil_div(m, BM) * ceil_div(n, BN), 1, nbatch);
     kern<<<grid, WM * WN * 32, smem, st>>>(m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC);
     HP_LAUNCHED();
     return 0;

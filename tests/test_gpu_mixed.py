@@ -78,6 +78,49 @@ def test_cgemm_tf32_is_exact_on_tf32_representable_integers():
     assert np.array_equal(_unplanes(Cr, Ci, m), C0 - A @ B)
 
 
+@pytest.mark.parametrize("m,n,k,alpha,beta", [
+    (128, 64, 32, 1.0, 0.0), (128, 256, 128, 1.0, 0.0), (256, 384, 96, -1.0, 1.0), (100, 50, 37, 1.0, 0.0),
+    (257, 129, 65, -1.0, 1.0), (32, 700, 32, 1.0, 0.0), (1000, 333, 200, -1.0, 1.0), (5, 3, 1, 2.0, -0.5),
+    (640, 256, 1024, -1.0, 1.0), (1, 1, 8, 1.0, 1.0)])
+def test_cgemm_3xtf32_matches_definition_to_fp32_accuracy(m, n, k, alpha, beta):
+    """hprmat_cgemm_3xtf32: operands split hi + lo in TF32 (dropped lo*lo term and the rounding of lo: <= 2^-21 relative
+    per product, taken as 2^-20 here), FP32 accumulation:  |C - C_def| <= (2^-20 + (k + 4) 2^-23) (|alpha| |A||B| + |beta||C0|).
+    On the same data the single-pass kernel is ~2^-10: a kernel that silently fell back to one pass fails this bound."""
+    rng = np.random.default_rng(m * 1000003 + n * 1009 + k + 7)
+    A = (rng.uniform(-1, 1, (m, k)) + 1j * rng.uniform(-1, 1, (m, k))).astype(np.complex64).astype(np.complex128)
+    B = (rng.uniform(-1, 1, (k, n)) + 1j * rng.uniform(-1, 1, (k, n))).astype(np.complex64).astype(np.complex128)
+    C0 = (rng.uniform(-1, 1, (m, n)) + 1j * rng.uniform(-1, 1, (m, n))).astype(np.complex64).astype(np.complex128)
+    lda, ldb, ldc = _rup(m, 4), _rup(k, 4), _rup(m, 4) + 4
+    Ar, Ai = _planes(A, lda)
+    Br, Bi = _planes(B, ldb)
+    Cr, Ci = _planes(C0, ldc)
+    hb.hprmat_cgemm_3xtf32(m, n, k, alpha, Ar, Ai, lda, Br, Bi, ldb, beta, Cr, Ci, ldc)
+    torch.cuda.synchronize()
+    got = _unplanes(Cr, Ci, m)
+    ref = beta * C0 + alpha * (A @ B)
+    absA = np.abs(A.real) + np.abs(A.imag)
+    absB = np.abs(B.real) + np.abs(B.imag)
+    bound = (2.0 ** -20 + (k + 4) * 2.0 ** -23) * (abs(alpha) * (absA @ absB) + abs(beta) * (np.abs(C0.real) + np.abs(C0.imag)))
+    err = np.abs(got - ref)
+    assert np.all(err <= bound + 1e-30), (err.max(), bound.max(), np.unravel_index(np.argmax(err - bound), err.shape))
+    assert float(Cr[:, m:].abs().max()) == 0.0 and float(Ci[:, m:].abs().max()) == 0.0
+
+
+def test_cgemm_3xtf32_in_place_leaf_product():
+    """The triangular-solve leaf runs B <- A B in place (m = k <= 128, beta = 0): C aliases B."""
+    m, n = 128, 300
+    rng = np.random.default_rng(11)
+    A = (rng.uniform(-1, 1, (m, m)) + 1j * rng.uniform(-1, 1, (m, m))).astype(np.complex64).astype(np.complex128)
+    B = (rng.uniform(-1, 1, (m, n)) + 1j * rng.uniform(-1, 1, (m, n))).astype(np.complex64).astype(np.complex128)
+    Ar, Ai = _planes(A, m)
+    Br, Bi = _planes(B, m)
+    hb.hprmat_cgemm_3xtf32(m, n, m, 1.0, Ar, Ai, m, Br, Bi, m, 0.0, Br, Bi, m)
+    torch.cuda.synchronize()
+    absA = np.abs(A.real) + np.abs(A.imag)
+    absB = np.abs(B.real) + np.abs(B.imag)
+    assert np.all(np.abs(_unplanes(Br, Bi, m) - A @ B) <= (2.0 ** -20 + (m + 4) * 2.0 ** -23) * (absA @ absB))
+
+
 # ---------------------------------------------------------------------------------------------------- whole path, mixed
 import oracle  # noqa: E402
 from paper_2512_11590_b200.workloads import make_workload  # noqa: E402
