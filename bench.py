@@ -241,8 +241,9 @@ def main():
     V = V_host.to("cuda")
     R = torch.empty((w.nch, w.nch), dtype=torch.complex128, device="cuda")
     R_host = torch.empty((w.nch, w.nch), dtype=torch.complex128).pin_memory()
-    # rank k takes the k-th point of an energy scan around the config's energy (replicas; weak scaling)
-    E = float(w.energies[0]) + 0.5 * rank
+    # rank k takes the k-th point of the config's energy scan (replicas; weak scaling)
+    from paper_2512_11590_b200 import scan
+    E = scan.bench_energy(w.energies, rank)
     N = w.n
 
     for _ in range(args.warmup):
@@ -262,10 +263,7 @@ def main():
     launches = hb.hprmat_launch_count() - l0
     clocks = sampler.stop() if sampler else None
     t_dev = e0.elapsed_time(e1) * 1e-3
-    tt = torch.tensor([t_dev], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_max = float(tt.item())
+    t_max = scan.max_over_ranks(t_dev, device="cuda")
     sec_per_step = t_max / args.steps
 
     # ---- end to end: host V in, host R out, through hprmat_solve_host, copies inside the timed region
@@ -277,10 +275,7 @@ def main():
         ctx.solve_host(E, Vh_np, mode, R_host=Rh_np)
     torch.cuda.synchronize()
     te = time.perf_counter() - t0
-    tt = torch.tensor([te], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    e2e_sec = float(tt.item()) / args.steps
+    e2e_sec = scan.max_over_ranks(te, device="cuda") / args.steps
 
     # ---- roofline leg: one more step with a CUDA-event pair around every GEMM launch (the trailing-update kernel)
     roof = None
