@@ -112,7 +112,9 @@ size_t hprmat_workspace_bytes(int n, int nrhs, int mode);
  * ipiv dev int[n], 1-based LAPACK row interchanges (of the matrix actually factorised: A itself in FP64 mode).
  * HPRMAT_FP64: A is OVERWRITTEN by its LU factors (unit-lower L and U, LAPACK zgetrf layout).
  * HPRMAT_MIXED / HPRMAT_MIXED_REFINE: A is preserved; the factors of the row/column-equilibrated complex64 copy live
- * in the workspace; refinement uses the FP64 residual B - A X.
+ * in the workspace; refinement uses the FP64 residual B - A X and contracts by ~sqrt(n) 2^-11 kappa per
+ * step (single-pass TF32 trailing update), so max_refine < 0 means 12 here; beyond kappa ~ 1e3 the call returns
+ * HPRMAT_ENOTCONVERGED with the last iterate and HPRMAT_FP64 is the mode to use.
  * workspace dev, workspace_bytes >= hprmat_workspace_bytes(n, nrhs, mode). */
 int hprmat_zsolve(void *cuda_stream, int n, int nrhs, void *A, int lda, void *B, int ldb, int *ipiv, int mode,
                   int max_refine, double tol, void *workspace, size_t workspace_bytes, hprmat_info *info);

@@ -1,17 +1,21 @@
 // api_raw.cu -- raw dense complex entries of the C ABI: LU, triangular solves, workspace query (FP64 part).
 // PAPER.md:119 ("all solvers take the matrix M and right-hand side b and return c"), :125-137 (ZGESV semantics).
+#include <algorithm>
+
 #include "lu.cuh"
 
 using namespace hp;
 
 namespace hp {
 size_t raw_workspace_fp64(int n) { return LuWork<ZView>::bytes(n) + 256; }  // + one int for the zero-pivot flag
+size_t raw_workspace_mixed(int n, int nrhs);
+int zsolve_mixed(cudaStream_t st, int n, int nrhs, const double2 *A, long lda, double2 *B, long ldb, int *ipiv, bool refine,
+                 int max_refine, double tol, void *workspace, hprmat_info *info);
 }  // namespace hp
 
 extern "C" size_t hprmat_workspace_bytes(int n, int nrhs, int mode) {
-    (void)nrhs;
-    (void)mode;
-    if (n < 0) return 0;
+    if (n < 0 || nrhs < 0) return 0;
+    if (mode == HPRMAT_MIXED || mode == HPRMAT_MIXED_REFINE) return std::max(raw_workspace_mixed(n, nrhs), raw_workspace_fp64(n));
     return raw_workspace_fp64(n);
 }
 
@@ -49,8 +53,6 @@ extern "C" int hprmat_zgetrs(void *cuda_stream, int n, int nrhs, const void *A, 
 
 extern "C" int hprmat_zsolve(void *cuda_stream, int n, int nrhs, void *A, int lda, void *B, int ldb, int *ipiv, int mode,
                              int max_refine, double tol, void *workspace, size_t workspace_bytes, hprmat_info *info) {
-    (void)max_refine;
-    (void)tol;
     if (n < 0) return -2;
     if (nrhs < 0) return -3;
     if (!A && n > 0) return -4;
@@ -58,10 +60,21 @@ extern "C" int hprmat_zsolve(void *cuda_stream, int n, int nrhs, void *A, int ld
     if (!B && n > 0 && nrhs > 0) return -6;
     if (ldb < (n > 1 ? n : 1)) return -7;
     if (!ipiv && n > 0) return -8;
-    if (mode != HPRMAT_FP64) return -9;  // mixed raw solve: not built yet
+    if (mode != HPRMAT_FP64 && mode != HPRMAT_MIXED && mode != HPRMAT_MIXED_REFINE) return -9;
     if (!workspace || ((uintptr_t)workspace & 255)) return -12;
-    if (workspace_bytes < raw_workspace_fp64(n)) return HPRMAT_ENOMEM;
+    if (workspace_bytes < hprmat_workspace_bytes(n, nrhs, mode)) return HPRMAT_ENOMEM;
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (mode != HPRMAT_FP64) {
+        if (info) {
+            *info = hprmat_info();
+            info->backward_err = -1.0;
+        }
+        if (n == 0 || nrhs == 0) return HPRMAT_OK;
+        const int rc = zsolve_mixed(st, n, nrhs, (const double2 *)A, lda, (double2 *)B, ldb, ipiv, mode == HPRMAT_MIXED_REFINE,
+                                    max_refine, tol, workspace, info);
+        if (info) info->status = rc;
+        return rc;
+    }
     if (info) {
         *info = hprmat_info();
         info->backward_err = -1.0;  // A is overwritten by its factors in FP64 mode: no residual can be formed

@@ -15,6 +15,7 @@
 
 #include "lu.cuh"
 #include "precond.cuh"
+#include "refine.cuh"
 #include "structured.cuh"
 
 using namespace hp;
@@ -256,19 +257,6 @@ extern "C" int hprmat_get_x(const hprmat_ctx *ctx, void *X) {
 }
 
 namespace {
-
-// Decide from the correction norms whether the refinement has converged (reading R9):
-// dn = max|d_k|, xn = max|X|, dprev = max|d_{k-1}| (k = 1: max|X_0|).  The error left after this step is estimated as
-// dn * rho / (1 - rho) with the observed contraction rho = dn / dprev.
-enum { REF_CONTINUE = 0, REF_CONVERGED = 1, REF_STAGNATED = 2 };
-int refine_verdict(double dn, double xn, double dprev, double tol) {
-    if (!(dn == dn) || !(xn == xn)) return REF_STAGNATED;  // NaN
-    if (dn <= tol * xn * 1e-3) return REF_CONVERGED;        // correction already far below the target
-    const double rho = dprev > 0.0 ? dn / dprev : 1.0;
-    if (rho >= 0.5) return REF_STAGNATED;
-    if (dn * rho / (1.0 - rho) <= tol * xn) return REF_CONVERGED;
-    return REF_CONTINUE;
-}
 
 int solve_fp64(hprmat_ctx *c, double energy, const double2 *V, int max_refine, double tol, double2 *R, hprmat_info *info) {
     cudaStream_t st = c->st;

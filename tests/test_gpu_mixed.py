@@ -206,3 +206,72 @@ def test_mixed_matches_fp64_mode_on_the_same_context():
     assert info["status"] == 0
     assert _relmax(R2.cpu().numpy(), R1.cpu().numpy()) <= 1e-10
     ctx.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------- raw solve, mixed
+from paper_2512_11590_b200.workloads import dense_test_matrix  # noqa: E402
+
+
+def _dev_colmajor(a: np.ndarray) -> torch.Tensor:
+    return torch.from_numpy(np.ascontiguousarray(a.T)).to(DEV)
+
+
+@pytest.mark.parametrize("n,nrhs", [(1, 1), (33, 2), (100, 7), (257, 4), (640, 64), (1500, 3)])
+def test_zsolve_mixed_refine_matches_oracle_and_preserves_A(n, nrhs):
+    """Raw dense solve, complex64 factors + FP64 refinement: x to FP64 accuracy, A untouched,
+    with the equations scaled badly on purpose (rows spread over 2^+-20) so that the equilibration is exercised.  (A
+    column spread would spread the unknowns of the equilibrated system as widely, and a solve with single-pass TF32 factors
+    is only normwise accurate, contraction ~sqrt(n) 2^-11 per step: that regime belongs to HPRMAT_FP64.)"""
+    A = dense_test_matrix(n, nrhs, seed=9000 + n)
+    rng = np.random.default_rng(n)
+    A = np.asfortranarray((2.0 ** rng.integers(-20, 21, n))[:, None] * A)
+    B = np.asfortranarray(A @ np.ones((n, nrhs), dtype=np.complex128))
+    Xo = oracle.solve(A, B, mode=0, nrefine=2)
+    Ad, Bd = _dev_colmajor(A), _dev_colmajor(B)
+    _, info = hb.hprmat_zsolve(n, nrhs, Ad, n, Bd, n, mode=hb.HPRMAT_MIXED_REFINE)
+    assert info["status"] == 0 and info["refine_steps"] >= 1
+    assert np.array_equal(_host(Ad), A)                                       # mixed modes preserve A
+    X = _host(Bd)
+    assert np.abs(X - Xo).max() / np.abs(Xo).max() <= 1e-10
+    assert 0 <= info["backward_err"] <= 50 * max(n, 64) * 2.0 ** -53    # converged to tol = 1e-13, not to the last bit
+
+
+def test_zsolve_mixed_without_refinement_is_single_precision_class():
+    n, nrhs = 640, 8
+    A = dense_test_matrix(n, nrhs, seed=4242)
+    B = np.asfortranarray(A @ np.ones((n, nrhs), dtype=np.complex128))
+    Ad, Bd = _dev_colmajor(A), _dev_colmajor(B)
+    _, info = hb.hprmat_zsolve(n, nrhs, Ad, n, Bd, n, mode=hb.HPRMAT_MIXED)
+    assert info["status"] == 0 and info["refine_steps"] == 0
+    err = np.abs(_host(Bd) - 1.0).max()
+    assert 1e-12 < err <= 1e-2          # single-pass TF32 factors of a general matrix: ~sqrt(n) 2^-11, honestly reported
+
+
+def _householder_graded(n, kappa, seed):
+    """Hermitian test matrix of prescribed condition number: Householder similarity of a graded diagonal (the paper's
+    Fig. 5 construction)."""
+    rng = np.random.default_rng(seed)
+    v = rng.normal(size=n) + 1j * rng.normal(size=n)
+    v /= np.linalg.norm(v)
+    H = np.eye(n) - 2.0 * np.outer(v, v.conj())
+    d = kappa ** (-np.arange(n) / (n - 1.0))
+    return np.asfortranarray(H @ np.diag(d) @ H.conj().T)
+
+
+@pytest.mark.parametrize("kappa", [1e1, 1e2, 1e5, 1e8])
+def test_zsolve_mixed_never_returns_a_silent_low_precision_result(kappa):
+    """PAPER.md:561, Fig. 5: refinement recovers FP64 accuracy while kappa * u_low < 1 and breaks down beyond; the solver
+    must then SAY so.  Either status 0 and a forward error at the FP64 level for this kappa, or HPRMAT_ENOTCONVERGED."""
+    n, nrhs = 512, 4
+    A = _householder_graded(n, kappa, seed=31)
+    B = np.asfortranarray(A @ np.ones((n, nrhs), dtype=np.complex128))
+    Ad, Bd = _dev_colmajor(A), _dev_colmajor(B)
+    _, info = hb.hprmat_zsolve(n, nrhs, Ad, n, Bd, n, mode=hb.HPRMAT_MIXED_REFINE, max_refine=30,
+                               allow=(hb.HPRMAT_OK, hb.HPRMAT_ENOTCONVERGED))
+    err = np.abs(_host(Bd) - 1.0).max()
+    if info["status"] == hb.HPRMAT_OK:
+        assert err <= 100 * kappa * 2.0 ** -53 * n
+    else:
+        assert info["status"] == hb.HPRMAT_ENOTCONVERGED
+    if kappa <= 1e2:
+        assert info["status"] == hb.HPRMAT_OK                                  # well inside the convergence domain
