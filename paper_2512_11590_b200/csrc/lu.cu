@@ -763,63 +763,63 @@ __global__ void __launch_bounds__(INV_NT) inv_double_kernel(V A, int h, int w, V
     const V M = isU ? A.sub(0, h) : A.sub(h, 0);   // p x q factor block
     const int li0 = isU ? i0 : i0 - h;             // row offset inside XL
     const int ocol = isU ? h : 0;                  // column offset of the product inside the output
+    constexpr int HL = LEAF / 2;                   // p, q <= HL
     E *xs = reinterpret_cast<E *>(smraw);          // [p][INV_RS]: XL[I, k] at xs[k*INV_RS + r]
-    E *ts = xs + (size_t)(LEAF / 2) * INV_RS;      // [q][INV_RS]: T[r, j] at ts[j*INV_RS + r]
+    E *ts = xs + (size_t)HL * INV_RS;              // [q][INV_RS]: T[r, j] at ts[j*INV_RS + r]
+    E *ms = ts + (size_t)HL * INV_RS;              // [q][p]: M[k, j] at ms[j*p + k]   (column-major, as in memory)
+    E *xr = ms + (size_t)HL * HL;                  // [q][q]: XR[j, c] at xr[c*q + j]
     for (int idx = tid; idx < INV_RS * p; idx += INV_NT) {
         const int r = idx % INV_RS, k = idx / INV_RS;
         xs[idx] = r < nr ? XL.get(li0 + r, k) : mk((T)0, (T)0);
     }
+    for (int idx = tid; idx < p * q; idx += INV_NT) ms[idx] = M.get(idx % p, idx / p);
+    for (int idx = tid; idx < q * q; idx += INV_NT) xr[idx] = XR.get(idx % q, idx / q);
     // the diagonal-block copy of this strip
     for (int idx = tid; idx < nr * p; idx += INV_NT) {
         const int r = idx % nr, c = idx / nr;
         O.set(i0 + r, (isU ? 0 : h) + c, XL.get(li0 + r, c));
     }
     __syncthreads();
-    // phase 1: T = XL[I,:] * M   (warp per column j of M, lanes over k)
-    for (int j = warp; j < q; j += INV_NT / 32) {
-        E acc[INV_RS];
+    // thread = row r of the strip x columns jg, jg + 16, jg + 32, jg + 48
+    const int r = tid % INV_RS, jg = tid / INV_RS;
+    constexpr int NJ = HL / (INV_NT / INV_RS);
+    {   // phase 1: T = XL[I,:] * M
+        E acc[NJ];
 #pragma unroll
-        for (int r = 0; r < INV_RS; ++r) acc[r] = mk((T)0, (T)0);
-        for (int k = lane; k < p; k += 32) {
-            const E m = M.get(k, j);
+        for (int t = 0; t < NJ; ++t) acc[t] = mk((T)0, (T)0);
+        for (int k = 0; k < p; ++k) {
+            const E x = xs[k * INV_RS + r];
+            const E nx = mk(-x.x, -x.y);
 #pragma unroll
-            for (int r = 0; r < INV_RS; ++r) acc[r] = cfnma(acc[r], mk(-xs[k * INV_RS + r].x, -xs[k * INV_RS + r].y), m);
-        }
-#pragma unroll
-        for (int r = 0; r < INV_RS; ++r) {
-#pragma unroll
-            for (int off = 16; off > 0; off >>= 1) {
-                acc[r].x += __shfl_xor_sync(0xffffffffu, acc[r].x, off);
-                acc[r].y += __shfl_xor_sync(0xffffffffu, acc[r].y, off);
+            for (int t = 0; t < NJ; ++t) {
+                const int j = jg + (INV_NT / INV_RS) * t;
+                if (j < q) acc[t] = cfnma(acc[t], nx, ms[j * p + k]);
             }
         }
-        if (lane == 0) {
 #pragma unroll
-            for (int r = 0; r < INV_RS; ++r) ts[j * INV_RS + r] = acc[r];
+        for (int t = 0; t < NJ; ++t) {
+            const int j = jg + (INV_NT / INV_RS) * t;
+            if (j < q) ts[j * INV_RS + r] = acc[t];
         }
     }
     __syncthreads();
-    // phase 2: out = -T * XR   (warp per column c of XR, lanes over j)
-    for (int c = warp; c < q; c += INV_NT / 32) {
-        E acc[INV_RS];
+    {   // phase 2: out = -T * XR
+        E acc[NJ];
 #pragma unroll
-        for (int r = 0; r < INV_RS; ++r) acc[r] = mk((T)0, (T)0);
-        for (int j = lane; j < q; j += 32) {
-            const E x = XR.get(j, c);
+        for (int t = 0; t < NJ; ++t) acc[t] = mk((T)0, (T)0);
+        for (int j = 0; j < q; ++j) {
+            const E tv = ts[j * INV_RS + r];
 #pragma unroll
-            for (int r = 0; r < INV_RS; ++r) acc[r] = cfnma(acc[r], ts[j * INV_RS + r], x);
-        }
-#pragma unroll
-        for (int r = 0; r < INV_RS; ++r) {
-#pragma unroll
-            for (int off = 16; off > 0; off >>= 1) {
-                acc[r].x += __shfl_xor_sync(0xffffffffu, acc[r].x, off);
-                acc[r].y += __shfl_xor_sync(0xffffffffu, acc[r].y, off);
+            for (int t = 0; t < NJ; ++t) {
+                const int c = jg + (INV_NT / INV_RS) * t;
+                if (c < q) acc[t] = cfnma(acc[t], tv, xr[c * q + j]);
             }
         }
 #pragma unroll
-        for (int r = 0; r < INV_RS; ++r)
-            if (lane == r && r < nr) O.set(i0 + r, ocol + c, acc[r]);
+        for (int t = 0; t < NJ; ++t) {
+            const int c = jg + (INV_NT / INV_RS) * t;
+            if (c < q && r < nr) O.set(i0 + r, ocol + c, acc[t]);
+        }
     }
 }
 
@@ -849,7 +849,13 @@ template <class V> static int inv_double(cudaStream_t st, V A, int c0, int h, in
     typedef typename V::elem_t E;
     V La = dinv_of(wk.dinvL, c0, h), Lb = dinv_of(wk.dinvL, c0 + h, w - h), Lo = dinv_of(wk.dinvL, c0, w);
     V Ua = dinv_of(wk.dinvU, c0, h), Ub = dinv_of(wk.dinvU, c0 + h, w - h), Uo = dinv_of(wk.dinvU, c0, w);
-    const size_t smem = 2 * (size_t)(LEAF / 2) * INV_RS * sizeof(E);  // p, q <= LEAF/2
+    constexpr int HL = LEAF / 2;  // p, q <= LEAF/2
+    const size_t smem = (2 * (size_t)HL * INV_RS + 2 * (size_t)HL * HL) * sizeof(E);
+    static bool configured = false;
+    if (!configured) {
+        HP_CUDA(cudaFuncSetAttribute(inv_double_kernel<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = true;
+    }
     ProfCat pc(PROF_OTHER);
     const bool prof = prof_enabled();
     if (prof) prof_begin(st, 0.0);
