@@ -82,7 +82,8 @@ int hprmat_mesh(const hprmat_ctx *ctx, double *r, double *fa);
  *   V    dev, complex [nbasis][nch][nch]: V[(i*nch + c2)*nch + c1] = V_{c1 c2}(r_i), MeV (Eq. 4)
  *   mode one of HPRMAT_FP64 / HPRMAT_MIXED / HPRMAT_MIXED_REFINE (must be inside max_mode)
  *   max_refine  maximum refinement steps; <0 = default (2 for FP64, 5 for MIXED_REFINE)
- *   tol  refinement stops when max|r| <= tol * max|B|; <=0 = default 1e-13
+ *   tol  refinement stops when the estimated relative error left in X (correction norm x observed contraction, DESIGN.md
+ *        reading R9) is <= tol; <=0 = default: 1e-13 in FP64 mode, 1e-12 in the mixed modes
  *   R    dev, complex nch x nch column-major (output)
  *   info host, may be NULL (then the call does not synchronise) */
 int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int max_refine, double tol, void *R,

@@ -186,7 +186,7 @@ int zsolve_mixed(cudaStream_t st, int n, int nrhs, const double2 *A, long lda, d
     w.carve(workspace, n, nrhs);
     if (max_refine < 0) max_refine = 12;  // the contraction per step is ~ sqrt(n) 2^-11 kappa(S): a few 1e-3 at best
     if (!refine) max_refine = 0;
-    if (!(tol > 0.0)) tol = 1e-13;
+    if (!(tol > 0.0)) tol = 1e-12;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     for (auto &e : ev) HP_CUDA(cudaEventCreate(&e));
     auto cleanup = [&]() { for (auto &e : ev) cudaEventDestroy(e); };

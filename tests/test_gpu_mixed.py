@@ -275,3 +275,30 @@ def test_zsolve_mixed_never_returns_a_silent_low_precision_result(kappa):
         assert info["status"] == hb.HPRMAT_ENOTCONVERGED
     if kappa <= 1e2:
         assert info["status"] == hb.HPRMAT_OK                                  # well inside the convergence domain
+
+
+# ---------------------------------------------------------------------------------------------------- headline size, mixed
+@pytest.mark.slow
+@pytest.mark.parametrize("mode,tol", [(hb.HPRMAT_MIXED_REFINE, 1e-10), (hb.HPRMAT_MIXED, 1e-3)])
+def test_rmatrix_mixed_cfg3_headline_size_certificate(mode, tol):
+    """BASELINE.json configs[3] (N = 25600) in the launch configuration bench.py times, mixed modes.  The full oracle
+    needs ~10 core-hours here, so correctness is certified a posteriori: since C = C^T,
+    R_exact - R~ = (h2m/a) X~^T (B - C X~) + O(r^2), with the residual of the GPU solution evaluated by the ORACLE in long
+    double with the matrix-free operator (for the unrefined mode the first-order term IS the error estimate)."""
+    w = make_workload(3)
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    R, info = ctx.solve(30.0, V, mode)
+    assert info["status"] == 0
+    X = _host(ctx.get_x())
+    Rg = _host(R)
+    ro = oracle.mesh(w.nb, w.a)[2]
+    res = oracle.structured_residual(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, 30.0, w.potential(ro), X)
+    est = np.abs((w.h2m / w.a) * (X.T @ res)).max() / np.abs(Rg).max()
+    assert est <= tol, (est, np.abs(res).max(), info)
+    assert _relmax(Rg, Rg.T) <= 10 * tol
+    fa = oracle.mesh(w.nb, w.a)[3]
+    for (c1, c2) in [(0, 0), (3, 200), (255, 255), (17, 4)]:                  # sampled outputs, one by one
+        assert abs(Rg[c1, c2] - (w.h2m / w.a) * np.dot(fa, X[c1 * w.nb:(c1 + 1) * w.nb, c2])) <= 1e-13 * np.abs(Rg).max()
+    ctx.destroy()
