@@ -45,6 +45,16 @@ def peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
 
 
+# DRAM traffic of the trailing-update kernels from the `ncu --set full` captures in profiles/r01_ncu_full.md (section 4,
+# after the grouped rasterisation): dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the probe shape, next to
+# the algorithmic bytes of that launch (A and B once, C read + written).
+NCU_TRAFFIC = {
+    "fp64": {"bytes": 5.778497e9 + 2.597679e9, "launch": "hprmat_zgemm m=n=12800 k=1024",
+             "algorithmic_bytes": 16.0 * (2 * 12800 * 1024 + 2 * 12800 * 12800)},
+    "tf32": {"bytes": 18.979252e9 + 1.300858e9, "launch": "hprmat_cgemm_tf32 m=n=12800 k=6400",
+             "algorithmic_bytes": 8.0 * (2 * 12800 * 6400 + 2 * 12800 * 12800)},
+}
+
 # FP64 tensor (DMMA) peak: 148 SMs x 128 FP64 flop/clk/SM x 1.965 GHz = 37.2 TFLOP/s; measured on this pool with a
 # register-resident mma.sync.m8n8k4.f64 loop: 37.15 TFLOP/s burst and sustained (profiles/r01_dmma_peak.md).  The ratio
 # to the driver's measured bf16 figure is not used because FP64 DMMA is not power-capped on this part.
@@ -198,6 +208,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--mode", default="fp64", choices=["fp64", "mixed", "mixed_refine"])
     ap.add_argument("--cfg", type=int, default=3)
+    ap.add_argument("--also", default="mixed_refine", choices=["none", "fp64", "mixed", "mixed_refine"],
+                    help="a second precision mode measured in the same run and reported under other_modes")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--probe", default=None, choices=["zgemm", "cgemm", "dmma", "panel"],
@@ -234,98 +246,113 @@ def main():
         torch.cuda.synchronize()
 
     w = make_workload(args.cfg)
-    mode = hb.MODES[args.mode]
-    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
-    r, _ = ctx.mesh()
-    V_host = torch.from_numpy(w.potential(r)).pin_memory()
-    V = V_host.to("cuda")
-    R = torch.empty((w.nch, w.nch), dtype=torch.complex128, device="cuda")
-    R_host = torch.empty((w.nch, w.nch), dtype=torch.complex128).pin_memory()
-    # rank k takes the k-th point of the config's energy scan (replicas; weak scaling)
     from paper_2512_11590_b200 import scan
-    E = scan.bench_energy(w.energies, rank)
+    E = scan.bench_energy(w.energies, rank)   # rank k takes the k-th point of the config's energy scan (replicas)
     N = w.n
 
-    for _ in range(args.warmup):
-        ctx.solve(E, V, mode, R=R)
-    # ---- timed region: K steps, device-resident inputs
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    infos = []
-    barrier()
-    sampler = ClockSampler(local) if rank == 0 else None
-    l0 = hb.hprmat_launch_count()
-    e0.record()
-    for _ in range(args.steps):
-        _, info = ctx.solve(E, V, mode, R=R)
-        infos.append(info)
-    e1.record()
-    barrier()
-    launches = hb.hprmat_launch_count() - l0
-    clocks = sampler.stop() if sampler else None
-    t_dev = e0.elapsed_time(e1) * 1e-3
-    t_max = scan.max_over_ranks(t_dev, device="cuda")
-    sec_per_step = t_max / args.steps
+    def measure(mode_name):
+        mode = hb.MODES[mode_name]
+        ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
+        r, _ = ctx.mesh()
+        V_host = torch.from_numpy(w.potential(r)).pin_memory()
+        V = V_host.to("cuda")
+        R = torch.empty((w.nch, w.nch), dtype=torch.complex128, device="cuda")
+        R_host = torch.empty((w.nch, w.nch), dtype=torch.complex128).pin_memory()
 
-    # ---- end to end: host V in, host R out, through hprmat_solve_host, copies inside the timed region
-    Vh_np, Rh_np = V_host.numpy(), R_host.numpy()
-    ctx.solve_host(E, Vh_np, mode, R_host=Rh_np)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
+        for _ in range(args.warmup):
+            ctx.solve(E, V, mode, R=R)
+        # ---- timed region: K steps, device-resident inputs
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        infos = []
+        barrier()
+        sampler = ClockSampler(local) if rank == 0 else None
+        l0 = hb.hprmat_launch_count()
+        e0.record()
+        for _ in range(args.steps):
+            _, info = ctx.solve(E, V, mode, R=R)
+            infos.append(info)
+        e1.record()
+        barrier()
+        launches = hb.hprmat_launch_count() - l0
+        clocks = sampler.stop() if sampler else None
+        t_dev = e0.elapsed_time(e1) * 1e-3
+        t_max = scan.max_over_ranks(t_dev, device="cuda")
+        sec_per_step = t_max / args.steps
+
+        # ---- end to end: host V in, host R out, through hprmat_solve_host, copies inside the timed region
+        Vh_np, Rh_np = V_host.numpy(), R_host.numpy()
         ctx.solve_host(E, Vh_np, mode, R_host=Rh_np)
-    torch.cuda.synchronize()
-    te = time.perf_counter() - t0
-    e2e_sec = scan.max_over_ranks(te, device="cuda") / args.steps
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            ctx.solve_host(E, Vh_np, mode, R_host=Rh_np)
+        torch.cuda.synchronize()
+        te = time.perf_counter() - t0
+        e2e_sec = scan.max_over_ranks(te, device="cuda") / args.steps
 
-    # ---- roofline leg: one more step with a CUDA-event pair around every GEMM launch (the trailing-update kernel)
-    roof = None
-    if rank == 0:
-        hb.hprmat_profile(True)
-        _, pinfo = ctx.solve(E, V, mode, R=R)
-        hb.hprmat_profile(False)
-        hb.hprmat_profile_read()
-        cats = {name: dict(zip(("ms", "flops", "launches"), hb.hprmat_profile_cat(i))) for i, name in enumerate(hb.PROF_CATS)}
-        g_ms, g_fl, g_n = cats["lu_gemm"]["ms"], cats["lu_gemm"]["flops"], cats["lu_gemm"]["launches"]
-        pk, how = peaks()
-        if mode == hb.HPRMAT_FP64:
-            peak, pname = FP64_TENSOR_PEAK_TFLOPS, "FP64 DMMA peak measured on this pool with a register-resident mma.sync loop"
-        else:
-            peak = 0.5 * pk["bf16_tflops_sustained"]
-            pname = f"TF32 dense = 0.5 x bf16 sustained ({how})"
-        ach = g_fl / (g_ms * 1e-3) * 1e-12 if g_ms > 0 else 0.0
-        roof = {"bound": "tensor", "kernel": ("zgemm_kernel" if mode == hb.HPRMAT_FP64 else "cgemm_tf32_kernel") +
-                " (trailing update A22 -= L21 U12 of the LU)", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                "frac": ach / peak, "traffic": None, "peak_source": pname, "launches": g_n, "kernel_ms_per_step": g_ms,
-                "share_of_step": g_ms / pinfo["ms_total"] if pinfo["ms_total"] else None,
-                "algorithmic_flops_per_step": g_fl,
-                "breakdown_ms": {k: round(v["ms"], 3) for k, v in cats.items()},
-                "breakdown_launches": {k: v["launches"] for k, v in cats.items()}}
+        # ---- roofline leg: one more step with a CUDA-event pair around every GEMM launch (the trailing-update kernel)
+        roof = None
+        if rank == 0:
+            hb.hprmat_profile(True)
+            _, pinfo = ctx.solve(E, V, mode, R=R)
+            hb.hprmat_profile(False)
+            hb.hprmat_profile_read()
+            cats = {name: dict(zip(("ms", "flops", "launches"), hb.hprmat_profile_cat(i))) for i, name in enumerate(hb.PROF_CATS)}
+            g_ms, g_fl, g_n = cats["lu_gemm"]["ms"], cats["lu_gemm"]["flops"], cats["lu_gemm"]["launches"]
+            pk, how = peaks()
+            if mode == hb.HPRMAT_FP64:
+                peak, pname = FP64_TENSOR_PEAK_TFLOPS, "FP64 DMMA peak measured on this pool with a register-resident mma.sync loop"
+            else:
+                peak = 0.5 * pk["bf16_tflops_sustained"]
+                pname = f"TF32 dense = 0.5 x bf16 sustained ({how})"
+            ach = g_fl / (g_ms * 1e-3) * 1e-12 if g_ms > 0 else 0.0
+            roof = {"bound": "tensor", "kernel": ("zgemm_kernel" if mode == hb.HPRMAT_FP64 else "cgemm_tf32_kernel") +
+                    " (trailing update A22 -= L21 U12 of the LU)", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                    "frac": ach / peak, "traffic": NCU_TRAFFIC["fp64" if mode == hb.HPRMAT_FP64 else "tf32"]["bytes"],
+                "traffic_of": NCU_TRAFFIC["fp64" if mode == hb.HPRMAT_FP64 else "tf32"], "peak_source": pname, "launches": g_n, "kernel_ms_per_step": g_ms,
+                    "share_of_step": g_ms / pinfo["ms_total"] if pinfo["ms_total"] else None,
+                    "algorithmic_flops_per_step": g_fl,
+                    "breakdown_ms": {k: round(v["ms"], 3) for k, v in cats.items()},
+                    "breakdown_launches": {k: v["launches"] for k, v in cats.items()}}
 
-    if rank == 0:
         info = infos[-1]
-        value = world * lu_flops(N) / sec_per_step * 1e-12
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": None, "dtype": "f64" if mode == hb.HPRMAT_FP64 else "tf32/f32 factors + f64 refinement",
-                "data": "synthetic",
+        res = {"mode": mode_name, "value": world * lu_flops(N) / sec_per_step * 1e-12, "ms_per_step": sec_per_step * 1e3,
+               "dtype": "f64" if mode == hb.HPRMAT_FP64 else "tf32/f32 factors + f64 refinement",
+               "time_to_rmatrix_s": sec_per_step, "lu_tflops": info["lu_tflops"],
+               "stages_ms": {k: info[k] for k in ("ms_assemble", "ms_lu", "ms_solve", "ms_refine", "ms_contract", "ms_total")},
+               "refine_steps": info["refine_steps"], "backward_err": info["backward_err"], "status": info["status"],
+               "e2e": {"value": world * lu_flops(N) / e2e_sec * 1e-12, "unit": UNIT, "seconds_per_step": e2e_sec,
+                       "h2d_bytes_per_step": int(V_host.numel() * 16), "d2h_bytes_per_step": int(R_host.numel() * 16)},
+               "gpu_launches": int(launches), "clocks": clocks, "roofline": roof}
+        ctx.destroy()
+        del V, R, ctx
+        torch.cuda.empty_cache()
+        return res
+
+    m = measure(args.mode)
+    others = {}
+    if args.also != "none" and args.also != args.mode:
+        others[args.also] = measure(args.also)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": m["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": m["dtype"], "data": "synthetic",
                 "config": {"workload": f"BASELINE.json configs[{args.cfg}]: Nc={w.nch}, Nb={w.nb}, N={N}, a={w.a} fm, "
                                        f"E={E} MeV, mode={args.mode}", "parallelism": f"replicas x{world}",
-                           "l2": "inputs_larger_than_L2 (matrix 16 N^2 B >> 126 MB)"},
-                "time_to_rmatrix_s": sec_per_step,
-                "lu_tflops": info["lu_tflops"],
-                "stages_ms": {k: info[k] for k in ("ms_assemble", "ms_lu", "ms_solve", "ms_refine", "ms_contract", "ms_total")},
-                "refine_steps": info["refine_steps"], "backward_err": info["backward_err"],
-                "e2e": {"value": world * lu_flops(N) / e2e_sec * 1e-12, "unit": UNIT, "seconds_per_step": e2e_sec,
-                        "h2d_bytes_per_step": int(V_host.numel() * 16), "d2h_bytes_per_step": int(R_host.numel() * 16)},
-                "gpu_launches": int(launches), "clocks": clocks, "roofline": roof,
-                "paper_context": {"rtx3090_fp32_s": 3.554, "rtx3090_hybrid_s": 9.85, "xeon48_zgesv_s": 52.098,
-                                  "legacy_inversion_s": 144.948, "note": "PAPER.md Tables 3-4, N=25600, other hardware"}}
+                           "l2": "inputs_larger_than_L2 (matrix 16 N^2 B >> 126 MB)"}}
+        for k in ("time_to_rmatrix_s", "lu_tflops", "stages_ms", "refine_steps", "backward_err", "e2e", "gpu_launches",
+                  "clocks", "roofline"):
+            line[k] = m[k]
+        # the metric names FP64 AND mixed: the other precision mode, measured the same way in the same run
+        line["other_modes"] = others
+        line["paper_context"] = {"rtx3090_fp32_s": 3.554, "rtx3090_hybrid_s": 9.85, "xeon48_zgesv_s": 52.098,
+                                 "legacy_inversion_s": 144.948, "note": "PAPER.md Tables 3-4, N=25600, other hardware"}
         if not args.no_cpu_baseline and world == 1:
             v, t, cores, text = oracle_sample(args.cfg, 1, 0)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text,
                                     "seconds": t}
         print(json.dumps(line))
-    ctx.destroy()
     if dist is not None:
         dist.destroy_process_group()
     return 0
