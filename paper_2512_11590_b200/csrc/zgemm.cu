@@ -129,24 +129,41 @@ __global__ void __launch_bounds__(WM *WN * 32, MINB)
     }
     cp_async_wait<0>();
 
-    // epilogue: lane holds C~[real row 8*ai + r][cols 8*bi + 2*kk + {0,1}] of the warp tile
+    // epilogue: lane holds C~[real row 8*ai + r][cols 8*bi + 2*kk + {0,1}] of the warp tile.  The old values of C are
+    // fetched in batches of 16 independent loads before the corresponding stores (a load-store-load-store chain would
+    // pay one L2 round trip per element: ~25 us per tile).
     double *Cd = reinterpret_cast<double *>(C);
 #pragma unroll
-    for (int ai = 0; ai < 8; ++ai) {
-        long crow = m0 + wm * 32 + ai * 4 + (r >> 1);
-        if (crow >= M) continue;
+    for (int ap = 0; ap < 8; ap += 2) {
+        double old[2][4][2];
+        if (beta != 0.0) {
 #pragma unroll
-        for (int bi = 0; bi < 4; ++bi) {
+            for (int a2 = 0; a2 < 2; ++a2) {
+                const long crow = m0 + wm * 32 + (ap + a2) * 4 + (r >> 1);
 #pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                long col = n0 + wn * 32 + bi * 8 + 2 * kk + e;
-                if (col < N) {
-                    double *p = Cd + (col * ldc + crow) * 2 + (r & 1);
-                    double v = alpha * acc[ai][bi][e];
-                    if (beta != 0.0) v += beta * (*p);
-                    *p = v;
-                }
+                for (int bi = 0; bi < 4; ++bi)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const long col = n0 + wn * 32 + bi * 8 + 2 * kk + e;
+                        old[a2][bi][e] = (crow < M && col < N) ? Cd[(col * ldc + crow) * 2 + (r & 1)] : 0.0;
+                    }
             }
+        }
+#pragma unroll
+        for (int a2 = 0; a2 < 2; ++a2) {
+            const long crow = m0 + wm * 32 + (ap + a2) * 4 + (r >> 1);
+            if (crow >= M) continue;
+#pragma unroll
+            for (int bi = 0; bi < 4; ++bi)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const long col = n0 + wn * 32 + bi * 8 + 2 * kk + e;
+                    if (col < N) {
+                        double v = alpha * acc[ap + a2][bi][e];
+                        if (beta != 0.0) v += beta * old[a2][bi][e];
+                        Cd[(col * ldc + crow) * 2 + (r & 1)] = v;
+                    }
+                }
         }
     }
 }
