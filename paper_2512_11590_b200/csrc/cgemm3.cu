@@ -60,8 +60,15 @@ constexpr size_t C3_SMEM = (size_t)C3_STAGES * C3_STAGE * sizeof(float);
 
 __global__ void __launch_bounds__(C3_NT, 1)
     cgemm3_kernel(int M, int N, int K, float alpha, const float *__restrict__ Are, const float *__restrict__ Aim, long lda,
-                  const float *Bre, const float *Bim, long ldb, float beta, float *Cre, float *Cim, long ldc) {
+                  const float *Bre, const float *Bim, long ldb, float beta, float *Cre, float *Cim, long ldc, long strideA,
+                  long strideB, long strideC) {
     extern __shared__ __align__(16) float sm3[];
+    Are += (long)blockIdx.y * strideA;
+    Aim += (long)blockIdx.y * strideA;
+    Bre += (long)blockIdx.y * strideB;
+    Bim += (long)blockIdx.y * strideB;
+    Cre += (long)blockIdx.y * strideC;
+    Cim += (long)blockIdx.y * strideC;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int wm = warp % C3_WM, wn = warp / C3_WM;
     const int g = lane >> 2, t = lane & 3;
@@ -185,19 +192,25 @@ __global__ void __launch_bounds__(C3_NT, 1)
 // C <- beta*C + alpha*A*B on split-complex float planes, 3xTF32.  Plane base addresses 16-byte aligned, lda and ldb
 // multiples of 4 floats (met by every caller in lu.cu).
 int cgemm3(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C) {
-    if (m <= 0 || n <= 0) return 0;
+    return cgemm3_batched(st, m, n, k, alpha, A, 0, B, 0, beta, C, 0, 1);
+}
+
+// nbatch independent products; operand b of batch i lives at view + i * stride (in elements of a plane)
+int cgemm3_batched(cudaStream_t st, int m, int n, int k, double alpha, CView A, long strideA, CView B, long strideB, double beta,
+                   CView C, long strideC, int nbatch) {
+    if (m <= 0 || n <= 0 || nbatch <= 0) return 0;
     if (k <= 0 && beta == 1.0) return 0;
     if (((uintptr_t)A.re | (uintptr_t)A.im | (uintptr_t)B.re | (uintptr_t)B.im) & 15) return -6;
-    if ((A.ld | B.ld) & 3) return -7;
+    if ((A.ld | B.ld | strideA | strideB) & 3) return -7;
     static bool configured = false;
     if (!configured) {
         HP_CUDA(cudaFuncSetAttribute(cgemm3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C3_SMEM));
         configured = true;
     }
     const bool prof = prof_enabled() && k > 0;
-    if (prof) prof_begin(st, 8.0 * m * n * k);
-    cgemm3_kernel<<<ceil_div(m, C3_BM) * ceil_div(n, C3_BN), C3_NT, C3_SMEM, st>>>(m, n, k, (float)alpha, A.re, A.im, A.ld, B.re,
-                                                                                 B.im, B.ld, (float)beta, C.re, C.im, C.ld);
+    if (prof) prof_begin(st, 8.0 * m * n * k * nbatch);
+    cgemm3_kernel<<<dim3(ceil_div(m, C3_BM) * ceil_div(n, C3_BN), nbatch), C3_NT, C3_SMEM, st>>>(
+        m, n, k, (float)alpha, A.re, A.im, A.ld, B.re, B.im, B.ld, (float)beta, C.re, C.im, C.ld, strideA, strideB, strideC);
     if (prof) prof_end(st);
     HP_LAUNCHED();
     return 0;

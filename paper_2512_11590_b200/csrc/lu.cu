@@ -12,6 +12,8 @@
 //   applied to ALL other columns of the matrix by a gather/scatter kernel (independent loads, no swap chain).
 #include "lu.cuh"
 
+#include <algorithm>
+
 #include <cooperative_groups.h>
 
 namespace hp {
@@ -53,6 +55,12 @@ template <class V> size_t LuWork<V>::carve(void *base, int n_) {
         const long sz = (long)IB << lev;
         dinvL[lev] = alloc_view<V>(p, sz, (long)ceil_div(n, sz) * sz);
         dinvU[lev] = alloc_view<V>(p, sz, (long)ceil_div(n, sz) * sz);
+    }
+    sbld = std::min<long>(SB, round_up(std::max(n, 1), 32));
+    if (n > LEAF) {
+        binvL = alloc_view<V>(p, sbld, (long)ceil_div(n, SB) * sbld);
+        binvU = alloc_view<V>(p, sbld, (long)ceil_div(n, SB) * sbld);
+        tmp = alloc_view<V>(p, sbld, std::max<long>(n, 256));
     }
     perm = (int *)take(sizeof(int) * (size_t)nblk * PERM_STRIDE);
     cand_val = (T *)take(sizeof(T) * 2 * MAXG);
@@ -825,8 +833,10 @@ __global__ void __launch_bounds__(INV_NT) inv_double_kernel(V A, int h, int w, V
 
 // ------------------------------------------------------------------------------------------------- host recursion
 // Column split of a node of width w: below LEAF the tree is binary on power-of-two multiples of IB, so that every left
-// child is a full block of its size class (its inverse is kept, see LuWork); above, splits fall on multiples of LEAF.
+// child is a full block of its size class (its inverse is kept, see LuWork); above, splits fall on multiples of LEAF, and
+// above SB on multiples of SB, so that every SB-aligned block is a node of the recursion (its full inverse is kept too).
 static inline int split(int w) {
+    if (w > SB) return (int)round_up((w + 1) / 2, SB);
     if (w > LEAF) return (int)round_up((w + 1) / 2, LEAF);
     int h = IB;
     while (2 * h < w) h *= 2;
@@ -932,6 +942,74 @@ template <class V> static int panel(cudaStream_t st, int n, V A, int c0, int w, 
     return laswp(st, A, 0, c0, c0 + w, n, wk.perm, blk, blk + 1);
 }
 
+// ---- helpers of the SB-block ("big leaf") level -------------------------------------------------------------------------
+template <class V> __global__ void __launch_bounds__(256) set_identity_kernel(V X, int s) {
+    typedef typename V::real_t T;
+    const long idx = (long)blockIdx.x * 256 + threadIdx.x;
+    if (idx >= (long)s * s) return;
+    const int i = (int)(idx % s), j = (int)(idx / s);
+    X.set(i, j, mk((T)(i == j ? 1 : 0), (T)0));
+}
+template <class V> __global__ void __launch_bounds__(256) copy_block_kernel(V Src, V Dst, int rows, long cols) {
+    const long idx = (long)blockIdx.x * 256 + threadIdx.x;
+    if (idx >= (long)rows * cols) return;
+    const int i = (int)(idx % rows);
+    const long j = idx / rows;
+    Dst.set(i, j, Src.get(i, j));
+}
+// zero the LEAF x LEAF diagonal blocks of the s x s matrix X
+template <class V> __global__ void __launch_bounds__(256) strip_diag_kernel(V X, int s) {
+    typedef typename V::real_t T;
+    const long idx = (long)blockIdx.x * 256 + threadIdx.x;
+    if (idx >= (long)s * LEAF) return;
+    const int i = (int)(idx % s), jj = (int)(idx / s);  // jj: column inside the diagonal block of row i
+    const int j = (i / LEAF) * LEAF + jj;
+    if (j < s) X.set(i, j, mk((T)0, (T)0));
+}
+template <class V> static int copy_block(cudaStream_t st, V Src, V Dst, int rows, long cols) {
+    if (rows <= 0 || cols <= 0) return 0;
+    copy_block_kernel<V><<<ceil_div((long)rows * cols, 256), 256, 0, st>>>(Src, Dst, rows, cols);
+    HP_LAUNCHED();
+    return 0;
+}
+// does the SB-aligned block starting at d0 have a kept full inverse, and is [d0, d0 + s) exactly that block?
+static inline bool is_big_block(int n, int d0, int s) { return d0 % SB == 0 && s > LEAF && s == std::min(SB, n - d0); }
+template <class V> static V binv_of(const V &tab, long sbld, int d0) { return tab.sub(0, (long)(d0 / SB) * sbld); }
+
+// the (batched) 3xTF32 product with the LEAF-diagonal blocks of an SB block, complex64 type only
+static int diag_blocks_product(cudaStream_t, const ZView *, int, int, ZView, int, ZView) { return 0; }
+static int diag_blocks_product(cudaStream_t st, const CView *dtab, int d0, int s, CView B, int ncols, CView T) {
+    const int nfull = s / LEAF, rag = s - nfull * LEAF;
+    const CView D = dtab[NLEV - 1].sub(0, (long)(d0 / LEAF) * LEAF);  // blocks contiguous: stride LEAF*LEAF
+    if (nfull > 0)
+        HP_TRY(cgemm3_batched(st, LEAF, ncols, LEAF, 1.0, D, (long)LEAF * LEAF, B, LEAF, 0.0, T, LEAF, nfull));
+    if (rag > 0)
+        HP_TRY(cgemm3(st, rag, ncols, rag, 1.0, dinv_of(dtab, d0 + nfull * LEAF, rag), B.sub(nfull * LEAF, 0), 0.0,
+                      T.sub(nfull * LEAF, 0)));
+    return 0;
+}
+template <class V> struct IsPlanar { static constexpr bool value = false; };
+template <> struct IsPlanar<CView> { static constexpr bool value = true; };
+
+// B <- inv * B for an SB block: out of place into the scratch, then copied back.  acc (complex64 solves): the kept inverse
+// has its LEAF-diagonal blocks zeroed; those are applied from the dinv table with the 3xTF32 kernel.
+template <class V>
+static int big_leaf(cudaStream_t st, const V &binv, const V *dtab, int d0, int s, V B, int ncols, LuWork<V> &wk, bool acc) {
+    const long cap = std::max<long>(wk.n, 256);
+    for (long c = 0; c < ncols; c += cap) {
+        const int nc = (int)std::min<long>(cap, ncols - c);
+        V Bc = B.sub(0, c), T = wk.tmp;
+        if (acc && IsPlanar<V>::value) {
+            HP_TRY(diag_blocks_product(st, dtab, d0, s, Bc, nc, T));
+            HP_TRY(gemm(st, s, nc, s, 1.0, binv_of(binv, wk.sbld, d0), Bc, 1.0, T));
+        } else {
+            HP_TRY(gemm(st, s, nc, s, 1.0, binv_of(binv, wk.sbld, d0), Bc, 0.0, T));
+        }
+        HP_TRY(copy_block(st, T, Bc, s, nc));
+    }
+    return 0;
+}
+
 // Leaf product of the triangular solves (inverted diagonal block times the right-hand sides): acc = FP32-class accuracy
 // for the complex64 type (3xTF32).  The diagonal blocks are O(1) (their rounding to 10 mantissa bits would cap the solve
 // at ~1e-3); the off-diagonal updates B2 -= L21 X1 stay single-pass like the trailing update of the factorisation, their
@@ -948,6 +1026,7 @@ static int gemm_sel(bool acc, cudaStream_t st, int m, int n, int k, double alpha
 template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk, bool acc = false) {
     if (s <= 0 || ncols <= 0) return 0;
     if (s <= LEAF) return gemm_sel(acc, st, s, ncols, s, 1.0, dinv_of(wk.dinvL, d0, s), B, 0.0, B);
+    if (wk.use_big && is_big_block(wk.n, d0, s)) return big_leaf(st, wk.binvL, wk.dinvL, d0, s, B, ncols, wk, acc);
     const int h = split(s);
     HP_TRY(trsm_lower(st, A, d0, h, B, ncols, wk, acc));
     HP_TRY(gemm(st, s - h, ncols, h, -1.0, A.sub(d0 + h, d0), B, 1.0, B.sub(h, 0)));
@@ -958,10 +1037,28 @@ template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V 
 template <class V> static int trsm_upper(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk, bool acc = false) {
     if (s <= 0 || ncols <= 0) return 0;
     if (s <= LEAF) return gemm_sel(acc, st, s, ncols, s, 1.0, dinv_of(wk.dinvU, d0, s), B, 0.0, B);
+    if (wk.use_big && is_big_block(wk.n, d0, s)) return big_leaf(st, wk.binvU, wk.dinvU, d0, s, B, ncols, wk, acc);
     const int h = split(s);
     HP_TRY(trsm_upper(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk, acc));
     HP_TRY(gemm(st, h, ncols, s - h, -1.0, A.sub(d0, d0 + h), B.sub(h, 0), 1.0, B));
     return trsm_upper(st, A, d0, h, B, ncols, wk, acc);
+}
+
+// Full inverses of the unit-lower and upper triangles of the SB block [c0, c0 + s): triangular solves on the identity with
+// the LEAF-level recursion (the block's own big leaf does not exist yet).
+template <class V> static int build_binv(cudaStream_t st, V A, int c0, int s, LuWork<V> &wk) {
+    ProfCat pc(PROF_OTHER);
+    V XL = binv_of(wk.binvL, wk.sbld, c0), XU = binv_of(wk.binvU, wk.sbld, c0);
+    set_identity_kernel<V><<<ceil_div((long)s * s, 256), 256, 0, st>>>(XL, s);
+    HP_LAUNCHED();
+    set_identity_kernel<V><<<ceil_div((long)s * s, 256), 256, 0, st>>>(XU, s);
+    HP_LAUNCHED();
+    const bool was = wk.use_big;
+    wk.use_big = false;
+    int rc = trsm_lower(st, A, c0, s, XL, s, wk, false);
+    if (rc == 0) rc = trsm_upper(st, A, c0, s, XU, s, wk, false);
+    wk.use_big = was;
+    return rc;
 }
 
 template <class V> static int getrf_rec(cudaStream_t st, int n, V A, int c0, int c1, int *ipiv, int *info_dev, LuWork<V> &wk) {
@@ -980,6 +1077,7 @@ template <class V> static int getrf_rec(cudaStream_t st, int n, V A, int c0, int
     HP_TRY(getrf_rec(st, n, A, mid, c1, ipiv, info_dev, wk));
     // the node's diagonal block is final: keep its inverse for the triangular solves further up / in getrs
     if (w <= LEAF) HP_TRY(inv_double(st, A, c0, h, w, wk));
+    if (is_big_block(n, c0, w)) HP_TRY(build_binv(st, A, c0, w, wk));
     return 0;
 }
 
@@ -989,12 +1087,27 @@ template <class V> int getrf(cudaStream_t st, int n, V A, int *ipiv, int *info_d
     HP_CUDA(cudaMemsetAsync(wk.slots, 0, sizeof(unsigned long long) * LL_WORDS, st));
     wk.bar_base = 0;
     wk.ep_base = 0;
-    return getrf_rec(st, n, A, 0, n, ipiv, info_dev, wk);
+    wk.use_big = true;
+    HP_TRY(getrf_rec(st, n, A, 0, n, ipiv, info_dev, wk));
+    if (IsPlanar<V>::value && n > LEAF) {
+        // the solves apply the LEAF-diagonal blocks of the kept inverses separately, with FP32-class products
+        ProfCat pc(PROF_OTHER);
+        for (int d0 = 0; d0 < n; d0 += SB) {
+            const int sblk = std::min(SB, n - d0);
+            if (sblk <= LEAF) continue;
+            strip_diag_kernel<V><<<ceil_div((long)sblk * LEAF, 256), 256, 0, st>>>(binv_of(wk.binvL, wk.sbld, d0), sblk);
+            HP_LAUNCHED();
+            strip_diag_kernel<V><<<ceil_div((long)sblk * LEAF, 256), 256, 0, st>>>(binv_of(wk.binvU, wk.sbld, d0), sblk);
+            HP_LAUNCHED();
+        }
+    }
+    return 0;
 }
 
 template <class V> int getrs(cudaStream_t st, int n, int nrhs, V A, V B, LuWork<V> &wk) {
     if (n <= 0 || nrhs <= 0) return 0;
     ProfCat pc(PROF_SOLVE);
+    wk.use_big = true;
     HP_TRY(laswp(st, B, 0, nrhs, 0, 0, wk.perm, 0, wk.nblk));
     // the right-hand sides and the solution are O(1): FP32-class diagonal-block products (3xTF32 for the complex64 type)
     HP_TRY(trsm_lower(st, A, 0, n, B, nrhs, wk, true));

@@ -8,6 +8,8 @@ constexpr int IB = 32;        // panel width = swap batch = smallest inverted di
 constexpr int LEAF = 128;     // largest inverted diagonal block = leaf of the triangular-solve recursion (one GEMM M tile,
                               // so that the leaf product B <- inv * B may run in place)
 constexpr int NLEV = 3;       // inverted diagonal blocks are kept at sizes IB << lev, lev = 0 .. NLEV-1
+constexpr int SB = 1024;      // "solve block": the full inverses of the SB x SB diagonal blocks of L and U are kept as well, so
+                              // that a triangular solve is N/SB dependent steps of large dense GEMMs instead of N/LEAF
 constexpr int MAXG = kNumSMs; // CTAs of the cooperative panel kernel (one per SM)
 
 // GEMM back-ends (zgemm.cu / cgemm.cu): C <- beta*C + alpha*A*B.  nbatch > 1: operand b lives at view + b*stride
@@ -16,6 +18,8 @@ int gemm(cudaStream_t st, int m, int n, int k, double alpha, ZView A, ZView B, d
 int gemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
 // FP32-class accuracy variant for the planar complex64 type (3xTF32, cgemm3.cu); C may alias B when m <= 128, beta == 0
 int cgemm3(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
+int cgemm3_batched(cudaStream_t st, int m, int n, int k, double alpha, CView A, long strideA, CView B, long strideB, double beta,
+                   CView C, long strideC, int nbatch);
 int zgemm_batched(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda, long strideA,
                   const double2 *B, long ldb, long strideB, double beta, double2 *C, long ldc, long strideC, int nbatch);
 
@@ -26,6 +30,12 @@ template <class V> struct LuWork {
     int n = 0, nblk = 0;
     V dinvL[NLEV], dinvU[NLEV];  // level lev: blocks of s x s, s = IB << lev, block b at column offset b*s, ld = s:
                                  // inverses of the unit-lower / upper triangle of the diagonal block at (b*s, b*s)
+    V binvL, binvU;      // inverses of the SB-aligned diagonal blocks (of size min(SB, n - b SB) > LEAF), ld = sbld, block b at
+                         // column offset b*sbld; for the complex64 type getrf leaves their LEAF-diagonal blocks zeroed
+                         // (the solves apply those from dinvL/dinvU[NLEV-1] with the 3xTF32 kernel)
+    V tmp;               // sbld x max(n, 256) scratch: out-of-place leaf product
+    long sbld = 0;
+    bool use_big = true; // host-side switch: off while an SB inverse is being built from the LEAF-level recursion
     int *perm = nullptr; // nblk x (1 + 4*IB): count, dst rows[2*IB], src rows[2*IB]  (net permutation of each swap batch)
     T *cand_val = nullptr;
     int *cand_row = nullptr;
