@@ -1026,7 +1026,8 @@ static int gemm_sel(bool acc, cudaStream_t st, int m, int n, int k, double alpha
 template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk, bool acc = false) {
     if (s <= 0 || ncols <= 0) return 0;
     if (s <= LEAF) return gemm_sel(acc, st, s, ncols, s, 1.0, dinv_of(wk.dinvL, d0, s), B, 0.0, B);
-    if (wk.use_big && is_big_block(wk.n, d0, s)) return big_leaf(st, wk.binvL, wk.dinvL, d0, s, B, ncols, wk, acc);
+    if (wk.use_big && (acc || IsPlanar<V>::value) && is_big_block(wk.n, d0, s))
+        return big_leaf(st, wk.binvL, wk.dinvL, d0, s, B, ncols, wk, acc);
     const int h = split(s);
     HP_TRY(trsm_lower(st, A, d0, h, B, ncols, wk, acc));
     HP_TRY(gemm(st, s - h, ncols, h, -1.0, A.sub(d0 + h, d0), B, 1.0, B.sub(h, 0)));
@@ -1037,7 +1038,8 @@ template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V 
 template <class V> static int trsm_upper(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk, bool acc = false) {
     if (s <= 0 || ncols <= 0) return 0;
     if (s <= LEAF) return gemm_sel(acc, st, s, ncols, s, 1.0, dinv_of(wk.dinvU, d0, s), B, 0.0, B);
-    if (wk.use_big && is_big_block(wk.n, d0, s)) return big_leaf(st, wk.binvU, wk.dinvU, d0, s, B, ncols, wk, acc);
+    if (wk.use_big && (acc || IsPlanar<V>::value) && is_big_block(wk.n, d0, s))
+        return big_leaf(st, wk.binvU, wk.dinvU, d0, s, B, ncols, wk, acc);
     const int h = split(s);
     HP_TRY(trsm_upper(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk, acc));
     HP_TRY(gemm(st, h, ncols, s - h, -1.0, A.sub(d0, d0 + h), B.sub(h, 0), 1.0, B));
@@ -1046,18 +1048,41 @@ template <class V> static int trsm_upper(cudaStream_t st, V A, int d0, int s, V 
 
 // Full inverses of the unit-lower and upper triangles of the SB block [c0, c0 + s): triangular solves on the identity with
 // the LEAF-level recursion (the block's own big leaf does not exist yet).
+// What the factorisation itself does not need (for complex128 both inverses: its U12 solves keep the LEAF-level recursion,
+// whose GEMMs run at full FP64 rate; for complex64 the upper one) is built on a side stream, under the rest of the LU.
+static cudaStream_t side_stream() {
+    static cudaStream_t s = nullptr;
+    if (!s && cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking) != cudaSuccess) s = nullptr;
+    return s;
+}
+// `to` waits for everything enqueued on `from` so far
+static int stream_follow(cudaStream_t from, cudaStream_t to) {
+    cudaEvent_t e;
+    HP_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    cudaError_t r1 = cudaEventRecord(e, from), r2 = cudaStreamWaitEvent(to, e, 0);
+    cudaEventDestroy(e);
+    HP_CUDA(r1);
+    HP_CUDA(r2);
+    return 0;
+}
+
 template <class V> static int build_binv(cudaStream_t st, V A, int c0, int s, LuWork<V> &wk) {
     ProfCat pc(PROF_OTHER);
     V XL = binv_of(wk.binvL, wk.sbld, c0), XU = binv_of(wk.binvU, wk.sbld, c0);
-    set_identity_kernel<V><<<ceil_div((long)s * s, 256), 256, 0, st>>>(XL, s);
+    cudaStream_t sd = side_stream();
+    if (!sd) sd = st;
+    if (sd != st) HP_TRY(stream_follow(st, sd));
+    cudaStream_t stl = IsPlanar<V>::value ? st : sd;  // the complex64 LU uses the lower inverse right away
+    set_identity_kernel<V><<<ceil_div((long)s * s, 256), 256, 0, stl>>>(XL, s);
     HP_LAUNCHED();
-    set_identity_kernel<V><<<ceil_div((long)s * s, 256), 256, 0, st>>>(XU, s);
+    set_identity_kernel<V><<<ceil_div((long)s * s, 256), 256, 0, sd>>>(XU, s);
     HP_LAUNCHED();
     const bool was = wk.use_big;
     wk.use_big = false;
-    int rc = trsm_lower(st, A, c0, s, XL, s, wk, false);
-    if (rc == 0) rc = trsm_upper(st, A, c0, s, XU, s, wk, false);
+    int rc = trsm_lower(stl, A, c0, s, XL, s, wk, false);
+    if (rc == 0) rc = trsm_upper(sd, A, c0, s, XU, s, wk, false);
     wk.use_big = was;
+    wk.side_used = (sd != st);
     return rc;
 }
 
@@ -1088,7 +1113,9 @@ template <class V> int getrf(cudaStream_t st, int n, V A, int *ipiv, int *info_d
     wk.bar_base = 0;
     wk.ep_base = 0;
     wk.use_big = true;
+    wk.side_used = false;
     HP_TRY(getrf_rec(st, n, A, 0, n, ipiv, info_dev, wk));
+    if (wk.side_used) HP_TRY(stream_follow(side_stream(), st));  // join: the kept inverses are complete
     if (IsPlanar<V>::value && n > LEAF) {
         // the solves apply the LEAF-diagonal blocks of the kept inverses separately, with FP32-class products
         ProfCat pc(PROF_OTHER);
