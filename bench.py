@@ -208,6 +208,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--mode", default="fp64", choices=["fp64", "mixed", "mixed_refine"])
     ap.add_argument("--cfg", type=int, default=3)
+    ap.add_argument("--zsolve", action="store_true",
+                    help="also time hprmat_zsolve alone on a dense random N x N system (raw solve, separately from assembly "
+                         "and contraction)")
     ap.add_argument("--also", default="mixed_refine", choices=["none", "fp64", "mixed", "mixed_refine"],
                     help="a second precision mode measured in the same run and reported under other_modes")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -329,6 +332,31 @@ def main():
         torch.cuda.empty_cache()
         return res
 
+    def raw_zsolve(mode_name):
+        """hprmat_zsolve alone (no assembly, no contraction) on a dense random diagonally shifted N x N system with Nc
+        right-hand sides, x_exact = 1 -- the analogue of the paper's Table 3/4 matrices."""
+        mode = hb.MODES[mode_name]
+        g = torch.Generator(device="cuda").manual_seed(251211590)
+        A = torch.empty((N, N), dtype=torch.complex128, device="cuda")            # memory = column-major N x N
+        Ar = torch.view_as_real(A)
+        Ar.uniform_(-1.0, 1.0, generator=g)
+        A.diagonal().add_(float(N) ** 0.5)
+        B = A.sum(dim=0, keepdim=True).expand(w.nch, N).contiguous()              # column-major N x Nc: B = A @ ones
+        A0 = A.clone() if mode == hb.HPRMAT_FP64 else None
+        out = None
+        for it in range(2):                                                        # one warm-up, one timed
+            if mode == hb.HPRMAT_FP64 and it:
+                A.copy_(A0)
+            Bx = B.clone()
+            _, info = hb.hprmat_zsolve(N, w.nch, A, N, Bx, N, mode=mode, allow=(hb.HPRMAT_OK, hb.HPRMAT_ENOTCONVERGED))
+            out = {"n": N, "nrhs": w.nch, "mode": mode_name, "status": info["status"], "ms_lu": info["ms_lu"],
+                   "ms_solve": info["ms_solve"], "ms_refine": info["ms_refine"], "ms_total": info["ms_total"],
+                   "lu_tflops": info["lu_tflops"], "refine_steps": info["refine_steps"],
+                   "max_abs_error_vs_x_exact": float((Bx - 1.0).abs().max().item())}
+        del A, A0, B, Bx
+        torch.cuda.empty_cache()
+        return out
+
     m = measure(args.mode)
     others = {}
     if args.also != "none" and args.also != args.mode:
@@ -346,6 +374,8 @@ def main():
             line[k] = m[k]
         # the metric names FP64 AND mixed: the other precision mode, measured the same way in the same run
         line["other_modes"] = others
+        if args.zsolve and world == 1:
+            line["raw_zsolve"] = [raw_zsolve("fp64"), raw_zsolve("mixed_refine")]
         line["paper_context"] = {"rtx3090_fp32_s": 3.554, "rtx3090_hybrid_s": 9.85, "xeon48_zgesv_s": 52.098,
                                  "legacy_inversion_s": 144.948, "note": "PAPER.md Tables 3-4, N=25600, other hardware"}
         if not args.no_cpu_baseline and world == 1:

@@ -33,7 +33,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() {
 }
 
 __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                  : "+d"(c0), "+d"(c1)
                  : "d"(a), "d"(b));
 }
@@ -110,21 +110,26 @@ __global__ void __launch_bounds__(WM *WN * 32, MINB)
         const int slot = kt % STAGES;
         const double *a_s = reinterpret_cast<const double *>(sA + slot * A_STAGE) + a_off0;
         const double *b_s = reinterpret_cast<const double *>(sB + slot * B_STAGE) + b_off0;
-#pragma unroll
-        for (int ks = 0; ks < KC / 2; ++ks) {
-            double af[8], bf[4];
+        // fragments of k-step ks + 1 are fetched (and the A signs applied) before the MMAs of k-step ks are issued
+        double af[2][8], bf[2][4];
+        auto load_frags = [&](int ks, int buf) {
 #pragma unroll
             for (int ai = 0; ai < 8; ++ai) {
                 double v = a_s[ks * (2 * LDA_S * 2) + ai * 8];
                 int hi = __double2hiint(v) ^ (int)sign_hi;
-                af[ai] = __hiloint2double(hi, __double2loint(v));
+                af[buf][ai] = __hiloint2double(hi, __double2loint(v));
             }
 #pragma unroll
-            for (int bi = 0; bi < 4; ++bi) bf[bi] = b_s[ks * 4 + bi * (8 * LDB_S * 2)];
+            for (int bi = 0; bi < 4; ++bi) bf[buf][bi] = b_s[ks * 4 + bi * (8 * LDB_S * 2)];
+        };
+        load_frags(0, 0);
+#pragma unroll
+        for (int ks = 0; ks < KC / 2; ++ks) {
+            if (ks + 1 < KC / 2) load_frags(ks + 1, (ks + 1) & 1);
 #pragma unroll
             for (int ai = 0; ai < 8; ++ai)
 #pragma unroll
-                for (int bi = 0; bi < 4; ++bi) dmma884(acc[ai][bi][0], acc[ai][bi][1], af[ai], bf[bi]);
+                for (int bi = 0; bi < 4; ++bi) dmma884(acc[ai][bi][0], acc[ai][bi][1], af[ks & 1][ai], bf[ks & 1][bi]);
         }
     }
     cp_async_wait<0>();
