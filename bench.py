@@ -315,6 +315,9 @@ def main():
                 "traffic_of": NCU_TRAFFIC["fp64" if mode == hb.HPRMAT_FP64 else "tf32"], "peak_source": pname, "launches": g_n, "kernel_ms_per_step": g_ms,
                     "share_of_step": g_ms / pinfo["ms_total"] if pinfo["ms_total"] else None,
                     "algorithmic_flops_per_step": g_fl,
+                "frac_of_other_peaks": ({"nominal_fp64_tensor_40": ach / 40.0} if mode == hb.HPRMAT_FP64 else
+                                        {"tf32_burst_0.5x_bf16_burst": ach / (0.5 * pk["bf16_tflops"]),
+                                         "tf32_nominal_1125": ach / 1125.0}),
                     "breakdown_ms": {k: round(v["ms"], 3) for k, v in cats.items()},
                     "breakdown_launches": {k: v["launches"] for k, v in cats.items()}}
 
