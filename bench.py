@@ -45,13 +45,13 @@ def peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
 
 
-# DRAM traffic of the trailing-update kernels from the `ncu --set full` captures in profiles/r01_ncu_full.md (section 4,
-# after the grouped rasterisation): dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the probe shape, next to
+# DRAM traffic of the trailing-update kernels from the `ncu --set full` captures in profiles/r01_ncu_full.md (section 5,
+# final kernels of the round): dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the probe shape, next to
 # the algorithmic bytes of that launch (A and B once, C read + written).
 NCU_TRAFFIC = {
-    "fp64": {"bytes": 5.778497e9 + 2.597679e9, "launch": "hprmat_zgemm m=n=12800 k=1024",
+    "fp64": {"bytes": 5.805085e9 + 2.600317e9, "launch": "hprmat_zgemm m=n=12800 k=1024",
              "algorithmic_bytes": 16.0 * (2 * 12800 * 1024 + 2 * 12800 * 12800)},
-    "tf32": {"bytes": 18.979252e9 + 1.300858e9, "launch": "hprmat_cgemm_tf32 m=n=12800 k=6400",
+    "tf32": {"bytes": 10.820277e9 + 1.285462e9, "launch": "hprmat_cgemm_tf32 m=n=12800 k=6400 (128 x 256 tiles)",
              "algorithmic_bytes": 8.0 * (2 * 12800 * 6400 + 2 * 12800 * 12800)},
 }
 

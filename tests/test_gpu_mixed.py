@@ -279,13 +279,14 @@ def test_zsolve_mixed_never_returns_a_silent_low_precision_result(kappa):
 
 # ---------------------------------------------------------------------------------------------------- headline size, mixed
 @pytest.mark.slow
-@pytest.mark.parametrize("mode,tol", [(hb.HPRMAT_MIXED_REFINE, 1e-10), (hb.HPRMAT_MIXED, 1e-3)])
-def test_rmatrix_mixed_cfg3_headline_size_certificate(mode, tol):
+@pytest.mark.parametrize("cfg,mode,tol", [(3, hb.HPRMAT_MIXED_REFINE, 1e-10), (3, hb.HPRMAT_MIXED, 1e-3),
+                                          (4, hb.HPRMAT_MIXED_REFINE, 1e-10)])
+def test_rmatrix_mixed_cfg3_headline_size_certificate(cfg, mode, tol):
     """BASELINE.json configs[3] (N = 25600) in the launch configuration bench.py times, mixed modes.  The full oracle
     needs ~10 core-hours here, so correctness is certified a posteriori: since C = C^T,
     R_exact - R~ = (h2m/a) X~^T (B - C X~) + O(r^2), with the residual of the GPU solution evaluated by the ORACLE in long
     double with the matrix-free operator (for the unrefined mode the first-order term IS the error estimate)."""
-    w = make_workload(3)
+    w = make_workload(cfg)
     ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
     r, _ = ctx.mesh()
     V = torch.from_numpy(w.potential(r)).to(DEV)

@@ -200,10 +200,13 @@ def _certificate(w, E, X, R):
 
 
 @pytest.mark.slow
-def test_rmatrix_fp64_cfg3_headline_size_certificate():
-    """BASELINE.json configs[3] (N = 25600) in the launch configuration bench.py times.  The full oracle needs ~10
-    core-hours here, so correctness is certified from the oracle's long-double residual of the GPU solution."""
-    w = make_workload(3)
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_rmatrix_fp64_cfg3_headline_size_certificate(cfg):
+    """BASELINE.json configs[3] (N = 25600) in the launch configuration bench.py times, and configs[4] (N = 51200: the 42 GB
+    matrix in core; its first panels are taller than the register-resident kernel holds, so the shared-memory panel
+    kernel runs too).  The full oracle needs ~10 / ~80 core-hours here, so correctness is certified from the oracle's
+    long-double residual of the GPU solution."""
+    w = make_workload(cfg)
     ctx = _ctx(w, 1 << hb.HPRMAT_FP64)
     r, _ = ctx.mesh()
     V = torch.from_numpy(w.potential(r)).to(DEV)
