@@ -133,6 +133,12 @@ int hprmat_zgetrs(void *cuda_stream, int n, int nrhs, const void *A, int lda, co
 int hprmat_zgemm(void *cuda_stream, int m, int n, int k, double alpha, const void *A, int lda, const void *B, int ldb,
                  double beta, void *C, int ldc);
 
+/* Real decomposition of the complex128 product inside hprmat_zgemm and the FP64 LU: 4 = four real products per complex
+ * product ("4M", componentwise accurate), 3 = three ("3M": 25 % fewer tensor-core instructions, imaginary part normwise
+ * accurate; the default, chosen by measurement).  Any other value only queries.  Returns the
+ * setting in force.  Process-wide; not thread-safe against concurrent solves. */
+int hprmat_zgemm_algo(int algo);
+
 /* C <- beta*C + alpha*A*B on SPLIT-complex (planar) complex64 operands: every matrix is a pair of column-major float
  * planes (re, im).  The tcgen05 (kind::tf32, FP32 accumulation in TMEM) kernel that performs the trailing update of the
  * low-precision LU of the mixed modes.  All pointers dev; plane base addresses 16-byte

@@ -208,6 +208,11 @@ def hprmat_zgemm(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, stream=None):
     _check(rc, "hprmat_zgemm")
 
 
+def hprmat_zgemm_algo(algo: int = 0) -> int:
+    """Select (3 or 4) or query (anything else) the real decomposition of the complex128 GEMM."""
+    return int(lib().hprmat_zgemm_algo(C.c_int(algo)))
+
+
 def hprmat_cgemm_tf32(m, n, k, alpha, A_re, A_im, lda, B_re, B_im, ldb, beta, C_re, C_im, ldc, stream=None):
     """Planar complex64 GEMM on the tcgen05 TF32 tensor cores; all operands torch float32 CUDA tensors (column-major)."""
     rc = lib().hprmat_cgemm_tf32(_stream(stream), C.c_int(m), C.c_int(n), C.c_int(k), C.c_float(alpha), _dev(A_re),

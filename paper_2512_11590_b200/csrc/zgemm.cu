@@ -191,11 +191,21 @@ static int launch_zgemm(cudaStream_t st, int m, int n, int k, double alpha, cons
     return 0;
 }
 
+// 3M variant (zgemm3m.cu) and the switch between the two decompositions (hprmat_zgemm_algo)
+int zgemm3m(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda, long strideA, const double2 *B,
+            long ldb, long strideB, double beta, double2 *C, long ldc, long strideC, int nbatch);
+int g_zgemm_algo = 3;
+// the 3M kernel has several M tiles per column strip (C must not alias B) and 64-column tiles
+static inline bool use_3m(int n, int k, const double2 *B, const double2 *C) {
+    return g_zgemm_algo == 3 && n > 32 && k >= 16 && (const void *)B != (const void *)C;
+}
+
 // C <- beta*C + alpha*A*B  (device pointers, column-major)
 int zgemm(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda, const double2 *B, long ldb,
           double beta, double2 *C, long ldc) {
     if (m <= 0 || n <= 0) return 0;
     if (k <= 0 && beta == 1.0) return 0;
+    if (use_3m(n, k, B, C)) return zgemm3m(st, m, n, k, alpha, A, lda, 0, B, ldb, 0, beta, C, ldc, 0, 1);
     if (n <= 32) return launch_zgemm<8, 1, 8, 4, 1>(st, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc);
     return launch_zgemm<4, 2, 16, 4, 1>(st, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc);
 }
@@ -211,12 +221,18 @@ int gemm(cudaStream_t st, int m, int n, int k, double alpha, ZView A, ZView B, d
 int zgemm_batched(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda, long strideA,
                   const double2 *B, long ldb, long strideB, double beta, double2 *C, long ldc, long strideC, int nbatch) {
     if (m <= 0 || n <= 0 || nbatch <= 0) return 0;
+    if (use_3m(n, k, B, C)) return zgemm3m(st, m, n, k, alpha, A, lda, strideA, B, ldb, strideB, beta, C, ldc, strideC, nbatch);
     if (n <= 32)
         return launch_zgemm<8, 1, 8, 4, 1>(st, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, strideA, strideB, strideC, nbatch);
     return launch_zgemm<4, 2, 16, 4, 1>(st, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, strideA, strideB, strideC, nbatch);
 }
 
 }  // namespace hp
+
+extern "C" int hprmat_zgemm_algo(int algo) {
+    if (algo == 3 || algo == 4) hp::g_zgemm_algo = algo;
+    return hp::g_zgemm_algo;
+}
 
 extern "C" int hprmat_zgemm(void *cuda_stream, int m, int n, int k, double alpha, const void *A, int lda, const void *B,
                             int ldb, double beta, void *C, int ldc) {

@@ -83,6 +83,29 @@ def test_zgemm_matches_definition(m, n, k):
     assert np.abs(_host(Cd) - ref).max() <= 4 * (k + 2) * 2.0 ** -53 * 2.0 * max(1.0, np.abs(ref).max())
 
 
+@pytest.mark.parametrize("algo", [3, 4])
+def test_zgemm_both_real_decompositions(algo):
+    """hprmat_zgemm_algo: the 3M kernel (three real products, imaginary part normwise accurate) and the 4M kernel against the
+    definition in long double, with the NORMWISE bound (k + 4) 2^-52 (|A| |B|)_ij + 2^-52 |C0| that holds for both, on a
+    ragged shape that spans several tiles of either kernel; and the switch reports what is in force."""
+    prev = hb.hprmat_zgemm_algo()
+    try:
+        assert hb.hprmat_zgemm_algo(algo) == algo and hb.hprmat_zgemm_algo(0) == algo
+        m, n, k = 333, 201, 150
+        rng = np.random.default_rng(77 + algo)
+        A = rng.normal(size=(m, k)) + 1j * rng.normal(size=(m, k))
+        B = rng.normal(size=(k, n)) + 1j * rng.normal(size=(k, n))
+        C0 = rng.normal(size=(m, n)) + 1j * rng.normal(size=(m, n))
+        Cd = _dev_colmajor(C0)
+        hb.hprmat_zgemm(m, n, k, -1.0, _dev_colmajor(A), m, _dev_colmajor(B), k, 1.0, Cd, m)
+        ref = C0 - (A.astype(np.clongdouble) @ B.astype(np.clongdouble)).astype(np.complex128)
+        absA, absB = np.abs(A.real) + np.abs(A.imag), np.abs(B.real) + np.abs(B.imag)
+        bound = (k + 4) * 2.0 ** -52 * (absA @ absB) + 2.0 ** -52 * np.abs(C0)
+        assert np.all(np.abs(_host(Cd) - ref) <= bound)
+    finally:
+        hb.hprmat_zgemm_algo(prev)
+
+
 @pytest.mark.parametrize("n,nrhs", [(1, 1), (2, 3), (31, 1), (32, 5), (33, 2), (100, 7), (257, 4), (640, 64), (1500, 3)])
 def test_zsolve_fp64_matches_oracle(n, nrhs):
     A = dense_test_matrix(n, nrhs, seed=7000 + n)
