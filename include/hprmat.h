@@ -128,8 +128,9 @@ int hprmat_zgetrf(void *cuda_stream, int n, void *A, int lda, int *ipiv, int *in
 int hprmat_zgetrs(void *cuda_stream, int n, int nrhs, const void *A, int lda, const int *ipiv, void *B, int ldb,
                   void *workspace, size_t workspace_bytes);
 
-/* C <- beta*C + alpha*A*B, complex128 column-major, real alpha and beta; the FP64 tensor-core (DMMA) kernel that
- * performs the trailing update of the LU.  A m x k, B k x n, C m x n. */
+/* C <- beta*C + alpha*A*B, complex128 column-major, real alpha and beta; the FP64 tensor-core (DMMA) kernels that
+ * perform the trailing update of the LU (3M decomposition by default, see hprmat_zgemm_algo).  A m x k, B k x n, C m x n.
+ * C may alias B only when m <= 128 and beta == 0. */
 int hprmat_zgemm(void *cuda_stream, int m, int n, int k, double alpha, const void *A, int lda, const void *B, int ldb,
                  double beta, void *C, int ldc);
 

@@ -13,7 +13,8 @@ constexpr int SB = 1024;      // "solve block": the full inverses of the SB x SB
 constexpr int MAXG = kNumSMs; // CTAs of the cooperative panel kernel (one per SM)
 
 // GEMM back-ends (zgemm.cu / cgemm.cu): C <- beta*C + alpha*A*B.  nbatch > 1: operand b lives at view + b*stride
-// elements.  C may alias B when m <= 32 and the whole K extent is one diagonal block (see trsm in lu.cu).
+// elements.  C may alias B when m <= 128 (a single M tile of the kernel that is chosen then) and beta == 0: the in-place
+// leaf product B <- inv * B of the triangular solves (lu.cu).
 int gemm(cudaStream_t st, int m, int n, int k, double alpha, ZView A, ZView B, double beta, ZView C);
 int gemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
 // FP32-class accuracy variant for the planar complex64 type (3xTF32, cgemm3.cu); C may alias B when m <= 128, beta == 0

@@ -6,7 +6,6 @@
 
 #include <algorithm>
 
-#include <cooperative_groups.h>
 
 namespace hp {
 

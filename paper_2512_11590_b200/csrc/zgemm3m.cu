@@ -103,28 +103,40 @@ __global__ void __launch_bounds__(WM *WN * 32, 1)
         }
         const double2 *a_s = sA + (kt % STAGES) * A_STAGE + a_off;
         const double2 *b_s = sB + (kt % STAGES) * B_STAGE + b_off;
+        // Software pipeline over the k-steps: the fragments of step ks + 1 are fetched before the MMAs of step ks are issued,
+        // and their sums (DADDs, which queue on the same FP64 pipe as the DMMAs) are formed after them, a whole step before use.
+        double2 af[2][4], bf[2][2];
+        double as[2][4], bs[2][2];
+        auto fetch = [&](int ks, int b) {
+#pragma unroll
+            for (int mi = 0; mi < 4; ++mi) af[b][mi] = a_s[ks * 4 * LDA_S + mi * 8];
+#pragma unroll
+            for (int ni = 0; ni < 2; ++ni) bf[b][ni] = b_s[ni * 8 * LDB_S + ks * 4];
+        };
+        auto sums = [&](int b) {
+#pragma unroll
+            for (int mi = 0; mi < 4; ++mi) as[b][mi] = af[b][mi].x + af[b][mi].y;
+#pragma unroll
+            for (int ni = 0; ni < 2; ++ni) bs[b][ni] = bf[b][ni].x + bf[b][ni].y;
+        };
+        fetch(0, 0);
+        sums(0);
 #pragma unroll
         for (int ks = 0; ks < KC / 4; ++ks) {
-            double2 af[4], bf[2];
-            double as[4], bs[2];
-#pragma unroll
-            for (int mi = 0; mi < 4; ++mi) {
-                af[mi] = a_s[ks * 4 * LDA_S + mi * 8];
-                as[mi] = af[mi].x + af[mi].y;
-            }
-#pragma unroll
-            for (int ni = 0; ni < 2; ++ni) {
-                bf[ni] = b_s[ni * 8 * LDB_S + ks * 4];
-                bs[ni] = bf[ni].x + bf[ni].y;
-            }
+            const int b = ks & 1;
+            if (ks + 1 < KC / 4) fetch(ks + 1, b ^ 1);
 #pragma unroll
             for (int mi = 0; mi < 4; ++mi)
 #pragma unroll
                 for (int ni = 0; ni < 2; ++ni) {
-                    dmma(t1[mi][ni], af[mi].x, bf[ni].x);
-                    dmma(t2[mi][ni], af[mi].y, bf[ni].y);
-                    dmma(t3[mi][ni], as[mi], bs[ni]);
+                    dmma(t1[mi][ni], af[b][mi].x, bf[b][ni].x);
+                    dmma(t2[mi][ni], af[b][mi].y, bf[b][ni].y);
                 }
+#pragma unroll
+            for (int mi = 0; mi < 4; ++mi)
+#pragma unroll
+                for (int ni = 0; ni < 2; ++ni) dmma(t3[mi][ni], as[b][mi], bs[b][ni]);
+            if (ks + 1 < KC / 4) sums(b ^ 1);
         }
     }
     cp_wait<0>();
