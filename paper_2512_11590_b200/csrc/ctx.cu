@@ -197,6 +197,7 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
         HP_ALLOC(c->d_workc, wb);
         if (cudaMemsetAsync(c->d_workc, 0, wb, c->st) != cudaSuccess) { free_ctx(c); return HPRMAT_ECUDA; }
         c->wc.carve(c->d_workc, (int)N);
+        c->wc.speculate = true;  // S = I + K_d^-1 V: the diagonal is the partial-pivoting choice; verified per panel (panel.cu)
     }
     HP_ALLOC(c->d_X, sizeof(double2) * N * nch);
     HP_ALLOC(c->d_Rr, sizeof(double2) * N * nch);

@@ -36,6 +36,9 @@ template <class V> struct LuWork {
                          // (the solves apply those from dinvL/dinvU[NLEV-1] with the 3xTF32 kernel)
     V tmp;               // sbld x max(n, 256) scratch: out-of-place leaf product
     long sbld = 0;
+    V backup;            // n x IB: the panel as it was before a speculative (diagonal-pivot) factorisation (panel.cu)
+    int *spec_flags = nullptr; // nblk: 1 = the speculation of that panel was refuted
+    bool speculate = false;    // host-side: try diagonal pivots first (set by the structured mixed path)
     bool side_used = false; // host-side: something of this factorisation was enqueued on the side stream
     bool use_big = true; // host-side switch: off while an SB inverse is being built from the LEAF-level recursion
     int *perm = nullptr; // nblk x (1 + 4*IB): count, dst rows[2*IB], src rows[2*IB]  (net permutation of each swap batch)

@@ -332,6 +332,38 @@ __device__ __forceinline__ void warp_argmax(double &v, int &li) {
     li = idx == 0x7fffffff ? -1 : idx;
 }
 
+// Inverses of the unit-lower and upper triangles of the factored top block (topb: column-major jb x jb, ld = IB, multipliers
+// already scaled; invp[k] = 1/u_kk) -> dinvL / dinvU, the IB-level leaves of the triangular-solve recursion.  Threads
+// 0 .. jb-1 do the columns of inv(L), threads 32 .. 32+jb-1 those of inv(U); inv_s is [2][IB][IB] scratch.
+template <class V>
+__device__ __forceinline__ void top_block_inverses(const typename V::elem_t *topb, const typename V::elem_t *invp,
+                                                   typename V::elem_t *inv_s, int jb, V dinvL, V dinvU, int tid) {
+    typedef typename V::elem_t E;
+    typedef typename V::real_t T;
+    E *xl = inv_s, *xu = inv_s + IB * IB;  // column-major jb x jb, ld = IB
+    if (tid < jb) {
+        const int cc = tid;  // column cc of inv(L): forward substitution on e_cc
+        for (int i = 0; i < jb; ++i) xl[cc * IB + i] = mk((T)(i == cc ? 1 : 0), (T)0);
+        for (int i = cc + 1; i < jb; ++i) {
+            E s = mk((T)0, (T)0);
+            for (int k = cc; k < i; ++k) s = cadd(s, cmul(topb[k * IB + i], xl[cc * IB + k]));
+            xl[cc * IB + i] = mk(-s.x, -s.y);
+        }
+        for (int i = 0; i < jb; ++i) dinvL.set(i, cc, xl[cc * IB + i]);
+    } else if (tid >= 32 && tid < 32 + jb) {
+        const int cc = tid - 32;  // column cc of inv(U): back substitution on e_cc
+        for (int i = 0; i < jb; ++i) xu[cc * IB + i] = mk((T)0, (T)0);
+        xu[cc * IB + cc] = invp[cc];
+        for (int i = cc - 1; i >= 0; --i) {
+            E s = mk((T)0, (T)0);
+            for (int k = i + 1; k <= cc; ++k) s = cadd(s, cmul(topb[k * IB + i], xu[cc * IB + k]));
+            E q = cmul(s, invp[i]);
+            xu[cc * IB + i] = mk(-q.x, -q.y);
+        }
+        for (int i = 0; i < jb; ++i) dinvU.set(i, cc, xu[cc * IB + i]);
+    }
+}
+
 // compile-time loop: f(integral_constant<int, I>) for I = B .. E-1 (keeps the register-resident panel statically indexed)
 template <int I> struct IntC { static constexpr int value = I; };
 template <int B, int E_, class F> __device__ __forceinline__ void static_for(F &&f) {
@@ -344,7 +376,11 @@ template <int B, int E_, class F> __device__ __forceinline__ void static_for(F &
 template <class V, int RPT, bool TIMING = false>
 __global__ void __launch_bounds__(PANEL_NT, 1)
     panel_reg_kernel(V A, int m, int jb, int j0, int rpc, int *ipiv, int *info, unsigned long long *ll, unsigned ep_base,
-                     V dinvL, V dinvU, int *perm, long long *dbg) {
+                     V dinvL, V dinvU, int *perm, long long *dbg, const int *spec_flag, V backup) {
+    // After a speculative (diagonal-pivot) factorisation of this panel: nothing to do if it was verified, else redo it with
+    // pivoting from the saved copy of the panel.  The flag is final (stream order) and read identically by all CTAs.
+    if (spec_flag != nullptr && *spec_flag == 0) return;
+    const V Src = spec_flag != nullptr ? backup : A;
     typedef typename V::elem_t E;
     typedef typename V::real_t T;
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -381,7 +417,7 @@ __global__ void __launch_bounds__(PANEL_NT, 1)
     for (int r = 0; r < RPT; ++r) {
         const int li = tid + r * PANEL_NT;
 #pragma unroll
-        for (int c = 0; c < IB; ++c) a[r][c] = (li < nloc && c < jb) ? A.get(row0 + li, c) : mk((T)0, (T)0);
+        for (int c = 0; c < IB; ++c) a[r][c] = (li < nloc && c < jb) ? Src.get(row0 + li, c) : mk((T)0, (T)0);
     }
     tick(0);
 
@@ -585,30 +621,101 @@ __global__ void __launch_bounds__(PANEL_NT, 1)
         for (int c = 0; c < IB; ++c) topb[c * IB + tid] = a[0][c];
     }
     __syncthreads();
-    E *xl = inv_s, *xu = inv_s + IB * IB;  // column-major jb x jb, ld = IB
-    if (tid < jb) {
-        const int cc = tid;  // column cc of inv(L): forward substitution on e_cc
-        for (int i = 0; i < jb; ++i) xl[cc * IB + i] = mk((T)(i == cc ? 1 : 0), (T)0);
-        for (int i = cc + 1; i < jb; ++i) {
-            E s = mk((T)0, (T)0);
-            for (int k = cc; k < i; ++k) s = cadd(s, cmul(topb[k * IB + i], xl[cc * IB + k]));
-            xl[cc * IB + i] = mk(-s.x, -s.y);
-        }
-        for (int i = 0; i < jb; ++i) dinvL.set(i, cc, xl[cc * IB + i]);
-    } else if (tid >= 32 && tid < 32 + jb) {
-        const int cc = tid - 32;  // column cc of inv(U): back substitution on e_cc
-        for (int i = 0; i < jb; ++i) xu[cc * IB + i] = mk((T)0, (T)0);
-        xu[cc * IB + cc] = invp[cc];
-        for (int i = cc - 1; i >= 0; --i) {
-            E s = mk((T)0, (T)0);
-            for (int k = i + 1; k <= cc; ++k) s = cadd(s, cmul(topb[k * IB + i], xu[cc * IB + k]));
-            E q = cmul(s, invp[i]);
-            xu[cc * IB + i] = mk(-q.x, -q.y);
-        }
-        for (int i = 0; i < jb; ++i) dinvU.set(i, cc, xu[cc * IB + i]);
-    } else if (warp == 2) {
+    top_block_inverses<V>(topb, invp, inv_s, jb, dinvL, dinvU, tid);
+    if (warp == 2) {
         net_permutation(piv, jb, j0, perm, lane);
     }
+}
+
+// ------------------------------------------------------------------------------------------------- speculative panel
+// Partial pivoting picks, in column j, the first row of maximal |re| + |im| among rows >= j.  When that is row j itself in
+// every column of the panel (always the case for the block-preconditioned matrix S = I + K_d^-1 V of the mixed path,
+// whose off-diagonal entries are coupling-sized), the panel factorisation needs no exchange between CTAs at all:
+// every CTA factors the jb x jb top block (no interchanges) and each thread forward-substitutes its own row,
+//     a_ij^(j) = a_ij - sum_{k<j} l_ik u_kj,     l_ij = a_ij^(j) / u_jj,
+// in the same operation order as the rank-1 updates.  The a_ij^(j) are exactly the candidates partial pivoting would
+// compare, so the speculation is VERIFIED on the fly: |a_ij^(j)| <= |u_jj| for all i > j (ties go to the smaller row, i.e.
+// to the diagonal); any violation (or a zero pivot) raises the panel's flag, and the pivoting kernel that is always
+// enqueued right behind redoes the panel from the saved copy.  The result is partial pivoting's in both cases.
+template <class V>
+__global__ void __launch_bounds__(PANEL_NT) panel_spec_kernel(V A, int m, int jb, int j0, int *ipiv, int *flag, V backup,
+                                                             V dinvL, V dinvU, int *perm) {
+    typedef typename V::elem_t E;
+    typedef typename V::real_t T;
+    extern __shared__ __align__(16) unsigned char smraw[];
+    E *topb = reinterpret_cast<E *>(smraw);  // [IB][IB] column-major, ld = IB: the top block, factored in place
+    E *inv_s = topb + IB * IB;               // [2][IB][IB] scratch (CTA 0)
+    __shared__ E invp[IB];
+    __shared__ int s_bad;
+    const int tid = threadIdx.x;
+    const int row = blockIdx.x * PANEL_NT + tid;  // panel row of this thread
+
+    // every thread saves and keeps its own row; the top block goes to shared memory in every CTA
+    E a[IB];
+#pragma unroll
+    for (int c = 0; c < IB; ++c) {
+        a[c] = (row < m && c < jb) ? A.get(row, c) : mk((T)0, (T)0);
+        if (row < m && c < jb) backup.set(row, c, a[c]);
+    }
+    for (int idx = tid; idx < IB * IB; idx += PANEL_NT) {
+        const int i = idx % IB, c = idx / IB;
+        topb[idx] = (i < jb && c < jb && i < m) ? A.get(i, c) : mk((T)(i == c ? 1 : 0), (T)0);
+    }
+    if (tid == 0) s_bad = 0;
+    __syncthreads();
+    // ---- top block, no interchanges: 8 threads per row; step j: scale column j, rank-1 update of the rest
+    {
+        const int i = tid >> 3, c8 = tid & 7;
+        for (int j = 0; j < jb; ++j) {
+            const E pv = topb[j * IB + j];
+            const bool sing = (pv.x == (T)0 && pv.y == (T)0);
+            const E ip = sing ? mk((T)0, (T)0) : crecip_fast(pv);
+            E l = mk((T)0, (T)0);
+            if (i > j && i < jb) {
+                const E v = topb[j * IB + i];
+                if (sing || cabs1(v) > cabs1(pv)) s_bad = 1;
+                l = cmul(v, ip);
+            }
+            __syncthreads();  // everybody has read column j and the pivot
+            if (i > j && i < jb) {
+                if (c8 == 0) topb[j * IB + i] = l;
+                for (int c = j + 1 + c8; c < jb; c += 8) topb[c * IB + i] = cfnma(topb[c * IB + i], l, topb[c * IB + j]);
+            }
+            if (tid == 0) invp[j] = ip;
+            __syncthreads();
+        }
+    }
+    // ---- rows below the top block: forward substitution against U11, verified column by column
+    bool bad = false;
+    if (row >= jb && row < m) {
+        static_for<0, IB>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            if (j < jb) {
+                E v = a[j];
+                static_for<0, j>([&](auto kc) {
+                    constexpr int k = decltype(kc)::value;
+                    v = cfnma(v, a[k], topb[j * IB + k]);
+                });
+                if (cabs1(v) > cabs1(topb[j * IB + j])) bad = true;
+                a[j] = cmul(v, invp[j]);
+            }
+        });
+#pragma unroll
+        for (int c = 0; c < IB; ++c)
+            if (c < jb) A.set(row, c, a[c]);
+    }
+    if (bad) s_bad = 1;
+    __syncthreads();
+    if (tid == 0 && s_bad) atomicExch(flag, 1);
+    if (blockIdx.x != 0) return;
+    // ---- CTA 0: the factored top block, the (identity) interchanges, the IB-level inverses, an empty swap batch
+    for (int idx = tid; idx < IB * IB; idx += PANEL_NT) {
+        const int i = idx % IB, c = idx / IB;
+        if (i < jb && c < jb && i < m) A.set(i, c, topb[idx]);
+    }
+    if (tid < jb) ipiv[j0 + tid] = j0 + tid + 1;
+    if (tid == 0) perm[0] = 0;
+    top_block_inverses<V>(topb, invp, inv_s, jb, dinvL, dinvU, tid);
 }
 
 template <class V, int RPT>
@@ -624,7 +731,21 @@ static int launch_panel_reg(cudaStream_t st, V Asub, int m, int w, int c0, int r
     }
     unsigned ep = wk.ep_base;
     long long *dbg = nullptr;
-    void *args[] = {&Asub, &m, &w, &c0, &rpc, &ipiv, &info_dev, &wk.slots, &ep, &dl, &du, &perm, &dbg};
+    const int *spec_flag = nullptr;
+    if (wk.speculate) {
+        // diagonal-pivot attempt first; the pivoting kernel behind it returns at once if the attempt was verified
+        auto spec = panel_spec_kernel<V>;
+        static bool spec_configured = false;
+        if (!spec_configured) {
+            HP_CUDA(cudaFuncSetAttribute(spec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            spec_configured = true;
+        }
+        int *flag = wk.spec_flags + c0 / IB;
+        spec<<<ceil_div(m, PANEL_NT), PANEL_NT, smem, st>>>(Asub, m, w, c0, ipiv, flag, wk.backup, dl, du, perm);
+        HP_LAUNCHED();
+        spec_flag = flag;
+    }
+    void *args[] = {&Asub, &m, &w, &c0, &rpc, &ipiv, &info_dev, &wk.slots, &ep, &dl, &du, &perm, &dbg, &spec_flag, &wk.backup};
     HP_CUDA(cudaLaunchCooperativeKernel((void *)kern, dim3(G), dim3(PANEL_NT), args, smem, st));
     wk.ep_base += (unsigned)w;
     return 0;
@@ -688,7 +809,8 @@ int probe_panel(cudaStream_t st, int m, int reps, float *A_re, float *A_im, long
     for (int it = 0; it <= reps; ++it) {
         if (it == 1) HP_CUDA(cudaEventRecord(e0, st));
         unsigned ep = wk.ep_base;
-        void *args[] = {&A, &m, &w, &c0, &rpc, &ipiv, &info, &wk.slots, &ep, &dl, &du, &wk.perm, &dbg};
+        const int *spec_flag = nullptr;
+        void *args[] = {&A, &m, &w, &c0, &rpc, &ipiv, &info, &wk.slots, &ep, &dl, &du, &wk.perm, &dbg, &spec_flag, &wk.backup};
         HP_CUDA(cudaLaunchCooperativeKernel((void *)kern, dim3(G), dim3(PANEL_NT), args, smem, st));
         HP_LAUNCHED();
         wk.ep_base += IB;

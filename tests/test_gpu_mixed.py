@@ -195,6 +195,29 @@ def test_mixed_strong_coupling_needs_and_gets_more_refinement():
     ctx.destroy()
 
 
+def test_mixed_speculative_panel_falls_back_to_pivoting_when_refuted():
+    """The mixed path first tries diagonal pivots in every panel (verified on the fly, panel.cu) and redoes a panel with
+    partial pivoting when the verification fails.  Couplings 300x the configs' make S = K_d^-1 (C - E) pivot off the
+    diagonal (25 of 360 pivots in a complex64 LAPACK factorisation of the same S), so the fall-back path runs: the unrefined
+    result must still be a low-precision solution (kappa(S) ~ 1e3, TF32 factors), not garbage, and a converged refinement
+    must reach the oracle."""
+    w = make_workload(1, nch=6, nb=60)
+    w.beta *= 300.0
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=0)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    Ro, _ = _oracle_R(w, 20.0)
+    R0, info0 = ctx.solve(20.0, V, hb.HPRMAT_MIXED)
+    assert info0["status"] == 0 and np.all(np.isfinite(_host(R0)))
+    assert _relmax(_host(R0), Ro) <= 0.2, info0
+    R, info = ctx.solve(20.0, V, hb.HPRMAT_MIXED_REFINE, max_refine=40, allow=(hb.HPRMAT_OK, hb.HPRMAT_ENOTCONVERGED))
+    if info["status"] == hb.HPRMAT_OK:
+        assert _relmax(_host(R), Ro) <= 1e-10, info
+    Rf, _ = ctx.solve(20.0, V, hb.HPRMAT_FP64)
+    assert _relmax(_host(Rf), Ro) <= 1e-10
+    ctx.destroy()
+
+
 def test_mixed_matches_fp64_mode_on_the_same_context():
     w = make_workload(2, nch=10, nb=100)
     ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=0)
