@@ -644,18 +644,28 @@ __global__ void __launch_bounds__(PANEL_NT) panel_spec_kernel(V A, int m, int jb
     typedef typename V::real_t T;
     extern __shared__ __align__(16) unsigned char smraw[];
     E *topb = reinterpret_cast<E *>(smraw);  // [IB][IB] column-major, ld = IB: the top block, factored in place
-    E *inv_s = topb + IB * IB;               // [2][IB][IB] scratch (CTA 0)
+    E *inv_s = topb + IB * IB;               // [2][IB][IB] scratch for the triangular inverses (last CTA)
+    E *rows = inv_s + 2 * IB * IB;           // [IB][PANEL_NT]: element c of this thread's row at rows[c*PANEL_NT + tid]
     __shared__ E invp[IB];
     __shared__ int s_bad;
     const int tid = threadIdx.x;
-    const int row = blockIdx.x * PANEL_NT + tid;  // panel row of this thread
+    const bool top_cta = blockIdx.x == gridDim.x - 1;  // the extra CTA that owns the top block's outputs
+    const int row = blockIdx.x * PANEL_NT + tid;        // panel row of this thread (row CTAs)
+    const bool has_row = !top_cta && row < m;
 
-    // every thread saves and keeps its own row; the top block goes to shared memory in every CTA
-    E a[IB];
+    // every row thread saves its row and parks it in shared memory; the top block goes to shared memory in every CTA
+    if (has_row) {
+        for (int c0 = 0; c0 < jb; c0 += 8) {  // eight independent loads in flight, then their stores
+            E v[8];
 #pragma unroll
-    for (int c = 0; c < IB; ++c) {
-        a[c] = (row < m && c < jb) ? A.get(row, c) : mk((T)0, (T)0);
-        if (row < m && c < jb) backup.set(row, c, a[c]);
+            for (int q = 0; q < 8; ++q) v[q] = (c0 + q < jb) ? A.get(row, c0 + q) : mk((T)0, (T)0);
+#pragma unroll
+            for (int q = 0; q < 8; ++q)
+                if (c0 + q < jb) {
+                    backup.set(row, c0 + q, v[q]);
+                    rows[(c0 + q) * PANEL_NT + tid] = v[q];
+                }
+        }
     }
     for (int idx = tid; idx < IB * IB; idx += PANEL_NT) {
         const int i = idx % IB, c = idx / IB;
@@ -663,9 +673,10 @@ __global__ void __launch_bounds__(PANEL_NT) panel_spec_kernel(V A, int m, int jb
     }
     if (tid == 0) s_bad = 0;
     __syncthreads();
-    // ---- top block, no interchanges: 8 threads per row; step j: scale column j, rank-1 update of the rest
+    // ---- top block, no interchanges: lane = row, warp = column residue (conflict-free column-major accesses);
+    //      step j: scale column j, rank-1 update of the rest
     {
-        const int i = tid >> 3, c8 = tid & 7;
+        const int i = tid & 31, c8 = tid >> 5;
         for (int j = 0; j < jb; ++j) {
             const E pv = topb[j * IB + j];
             const bool sing = (pv.x == (T)0 && pv.y == (T)0);
@@ -685,37 +696,42 @@ __global__ void __launch_bounds__(PANEL_NT) panel_spec_kernel(V A, int m, int jb
             __syncthreads();
         }
     }
-    // ---- rows below the top block: forward substitution against U11, verified column by column
-    bool bad = false;
-    if (row >= jb && row < m) {
-        static_for<0, IB>([&](auto jc) {
-            constexpr int j = decltype(jc)::value;
-            if (j < jb) {
-                E v = a[j];
-                static_for<0, j>([&](auto kc) {
-                    constexpr int k = decltype(kc)::value;
-                    v = cfnma(v, a[k], topb[j * IB + k]);
-                });
-                if (cabs1(v) > cabs1(topb[j * IB + j])) bad = true;
-                a[j] = cmul(v, invp[j]);
+    if (top_cta) {
+        // ---- the factored top block, the (identity) interchanges, the IB-level inverses, an empty swap batch
+        for (int idx = tid; idx < IB * IB; idx += PANEL_NT) {
+            const int i = idx % IB, c = idx / IB;
+            if (i < jb && c < jb && i < m) A.set(i, c, topb[idx]);
+        }
+        if (tid < jb) ipiv[j0 + tid] = j0 + tid + 1;
+        if (tid == 0) {
+            perm[0] = 0;
+            if (s_bad) atomicExch(flag, 1);
+        }
+        top_block_inverses<V>(topb, invp, inv_s, jb, dinvL, dinvU, tid);
+        return;
+    }
+    // ---- rows below the top block: forward substitution against U11 (rolled loops, the row lives in shared memory),
+    //      verified column by column
+    if (has_row && row >= jb) {
+        E *my = rows + tid;
+        bool bad = false;
+        for (int j = 0; j < jb; ++j) {
+            const E *u = topb + j * IB;  // column j of U11: u[k] = u_kj
+            E v = my[j * PANEL_NT], v1 = mk((T)0, (T)0);  // two accumulation chains
+            int k = 0;
+            for (; k + 1 < j; k += 2) {
+                v = cfnma(v, my[k * PANEL_NT], u[k]);
+                v1 = cfnma(v1, my[(k + 1) * PANEL_NT], u[k + 1]);
             }
-        });
-#pragma unroll
-        for (int c = 0; c < IB; ++c)
-            if (c < jb) A.set(row, c, a[c]);
+            if (k < j) v = cfnma(v, my[k * PANEL_NT], u[k]);
+            v = cadd(v, v1);
+            if (cabs1(v) > cabs1(u[j])) bad = true;
+            my[j * PANEL_NT] = cmul(v, invp[j]);
+        }
+        if (bad) atomicExch(flag, 1);
+#pragma unroll 8
+        for (int c = 0; c < jb; ++c) A.set(row, c, my[c * PANEL_NT]);
     }
-    if (bad) s_bad = 1;
-    __syncthreads();
-    if (tid == 0 && s_bad) atomicExch(flag, 1);
-    if (blockIdx.x != 0) return;
-    // ---- CTA 0: the factored top block, the (identity) interchanges, the IB-level inverses, an empty swap batch
-    for (int idx = tid; idx < IB * IB; idx += PANEL_NT) {
-        const int i = idx % IB, c = idx / IB;
-        if (i < jb && c < jb && i < m) A.set(i, c, topb[idx]);
-    }
-    if (tid < jb) ipiv[j0 + tid] = j0 + tid + 1;
-    if (tid == 0) perm[0] = 0;
-    top_block_inverses<V>(topb, invp, inv_s, jb, dinvL, dinvU, tid);
 }
 
 template <class V, int RPT>
@@ -735,13 +751,15 @@ static int launch_panel_reg(cudaStream_t st, V Asub, int m, int w, int c0, int r
     if (wk.speculate) {
         // diagonal-pivot attempt first; the pivoting kernel behind it returns at once if the attempt was verified
         auto spec = panel_spec_kernel<V>;
+        const size_t spec_smem = smem + (size_t)IB * PANEL_NT * sizeof(E);
         static bool spec_configured = false;
         if (!spec_configured) {
-            HP_CUDA(cudaFuncSetAttribute(spec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            HP_CUDA(cudaFuncSetAttribute(spec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)spec_smem));
             spec_configured = true;
         }
         int *flag = wk.spec_flags + c0 / IB;
-        spec<<<ceil_div(m, PANEL_NT), PANEL_NT, smem, st>>>(Asub, m, w, c0, ipiv, flag, wk.backup, dl, du, perm);
+        // one CTA per PANEL_NT rows plus one that owns the top block's outputs
+        spec<<<ceil_div(m, PANEL_NT) + 1, PANEL_NT, spec_smem, st>>>(Asub, m, w, c0, ipiv, flag, wk.backup, dl, du, perm);
         HP_LAUNCHED();
         spec_flag = flag;
     }
