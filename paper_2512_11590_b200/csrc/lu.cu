@@ -52,7 +52,7 @@ template <class V> size_t LuWork<V>::carve(void *base, int n_) {
         tmp = alloc_view<V>(p, sbld, std::max<long>(n, 256));
     }
     backup = alloc_view<V>(p, round_up(std::max(n, 1), 32), IB);
-    spec_flags = (int *)take(sizeof(int) * (size_t)std::max(nblk, 1));
+    spec_flags = (int *)take(sizeof(int) * 2 * (size_t)std::max(nblk, 1));  // [nblk] refuted, [nblk] interchanges published
     perm = (int *)take(sizeof(int) * (size_t)nblk * PERM_STRIDE);
     cand_val = (T *)take(sizeof(T) * 2 * MAXG);
     cand_row = (int *)take(sizeof(int) * 2 * MAXG);
@@ -279,6 +279,7 @@ template <class V> static int panel(cudaStream_t st, int n, V A, int c0, int w, 
     }
     HP_LAUNCHED();
     // this batch's interchanges on every other column of the matrix
+    if (panel_applies_swaps<V>(wk, m)) return 0;
     return laswp(st, A, 0, c0, c0 + w, n, wk.perm, blk, blk + 1);
 }
 
@@ -451,7 +452,7 @@ template <class V> int getrf(cudaStream_t st, int n, V A, int *ipiv, int *info_d
     if (n <= 0) return 0;
     HP_CUDA(cudaMemsetAsync(wk.counter, 0, sizeof(unsigned), st));
     HP_CUDA(cudaMemsetAsync(wk.slots, 0, sizeof(unsigned long long) * LL_WORDS, st));
-    HP_CUDA(cudaMemsetAsync(wk.spec_flags, 0, sizeof(int) * (size_t)std::max(wk.nblk, 1), st));
+    HP_CUDA(cudaMemsetAsync(wk.spec_flags, 0, sizeof(int) * 2 * (size_t)std::max(wk.nblk, 1), st));
     wk.bar_base = 0;
     wk.ep_base = 0;
     wk.use_big = true;

@@ -376,7 +376,8 @@ template <int B, int E_, class F> __device__ __forceinline__ void static_for(F &
 template <class V, int RPT, bool TIMING = false>
 __global__ void __launch_bounds__(PANEL_NT, 1)
     panel_reg_kernel(V A, int m, int jb, int j0, int rpc, int *ipiv, int *info, unsigned long long *ll, unsigned ep_base,
-                     V dinvL, V dinvU, int *perm, long long *dbg, const int *spec_flag, V backup) {
+                     V dinvL, V dinvU, int *perm, long long *dbg, const int *spec_flag, V backup, int *swap_ready,
+                     int ncols_total) {
     // After a speculative (diagonal-pivot) factorisation of this panel: nothing to do if it was verified, else redo it with
     // pivoting from the saved copy of the panel.  The flag is final (stream order) and read identically by all CTAs.
     if (spec_flag != nullptr && *spec_flag == 0) return;
@@ -613,17 +614,50 @@ __global__ void __launch_bounds__(PANEL_NT, 1)
                 if (c < jb) A.set(row0 + li, c, a[r][c]);
         }
     }
-    if (cta != 0) return;
-    // ---- CTA 0 owns the top jb x jb block: inverses of its unit-lower and upper triangles (leaves of the TRSM
-    //      recursion), and the net row permutation of this swap batch.
-    if (tid < IB) {
+    if (cta == 0) {
+        // ---- CTA 0 owns the top jb x jb block: inverses of its unit-lower and upper triangles (leaves of the TRSM
+        //      recursion), and the net row permutation of this swap batch.
+        if (tid < IB) {
 #pragma unroll
-        for (int c = 0; c < IB; ++c) topb[c * IB + tid] = a[0][c];
+            for (int c = 0; c < IB; ++c) topb[c * IB + tid] = a[0][c];
+        }
+        __syncthreads();
+        top_block_inverses<V>(topb, invp, inv_s, jb, dinvL, dinvU, tid);
+        if (warp == 2) net_permutation(piv, jb, j0, perm, lane);
+    }
+    if (spec_flag == nullptr) return;
+    // ---- Re-done speculative panel: the host did not enqueue the row-interchange kernel behind this panel (a verified
+    //      speculation has none), so the batch's net permutation is applied to all other columns here, by all CTAs, once
+    //      CTA 0 has published it.  A is the panel's view: full-matrix column C is column C - j0, row r is row r - j0.
+    if (cta == 0) {
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence();
+            atomicExch(swap_ready, 1);
+        }
+    } else if (tid == 0) {
+        while (atomicAdd(swap_ready, 0) == 0) {
+        }
+        __threadfence();
     }
     __syncthreads();
-    top_block_inverses<V>(topb, invp, inv_s, jb, dinvL, dinvU, tid);
-    if (warp == 2) {
-        net_permutation(piv, jb, j0, perm, lane);
+    const int cnt = perm[0];
+    if (cnt == 0) return;
+    const int nother = ncols_total - jb;             // all columns but the panel's own
+    const int q = tid & (2 * IB - 1), cl = tid >> 6;  // pair slot, column inside a group of four
+    int dst = 0, src = 0;
+    if (q < cnt) {
+        dst = perm[1 + q] - j0;
+        src = perm[1 + 2 * IB + q] - j0;
+    }
+    for (int g0 = cta * 4; g0 < nother; g0 += G * 4) {  // uniform trip count: four columns per pass, 64 pair slots each
+        const int g = g0 + cl;
+        const bool ok = g < nother && q < cnt;
+        const long col = (g < j0 ? g : g + jb) - (long)j0;
+        E val = mk((T)0, (T)0);
+        if (ok) val = A.get(src, col);  // a net permutation: gather all sources of the column, then scatter
+        __syncthreads();
+        if (ok) A.set(dst, col, val);
     }
 }
 
@@ -763,7 +797,10 @@ static int launch_panel_reg(cudaStream_t st, V Asub, int m, int w, int c0, int r
         HP_LAUNCHED();
         spec_flag = flag;
     }
-    void *args[] = {&Asub, &m, &w, &c0, &rpc, &ipiv, &info_dev, &wk.slots, &ep, &dl, &du, &perm, &dbg, &spec_flag, &wk.backup};
+    int *swap_ready = wk.spec_flags + wk.nblk + c0 / IB;
+    int ncols_total = wk.n;
+    void *args[] = {&Asub, &m, &w, &c0, &rpc, &ipiv, &info_dev, &wk.slots, &ep, &dl, &du, &perm, &dbg, &spec_flag, &wk.backup,
+                    &swap_ready, &ncols_total};
     HP_CUDA(cudaLaunchCooperativeKernel((void *)kern, dim3(G), dim3(PANEL_NT), args, smem, st));
     wk.ep_base += (unsigned)w;
     return 0;
@@ -772,6 +809,12 @@ static int launch_panel_reg(cudaStream_t st, V Asub, int m, int w, int c0, int r
 template <class V> struct PanelRows;  // rows one CTA of the register-resident kernel can hold
 template <> struct PanelRows<ZView> { static constexpr int max_rpt = 1; };
 template <> struct PanelRows<CView> { static constexpr int max_rpt = 2; };
+
+template <class V> bool panel_applies_swaps(const LuWork<V> &wk, int m) {
+    int rpc = std::max(ceil_div(m, MAXG), PANEL_MINROWS);
+    rpc = (int)round_up(rpc, 2);
+    return wk.speculate && rpc <= PanelRows<V>::max_rpt * PANEL_NT;
+}
 
 template <class V>
 int panel_launch(cudaStream_t st, V Asub, int m, int w, int c0, int *ipiv, int *info_dev, LuWork<V> &wk, V dl, V du, int *perm) {
@@ -828,7 +871,10 @@ int probe_panel(cudaStream_t st, int m, int reps, float *A_re, float *A_im, long
         if (it == 1) HP_CUDA(cudaEventRecord(e0, st));
         unsigned ep = wk.ep_base;
         const int *spec_flag = nullptr;
-        void *args[] = {&A, &m, &w, &c0, &rpc, &ipiv, &info, &wk.slots, &ep, &dl, &du, &wk.perm, &dbg, &spec_flag, &wk.backup};
+        int *swap_ready = nullptr;
+        int ncols_total = 0;
+        void *args[] = {&A, &m, &w, &c0, &rpc, &ipiv, &info, &wk.slots, &ep, &dl, &du, &wk.perm, &dbg, &spec_flag, &wk.backup,
+                        &swap_ready, &ncols_total};
         HP_CUDA(cudaLaunchCooperativeKernel((void *)kern, dim3(G), dim3(PANEL_NT), args, smem, st));
         HP_LAUNCHED();
         wk.ep_base += IB;
@@ -846,6 +892,8 @@ int probe_panel(cudaStream_t st, int m, int reps, float *A_re, float *A_im, long
     return 0;
 }
 
+template bool panel_applies_swaps<CView>(const LuWork<CView> &, int);
+template bool panel_applies_swaps<ZView>(const LuWork<ZView> &, int);
 template int panel_launch<CView>(cudaStream_t, CView, int, int, int, int *, int *, LuWork<CView> &, CView, CView, int *);
 template int panel_launch<ZView>(cudaStream_t, ZView, int, int, int, int *, int *, LuWork<ZView> &, ZView, ZView, int *);
 

@@ -19,4 +19,8 @@ constexpr size_t LL_WORDS = LL_SLOTS + LL_ROWS;
 template <class V>
 int panel_launch(cudaStream_t st, V Asub, int m, int w, int c0, int *ipiv, int *info_dev, LuWork<V> &wk, V dl, V du, int *perm);
 
+// true when the kernels enqueued by panel_launch apply the batch's row interchanges to the other columns themselves
+// (speculative mode: a verified panel has none, a re-done one applies them in its pivoting kernel)
+template <class V> bool panel_applies_swaps(const LuWork<V> &wk, int m);
+
 }  // namespace hp
