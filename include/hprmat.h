@@ -17,7 +17,9 @@
  *   - Pointers marked  dev  are CUDA device pointers, those marked  host  are host pointers.  The library never
  *     allocates device memory inside hprmat_solve / hprmat_zsolve / hprmat_zgetrf / hprmat_zgetrs / hprmat_zgemm.
  *   - Every call enqueues its kernels on the stream given at setup (or as argument); calls that fill a host
- *     hprmat_info synchronise that stream before returning, the others do not.
+ *     hprmat_info synchronise that stream before returning, the others do not (exception: refinement in the mixed modes).
+ *     Part of a factorisation (the kept block inverses) runs on a library-owned side stream, joined before the call's work
+ *     on the caller's stream continues.
  *   - Return value: 0 success; -k = argument k (1-based) invalid; >0 = one of the HPRMAT_E* codes below.
  *   - There is NO CPU fallback: without a CUDA device every compute entry returns HPRMAT_ECUDA.
  *   - One context per host thread / stream.  The caller owns V, R, A, B, ipiv and the workspace; the context owns
@@ -85,7 +87,8 @@ int hprmat_mesh(const hprmat_ctx *ctx, double *r, double *fa);
  *   tol  refinement stops when the estimated relative error left in X (correction norm x observed contraction, DESIGN.md
  *        reading R9) is <= tol; <=0 = default: 1e-13 in FP64 mode, 1e-12 in the mixed modes
  *   R    dev, complex nch x nch column-major (output)
- *   info host, may be NULL (then the call does not synchronise) */
+ *   info host, may be NULL: then HPRMAT_FP64 and HPRMAT_MIXED only enqueue work (no synchronisation, max_refine steps are
+ *        taken unconditionally in FP64 mode); HPRMAT_MIXED_REFINE always reads the correction norms back between steps */
 int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int max_refine, double tol, void *R,
                  hprmat_info *info);
 
