@@ -145,3 +145,44 @@ def rmatrix(nch, nb, a, h2m, lval, ethr, energy, V, mode: int = 0, nrefine: int 
     if return_seconds:
         out.append(sec.value)
     return out[0] if len(out) == 1 else tuple(out)
+
+
+def collision_matrix(R, lval, ethr, energy, h2m, a):
+    """Collision (S) matrix of the OPEN channels from the R-matrix at the channel radius, neutral case (eta = 0).
+
+    PAPER.md:35, 53, 71 name the step ("matching to asymptotic solutions", "collision matrix") without printing it; the
+    reading taken (R14) is the standard one of the paper's ref. [2] (Descouvemont & Baye 2010):
+        Z^O_cc' = (k_c' a)^-1/2 [ O_c(k_c a) delta_cc' - a R_cc' dO_c'/dr (a) ],      Z^I likewise with I,
+        U = open rows of (Z^O)^-1 Z^I   (columns: open channels only),
+    with k_c = sqrt(|E - E_c| / h2m); open channels: O = G + iF, I = G - iF, F = x j_l(x), G = -x y_l(x), x = k r;
+    closed channels (E < E_c) carry no incoming wave and their outgoing function is the decaying one, the eta = 0
+    Whittaker function W(r) = x k_l(x), x = kappa r (modified spherical Bessel function of the second kind).
+    Returns (U, open) with U nopen x nopen and `open` the indices of the open channels.  Plain numpy / scipy.special.
+    """
+    from scipy.special import spherical_jn, spherical_yn, spherical_kn
+    R = np.asarray(R, dtype=np.complex128)
+    nch = R.shape[0]
+    ekin = float(energy) - np.asarray(ethr, dtype=float)
+    x = np.sqrt(np.abs(ekin) / h2m) * a
+    O = np.zeros(nch, dtype=complex)
+    dO = np.zeros(nch, dtype=complex)   # x * dO/dx = a * dO/dr at r = a
+    I = np.zeros(nch, dtype=complex)
+    dI = np.zeros(nch, dtype=complex)
+    for c in range(nch):
+        l, xc = int(lval[c]), x[c]
+        if ekin[c] > 0:
+            F = xc * spherical_jn(l, xc)
+            dF = spherical_jn(l, xc) + xc * spherical_jn(l, xc, derivative=True)
+            G = -xc * spherical_yn(l, xc)
+            dG = -spherical_yn(l, xc) - xc * spherical_yn(l, xc, derivative=True)
+            O[c], dO[c] = G + 1j * F, xc * (dG + 1j * dF)
+            I[c], dI[c] = G - 1j * F, xc * (dG - 1j * dF)
+        else:
+            W = xc * spherical_kn(l, xc)
+            dW = spherical_kn(l, xc) + xc * spherical_kn(l, xc, derivative=True)
+            O[c], dO[c] = W, xc * dW
+    opn = np.nonzero(ekin > 0)[0]
+    ZO = (np.diag(O) - R * dO[None, :]) / np.sqrt(x)[None, :]
+    ZI = ((np.diag(I) - R * dI[None, :]) / np.sqrt(x)[None, :])[:, opn]
+    Ufull = np.linalg.solve(ZO, ZI)
+    return Ufull[opn, :], opn

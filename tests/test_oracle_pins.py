@@ -402,3 +402,72 @@ def test_rmatrix_equals_definition_via_dense_solve_and_certificate():
     res = oracle.structured_residual(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, V, X)
     cert = (w.h2m / w.a) * X.T @ res
     assert np.abs(cert).max() < 1e-13 * np.abs(R).max()
+
+
+# ----------------------------------------------------------------- collision matrix (neutral case)
+def _ws_potential(nb, a, nch, beta, V0=50.0, W0=0.0, Rws=3.0, aws=0.65):
+    r = oracle.mesh(nb, a)[2]
+    u = np.exp((r - Rws) / aws)
+    f, df = 1.0 / (1.0 + u), -u / (aws * (1.0 + u) ** 2)
+    V = np.zeros((nb, nch, nch), dtype=complex)
+    for i in range(nb):
+        V[i] = beta * df[i]
+        V[i][np.diag_indices(nch)] = -(V0 + 1j * W0) * f[i]
+    return V
+
+
+def test_collision_matrix_free_particles_scatter_nothing_closed_channel_present():
+    """V = 0 with thresholds, one channel closed: U = 1 on the open channels (pins signs, derivatives and the k^-1/2
+    normalisation of the matching formula)."""
+    nb, a, E = 40, 8.0, 6.0
+    lval, ethr = [0, 2, 1, 3], [0.0, 1.5, 3.0, 9.0]
+    R = oracle.rmatrix(4, nb, a, H2M, lval, ethr, E, np.zeros((nb, 4, 4), dtype=complex))
+    U, opn = oracle.collision_matrix(R, lval, ethr, E, H2M, a)
+    assert list(opn) == [0, 1, 2]
+    assert np.abs(U - np.eye(3)).max() < 1e-9
+
+
+def test_collision_matrix_unitary_and_symmetric_with_a_closed_channel():
+    """Real symmetric couplings, one closed channel: flux conservation among the OPEN channels (U^dagger U = 1) holds only if
+    the closed channel is matched to the decaying function; U = U^T from C = C^T.  With absorption (W0 > 0) all singular
+    values drop below 1."""
+    nb, a, E = 40, 8.0, 6.0
+    lval, ethr = [0, 2, 1, 3], [0.0, 1.5, 3.0, 9.0]
+    rng = np.random.default_rng(3)
+    beta = rng.uniform(5.0, 20.0, (4, 4))
+    beta = 0.5 * (beta + beta.T)
+    np.fill_diagonal(beta, 0.0)
+    R = oracle.rmatrix(4, nb, a, H2M, lval, ethr, E, _ws_potential(nb, a, 4, beta))
+    U, opn = oracle.collision_matrix(R, lval, ethr, E, H2M, a)
+    assert len(opn) == 3 and np.abs(U).max() < 1.0 + 1e-12 and np.abs(U[0, 1]) > 0.05      # genuinely coupled
+    assert np.abs(U.conj().T @ U - np.eye(3)).max() < 1e-12
+    assert np.abs(U - U.T).max() < 1e-12
+    Ra = oracle.rmatrix(4, nb, a, H2M, lval, ethr, E, _ws_potential(nb, a, 4, beta, W0=10.0))
+    Ua, _ = oracle.collision_matrix(Ra, lval, ethr, E, H2M, a)
+    assert np.linalg.svd(Ua, compute_uv=False).max() < 1.0 - 1e-3
+
+
+def test_collision_matrix_reduces_to_the_all_open_formula_and_ignores_a_decoupled_closed_channel():
+    nb, a = 40, 8.0
+    lval, ethr = [0, 2, 1, 3], [0.0, 1.5, 3.0, 9.0]
+    rng = np.random.default_rng(4)
+    beta = rng.uniform(5.0, 20.0, (4, 4))
+    beta = 0.5 * (beta + beta.T)
+    np.fill_diagonal(beta, 0.0)
+    V = _ws_potential(nb, a, 4, beta)
+    # all channels open: the independent test-side helper (scatter.smatrix) gives the same matrix
+    E = 12.0
+    R = oracle.rmatrix(4, nb, a, H2M, lval, ethr, E, V)
+    U, opn = oracle.collision_matrix(R, lval, ethr, E, H2M, a)
+    assert len(opn) == 4
+    assert np.abs(U - smatrix(R, lval, np.sqrt((E - np.array(ethr)) / H2M), a)).max() < 1e-12
+    # a closed channel that is not coupled to the others cannot change their collision matrix
+    E = 6.0
+    V3 = V.copy()
+    V3[:, 3, :3] = 0.0
+    V3[:, :3, 3] = 0.0
+    R4 = oracle.rmatrix(4, nb, a, H2M, lval, ethr, E, V3)
+    R3 = oracle.rmatrix(3, nb, a, H2M, lval[:3], ethr[:3], E, np.ascontiguousarray(V3[:, :3, :3]))
+    U4, _ = oracle.collision_matrix(R4, lval, ethr, E, H2M, a)
+    U3, _ = oracle.collision_matrix(R3, lval[:3], ethr[:3], E, H2M, a)
+    assert np.abs(U4 - U3).max() < 1e-12
