@@ -154,6 +154,9 @@ def collision_matrix(R, lval, ethr, energy, h2m, a):
     reading taken (R14) is the standard one of the paper's ref. [2] (Descouvemont & Baye 2010):
         Z^O_cc' = (k_c' a)^-1/2 [ O_c(k_c a) delta_cc' - a R_cc' dO_c'/dr (a) ],      Z^I likewise with I,
         U = open rows of (Z^O)^-1 Z^I   (columns: open channels only),
+    evaluated with I = O - 2iF substituted, Z^I = Z^O - 2i Z^F, i.e. U = 1 - 2i (Z^O)^-1 Z^F: the same matrix, but a
+    channel far below its centrifugal barrier (G/F ~ 1e30) no longer loses F against G in the difference of two
+    nearly equal columns (the literal form is what tests/scatter.smatrix evaluates; the two are compared in the pins).
     with k_c = sqrt(|E - E_c| / h2m); open channels: O = G + iF, I = G - iF, F = x j_l(x), G = -x y_l(x), x = k r;
     closed channels (E < E_c) carry no incoming wave and their outgoing function is the decaying one, the eta = 0
     Whittaker function W(r) = x k_l(x), x = kappa r (modified spherical Bessel function of the second kind).
@@ -166,8 +169,8 @@ def collision_matrix(R, lval, ethr, energy, h2m, a):
     x = np.sqrt(np.abs(ekin) / h2m) * a
     O = np.zeros(nch, dtype=complex)
     dO = np.zeros(nch, dtype=complex)   # x * dO/dx = a * dO/dr at r = a
-    I = np.zeros(nch, dtype=complex)
-    dI = np.zeros(nch, dtype=complex)
+    Fr = np.zeros(nch)
+    dFr = np.zeros(nch)                 # x * dF/dx
     for c in range(nch):
         l, xc = int(lval[c]), x[c]
         if ekin[c] > 0:
@@ -176,13 +179,13 @@ def collision_matrix(R, lval, ethr, energy, h2m, a):
             G = -xc * spherical_yn(l, xc)
             dG = -spherical_yn(l, xc) - xc * spherical_yn(l, xc, derivative=True)
             O[c], dO[c] = G + 1j * F, xc * (dG + 1j * dF)
-            I[c], dI[c] = G - 1j * F, xc * (dG - 1j * dF)
+            Fr[c], dFr[c] = F, xc * dF
         else:
             W = xc * spherical_kn(l, xc)
             dW = spherical_kn(l, xc) + xc * spherical_kn(l, xc, derivative=True)
             O[c], dO[c] = W, xc * dW
     opn = np.nonzero(ekin > 0)[0]
     ZO = (np.diag(O) - R * dO[None, :]) / np.sqrt(x)[None, :]
-    ZI = ((np.diag(I) - R * dI[None, :]) / np.sqrt(x)[None, :])[:, opn]
-    Ufull = np.linalg.solve(ZO, ZI)
-    return Ufull[opn, :], opn
+    ZF = ((np.diag(Fr) - R * dFr[None, :]) / np.sqrt(x)[None, :])[:, opn]
+    Y = np.linalg.solve(ZO, ZF)
+    return np.eye(len(opn)) - 2j * Y[opn, :], opn

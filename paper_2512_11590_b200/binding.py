@@ -52,6 +52,7 @@ def lib():
         L.hprmat_last_cuda_error.restype = C.c_char_p
         L.hprmat_launch_count.restype = C.c_longlong
         L.hprmat_workspace_bytes.restype = C.c_size_t
+        L.hprmat_collision_workspace_bytes.restype = C.c_size_t
         _lib = L
     return _lib
 
@@ -227,6 +228,30 @@ def hprmat_cgemm_3xtf32(m, n, k, alpha, A_re, A_im, lda, B_re, B_im, ldb, beta, 
                                    _dev(A_im), C.c_int(lda), _dev(B_re), _dev(B_im), C.c_int(ldb), C.c_float(beta),
                                    _dev(C_re), _dev(C_im), C.c_int(ldc))
     _check(rc, "hprmat_cgemm_3xtf32")
+
+
+def hprmat_collision_workspace_bytes(nch) -> int:
+    return int(lib().hprmat_collision_workspace_bytes(C.c_int(nch)))
+
+
+def hprmat_collision(lval, ethr, energy, h2m, a, R, info_dev=None, ws=None, stream=None):
+    """Collision matrix of the open channels from the device R-matrix (neutral case).  R: torch complex128 CUDA tensor
+    holding the column-major nch x nch matrix.  Returns (U, nopen): U a torch complex128 CUDA tensor of nopen*nopen
+    elements (column-major) -- read U.view(nopen, nopen).T as the matrix."""
+    nch = len(lval)
+    if ws is None:
+        ws = torch.empty(hprmat_collision_workspace_bytes(nch) + 256, dtype=torch.uint8, device=R.device)
+    if info_dev is None:
+        info_dev = torch.zeros(1, dtype=torch.int32, device=R.device)
+    U = torch.empty(nch * nch, dtype=torch.complex128, device=R.device)
+    lv = (C.c_int * nch)(*[int(v) for v in lval])
+    et = (C.c_double * nch)(*[float(v) for v in ethr])
+    nopen = C.c_int(0)
+    rc = lib().hprmat_collision(_stream(stream), C.c_int(nch), lv, et, C.c_double(energy), C.c_double(h2m), C.c_double(a),
+                                _dev(R), _dev(U), C.byref(nopen), _dev(info_dev), _aligned(ws),
+                                C.c_size_t(ws.numel() - 256))
+    _check(rc, "hprmat_collision")
+    return U[:nopen.value * nopen.value], nopen.value
 
 
 def hprmat_zgetrf(n, A, lda, ipiv, info_dev, ws=None, stream=None):

@@ -471,3 +471,18 @@ def test_collision_matrix_reduces_to_the_all_open_formula_and_ignores_a_decouple
     U4, _ = oracle.collision_matrix(R4, lval, ethr, E, H2M, a)
     U3, _ = oracle.collision_matrix(R3, lval[:3], ethr[:3], E, H2M, a)
     assert np.abs(U4 - U3).max() < 1e-12
+
+
+def test_collision_matrix_stays_unitary_far_below_the_centrifugal_barrier():
+    """l = 12 at k a = 0.56 (G/F ~ 1e27): flux conservation and symmetry to rounding, which the literal (Z^O)^-1 Z^I form
+    cannot deliver in FP64 (reading R14); the barely penetrable channel decouples, |U_11| = 1."""
+    nb, a, E = 40, 8.0, 6.0
+    lval, ethr = [0, 12, 1], [0.0, 5.9, 3.0]
+    beta = np.array([[0.0, 12.0, 9.0], [12.0, 0.0, 15.0], [9.0, 15.0, 0.0]])
+    R = oracle.rmatrix(3, nb, a, H2M, lval, ethr, E, _ws_potential(nb, a, 3, beta))
+    U, opn = oracle.collision_matrix(R, lval, ethr, E, H2M, a)
+    assert len(opn) == 3
+    assert np.abs(U.conj().T @ U - np.eye(3)).max() < 1e-12
+    assert np.abs(U - U.T).max() < 1e-12
+    assert abs(abs(U[1, 1]) - 1.0) < 1e-12 and np.abs(U[1, [0, 2]]).max() < 1e-15
+    assert np.abs(U[0, 2]) > 1e-3
