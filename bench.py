@@ -345,10 +345,30 @@ def main():
                "e2e": {"value": world * lu_flops(N) / e2e_sec * 1e-12, "unit": UNIT, "seconds_per_step": e2e_sec,
                        "h2d_bytes_per_step": int(V_host.numel() * 16), "d2h_bytes_per_step": int(R_host.numel() * 16)},
                "gpu_launches": int(launches), "clocks": clocks, "roofline": roof}
+        res["_R"] = R.clone()
         ctx.destroy()
         del V, R, ctx
         torch.cuda.empty_cache()
         return res
+
+    def matching_leg(R):
+        """hprmat_collision on the R-matrix the timed steps produced: CUDA-event time of one call, which
+        holds the host evaluation of the 4 Nc channel constants, their upload, two small kernels and an Nc x Nc FP64 LU solve."""
+        ws = torch.empty(hb.hprmat_collision_workspace_bytes(w.nch) + 256, dtype=torch.uint8, device="cuda")
+        info_dev = torch.zeros(1, dtype=torch.int32, device="cuda")
+        reps, nopen = 10, 0
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        for it in range(2):
+            torch.cuda.synchronize()
+            ev[0].record()
+            for _ in range(reps):
+                U, nopen = hb.hprmat_collision(w.lval, w.ethr, E, w.h2m, w.a, R, info_dev=info_dev, ws=ws)
+            ev[1].record()
+            torch.cuda.synchronize()
+        Um = U.view(nopen, nopen)
+        return {"ms_per_call": ev[0].elapsed_time(ev[1]) / reps, "nch": w.nch, "nopen": nopen,
+                "zero_pivot": int(info_dev.item()), "max_abs_U": float(Um.abs().max().item()),
+                "asymmetry": float((Um - Um.T).abs().max().item())}
 
     def raw_zsolve(mode_name):
         """hprmat_zsolve alone (no assembly, no contraction) on a dense random diagonally shifted N x N system with Nc
@@ -376,9 +396,11 @@ def main():
         return out
 
     m = measure(args.mode)
+    R_last = m.pop("_R")
     others = {}
     if args.also != "none" and args.also != args.mode:
         others[args.also] = measure(args.also)
+        others[args.also].pop("_R")
 
     if rank == 0:
         line = {"metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -392,6 +414,8 @@ def main():
             line[k] = m[k]
         # the metric names FP64 AND mixed: the other precision mode, measured the same way in the same run
         line["other_modes"] = others
+        if world == 1:
+            line["matching"] = matching_leg(R_last)
         if args.zsolve and world == 1:
             line["raw_zsolve"] = [raw_zsolve("fp64"), raw_zsolve("mixed_refine")]
         line["paper_context"] = {"rtx3090_fp32_s": 3.554, "rtx3090_hybrid_s": 9.85, "xeon48_zgesv_s": 52.098,

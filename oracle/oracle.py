@@ -147,8 +147,31 @@ def rmatrix(nch, nb, a, h2m, lval, ethr, energy, V, mode: int = 0, nrefine: int 
     return out[0] if len(out) == 1 else tuple(out)
 
 
-def collision_matrix(R, lval, ethr, energy, h2m, a):
-    """Collision (S) matrix of the OPEN channels from the R-matrix at the channel radius, neutral case (eta = 0).
+def _coulomb_channel(l, eta, x, is_open):
+    """(F, x dF/dx, G, x dG/dx) of an open channel -- Coulomb wave functions F_l(eta, x), G_l(eta, x) -- or
+    (0, 0, 1, x W'/W) of a closed one, W = W_{-eta, l+1/2}(2x) the decaying Whittaker function (only its logarithmic
+    derivative matters: a column scale of Z^O drops out of the open rows).  mpmath at 30 digits; derivatives of F and G
+    from the textbook recurrence  u_l' = S_{l+1} u_l - R_{l+1} u_{l+1},  S_l = l/x + eta/l,  R_l = sqrt(1 + eta^2/l^2)
+    (Abramowitz & Stegun 14.2.2), the derivative of W numerically (mp.diff)."""
+    import mpmath as mp
+    with mp.workdps(30):
+        xm, em = mp.mpf(float(x)), mp.mpf(float(eta))
+        if is_open:
+            S = (l + 1) / xm + em / (l + 1)
+            Rr = mp.sqrt(1 + (em / (l + 1)) ** 2)
+            F, F1 = mp.coulombf(l, em, xm), mp.coulombf(l + 1, em, xm)
+            G, G1 = mp.coulombg(l, em, xm), mp.coulombg(l + 1, em, xm)
+            return float(F), float(xm * (S * F - Rr * F1)), float(G), float(xm * (S * G - Rr * G1))
+        W = mp.whitw(-em, l + mp.mpf(1) / 2, 2 * xm)
+        dW = mp.diff(lambda t: mp.whitw(-em, l + mp.mpf(1) / 2, 2 * t), xm)
+        return 0.0, 0.0, 1.0, float(xm * dW / W)
+
+
+def collision_matrix(R, lval, ethr, energy, h2m, a, zze2=None):
+    """Collision (S) matrix of the OPEN channels from the R-matrix at the channel radius.
+
+    zze2: None (neutral case, eta = 0) or the per-channel products Z1 Z2 e^2 (MeV fm); then the Sommerfeld parameter of
+    channel c is eta_c = zze2_c / (2 h2m k_c) and F, G are the Coulomb wave functions, W the Whittaker function (below).
 
     PAPER.md:35, 53, 71 name the step ("matching to asymptotic solutions", "collision matrix") without printing it; the
     reading taken (R14) is the standard one of the paper's ref. [2] (Descouvemont & Baye 2010):
@@ -160,7 +183,8 @@ def collision_matrix(R, lval, ethr, energy, h2m, a):
     with k_c = sqrt(|E - E_c| / h2m); open channels: O = G + iF, I = G - iF, F = x j_l(x), G = -x y_l(x), x = k r;
     closed channels (E < E_c) carry no incoming wave and their outgoing function is the decaying one, the eta = 0
     Whittaker function W(r) = x k_l(x), x = kappa r (modified spherical Bessel function of the second kind).
-    Returns (U, open) with U nopen x nopen and `open` the indices of the open channels.  Plain numpy / scipy.special.
+    Returns (U, open) with U nopen x nopen and `open` the indices of the open channels.  Plain numpy / scipy.special
+    (neutral case) or mpmath (charged case) for the channel functions.
     """
     from scipy.special import spherical_jn, spherical_yn, spherical_kn
     R = np.asarray(R, dtype=np.complex128)
@@ -171,9 +195,15 @@ def collision_matrix(R, lval, ethr, energy, h2m, a):
     dO = np.zeros(nch, dtype=complex)   # x * dO/dx = a * dO/dr at r = a
     Fr = np.zeros(nch)
     dFr = np.zeros(nch)                 # x * dF/dx
+    charged = zze2 is not None and np.any(np.asarray(zze2, dtype=float) != 0.0)
     for c in range(nch):
         l, xc = int(lval[c]), x[c]
-        if ekin[c] > 0:
+        if charged:
+            eta = float(zze2[c]) / (2.0 * h2m * (xc / a))
+            F, xdF, G, xdG = _coulomb_channel(l, eta, xc, ekin[c] > 0)
+            O[c], dO[c] = G + 1j * F, xdG + 1j * xdF
+            Fr[c], dFr[c] = F, xdF
+        elif ekin[c] > 0:
             F = xc * spherical_jn(l, xc)
             dF = spherical_jn(l, xc) + xc * spherical_jn(l, xc, derivative=True)
             G = -xc * spherical_yn(l, xc)

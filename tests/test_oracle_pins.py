@@ -486,3 +486,74 @@ def test_collision_matrix_stays_unitary_far_below_the_centrifugal_barrier():
     assert np.abs(U - U.T).max() < 1e-12
     assert abs(abs(U[1, 1]) - 1.0) < 1e-12 and np.abs(U[1, [0, 2]]).max() < 1e-15
     assert np.abs(U[0, 2]) > 1e-3
+
+
+# ----------------------------------------------------------------- charged case: Coulomb / Whittaker functions
+E2 = 1.43996  # e^2, MeV fm
+
+
+def test_coulomb_channel_functions_wronskian_and_neutral_limit():
+    """F'G - FG' = 1 (A&S 14.2.4) for the pair the oracle builds (function values and recurrence derivatives come from
+    different mpmath evaluations), and eta = 0 reproduces the Riccati-Bessel functions of the neutral branch."""
+    from oracle.oracle import _coulomb_channel
+    from scipy.special import spherical_jn, spherical_yn, spherical_kn
+    for l, eta, x in itertools.product([0, 1, 4, 11], [0.0, 0.3, 2.5, 8.0], [0.7, 4.0, 25.0]):
+        F, xdF, G, xdG = _coulomb_channel(l, eta, x, True)
+        assert abs((xdF * G - F * xdG) / x - 1.0) < 1e-12
+    for l, x in itertools.product([0, 2, 7], [0.5, 3.0, 12.0]):
+        F, xdF, G, xdG = _coulomb_channel(l, 0.0, x, True)
+        assert abs(F - x * spherical_jn(l, x)) < 1e-13 * max(1, abs(F)) and abs(G + x * spherical_yn(l, x)) < 1e-13 * abs(G)
+        _, _, one, xdW = _coulomb_channel(l, 0.0, x, False)
+        k, dk = spherical_kn(l, x), spherical_kn(l, x, derivative=True)
+        assert one == 1.0 and abs(xdW - x * (k + x * dk) / (x * k)) < 1e-12 * abs(xdW)
+
+
+def test_collision_matrix_charged_branch_reduces_to_neutral():
+    rng = np.random.default_rng(0)
+    R = rng.normal(size=(4, 4)) * 0.1
+    R = R + R.T + 0j
+    lval, ethr = [0, 2, 1, 3], [0.0, 1.5, 3.0, 9.0]
+    U0, _ = oracle.collision_matrix(R, lval, ethr, 6.0, H2M, 8.0)
+    U1, _ = oracle.collision_matrix(R, lval, ethr, 6.0, H2M, 8.0, zze2=[1e-300] * 4)     # forces the mpmath branch
+    assert np.abs(U0 - U1).max() < 1e-13
+
+
+def test_pure_coulomb_potential_scatters_nothing_relative_to_coulomb_waves():
+    """V_cc(r) = Z1 Z2 e^2 / r and nothing else, a different charge product per channel: the internal solution IS the
+    regular Coulomb function, so U = 1 (pins eta = zze2 / (2 h2m k), the Coulomb functions, their derivatives and the
+    per-channel indexing; accuracy = convergence of the Nb = 60 mesh)."""
+    nb, a, E = 60, 8.0, 6.0
+    lval, ethr = [0, 2, 1, 3], [0.0, 1.5, 3.0, 9.0]
+    zz = [2 * E2, 4 * E2, 1 * E2, 6 * E2]
+    r = oracle.mesh(nb, a)[2]
+    V = np.zeros((nb, 4, 4), dtype=complex)
+    for c in range(4):
+        V[:, c, c] = zz[c] / r
+    R = oracle.rmatrix(4, nb, a, H2M, lval, ethr, E, V)
+    U, opn = oracle.collision_matrix(R, lval, ethr, E, H2M, a, zze2=zz)
+    assert list(opn) == [0, 1, 2]
+    assert np.abs(U - np.eye(3)).max() < 1e-8
+
+
+@pytest.mark.parametrize("zz", [0.0, 3 * E2])
+def test_collision_matrix_does_not_depend_on_the_channel_radius(zz):
+    """Beyond the range of the nuclear potential U is independent of a -- but only if every channel is matched to the
+    right external solution: this pins the CLOSED-channel function (x k_l(x) / Whittaker), whose logarithmic derivative no
+    unitarity or decoupling test can see.  The closed channel lies 0.3 MeV below the energy (kappa a ~ 1), so its tail at a
+    is large: the correct functions agree to 1e-9 between the two radii, the growing solution gives 6e-4, eta dropped 5e-6,
+    a logarithmic derivative 5 % off 2e-6 (checked when the pin was written)."""
+    lval, ethr, E = [0, 1, 2], [0.0, 2.0, 6.3], 6.0
+    beta = np.array([[0.0, 30.0, 40.0], [30.0, 0.0, 35.0], [40.0, 35.0, 0.0]])
+    Us = []
+    for a, nb in [(9.0, 90), (11.0, 110)]:
+        r = oracle.mesh(nb, a)[2]
+        V = _ws_potential(nb, a, 3, beta, Rws=2.5, aws=0.25)
+        for c in range(3):
+            V[:, c, c] += zz / r
+        R = oracle.rmatrix(3, nb, a, H2M, lval, ethr, E, V)
+        U, opn = oracle.collision_matrix(R, lval, ethr, E, H2M, a, zze2=[zz] * 3 if zz else None)
+        assert list(opn) == [0, 1]
+        assert np.abs(U.conj().T @ U - np.eye(2)).max() < 1e-10
+        Us.append(U)
+    assert np.abs(Us[0][0, 1]) > 0.05
+    assert np.abs(Us[0] - Us[1]).max() < 5e-8
