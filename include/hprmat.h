@@ -108,26 +108,36 @@ int hprmat_destroy(hprmat_ctx *ctx);
 
 /* ---- matching at the channel radius ------------------------------------------------- */
 
-/* Collision matrix U of the open channels from the R-matrix, neutral case (eta = 0): PAPER.md:35, 53, 71 name the step
- * ("matching to asymptotic solutions", "collision matrix") and defer to the paper's ref. [2]; the formula taken is
- * DESIGN.md section 3, reading R14:
+/* Collision matrix U of the open channels from the R-matrix: PAPER.md:35, 53, 71 name the step ("matching to asymptotic
+ * solutions", "collision matrix") and defer to the paper's ref. [2]; the formula taken is DESIGN.md section 3, reading R14:
  *     Z^O_cc' = (k_c' a)^-1/2 [ O_c(a) delta_cc' - R_cc' a (dO_c'/dr)(a) ],  Z^I likewise,  U = open rows of (Z^O)^-1 Z^I,
- * with O = G + iF, I = G - iF (Riccati-Bessel functions of k_c a, k_c = sqrt((E - E_c)/h2m)) in an open channel and the
- * decaying solution kappa r k_l(kappa r), no incoming wave, in a closed one (E < E_c).
- * Evaluated as U = 1 - 2i (Z^O)^-1 Z^F (Z^I = Z^O - 2i Z^F), which stays accurate far below a centrifugal barrier.
+ * with O = G + iF, I = G - iF, F and G the Coulomb wave functions F_l(eta_c, k_c r), G_l(eta_c, k_c r),
+ * k_c = sqrt((E - E_c)/h2m), eta_c = zze2_c / (2 h2m k_c), in an open channel, and the decaying Whittaker function
+ * W_{-eta_c, l+1/2}(2 kappa_c r), no incoming wave, in a closed one (E < E_c).
+ * Evaluated as U = 1 - 2i (Z^O)^-1 Z^F (Z^I = Z^O - 2i Z^F), which stays accurate far below a barrier.
  *   nch, lval (host int[nch]), ethr (host double[nch], MeV), energy (MeV), h2m (MeV fm^2), a (fm): as in hprmat_setup
+ *   zze2   host double[nch]: Z1 Z2 e^2 of each channel, MeV fm (e^2 = 1.43996 MeV fm); NULL = neutral (eta = 0)
  *   R      dev, complex nch x nch column-major: the output of hprmat_solve at this energy (not modified)
  *   U      dev, complex nopen x nopen column-major, leading dimension nopen (output); open channels keep their order
  *   nopen  host int[1] (output): number of channels with energy > ethr[c]; known when the call returns
  *   info_dev  dev int[1]: 0, or the 1-based index of a zero pivot of Z^O (U is then meaningless)
  *   workspace dev, 256-byte aligned, >= hprmat_collision_workspace_bytes(nch); owned by the caller
- * The 4 nch channel constants are computed on the host in long double (recurrences in l) and uploaded; both matrices,
- * the FP64 LU solve (hprmat_zgetrf / hprmat_zgetrs code path) and the extraction run on the stream; no synchronisation.
- * Errors: negative = index of the offending argument (-5: energy equals a threshold, where k_c = 0), HPRMAT_ENOMEM,
- * HPRMAT_ECUDA. */
+ * The 4 nch channel constants are computed on the host in long double (hprmat_channel_functions) and uploaded; both
+ * matrices, the FP64 LU solve (hprmat_zgetrf / hprmat_zgetrs code path) and the extraction run on the stream; no
+ * synchronisation.
+ * Errors: negative = index of the offending argument (-6: energy equals a threshold, where k_c = 0, or lies so close to
+ * one that the continued fractions of the charged channel functions do not converge), HPRMAT_ENOMEM, HPRMAT_ECUDA. */
 size_t hprmat_collision_workspace_bytes(int nch);
-int hprmat_collision(void *cuda_stream, int nch, const int *lval, const double *ethr, double energy, double h2m, double a,
-                     const void *R, void *U, int *nopen, int *info_dev, void *workspace, size_t workspace_bytes);
+int hprmat_collision(void *cuda_stream, int nch, const int *lval, const double *ethr, const double *zze2, double energy,
+                     double h2m, double a, const void *R, void *U, int *nopen, int *info_dev, void *workspace,
+                     size_t workspace_bytes);
+
+/* Host-only helper (no CUDA call): the channel functions the matching uses, at x = k r (open) or kappa r (closed).
+ *   open != 0:  out[0..3] = F_l(eta, x), x dF/dx, G_l(eta, x), x dG/dx   (Coulomb wave functions; eta = 0: x j_l, -x y_l)
+ *   open == 0:  out[0..3] = 0, 0, 1, x W'/W   of W_{-eta, l+1/2}(2x)     (eta = 0: x k_l(x))
+ * Long double inside (Steed's continued fractions for eta != 0, Bessel recurrences for eta = 0), rounded to double.
+ * Returns 0, or minus the index of the offending argument (-3 also when x is too small for the continued fractions). */
+int hprmat_channel_functions(int l, double eta, double x, int open, double *out);
 
 /* ---- raw dense complex entries (PAPER.md:119 "take M, b, return c"; :125-137 ZGESV) -------------------------------- */
 

@@ -230,12 +230,21 @@ def hprmat_cgemm_3xtf32(m, n, k, alpha, A_re, A_im, lda, B_re, B_im, ldb, beta, 
     _check(rc, "hprmat_cgemm_3xtf32")
 
 
+def hprmat_channel_functions(l, eta, x, is_open=True):
+    """Host-only: (F, x dF/dx, G, x dG/dx) of an open channel or (0, 0, 1, x W'/W) of a closed one."""
+    out = (C.c_double * 4)()
+    rc = lib().hprmat_channel_functions(C.c_int(l), C.c_double(eta), C.c_double(x), C.c_int(1 if is_open else 0), out)
+    _check(rc, "hprmat_channel_functions")
+    return tuple(out)
+
+
 def hprmat_collision_workspace_bytes(nch) -> int:
     return int(lib().hprmat_collision_workspace_bytes(C.c_int(nch)))
 
 
-def hprmat_collision(lval, ethr, energy, h2m, a, R, info_dev=None, ws=None, stream=None):
-    """Collision matrix of the open channels from the device R-matrix (neutral case).  R: torch complex128 CUDA tensor
+def hprmat_collision(lval, ethr, energy, h2m, a, R, zze2=None, info_dev=None, ws=None, stream=None):
+    """Collision matrix of the open channels from the device R-matrix (zze2: per-channel Z1 Z2 e^2 in MeV fm, None =
+    neutral).  R: torch complex128 CUDA tensor
     holding the column-major nch x nch matrix.  Returns (U, nopen): U a torch complex128 CUDA tensor of nopen*nopen
     elements (column-major) -- read U.view(nopen, nopen).T as the matrix."""
     nch = len(lval)
@@ -247,7 +256,8 @@ def hprmat_collision(lval, ethr, energy, h2m, a, R, info_dev=None, ws=None, stre
     lv = (C.c_int * nch)(*[int(v) for v in lval])
     et = (C.c_double * nch)(*[float(v) for v in ethr])
     nopen = C.c_int(0)
-    rc = lib().hprmat_collision(_stream(stream), C.c_int(nch), lv, et, C.c_double(energy), C.c_double(h2m), C.c_double(a),
+    zz = None if zze2 is None else (C.c_double * nch)(*[float(v) for v in zze2])
+    rc = lib().hprmat_collision(_stream(stream), C.c_int(nch), lv, et, zz, C.c_double(energy), C.c_double(h2m), C.c_double(a),
                                 _dev(R), _dev(U), C.byref(nopen), _dev(info_dev), _aligned(ws),
                                 C.c_size_t(ws.numel() - 256))
     _check(rc, "hprmat_collision")

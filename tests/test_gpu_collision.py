@@ -1,5 +1,5 @@
 """Parity of hprmat_collision (collision matrix of the open channels from R, neutral
-case) with oracle.collision_matrix, through the C ABI.  Tolerance: max|U - U_orc| <= 1e-10 (|U| <= 1 for a unitary or
+and charged channels) with oracle.collision_matrix, through the C ABI.  Tolerance: max|U - U_orc| <= 1e-10 (|U| <= 1 for a unitary or
 absorptive problem, so absolute = relative to the scale of U); the channel constants are evaluated independently on the
 two sides (long double recurrences vs scipy.special)."""
 import numpy as np
@@ -18,9 +18,9 @@ def _dev_colmajor(a):
     return torch.from_numpy(np.ascontiguousarray(a.T)).to(DEV)
 
 
-def _U_gpu(lval, ethr, E, h2m, a, R_dev):
+def _U_gpu(lval, ethr, E, h2m, a, R_dev, zze2=None):
     info = torch.zeros(1, dtype=torch.int32, device=DEV)
-    U, nopen = hb.hprmat_collision(lval, ethr, E, h2m, a, R_dev, info_dev=info)
+    U, nopen = hb.hprmat_collision(lval, ethr, E, h2m, a, R_dev, zze2=zze2, info_dev=info)
     torch.cuda.synchronize()
     assert int(info.item()) == 0
     return U.cpu().numpy().reshape(nopen, nopen).T, nopen
@@ -92,7 +92,7 @@ def test_collision_edge_cases_and_errors():
     # energy exactly at a threshold
     with pytest.raises(hb.HprmatError) as e:
         hb.hprmat_collision([0, 1], [0.0, 3.0], 3.0, h2m, a, R)
-    assert e.value.code == -5
+    assert e.value.code == -6
     # negative orbital momentum
     with pytest.raises(hb.HprmatError) as e:
         hb.hprmat_collision([0, -1], [0.0, 3.0], 4.0, h2m, a, R)
@@ -121,4 +121,52 @@ def test_sub_barrier_channels_keep_unitarity_on_the_gpu():
     assert np.abs(Ug - Ug.T).max() < 1e-11
     Uo, _ = oracle.collision_matrix(oracle.rmatrix(3, nb, a, h2m, lval, ethr, E, V), lval, ethr, E, h2m, a)
     assert np.abs(Ug - Uo).max() <= 1e-10
+    ctx.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------- charged channels
+E2 = 1.43996
+
+
+@pytest.mark.parametrize("cfg,nch,nb,E,z1z2", [(0, None, None, 10.0, 2.0),    # all open, eta ~ 0.3
+                                               (0, None, None, 1.5, 8.0),     # two closed (Whittaker), eta ~ 3 under the barrier
+                                               (1, 24, 40, 9.0, 20.0),        # mixed open / closed, l up to 15, eta up to ~ 10
+                                               (2, 70, 30, 12.0, 6.0)])
+def test_charged_collision_matrix_end_to_end_parity(cfg, nch, nb, E, z1z2):
+    """Point-Coulomb repulsion added to the diagonal of the workload's potential; each channel gets its own charge product
+    (z1z2 (1 + c/nch)) so that a per-channel indexing slip cannot cancel."""
+    w = make_workload(cfg, nch=nch, nb=nb)
+    zz = z1z2 * E2 * (1.0 + np.arange(w.nch) / w.nch)
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << hb.HPRMAT_FP64)
+    r, _ = ctx.mesh()
+    V = w.potential(r)
+    idx = np.arange(w.nch)
+    V[:, idx, idx] += zz[None, :] / r[:, None]
+    R_dev, _ = ctx.solve(E, torch.from_numpy(V).to(DEV), mode=hb.HPRMAT_FP64)
+    Ug, nopen = _U_gpu(w.lval, w.ethr, E, w.h2m, w.a, R_dev, zze2=zz)
+    ro = oracle.mesh(w.nb, w.a)[2]
+    Vo = w.potential(ro)
+    Vo[:, idx, idx] += zz[None, :] / ro[:, None]
+    Ro = oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, Vo)
+    Uo, opn = oracle.collision_matrix(Ro, w.lval, w.ethr, E, w.h2m, w.a, zze2=zz)
+    assert nopen == len(opn)
+    assert np.abs(Ug - Uo).max() <= 1e-10
+    assert np.abs(Ug - Ug.T).max() <= 1e-10
+    ctx.destroy()
+
+
+def test_pure_coulomb_potential_gives_the_unit_matrix_on_the_gpu():
+    """V = Z1 Z2 e^2 / r only: U = 1 relative to Coulomb waves (oracle-independent; mesh convergence sets the 1e-8)."""
+    nb, a, h2m, E = 60, 8.0, 20.736 / 0.9, 6.0
+    lval, ethr = [0, 2, 1, 3], [0.0, 1.5, 3.0, 9.0]
+    zz = np.array([2.0, 4.0, 1.0, 6.0]) * E2
+    ctx = hb.Context(4, nb, a, h2m, lval, ethr, max_mode=1 << hb.HPRMAT_FP64)
+    r, _ = ctx.mesh()
+    V = np.zeros((nb, 4, 4), dtype=complex)
+    for c in range(4):
+        V[:, c, c] = zz[c] / r
+    R_dev, _ = ctx.solve(E, torch.from_numpy(V).to(DEV), mode=hb.HPRMAT_FP64)
+    Ug, nopen = _U_gpu(lval, ethr, E, h2m, a, R_dev, zze2=zz)
+    assert nopen == 3
+    assert np.abs(Ug - np.eye(3)).max() < 1e-8
     ctx.destroy()
