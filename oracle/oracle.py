@@ -147,6 +147,24 @@ def rmatrix(nch, nb, a, h2m, lval, ethr, energy, V, mode: int = 0, nrefine: int 
     return out[0] if len(out) == 1 else tuple(out)
 
 
+def rmatrix_nonlocal(nch, nb, a, h2m, lval, ethr, energy, W, return_x=False):
+    """R-matrix with NON-LOCAL potentials ("all blocks are full matrices").
+
+    W: N x N complex, index (c*nb + i) as everywhere: W[(c,i),(c',j)] = <f_i| W_cc' |f_j>, the matrix elements of the
+    potential in the Lagrange basis, MeV (for a kernel W_cc'(r,r') at the Gauss approximation of the Lagrange-mesh method:
+    a sqrt(lam_i lam_j) W_cc'(r_i, r_j); for a local potential V_cc'(r_i) delta_ij).  The matrix is Eq. (3)'s with the
+    potential blocks replaced by W:  C - E I = [kinetic + Bloch + centrifugal + threshold - E on the diagonal blocks] + W;
+    then Eq. (5), the Nc solves and the contraction exactly as in rmatrix() -- built from the same pinned pieces."""
+    N = nch * nb
+    W = np.asarray(W, dtype=np.complex128)
+    assert W.shape == (N, N)
+    x, lam, r, fa = mesh(nb, a)
+    C0 = assemble(nch, nb, a, h2m, lval, ethr, energy, np.zeros((nb, nch, nch), dtype=np.complex128))
+    X = solve(C0 + W, rhs(nch, nb, fa))
+    R = contract(nch, nb, a, h2m, fa, X)
+    return (R, X) if return_x else R
+
+
 def _coulomb_channel(l, eta, x, is_open):
     """(F, x dF/dx, G, x dG/dx) of an open channel -- Coulomb wave functions F_l(eta, x), G_l(eta, x) -- or
     (0, 0, 1, x W'/W) of a closed one, W = W_{-eta, l+1/2}(2x) the decaying Whittaker function (only its logarithmic

@@ -1,4 +1,6 @@
 // util.cu -- process-wide state behind the C ABI: error strings and the launch counter.
+#include <cstdio>
+#include <cstdlib>
 #include <vector>
 
 #include "common.cuh"
@@ -38,15 +40,20 @@ extern "C" int hprmat_profile_read(double *ms, double *flops, long long *launche
     double t = 0.0, f = 0.0;
     long long n = 0;
     for (int c = 0; c < hp::PROF_NCAT; ++c) { hp::g_cat_ms[c] = hp::g_cat_flops[c] = 0.0; hp::g_cat_n[c] = 0; }
+    // HPRMAT_PROF_DUMP=<file>: append one "category flops milliseconds" line per recorded launch (measurement aid)
+    const char *dump = getenv("HPRMAT_PROF_DUMP");
+    FILE *df = dump && *dump ? fopen(dump, "a") : nullptr;
     for (auto &r : hp::g_prof) {
-        if (cudaEventSynchronize(r.b) != cudaSuccess) return HPRMAT_ECUDA;
+        if (cudaEventSynchronize(r.b) != cudaSuccess) { if (df) fclose(df); return HPRMAT_ECUDA; }
         float m = 0.f;
         cudaEventElapsedTime(&m, r.a, r.b);
+        if (df) fprintf(df, "%d %.6e %.6f\n", r.cat, r.flops, m);
         hp::g_cat_ms[r.cat] += m; hp::g_cat_flops[r.cat] += r.flops; ++hp::g_cat_n[r.cat];
         if (r.flops > 0.0) { t += m; f += r.flops; ++n; }
         hp::g_prof_pool.push_back(r.a);
         hp::g_prof_pool.push_back(r.b);
     }
+    if (df) fclose(df);
     hp::g_prof.clear();
     if (ms) *ms = t;
     if (flops) *flops = f;

@@ -557,3 +557,39 @@ def test_collision_matrix_does_not_depend_on_the_channel_radius(zz):
         Us.append(U)
     assert np.abs(Us[0][0, 1]) > 0.05
     assert np.abs(Us[0] - Us[1]).max() < 5e-8
+
+
+# ----------------------------------------------------------------- non-local potentials
+def test_nonlocal_with_a_local_kernel_is_the_local_path():
+    """W = V(r_i) delta_ij in every block must reproduce rmatrix() (pins the index convention of W and the diagonal part)."""
+    w = make_workload(0, nch=3, nb=30)
+    E = 7.0
+    r = oracle.mesh(w.nb, w.a)[2]
+    V = w.potential(r)
+    W = np.zeros((w.n, w.n), dtype=complex)
+    for c1, c2 in itertools.product(range(3), range(3)):
+        W[c1 * w.nb + np.arange(w.nb), c2 * w.nb + np.arange(w.nb)] = V[:, c2, c1]
+    Rn = oracle.rmatrix_nonlocal(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, W)
+    Rl = oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, V)
+    assert np.abs(Rn - Rl).max() < 1e-13 * np.abs(Rl).max()
+
+
+@pytest.mark.parametrize("E", [0.5, 5.0, 30.0])
+def test_separable_potential_has_the_analytic_phase_shift(E):
+    """Rank-one kernel W(r,r') = -lambda exp(-beta r) exp(-beta r') (the s-wave Yamaguchi form), acting on u = r psi:
+    u'' + k^2 u = -Lambda c exp(-beta r), c = int_0^inf exp(-beta r) u dr, Lambda = lambda/h2m, solved by hand:
+        tan(delta) = Lambda k / [ (beta^2 + k^2)^2 + Lambda (k^2 - beta^2) / (2 beta) ].
+    A genuinely non-local problem with a closed form: pins the Gauss approximation a sqrt(lam_i lam_j) W(r_i, r_j), the full
+    (not diagonal) use of W, and the sign of the potential."""
+    nb, a, beta, lam0 = 60, 12.0, 2.0, 400.0
+    x, lam, r, fa = oracle.mesh(nb, a)
+    W = -lam0 * a * np.sqrt(np.outer(lam, lam)) * np.exp(-beta * (r[:, None] + r[None, :])) + 0j
+    R = oracle.rmatrix_nonlocal(1, nb, a, H2M, [0], [0.0], E, W)
+    U, _ = oracle.collision_matrix(R, [0], [0.0], E, H2M, a)
+    k = np.sqrt(E / H2M)
+    Lam = lam0 / H2M
+    tan_d = Lam * k / ((beta ** 2 + k ** 2) ** 2 + Lam * (k ** 2 - beta ** 2) / (2 * beta))
+    S_exact = (1 + 1j * tan_d) / (1 - 1j * tan_d)
+    assert abs(abs(U[0, 0]) - 1.0) < 1e-12
+    assert abs(tan_d) > 0.05
+    assert abs(U[0, 0] - S_exact) < 1e-8
