@@ -98,6 +98,20 @@ int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int ma
 int hprmat_solve_host(hprmat_ctx *ctx, double energy, const void *V_host, int mode, int max_refine, double tol,
                       void *R_host, hprmat_info *info);
 
+/* Non-local potentials ("all blocks are full matrices"): one energy point
+ * with a dense matrix of potential matrix elements instead of the mesh-diagonal V.
+ *   W    dev, complex N x N column-major, leading dimension ldw >= N, N = nch*nbasis, index (c*nbasis + i):
+ *        W[(c2*nbasis + j)*ldw + c1*nbasis + i] = <f_i| W_{c1 c2} |f_j>, MeV -- for a kernel W_{c1 c2}(r, r') at the Gauss
+ *        approximation of the Lagrange-mesh method  a sqrt(lambda_i lambda_j) W_{c1 c2}(r_i, r_j)  (lambda: the
+ *        Gauss-Legendre weights on (0,1)); a local potential is V_{c1 c2}(r_i) delta_ij.  Not modified.
+ *   mode HPRMAT_FP64 only (-5 otherwise; the context must have been set up with that mode)
+ *   max_refine, tol, R, info: as hprmat_solve.  The refinement residual B - (K + W) X is formed in working precision
+ *        (W X on the FP64 tensor cores): it restores the backward error, not digits beyond kappa 2^-53.
+ * The matrix is C - E I = W + [kinetic + Bloch + centrifugal + threshold - E on the diagonal blocks]; LU, solves,
+ * contraction and hprmat_get_x as in hprmat_solve. */
+int hprmat_solve_nonlocal(hprmat_ctx *ctx, double energy, const void *W, long ldw, int mode, int max_refine, double tol,
+                          void *R, hprmat_info *info);
+
 /* Solution block of the last hprmat_solve: X dev, complex N x nch column-major (copy out). */
 int hprmat_get_x(const hprmat_ctx *ctx, void *X);
 

@@ -154,6 +154,21 @@ class Context:
         _check(rc, "hprmat_solve", allow)
         return R, (info.as_dict() if want_info else None)
 
+    def solve_nonlocal(self, energy, W, ldw=None, mode=HPRMAT_FP64, max_refine=-1, tol=0.0, R=None, want_info=True,
+                       allow=(HPRMAT_OK,)):
+        """hprmat_solve_nonlocal: W torch complex128 CUDA tensor whose memory is the column-major N x N matrix."""
+        assert W.is_cuda and W.dtype == torch.complex128 and W.is_contiguous()
+        ldw = self.n if ldw is None else int(ldw)
+        assert W.numel() >= ldw * (self.n - 1) + self.n
+        if R is None:
+            R = torch.empty((self.nch, self.nch), dtype=torch.complex128, device=W.device)
+        info = hprmat_info() if want_info else None
+        rc = lib().hprmat_solve_nonlocal(self._h, C.c_double(energy), _dev(W), C.c_long(ldw), C.c_int(mode),
+                                         C.c_int(max_refine), C.c_double(tol), _dev(R),
+                                         C.byref(info) if want_info else None)
+        _check(rc, "hprmat_solve_nonlocal", allow)
+        return R, (info.as_dict() if want_info else None)
+
     def solve_host(self, energy, V_host, mode=HPRMAT_FP64, max_refine=-1, tol=0.0, R_host=None, allow=(HPRMAT_OK,)):
         """hprmat_solve_host: V and R are HOST buffers (numpy complex128); copies are inside the call."""
         V_host = np.ascontiguousarray(V_host, dtype=np.complex128)

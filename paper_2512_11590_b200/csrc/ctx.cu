@@ -436,6 +436,116 @@ int solve_mixed(hprmat_ctx *c, double energy, const double2 *V, bool refine, int
 
 }  // namespace
 
+// Non-local potentials: the same path with a dense potential matrix W.
+// Residual of the refinement: B - (K + W) X = [structured residual with V = 0, double-double] - W X, the product W X on the
+// FP64 tensor cores (the LU has overwritten C, W is the caller's and intact), i.e. a working-precision residual as in
+// LAPACK's refinement: it restores the backward error, it does not add digits beyond kappa * 2^-53.
+static int nonlocal_residual(hprmat_ctx *c, double energy, const double2 *W, long ldw, double *rmax_dev) {
+    cudaStream_t st = c->st;
+    const int N = c->n, nch = c->nch;
+    HP_TRY(structured_residual(st, c->tab, energy, c->d_V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, nullptr));
+    HP_TRY(gemm(st, N, nch, N, -1.0, ZView((double2 *)W, ldw), ZView(c->d_X, N), 1.0, ZView(c->d_Rr, N)));
+    if (rmax_dev) HP_TRY(maxabs(st, N, nch, c->d_Rr, N, rmax_dev));
+    return 0;
+}
+
+static int solve_nonlocal_fp64(hprmat_ctx *c, double energy, const double2 *W, long ldw, int max_refine, double tol,
+                               double2 *R, hprmat_info *info) {
+    cudaStream_t st = c->st;
+    const int N = c->n, nch = c->nch;
+    const bool timed = info != nullptr;
+    ZView A(c->d_C, N), X(c->d_X, N), D(c->d_Rr, N);
+    if (max_refine < 0) max_refine = 2;
+    if (!(tol > 0.0)) tol = 1e-13;
+    int steps = 0;
+
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[0], st));
+    HP_CUDA(cudaMemsetAsync(c->d_V, 0, sizeof(double2) * (size_t)c->nb * nch * nch, st));  // "no local potential"
+    HP_TRY(assemble_nonlocal(st, c->tab, energy, W, ldw, c->d_C, N));
+    if (timed) HP_TRY(dense_anorm(st, N, c->d_C, N, (double *)c->d_Rlo, c->d_scal + 4));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[1], st));
+    HP_CUDA(cudaMemsetAsync(c->d_info, 0, sizeof(int), st));
+    HP_TRY(getrf<ZView>(st, N, A, c->d_ipiv, c->d_info, c->wz));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[2], st));
+    if (timed) {
+        HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, sizeof(int), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        if (c->h_info[0] != 0) {
+            info->status = HPRMAT_ESINGULAR;
+            info->pivot_index = c->h_info[0];
+            return HPRMAT_ESINGULAR;
+        }
+    }
+    HP_TRY(build_rhs(st, c->tab, c->d_X, N));
+    HP_TRY(getrs<ZView>(st, N, nch, A, X, c->wz));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[3], st));
+    double dprev = 0.0;
+    if (timed && max_refine > 0) {
+        HP_TRY(maxabs(st, N, nch, c->d_X, N, c->d_scal + 2));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 2, c->d_scal + 2, sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        dprev = c->h_scal[2];
+    }
+    for (int k = 0; k < max_refine; ++k) {
+        HP_TRY(nonlocal_residual(c, energy, W, ldw, nullptr));
+        HP_TRY(getrs<ZView>(st, N, nch, A, D, c->wz));
+        HP_TRY(axpy_norm(st, N, nch, c->d_X, N, c->d_Rr, N, c->d_scal));
+        ++steps;
+        if (timed) {
+            HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+            HP_CUDA(cudaStreamSynchronize(st));
+            const double dn = c->h_scal[0], xn = c->h_scal[1];
+            const int v = refine_verdict(dn, xn, dprev, tol);
+            dprev = dn;
+            if (v != REF_CONTINUE) break;
+        }
+    }
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[4], st));
+    HP_TRY(contract(st, c->tab, c->d_X, N, R));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[5], st));
+    c->have_x = true;
+    if (timed) {
+        HP_TRY(nonlocal_residual(c, energy, W, ldw, c->d_scal + 3));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 3, c->d_scal + 3, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        double bn = 0.0;
+        for (double f : c->fa) bn = std::max(bn, fabs(f));
+        HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        info->status = HPRMAT_OK;
+        info->refine_steps = steps;
+        info->pivot_index = 0;
+        info->resid_max = c->h_scal[3];
+        info->backward_err = c->h_scal[5];
+        info->ms_assemble = ev_ms(c->ev[0], c->ev[1]);
+        info->ms_lu = ev_ms(c->ev[1], c->ev[2]);
+        info->ms_solve = ev_ms(c->ev[2], c->ev[3]);
+        info->ms_refine = ev_ms(c->ev[3], c->ev[4]);
+        info->ms_contract = ev_ms(c->ev[4], c->ev[5]);
+        info->ms_total = ev_ms(c->ev[0], c->ev[5]);
+        info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)N * N * N / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
+    }
+    return HPRMAT_OK;
+}
+
+extern "C" int hprmat_solve_nonlocal(hprmat_ctx *ctx, double energy, const void *W, long ldw, int mode, int max_refine,
+                                     double tol, void *R, hprmat_info *info) {
+    if (!ctx) return -1;
+    if (!W) return -3;
+    if (ldw < ctx->n) return -4;
+    if (mode != HPRMAT_FP64) return -5;  // the low-precision factorisation of the non-local matrix is not built yet
+    if (!(ctx->max_mode & (1 << HPRMAT_FP64))) return -5;
+    if (!R) return -8;
+    if (info) {
+        *info = hprmat_info();
+        info->backward_err = -1.0;
+    }
+    const int rc = solve_nonlocal_fp64(ctx, energy, (const double2 *)W, ldw, max_refine, tol, (double2 *)R, info);
+    if (info) info->status = rc;
+    return rc;
+}
+
 extern "C" int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int max_refine, double tol, void *R,
                             hprmat_info *info) {
     if (!ctx) return -1;

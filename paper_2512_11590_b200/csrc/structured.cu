@@ -53,6 +53,72 @@ int assemble_z(cudaStream_t st, const StructTables &t, double energy, const doub
     return 0;
 }
 
+// Non-local potentials (every block full): C = W + [kinetic + Bloch + centrifugal + threshold - E on the
+// diagonal blocks], W the caller's N x N matrix of potential matrix elements.  Same thread mapping as assemble_z_kernel; the
+// diagonal is evaluated as ((dg0 + (E_c - E)) + Re W_ii), the order of the local path.  Reads and writes 16 N^2 bytes each.
+__global__ void __launch_bounds__(ASM_NT) assemble_nonlocal_kernel(double2 *__restrict__ C, long ldc, int nch, int nb,
+                                                                   const double *__restrict__ hT,
+                                                                   const double *__restrict__ dg0,
+                                                                   const double *__restrict__ ethr, double energy,
+                                                                   const double2 *__restrict__ W, long ldw) {
+    const int N = nch * nb;
+    const int row = blockIdx.x * ASM_NT + threadIdx.x;
+    if (row >= N) return;
+    const int c1 = row / nb, i = row - c1 * nb;
+    const int col0 = blockIdx.y * ASM_CPT;
+    double2 w[ASM_CPT];
+#pragma unroll
+    for (int e = 0; e < ASM_CPT; ++e)
+        if (col0 + e < N) w[e] = W[(long)(col0 + e) * ldw + row];
+#pragma unroll
+    for (int e = 0; e < ASM_CPT; ++e) {
+        const int col = col0 + e;
+        if (col >= N) break;
+        const int c2 = col / nb, j = col - c2 * nb;
+        double2 v = w[e];
+        if (c1 == c2) {
+            if (i == j) v.x = __dadd_rn(__dadd_rn(dg0[row], __dsub_rn(ethr[c1], energy)), v.x);
+            else v.x = __dadd_rn(hT[(long)j * nb + i], v.x);
+        }
+        C[(long)col * ldc + row] = v;
+    }
+}
+
+int assemble_nonlocal(cudaStream_t st, const StructTables &t, double energy, const double2 *W, long ldw, double2 *C,
+                      long ldc) {
+    const int N = t.nch * t.nb;
+    dim3 grid(ceil_div(N, ASM_NT), ceil_div(N, ASM_CPT));
+    assemble_nonlocal_kernel<<<grid, ASM_NT, 0, st>>>(C, ldc, t.nch, t.nb, t.hT, t.dg0, t.ethr, energy, W, ldw);
+    HP_LAUNCHED();
+    return 0;
+}
+
+// ||A||_inf (max row sum of moduli) of a dense column-major matrix: one thread per row, a warp reads 512 contiguous bytes
+// of every column; columns are split over gridDim.y slices whose partial row sums meet in rowsum (pre-zeroed, n doubles).
+__global__ void __launch_bounds__(256) dense_rowsum_kernel(int n, const double2 *__restrict__ A, long lda,
+                                                           double *__restrict__ rowsum) {
+    const int row = blockIdx.x * 256 + threadIdx.x;
+    if (row >= n) return;
+    const int per = (n + gridDim.y - 1) / gridDim.y;
+    const int j0 = blockIdx.y * per, j1 = min(n, j0 + per);
+    double s = 0.0;
+#pragma unroll 4
+    for (int j = j0; j < j1; ++j) {
+        const double2 v = A[(long)j * lda + row];
+        s += sqrt(v.x * v.x + v.y * v.y);
+    }
+    atomicAdd(rowsum + row, s);
+}
+
+int dense_anorm(cudaStream_t st, int n, const double2 *A, long lda, double *rowsum_scratch, double *out_dev) {
+    HP_CUDA(cudaMemsetAsync(rowsum_scratch, 0, sizeof(double) * (size_t)n, st));
+    dim3 grid(ceil_div(n, 256), std::max(1, std::min(64, n / 256)));
+    dense_rowsum_kernel<<<grid, 256, 0, st>>>(n, A, lda, rowsum_scratch);
+    HP_LAUNCHED();
+    HP_CUDA(cudaMemsetAsync(out_dev, 0, sizeof(double), st));
+    return maxabs_real(st, n, rowsum_scratch, out_dev);
+}
+
 // ---------------------------------------------------------------------------------------------------- right-hand side
 __global__ void rhs_kernel(double2 *__restrict__ B, long ldb, int nch, int nb, const double *__restrict__ fa) {
     const long N = (long)nch * nb;
@@ -317,6 +383,23 @@ int maxabs(cudaStream_t st, long rows, int cols, const double2 *X, long ldx, dou
     if (tot <= 0) return 0;
     const int grid = (int)std::min<long>(ceil_div(tot, 256), 148L * 8);
     maxabs_kernel<<<grid, 256, 0, st>>>(rows, cols, X, ldx, out_dev);
+    HP_LAUNCHED();
+    return 0;
+}
+
+__global__ void __launch_bounds__(256) maxabs_real_kernel(long n, const double *__restrict__ x, double *out) {
+    __shared__ double shred[32];
+    double m = 0.0;
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) m = fmax(m, fabs(x[i]));
+    m = block_max(m, shred);
+    if (threadIdx.x == 0) atomic_max_nonneg(out, m);
+}
+
+// out (pre-zeroed by the caller) <- max(out, max_i |x_i|)
+int maxabs_real(cudaStream_t st, long n, const double *x, double *out_dev) {
+    if (n <= 0) return 0;
+    const int grid = (int)std::min<long>(ceil_div(n, 256), 148L * 8);
+    maxabs_real_kernel<<<grid, 256, 0, st>>>(n, x, out_dev);
     HP_LAUNCHED();
     return 0;
 }

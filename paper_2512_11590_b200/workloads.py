@@ -94,6 +94,40 @@ def make_workload(cfg: int, nch: int | None = None, nb: int | None = None, seed:
                     R_ws=t["R_ws"], modes=t["modes"])
 
 
+BETA_NL = 0.85   # fm, range of the non-locality (the Perey-Buck value)
+
+
+def nonlocal_matrix(w: "Workload", r, xp=np):
+    """Synthetic NON-LOCAL potential for SURVEY.md 8(f) row 4, Perey-Buck form built from the workload's local form factors:
+        W_cc'(r, r') = U_cc'((r + r')/2) exp(-((r - r')/BETA_NL)^2) / (sqrt(pi) BETA_NL),
+        U_cc = -(V0 + i W0) f(s),  U_cc' = beta_cc' df/ds (c != c'),
+    returned as the N x N matrix of Lagrange-mesh matrix elements  a sqrt(lam_i lam_j) W_cc'(r_i, r_j)  (Gauss
+    approximation; lam = Gauss-Legendre weights on (0,1) from numpy's leggauss), as an array of shape (nch, nb, nch, nb)
+    indexed [c2, j, c1, i] -- its memory is the column-major N x N matrix with index c*nb + i.  Input generation only (no
+    arithmetic of the method); xp = numpy, or torch for a device-resident build (r then a torch tensor on that device)."""
+    lam = np.polynomial.legendre.leggauss(w.nb)[1] / 2.0
+    if xp is np:
+        r = np.asarray(r, dtype=np.float64)
+        lamx, beta = lam, w.beta.astype(np.complex128)
+    else:
+        lamx = xp.as_tensor(lam, dtype=xp.float64, device=r.device)
+        beta = xp.as_tensor(w.beta, dtype=xp.complex128, device=r.device)
+    s = 0.5 * (r[:, None] + r[None, :])                     # [j, i]
+    u = xp.exp((s - w.R_ws) / A_WS)
+    f = 1.0 / (1.0 + u)
+    df = -u / (A_WS * (1.0 + u) ** 2)
+    g = xp.exp(-((r[:, None] - r[None, :]) / BETA_NL) ** 2) / (np.sqrt(np.pi) * BETA_NL)
+    g = g * (w.a * xp.sqrt(lamx[:, None] * lamx[None, :]))
+    Gdf = (g * df) + 0j
+    Gf = (g * f) * (-(w.V0 + 1j * w.W0))
+    shape = (w.nch, w.nb, w.nch, w.nb)
+    W = np.empty(shape, dtype=np.complex128) if xp is np else xp.empty(shape, dtype=xp.complex128, device=r.device)
+    W[...] = beta.T[:, None, :, None] * Gdf[None, :, None, :]   # [c2, j, c1, i] = beta[c1, c2] Gdf[j, i]; beta_cc = 0
+    for c in range(w.nch):
+        W[c, :, c, :] = Gf
+    return W
+
+
 def dense_test_matrix(n: int, nrhs: int, seed: int, shift: float | None = None):
     """Well-conditioned dense complex test system for the raw solve entry: A = G + shift*I with G_ij ~ U(-1,1) +
     i U(-1,1), x_exact = 1 (PAPER.md:563 manufactured solution), B = A @ 1 is left to the caller (it is arithmetic)."""
