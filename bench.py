@@ -215,6 +215,9 @@ def main():
     ap.add_argument("--zsolve", action="store_true",
                     help="also time hprmat_zsolve alone on a dense random N x N system (raw solve, separately from assembly "
                          "and contraction)")
+    ap.add_argument("--nonlocal", dest="nonlocal_leg", action="store_true",
+                    help="also time hprmat_solve_nonlocal (FP64, SURVEY 8(f) row 4) on the config with the synthetic Perey-Buck-type "
+                         "non-local potential of workloads.nonlocal_matrix, built on the device")
     ap.add_argument("--also", default="mixed_refine", choices=["none", "fp64", "mixed", "mixed_refine"],
                     help="a second precision mode measured in the same run and reported under other_modes")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -395,6 +398,32 @@ def main():
         torch.cuda.empty_cache()
         return out
 
+    def nonlocal_leg():
+        """hprmat_solve_nonlocal, FP64: W (16 N^2 B) resident in HBM, `steps` timed calls after one warm-up, CUDA events."""
+        from paper_2512_11590_b200.workloads import nonlocal_matrix
+        ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << hb.HPRMAT_FP64)
+        r, _ = ctx.mesh()
+        W = nonlocal_matrix(w, torch.from_numpy(r).to("cuda"), xp=torch)
+        R = torch.empty((w.nch, w.nch), dtype=torch.complex128, device="cuda")
+        _, info = ctx.solve_nonlocal(E, W, R=R)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for _ in range(args.steps):
+            ctx.solve_nonlocal(E, W, R=R, want_info=False)
+        ev[1].record()
+        torch.cuda.synchronize()
+        sec = ev[0].elapsed_time(ev[1]) * 1e-3 / args.steps
+        out = {"mode": "fp64", "time_to_rmatrix_s": sec, "value": lu_flops(N) / sec * 1e-12, "unit": UNIT,
+               "lu_tflops": info["lu_tflops"], "refine_steps_unconditional": 2, "backward_err": info["backward_err"],
+               "stages_ms_of_the_synchronised_call": {k: info[k] for k in ("ms_assemble", "ms_lu", "ms_solve", "ms_refine",
+                                                                            "ms_contract", "ms_total")},
+               "workload": "Perey-Buck-type kernel (range 0.85 fm) built from the config's form factors, every block full"}
+        ctx.destroy()
+        del W
+        torch.cuda.empty_cache()
+        return out
+
     m = measure(args.mode)
     R_last = m.pop("_R")
     others = {}
@@ -416,6 +445,8 @@ def main():
         line["other_modes"] = others
         if world == 1:
             line["matching"] = matching_leg(R_last)
+        if args.nonlocal_leg and world == 1:
+            line["nonlocal"] = nonlocal_leg()
         if args.zsolve and world == 1:
             line["raw_zsolve"] = [raw_zsolve("fp64"), raw_zsolve("mixed_refine")]
         line["paper_context"] = {"rtx3090_fp32_s": 3.554, "rtx3090_hybrid_s": 9.85, "xeon48_zgesv_s": 52.098,

@@ -109,3 +109,31 @@ def test_nonlocal_argument_errors_and_unsynchronised_call():
     assert e.value.code == -5
     ctx.destroy()
     ctx2.destroy()
+
+
+def test_nonlocal_full_size_properties():
+    """BASELINE.json configs[3] (Nc = 256, Nb = 100, N = 25600) with the non-local workload built on the device; the oracle
+    cannot reach this size, so what holds at any size is checked: backward error, symmetry of R, convergence status, and the
+    collision matrix of the absorptive problem (singular values <= 1, U = U^T)."""
+    w = make_workload(3)
+    E = float(w.energies[0])
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << hb.HPRMAT_FP64)
+    r, _ = ctx.mesh()
+    W_dev = nonlocal_matrix(w, torch.from_numpy(r).to(DEV), xp=torch)
+    assert W_dev.is_contiguous() and W_dev.numel() == w.n * w.n
+    R_dev, info = ctx.solve_nonlocal(E, W_dev)
+    assert info["status"] == hb.HPRMAT_OK
+    assert 0 <= info["backward_err"] <= 50 * w.n * 2.0 ** -53
+    Rg = R_dev.cpu().numpy().T
+    assert np.all(np.isfinite(Rg.real)) and np.all(np.isfinite(Rg.imag))
+    assert _relmax(Rg, Rg.T) <= 1e-10
+    U, nopen = hb.hprmat_collision(w.lval, w.ethr, E, w.h2m, w.a, R_dev)
+    Ug = U.cpu().numpy().reshape(nopen, nopen).T
+    assert nopen == int(np.sum(E > w.ethr))
+    assert np.abs(Ug - Ug.T).max() <= 1e-10
+    assert np.linalg.svd(Ug, compute_uv=False).max() <= 1.0 + 1e-10
+    print(f"non-local cfg3: lu {info['ms_lu']:.1f} ms, total {info['ms_total']:.1f} ms, backward error {info['backward_err']:.2e}, "
+          f"refine steps {info['refine_steps']}")
+    ctx.destroy()
+    del W_dev
+    torch.cuda.empty_cache()
