@@ -462,7 +462,7 @@ static int solve_nonlocal_fp64(hprmat_ctx *c, double energy, const double2 *W, l
     if (timed) HP_CUDA(cudaEventRecord(c->ev[0], st));
     HP_CUDA(cudaMemsetAsync(c->d_V, 0, sizeof(double2) * (size_t)c->nb * nch * nch, st));  // "no local potential"
     HP_TRY(assemble_nonlocal(st, c->tab, energy, W, ldw, c->d_C, N));
-    if (timed) HP_TRY(dense_anorm(st, N, c->d_C, N, (double *)c->d_Rlo, c->d_scal + 4));
+    if (timed) HP_TRY(nonlocal_anorm(st, c->tab, energy, W, ldw, (double *)c->d_Rlo, c->d_scal + 4));
     if (timed) HP_CUDA(cudaEventRecord(c->ev[1], st));
     HP_CUDA(cudaMemsetAsync(c->d_info, 0, sizeof(int), st));
     HP_TRY(getrf<ZView>(st, N, A, c->d_ipiv, c->d_info, c->wz));
@@ -529,19 +529,111 @@ static int solve_nonlocal_fp64(hprmat_ctx *c, double energy, const double2 *W, l
     return HPRMAT_OK;
 }
 
+// Mixed modes with non-local potentials: the block-diagonal preconditioner uses the full diagonal blocks K_c + W_cc, S has
+// full off-diagonal blocks Kinv_c W_cc'; the rest is solve_mixed with the working-precision dense residual.
+static int solve_nonlocal_mixed(hprmat_ctx *c, double energy, const double2 *W, long ldw, bool refine, int max_refine,
+                                double tol, double2 *R, hprmat_info *info) {
+    cudaStream_t st = c->st;
+    const int N = c->n, nch = c->nch, nb = c->nb;
+    const bool timed = info != nullptr;
+    CView S(c->d_Sre, c->d_Sim, c->ldS), Bs(c->d_Bre, c->d_Bim, c->ldS);
+    if (max_refine < 0) max_refine = 5;
+    if (!refine) max_refine = 0;
+    if (!(tol > 0.0)) tol = 1e-12;
+    int status = HPRMAT_OK, steps = 0;
+
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[0], st));
+    HP_CUDA(cudaMemsetAsync(c->d_V, 0, sizeof(double2) * (size_t)nb * nch * nch, st));  // "no local potential"
+    HP_CUDA(cudaMemsetAsync(c->d_info, 0, 2 * sizeof(int), st));
+    HP_TRY(precond_invert(st, c->tab, energy, c->d_V, c->d_Kinv, c->d_info + 1, W, ldw));
+    HP_TRY(precond_assemble_nonlocal(st, c->tab, c->d_Kinv, W, ldw, S, c->d_Rlo, N));
+    if (timed) HP_TRY(nonlocal_anorm(st, c->tab, energy, W, ldw, (double *)c->d_Rlo, c->d_scal + 4));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[1], st));
+    HP_TRY(getrf<CView>(st, N, S, c->d_ipiv, c->d_info, c->wc));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[2], st));
+    if (timed) {
+        HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        if (c->h_info[0] != 0 || c->h_info[1] != 0) {
+            info->status = HPRMAT_ESINGULAR;
+            info->pivot_index = c->h_info[0] ? c->h_info[0] : c->h_info[1];
+            return HPRMAT_ESINGULAR;
+        }
+    }
+    HP_TRY(precond_rhs(st, c->tab, c->d_Kinv, Bs));
+    HP_TRY(getrs<CView>(st, N, nch, S, Bs, c->wc));
+    HP_TRY(promote_add(st, N, nch, c->d_X, N, Bs, false, c->d_scal));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[3], st));
+    double dprev = 0.0;
+    if (max_refine > 0) {
+        HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        dprev = c->h_scal[1];
+        status = HPRMAT_ENOTCONVERGED;
+    }
+    for (int k = 0; k < max_refine; ++k) {
+        HP_TRY(nonlocal_residual(c, energy, W, ldw, nullptr));
+        HP_TRY(zgemm_batched(st, nb, nch, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, c->d_Rr, N, nb, 0.0, c->d_Rlo, N, nb, nch));
+        HP_TRY(demote(st, N, nch, c->d_Rlo, N, Bs));
+        HP_TRY(getrs<CView>(st, N, nch, S, Bs, c->wc));
+        HP_TRY(promote_add(st, N, nch, c->d_X, N, Bs, true, c->d_scal));
+        ++steps;
+        HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        const double dn = c->h_scal[0], xn = c->h_scal[1];
+        const int v = refine_verdict(dn, xn, dprev, tol);
+        dprev = dn;
+        if (v == REF_CONVERGED) { status = HPRMAT_OK; break; }
+        if (v == REF_STAGNATED) {
+            status = (dn <= 64.0 * 2.220446049250313e-16 * xn) ? HPRMAT_OK : HPRMAT_ENOTCONVERGED;
+            break;
+        }
+    }
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[4], st));
+    HP_TRY(contract(st, c->tab, c->d_X, N, R));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[5], st));
+    c->have_x = true;
+    if (timed) {
+        HP_TRY(nonlocal_residual(c, energy, W, ldw, c->d_scal + 3));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 3, c->d_scal + 3, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        double bn = 0.0;
+        for (double f : c->fa) bn = std::max(bn, fabs(f));
+        HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        info->status = status;
+        info->refine_steps = steps;
+        info->pivot_index = 0;
+        info->resid_max = c->h_scal[3];
+        info->backward_err = c->h_scal[5];
+        info->ms_assemble = ev_ms(c->ev[0], c->ev[1]);
+        info->ms_lu = ev_ms(c->ev[1], c->ev[2]);
+        info->ms_solve = ev_ms(c->ev[2], c->ev[3]);
+        info->ms_refine = ev_ms(c->ev[3], c->ev[4]);
+        info->ms_contract = ev_ms(c->ev[4], c->ev[5]);
+        info->ms_total = ev_ms(c->ev[0], c->ev[5]);
+        info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)N * N * N / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
+    }
+    return status;
+}
+
 extern "C" int hprmat_solve_nonlocal(hprmat_ctx *ctx, double energy, const void *W, long ldw, int mode, int max_refine,
                                      double tol, void *R, hprmat_info *info) {
     if (!ctx) return -1;
     if (!W) return -3;
     if (ldw < ctx->n) return -4;
-    if (mode != HPRMAT_FP64) return -5;  // the low-precision factorisation of the non-local matrix is not built yet
-    if (!(ctx->max_mode & (1 << HPRMAT_FP64))) return -5;
+    if (mode != HPRMAT_FP64 && mode != HPRMAT_MIXED && mode != HPRMAT_MIXED_REFINE) return -5;
+    if (!(ctx->max_mode & (1 << mode))) return -5;
     if (!R) return -8;
     if (info) {
         *info = hprmat_info();
         info->backward_err = -1.0;
     }
-    const int rc = solve_nonlocal_fp64(ctx, energy, (const double2 *)W, ldw, max_refine, tol, (double2 *)R, info);
+    const int rc = mode == HPRMAT_FP64
+                       ? solve_nonlocal_fp64(ctx, energy, (const double2 *)W, ldw, max_refine, tol, (double2 *)R, info)
+                       : solve_nonlocal_mixed(ctx, energy, (const double2 *)W, ldw, mode == HPRMAT_MIXED_REFINE, max_refine, tol,
+                                              (double2 *)R, info);
     if (info) info->status = rc;
     return rc;
 }

@@ -8,6 +8,7 @@
 // and solves  S X = K_d^-1 B;  the FP64 residual of the refinement is always that of the ORIGINAL system
 // (PAPER.md:151, 222), mapped through K_d^-1 before the low-precision correction solve.
 #include "precond.cuh"
+#include "lu.cuh"
 
 namespace hp {
 
@@ -18,7 +19,8 @@ constexpr int KI_NT = 512;
 
 __global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const double *__restrict__ hT,
                                                      const double *__restrict__ dg0, const double *__restrict__ ethr,
-                                                     double energy, const double2 *__restrict__ V, double2 *__restrict__ Kinv,
+                                                     double energy, const double2 *__restrict__ V,
+                                                     const double2 *__restrict__ W, long ldw, double2 *__restrict__ Kinv,
                                                      int use_smem, int *info) {
     extern __shared__ __align__(16) unsigned char smraw[];
     const int c = blockIdx.x, n = nb, tid = threadIdx.x;
@@ -34,7 +36,12 @@ __global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const doub
     for (int idx = tid; idx < n * n; idx += KI_NT) {
         const int i = idx % n, j = idx / n;
         double2 v = make_double2(hT[(size_t)j * n + i], 0.0);
-        if (i == j) {
+        if (W) {  // non-local potentials: the full diagonal block of W is added (same rounding order as the assembly)
+            const double2 wv = W[((size_t)c * n + j) * ldw + (size_t)c * n + i];
+            const double base = (i == j) ? __dadd_rn(dg0[(size_t)c * n + i], __dsub_rn(ethr[c], energy)) : v.x;
+            v.x = __dadd_rn(base, wv.x);
+            v.y = wv.y;
+        } else if (i == j) {
             const double2 vd = V[((size_t)i * nch + c) * nch + c];
             const double d2 = __dadd_rn(dg0[(size_t)c * n + i], __dsub_rn(ethr[c], energy));
             v.x = __dadd_rn(d2, vd.x);
@@ -111,7 +118,8 @@ __global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const doub
         for (int idx = tid; idx < n * n; idx += KI_NT) out[idx] = a[idx];
 }
 
-int precond_invert(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double2 *Kinv, int *info_dev) {
+int precond_invert(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double2 *Kinv, int *info_dev,
+                   const double2 *W, long ldw) {
     const int n = t.nb;
     const size_t small = sizeof(double2) * 2 * n + sizeof(int) * ((n + 3) & ~3);
     const size_t full = small + sizeof(double2) * (size_t)n * n;
@@ -122,7 +130,7 @@ int precond_invert(cudaStream_t st, const StructTables &t, double energy, const 
         HP_CUDA(cudaFuncSetAttribute(kinv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured = smem;
     }
-    kinv_kernel<<<t.nch, KI_NT, smem, st>>>(t.nch, n, t.hT, t.dg0, t.ethr, energy, V, Kinv, use_smem, info_dev);
+    kinv_kernel<<<t.nch, KI_NT, smem, st>>>(t.nch, n, t.hT, t.dg0, t.ethr, energy, V, W, ldw, Kinv, use_smem, info_dev);
     HP_LAUNCHED();
     return 0;
 }
@@ -166,6 +174,44 @@ int precond_assemble(cudaStream_t st, const StructTables &t, const double2 *Kinv
     dim3 grid(ceil_div(N, SA_NT), t.nb, ceil_div(t.nch, SA_CC));
     assemble_s_kernel<<<grid, SA_NT, 0, st>>>(t.nch, t.nb, Kinv, V, S.re, S.im, S.ld);
     HP_LAUNCHED();
+    return 0;
+}
+
+// Non-local potentials: S = K_d^-1 (C - E I) with full blocks.  Block row c of S is Kinv_c times block row c of W for the
+// off-diagonal blocks and the identity on the diagonal block.  The products run on the FP64 tensor cores, one column chunk
+// of nch columns at a time (nch batched nb x nch x nb GEMMs into the N x nch scratch T), and this kernel demotes the chunk
+// into the float planes, writing the identity where the column lies in the row's own channel.
+__global__ void __launch_bounds__(256) demote_offdiag_kernel(int nch, int nb, int j0, int w, const double2 *__restrict__ T,
+                                                             long ldt, float *__restrict__ Sre, float *__restrict__ Sim,
+                                                             long ld) {
+    const long N = (long)nch * nb;
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= N * w) return;
+    const int q = (int)(idx / N);
+    const long row = idx - (long)q * N;
+    const int col = j0 + q;
+    float re, im;
+    if (row / nb == col / nb) {
+        re = (row == col) ? 1.f : 0.f;
+        im = 0.f;
+    } else {
+        const double2 v = T[(long)q * ldt + row];
+        re = (float)v.x;
+        im = (float)v.y;
+    }
+    Sre[(long)col * ld + row] = re;
+    Sim[(long)col * ld + row] = im;
+}
+
+int precond_assemble_nonlocal(cudaStream_t st, const StructTables &t, const double2 *Kinv, const double2 *W, long ldw, CView S,
+                              double2 *T, long ldt) {
+    const int nch = t.nch, nb = t.nb, N = nch * nb;
+    for (int j0 = 0; j0 < N; j0 += nch) {
+        const int w = std::min(nch, N - j0);
+        HP_TRY(zgemm_batched(st, nb, w, nb, 1.0, Kinv, nb, (long)nb * nb, W + (long)j0 * ldw, ldw, nb, 0.0, T, ldt, nb, nch));
+        demote_offdiag_kernel<<<ceil_div((long)N * w, 256), 256, 0, st>>>(nch, nb, j0, w, T, ldt, S.re, S.im, S.ld);
+        HP_LAUNCHED();
+    }
     return 0;
 }
 

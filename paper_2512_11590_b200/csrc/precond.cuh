@@ -6,9 +6,14 @@ namespace hp {
 
 // Kinv[c] <- K_c^-1, K_c = diagonal block c of C - E*I (nb x nb complex128, column-major, blocks contiguous).
 // info_dev (pre-zeroed by the caller) receives c*nb + k + 1 if block c has no non-zero pivot at step k.
-int precond_invert(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double2 *Kinv, int *info_dev);
+// W != nullptr (non-local potentials): K_c = kinetic/diagonal terms + the full diagonal block (c,c) of the N x N matrix W
+int precond_invert(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double2 *Kinv, int *info_dev,
+                   const double2 *W = nullptr, long ldw = 0);
 // S <- K_d^-1 (C - E*I) in split complex64 (identity diagonal blocks, Kinv_c * diag V_cc' elsewhere)
 int precond_assemble(cudaStream_t st, const StructTables &t, const double2 *Kinv, const double2 *V, CView S);
+// non-local potentials: S <- K_d^-1 (C - E*I) with full blocks of W; T: N x nch complex128 scratch (ld ldt)
+int precond_assemble_nonlocal(cudaStream_t st, const StructTables &t, const double2 *Kinv, const double2 *W, long ldw, CView S,
+                              double2 *T, long ldt);
 // B <- K_d^-1 * (surface right-hand sides), split complex64, N x nch
 int precond_rhs(cudaStream_t st, const StructTables &t, const double2 *Kinv, CView B);
 // D <- (complex64) Z

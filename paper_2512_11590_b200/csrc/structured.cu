@@ -93,27 +93,41 @@ int assemble_nonlocal(cudaStream_t st, const StructTables &t, double energy, con
     return 0;
 }
 
-// ||A||_inf (max row sum of moduli) of a dense column-major matrix: one thread per row, a warp reads 512 contiguous bytes
-// of every column; columns are split over gridDim.y slices whose partial row sums meet in rowsum (pre-zeroed, n doubles).
-__global__ void __launch_bounds__(256) dense_rowsum_kernel(int n, const double2 *__restrict__ A, long lda,
-                                                           double *__restrict__ rowsum) {
+// ||W + diagonal-block terms||_inf (max row sum of moduli) without forming the matrix: one thread per row, a warp reads 512
+// contiguous bytes of every column of W; columns are split over gridDim.y slices whose partial row sums meet in rowsum
+// (pre-zeroed, N doubles).
+__global__ void __launch_bounds__(256) nonlocal_rowsum_kernel(int nch, int nb, const double *__restrict__ hT,
+                                                              const double *__restrict__ dg0,
+                                                              const double *__restrict__ ethr, double energy,
+                                                              const double2 *__restrict__ W, long ldw,
+                                                              double *__restrict__ rowsum) {
+    const int n = nch * nb;
     const int row = blockIdx.x * 256 + threadIdx.x;
     if (row >= n) return;
+    const int c1 = row / nb, i = row - c1 * nb;
     const int per = (n + gridDim.y - 1) / gridDim.y;
     const int j0 = blockIdx.y * per, j1 = min(n, j0 + per);
+    const double dterm = __dadd_rn(dg0[row], __dsub_rn(ethr[c1], energy));
     double s = 0.0;
 #pragma unroll 4
-    for (int j = j0; j < j1; ++j) {
-        const double2 v = A[(long)j * lda + row];
+    for (int col = j0; col < j1; ++col) {
+        double2 v = W[(long)col * ldw + row];
+        const int c2 = col / nb;
+        if (c2 == c1) {
+            const int j = col - c2 * nb;
+            v.x = (i == j) ? __dadd_rn(dterm, v.x) : __dadd_rn(hT[(long)j * nb + i], v.x);
+        }
         s += sqrt(v.x * v.x + v.y * v.y);
     }
     atomicAdd(rowsum + row, s);
 }
 
-int dense_anorm(cudaStream_t st, int n, const double2 *A, long lda, double *rowsum_scratch, double *out_dev) {
+int nonlocal_anorm(cudaStream_t st, const StructTables &t, double energy, const double2 *W, long ldw, double *rowsum_scratch,
+                   double *out_dev) {
+    const int n = t.nch * t.nb;
     HP_CUDA(cudaMemsetAsync(rowsum_scratch, 0, sizeof(double) * (size_t)n, st));
     dim3 grid(ceil_div(n, 256), std::max(1, std::min(64, n / 256)));
-    dense_rowsum_kernel<<<grid, 256, 0, st>>>(n, A, lda, rowsum_scratch);
+    nonlocal_rowsum_kernel<<<grid, 256, 0, st>>>(t.nch, t.nb, t.hT, t.dg0, t.ethr, energy, W, ldw, rowsum_scratch);
     HP_LAUNCHED();
     HP_CUDA(cudaMemsetAsync(out_dev, 0, sizeof(double), st));
     return maxabs_real(st, n, rowsum_scratch, out_dev);

@@ -19,8 +19,9 @@ struct StructTables {
 int assemble_z(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double2 *C, long ldc);
 // non-local potentials: C <- W + (kinetic + Bloch + centrifugal + threshold - E on the diagonal blocks); W N x N, ld ldw
 int assemble_nonlocal(cudaStream_t st, const StructTables &t, double energy, const double2 *W, long ldw, double2 *C, long ldc);
-// out_dev <- ||A||_inf of the dense n x n matrix; rowsum_scratch: n doubles
-int dense_anorm(cudaStream_t st, int n, const double2 *A, long lda, double *rowsum_scratch, double *out_dev);
+// out_dev <- ||W + diagonal-block terms||_inf; rowsum_scratch: N doubles
+int nonlocal_anorm(cudaStream_t st, const StructTables &t, double energy, const double2 *W, long ldw, double *rowsum_scratch,
+                   double *out_dev);
 int maxabs_real(cudaStream_t st, long n, const double *x, double *out_dev);
 int build_rhs(cudaStream_t st, const StructTables &t, double2 *B, long ldb);
 // R <- Bx - (C - E I) X (Bx == nullptr: the surface right-hand sides), double-double accumulation; Rlo is scratch of

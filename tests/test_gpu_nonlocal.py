@@ -1,6 +1,7 @@
 """Parity of hprmat_solve_nonlocal (non-local potentials, every block of the matrix full;
-PAPER.md:99, 155) with oracle.rmatrix_nonlocal, through the C ABI.  FP64 mode; tolerances as for the local FP64 path:
-max|R - R_orc| / max|R_orc| <= 1e-10, backward error <= 50 N 2^-53."""
+PAPER.md:99, 155) with oracle.rmatrix_nonlocal, through the C ABI.  Tolerances as for the local path (north_star):
+FP64 and mixed+refine max|R - R_orc| / max|R_orc| <= 1e-10, mixed without refinement <= 1e-3, backward error
+<= 50 N 2^-53 wherever refinement ran."""
 import itertools
 
 import numpy as np
@@ -87,10 +88,9 @@ def test_nonlocal_argument_errors_and_unsynchronised_call():
     ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=0)
     r, _ = ctx.mesh()
     W_dev = torch.from_numpy(nonlocal_matrix(w, r)).to(DEV)
-    for mode in (hb.HPRMAT_MIXED, hb.HPRMAT_MIXED_REFINE, 17):
-        with pytest.raises(hb.HprmatError) as e:
-            ctx.solve_nonlocal(10.0, W_dev, mode=mode)
-        assert e.value.code == -5
+    with pytest.raises(hb.HprmatError) as e:
+        ctx.solve_nonlocal(10.0, W_dev, mode=17)
+    assert e.value.code == -5
     with pytest.raises(hb.HprmatError) as e:
         hb._check(hb.lib().hprmat_solve_nonlocal(ctx._h, hb.C.c_double(10.0), hb._dev(W_dev), hb.C.c_long(w.n - 1),
                                                  hb.C.c_int(hb.HPRMAT_FP64), hb.C.c_int(-1), hb.C.c_double(0.0),
@@ -102,11 +102,16 @@ def test_nonlocal_argument_errors_and_unsynchronised_call():
     R2, none = ctx.solve_nonlocal(10.0, W_dev, want_info=False)
     torch.cuda.synchronize()
     assert none is None and _relmax(R2.cpu().numpy(), R1.cpu().numpy()) <= 1e-12
-    # a context without the FP64 buffers refuses
+    # a context without the FP64 buffers refuses the FP64 mode (and the other way round)
     ctx2 = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << hb.HPRMAT_MIXED_REFINE)
     with pytest.raises(hb.HprmatError) as e:
         ctx2.solve_nonlocal(10.0, W_dev)
     assert e.value.code == -5
+    ctx3 = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << hb.HPRMAT_FP64)
+    with pytest.raises(hb.HprmatError) as e:
+        ctx3.solve_nonlocal(10.0, W_dev, mode=hb.HPRMAT_MIXED_REFINE)
+    assert e.value.code == -5
+    ctx3.destroy()
     ctx.destroy()
     ctx2.destroy()
 
@@ -134,6 +139,51 @@ def test_nonlocal_full_size_properties():
     assert np.linalg.svd(Ug, compute_uv=False).max() <= 1.0 + 1e-10
     print(f"non-local cfg3: lu {info['ms_lu']:.1f} ms, total {info['ms_total']:.1f} ms, backward error {info['backward_err']:.2e}, "
           f"refine steps {info['refine_steps']}")
+    ctx.destroy()
+    del W_dev
+    torch.cuda.empty_cache()
+
+
+# ---------------------------------------------------------------------------------------------------- mixed modes
+@pytest.mark.parametrize("cfg,nch,nb,E", [(0, None, None, 10.0), (1, 7, 37, 9.0), (1, 8, 100, 25.0), (2, 12, 100, 12.0),
+                                          (3, 20, 130, 30.0)])
+def test_nonlocal_mixed_modes_parity(cfg, nch, nb, E):
+    """TF32 factors of S = K_d^-1 (K + W) (full blocks) with and without FP64 refinement."""
+    w = make_workload(cfg, nch=nch, nb=nb)
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr,
+                     max_mode=(1 << hb.HPRMAT_MIXED) | (1 << hb.HPRMAT_MIXED_REFINE))
+    r, _ = ctx.mesh()
+    W_dev = torch.from_numpy(nonlocal_matrix(w, r)).to(DEV)
+    Wo = nonlocal_matrix(w, oracle.mesh(w.nb, w.a)[2]).reshape(w.n, w.n).T
+    Ro = oracle.rmatrix_nonlocal(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, Wo)
+    R1, info1 = ctx.solve_nonlocal(E, W_dev, mode=hb.HPRMAT_MIXED)
+    assert info1["status"] == hb.HPRMAT_OK and info1["refine_steps"] == 0
+    assert _relmax(R1.cpu().numpy().T, Ro) <= 1e-3
+    R2, info2 = ctx.solve_nonlocal(E, W_dev, mode=hb.HPRMAT_MIXED_REFINE)
+    assert info2["status"] == hb.HPRMAT_OK and 1 <= info2["refine_steps"] <= 5
+    assert _relmax(R2.cpu().numpy().T, Ro) <= 1e-10
+    assert 0 <= info2["backward_err"] <= 50 * w.n * 2.0 ** -53
+    ctx.destroy()
+
+
+def test_nonlocal_mixed_full_size_properties():
+    """configs[3] size, mixed + refinement: converged status, backward error, R = R^T, and agreement with the FP64 mode
+    of the same entry (two different factorisations of two different matrices, S and C) to 1e-9."""
+    w = make_workload(3)
+    E = float(w.energies[0])
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=0)
+    r, _ = ctx.mesh()
+    W_dev = nonlocal_matrix(w, torch.from_numpy(r).to(DEV), xp=torch)
+    Rm, info = ctx.solve_nonlocal(E, W_dev, mode=hb.HPRMAT_MIXED_REFINE)
+    Rm = Rm.cpu().numpy().T.copy()
+    assert info["status"] == hb.HPRMAT_OK
+    assert 0 <= info["backward_err"] <= 50 * w.n * 2.0 ** -53
+    assert _relmax(Rm, Rm.T) <= 1e-10
+    Rf, info_f = ctx.solve_nonlocal(E, W_dev, mode=hb.HPRMAT_FP64)
+    assert _relmax(Rm, Rf.cpu().numpy().T) <= 1e-9
+    print(f"non-local cfg3 mixed+refine: assemble {info['ms_assemble']:.1f} ms, lu {info['ms_lu']:.1f} ms, total "
+          f"{info['ms_total']:.1f} ms, {info['refine_steps']} steps, backward error {info['backward_err']:.2e}; fp64 total "
+          f"{info_f['ms_total']:.1f} ms")
     ctx.destroy()
     del W_dev
     torch.cuda.empty_cache()
