@@ -104,7 +104,8 @@ int hprmat_solve_host(hprmat_ctx *ctx, double energy, const void *V_host, int mo
  *        W[(c2*nbasis + j)*ldw + c1*nbasis + i] = <f_i| W_{c1 c2} |f_j>, MeV -- for a kernel W_{c1 c2}(r, r') at the Gauss
  *        approximation of the Lagrange-mesh method  a sqrt(lambda_i lambda_j) W_{c1 c2}(r_i, r_j)  (lambda: the
  *        Gauss-Legendre weights on (0,1)); a local potential is V_{c1 c2}(r_i) delta_ij.  Not modified.
- *   mode HPRMAT_FP64 only (-5 otherwise; the context must have been set up with that mode)
+ *   mode any of the three modes the context was set up with (-5 otherwise).  The mixed modes factor, in TF32,
+ *        S = K_d^-1 (C - E I) with K_d the FULL diagonal blocks (kinetic terms + W_cc), inverted in FP64.
  *   max_refine, tol, R, info: as hprmat_solve.  The refinement residual B - (K + W) X is formed in working precision
  *        (W X on the FP64 tensor cores): it restores the backward error, not digits beyond kappa 2^-53.
  * The matrix is C - E I = W + [kinetic + Bloch + centrifugal + threshold - E on the diagonal blocks]; LU, solves,
