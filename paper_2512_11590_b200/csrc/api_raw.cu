@@ -83,9 +83,16 @@ extern "C" int hprmat_zsolve(void *cuda_stream, int n, int nrhs, void *A, int ld
     LuWork<ZView> wk;
     const size_t used = wk.carve(workspace, n);
     int *info_dev = (int *)((char *)workspace + used);
-    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    struct Events {  // destroyed on every return path
+        cudaEvent_t e[3] = {nullptr, nullptr, nullptr};
+        ~Events() {
+            for (auto &x : e)
+                if (x) cudaEventDestroy(x);
+        }
+    } evs;
+    cudaEvent_t *ev = evs.e;
     if (info)
-        for (auto &e : ev) HP_CUDA(cudaEventCreate(&e));
+        for (auto &e : evs.e) HP_CUDA(cudaEventCreate(&e));
     HP_CUDA(cudaMemsetAsync(info_dev, 0, sizeof(int), st));
     if (info) HP_CUDA(cudaEventRecord(ev[0], st));
     HP_TRY(getrf<ZView>(st, n, ZView((double2 *)A, lda), ipiv, info_dev, wk));
@@ -104,7 +111,6 @@ extern "C" int hprmat_zsolve(void *cuda_stream, int n, int nrhs, void *A, int ld
         info->ms_solve = ms;
         info->ms_total = info->ms_lu + info->ms_solve;
         info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)n * n * n / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
-        for (auto &e : ev) cudaEventDestroy(e);
         if (h != 0) {
             rc = HPRMAT_ESINGULAR;
             info->pivot_index = h;
