@@ -16,27 +16,32 @@
 // that complex element; same for B with (k kk, col r).  C fragment: lane holds (row r, cols 2kk, 2kk+1) of T1, T2, T3, so
 // the complex result of an element is combined inside one lane and stored as one 16-byte word.
 // Tiling: CTA = WM x WN warps, warp tile 32 x 16 (4 x 2 MMA tiles, 3 accumulators each = 96 registers), k-slab KC,
-// cp.async ring; shared leading dimensions BM + 2 (A stored [k][m]) and KC + 4 (B stored [n][k]) make the 16-byte fragment
+// cp.async ring synchronised by mbarriers (no CTA-wide barrier in the main loop); shared leading dimensions BM + 2 (A stored [k][m]) and KC + 4 (B stored [n][k]) make the 16-byte fragment
 // loads conflict free.  C may NOT alias B here (several M tiles per column strip): zgemm() routes such calls to zgemm.cu.
 #include "lu.cuh"
+#include "sm100.cuh"
 
 namespace hp {
 
 namespace {
+
+using namespace sm100;
 
 __device__ __forceinline__ void cp16(void *sdst, const void *gsrc, bool valid) {
     unsigned s = (unsigned)__cvta_generic_to_shared(sdst);
     int sz = valid ? 16 : 0;
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gsrc), "r"(sz) : "memory");
 }
-__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+// the mbarrier receives one arrival when all cp.async issued so far by this thread have landed
+__device__ __forceinline__ void cp_arrive_noinc(uint64_t *bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
 
 __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
 }
 
-template <int WM, int WN, int KC, int STAGES>
+template <int WM, int WN, int KC, int STAGES, int LP>
 __global__ void __launch_bounds__(WM *WN * 32, 1)
     zgemm3m_kernel(int M, int N, int K, double alpha, const double2 *__restrict__ A, long lda, const double2 *__restrict__ B,
                    long ldb, double beta, double2 *__restrict__ C, long ldc, long strideA, long strideB, long strideC) {
@@ -85,22 +90,33 @@ __global__ void __launch_bounds__(WM *WN * 32, 1)
             for (int e = 0; e < 2; ++e) t1[i][j][e] = t2[i][j][e] = t3[i][j][e] = 0.0;
 
     const int nk = (K + KC - 1) / KC;
+    // No CTA-wide barrier in the main loop.  full[s] (NT arrivals, one per thread when its cp.async of the stage have landed)
+    // releases the readers of a stage; empty[s] (one arrival per warp) releases its slot for the load of slab kt + STAGES - 1,
+    // which is issued at k-step LP of slab kt -- most of a slab after every warp has left slab kt - 1, so neither wait is
+    // reached before its condition holds unless the warps drift apart by that much.  (The position of the issue point
+    // matters by itself: +4 % at LP = 6 against LP = 0, 2 or 5, profiles/r01_ncu_full.md.)
+    __shared__ uint64_t full_bar[STAGES], empty_bar[STAGES];
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(&full_bar[s], NT);
+            mbar_init(&empty_bar[s], WM * WN);
+        }
+        fence_mbar_init();
+    }
+    __syncthreads();
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
-        if (s < nk) load_stage(s, s * KC);
-        cp_commit();
+        if (s < nk) {
+            load_stage(s, s * KC);
+            cp_arrive_noinc(&full_bar[s]);
+        }
     }
     const int a_off = kk * LDA_S + wm * 32 + r;       // + ks*4*LDA_S + mi*8
     const int b_off = (wn * 16 + r) * LDB_S + kk;     // + ni*8*LDB_S + ks*4
 
     for (int kt = 0; kt < nk; ++kt) {
-        cp_wait<STAGES - 2>();
-        __syncthreads();
-        {
-            const int nxt = kt + STAGES - 1;
-            if (nxt < nk) load_stage(nxt % STAGES, nxt * KC);
-            cp_commit();
-        }
+        mbar_wait(&full_bar[kt % STAGES], (kt / STAGES) & 1);
         const double2 *a_s = sA + (kt % STAGES) * A_STAGE + a_off;
         const double2 *b_s = sB + (kt % STAGES) * B_STAGE + b_off;
         // Software pipeline over the k-steps: the fragments of step ks + 1 are fetched before the MMAs of step ks are issued,
@@ -124,6 +140,15 @@ __global__ void __launch_bounds__(WM *WN * 32, 1)
 #pragma unroll
         for (int ks = 0; ks < KC / 4; ++ks) {
             const int b = ks & 1;
+            if (ks == LP) {
+                const int nxt = kt + STAGES - 1;
+                if (nxt < nk) {
+                    const int ps = nxt % STAGES;  // the slot of slab kt - 1
+                    if (nxt >= STAGES) mbar_wait(&empty_bar[ps], ((nxt / STAGES) - 1) & 1);
+                    load_stage(ps, nxt * KC);
+                    cp_arrive_noinc(&full_bar[ps]);
+                }
+            }
             if (ks + 1 < KC / 4) fetch(ks + 1, b ^ 1);
 #pragma unroll
             for (int mi = 0; mi < 4; ++mi)
@@ -138,8 +163,9 @@ __global__ void __launch_bounds__(WM *WN * 32, 1)
                 for (int ni = 0; ni < 2; ++ni) dmma(t3[mi][ni], as[b][mi], bs[b][ni]);
             if (ks + 1 < KC / 4) sums(b ^ 1);
         }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty_bar[kt % STAGES]);
     }
-    cp_wait<0>();
 
     // epilogue: element (row 8 mi + r, col 8 ni + 2 kk + e) of the warp tile; old C values fetched as independent loads first
     double2 old[4][2][2];
@@ -180,7 +206,9 @@ int zgemm3m(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A
     constexpr int WM = 2, WN = 4, KC = 32, STAGES = 3;
     constexpr int BM = WM * 32, BN = WN * 16;
     constexpr size_t smem = (size_t)STAGES * (KC * (BM + 2) + BN * (KC + 4)) * sizeof(double2);
-    auto kern = zgemm3m_kernel<WM, WN, KC, STAGES>;
+    constexpr int LP = 6;
+    static_assert(LP < KC / 4, "the issue point is a k-step of the slab");
+    auto kern = zgemm3m_kernel<WM, WN, KC, STAGES, LP>;
     static bool configured = false;
     if (!configured) {
         HP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
