@@ -225,6 +225,9 @@ def main():
     ap.add_argument("--probe", default=None, choices=["zgemm", "cgemm", "dmma", "panel"],
                     help="kernel probes instead of the step: zgemm = hprmat_zgemm alone at --m/--n/--k; dmma = FP64 "
                          "tensor-core issue-rate ceiling (hprmat_probe_dmma)")
+    ap.add_argument("--fp64-algo", type=int, default=0, choices=[0, 1, 2],
+                    help="what the FP64 LU factors: 1 = C - E I (the paper's Type 1), 2 = the block-preconditioned matrix with "
+                         "verified diagonal pivots; 0 = the library default (2)")
     ap.add_argument("--zgemm-algo", type=int, default=0, choices=[0, 3, 4],
                     help="real decomposition of the complex128 GEMM (3M / 4M); 0 = the library default")
     ap.add_argument("--m", type=int, default=12800)
@@ -242,6 +245,8 @@ def main():
 
     if args.zgemm_algo:
         hb.hprmat_zgemm_algo(args.zgemm_algo)
+    if args.fp64_algo:
+        hb.hprmat_fp64_algo(args.fp64_algo)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -440,6 +445,8 @@ def main():
                 "vs_baseline": None, "dtype": m["dtype"], "data": "synthetic",
                 "config": {"workload": f"BASELINE.json configs[{args.cfg}]: Nc={w.nch}, Nb={w.nb}, N={N}, a={w.a} fm, "
                                        f"E={E} MeV, mode={args.mode}", "parallelism": f"replicas x{world}",
+                           "fp64_factorisation": {1: "LU of C - E I", 2: "LU of K_d^-1 (C - E I), verified diagonal pivots"}[
+                               hb.hprmat_fp64_algo()],
                            "l2": "inputs_larger_than_L2 (matrix 16 N^2 B >> 126 MB)"}}
         for k in ("time_to_rmatrix_s", "lu_tflops", "stages_ms", "refine_steps", "backward_err", "e2e", "gpu_launches",
                   "clocks", "roofline"):

@@ -92,6 +92,15 @@ int hprmat_mesh(const hprmat_ctx *ctx, double *r, double *fa);
 int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int max_refine, double tol, void *R,
                  hprmat_info *info);
 
+/* What the FP64 LU of hprmat_solve(HPRMAT_FP64) is applied to:
+ *   1 = C - E I itself (the paper's Type 1: ZGESV semantics on the assembled matrix);
+ *   2 = S = K_d^-1 (C - E I), K_d = the nch diagonal blocks inverted in FP64 (the matrix of the paper's Type 3, Eqs. 7-9, here
+ *       in FP64): the same N x N LU with partial pivoting and 8N^3/3 flops, but the pivots are the diagonal ones, which the
+ *       panel kernel verifies instead of searching.  Default, chosen by measurement.
+ * Residual, refinement and the reported backward error always refer to the original system.  Any other value only
+ * queries.  Returns the setting in force.  Process-wide; hprmat_solve_nonlocal and hprmat_zsolve are not affected. */
+int hprmat_fp64_algo(int algo);
+
 /* Same call with HOST buffers (the end-to-end entry): V_host complex [nbasis][nch][nch] and R_host complex nch x nch are
  * host pointers (pinned memory makes the copies asynchronous); the host->device copy of V, all kernels and the
  * device->host copy of R are enqueued on the context's stream, which is synchronised before returning. */

@@ -224,6 +224,11 @@ def hprmat_zgemm(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, stream=None):
     _check(rc, "hprmat_zgemm")
 
 
+def hprmat_fp64_algo(algo: int = 0) -> int:
+    """Select (1: LU of C - E I, 2: LU of the block-preconditioned matrix) or query the FP64 factorisation of hprmat_solve."""
+    return int(lib().hprmat_fp64_algo(C.c_int(algo)))
+
+
 def hprmat_zgemm_algo(algo: int = 0) -> int:
     """Select (3 or 4) or query (anything else) the real decomposition of the complex128 GEMM."""
     return int(lib().hprmat_zgemm_algo(C.c_int(algo)))

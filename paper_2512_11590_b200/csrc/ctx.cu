@@ -185,6 +185,7 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
         const size_t wb = LuWork<ZView>::bytes((int)N);
         HP_ALLOC(c->d_work, wb);
         c->wz.carve(c->d_work, (int)N);
+        HP_ALLOC(c->d_Kinv, sizeof(double2) * (size_t)nch * nb * nb);
     }
     if (max_mode & ((1 << HPRMAT_MIXED) | (1 << HPRMAT_MIXED_REFINE))) {
         c->ldS = round_up(N, 32);
@@ -192,7 +193,7 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
         HP_ALLOC(c->d_Sim, sizeof(float) * c->ldS * N);
         HP_ALLOC(c->d_Bre, sizeof(float) * c->ldS * nch);
         HP_ALLOC(c->d_Bim, sizeof(float) * c->ldS * nch);
-        HP_ALLOC(c->d_Kinv, sizeof(double2) * (size_t)nch * nb * nb);
+        if (!c->d_Kinv) HP_ALLOC(c->d_Kinv, sizeof(double2) * (size_t)nch * nb * nb);
         const size_t wb = LuWork<CView>::bytes((int)N);
         HP_ALLOC(c->d_workc, wb);
         if (cudaMemsetAsync(c->d_workc, 0, wb, c->st) != cudaSuccess) { free_ctx(c); return HPRMAT_ECUDA; }
@@ -339,6 +340,97 @@ int solve_fp64(hprmat_ctx *c, double energy, const double2 *V, int max_refine, d
         (void)rmax;
     }
     return status;
+}
+
+// FP64 mode, preconditioned form (the default; hprmat_fp64_algo): the FP64 LU is applied to S = K_d^-1 (C - E I), the matrix
+// of the paper's Type 3 (Eqs. 7-9), instead of C - E I itself.  Same N x N complex LU with partial pivoting and the same
+// 8N^3/3 flops, but S = I + (coupling-sized entries): the pivots partial pivoting selects are the diagonal ones, which the
+// speculative panel (panel.cu) verifies column by column -- the sequential pivot search across all SMs (N dependent
+// exchanges, ~0.1 s at N = 25600) disappears, and with kappa(S) = O(1) the first solve is already at the rounding floor.
+// The residual of the refinement and the reported backward error are those of the ORIGINAL system (C - E I) X = B.
+int solve_fp64_precond(hprmat_ctx *c, double energy, const double2 *V, int max_refine, double tol, double2 *R,
+                       hprmat_info *info) {
+    cudaStream_t st = c->st;
+    const int N = c->n, nch = c->nch, nb = c->nb;
+    const bool timed = info != nullptr;
+    ZView S(c->d_C, N), X(c->d_X, N), D(c->d_Rlo, N);
+    if (max_refine < 0) max_refine = 2;
+    if (!(tol > 0.0)) tol = 1e-13;
+    int steps = 0;
+
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[0], st));
+    HP_CUDA(cudaMemsetAsync(c->d_info, 0, 2 * sizeof(int), st));
+    HP_TRY(precond_invert(st, c->tab, energy, V, c->d_Kinv, c->d_info + 1));
+    HP_TRY(precond_assemble_z(st, c->tab, c->d_Kinv, V, S));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[1], st));
+    c->wz.speculate = true;
+    const int rc_lu = getrf<ZView>(st, N, S, c->d_ipiv, c->d_info, c->wz);
+    c->wz.speculate = false;
+    HP_TRY(rc_lu);
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[2], st));
+    if (timed) {
+        HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        if (c->h_info[0] != 0 || c->h_info[1] != 0) {
+            info->status = HPRMAT_ESINGULAR;
+            info->pivot_index = c->h_info[0] ? c->h_info[0] : c->h_info[1];
+            return HPRMAT_ESINGULAR;
+        }
+    }
+    HP_TRY(precond_rhs_z(st, c->tab, c->d_Kinv, X));
+    HP_TRY(getrs<ZView>(st, N, nch, S, X, c->wz));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[3], st));
+    double dprev = 0.0;
+    if (timed && max_refine > 0) {
+        HP_TRY(maxabs(st, N, nch, c->d_X, N, c->d_scal + 2));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 2, c->d_scal + 2, sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        dprev = c->h_scal[2];
+    }
+    for (int k = 0; k < max_refine; ++k) {
+        HP_TRY(structured_residual(st, c->tab, energy, V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, c->d_scal + 3));
+        // z = K_d^-1 r (one nb x nb by nb x nch product per channel), d = S^-1 z
+        HP_TRY(zgemm_batched(st, nb, nch, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, c->d_Rr, N, nb, 0.0, c->d_Rlo, N, nb, nch));
+        HP_TRY(getrs<ZView>(st, N, nch, S, D, c->wz));
+        HP_TRY(axpy_norm(st, N, nch, c->d_X, N, c->d_Rlo, N, c->d_scal));
+        ++steps;
+        if (timed) {
+            HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
+            HP_CUDA(cudaStreamSynchronize(st));
+            const double dn = c->h_scal[0], xn = c->h_scal[1];
+            const int v = refine_verdict(dn, xn, dprev, tol);
+            dprev = dn;
+            if (v != REF_CONTINUE) break;  // FP64 mode: a stagnated correction is at the rounding floor, not a failure
+        }
+    }
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[4], st));
+    HP_TRY(contract(st, c->tab, c->d_X, N, R));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[5], st));
+    c->have_x = true;
+    if (timed) {
+        HP_TRY(structured_residual(st, c->tab, energy, V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, c->d_scal + 3));
+        HP_TRY(structured_anorm(st, c->tab, energy, V, c->d_scal + 4));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 3, c->d_scal + 3, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        double bn = 0.0;
+        for (double f : c->fa) bn = std::max(bn, fabs(f));
+        HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        info->status = HPRMAT_OK;
+        info->refine_steps = steps;
+        info->pivot_index = 0;
+        info->resid_max = c->h_scal[3];
+        info->backward_err = c->h_scal[5];
+        info->ms_assemble = ev_ms(c->ev[0], c->ev[1]);
+        info->ms_lu = ev_ms(c->ev[1], c->ev[2]);
+        info->ms_solve = ev_ms(c->ev[2], c->ev[3]);
+        info->ms_refine = ev_ms(c->ev[3], c->ev[4]);
+        info->ms_contract = ev_ms(c->ev[4], c->ev[5]);
+        info->ms_total = ev_ms(c->ev[0], c->ev[5]);
+        info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)N * N * N / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
+    }
+    return HPRMAT_OK;
 }
 
 // Mixed modes (PAPER.md:147-151 Type 2, :192-230 Type 4; preconditioned per reading R10):
@@ -638,6 +730,12 @@ extern "C" int hprmat_solve_nonlocal(hprmat_ctx *ctx, double energy, const void 
     return rc;
 }
 
+static int g_fp64_algo = 2;
+extern "C" int hprmat_fp64_algo(int algo) {
+    if (algo == 1 || algo == 2) g_fp64_algo = algo;
+    return g_fp64_algo;
+}
+
 extern "C" int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int max_refine, double tol, void *R,
                             hprmat_info *info) {
     if (!ctx) return -1;
@@ -651,7 +749,8 @@ extern "C" int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int m
     }
     int rc;
     if (mode == HPRMAT_FP64) {
-        rc = solve_fp64(ctx, energy, (const double2 *)V, max_refine, tol, (double2 *)R, info);
+        rc = g_fp64_algo == 2 ? solve_fp64_precond(ctx, energy, (const double2 *)V, max_refine, tol, (double2 *)R, info)
+                              : solve_fp64(ctx, energy, (const double2 *)V, max_refine, tol, (double2 *)R, info);
     } else {
         rc = solve_mixed(ctx, energy, (const double2 *)V, mode == HPRMAT_MIXED_REFINE, max_refine, tol, (double2 *)R, info);
     }

@@ -177,6 +177,66 @@ int precond_assemble(cudaStream_t st, const StructTables &t, const double2 *Kinv
     return 0;
 }
 
+// FP64 variants (the preconditioned FP64 factorisation, ctx.cu solve_fp64_precond): same entries, interleaved complex128.
+__global__ void __launch_bounds__(SA_NT) assemble_s_z_kernel(int nch, int nb, const double2 *__restrict__ Kinv,
+                                                             const double2 *__restrict__ V, double2 *__restrict__ S, long ld) {
+    const int N = nch * nb;
+    const int row = blockIdx.x * SA_NT + threadIdx.x;
+    if (row >= N) return;
+    const int c = row / nb, i = row - c * nb;
+    const int j = blockIdx.y;
+    const int cc0 = blockIdx.z * SA_CC;
+    const double2 kij = Kinv[((size_t)c * nb + j) * nb + i];
+#pragma unroll
+    for (int e = 0; e < SA_CC; ++e) {
+        const int c2 = cc0 + e;
+        if (c2 >= nch) break;
+        double2 out;
+        if (c2 == c) {
+            out = make_double2((i == j) ? 1.0 : 0.0, 0.0);
+        } else {
+            const double2 v = V[((size_t)j * nch + c2) * nch + c];
+            out = make_double2(kij.x * v.x - kij.y * v.y, kij.x * v.y + kij.y * v.x);
+        }
+        S[(size_t)(c2 * nb + j) * ld + row] = out;
+    }
+}
+
+int precond_assemble_z(cudaStream_t st, const StructTables &t, const double2 *Kinv, const double2 *V, ZView S) {
+    const int N = t.nch * t.nb;
+    dim3 grid(ceil_div(N, SA_NT), t.nb, ceil_div(t.nch, SA_CC));
+    assemble_s_z_kernel<<<grid, SA_NT, 0, st>>>(t.nch, t.nb, Kinv, V, S.p, S.ld);
+    HP_LAUNCHED();
+    return 0;
+}
+
+__global__ void __launch_bounds__(256) rhs_s_z_kernel(int nch, int nb, const double2 *__restrict__ Kinv,
+                                                      const double *__restrict__ fa, double2 *__restrict__ B, long ld) {
+    const long N = (long)nch * nb;
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= N * nch) return;
+    const int q = (int)(idx / N);
+    const int row = (int)(idx - (long)q * N);
+    const int c = row / nb, i = row - c * nb;
+    double sr = 0.0, si = 0.0;
+    if (c == q) {
+        const double2 *k = Kinv + (size_t)c * nb * nb + i;
+        for (int j = 0; j < nb; ++j) {
+            const double2 v = k[(size_t)j * nb];
+            sr = fma(v.x, fa[j], sr);
+            si = fma(v.y, fa[j], si);
+        }
+    }
+    B[(size_t)q * ld + row] = make_double2(sr, si);
+}
+
+int precond_rhs_z(cudaStream_t st, const StructTables &t, const double2 *Kinv, ZView B) {
+    const long tot = (long)t.nch * t.nb * t.nch;
+    rhs_s_z_kernel<<<ceil_div(tot, 256), 256, 0, st>>>(t.nch, t.nb, Kinv, t.fa, B.p, B.ld);
+    HP_LAUNCHED();
+    return 0;
+}
+
 // Non-local potentials: S = K_d^-1 (C - E I) with full blocks.  Block row c of S is Kinv_c times block row c of W for the
 // off-diagonal blocks and the identity on the diagonal block.  The products run on the FP64 tensor cores, one column chunk
 // of nch columns at a time (nch batched nb x nch x nb GEMMs into the N x nch scratch T), and this kernel demotes the chunk

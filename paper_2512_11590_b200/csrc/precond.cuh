@@ -14,6 +14,9 @@ int precond_assemble(cudaStream_t st, const StructTables &t, const double2 *Kinv
 // non-local potentials: S <- K_d^-1 (C - E*I) with full blocks of W; T: N x nch complex128 scratch (ld ldt)
 int precond_assemble_nonlocal(cudaStream_t st, const StructTables &t, const double2 *Kinv, const double2 *W, long ldw, CView S,
                               double2 *T, long ldt);
+// the same two in complex128 (preconditioned FP64 factorisation)
+int precond_assemble_z(cudaStream_t st, const StructTables &t, const double2 *Kinv, const double2 *V, ZView S);
+int precond_rhs_z(cudaStream_t st, const StructTables &t, const double2 *Kinv, ZView B);
 // B <- K_d^-1 * (surface right-hand sides), split complex64, N x nch
 int precond_rhs(cudaStream_t st, const StructTables &t, const double2 *Kinv, CView B);
 // D <- (complex64) Z

@@ -245,3 +245,53 @@ def test_rmatrix_fp64_cfg3_headline_size_certificate(cfg):
     for (c1, c2) in [(0, 0), (3, 200), (255, 255), (17, 4)]:
         assert abs(Rg[c1, c2] - (w.h2m / w.a) * np.dot(fa, X[c1 * w.nb:(c1 + 1) * w.nb, c2])) <= 1e-13 * np.abs(Rg).max()
     ctx.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------- FP64 factorisation variants
+@pytest.mark.parametrize("cfg,nch,nb,E", [(0, None, None, 10.0), (1, 5, 37, 9.0), (1, 12, 100, 25.0), (3, 20, 130, 30.0)])
+def test_both_fp64_factorisations_match_the_oracle(cfg, nch, nb, E):
+    """hprmat_fp64_algo: 1 = LU of C - E I (the paper's Type 1), 2 = LU of the block-preconditioned S = K_d^-1 (C - E I)
+    with verified diagonal pivots (default).  Both must meet the FP64 bar on R, X and the backward error of the ORIGINAL
+    system."""
+    w = make_workload(cfg, nch=nch, nb=nb)
+    ctx = _ctx(w, 1 << hb.HPRMAT_FP64)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    Ro, Xo = oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, w.potential(oracle.mesh(w.nb, w.a)[2]), return_x=True)
+    default = hb.hprmat_fp64_algo()
+    assert default == 2
+    try:
+        for algo in (1, 2):
+            assert hb.hprmat_fp64_algo(algo) == algo
+            R, info = ctx.solve(E, V, hb.HPRMAT_FP64)
+            assert _relmax(_host(R), Ro) <= 1e-10, algo
+            assert _relmax(_host(ctx.get_x()), Xo) <= 1e-9, algo
+            assert 0 <= info["backward_err"] <= 50 * w.n * 2.0 ** -53, algo
+            R2, none = ctx.solve(E, V, hb.HPRMAT_FP64, want_info=False)     # unsynchronised call, two unconditional steps
+            torch.cuda.synchronize()
+            assert none is None and _relmax(_host(R2), Ro) <= 1e-10, algo
+    finally:
+        hb.hprmat_fp64_algo(default)
+    ctx.destroy()
+
+
+def test_preconditioned_fp64_falls_back_to_pivoting_when_the_diagonal_is_refuted():
+    """Couplings 300x the configs' make S pivot off the diagonal: the speculative FP64 panels are refuted and redone with
+    partial pivoting (panel.cu); the result must still meet the FP64 bar, and equal the classic factorisation's."""
+    w = make_workload(1, nch=12, nb=100)
+    w.beta *= 300.0
+    E = 20.0
+    ctx = _ctx(w, 1 << hb.HPRMAT_FP64)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    Ro = oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, w.potential(oracle.mesh(w.nb, w.a)[2]))
+    R2, info2 = ctx.solve(E, V, hb.HPRMAT_FP64)
+    R2 = _host(R2).copy()
+    assert _relmax(R2, Ro) <= 1e-10 and info2["backward_err"] <= 50 * w.n * 2.0 ** -53
+    try:
+        hb.hprmat_fp64_algo(1)
+        R1, _ = ctx.solve(E, V, hb.HPRMAT_FP64)
+        assert _relmax(_host(R1), Ro) <= 1e-10
+    finally:
+        hb.hprmat_fp64_algo(2)
+    ctx.destroy()
