@@ -97,7 +97,11 @@ int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int ma
  *   2 = S = K_d^-1 (C - E I), K_d = the nch diagonal blocks inverted in FP64 (the matrix of the paper's Type 3, Eqs. 7-9, here
  *       in FP64): the same N x N LU with partial pivoting and 8N^3/3 flops, but the pivots are the diagonal ones, which the
  *       panel kernel verifies instead of searching.  Default, chosen by measurement.
- * Residual, refinement and the reported backward error always refer to the original system.  Any other value only
+ * Residual, refinement and the reported backward error always refer to the original system.  A synchronised call
+ * (info != NULL) falls back to variant 1 by itself when a diagonal block is singular, the correction of the refinement
+ * step stays above 1e-9 |X| or the backward error exceeds 50 N 2^-53 (E on or next to a pole of an UNCOUPLED channel,
+ * possible with real potentials only); an unsynchronised call cannot, and its caller should use variant 1 at such
+ * energies.  Any other value only
  * queries.  Returns the setting in force.  Process-wide; hprmat_solve_nonlocal and hprmat_zsolve are not affected. */
 int hprmat_fp64_algo(int algo);
 

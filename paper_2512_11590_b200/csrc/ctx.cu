@@ -348,6 +348,8 @@ int solve_fp64(hprmat_ctx *c, double energy, const double2 *V, int max_refine, d
 // speculative panel (panel.cu) verifies column by column -- the sequential pivot search across all SMs (N dependent
 // exchanges, ~0.1 s at N = 25600) disappears, and with kappa(S) = O(1) the first solve is already at the rounding floor.
 // The residual of the refinement and the reported backward error are those of the ORIGINAL system (C - E I) X = B.
+constexpr int PRECOND_UNUSABLE = -1000;  // internal: the synchronised call falls back to the LU of C - E I
+
 int solve_fp64_precond(hprmat_ctx *c, double energy, const double2 *V, int max_refine, double tol, double2 *R,
                        hprmat_info *info) {
     cudaStream_t st = c->st;
@@ -371,11 +373,7 @@ int solve_fp64_precond(hprmat_ctx *c, double energy, const double2 *V, int max_r
     if (timed) {
         HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
         HP_CUDA(cudaStreamSynchronize(st));
-        if (c->h_info[0] != 0 || c->h_info[1] != 0) {
-            info->status = HPRMAT_ESINGULAR;
-            info->pivot_index = c->h_info[0] ? c->h_info[0] : c->h_info[1];
-            return HPRMAT_ESINGULAR;
-        }
+        if (c->h_info[0] != 0 || c->h_info[1] != 0) return PRECOND_UNUSABLE;  // e.g. E on a pole of an uncoupled channel
     }
     HP_TRY(precond_rhs_z(st, c->tab, c->d_Kinv, X));
     HP_TRY(getrs<ZView>(st, N, nch, S, X, c->wz));
@@ -400,7 +398,12 @@ int solve_fp64_precond(hprmat_ctx *c, double energy, const double2 *V, int max_r
             const double dn = c->h_scal[0], xn = c->h_scal[1];
             const int v = refine_verdict(dn, xn, dprev, tol);
             dprev = dn;
-            if (v != REF_CONTINUE) break;  // FP64 mode: a stagnated correction is at the rounding floor, not a failure
+            if (v != REF_CONTINUE) {
+                // FP64 mode: a stagnated correction is at the rounding floor, not a failure -- unless it is large: then the
+                // preconditioner is ill-conditioned at this energy (near a pole of an uncoupled channel)
+                if (!(dn <= 1e-9 * xn)) return PRECOND_UNUSABLE;
+                break;
+            }
         }
     }
     if (timed) HP_CUDA(cudaEventRecord(c->ev[4], st));
@@ -417,6 +420,7 @@ int solve_fp64_precond(hprmat_ctx *c, double energy, const double2 *V, int max_r
         HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
         HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
         HP_CUDA(cudaStreamSynchronize(st));
+        if (!(c->h_scal[5] <= 50.0 * N * 1.1102230246251565e-16)) return PRECOND_UNUSABLE;
         info->status = HPRMAT_OK;
         info->refine_steps = steps;
         info->pivot_index = 0;
@@ -751,6 +755,11 @@ extern "C" int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int m
     if (mode == HPRMAT_FP64) {
         rc = g_fp64_algo == 2 ? solve_fp64_precond(ctx, energy, (const double2 *)V, max_refine, tol, (double2 *)R, info)
                               : solve_fp64(ctx, energy, (const double2 *)V, max_refine, tol, (double2 *)R, info);
+        if (rc == PRECOND_UNUSABLE) {  // only reachable from a synchronised call (info != NULL)
+            *info = hprmat_info();
+            info->backward_err = -1.0;
+            rc = solve_fp64(ctx, energy, (const double2 *)V, max_refine, tol, (double2 *)R, info);
+        }
     } else {
         rc = solve_mixed(ctx, energy, (const double2 *)V, mode == HPRMAT_MIXED_REFINE, max_refine, tol, (double2 *)R, info);
     }

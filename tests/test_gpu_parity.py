@@ -295,3 +295,29 @@ def test_preconditioned_fp64_falls_back_to_pivoting_when_the_diagonal_is_refuted
     finally:
         hb.hprmat_fp64_algo(2)
     ctx.destroy()
+
+
+def test_preconditioned_fp64_falls_back_on_a_pole_of_an_uncoupled_channel():
+    """Real potentials: at an eigenvalue of one diagonal block K_c (a pole of the UNCOUPLED channel) the preconditioner does
+    not exist although the coupled matrix is regular; the synchronised FP64 call must notice and factor C - E I itself."""
+    w = make_workload(0, nch=3, nb=40)
+    w.W0 = 0.0
+    ro = oracle.mesh(w.nb, w.a)[2]
+    C0 = oracle.assemble(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, 0.0, w.potential(ro))
+    ev = np.linalg.eigvalsh(C0[: w.nb, : w.nb].real)              # K_0 at E = 0: its eigenvalues are the poles of channel 0
+    E = float(ev[np.argmin(np.abs(ev - 8.0))])
+    ctx = _ctx(w, 1 << hb.HPRMAT_FP64)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    Ro = oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, w.potential(ro))
+    assert hb.hprmat_fp64_algo() == 2
+    R, info = ctx.solve(E, V, hb.HPRMAT_FP64)
+    assert info["status"] == hb.HPRMAT_OK
+    assert _relmax(_host(R), Ro) <= 1e-10
+    assert 0 <= info["backward_err"] <= 50 * w.n * 2.0 ** -53
+    # a hair off the pole the preconditioner exists but is ill-conditioned
+    for dE in (1e-9, 1e-6, 1e-3):
+        Ro2 = oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E + dE, w.potential(ro))
+        R2, info2 = ctx.solve(E + dE, V, hb.HPRMAT_FP64)
+        assert info2["status"] == hb.HPRMAT_OK and _relmax(_host(R2), Ro2) <= 1e-10, dE
+    ctx.destroy()
