@@ -2,6 +2,11 @@
 
 Every function cites the passage of /root/reference/PAPER.md it follows in hprmat_oracle.c.  Arrays are column-major
 (Fortran order) complex128 unless stated.  V has shape (nb, nch, nch) C-order with V[i, c2, c1] = V_{c1 c2}(r_i).
+
+Beside the bindings, three functions are written here in plain numpy / scipy / mpmath on top of them: collision_matrix
+(matching at the channel radius, neutral and charged), rmatrix_nonlocal (full potential blocks) and the channel-function
+helper _coulomb_channel.  All functions are pinned in tests/test_oracle_pins.py (list in DESIGN.md section 5.1); none is
+"parity unpinned".
 """
 import ctypes as C
 
