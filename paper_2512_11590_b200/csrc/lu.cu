@@ -363,11 +363,27 @@ static int gemm_sel(bool acc, cudaStream_t st, int m, int n, int k, double alpha
     return acc ? cgemm3(st, m, n, k, alpha, A, B, beta, C) : gemm(st, m, n, k, alpha, A, B, beta, C);
 }
 
+// LEAF product  B <- dinv * B  (s <= LEAF).  The complex128 type goes out of place through the scratch when the shape suits
+// the 3M kernel (it cannot run in place: several M tiles per column strip) and copies back; everything else multiplies in
+// place with the one-M-tile kernels.  Not while the kept block inverses are being built (use_big == false): that runs on
+// the side stream, concurrently with leaf products of the main stream that own the scratch.  cfg 1: 53.4 -> 50.5 ms per step,
+// cfg 3: 1318 -> 1306 ms.
+static int leaf_product(bool acc, cudaStream_t st, int s, int ncols, ZView dinv, ZView B, LuWork<ZView> &wk) {
+    if (wk.use_big && wk.tmp.p && s > 64 && ncols > 32 && ncols <= std::max<long>(wk.n, 256)) {
+        HP_TRY(gemm(st, s, ncols, s, 1.0, dinv, B, 0.0, wk.tmp));
+        return copy_block(st, wk.tmp, B, s, ncols);
+    }
+    return gemm_sel(acc, st, s, ncols, s, 1.0, dinv, B, 0.0, B);
+}
+static int leaf_product(bool acc, cudaStream_t st, int s, int ncols, CView dinv, CView B, LuWork<CView> &) {
+    return gemm_sel(acc, st, s, ncols, s, 1.0, dinv, B, 0.0, B);
+}
+
 // B <- L^-1 B, L = unit lower triangle of the s x s diagonal block of A at (d0,d0); B is s x ncols.  d0 is a multiple of
 // LEAF, or s <= LEAF is a full block of its size class (or the ragged last block).
 template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk, bool acc = false) {
     if (s <= 0 || ncols <= 0) return 0;
-    if (s <= LEAF) return gemm_sel(acc, st, s, ncols, s, 1.0, dinv_of(wk.dinvL, d0, s), B, 0.0, B);
+    if (s <= LEAF) return leaf_product(acc, st, s, ncols, dinv_of(wk.dinvL, d0, s), B, wk);
     if (wk.use_big && (acc || IsPlanar<V>::value) && is_big_block(wk.n, d0, s))
         return big_leaf(st, wk.binvL, wk.dinvL, d0, s, B, ncols, wk, acc);
     const int h = split(s);
@@ -379,7 +395,7 @@ template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V 
 // B <- U^-1 B, U = upper triangle (with diagonal) of the s x s diagonal block of A at (d0,d0)
 template <class V> static int trsm_upper(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk, bool acc = false) {
     if (s <= 0 || ncols <= 0) return 0;
-    if (s <= LEAF) return gemm_sel(acc, st, s, ncols, s, 1.0, dinv_of(wk.dinvU, d0, s), B, 0.0, B);
+    if (s <= LEAF) return leaf_product(acc, st, s, ncols, dinv_of(wk.dinvU, d0, s), B, wk);
     if (wk.use_big && (acc || IsPlanar<V>::value) && is_big_block(wk.n, d0, s))
         return big_leaf(st, wk.binvU, wk.dinvU, d0, s, B, ncols, wk, acc);
     const int h = split(s);
