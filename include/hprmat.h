@@ -101,7 +101,8 @@ int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int ma
  * (info != NULL) falls back to variant 1 by itself when a diagonal block is singular, the correction of the refinement
  * step stays above 1e-9 |X| or the backward error exceeds 50 N 2^-53 (E on or next to a pole of an UNCOUPLED channel,
  * possible with real potentials only); an unsynchronised call cannot, and its caller should use variant 1 at such
- * energies.  Any other value only queries.  Returns the setting in force.  Process-wide; hprmat_solve_nonlocal and hprmat_zsolve are not affected. */
+ * energies.  Any other value only queries.  Returns the setting in force.  Process-wide; hprmat_solve_nonlocal follows it
+ * (K_d then holds the full diagonal blocks), hprmat_zsolve / hprmat_zgetrf always factor the matrix they are given. */
 int hprmat_fp64_algo(int algo);
 
 /* Same call with HOST buffers (the end-to-end entry): V_host complex [nbasis][nch][nch] and R_host complex nch x nch are

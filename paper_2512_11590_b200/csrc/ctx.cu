@@ -532,6 +532,8 @@ int solve_mixed(hprmat_ctx *c, double energy, const double2 *V, bool refine, int
 
 }  // namespace
 
+static int g_fp64_algo = 2;  // hprmat_fp64_algo
+
 // Non-local potentials: the same path with a dense potential matrix W.
 // Residual of the refinement: B - (K + W) X = [structured residual with V = 0, double-double] - W X, the product W X on the
 // FP64 tensor cores (the LU has overwritten C, W is the caller's and intact), i.e. a working-precision residual as in
@@ -609,6 +611,109 @@ static int solve_nonlocal_fp64(hprmat_ctx *c, double energy, const double2 *W, l
         HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
         HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
         HP_CUDA(cudaStreamSynchronize(st));
+        info->status = HPRMAT_OK;
+        info->refine_steps = steps;
+        info->pivot_index = 0;
+        info->resid_max = c->h_scal[3];
+        info->backward_err = c->h_scal[5];
+        info->ms_assemble = ev_ms(c->ev[0], c->ev[1]);
+        info->ms_lu = ev_ms(c->ev[1], c->ev[2]);
+        info->ms_solve = ev_ms(c->ev[2], c->ev[3]);
+        info->ms_refine = ev_ms(c->ev[3], c->ev[4]);
+        info->ms_contract = ev_ms(c->ev[4], c->ev[5]);
+        info->ms_total = ev_ms(c->ev[0], c->ev[5]);
+        info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)N * N * N / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
+    }
+    return HPRMAT_OK;
+}
+
+// FP64 mode with non-local potentials, preconditioned form (hprmat_fp64_algo = 2): S = K_d^-1 (K + W) in FP64 with the full
+// diagonal blocks K_c + W_cc inverted; block row c of S is one batched DMMA product Kinv_c x (block row c of W), the diagonal
+// blocks are then overwritten by the identity.  Verified diagonal pivots as in solve_fp64_precond.
+__global__ void __launch_bounds__(256) set_diag_blocks_identity_kernel(int nch, int nb, double2 *__restrict__ S, long ld) {
+    const long tot = (long)nch * nb * nb;
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < tot; idx += (long)gridDim.x * blockDim.x) {
+        const int c = (int)(idx / ((long)nb * nb));
+        const int rem = (int)(idx - (long)c * nb * nb);
+        const int i = rem % nb, j = rem / nb;
+        S[((long)c * nb + j) * ld + (long)c * nb + i] = make_double2(i == j ? 1.0 : 0.0, 0.0);
+    }
+}
+
+static int solve_nonlocal_fp64_precond(hprmat_ctx *c, double energy, const double2 *W, long ldw, int max_refine, double tol,
+                                       double2 *R, hprmat_info *info) {
+    cudaStream_t st = c->st;
+    const int N = c->n, nch = c->nch, nb = c->nb;
+    const bool timed = info != nullptr;
+    ZView S(c->d_C, N), X(c->d_X, N), D(c->d_Rlo, N);
+    if (max_refine < 0) max_refine = 2;
+    if (!(tol > 0.0)) tol = 1e-13;
+    int steps = 0;
+
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[0], st));
+    HP_CUDA(cudaMemsetAsync(c->d_V, 0, sizeof(double2) * (size_t)nb * nch * nch, st));  // "no local potential"
+    HP_CUDA(cudaMemsetAsync(c->d_info, 0, 2 * sizeof(int), st));
+    HP_TRY(precond_invert(st, c->tab, energy, c->d_V, c->d_Kinv, c->d_info + 1, W, ldw));
+    HP_TRY(zgemm_batched(st, nb, N, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, W, ldw, nb, 0.0, c->d_C, N, nb, nch));
+    {
+        const long tot = (long)nch * nb * nb;
+        set_diag_blocks_identity_kernel<<<(int)std::min<long>((tot + 255) / 256, 148 * 8), 256, 0, st>>>(nch, nb, c->d_C, N);
+        HP_LAUNCHED();
+    }
+    if (timed) HP_TRY(nonlocal_anorm(st, c->tab, energy, W, ldw, (double *)c->d_Rlo, c->d_scal + 4));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[1], st));
+    c->wz.speculate = true;
+    const int rc_lu = getrf<ZView>(st, N, S, c->d_ipiv, c->d_info, c->wz);
+    c->wz.speculate = false;
+    HP_TRY(rc_lu);
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[2], st));
+    if (timed) {
+        HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        if (c->h_info[0] != 0 || c->h_info[1] != 0) return PRECOND_UNUSABLE;
+    }
+    HP_TRY(precond_rhs_z(st, c->tab, c->d_Kinv, X));
+    HP_TRY(getrs<ZView>(st, N, nch, S, X, c->wz));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[3], st));
+    double dprev = 0.0;
+    if (timed && max_refine > 0) {
+        HP_TRY(maxabs(st, N, nch, c->d_X, N, c->d_scal + 2));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 2, c->d_scal + 2, sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        dprev = c->h_scal[2];
+    }
+    for (int k = 0; k < max_refine; ++k) {
+        HP_TRY(nonlocal_residual(c, energy, W, ldw, nullptr));
+        HP_TRY(zgemm_batched(st, nb, nch, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, c->d_Rr, N, nb, 0.0, c->d_Rlo, N, nb, nch));
+        HP_TRY(getrs<ZView>(st, N, nch, S, D, c->wz));
+        HP_TRY(axpy_norm(st, N, nch, c->d_X, N, c->d_Rlo, N, c->d_scal));
+        ++steps;
+        if (timed) {
+            HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+            HP_CUDA(cudaStreamSynchronize(st));
+            const double dn = c->h_scal[0], xn = c->h_scal[1];
+            const int v = refine_verdict(dn, xn, dprev, tol);
+            dprev = dn;
+            if (v != REF_CONTINUE) {
+                if (!(dn <= 1e-9 * xn)) return PRECOND_UNUSABLE;
+                break;
+            }
+        }
+    }
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[4], st));
+    HP_TRY(contract(st, c->tab, c->d_X, N, R));
+    if (timed) HP_CUDA(cudaEventRecord(c->ev[5], st));
+    c->have_x = true;
+    if (timed) {
+        HP_TRY(nonlocal_residual(c, energy, W, ldw, c->d_scal + 3));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 3, c->d_scal + 3, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        double bn = 0.0;
+        for (double f : c->fa) bn = std::max(bn, fabs(f));
+        HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
+        HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
+        HP_CUDA(cudaStreamSynchronize(st));
+        if (!(c->h_scal[5] <= 50.0 * N * 1.1102230246251565e-16)) return PRECOND_UNUSABLE;
         info->status = HPRMAT_OK;
         info->refine_steps = steps;
         info->pivot_index = 0;
@@ -726,6 +831,16 @@ extern "C" int hprmat_solve_nonlocal(hprmat_ctx *ctx, double energy, const void 
         *info = hprmat_info();
         info->backward_err = -1.0;
     }
+    if (mode == HPRMAT_FP64 && g_fp64_algo == 2) {
+        int rc2 = solve_nonlocal_fp64_precond(ctx, energy, (const double2 *)W, ldw, max_refine, tol, (double2 *)R, info);
+        if (rc2 == PRECOND_UNUSABLE) {  // synchronised calls only
+            *info = hprmat_info();
+            info->backward_err = -1.0;
+            rc2 = solve_nonlocal_fp64(ctx, energy, (const double2 *)W, ldw, max_refine, tol, (double2 *)R, info);
+        }
+        if (info) info->status = rc2;
+        return rc2;
+    }
     const int rc = mode == HPRMAT_FP64
                        ? solve_nonlocal_fp64(ctx, energy, (const double2 *)W, ldw, max_refine, tol, (double2 *)R, info)
                        : solve_nonlocal_mixed(ctx, energy, (const double2 *)W, ldw, mode == HPRMAT_MIXED_REFINE, max_refine, tol,
@@ -734,7 +849,6 @@ extern "C" int hprmat_solve_nonlocal(hprmat_ctx *ctx, double energy, const void 
     return rc;
 }
 
-static int g_fp64_algo = 2;
 extern "C" int hprmat_fp64_algo(int algo) {
     if (algo == 1 || algo == 2) g_fp64_algo = algo;
     return g_fp64_algo;
