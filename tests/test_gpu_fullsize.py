@@ -1,0 +1,87 @@
+"""BASELINE.json configs[1] and configs[2] at FULL size, every listed mode, every energy of their sweeps, through ONE context
+per mode (the paper's "reuse across the energy scan").  All tests need a B200 ("-m gpu").
+
+What is compared:
+  * every energy: the a-posteriori certificate of tests/certificate.py -- first-order term (h2m/a) X~^T r with the ORACLE's
+    long-double residual r of the GPU solution, the oracle-evaluated backward error of that r against 50 N 2^-53 (FP64,
+    mixed+refine), and an explicit estimate of the dropped second-order term;
+  * configs[1], one energy per mode: the FULL long-double oracle (orc_rmatrix, ~17 s), R and X element by element;
+  * configs[2], E = 27.5 MeV: the stored oracle R (tests/golden/oracle_R_cfg2_E27.5.npz, written once by
+    tests/golden/make_oracle_R.py from oracle/ only, keyed by a hash of the inputs).
+Tolerances (north_star): FP64 and mixed+refine <= 1e-10 in R, backward error <= 50 N 2^-53; mixed without refinement <= 1e-3.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from certificate import certificate
+from golden.make_oracle_R import golden_path, input_key
+from paper_2512_11590_b200 import binding as hb
+from paper_2512_11590_b200.workloads import make_workload
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+DEV = "cuda"
+TOL = {hb.HPRMAT_FP64: 1e-10, hb.HPRMAT_MIXED_REFINE: 1e-10, hb.HPRMAT_MIXED: 1e-3}
+MODE = {"fp64": hb.HPRMAT_FP64, "mixed": hb.HPRMAT_MIXED, "mixed_refine": hb.HPRMAT_MIXED_REFINE}
+
+
+def _host(t: torch.Tensor) -> np.ndarray:
+    return t.cpu().numpy().T
+
+
+def _relmax(a, b):
+    return np.abs(a - b).max() / np.abs(b).max()
+
+
+def _sweep(cfg, mode_name, full_oracle_at=None, golden_at=None):
+    w = make_workload(cfg)
+    mode = MODE[mode_name]
+    assert mode_name in w.modes
+    tol = TOL[mode]
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
+    r, _ = ctx.mesh()
+    Vh = w.potential(r)
+    V = torch.from_numpy(Vh).to(DEV)
+    for k, E in enumerate(w.energies):
+        E = float(E)
+        R, info = ctx.solve(E, V, mode)
+        assert info["status"] == hb.HPRMAT_OK, (E, info)
+        Rg, X = _host(R), _host(ctx.get_x())
+        c = certificate(w, E, X, Rg, jacobi_steps=2 if mode == hb.HPRMAT_MIXED else 1)
+        assert c["est"] <= tol, (E, c, info)
+        assert c["second"] <= 1e-2 * tol, (E, c)                      # the dropped term, estimated: far below the bar
+        assert c["contraction"] < 0.5, (E, c)
+        if mode != hb.HPRMAT_MIXED:
+            assert c["backward_err"] <= 50 * w.n * 2.0 ** -53, (E, c)  # the ORACLE's residual of the GPU's X
+            assert 0 <= info["backward_err"] <= 50 * w.n * 2.0 ** -53
+        assert _relmax(Rg, Rg.T) <= 10 * tol
+        if full_oracle_at == k:
+            ro = oracle.mesh(w.nb, w.a)[2]
+            Ro, Xo = oracle.rmatrix(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, E, w.potential(ro), mode=0, nrefine=2,
+                                    return_x=True)
+            assert _relmax(Rg, Ro) <= tol, (E, _relmax(Rg, Ro), info)
+            assert _relmax(X, Xo) <= (1e-9 if mode != hb.HPRMAT_MIXED else 1e-2)
+        if golden_at is not None and abs(E - golden_at) < 1e-12:
+            path = golden_path(cfg, golden_at)
+            assert os.path.exists(path), f"{path} missing: run tests/golden/make_oracle_R.py --cfg {cfg} --energy {golden_at}"
+            g = np.load(path)
+            ro = oracle.mesh(w.nb, w.a)[2]
+            assert str(g["key"]) == input_key(w, E, w.potential(ro)), "stored oracle R belongs to other inputs"
+            assert np.array_equal(ro, r) or np.abs(ro - r).max() <= np.spacing(ro).max()
+            assert _relmax(Rg, g["R"]) <= tol, (E, _relmax(Rg, g["R"]), info)
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("mode_name,full_at", [("fp64", 6), ("mixed_refine", 2)])
+def test_cfg1_full_size_energy_sweep(mode_name, full_at):
+    """configs[1]: Nc = 64, Nb = 100 (N = 6400), 10 energies 5..50 MeV, FP64 and mixed+refinement."""
+    _sweep(1, mode_name, full_oracle_at=full_at)
+
+
+@pytest.mark.parametrize("mode_name", ["fp64", "mixed", "mixed_refine"])
+def test_cfg2_full_size_energy_sweep(mode_name):
+    """configs[2]: Nc = 128, Nb = 100 (N = 12800), a = 15 fm, 5 energies, FP64 / mixed without refinement / mixed+refinement."""
+    _sweep(2, mode_name, golden_at=27.5)

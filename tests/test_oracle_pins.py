@@ -488,6 +488,56 @@ def test_collision_matrix_stays_unitary_far_below_the_centrifugal_barrier():
     assert np.abs(U[0, 2]) > 1e-3
 
 
+def test_collision_matrix_equals_the_literal_definition_in_60_digit_arithmetic():
+    """The oracle evaluates U = 1 - 2i (Z^O)^-1 Z^F; reading R14's DEFINITION is U = (Z^O)^-1 Z^I with
+    Z^O_cc' = (k_c' a)^-1/2 [O_c delta_cc' - R_cc' x_c' O'_c'(x_c')] and Z^I likewise with I = G - iF.  Here the literal
+    definition is evaluated in mpmath at 60 digits (Riccati-Bessel functions from mpmath's besselj / bessely, derivatives by
+    the recurrence f_l' = f_{l-1} - (l/x) f_l, an mpmath LU solve) on the sub-barrier case l = 12, k a = 0.56 -- where the
+    literal form loses everything in FP64 -- and on an ordinary case; the oracle must agree to 1e-12."""
+    import mpmath as mp
+
+    def literal(R, lval, ethr, E, a):
+        with mp.workdps(60):
+            n = len(lval)
+            x = [mp.sqrt((mp.mpf(E) - mp.mpf(float(e))) / mp.mpf(H2M)) * mp.mpf(a) for e in ethr]   # all channels open here
+            half = mp.mpf(1) / 2
+            Ff = lambda l, t: mp.sqrt(mp.pi * t / 2) * mp.besselj(l + half, t)       # F_l(t) = t j_l(t)
+            Gf = lambda l, t: -mp.sqrt(mp.pi * t / 2) * mp.bessely(l + half, t)      # G_l(t) = -t y_l(t)
+            O, dO, I, dI = [], [], [], []
+            for l, t in zip(lval, x):
+                F, G = Ff(l, t), Gf(l, t)
+                # Riccati-Bessel recurrence u_l' = u_{l-1} - (l/t) u_l  
+                dF = Ff(l - 1, t) - l / t * F
+                dG = Gf(l - 1, t) - l / t * G
+                O.append(G + 1j * F)
+                dO.append(t * (dG + 1j * dF))
+                I.append(G - 1j * F)
+                dI.append(t * (dG - 1j * dF))
+            Rm = mp.matrix(n, n)
+            for i in range(n):
+                for j in range(n):
+                    Rm[i, j] = mp.mpc(complex(R[i, j]))
+            ZO, ZI = mp.matrix(n, n), mp.matrix(n, n)
+            for i in range(n):
+                for j in range(n):
+                    s = 1 / mp.sqrt(x[j])
+                    ZO[i, j] = ((O[i] if i == j else 0) - Rm[i, j] * dO[j]) * s
+                    ZI[i, j] = ((I[i] if i == j else 0) - Rm[i, j] * dI[j]) * s
+            cols = [mp.lu_solve(ZO, ZI[:, j]) for j in range(n)]
+            return np.array([[complex(cols[j][i]) for j in range(n)] for i in range(n)])
+
+    nb, a = 40, 8.0
+    cases = [([0, 12, 1], [0.0, 5.9, 3.0], 6.0,                                       # k a = 0.56 in the l = 12 channel
+              np.array([[0.0, 12.0, 9.0], [12.0, 0.0, 15.0], [9.0, 15.0, 0.0]])),
+             ([0, 2, 1], [0.0, 1.5, 3.0], 12.0,
+              np.array([[0.0, 7.0, 11.0], [7.0, 0.0, 5.0], [11.0, 5.0, 0.0]]))]
+    for lval, ethr, E, beta in cases:
+        R = oracle.rmatrix(3, nb, a, H2M, lval, ethr, E, _ws_potential(nb, a, 3, beta))
+        U, opn = oracle.collision_matrix(R, lval, ethr, E, H2M, a)
+        assert len(opn) == 3
+        assert np.abs(U - literal(R, lval, ethr, E, a)).max() < 1e-12, (lval, E)
+
+
 # ----------------------------------------------------------------- charged case: Coulomb / Whittaker functions
 E2 = 1.43996  # e^2, MeV fm
 
