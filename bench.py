@@ -55,10 +55,19 @@ NCU_TRAFFIC = {
              "algorithmic_bytes": 8.0 * (2 * 12800 * 6400 + 2 * 12800 * 12800)},
 }
 
-# FP64 tensor (DMMA) peak: 148 SMs x 128 FP64 flop/clk/SM x 1.965 GHz = 37.2 TFLOP/s; measured on this pool with a
-# register-resident mma.sync.m8n8k4.f64 loop: 37.15 TFLOP/s burst and sustained (profiles/r01_dmma_peak.md).  The ratio
-# to the driver's measured bf16 figure is not used because FP64 DMMA is not power-capped on this part.
-FP64_TENSOR_PEAK_TFLOPS = 37.15
+_DMMA_PEAK = None
+
+
+def fp64_tensor_peak():
+    """FP64 tensor (DMMA) peak, MEASURED IN THIS RUN with a register-resident mma.sync.m8n8k4.f64 loop (libhprmat_bench.so,
+    include/hprmat_profile.h): best of 1/2/4 CTAs per SM.  148 SMs x 128 FP64 flop/clk/SM x 1.965 GHz = 37.2 TFLOP/s is
+    the hardware ceiling it approaches; MEASURED_PEAKS.json has no FP64 entry and the guide no FP64 ratio."""
+    global _DMMA_PEAK
+    if _DMMA_PEAK is None:
+        from paper_2512_11590_b200 import binding as hb
+        runs = [{"ctas_per_sm": c, "tflops": hb.hprmat_bench_dmma_peak(40000, c)[0]} for c in (1, 2, 4)]
+        _DMMA_PEAK = {"tflops": max(r["tflops"] for r in runs), "runs": runs}
+    return _DMMA_PEAK
 
 
 def oracle_sample(cfg, steps, warmup):
@@ -92,71 +101,6 @@ def run_reference(args):
             "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
-    return 0
-
-
-def run_probe(args):
-    """Kernel probes (one JSON line each): the GEMM entry alone, or the DMMA ceiling."""
-    import torch
-    from paper_2512_11590_b200 import binding as hb
-    torch.cuda.set_device(0)
-    if args.zgemm_algo:
-        hb.hprmat_zgemm_algo(args.zgemm_algo)
-    if args.probe == "dmma":
-        out = []
-        for cps in (1, 2, 4):
-            tf, ms = hb.hprmat_probe_dmma(40000, cps)
-            out.append({"ctas_per_sm": cps, "tflops": tf, "ms": ms})
-        print(json.dumps({"probe": "dmma", "runs": out, "peak_tflops": max(o["tflops"] for o in out)}))
-        return 0
-    if args.probe == "panel":
-        for m in (256, 2048, 12800, 25600, 37888):
-            us, ph = hb.hprmat_probe_panel(m, 20)
-            G = sum(1 for r in ph if any(r))
-            names = ("load", "argmax", "publish", "wait_all", "fetch_row", "update")
-            for c in sorted({0, G // 2, G - 1}):
-                print(json.dumps({"probe": "panel", "m": m, "us_per_panel": us, "ctas": G, "cta": c,
-                                  "cycles": dict(zip(names, ph[c]))}))
-        return 0
-    m, n, k = args.m, args.n, args.k
-    if args.probe == "cgemm":
-        g = torch.Generator(device="cuda").manual_seed(1)
-        pl = lambda r, c: torch.randn((c, r), dtype=torch.float32, device="cuda", generator=g)   # column-major r x c
-        Ar, Ai, Br, Bi, Cr, Ci = pl(m, k), pl(m, k), pl(k, n), pl(k, n), pl(m, n), pl(m, n)
-        for _ in range(args.warmup):
-            hb.hprmat_cgemm_tf32(m, n, k, -1.0, Ar, Ai, m, Br, Bi, k, 1.0, Cr, Ci, m)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        e0.record()
-        for _ in range(args.steps):
-            hb.hprmat_cgemm_tf32(m, n, k, -1.0, Ar, Ai, m, Br, Bi, k, 1.0, Cr, Ci, m)
-        e1.record()
-        torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1) / args.steps
-        tf = 8.0 * m * n * k / (ms * 1e-3) * 1e-12
-        pk, how = peaks()
-        print(json.dumps({"probe": "cgemm_tf32", "m": m, "n": n, "k": k, "ms": ms, "tflops": tf,
-                          "frac_of_tf32_peak": tf / (0.5 * pk["bf16_tflops_sustained"]), "peak_source": how}))
-        return 0
-    g = torch.Generator(device="cuda").manual_seed(1)
-    A = torch.randn((k, m), dtype=torch.complex128, device="cuda", generator=g)   # column-major m x k
-    B = torch.randn((n, k), dtype=torch.complex128, device="cuda", generator=g)   # column-major k x n
-    Cm = torch.randn((n, m), dtype=torch.complex128, device="cuda", generator=g)  # column-major m x n
-    for _ in range(args.warmup):
-        hb.hprmat_zgemm(m, n, k, -1.0, A, m, B, k, 1.0, Cm, m)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    e0.record()
-    for _ in range(args.steps):
-        hb.hprmat_zgemm(m, n, k, -1.0, A, m, B, k, 1.0, Cm, m)
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / args.steps
-    tf = 8.0 * m * n * k / (ms * 1e-3) * 1e-12
-    algo = hb.hprmat_zgemm_algo()
-    hw = tf * (0.75 if algo == 3 else 1.0)
-    print(json.dumps({"probe": "zgemm", "algo": f"{algo}M", "m": m, "n": n, "k": k, "ms": ms, "tflops_8mnk_convention": tf,
-                      "hardware_tflops": hw, "hardware_frac_of_dmma_peak": hw / FP64_TENSOR_PEAK_TFLOPS}))
     return 0
 
 
@@ -222,22 +166,14 @@ def main():
                     help="a second precision mode measured in the same run and reported under other_modes")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--probe", default=None, choices=["zgemm", "cgemm", "dmma", "panel"],
-                    help="kernel probes instead of the step: zgemm = hprmat_zgemm alone at --m/--n/--k; dmma = FP64 "
-                         "tensor-core issue-rate ceiling (hprmat_probe_dmma)")
     ap.add_argument("--fp64-algo", type=int, default=0, choices=[0, 1, 2],
                     help="what the FP64 LU factors: 1 = C - E I (the paper's Type 1), 2 = the block-preconditioned matrix with "
                          "verified diagonal pivots; 0 = the library default (2)")
     ap.add_argument("--zgemm-algo", type=int, default=0, choices=[0, 3, 4],
                     help="real decomposition of the complex128 GEMM (3M / 4M); 0 = the library default")
-    ap.add_argument("--m", type=int, default=12800)
-    ap.add_argument("--n", type=int, default=12800)
-    ap.add_argument("--k", type=int, default=1024)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
-    if args.probe:
-        return run_probe(args)
 
     import torch
     from paper_2512_11590_b200 import binding as hb
@@ -320,7 +256,8 @@ def main():
             g_ms, g_fl, g_n = cats["lu_gemm"]["ms"], cats["lu_gemm"]["flops"], cats["lu_gemm"]["launches"]
             pk, how = peaks()
             if mode == hb.HPRMAT_FP64:
-                peak, pname = FP64_TENSOR_PEAK_TFLOPS, "FP64 DMMA peak measured on this pool with a register-resident mma.sync loop"
+                peak = fp64_tensor_peak()["tflops"]
+                pname = "FP64 DMMA peak measured in this run with a register-resident mma.sync.m8n8k4.f64 loop (libhprmat_bench.so)"
             else:
                 peak = 0.5 * pk["bf16_tflops_sustained"]
                 pname = f"TF32 dense = 0.5 x bf16 sustained ({how})"

@@ -17,13 +17,18 @@
  *   - Pointers marked  dev  are CUDA device pointers, those marked  host  are host pointers.  The library never
  *     allocates device memory inside hprmat_solve / hprmat_zsolve / hprmat_zgetrf / hprmat_zgetrs / hprmat_zgemm.
  *   - Every call enqueues its kernels on the stream given at setup (or as argument); calls that fill a host
- *     hprmat_info synchronise that stream before returning, the others do not (exception: refinement in the mixed modes).
- *     Part of a factorisation (the kept block inverses) runs on a library-owned side stream, joined before the call's work
- *     on the caller's stream continues.
+ *     hprmat_info synchronise that stream ONCE, at the end, to read the device-side status (the stopping rule of the
+ *     refinement is evaluated on the device after every step); calls with info == NULL never synchronise -- their status
+ *     stays on the device and is fetched with hprmat_last_status.
+ *     Part of a factorisation (the kept block inverses) runs on a side stream owned by the context (by the library, per
+ *     device, for the raw entries), joined before the call's work on the caller's stream continues.
  *   - Return value: 0 success; -k = argument k (1-based) invalid; >0 = one of the HPRMAT_E* codes below.
  *   - There is NO CPU fallback: without a CUDA device every compute entry returns HPRMAT_ECUDA.
- *   - One context per host thread / stream.  The caller owns V, R, A, B, ipiv and the workspace; the context owns
- *     everything else and is reused across an energy scan.
+ *   - One context per host thread / stream; different contexts may be used concurrently from different host threads
+ *     (algorithm switches, side streams and status words are per context; the only process-wide state are the defaults
+ *     hprmat_fp64_algo / hprmat_zgemm_algo, the launch counter and the optional profile record of hprmat_profile.h).
+ *     The caller owns V, R, A, B, ipiv and the workspace; the context owns everything else and is reused across an
+ *     energy scan.
  */
 #ifndef HPRMAT_H
 #define HPRMAT_H
@@ -49,14 +54,19 @@ enum {
     HPRMAT_ESINGULAR = 1,     /* exact zero pivot; info->pivot_index = 1-based column                                  */
     HPRMAT_ENOTCONVERGED = 2, /* refinement hit max_refine or stagnated; X / R hold the last iterate    */
     HPRMAT_ENOMEM = 3,        /* device allocation failed at setup, or workspace too small                             */
-    HPRMAT_ECUDA = 4          /* CUDA error (no device, launch failure, ...); see hprmat_last_cuda_error()             */
+    HPRMAT_ECUDA = 4,         /* CUDA error (no device, launch failure, ...); see hprmat_last_cuda_error()             */
+    HPRMAT_EUNVERIFIED = 5    /* hprmat_last_status only: the factorisation with verified diagonal pivots of an          */
+                              /* UNSYNCHRONISED call was refuted (or its preconditioner is singular / ill-conditioned at */
+                              /* this energy); X / R are not certified -- repeat the call with info != NULL, which falls  */
+                              /* back to the pivoting factorisation by itself                                            */
 };
 
 typedef struct {
     int status;            /* same as the return value                                                                  */
     int refine_steps;      /* refinement steps actually taken                                                           */
     int pivot_index;       /* first zero pivot (1-based) or 0                                                           */
-    int reserved;
+    int reserved;          /* block panels whose diagonal-pivot speculation was refuted in the first attempt (the call   */
+                           /* then refactored with pivoting); 0 in the normal case                                       */
     double resid_max;      /* max_ij |B - A X|_ij of the last residual evaluated (absolute)                             */
     double backward_err;   /* max_j ||b_j - A x_j||_inf / (||A||_inf ||x_j||_inf + ||b_j||_inf); <0 if not evaluated     */
     double ms_assemble, ms_lu, ms_solve, ms_refine, ms_contract, ms_total; /* CUDA-event stage times, milliseconds      */
@@ -87,8 +97,11 @@ int hprmat_mesh(const hprmat_ctx *ctx, double *r, double *fa);
  *   tol  refinement stops when the estimated relative error left in X (correction norm x observed contraction, DESIGN.md
  *        reading R9) is <= tol; <=0 = default: 1e-13 in FP64 mode, 1e-12 in the mixed modes
  *   R    dev, complex nch x nch column-major (output)
- *   info host, may be NULL: then HPRMAT_FP64 and HPRMAT_MIXED only enqueue work (no synchronisation, max_refine steps are
- *        taken unconditionally in FP64 mode); HPRMAT_MIXED_REFINE always reads the correction norms back between steps */
+ *   info host, may be NULL: then the call only enqueues work (no synchronisation in any mode): up to max_refine refinement
+ *        steps in FP64 mode, one more than the previous solve needed in HPRMAT_MIXED_REFINE; the device-side stopping rule
+ *        turns the steps after convergence into no-ops, and hprmat_last_status reports the outcome.
+ *        With info the call enqueues as many steps as the previous solve of this context in this mode needed, reads the
+ *        device status once, and continues step by step only if the stopping rule has not fired yet. */
 int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int max_refine, double tol, void *R,
                  hprmat_info *info);
 
@@ -98,12 +111,27 @@ int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int ma
  *       in FP64): the same N x N LU with partial pivoting and 8N^3/3 flops, but the pivots are the diagonal ones, which the
  *       panel kernel verifies instead of searching.  Default, chosen by measurement.
  * Residual, refinement and the reported backward error always refer to the original system.  A synchronised call
- * (info != NULL) falls back to variant 1 by itself when a diagonal block is singular, the correction of the refinement
- * step stays above 1e-9 |X| or the backward error exceeds 50 N 2^-53 (E on or next to a pole of an UNCOUPLED channel,
- * possible with real potentials only); an unsynchronised call cannot, and its caller should use variant 1 at such
- * energies.  Any other value only queries.  Returns the setting in force.  Process-wide; hprmat_solve_nonlocal follows it
- * (K_d then holds the full diagonal blocks), hprmat_zsolve / hprmat_zgetrf always factor the matrix they are given. */
+ * (info != NULL) falls back to variant 1 by itself when a diagonal block is singular, a multiplier refutes the diagonal
+ * pivots, the correction of the refinement step stays above 1e-9 |X| or the backward error exceeds 50 N 2^-53 (E on or
+ * next to a pole of an UNCOUPLED channel, possible with real potentials only); an unsynchronised call cannot, and
+ * hprmat_last_status then returns HPRMAT_EUNVERIFIED.  Any other value only queries.  Returns the setting in force.
+ * This is the PROCESS DEFAULT, read by every context that has no setting of its own (hprmat_set_option);
+ * hprmat_solve_nonlocal follows the same switch (K_d then holds the full diagonal blocks), hprmat_zsolve / hprmat_zgetrf
+ * always factor the matrix they are given. */
 int hprmat_fp64_algo(int algo);
+
+/* Per-context settings.  value 0 = follow the process default again. */
+enum {
+    HPRMAT_OPT_FP64_ALGO = 1,  /* 1 or 2, see hprmat_fp64_algo                                                           */
+    HPRMAT_OPT_ZGEMM_ALGO = 2  /* 3 or 4, see hprmat_zgemm_algo                                                          */
+};
+int hprmat_set_option(hprmat_ctx *ctx, int option, int value);
+
+/* Outcome of the last hprmat_solve / hprmat_solve_nonlocal of this context -- for calls made with info == NULL, which
+ * leave their status on the device.  Synchronises the context's stream, then decodes the device status words as a
+ * synchronised call does: HPRMAT_OK, HPRMAT_ESINGULAR (pivot_index: 1-based column), HPRMAT_ENOTCONVERGED (mixed+refine),
+ * or HPRMAT_EUNVERIFIED (see above).  refine_steps / pivot_index: host, may be NULL.  -1 if nothing was solved yet. */
+int hprmat_last_status(hprmat_ctx *ctx, int *refine_steps, int *pivot_index);
 
 /* Same call with HOST buffers (the end-to-end entry): V_host complex [nbasis][nch][nch] and R_host complex nch x nch are
  * host pointers (pinned memory makes the copies asynchronous); the host->device copy of V, all kernels and the
@@ -201,7 +229,7 @@ int hprmat_zgemm(void *cuda_stream, int m, int n, int k, double alpha, const voi
 /* Real decomposition of the complex128 product inside hprmat_zgemm and the FP64 LU: 4 = four real products per complex
  * product ("4M", componentwise accurate), 3 = three ("3M": 25 % fewer tensor-core instructions, imaginary part normwise
  * accurate; the default, chosen by measurement).  Any other value only queries.  Returns the
- * setting in force.  Process-wide; not thread-safe against concurrent solves. */
+ * setting in force.  Process default; a context may carry its own (hprmat_set_option). */
 int hprmat_zgemm_algo(int algo);
 
 /* C <- beta*C + alpha*A*B on SPLIT-complex (planar) complex64 operands: every matrix is a pair of column-major float
@@ -219,30 +247,6 @@ int hprmat_cgemm_3xtf32(void *cuda_stream, int m, int n, int k, float alpha, con
 
 const char *hprmat_strerror(int code);
 const char *hprmat_last_cuda_error(void);
-/* Measurement aid (bench.py's roofline leg): while enabled, every launch of the GEMM kernel inside the LU and the
- * triangular solves is bracketed by a CUDA-event pair on its stream.  hprmat_profile_read synchronises those events,
- * returns the summed kernel milliseconds, the summed algorithmic flops (8 m n k per launch) and the launch count, and
- * resets the record. */
-int hprmat_profile(int enable);
-int hprmat_profile_read(double *ms, double *flops, long long *launches);
-/* Per-category totals of the record consumed by the last hprmat_profile_read: cat 0 = trailing-update GEMMs of the LU,
- * 1 = GEMMs of the U12 triangular solves inside the LU, 2 = panel factorisations, 3 = row interchanges, 4 = GEMMs of the
- * right-hand-side triangular solves, 5 = other.  ms/flops/launches host, may be NULL. */
-int hprmat_profile_cat(int cat, double *ms, double *flops, long long *launches);
-/* Measurement aid: FP64 tensor-core (DMMA, mma.sync.m8n8k4.f64) issue-rate ceiling of the device, measured with a
- * register-resident loop (no memory traffic) on 148*ctas_per_sm CTAs of 8 warps, `iters` x 8 MMAs per warp.
- * tflops (host, out): real TFLOP/s; ms (host, out, may be NULL): device time of the timed launch.  Synchronises. */
-int hprmat_probe_dmma(void *cuda_stream, int iters, int ctas_per_sm, double *tflops, double *ms);
-/* Measurement aid: `reps` back-to-back launches of the register-resident panel-factorisation kernel (complex64 planes) on
- * the m x 32 panel A (dev, lda >= m, contents destroyed), m <= 148*256.  workspace: dev, hprmat_workspace_bytes(m, 0,
- * HPRMAT_MIXED) bytes.  us_per_panel (host, out): mean device time per launch.  phase_cycles (host, out, may be NULL):
- * long long[148*8]; [cta*8 + k] = SM cycles thread 0 of CTA cta spent in phase k of the last launch (0 load, 1 local
- * arg-max, 2 publish, 3 wait for all candidates, 4 fetch pivot row, 5 interchange + rank-1 update).  Synchronises. */
-int hprmat_probe_panel(void *cuda_stream, int m, int reps, float *A_re, float *A_im, int lda, void *workspace,
-                       double *us_per_panel, long long *phase_cycles);
-/* number of kernel launches issued by this library since process start (bench.py's gpu_launches) */
-long long hprmat_launch_count(void);
-
 #ifdef __cplusplus
 }
 #endif

@@ -1,0 +1,38 @@
+/*
+ * hprmat_profile.h -- measurement aids of bench.py; NOT part of the product interface (include/hprmat.h).
+ *
+ * libhprmat.so exports the per-launch timing record and the launch counter below; the FP64 tensor-core peak probe lives
+ * in a library of its own (libhprmat_bench.so, built from paper_2512_11590_b200/bench_csrc/) that the product never loads.
+ */
+#ifndef HPRMAT_PROFILE_H
+#define HPRMAT_PROFILE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* While enabled, every launch of the GEMM, panel, row-interchange and inverse kernels inside the LU and the triangular
+ * solves is bracketed by a CUDA-event pair on its stream (which also serialises the side stream's work into the sums, and
+ * switches the CUDA-graph replay of the factorisation off).  Process-wide record; hprmat_profile_read synchronises those
+ * events, returns the summed GEMM milliseconds, the summed algorithmic flops (8 m n k per launch) and the launch count, and
+ * resets the record. */
+int hprmat_profile(int enable);
+int hprmat_profile_read(double *ms, double *flops, long long *launches);
+/* Per-category totals of the record consumed by the last hprmat_profile_read: cat 0 = trailing-update GEMMs of the LU,
+ * 1 = GEMMs of the U12 triangular solves inside the LU, 2 = panel factorisations (top-block kernel, L21 product and its
+ * check; or the pivoting panel kernels), 3 = row interchanges, 4 = GEMMs of the right-hand-side triangular solves,
+ * 5 = other.  ms/flops/launches host, may be NULL. */
+int hprmat_profile_cat(int cat, double *ms, double *flops, long long *launches);
+/* number of kernel launches issued by libhprmat.so since process start, kernels replayed from a CUDA graph included
+ * (bench.py's gpu_launches) */
+long long hprmat_launch_count(void);
+
+/* libhprmat_bench.so: FP64 tensor-core (DMMA, mma.sync.m8n8k4.f64) issue-rate ceiling of the device, measured with a
+ * register-resident loop (no memory traffic) on 148*ctas_per_sm CTAs of 8 warps, `iters` x 8 MMAs per warp.
+ * tflops (host, out): real TFLOP/s; ms (host, out, may be NULL): device time of the timed launch.  Synchronises. */
+int hprmat_bench_dmma_peak(void *cuda_stream, int iters, int ctas_per_sm, double *tflops, double *ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HPRMAT_PROFILE_H */

@@ -14,7 +14,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIBPATH = os.path.join(HERE, "libhprmat.so")
 
 HPRMAT_FP64, HPRMAT_MIXED, HPRMAT_MIXED_REFINE = 1, 2, 3
-HPRMAT_OK, HPRMAT_ESINGULAR, HPRMAT_ENOTCONVERGED, HPRMAT_ENOMEM, HPRMAT_ECUDA = 0, 1, 2, 3, 4
+HPRMAT_OK, HPRMAT_ESINGULAR, HPRMAT_ENOTCONVERGED, HPRMAT_ENOMEM, HPRMAT_ECUDA, HPRMAT_EUNVERIFIED = 0, 1, 2, 3, 4, 5
+HPRMAT_OPT_FP64_ALGO, HPRMAT_OPT_ZGEMM_ALGO = 1, 2
 MODES = {"fp64": HPRMAT_FP64, "mixed": HPRMAT_MIXED, "mixed_refine": HPRMAT_MIXED_REFINE}
 
 
@@ -96,28 +97,22 @@ def hprmat_profile_cat(cat: int):
     return ms.value, fl.value, n.value
 
 
-def hprmat_probe_dmma(iters=20000, ctas_per_sm=2, stream=None):
+_bench_lib = None
+
+
+def hprmat_bench_dmma_peak(iters=20000, ctas_per_sm=2, stream=None):
+    """FP64 tensor-core issue-rate ceiling (TFLOP/s, ms) from libhprmat_bench.so -- bench.py's roofline denominator; the
+    product library does not contain this probe (include/hprmat_profile.h)."""
+    global _bench_lib
+    if _bench_lib is None:
+        path = os.path.join(HERE, "libhprmat_bench.so")
+        if not os.path.exists(path):
+            raise ImportError(f"{path} not found: run `python -m paper_2512_11590_b200.build`")
+        _bench_lib = C.CDLL(path)
     tf, ms = C.c_double(0), C.c_double(0)
-    _check(lib().hprmat_probe_dmma(_stream(stream), C.c_int(iters), C.c_int(ctas_per_sm), C.byref(tf), C.byref(ms)),
-           "hprmat_probe_dmma")
+    _check(_bench_lib.hprmat_bench_dmma_peak(_stream(stream), C.c_int(iters), C.c_int(ctas_per_sm), C.byref(tf), C.byref(ms)),
+           "hprmat_bench_dmma_peak")
     return tf.value, ms.value
-
-
-def hprmat_probe_panel(m: int, reps: int = 20, stream=None):
-    """Mean device time (us) of the panel-factorisation kernel on an m x 32 complex64 panel + per-phase cycles."""
-    import torch
-    g = torch.Generator(device="cuda").manual_seed(7)
-    Are = torch.rand((32, m), dtype=torch.float32, device="cuda", generator=g)
-    Aim = torch.rand((32, m), dtype=torch.float32, device="cuda", generator=g)
-    wsb = int(lib().hprmat_workspace_bytes(C.c_int(m), C.c_int(0), C.c_int(HPRMAT_MIXED)))
-    ws = torch.empty(wsb + 256, dtype=torch.uint8, device="cuda")
-    wp = (ws.data_ptr() + 255) // 256 * 256
-    us = C.c_double(0)
-    ph = (C.c_longlong * (148 * 8))()
-    _check(lib().hprmat_probe_panel(_stream(stream), C.c_int(m), C.c_int(reps), C.c_void_p(Are.data_ptr()),
-                                    C.c_void_p(Aim.data_ptr()), C.c_int(m), C.c_void_p(wp), C.byref(us), ph),
-           "hprmat_probe_panel")
-    return us.value, [[int(ph[c * 8 + k]) for k in range(6)] for c in range(148)]
 
 
 # ---- structured R-matrix path ---------------------------------------------------------------------------------------
@@ -180,6 +175,18 @@ class Context:
                                      C.byref(info))
         _check(rc, "hprmat_solve_host", allow)
         return R_host, info.as_dict()
+
+    def set_option(self, option, value):
+        """hprmat_set_option: per-context algorithm switches (0 = follow the process default)."""
+        _check(lib().hprmat_set_option(self._h, C.c_int(option), C.c_int(value)), "hprmat_set_option")
+
+    def last_status(self):
+        """hprmat_last_status: (status code, refinement steps, pivot index) of the last solve; synchronises."""
+        steps, piv = C.c_int(0), C.c_int(0)
+        rc = lib().hprmat_last_status(self._h, C.byref(steps), C.byref(piv))
+        if rc < 0:
+            raise HprmatError(rc, "hprmat_last_status")
+        return rc, steps.value, piv.value
 
     def get_x(self, device="cuda"):
         X = torch.empty((self.nch, self.n), dtype=torch.complex128, device=device)  # column-major N x nch

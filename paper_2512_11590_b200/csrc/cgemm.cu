@@ -228,11 +228,8 @@ template <int BN>
 int launch_cgemm(cudaStream_t st, int m, int n, int k, float alpha, CView A, CView B, float beta, CView C) {
     typedef CgCfg<BN> Cfg;
     auto kern = cgemm_tf32_kernel<BN>;
-    static bool configured = false;
-    if (!configured) {
-        HP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM));
-        configured = true;
-    }
+    static SmemCfg cfg;
+    HP_TRY(configure_smem(cfg, kern, Cfg::SMEM));
     CgMaps maps;
     const int kk = k > 0 ? k : 1;
     HP_TRY(make_map(&maps.a_re, A.re, m, kk, A.ld, 32, CG_KC, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B));

@@ -202,11 +202,8 @@ int cgemm3_batched(cudaStream_t st, int m, int n, int k, double alpha, CView A, 
     if (k <= 0 && beta == 1.0) return 0;
     if (((uintptr_t)A.re | (uintptr_t)A.im | (uintptr_t)B.re | (uintptr_t)B.im) & 15) return -6;
     if ((A.ld | B.ld | strideA | strideB) & 3) return -7;
-    static bool configured = false;
-    if (!configured) {
-        HP_CUDA(cudaFuncSetAttribute(cgemm3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C3_SMEM));
-        configured = true;
-    }
+    static SmemCfg cfg;
+    HP_TRY(configure_smem(cfg, cgemm3_kernel, C3_SMEM));
     const bool prof = prof_enabled() && k > 0;
     if (prof) prof_begin(st, 8.0 * m * n * k * nbatch);
     cgemm3_kernel<<<dim3(ceil_div(m, C3_BM) * ceil_div(n, C3_BN), nbatch), C3_NT, C3_SMEM, st>>>(

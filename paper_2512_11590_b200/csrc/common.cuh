@@ -4,13 +4,15 @@
 #include <stdint.h>
 #include <stdio.h>
 
+#include <atomic>
+
 #include "../../include/hprmat.h"
 
 namespace hp {
 
 // ---- error plumbing ------------------------------------------------------------------------------------------------
 extern thread_local char g_cuda_err[256];
-extern long long g_launches;
+extern std::atomic<long long> g_launches;
 
 inline int cuda_fail(cudaError_t e, const char *file, int line) {
     snprintf(g_cuda_err, sizeof(g_cuda_err), "%s (%s:%d)", cudaGetErrorString(e), file, line);
@@ -29,7 +31,7 @@ inline int cuda_fail(cudaError_t e, const char *file, int line) {
 // after a kernel launch: count it and pick up launch-configuration errors
 #define HP_LAUNCHED()                  \
     do {                               \
-        ++hp::g_launches;              \
+        hp::g_launches.fetch_add(1, std::memory_order_relaxed); \
         HP_CUDA(cudaPeekAtLastError()); \
     } while (0)
 
@@ -37,7 +39,7 @@ constexpr int kNumSMs = 148;  // B200
 
 // launch categories of the per-launch timing (hprmat_profile_cat)
 enum { PROF_LU_GEMM = 0, PROF_LU_TRSM = 1, PROF_PANEL = 2, PROF_LASWP = 3, PROF_SOLVE = 4, PROF_OTHER = 5, PROF_NCAT = 6 };
-extern int g_prof_cat;
+extern thread_local int g_prof_cat;
 struct ProfCat {  // RAII: category of the launches issued in this scope
     int prev;
     explicit ProfCat(int c) : prev(g_prof_cat) { g_prof_cat = c; }
@@ -59,6 +61,34 @@ __device__ __forceinline__ void raster(int pid, int tiles_m, int tiles_n, int gr
     tm = first + r % gsz;
     tn = r / gsz;
 }
+
+// Lazy, thread-safe, per-device configuration of a kernel's dynamic shared-memory limit (cudaFuncSetAttribute is per
+// device; setting it twice is harmless, so the only shared state is a monotone per-device maximum).
+struct SmemCfg {
+    std::atomic<int> bytes[32];
+};
+template <class K> inline int configure_smem(SmemCfg &c, K kern, size_t bytes) {
+    int dev = 0;
+    HP_CUDA(cudaGetDevice(&dev));
+    const bool tracked = dev >= 0 && dev < 32;
+    if (tracked && c.bytes[dev].load(std::memory_order_acquire) >= (int)bytes) return 0;
+    HP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    if (tracked) {
+        int cur = c.bytes[dev].load(std::memory_order_relaxed);
+        while (cur < (int)bytes && !c.bytes[dev].compare_exchange_weak(cur, (int)bytes, std::memory_order_release)) {
+        }
+    }
+    return 0;
+}
+
+// Real decomposition of the complex128 GEMM (3 = 3M, 4 = 4M) in force on this host thread: the process default
+// (hprmat_zgemm_algo) unless a context's own setting is installed for the duration of one of its calls.
+int zgemm_algo_in_force();
+struct ScopedZgemmAlgo {
+    int prev;
+    explicit ScopedZgemmAlgo(int algo);
+    ~ScopedZgemmAlgo();
+};
 
 inline int ceil_div(long a, long b) { return (int)((a + b - 1) / b); }
 inline long round_up(long a, long b) { return (a + b - 1) / b * b; }
@@ -126,6 +156,29 @@ template <class E> __device__ __forceinline__ E crecip(E a) {
     } else {
         T r = a.x / a.y, d = a.x * r + a.y;
         return mk(r / d, (T)-1 / d);
+    }
+}
+
+// 1/a by Smith's formula on the reciprocal intrinsics (two dependent reciprocals, no IEEE-division slow paths)
+__device__ __forceinline__ float rcp_rn(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ double rcp_rn(double x) { return __drcp_rn(x); }
+template <class E> __device__ __forceinline__ E crecip_fast(E a) {
+    typedef typename real_of<E>::type T;
+    if (fabs(a.x) >= fabs(a.y)) {
+        const T r = a.y * rcp_rn(a.x), id = rcp_rn(a.x + a.y * r);
+        return mk(id, -r * id);
+    } else {
+        const T r = a.x * rcp_rn(a.y), id = rcp_rn(a.x * r + a.y);
+        return mk(r * id, -id);
+    }
+}
+
+// compile-time loop: f(IntC<I>) for I = B .. E-1 (keeps register-resident tiles statically indexed)
+template <int I> struct IntC { static constexpr int value = I; };
+template <int B, int E_, class F> __device__ __forceinline__ void static_for(F &&f) {
+    if constexpr (B < E_) {
+        f(IntC<B>{});
+        static_for<B + 1, E_>(f);
     }
 }
 

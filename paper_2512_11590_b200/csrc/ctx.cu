@@ -1,5 +1,7 @@
-// ctx.cu -- the structured entries of the C ABI: hprmat_setup / mesh / solve / solve_host / get_x / get_matrix / destroy.
-// Host side only sequences kernels on the context's stream; every arithmetic step of the path runs on the GPU.
+// ctx.cu -- the structured entries of the C ABI: hprmat_setup / mesh / solve / solve_nonlocal / solve_host / get_x /
+// get_matrix / last_status / set_option / destroy.
+// Host side only sequences kernels on the context's stream; every arithmetic step of the path runs on the GPU, including
+// the stopping rule of the refinement (refine_verdict_kernel): a synchronised call reads the device status once, at the end.
 //
 // Setup (once per context, host, long double): Gauss-Legendre mesh on (0,a), surface values f_i(a)
 // (the q2(r_i) of PAPER.md:85,133) and the kinetic + Bloch table T.  The paper only names these
@@ -11,6 +13,7 @@
 //          * [nb^2 + nb + 1 + (x_i + x_j - 2 x_i x_j)/(x_i - x_j)^2 - 1/(1-x_i) - 1/(1-x_j)]
 #include <math.h>
 
+#include <algorithm>
 #include <vector>
 
 #include "lu.cuh"
@@ -45,6 +48,17 @@ struct hprmat_ctx {
     cudaEvent_t ev[8] = {};
     bool have_x = false;
     StructTables tab;
+    // per-context settings (0 = follow the process default), see hprmat_set_option
+    int fp64_algo = 0, zgemm_algo = 0;
+    // side stream of the factorisations of this context + its fork/join events
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    // refinement steps the last solve in each mode took: that many are enqueued before the single read-back of the next
+    // solve (index: HPRMAT_FP64 .. HPRMAT_MIXED_REFINE)
+    int plan_steps[4] = {0, 1, 0, 2};
+    // what the last solve was, for hprmat_last_status
+    int last_fac = -1, last_mode = 0, last_max_refine = 0;
+    bool last_valid = false;
 };
 
 namespace {
@@ -94,6 +108,9 @@ int free_ctx(hprmat_ctx *c) {
     if (c->h_info) cudaFreeHost(c->h_info);
     for (auto &e : c->ev)
         if (e) cudaEventDestroy(e);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->side) cudaStreamDestroy(c->side);
     delete c;
     return 0;
 }
@@ -198,7 +215,7 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
         HP_ALLOC(c->d_workc, wb);
         if (cudaMemsetAsync(c->d_workc, 0, wb, c->st) != cudaSuccess) { free_ctx(c); return HPRMAT_ECUDA; }
         c->wc.carve(c->d_workc, (int)N);
-        c->wc.speculate = true;  // S = I + K_d^-1 V: the diagonal is the partial-pivoting choice; verified per panel (panel.cu)
+        c->wc.speculate = true;  // S = I + K_d^-1 V: the diagonal is the partial-pivoting choice; verified (toplu.cu)
     }
     HP_ALLOC(c->d_X, sizeof(double2) * N * nch);
     HP_ALLOC(c->d_Rr, sizeof(double2) * N * nch);
@@ -206,16 +223,35 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
     HP_ALLOC(c->d_V, sizeof(double2) * (size_t)nb * nch * nch);
     HP_ALLOC(c->d_R, sizeof(double2) * (size_t)nch * nch);
     HP_ALLOC(c->d_ipiv, sizeof(int) * N);
-    HP_ALLOC(c->d_info, sizeof(int) * 4);
-    HP_ALLOC(c->d_scal, sizeof(double) * 16);
-    if (cudaMallocHost((void **)&c->h_scal, sizeof(double) * 16) != cudaSuccess ||
-        cudaMallocHost((void **)&c->h_info, sizeof(int) * 4) != cudaSuccess) {
+    HP_ALLOC(c->d_info, sizeof(int) * IN_NWORDS);
+    HP_ALLOC(c->d_scal, sizeof(double) * SC_NWORDS);
+    if (cudaMallocHost((void **)&c->h_scal, sizeof(double) * SC_NWORDS) != cudaSuccess ||
+        cudaMallocHost((void **)&c->h_info, sizeof(int) * IN_NWORDS) != cudaSuccess) {
         cudaGetLastError();
         free_ctx(c);
         return HPRMAT_ENOMEM;
     }
     for (auto &e : c->ev)
         if (cudaEventCreate(&e) != cudaSuccess) { free_ctx(c); return HPRMAT_ECUDA; }
+    if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        free_ctx(c);
+        return HPRMAT_ECUDA;
+    }
+    for (LuWork<ZView> *w : {&c->wz}) { w->side = c->side; w->ev_fork = c->ev_fork; w->ev_join = c->ev_join; w->refuted = c->d_info + IN_REFUTED; }
+    for (LuWork<CView> *w : {&c->wc}) { w->side = c->side; w->ev_fork = c->ev_fork; w->ev_join = c->ev_join; w->refuted = c->d_info + IN_REFUTED; }
+    {   // ||B||_inf of the surface right-hand sides, read by the backward-error kernel from device memory
+        double bn = 0.0;
+        for (double f : c->fa) bn = std::max(bn, fabs(f));
+        cudaError_t e0 = cudaMemsetAsync(c->d_scal, 0, sizeof(double) * SC_NWORDS, c->st);
+        cudaError_t e1 = cudaMemcpyAsync(c->d_scal + SC_BNORM, &bn, sizeof(double), cudaMemcpyHostToDevice, c->st);
+        cudaError_t e2 = cudaMemsetAsync(c->d_info, 0, sizeof(int) * IN_NWORDS, c->st);
+        cudaError_t e3 = cudaStreamSynchronize(c->st);
+        for (cudaError_t e : {e0, e1, e2, e3})
+            if (e != cudaSuccess) { free_ctx(c); return hp::cuda_fail(e, __FILE__, __LINE__); }
+    }
     cudaError_t e1 = cudaMemcpyAsync(c->d_hT, hT.data(), sizeof(double) * nb * nb, cudaMemcpyHostToDevice, c->st);
     cudaError_t e2 = cudaMemcpyAsync(c->d_dg0, dg0.data(), sizeof(double) * N, cudaMemcpyHostToDevice, c->st);
     cudaError_t e3 = cudaMemcpyAsync(c->d_ethr, ethr, sizeof(double) * nch, cudaMemcpyHostToDevice, c->st);
@@ -258,378 +294,50 @@ extern "C" int hprmat_get_x(const hprmat_ctx *ctx, void *X) {
     return HPRMAT_OK;
 }
 
+
+// ======================================================================================================================
+// One driver for every structured solve.  What varies:
+//   the problem   local potentials V (mesh-diagonal couplings, Eq. 4) or a dense non-local potential matrix W (reading R15);
+//   the factored matrix
+//     FAC_C_Z   C - E I itself, FP64 LU with partial pivoting               (the paper's Type 1)
+//     FAC_S_Z   S = K_d^-1 (C - E I) in FP64, verified diagonal pivots      (the matrix of the paper's Type 3, Eqs. 7-9)
+//     FAC_S_C   S in planar complex64, TF32 tensor-core trailing update     (Types 2/4)
+//   whether non-convergence of the refinement is an error (mixed+refine) or the rounding floor (FP64).
+// Residual, stopping rule and reported backward error always refer to the ORIGINAL system (C - E I) X = B.
+// ======================================================================================================================
 namespace {
 
-int solve_fp64(hprmat_ctx *c, double energy, const double2 *V, int max_refine, double tol, double2 *R, hprmat_info *info) {
-    cudaStream_t st = c->st;
-    const int N = c->n, nch = c->nch;
-    const bool timed = info != nullptr;
-    ZView A(c->d_C, N), X(c->d_X, N), D(c->d_Rr, N);
-    if (max_refine < 0) max_refine = 2;
-    if (!(tol > 0.0)) tol = 1e-13;
-    int status = HPRMAT_OK, steps = 0;
-    double rmax = 0.0;
+enum Fac { FAC_C_Z = 0, FAC_S_Z = 1, FAC_S_C = 2 };
+constexpr int UNUSABLE = -1000;  // internal: the verified-diagonal factorisation cannot be trusted here (refuted pivots,
+                                 // singular diagonal block, ill-conditioned preconditioner): factor with pivoting instead
 
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[0], st));
-    HP_TRY(assemble_z(st, c->tab, energy, V, c->d_C, N));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[1], st));
-    HP_CUDA(cudaMemsetAsync(c->d_info, 0, sizeof(int), st));
-    HP_TRY(getrf<ZView>(st, N, A, c->d_ipiv, c->d_info, c->wz));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[2], st));
-    if (timed) {
-        HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, sizeof(int), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        if (c->h_info[0] != 0) {
-            info->status = HPRMAT_ESINGULAR;
-            info->pivot_index = c->h_info[0];
-            return HPRMAT_ESINGULAR;
-        }
-    }
-    HP_TRY(build_rhs(st, c->tab, c->d_X, N));
-    HP_TRY(getrs<ZView>(st, N, nch, A, X, c->wz));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[3], st));
-    double dprev = 0.0;
-    if (timed && max_refine > 0) {
-        HP_TRY(maxabs(st, N, nch, c->d_X, N, c->d_scal + 2));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 2, c->d_scal + 2, sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        dprev = c->h_scal[2];
-    }
-    for (int k = 0; k < max_refine; ++k) {
-        HP_TRY(structured_residual(st, c->tab, energy, V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, c->d_scal + 3));
-        HP_TRY(getrs<ZView>(st, N, nch, A, D, c->wz));
-        HP_TRY(axpy_norm(st, N, nch, c->d_X, N, c->d_Rr, N, c->d_scal));
-        ++steps;
-        if (timed) {
-            HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
-            HP_CUDA(cudaStreamSynchronize(st));
-            const double dn = c->h_scal[0], xn = c->h_scal[1];
-            rmax = c->h_scal[3];
-            const int v = refine_verdict(dn, xn, dprev, tol);
-            dprev = dn;
-            if (v != REF_CONTINUE) break;  // FP64 mode: a stagnated correction is at the rounding floor, not a failure
-        }
-    }
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[4], st));
-    HP_TRY(contract(st, c->tab, c->d_X, N, R));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[5], st));
-    c->have_x = true;
-    if (timed) {
-        // backward error of the returned X (PAPER.md:139 accuracy reference; definition in DESIGN.md reading R8)
-        HP_TRY(structured_residual(st, c->tab, energy, V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, c->d_scal + 3));
-        HP_TRY(structured_anorm(st, c->tab, energy, V, c->d_scal + 4));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 3, c->d_scal + 3, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        double bn = 0.0;
-        for (double f : c->fa) bn = std::max(bn, fabs(f));
-        HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        info->status = status;
-        info->refine_steps = steps;
-        info->pivot_index = 0;
-        info->resid_max = c->h_scal[3];
-        info->backward_err = c->h_scal[5];
-        info->ms_assemble = ev_ms(c->ev[0], c->ev[1]);
-        info->ms_lu = ev_ms(c->ev[1], c->ev[2]);
-        info->ms_solve = ev_ms(c->ev[2], c->ev[3]);
-        info->ms_refine = ev_ms(c->ev[3], c->ev[4]);
-        info->ms_contract = ev_ms(c->ev[4], c->ev[5]);
-        info->ms_total = ev_ms(c->ev[0], c->ev[5]);
-        info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)N * N * N / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
-        (void)rmax;
-    }
-    return status;
+struct Problem {
+    const double2 *V = nullptr;  // local: dev [nb][nch][nch]; non-local: the context's zeroed d_V ("no local potential")
+    const double2 *W = nullptr;  // non-local: dev N x N, ld ldw
+    long ldw = 0;
+};
+
+// ---- the device-side stopping rule --------------------------------------------------------------------------------------
+__global__ void refine_begin_kernel(double *scal, int *info, int x0_word) {
+    scal[SC_DPREV] = scal[x0_word];
+    scal[SC_DN_LAST] = 0.0;
+    scal[SC_XN_LAST] = scal[x0_word];
+    info[IN_VERDICT] = REF_CONTINUE;
+    info[IN_STEPS] = 0;
+}
+// after the (gated) update of step k: norms of the correction and of X are in scal[SC_DN], scal[SC_XN]
+__global__ void refine_verdict_kernel(double *scal, int *info, double tol) {
+    if (info[IN_VERDICT] != REF_CONTINUE) return;  // stopped earlier: this step did not touch X
+    const double dn = scal[SC_DN], xn = scal[SC_XN];
+    info[IN_VERDICT] = refine_verdict(dn, xn, scal[SC_DPREV], tol);
+    info[IN_STEPS] += 1;
+    scal[SC_DPREV] = dn;
+    scal[SC_DN_LAST] = dn;
+    scal[SC_XN_LAST] = xn;
 }
 
-// FP64 mode, preconditioned form (the default; hprmat_fp64_algo): the FP64 LU is applied to S = K_d^-1 (C - E I), the matrix
-// of the paper's Type 3 (Eqs. 7-9), instead of C - E I itself.  Same N x N complex LU with partial pivoting and the same
-// 8N^3/3 flops, but S = I + (coupling-sized entries): the pivots partial pivoting selects are the diagonal ones, which the
-// speculative panel (panel.cu) verifies column by column -- the sequential pivot search across all SMs (N dependent
-// exchanges, ~0.1 s at N = 25600) disappears, and with kappa(S) = O(1) the first solve is already at the rounding floor.
-// The residual of the refinement and the reported backward error are those of the ORIGINAL system (C - E I) X = B.
-constexpr int PRECOND_UNUSABLE = -1000;  // internal: the synchronised call falls back to the LU of C - E I
-
-int solve_fp64_precond(hprmat_ctx *c, double energy, const double2 *V, int max_refine, double tol, double2 *R,
-                       hprmat_info *info) {
-    cudaStream_t st = c->st;
-    const int N = c->n, nch = c->nch, nb = c->nb;
-    const bool timed = info != nullptr;
-    ZView S(c->d_C, N), X(c->d_X, N), D(c->d_Rlo, N);
-    if (max_refine < 0) max_refine = 2;
-    if (!(tol > 0.0)) tol = 1e-13;
-    int steps = 0;
-
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[0], st));
-    HP_CUDA(cudaMemsetAsync(c->d_info, 0, 2 * sizeof(int), st));
-    HP_TRY(precond_invert(st, c->tab, energy, V, c->d_Kinv, c->d_info + 1));
-    HP_TRY(precond_assemble_z(st, c->tab, c->d_Kinv, V, S));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[1], st));
-    c->wz.speculate = true;
-    const int rc_lu = getrf<ZView>(st, N, S, c->d_ipiv, c->d_info, c->wz);
-    c->wz.speculate = false;
-    HP_TRY(rc_lu);
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[2], st));
-    if (timed) {
-        HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        if (c->h_info[0] != 0 || c->h_info[1] != 0) return PRECOND_UNUSABLE;  // e.g. E on a pole of an uncoupled channel
-    }
-    HP_TRY(precond_rhs_z(st, c->tab, c->d_Kinv, X));
-    HP_TRY(getrs<ZView>(st, N, nch, S, X, c->wz));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[3], st));
-    double dprev = 0.0;
-    if (timed && max_refine > 0) {
-        HP_TRY(maxabs(st, N, nch, c->d_X, N, c->d_scal + 2));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 2, c->d_scal + 2, sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        dprev = c->h_scal[2];
-    }
-    for (int k = 0; k < max_refine; ++k) {
-        HP_TRY(structured_residual(st, c->tab, energy, V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, c->d_scal + 3));
-        // z = K_d^-1 r (one nb x nb by nb x nch product per channel), d = S^-1 z
-        HP_TRY(zgemm_batched(st, nb, nch, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, c->d_Rr, N, nb, 0.0, c->d_Rlo, N, nb, nch));
-        HP_TRY(getrs<ZView>(st, N, nch, S, D, c->wz));
-        HP_TRY(axpy_norm(st, N, nch, c->d_X, N, c->d_Rlo, N, c->d_scal));
-        ++steps;
-        if (timed) {
-            HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
-            HP_CUDA(cudaStreamSynchronize(st));
-            const double dn = c->h_scal[0], xn = c->h_scal[1];
-            const int v = refine_verdict(dn, xn, dprev, tol);
-            dprev = dn;
-            if (v != REF_CONTINUE) {
-                // FP64 mode: a stagnated correction is at the rounding floor, not a failure -- unless it is large: then the
-                // preconditioner is ill-conditioned at this energy (near a pole of an uncoupled channel)
-                if (!(dn <= 1e-9 * xn)) return PRECOND_UNUSABLE;
-                break;
-            }
-        }
-    }
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[4], st));
-    HP_TRY(contract(st, c->tab, c->d_X, N, R));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[5], st));
-    c->have_x = true;
-    if (timed) {
-        HP_TRY(structured_residual(st, c->tab, energy, V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, c->d_scal + 3));
-        HP_TRY(structured_anorm(st, c->tab, energy, V, c->d_scal + 4));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 3, c->d_scal + 3, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        double bn = 0.0;
-        for (double f : c->fa) bn = std::max(bn, fabs(f));
-        HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        if (!(c->h_scal[5] <= 50.0 * N * 1.1102230246251565e-16)) return PRECOND_UNUSABLE;
-        info->status = HPRMAT_OK;
-        info->refine_steps = steps;
-        info->pivot_index = 0;
-        info->resid_max = c->h_scal[3];
-        info->backward_err = c->h_scal[5];
-        info->ms_assemble = ev_ms(c->ev[0], c->ev[1]);
-        info->ms_lu = ev_ms(c->ev[1], c->ev[2]);
-        info->ms_solve = ev_ms(c->ev[2], c->ev[3]);
-        info->ms_refine = ev_ms(c->ev[3], c->ev[4]);
-        info->ms_contract = ev_ms(c->ev[4], c->ev[5]);
-        info->ms_total = ev_ms(c->ev[0], c->ev[5]);
-        info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)N * N * N / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
-    }
-    return HPRMAT_OK;
-}
-
-// Mixed modes (PAPER.md:147-151 Type 2, :192-230 Type 4; preconditioned per reading R10):
-//   Kinv = K_d^-1 (FP64) -> S = K_d^-1 (C - E I) in split complex64 -> P L U = S (TF32 tensor-core trailing update)
-//   -> X0 = S^-1 (K_d^-1 B)  [HPRMAT_MIXED stops here]
-//   -> repeat: r = B - (C - E I) X (FP64, double-double, matrix-free); z = K_d^-1 r (FP64); d = S^-1 z (complex64
-//      factors); X += d; until the correction is below tol or stagnates.
-int solve_mixed(hprmat_ctx *c, double energy, const double2 *V, bool refine, int max_refine, double tol, double2 *R,
-                hprmat_info *info) {
-    cudaStream_t st = c->st;
-    const int N = c->n, nch = c->nch, nb = c->nb;
-    const bool timed = info != nullptr;
-    CView S(c->d_Sre, c->d_Sim, c->ldS), Bs(c->d_Bre, c->d_Bim, c->ldS);
-    if (max_refine < 0) max_refine = 5;
-    if (!refine) max_refine = 0;
-    if (!(tol > 0.0)) tol = 1e-12;  // estimated relative error left in X; the north-star asks 1e-10 of R
-    int status = HPRMAT_OK, steps = 0;
-
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[0], st));
-    HP_CUDA(cudaMemsetAsync(c->d_info, 0, 2 * sizeof(int), st));
-    HP_TRY(precond_invert(st, c->tab, energy, V, c->d_Kinv, c->d_info + 1));
-    HP_TRY(precond_assemble(st, c->tab, c->d_Kinv, V, S));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[1], st));
-    HP_TRY(getrf<CView>(st, N, S, c->d_ipiv, c->d_info, c->wc));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[2], st));
-    if (timed) {
-        HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        if (c->h_info[0] != 0 || c->h_info[1] != 0) {
-            info->status = HPRMAT_ESINGULAR;
-            info->pivot_index = c->h_info[0] ? c->h_info[0] : c->h_info[1];
-            return HPRMAT_ESINGULAR;
-        }
-    }
-    HP_TRY(precond_rhs(st, c->tab, c->d_Kinv, Bs));
-    HP_TRY(getrs<CView>(st, N, nch, S, Bs, c->wc));
-    HP_TRY(promote_add(st, N, nch, c->d_X, N, Bs, false, c->d_scal));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[3], st));
-    double dprev = 0.0;
-    if (max_refine > 0) {
-        HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        dprev = c->h_scal[1];
-        status = HPRMAT_ENOTCONVERGED;
-    }
-    for (int k = 0; k < max_refine; ++k) {
-        HP_TRY(structured_residual(st, c->tab, energy, V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, c->d_scal + 3));
-        // z = K_d^-1 r: one nb x nb by nb x nch product per channel (FP64 tensor cores), into Rlo
-        HP_TRY(zgemm_batched(st, nb, nch, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, c->d_Rr, N, nb, 0.0, c->d_Rlo, N, nb, nch));
-        HP_TRY(demote(st, N, nch, c->d_Rlo, N, Bs));
-        HP_TRY(getrs<CView>(st, N, nch, S, Bs, c->wc));
-        HP_TRY(promote_add(st, N, nch, c->d_X, N, Bs, true, c->d_scal));
-        ++steps;
-        HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        const double dn = c->h_scal[0], xn = c->h_scal[1];
-        const int v = refine_verdict(dn, xn, dprev, tol);
-        dprev = dn;
-        if (v == REF_CONVERGED) { status = HPRMAT_OK; break; }
-        if (v == REF_STAGNATED) {
-            // a correction at the FP64 rounding floor of X is convergence, not failure
-            status = (dn <= 64.0 * 2.220446049250313e-16 * xn) ? HPRMAT_OK : HPRMAT_ENOTCONVERGED;
-            break;
-        }
-    }
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[4], st));
-    HP_TRY(contract(st, c->tab, c->d_X, N, R));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[5], st));
-    c->have_x = true;
-    if (timed) {
-        HP_TRY(structured_residual(st, c->tab, energy, V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, c->d_scal + 3));
-        HP_TRY(structured_anorm(st, c->tab, energy, V, c->d_scal + 4));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 3, c->d_scal + 3, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        double bn = 0.0;
-        for (double f : c->fa) bn = std::max(bn, fabs(f));
-        HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        info->status = status;
-        info->refine_steps = steps;
-        info->pivot_index = 0;
-        info->resid_max = c->h_scal[3];
-        info->backward_err = c->h_scal[5];
-        info->ms_assemble = ev_ms(c->ev[0], c->ev[1]);
-        info->ms_lu = ev_ms(c->ev[1], c->ev[2]);
-        info->ms_solve = ev_ms(c->ev[2], c->ev[3]);
-        info->ms_refine = ev_ms(c->ev[3], c->ev[4]);
-        info->ms_contract = ev_ms(c->ev[4], c->ev[5]);
-        info->ms_total = ev_ms(c->ev[0], c->ev[5]);
-        info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)N * N * N / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
-    }
-    return status;
-}
-
-}  // namespace
-
-static int g_fp64_algo = 2;  // hprmat_fp64_algo
-
-// Non-local potentials: the same path with a dense potential matrix W.
-// Residual of the refinement: B - (K + W) X = [structured residual with V = 0, double-double] - W X, the product W X on the
-// FP64 tensor cores (the LU has overwritten C, W is the caller's and intact), i.e. a working-precision residual as in
-// LAPACK's refinement: it restores the backward error, it does not add digits beyond kappa * 2^-53.
-static int nonlocal_residual(hprmat_ctx *c, double energy, const double2 *W, long ldw, double *rmax_dev) {
-    cudaStream_t st = c->st;
-    const int N = c->n, nch = c->nch;
-    HP_TRY(structured_residual(st, c->tab, energy, c->d_V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, nullptr));
-    HP_TRY(gemm(st, N, nch, N, -1.0, ZView((double2 *)W, ldw), ZView(c->d_X, N), 1.0, ZView(c->d_Rr, N)));
-    if (rmax_dev) HP_TRY(maxabs(st, N, nch, c->d_Rr, N, rmax_dev));
-    return 0;
-}
-
-static int solve_nonlocal_fp64(hprmat_ctx *c, double energy, const double2 *W, long ldw, int max_refine, double tol,
-                               double2 *R, hprmat_info *info) {
-    cudaStream_t st = c->st;
-    const int N = c->n, nch = c->nch;
-    const bool timed = info != nullptr;
-    ZView A(c->d_C, N), X(c->d_X, N), D(c->d_Rr, N);
-    if (max_refine < 0) max_refine = 2;
-    if (!(tol > 0.0)) tol = 1e-13;
-    int steps = 0;
-
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[0], st));
-    HP_CUDA(cudaMemsetAsync(c->d_V, 0, sizeof(double2) * (size_t)c->nb * nch * nch, st));  // "no local potential"
-    HP_TRY(assemble_nonlocal(st, c->tab, energy, W, ldw, c->d_C, N));
-    if (timed) HP_TRY(nonlocal_anorm(st, c->tab, energy, W, ldw, (double *)c->d_Rlo, c->d_scal + 4));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[1], st));
-    HP_CUDA(cudaMemsetAsync(c->d_info, 0, sizeof(int), st));
-    HP_TRY(getrf<ZView>(st, N, A, c->d_ipiv, c->d_info, c->wz));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[2], st));
-    if (timed) {
-        HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, sizeof(int), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        if (c->h_info[0] != 0) {
-            info->status = HPRMAT_ESINGULAR;
-            info->pivot_index = c->h_info[0];
-            return HPRMAT_ESINGULAR;
-        }
-    }
-    HP_TRY(build_rhs(st, c->tab, c->d_X, N));
-    HP_TRY(getrs<ZView>(st, N, nch, A, X, c->wz));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[3], st));
-    double dprev = 0.0;
-    if (timed && max_refine > 0) {
-        HP_TRY(maxabs(st, N, nch, c->d_X, N, c->d_scal + 2));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 2, c->d_scal + 2, sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        dprev = c->h_scal[2];
-    }
-    for (int k = 0; k < max_refine; ++k) {
-        HP_TRY(nonlocal_residual(c, energy, W, ldw, nullptr));
-        HP_TRY(getrs<ZView>(st, N, nch, A, D, c->wz));
-        HP_TRY(axpy_norm(st, N, nch, c->d_X, N, c->d_Rr, N, c->d_scal));
-        ++steps;
-        if (timed) {
-            HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-            HP_CUDA(cudaStreamSynchronize(st));
-            const double dn = c->h_scal[0], xn = c->h_scal[1];
-            const int v = refine_verdict(dn, xn, dprev, tol);
-            dprev = dn;
-            if (v != REF_CONTINUE) break;
-        }
-    }
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[4], st));
-    HP_TRY(contract(st, c->tab, c->d_X, N, R));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[5], st));
-    c->have_x = true;
-    if (timed) {
-        HP_TRY(nonlocal_residual(c, energy, W, ldw, c->d_scal + 3));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 3, c->d_scal + 3, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        double bn = 0.0;
-        for (double f : c->fa) bn = std::max(bn, fabs(f));
-        HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        info->status = HPRMAT_OK;
-        info->refine_steps = steps;
-        info->pivot_index = 0;
-        info->resid_max = c->h_scal[3];
-        info->backward_err = c->h_scal[5];
-        info->ms_assemble = ev_ms(c->ev[0], c->ev[1]);
-        info->ms_lu = ev_ms(c->ev[1], c->ev[2]);
-        info->ms_solve = ev_ms(c->ev[2], c->ev[3]);
-        info->ms_refine = ev_ms(c->ev[3], c->ev[4]);
-        info->ms_contract = ev_ms(c->ev[4], c->ev[5]);
-        info->ms_total = ev_ms(c->ev[0], c->ev[5]);
-        info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)N * N * N / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
-    }
-    return HPRMAT_OK;
-}
-
-// FP64 mode with non-local potentials, preconditioned form (hprmat_fp64_algo = 2): S = K_d^-1 (K + W) in FP64 with the full
-// diagonal blocks K_c + W_cc inverted; block row c of S is one batched DMMA product Kinv_c x (block row c of W), the diagonal
-// blocks are then overwritten by the identity.  Verified diagonal pivots as in solve_fp64_precond.
+// FP64 mode with non-local potentials, preconditioned form: block row c of S is one batched DMMA product Kinv_c x (block
+// row c of W); the diagonal blocks are then overwritten by the identity.
 __global__ void __launch_bounds__(256) set_diag_blocks_identity_kernel(int nch, int nb, double2 *__restrict__ S, long ld) {
     const long tot = (long)nch * nb * nb;
     for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < tot; idx += (long)gridDim.x * blockDim.x) {
@@ -640,184 +348,258 @@ __global__ void __launch_bounds__(256) set_diag_blocks_identity_kernel(int nch, 
     }
 }
 
-static int solve_nonlocal_fp64_precond(hprmat_ctx *c, double energy, const double2 *W, long ldw, int max_refine, double tol,
-                                       double2 *R, hprmat_info *info) {
+// ---- stages ---------------------------------------------------------------------------------------------------------------
+int assemble(hprmat_ctx *c, Fac fac, const Problem &p, double energy, bool want_anorm) {
     cudaStream_t st = c->st;
     const int N = c->n, nch = c->nch, nb = c->nb;
-    const bool timed = info != nullptr;
-    ZView S(c->d_C, N), X(c->d_X, N), D(c->d_Rlo, N);
-    if (max_refine < 0) max_refine = 2;
-    if (!(tol > 0.0)) tol = 1e-13;
-    int steps = 0;
-
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[0], st));
-    HP_CUDA(cudaMemsetAsync(c->d_V, 0, sizeof(double2) * (size_t)nb * nch * nch, st));  // "no local potential"
-    HP_CUDA(cudaMemsetAsync(c->d_info, 0, 2 * sizeof(int), st));
-    HP_TRY(precond_invert(st, c->tab, energy, c->d_V, c->d_Kinv, c->d_info + 1, W, ldw));
-    HP_TRY(zgemm_batched(st, nb, N, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, W, ldw, nb, 0.0, c->d_C, N, nb, nch));
-    {
-        const long tot = (long)nch * nb * nb;
-        set_diag_blocks_identity_kernel<<<(int)std::min<long>((tot + 255) / 256, 148 * 8), 256, 0, st>>>(nch, nb, c->d_C, N);
-        HP_LAUNCHED();
-    }
-    if (timed) HP_TRY(nonlocal_anorm(st, c->tab, energy, W, ldw, (double *)c->d_Rlo, c->d_scal + 4));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[1], st));
-    c->wz.speculate = true;
-    const int rc_lu = getrf<ZView>(st, N, S, c->d_ipiv, c->d_info, c->wz);
-    c->wz.speculate = false;
-    HP_TRY(rc_lu);
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[2], st));
-    if (timed) {
-        HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        if (c->h_info[0] != 0 || c->h_info[1] != 0) return PRECOND_UNUSABLE;
-    }
-    HP_TRY(precond_rhs_z(st, c->tab, c->d_Kinv, X));
-    HP_TRY(getrs<ZView>(st, N, nch, S, X, c->wz));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[3], st));
-    double dprev = 0.0;
-    if (timed && max_refine > 0) {
-        HP_TRY(maxabs(st, N, nch, c->d_X, N, c->d_scal + 2));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 2, c->d_scal + 2, sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        dprev = c->h_scal[2];
-    }
-    for (int k = 0; k < max_refine; ++k) {
-        HP_TRY(nonlocal_residual(c, energy, W, ldw, nullptr));
-        HP_TRY(zgemm_batched(st, nb, nch, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, c->d_Rr, N, nb, 0.0, c->d_Rlo, N, nb, nch));
-        HP_TRY(getrs<ZView>(st, N, nch, S, D, c->wz));
-        HP_TRY(axpy_norm(st, N, nch, c->d_X, N, c->d_Rlo, N, c->d_scal));
-        ++steps;
-        if (timed) {
-            HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-            HP_CUDA(cudaStreamSynchronize(st));
-            const double dn = c->h_scal[0], xn = c->h_scal[1];
-            const int v = refine_verdict(dn, xn, dprev, tol);
-            dprev = dn;
-            if (v != REF_CONTINUE) {
-                if (!(dn <= 1e-9 * xn)) return PRECOND_UNUSABLE;
-                break;
+    HP_CUDA(cudaMemsetAsync(c->d_info, 0, sizeof(int) * IN_NWORDS, st));
+    if (p.W) HP_CUDA(cudaMemsetAsync(c->d_V, 0, sizeof(double2) * (size_t)nb * nch * nch, st));  // "no local potential"
+    if (fac == FAC_C_Z) {
+        if (p.W) HP_TRY(assemble_nonlocal(st, c->tab, energy, p.W, p.ldw, c->d_C, N));
+        else HP_TRY(assemble_z(st, c->tab, energy, p.V, c->d_C, N));
+    } else {
+        HP_TRY(precond_invert(st, c->tab, energy, p.V, c->d_Kinv, c->d_info + IN_KBLOCK_SINGULAR, p.W, p.ldw));
+        if (fac == FAC_S_Z) {
+            if (p.W) {
+                HP_TRY(zgemm_batched(st, nb, N, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, p.W, p.ldw, nb, 0.0, c->d_C, N, nb, nch));
+                const long tot = (long)nch * nb * nb;
+                set_diag_blocks_identity_kernel<<<(int)std::min<long>((tot + 255) / 256, 148 * 8), 256, 0, st>>>(nch, nb, c->d_C, N);
+                HP_LAUNCHED();
+            } else {
+                HP_TRY(precond_assemble_z(st, c->tab, c->d_Kinv, p.V, ZView(c->d_C, N)));
             }
+        } else {
+            CView S(c->d_Sre, c->d_Sim, c->ldS);
+            if (p.W) HP_TRY(precond_assemble_nonlocal(st, c->tab, c->d_Kinv, p.W, p.ldw, S, c->d_Rlo, N));
+            else HP_TRY(precond_assemble(st, c->tab, c->d_Kinv, p.V, S));
         }
     }
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[4], st));
-    HP_TRY(contract(st, c->tab, c->d_X, N, R));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[5], st));
-    c->have_x = true;
-    if (timed) {
-        HP_TRY(nonlocal_residual(c, energy, W, ldw, c->d_scal + 3));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 3, c->d_scal + 3, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        double bn = 0.0;
-        for (double f : c->fa) bn = std::max(bn, fabs(f));
-        HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        if (!(c->h_scal[5] <= 50.0 * N * 1.1102230246251565e-16)) return PRECOND_UNUSABLE;
-        info->status = HPRMAT_OK;
-        info->refine_steps = steps;
-        info->pivot_index = 0;
-        info->resid_max = c->h_scal[3];
-        info->backward_err = c->h_scal[5];
-        info->ms_assemble = ev_ms(c->ev[0], c->ev[1]);
-        info->ms_lu = ev_ms(c->ev[1], c->ev[2]);
-        info->ms_solve = ev_ms(c->ev[2], c->ev[3]);
-        info->ms_refine = ev_ms(c->ev[3], c->ev[4]);
-        info->ms_contract = ev_ms(c->ev[4], c->ev[5]);
-        info->ms_total = ev_ms(c->ev[0], c->ev[5]);
-        info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)N * N * N / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
-    }
-    return HPRMAT_OK;
+    if (want_anorm && p.W) HP_TRY(nonlocal_anorm(st, c->tab, energy, p.W, p.ldw, (double *)c->d_Rlo, c->d_scal + SC_ANORM));
+    return 0;
 }
 
-// Mixed modes with non-local potentials: the block-diagonal preconditioner uses the full diagonal blocks K_c + W_cc, S has
-// full off-diagonal blocks Kinv_c W_cc'; the rest is solve_mixed with the working-precision dense residual.
-static int solve_nonlocal_mixed(hprmat_ctx *c, double energy, const double2 *W, long ldw, bool refine, int max_refine,
-                                double tol, double2 *R, hprmat_info *info) {
+int factor(hprmat_ctx *c, Fac fac, bool pivoting_fallback) {
+    cudaStream_t st = c->st;
+    const int N = c->n;
+    int *zp = c->d_info + IN_ZERO_PIVOT;
+    if (fac == FAC_S_C) {
+        c->wc.speculate = !pivoting_fallback;
+        return getrf<CView>(st, N, CView(c->d_Sre, c->d_Sim, c->ldS), c->d_ipiv, zp, c->wc);
+    }
+    c->wz.speculate = (fac == FAC_S_Z);
+    return getrf<ZView>(st, N, ZView(c->d_C, N), c->d_ipiv, zp, c->wz);
+}
+
+// X <- (factored matrix)^-1 (its right-hand sides); leaves max|X| in scal[SC_X0] (FP64) or scal[SC_XN] (complex64 factors)
+int first_solve(hprmat_ctx *c, Fac fac, int *x0_word) {
+    cudaStream_t st = c->st;
+    const int N = c->n, nch = c->nch;
+    if (fac == FAC_S_C) {
+        CView S(c->d_Sre, c->d_Sim, c->ldS), Bs(c->d_Bre, c->d_Bim, c->ldS);
+        HP_TRY(precond_rhs(st, c->tab, c->d_Kinv, Bs));
+        HP_TRY(getrs<CView>(st, N, nch, S, Bs, c->wc));
+        HP_TRY(promote_add(st, N, nch, c->d_X, N, Bs, false, c->d_scal + SC_DN));
+        *x0_word = SC_XN;
+        return 0;
+    }
+    ZView A(c->d_C, N), X(c->d_X, N);
+    if (fac == FAC_S_Z) HP_TRY(precond_rhs_z(st, c->tab, c->d_Kinv, X));
+    else HP_TRY(build_rhs(st, c->tab, c->d_X, N));
+    HP_TRY(getrs<ZView>(st, N, nch, A, X, c->wz));
+    HP_TRY(maxabs(st, N, nch, c->d_X, N, c->d_scal + SC_X0));
+    *x0_word = SC_X0;
+    return 0;
+}
+
+// Rr <- B - (C - E I) X.  Local potentials: matrix-free, double-double accumulation (exact to the rounding of the result).
+// Non-local: [structured part with V = 0, double-double] - W X on the FP64 tensor cores (working precision, reading R15).
+int residual(hprmat_ctx *c, const Problem &p, double energy, double *rmax_dev) {
+    cudaStream_t st = c->st;
+    const int N = c->n, nch = c->nch;
+    if (!p.W)
+        return structured_residual(st, c->tab, energy, p.V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, rmax_dev);
+    HP_TRY(structured_residual(st, c->tab, energy, c->d_V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, nullptr));
+    HP_TRY(gemm(st, N, nch, N, -1.0, ZView((double2 *)p.W, p.ldw), ZView(c->d_X, N), 1.0, ZView(c->d_Rr, N)));
+    if (rmax_dev) HP_TRY(maxabs(st, N, nch, c->d_Rr, N, rmax_dev));
+    return 0;
+}
+
+// X += (factored matrix)^-1 [K_d^-1] Rr, unless the device-side stopping rule has already fired
+int correction(hprmat_ctx *c, Fac fac) {
     cudaStream_t st = c->st;
     const int N = c->n, nch = c->nch, nb = c->nb;
-    const bool timed = info != nullptr;
+    const int *gate = c->d_info + IN_VERDICT;
+    if (fac == FAC_C_Z) {
+        HP_TRY(getrs<ZView>(st, N, nch, ZView(c->d_C, N), ZView(c->d_Rr, N), c->wz));
+        return axpy_norm(st, N, nch, c->d_X, N, c->d_Rr, N, c->d_scal + SC_DN, gate);
+    }
+    // z = K_d^-1 r: one nb x nb by nb x nch product per channel (FP64 tensor cores), into Rlo
+    HP_TRY(zgemm_batched(st, nb, nch, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, c->d_Rr, N, nb, 0.0, c->d_Rlo, N, nb, nch));
+    if (fac == FAC_S_Z) {
+        HP_TRY(getrs<ZView>(st, N, nch, ZView(c->d_C, N), ZView(c->d_Rlo, N), c->wz));
+        return axpy_norm(st, N, nch, c->d_X, N, c->d_Rlo, N, c->d_scal + SC_DN, gate);
+    }
     CView S(c->d_Sre, c->d_Sim, c->ldS), Bs(c->d_Bre, c->d_Bim, c->ldS);
-    if (max_refine < 0) max_refine = 5;
-    if (!refine) max_refine = 0;
-    if (!(tol > 0.0)) tol = 1e-12;
-    int status = HPRMAT_OK, steps = 0;
-
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[0], st));
-    HP_CUDA(cudaMemsetAsync(c->d_V, 0, sizeof(double2) * (size_t)nb * nch * nch, st));  // "no local potential"
-    HP_CUDA(cudaMemsetAsync(c->d_info, 0, 2 * sizeof(int), st));
-    HP_TRY(precond_invert(st, c->tab, energy, c->d_V, c->d_Kinv, c->d_info + 1, W, ldw));
-    HP_TRY(precond_assemble_nonlocal(st, c->tab, c->d_Kinv, W, ldw, S, c->d_Rlo, N));
-    if (timed) HP_TRY(nonlocal_anorm(st, c->tab, energy, W, ldw, (double *)c->d_Rlo, c->d_scal + 4));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[1], st));
-    HP_TRY(getrf<CView>(st, N, S, c->d_ipiv, c->d_info, c->wc));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[2], st));
-    if (timed) {
-        HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        if (c->h_info[0] != 0 || c->h_info[1] != 0) {
-            info->status = HPRMAT_ESINGULAR;
-            info->pivot_index = c->h_info[0] ? c->h_info[0] : c->h_info[1];
-            return HPRMAT_ESINGULAR;
-        }
-    }
-    HP_TRY(precond_rhs(st, c->tab, c->d_Kinv, Bs));
+    HP_TRY(demote(st, N, nch, c->d_Rlo, N, Bs));
     HP_TRY(getrs<CView>(st, N, nch, S, Bs, c->wc));
-    HP_TRY(promote_add(st, N, nch, c->d_X, N, Bs, false, c->d_scal));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[3], st));
-    double dprev = 0.0;
+    return promote_add(st, N, nch, c->d_X, N, Bs, true, c->d_scal + SC_DN, gate);
+}
+
+int refine_step(hprmat_ctx *c, Fac fac, const Problem &p, double energy, double tol) {
+    HP_TRY(residual(c, p, energy, nullptr));
+    HP_TRY(correction(c, fac));
+    refine_verdict_kernel<<<1, 1, 0, c->st>>>(c->d_scal, c->d_info, tol);
+    HP_LAUNCHED();
+    return 0;
+}
+
+// backward error of the returned X (definition in DESIGN.md reading R8), everything enqueued, nothing read back here
+int report(hprmat_ctx *c, const Problem &p, double energy) {
+    cudaStream_t st = c->st;
+    HP_TRY(residual(c, p, energy, c->d_scal + SC_RMAX));
+    if (!p.W) HP_TRY(structured_anorm(st, c->tab, energy, p.V, c->d_scal + SC_ANORM));
+    return backward_error(st, c->n, c->nch, c->d_Rr, c->n, c->d_X, c->n, c->d_scal + SC_ANORM, c->d_scal + SC_BNORM,
+                          c->d_scal + SC_BERR);
+}
+
+int read_back(hprmat_ctx *c) {
+    HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, sizeof(double) * SC_NWORDS, cudaMemcpyDeviceToHost, c->st));
+    HP_CUDA(cudaMemcpyAsync(c->h_info, c->d_info, sizeof(int) * IN_NWORDS, cudaMemcpyDeviceToHost, c->st));
+    HP_CUDA(cudaStreamSynchronize(c->st));
+    return 0;
+}
+
+// status of a finished solve from the device words (host copies in h_scal / h_info); pivot_index out
+int decode_status(const hprmat_ctx *c, Fac fac, bool must_converge, bool pivoting_fallback, int max_refine, bool have_berr,
+                  int *pivot_index) {
+    const int *hi = c->h_info;
+    const double *hs = c->h_scal;
+    *pivot_index = 0;
+    const bool verified_fac = (fac == FAC_S_Z) || (fac == FAC_S_C && !pivoting_fallback);
+    if (verified_fac && hi[IN_REFUTED] != 0) return UNUSABLE;
+    if (hi[IN_ZERO_PIVOT] != 0 || (fac != FAC_C_Z && hi[IN_KBLOCK_SINGULAR] != 0)) {
+        if (fac == FAC_S_Z) return UNUSABLE;  // e.g. E on a pole of an uncoupled channel: C - E I itself may be regular
+        *pivot_index = hi[IN_ZERO_PIVOT] ? hi[IN_ZERO_PIVOT] : hi[IN_KBLOCK_SINGULAR];
+        return HPRMAT_ESINGULAR;
+    }
+    const double dn = hs[SC_DN_LAST], xn = hs[SC_XN_LAST];
+    const int v = hi[IN_VERDICT];
+    if (fac == FAC_S_Z) {
+        // a correction that stopped shrinking while still large: the preconditioner is ill-conditioned at this energy
+        if (max_refine > 0 && v != REF_CONTINUE && !(dn <= 1e-9 * xn)) return UNUSABLE;
+        if (have_berr && !(hs[SC_BERR] <= 50.0 * c->n * 1.1102230246251565e-16)) return UNUSABLE;
+    }
+    if (must_converge && max_refine > 0) {
+        if (v == REF_CONVERGED) return HPRMAT_OK;
+        // a correction at the FP64 rounding floor of X is convergence, not failure
+        if (v == REF_STAGNATED && dn <= 64.0 * 2.220446049250313e-16 * xn) return HPRMAT_OK;
+        return HPRMAT_ENOTCONVERGED;  // stagnated above the floor, or max_refine steps were not enough
+    }
+    return HPRMAT_OK;  // FP64 modes: a stagnated correction is the rounding floor, not a failure
+}
+
+int run(hprmat_ctx *c, Fac fac, const Problem &p, double energy, int mode, int max_refine, double tol, double2 *R,
+        hprmat_info *info, bool pivoting_fallback) {
+    cudaStream_t st = c->st;
+    const bool sync = info != nullptr;
+    const bool mixed = fac == FAC_S_C;
+    const bool must_converge = mode == HPRMAT_MIXED_REFINE;
+    if (max_refine < 0) max_refine = mixed ? 5 : 2;
+    if (mode == HPRMAT_MIXED) max_refine = 0;
+    if (!(tol > 0.0)) tol = mixed ? 1e-12 : 1e-13;  // estimated relative error left in X; the north-star asks 1e-10 of R
+    ScopedZgemmAlgo algo_scope(c->zgemm_algo);
+
+    HP_CUDA(cudaEventRecord(c->ev[0], st));
+    HP_TRY(assemble(c, fac, p, energy, sync));
+    HP_CUDA(cudaEventRecord(c->ev[1], st));
+    HP_TRY(factor(c, fac, pivoting_fallback));
+    HP_CUDA(cudaEventRecord(c->ev[2], st));
+    int x0_word = SC_X0;
+    HP_TRY(first_solve(c, fac, &x0_word));
+    HP_CUDA(cudaEventRecord(c->ev[3], st));
+    int enq = 0;
     if (max_refine > 0) {
-        HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        dprev = c->h_scal[1];
-        status = HPRMAT_ENOTCONVERGED;
+        refine_begin_kernel<<<1, 1, 0, st>>>(c->d_scal, c->d_info, x0_word);
+        HP_LAUNCHED();
+        // as many steps as the previous solve in this mode needed go out before anything is read back; a step enqueued
+        // after the stopping rule has fired leaves X alone (gated update).  Unsynchronised calls get one spare step.
+        int plan = std::max(1, c->plan_steps[mode]);
+        if (!sync) plan = mixed ? plan + 1 : max_refine;
+        plan = std::min(plan, max_refine);
+        for (; enq < plan; ++enq) HP_TRY(refine_step(c, fac, p, energy, tol));
     }
-    for (int k = 0; k < max_refine; ++k) {
-        HP_TRY(nonlocal_residual(c, energy, W, ldw, nullptr));
-        HP_TRY(zgemm_batched(st, nb, nch, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, c->d_Rr, N, nb, 0.0, c->d_Rlo, N, nb, nch));
-        HP_TRY(demote(st, N, nch, c->d_Rlo, N, Bs));
-        HP_TRY(getrs<CView>(st, N, nch, S, Bs, c->wc));
-        HP_TRY(promote_add(st, N, nch, c->d_X, N, Bs, true, c->d_scal));
-        ++steps;
-        HP_CUDA(cudaMemcpyAsync(c->h_scal, c->d_scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        const double dn = c->h_scal[0], xn = c->h_scal[1];
-        const int v = refine_verdict(dn, xn, dprev, tol);
-        dprev = dn;
-        if (v == REF_CONVERGED) { status = HPRMAT_OK; break; }
-        if (v == REF_STAGNATED) {
-            status = (dn <= 64.0 * 2.220446049250313e-16 * xn) ? HPRMAT_OK : HPRMAT_ENOTCONVERGED;
-            break;
-        }
-    }
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[4], st));
-    HP_TRY(contract(st, c->tab, c->d_X, N, R));
-    if (timed) HP_CUDA(cudaEventRecord(c->ev[5], st));
+    HP_CUDA(cudaEventRecord(c->ev[4], st));
+    HP_TRY(contract(st, c->tab, c->d_X, c->n, R));
+    HP_CUDA(cudaEventRecord(c->ev[5], st));
     c->have_x = true;
-    if (timed) {
-        HP_TRY(nonlocal_residual(c, energy, W, ldw, c->d_scal + 3));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 3, c->d_scal + 3, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        double bn = 0.0;
-        for (double f : c->fa) bn = std::max(bn, fabs(f));
-        HP_TRY(backward_error(st, N, nch, c->d_Rr, N, c->d_X, N, c->h_scal[4], bn, c->d_scal + 5));
-        HP_CUDA(cudaMemcpyAsync(c->h_scal + 5, c->d_scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
-        HP_CUDA(cudaStreamSynchronize(st));
-        info->status = status;
-        info->refine_steps = steps;
-        info->pivot_index = 0;
-        info->resid_max = c->h_scal[3];
-        info->backward_err = c->h_scal[5];
-        info->ms_assemble = ev_ms(c->ev[0], c->ev[1]);
-        info->ms_lu = ev_ms(c->ev[1], c->ev[2]);
-        info->ms_solve = ev_ms(c->ev[2], c->ev[3]);
-        info->ms_refine = ev_ms(c->ev[3], c->ev[4]);
-        info->ms_contract = ev_ms(c->ev[4], c->ev[5]);
-        info->ms_total = ev_ms(c->ev[0], c->ev[5]);
-        info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)N * N * N / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
+    c->last_fac = fac;
+    c->last_mode = mode;
+    c->last_max_refine = max_refine;
+    c->last_valid = true;
+    if (!sync) return HPRMAT_OK;  // the status stays on the device: hprmat_last_status
+
+    HP_TRY(report(c, p, energy));
+    HP_TRY(read_back(c));
+    bool extra = false;
+    while (max_refine > 0 && c->h_info[IN_VERDICT] == REF_CONTINUE && enq < max_refine && c->h_info[IN_REFUTED] == 0 &&
+           c->h_info[IN_ZERO_PIVOT] == 0 && c->h_info[IN_KBLOCK_SINGULAR] == 0) {
+        // the prediction was short (first solve of a scan, or harder physics than the last point): one step at a time
+        HP_TRY(refine_step(c, fac, p, energy, tol));
+        ++enq;
+        extra = true;
+        HP_TRY(read_back(c));
     }
+    if (extra) {
+        HP_CUDA(cudaEventRecord(c->ev[4], st));
+        HP_TRY(contract(st, c->tab, c->d_X, c->n, R));
+        HP_CUDA(cudaEventRecord(c->ev[5], st));
+        HP_TRY(report(c, p, energy));
+        HP_TRY(read_back(c));
+    }
+    int pivot_index = 0;
+    const int status = decode_status(c, fac, must_converge, pivoting_fallback, max_refine, true, &pivot_index);
+    if (status == UNUSABLE) return UNUSABLE;
+    if (max_refine > 0 && status == HPRMAT_OK) c->plan_steps[mode] = std::max(1, c->h_info[IN_STEPS]);
+    info->status = status;
+    info->refine_steps = c->h_info[IN_STEPS];
+    info->pivot_index = pivot_index;
+    info->reserved = c->h_info[IN_REFUTED];
+    info->resid_max = c->h_scal[SC_RMAX];
+    info->backward_err = status == HPRMAT_ESINGULAR ? -1.0 : c->h_scal[SC_BERR];
+    info->ms_assemble = ev_ms(c->ev[0], c->ev[1]);
+    info->ms_lu = ev_ms(c->ev[1], c->ev[2]);
+    info->ms_solve = ev_ms(c->ev[2], c->ev[3]);
+    info->ms_refine = ev_ms(c->ev[3], c->ev[4]);
+    info->ms_contract = ev_ms(c->ev[4], c->ev[5]);
+    info->ms_total = ev_ms(c->ev[0], c->ev[5]);
+    info->lu_tflops = info->ms_lu > 0 ? (8.0 / 3.0) * (double)c->n * c->n * c->n / (info->ms_lu * 1e-3) * 1e-12 : 0.0;
     return status;
 }
+
+std::atomic<int> g_fp64_algo{2};  // process default of hprmat_fp64_algo; a context may carry its own (hprmat_set_option)
+
+int solve_any(hprmat_ctx *c, const Problem &p, double energy, int mode, int max_refine, double tol, double2 *R, hprmat_info *info) {
+    if (info) {
+        *info = hprmat_info();
+        info->backward_err = -1.0;
+    }
+    const int algo = c->fp64_algo ? c->fp64_algo : g_fp64_algo.load();
+    Fac fac = mode == HPRMAT_FP64 ? (algo == 2 ? FAC_S_Z : FAC_C_Z) : FAC_S_C;
+    int rc = run(c, fac, p, energy, mode, max_refine, tol, R, info, false);
+    if (rc == UNUSABLE) {  // only reachable from a synchronised call: redo with pivoting
+        *info = hprmat_info();
+        info->backward_err = -1.0;
+        const int refuted = c->h_info[IN_REFUTED];
+        if (fac == FAC_S_Z) rc = run(c, FAC_C_Z, p, energy, mode, max_refine, tol, R, info, false);
+        else rc = run(c, FAC_S_C, p, energy, mode, max_refine, tol, R, info, true);
+        if (rc == UNUSABLE) rc = HPRMAT_ECUDA;  // cannot happen: neither fallback is a verified factorisation
+        info->reserved = refuted;               // how many block panels refuted the diagonal (0: another reason)
+    }
+    if (info) info->status = rc;
+    return rc;
+}
+
+}  // namespace
 
 extern "C" int hprmat_solve_nonlocal(hprmat_ctx *ctx, double energy, const void *W, long ldw, int mode, int max_refine,
                                      double tol, void *R, hprmat_info *info) {
@@ -827,31 +609,31 @@ extern "C" int hprmat_solve_nonlocal(hprmat_ctx *ctx, double energy, const void 
     if (mode != HPRMAT_FP64 && mode != HPRMAT_MIXED && mode != HPRMAT_MIXED_REFINE) return -5;
     if (!(ctx->max_mode & (1 << mode))) return -5;
     if (!R) return -8;
-    if (info) {
-        *info = hprmat_info();
-        info->backward_err = -1.0;
-    }
-    if (mode == HPRMAT_FP64 && g_fp64_algo == 2) {
-        int rc2 = solve_nonlocal_fp64_precond(ctx, energy, (const double2 *)W, ldw, max_refine, tol, (double2 *)R, info);
-        if (rc2 == PRECOND_UNUSABLE) {  // synchronised calls only
-            *info = hprmat_info();
-            info->backward_err = -1.0;
-            rc2 = solve_nonlocal_fp64(ctx, energy, (const double2 *)W, ldw, max_refine, tol, (double2 *)R, info);
-        }
-        if (info) info->status = rc2;
-        return rc2;
-    }
-    const int rc = mode == HPRMAT_FP64
-                       ? solve_nonlocal_fp64(ctx, energy, (const double2 *)W, ldw, max_refine, tol, (double2 *)R, info)
-                       : solve_nonlocal_mixed(ctx, energy, (const double2 *)W, ldw, mode == HPRMAT_MIXED_REFINE, max_refine, tol,
-                                              (double2 *)R, info);
-    if (info) info->status = rc;
-    return rc;
+    Problem p;
+    p.V = ctx->d_V;
+    p.W = (const double2 *)W;
+    p.ldw = ldw;
+    return solve_any(ctx, p, energy, mode, max_refine, tol, (double2 *)R, info);
 }
 
 extern "C" int hprmat_fp64_algo(int algo) {
-    if (algo == 1 || algo == 2) g_fp64_algo = algo;
-    return g_fp64_algo;
+    if (algo == 1 || algo == 2) g_fp64_algo.store(algo);
+    return g_fp64_algo.load();
+}
+
+extern "C" int hprmat_set_option(hprmat_ctx *ctx, int option, int value) {
+    if (!ctx) return -1;
+    switch (option) {
+        case HPRMAT_OPT_FP64_ALGO:
+            if (value != 0 && value != 1 && value != 2) return -3;
+            ctx->fp64_algo = value;
+            return HPRMAT_OK;
+        case HPRMAT_OPT_ZGEMM_ALGO:
+            if (value != 0 && value != 3 && value != 4) return -3;
+            ctx->zgemm_algo = value;
+            return HPRMAT_OK;
+        default: return -2;
+    }
 }
 
 extern "C" int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int mode, int max_refine, double tol, void *R,
@@ -861,23 +643,22 @@ extern "C" int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int m
     if (mode != HPRMAT_FP64 && mode != HPRMAT_MIXED && mode != HPRMAT_MIXED_REFINE) return -4;
     if (!(ctx->max_mode & (1 << mode))) return -4;
     if (!R) return -7;
-    if (info) {
-        *info = hprmat_info();
-        info->backward_err = -1.0;
-    }
-    int rc;
-    if (mode == HPRMAT_FP64) {
-        rc = g_fp64_algo == 2 ? solve_fp64_precond(ctx, energy, (const double2 *)V, max_refine, tol, (double2 *)R, info)
-                              : solve_fp64(ctx, energy, (const double2 *)V, max_refine, tol, (double2 *)R, info);
-        if (rc == PRECOND_UNUSABLE) {  // only reachable from a synchronised call (info != NULL)
-            *info = hprmat_info();
-            info->backward_err = -1.0;
-            rc = solve_fp64(ctx, energy, (const double2 *)V, max_refine, tol, (double2 *)R, info);
-        }
-    } else {
-        rc = solve_mixed(ctx, energy, (const double2 *)V, mode == HPRMAT_MIXED_REFINE, max_refine, tol, (double2 *)R, info);
-    }
-    if (info) info->status = rc;
+    Problem p;
+    p.V = (const double2 *)V;
+    return solve_any(ctx, p, energy, mode, max_refine, tol, (double2 *)R, info);
+}
+
+// Status of the last solve of this context, for calls made with info == NULL: synchronises the stream, reads the device
+// status words and decodes them exactly as a synchronised call would have.
+extern "C" int hprmat_last_status(hprmat_ctx *ctx, int *refine_steps, int *pivot_index) {
+    if (!ctx) return -1;
+    if (!ctx->last_valid) return -1;
+    HP_TRY(read_back(ctx));
+    int piv = 0;
+    int rc = decode_status(ctx, (Fac)ctx->last_fac, ctx->last_mode == HPRMAT_MIXED_REFINE, false, ctx->last_max_refine, false, &piv);
+    if (rc == UNUSABLE) rc = HPRMAT_EUNVERIFIED;
+    if (refine_steps) *refine_steps = ctx->h_info[IN_STEPS];
+    if (pivot_index) *pivot_index = piv;
     return rc;
 }
 

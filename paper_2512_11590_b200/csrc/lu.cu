@@ -13,6 +13,7 @@
 #include "panel.cuh"
 
 #include <algorithm>
+#include <mutex>
 
 namespace hp {
 
@@ -51,8 +52,7 @@ template <class V> size_t LuWork<V>::carve(void *base, int n_) {
         binvU = alloc_view<V>(p, sbld, (long)ceil_div(n, SB) * sbld);
         tmp = alloc_view<V>(p, sbld, std::max<long>(n, 256));
     }
-    backup = alloc_view<V>(p, round_up(std::max(n, 1), 32), IB);
-    spec_flags = (int *)take(sizeof(int) * 2 * (size_t)std::max(nblk, 1));  // [nblk] refuted, [nblk] interchanges published
+    refuted = (int *)take(256);
     perm = (int *)take(sizeof(int) * (size_t)nblk * PERM_STRIDE);
     cand_val = (T *)take(sizeof(T) * 2 * MAXG);
     cand_row = (int *)take(sizeof(int) * 2 * MAXG);
@@ -250,11 +250,8 @@ template <class V> static int inv_double(cudaStream_t st, V A, int c0, int h, in
     V Ua = dinv_of(wk.dinvU, c0, h), Ub = dinv_of(wk.dinvU, c0 + h, w - h), Uo = dinv_of(wk.dinvU, c0, w);
     constexpr int HL = LEAF / 2;  // p, q <= LEAF/2
     const size_t smem = (2 * (size_t)HL * INV_RS + 2 * (size_t)HL * HL) * sizeof(E);
-    static bool configured = false;
-    if (!configured) {
-        HP_CUDA(cudaFuncSetAttribute(inv_double_kernel<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = true;
-    }
+    static SmemCfg cfg;
+    HP_TRY(configure_smem(cfg, inv_double_kernel<V>, smem));
     ProfCat pc(PROF_OTHER);
     const bool prof = prof_enabled();
     if (prof) prof_begin(st, 0.0);
@@ -279,7 +276,6 @@ template <class V> static int panel(cudaStream_t st, int n, V A, int c0, int w, 
     }
     HP_LAUNCHED();
     // this batch's interchanges on every other column of the matrix
-    if (panel_applies_swaps<V>(wk, m)) return 0;
     return laswp(st, A, 0, c0, c0 + w, n, wk.perm, blk, blk + 1);
 }
 
@@ -408,28 +404,54 @@ template <class V> static int trsm_upper(cudaStream_t st, V A, int d0, int s, V 
 // the LEAF-level recursion (the block's own big leaf does not exist yet).
 // What the factorisation itself does not need (for complex128 both inverses: its U12 solves keep the LEAF-level recursion,
 // whose GEMMs run at full FP64 rate; for complex64 the upper one) is built on a side stream, under the rest of the LU.
-static cudaStream_t side_stream() {
-    static cudaStream_t s = nullptr;
-    if (!s && cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking) != cudaSuccess) s = nullptr;
-    return s;
+// Raw entries (no context): one side stream + event pair per device, created on first use under a lock.  Host threads that
+// share a device share it; every use is bracketed by its own fork/join events, so sharing only serialises side work.
+struct SideRes {
+    cudaStream_t s = nullptr;
+    cudaEvent_t fork = nullptr, join = nullptr;
+};
+static SideRes *pooled_side() {
+    static std::mutex mu;
+    static SideRes pool[32];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 32) return nullptr;
+    std::lock_guard<std::mutex> lk(mu);
+    SideRes &r = pool[dev];
+    if (!r.s) {
+        if (cudaStreamCreateWithFlags(&r.s, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&r.fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&r.join, cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
+            r = SideRes();
+            return nullptr;
+        }
+    }
+    return &r;
+}
+template <class V> static SideRes side_of(const LuWork<V> &wk) {
+    SideRes r;
+    if (wk.side) {
+        r.s = wk.side;
+        r.fork = wk.ev_fork;
+        r.join = wk.ev_join;
+    } else if (SideRes *p = pooled_side()) {
+        r = *p;
+    }
+    return r;
 }
 // `to` waits for everything enqueued on `from` so far
-static int stream_follow(cudaStream_t from, cudaStream_t to) {
-    cudaEvent_t e;
-    HP_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-    cudaError_t r1 = cudaEventRecord(e, from), r2 = cudaStreamWaitEvent(to, e, 0);
-    cudaEventDestroy(e);
-    HP_CUDA(r1);
-    HP_CUDA(r2);
+static int stream_follow(cudaStream_t from, cudaStream_t to, cudaEvent_t e) {
+    HP_CUDA(cudaEventRecord(e, from));
+    HP_CUDA(cudaStreamWaitEvent(to, e, 0));
     return 0;
 }
 
 template <class V> static int build_binv(cudaStream_t st, V A, int c0, int s, LuWork<V> &wk) {
     ProfCat pc(PROF_OTHER);
     V XL = binv_of(wk.binvL, wk.sbld, c0), XU = binv_of(wk.binvU, wk.sbld, c0);
-    cudaStream_t sd = side_stream();
-    if (!sd) sd = st;
-    if (sd != st) HP_TRY(stream_follow(st, sd));
+    const SideRes sr = side_of(wk);
+    cudaStream_t sd = sr.s ? sr.s : st;
+    if (sd != st) HP_TRY(stream_follow(st, sd, sr.fork));
     cudaStream_t stl = IsPlanar<V>::value ? st : sd;  // the complex64 LU uses the lower inverse right away
     set_identity_kernel<V><<<ceil_div((long)s * s, 256), 256, 0, stl>>>(XL, s);
     HP_LAUNCHED();
@@ -440,12 +462,16 @@ template <class V> static int build_binv(cudaStream_t st, V A, int c0, int s, Lu
     int rc = trsm_lower(stl, A, c0, s, XL, s, wk, false);
     if (rc == 0) rc = trsm_upper(sd, A, c0, s, XU, s, wk, false);
     wk.use_big = was;
-    wk.side_used = (sd != st);
+    if (sd != st) wk.side_used = true;
     return rc;
 }
 
 template <class V> static int getrf_rec(cudaStream_t st, int n, V A, int c0, int c1, int *ipiv, int *info_dev, LuWork<V> &wk) {
     const int w = c1 - c0;
+    if (wk.speculate && w <= TW) {
+        ProfCat pc(PROF_PANEL);
+        return block_panel<V>(st, n, A, c0, w, ipiv, info_dev, wk, dinv_of(wk.dinvL, c0, w), dinv_of(wk.dinvU, c0, w));
+    }
     if (w <= IB) return panel(st, n, A, c0, w, ipiv, info_dev, wk);
     const int h = split(w), mid = c0 + h;
     HP_TRY(getrf_rec(st, n, A, c0, mid, ipiv, info_dev, wk));
@@ -468,13 +494,16 @@ template <class V> int getrf(cudaStream_t st, int n, V A, int *ipiv, int *info_d
     if (n <= 0) return 0;
     HP_CUDA(cudaMemsetAsync(wk.counter, 0, sizeof(unsigned), st));
     HP_CUDA(cudaMemsetAsync(wk.slots, 0, sizeof(unsigned long long) * LL_WORDS, st));
-    HP_CUDA(cudaMemsetAsync(wk.spec_flags, 0, sizeof(int) * 2 * (size_t)std::max(wk.nblk, 1), st));
+    HP_CUDA(cudaMemsetAsync(wk.refuted, 0, sizeof(int), st));
     wk.bar_base = 0;
     wk.ep_base = 0;
     wk.use_big = true;
     wk.side_used = false;
     HP_TRY(getrf_rec(st, n, A, 0, n, ipiv, info_dev, wk));
-    if (wk.side_used) HP_TRY(stream_follow(side_stream(), st));  // join: the kept inverses are complete
+    if (wk.side_used) {  // join: the kept inverses are complete
+        const SideRes sr = side_of(wk);
+        HP_TRY(stream_follow(sr.s, st, sr.join));
+    }
     if (IsPlanar<V>::value && n > LEAF) {
         // the solves apply the LEAF-diagonal blocks of the kept inverses separately, with FP32-class products
         ProfCat pc(PROF_OTHER);

@@ -11,6 +11,8 @@ constexpr int NLEV = 3;       // inverted diagonal blocks are kept at sizes IB <
 constexpr int SB = 1024;      // "solve block": the full inverses of the SB x SB diagonal blocks of L and U are kept as well, so
                               // that a triangular solve is N/SB dependent steps of large dense GEMMs instead of N/LEAF
 constexpr int MAXG = kNumSMs; // CTAs of the cooperative panel kernel (one per SM)
+constexpr int TW = 64;        // width of the block panel of a factorisation with verified diagonal pivots (toplu.cu): its top
+                              // block is factored and inverted by one CTA out of registers and shared memory
 
 // GEMM back-ends (zgemm.cu / cgemm.cu): C <- beta*C + alpha*A*B.  nbatch > 1: operand b lives at view + b*stride
 // elements.  C may alias B when m <= 128 (a single M tile of the kernel that is chosen then) and beta == 0: the in-place
@@ -36,10 +38,14 @@ template <class V> struct LuWork {
                          // (the solves apply those from dinvL/dinvU[NLEV-1] with the 3xTF32 kernel)
     V tmp;               // sbld x max(n, 256) scratch: out-of-place leaf product
     long sbld = 0;
-    V backup;            // n x IB: the panel as it was before a speculative (diagonal-pivot) factorisation (panel.cu)
-    int *spec_flags = nullptr; // nblk: 1 = the speculation of that panel was refuted
-    bool speculate = false;    // host-side: try diagonal pivots first (set by the structured mixed path)
+    int *refuted = nullptr;    // device counter: multipliers that refuted the diagonal-pivot speculation (toplu.cu); zeroed by getrf
+    bool speculate = false;    // host-side: the matrix is expected to pivot on its diagonal (S = K_d^-1 (C - E I)): factor
+                               // without interchanges and VERIFY (toplu.cu); the caller checks *refuted afterwards
     bool side_used = false; // host-side: something of this factorisation was enqueued on the side stream
+    // host-side resources for the side stream (kept block inverses are built under the factorisation).  A context sets its
+    // own (hprmat_setup); when null, a per-device pool serves the raw entries (lu.cu)
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     bool use_big = true; // host-side switch: off while an SB inverse is being built from the LEAF-level recursion
     int *perm = nullptr; // nblk x (1 + 4*IB): count, dst rows[2*IB], src rows[2*IB]  (net permutation of each swap batch)
     T *cand_val = nullptr;

@@ -1,7 +1,7 @@
 // panel.cu -- panel factorisation of the blocked LU with partial pivoting (PAPER.md:125-131, Eq. 5; :127 "partial
 // pivoting"): the register-resident cooperative kernel (fence-free epoch-tagged exchange between the CTAs), its
-// shared-memory predecessor (kept for panels taller than the register file allows) and the probe entry behind
-// hprmat_probe_panel.  See DESIGN.md section 6 and profiles/r01_panel_probe.md.
+// shared-memory predecessor (kept for panels taller than the register file allows).  The factorisations whose pivots
+// are verified to be the diagonal ones do not come here (toplu.cu).  See DESIGN.md section 6.
 #include "panel.cuh"
 
 #include <algorithm>
@@ -299,20 +299,6 @@ __device__ __forceinline__ void lds_e(unsigned addr, double2 &v) {
     asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];\n" : "=d"(v.x), "=d"(v.y) : "r"(addr));
 }
 
-// 1/a by Smith's formula on the reciprocal intrinsics (two dependent reciprocals, no IEEE-division slow paths)
-__device__ __forceinline__ float rcp_rn(float x) { return __frcp_rn(x); }
-__device__ __forceinline__ double rcp_rn(double x) { return __drcp_rn(x); }
-template <class E> __device__ __forceinline__ E crecip_fast(E a) {
-    typedef typename real_of<E>::type T;
-    if (fabs(a.x) >= fabs(a.y)) {
-        const T r = a.y * rcp_rn(a.x), id = rcp_rn(a.x + a.y * r);
-        return mk(id, -r * id);
-    } else {
-        const T r = a.x * rcp_rn(a.y), id = rcp_rn(a.x * r + a.y);
-        return mk(r * id, -id);
-    }
-}
-
 // Warp-wide arg-max of (v, li): v >= 0 a modulus (or li < 0: no candidate); the largest v wins, ties go to the smallest
 // li.  Integer redux.sync on the (order-preserving) bit patterns.  Result valid in every lane; li = -1 if none.
 __device__ __forceinline__ void warp_argmax(float &v, int &li) {
@@ -364,24 +350,10 @@ __device__ __forceinline__ void top_block_inverses(const typename V::elem_t *top
     }
 }
 
-// compile-time loop: f(integral_constant<int, I>) for I = B .. E-1 (keeps the register-resident panel statically indexed)
-template <int I> struct IntC { static constexpr int value = I; };
-template <int B, int E_, class F> __device__ __forceinline__ void static_for(F &&f) {
-    if constexpr (B < E_) {
-        f(IntC<B>{});
-        static_for<B + 1, E_>(f);
-    }
-}
-
-template <class V, int RPT, bool TIMING = false>
+template <class V, int RPT>
 __global__ void __launch_bounds__(PANEL_NT, 1)
     panel_reg_kernel(V A, int m, int jb, int j0, int rpc, int *ipiv, int *info, unsigned long long *ll, unsigned ep_base,
-                     V dinvL, V dinvU, int *perm, long long *dbg, const int *spec_flag, V backup, int *swap_ready,
-                     int ncols_total) {
-    // After a speculative (diagonal-pivot) factorisation of this panel: nothing to do if it was verified, else redo it with
-    // pivoting from the saved copy of the panel.  The flag is final (stream order) and read identically by all CTAs.
-    if (spec_flag != nullptr && *spec_flag == 0) return;
-    const V Src = spec_flag != nullptr ? backup : A;
+                     V dinvL, V dinvU, int *perm) {
     typedef typename V::elem_t E;
     typedef typename V::real_t T;
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -404,23 +376,13 @@ __global__ void __launch_bounds__(PANEL_NT, 1)
     const int row0 = cta * rpc;
     const int nloc = max(0, min(rpc, m - row0));
 
-    long long tph[6] = {0, 0, 0, 0, 0, 0}, tlast = 0;  // TIMING: cycles of thread 0 per phase
-    auto tick = [&](int ph) {
-        if constexpr (TIMING) {
-            const long long now = clock64();
-            tph[ph] += now - tlast;
-            tlast = now;
-        }
-    };
-    if constexpr (TIMING) tlast = clock64();
     E a[RPT][IB];
 #pragma unroll
     for (int r = 0; r < RPT; ++r) {
         const int li = tid + r * PANEL_NT;
 #pragma unroll
-        for (int c = 0; c < IB; ++c) a[r][c] = (li < nloc && c < jb) ? Src.get(row0 + li, c) : mk((T)0, (T)0);
+        for (int c = 0; c < IB; ++c) a[r][c] = (li < nloc && c < jb) ? A.get(row0 + li, c) : mk((T)0, (T)0);
     }
-    tick(0);
 
     T myval = (T)-1;
     int myli = -1;
@@ -449,7 +411,6 @@ __global__ void __launch_bounds__(PANEL_NT, 1)
             T bval = lane < PANEL_NT / 32 ? red_val[lane] : (T)0;
             int bli = lane < PANEL_NT / 32 ? red_idx[lane] : -1;
             warp_argmax(bval, bli);
-            tick(1);
             // ---- publish: the candidate's value and row (thread 0), the candidate row and row j (their owners)
             if (warp == POLLW) {
                 // push this CTA's candidate into every CTA's mailbox (each CTA then polls only its own lines)
@@ -477,7 +438,6 @@ __global__ void __launch_bounds__(PANEL_NT, 1)
                     }
                 }
             }
-            tick(2);
             // ---- all CTAs' candidates: poll until every slot carries this column's epoch, pick the same winner
             if (warp == POLLW) {
                 constexpr int NS = (MAXG + 31) / 32;
@@ -497,7 +457,6 @@ __global__ void __launch_bounds__(PANEL_NT, 1)
                     for (int q = 0; q < NS; ++q)
                         if (!(have >> q & 1u) && (w0[q] >> 48) == ep && (w1[q] >> 48) == ep) have |= 1u << q;
                 } while (!__all_sync(0xffffffffu, have == (1u << NS) - 1u));
-                tick(3);
                 double bv = -1.0;
                 int br = -1;
 #pragma unroll
@@ -542,7 +501,6 @@ __global__ void __launch_bounds__(PANEL_NT, 1)
                 }
             }
             __syncthreads();
-            tick(4);
             const int p = s_p;
             const E ip = s_ip;
             const bool sing = (ip.x == (T)0 && ip.y == (T)0);
@@ -588,7 +546,6 @@ __global__ void __launch_bounds__(PANEL_NT, 1)
                     }
                 }
             }
-            tick(5);
         }
         // ---- rotate the window: the finished column goes to the back
 #pragma unroll
@@ -598,10 +555,6 @@ __global__ void __launch_bounds__(PANEL_NT, 1)
             for (int c = 0; c + 1 < IB; ++c) a[r][c] = a[r][c + 1];
             a[r][IB - 1] = first;
         }
-    }
-    if constexpr (TIMING) {
-        if (tid == POLLW * 32 && dbg)
-            for (int k = 0; k < 6; ++k) dbg[cta * 8 + k] = tph[k];
     }
 
     // ---- write back (multipliers are already scaled)
@@ -625,147 +578,6 @@ __global__ void __launch_bounds__(PANEL_NT, 1)
         top_block_inverses<V>(topb, invp, inv_s, jb, dinvL, dinvU, tid);
         if (warp == 2) net_permutation(piv, jb, j0, perm, lane);
     }
-    if (spec_flag == nullptr) return;
-    // ---- Re-done speculative panel: the host did not enqueue the row-interchange kernel behind this panel (a verified
-    //      speculation has none), so the batch's net permutation is applied to all other columns here, by all CTAs, once
-    //      CTA 0 has published it.  A is the panel's view: full-matrix column C is column C - j0, row r is row r - j0.
-    if (cta == 0) {
-        __syncthreads();
-        if (tid == 0) {
-            __threadfence();
-            atomicExch(swap_ready, 1);
-        }
-    } else if (tid == 0) {
-        while (atomicAdd(swap_ready, 0) == 0) {
-        }
-        __threadfence();
-    }
-    __syncthreads();
-    const int cnt = perm[0];
-    if (cnt == 0) return;
-    const int nother = ncols_total - jb;             // all columns but the panel's own
-    const int q = tid & (2 * IB - 1), cl = tid >> 6;  // pair slot, column inside a group of four
-    int dst = 0, src = 0;
-    if (q < cnt) {
-        dst = perm[1 + q] - j0;
-        src = perm[1 + 2 * IB + q] - j0;
-    }
-    for (int g0 = cta * 4; g0 < nother; g0 += G * 4) {  // uniform trip count: four columns per pass, 64 pair slots each
-        const int g = g0 + cl;
-        const bool ok = g < nother && q < cnt;
-        const long col = (g < j0 ? g : g + jb) - (long)j0;
-        E val = mk((T)0, (T)0);
-        if (ok) val = A.get(src, col);  // a net permutation: gather all sources of the column, then scatter
-        __syncthreads();
-        if (ok) A.set(dst, col, val);
-    }
-}
-
-// ------------------------------------------------------------------------------------------------- speculative panel
-// Partial pivoting picks, in column j, the first row of maximal |re| + |im| among rows >= j.  When that is row j itself in
-// every column of the panel (always the case for the block-preconditioned matrix S = I + K_d^-1 V of the mixed path,
-// whose off-diagonal entries are coupling-sized), the panel factorisation needs no exchange between CTAs at all:
-// every CTA factors the jb x jb top block (no interchanges) and each thread forward-substitutes its own row,
-//     a_ij^(j) = a_ij - sum_{k<j} l_ik u_kj,     l_ij = a_ij^(j) / u_jj,
-// in the same operation order as the rank-1 updates.  The a_ij^(j) are exactly the candidates partial pivoting would
-// compare, so the speculation is VERIFIED on the fly: |a_ij^(j)| <= |u_jj| for all i > j (ties go to the smaller row, i.e.
-// to the diagonal); any violation (or a zero pivot) raises the panel's flag, and the pivoting kernel that is always
-// enqueued right behind redoes the panel from the saved copy.  The result is partial pivoting's in both cases.
-template <class V>
-__global__ void __launch_bounds__(PANEL_NT) panel_spec_kernel(V A, int m, int jb, int j0, int *ipiv, int *flag, V backup,
-                                                             V dinvL, V dinvU, int *perm) {
-    typedef typename V::elem_t E;
-    typedef typename V::real_t T;
-    extern __shared__ __align__(16) unsigned char smraw[];
-    E *topb = reinterpret_cast<E *>(smraw);  // [IB][IB] column-major, ld = IB: the top block, factored in place
-    E *inv_s = topb + IB * IB;               // [2][IB][IB] scratch for the triangular inverses (last CTA)
-    E *rows = inv_s + 2 * IB * IB;           // [IB][PANEL_NT]: element c of this thread's row at rows[c*PANEL_NT + tid]
-    __shared__ E invp[IB];
-    __shared__ int s_bad;
-    const int tid = threadIdx.x;
-    const bool top_cta = blockIdx.x == gridDim.x - 1;  // the extra CTA that owns the top block's outputs
-    const int row = blockIdx.x * PANEL_NT + tid;        // panel row of this thread (row CTAs)
-    const bool has_row = !top_cta && row < m;
-
-    // every row thread saves its row and parks it in shared memory; the top block goes to shared memory in every CTA
-    if (has_row) {
-        for (int c0 = 0; c0 < jb; c0 += 8) {  // eight independent loads in flight, then their stores
-            E v[8];
-#pragma unroll
-            for (int q = 0; q < 8; ++q) v[q] = (c0 + q < jb) ? A.get(row, c0 + q) : mk((T)0, (T)0);
-#pragma unroll
-            for (int q = 0; q < 8; ++q)
-                if (c0 + q < jb) {
-                    backup.set(row, c0 + q, v[q]);
-                    rows[(c0 + q) * PANEL_NT + tid] = v[q];
-                }
-        }
-    }
-    for (int idx = tid; idx < IB * IB; idx += PANEL_NT) {
-        const int i = idx % IB, c = idx / IB;
-        topb[idx] = (i < jb && c < jb && i < m) ? A.get(i, c) : mk((T)(i == c ? 1 : 0), (T)0);
-    }
-    if (tid == 0) s_bad = 0;
-    __syncthreads();
-    // ---- top block, no interchanges: lane = row, warp = column residue (conflict-free column-major accesses);
-    //      step j: scale column j, rank-1 update of the rest
-    {
-        const int i = tid & 31, c8 = tid >> 5;
-        for (int j = 0; j < jb; ++j) {
-            const E pv = topb[j * IB + j];
-            const bool sing = (pv.x == (T)0 && pv.y == (T)0);
-            const E ip = sing ? mk((T)0, (T)0) : crecip_fast(pv);
-            E l = mk((T)0, (T)0);
-            if (i > j && i < jb) {
-                const E v = topb[j * IB + i];
-                if (sing || cabs1(v) > cabs1(pv)) s_bad = 1;
-                l = cmul(v, ip);
-            }
-            __syncthreads();  // everybody has read column j and the pivot
-            if (i > j && i < jb) {
-                if (c8 == 0) topb[j * IB + i] = l;
-                for (int c = j + 1 + c8; c < jb; c += 8) topb[c * IB + i] = cfnma(topb[c * IB + i], l, topb[c * IB + j]);
-            }
-            if (tid == 0) invp[j] = ip;
-            __syncthreads();
-        }
-    }
-    if (top_cta) {
-        // ---- the factored top block, the (identity) interchanges, the IB-level inverses, an empty swap batch
-        for (int idx = tid; idx < IB * IB; idx += PANEL_NT) {
-            const int i = idx % IB, c = idx / IB;
-            if (i < jb && c < jb && i < m) A.set(i, c, topb[idx]);
-        }
-        if (tid < jb) ipiv[j0 + tid] = j0 + tid + 1;
-        if (tid == 0) {
-            perm[0] = 0;
-            if (s_bad) atomicExch(flag, 1);
-        }
-        top_block_inverses<V>(topb, invp, inv_s, jb, dinvL, dinvU, tid);
-        return;
-    }
-    // ---- rows below the top block: forward substitution against U11 (rolled loops, the row lives in shared memory),
-    //      verified column by column
-    if (has_row && row >= jb) {
-        E *my = rows + tid;
-        bool bad = false;
-        for (int j = 0; j < jb; ++j) {
-            const E *u = topb + j * IB;  // column j of U11: u[k] = u_kj
-            E v = my[j * PANEL_NT], v1 = mk((T)0, (T)0);  // two accumulation chains
-            int k = 0;
-            for (; k + 1 < j; k += 2) {
-                v = cfnma(v, my[k * PANEL_NT], u[k]);
-                v1 = cfnma(v1, my[(k + 1) * PANEL_NT], u[k + 1]);
-            }
-            if (k < j) v = cfnma(v, my[k * PANEL_NT], u[k]);
-            v = cadd(v, v1);
-            if (cabs1(v) > cabs1(u[j])) bad = true;
-            my[j * PANEL_NT] = cmul(v, invp[j]);
-        }
-        if (bad) atomicExch(flag, 1);
-#pragma unroll 8
-        for (int c = 0; c < jb; ++c) A.set(row, c, my[c * PANEL_NT]);
-    }
 }
 
 template <class V, int RPT>
@@ -774,33 +586,10 @@ static int launch_panel_reg(cudaStream_t st, V Asub, int m, int w, int c0, int r
     typedef typename V::elem_t E;
     const size_t smem = 3 * (size_t)IB * IB * sizeof(E);
     auto kern = panel_reg_kernel<V, RPT>;
-    static bool configured = false;
-    if (!configured) {
-        HP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = true;
-    }
+    static SmemCfg cfg;
+    HP_TRY(configure_smem(cfg, kern, smem));
     unsigned ep = wk.ep_base;
-    long long *dbg = nullptr;
-    const int *spec_flag = nullptr;
-    if (wk.speculate) {
-        // diagonal-pivot attempt first; the pivoting kernel behind it returns at once if the attempt was verified
-        auto spec = panel_spec_kernel<V>;
-        const size_t spec_smem = smem + (size_t)IB * PANEL_NT * sizeof(E);
-        static bool spec_configured = false;
-        if (!spec_configured) {
-            HP_CUDA(cudaFuncSetAttribute(spec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)spec_smem));
-            spec_configured = true;
-        }
-        int *flag = wk.spec_flags + c0 / IB;
-        // one CTA per PANEL_NT rows plus one that owns the top block's outputs
-        spec<<<ceil_div(m, PANEL_NT) + 1, PANEL_NT, spec_smem, st>>>(Asub, m, w, c0, ipiv, flag, wk.backup, dl, du, perm);
-        HP_LAUNCHED();
-        spec_flag = flag;
-    }
-    int *swap_ready = wk.spec_flags + wk.nblk + c0 / IB;
-    int ncols_total = wk.n;
-    void *args[] = {&Asub, &m, &w, &c0, &rpc, &ipiv, &info_dev, &wk.slots, &ep, &dl, &du, &perm, &dbg, &spec_flag, &wk.backup,
-                    &swap_ready, &ncols_total};
+    void *args[] = {&Asub, &m, &w, &c0, &rpc, &ipiv, &info_dev, &wk.slots, &ep, &dl, &du, &perm};
     HP_CUDA(cudaLaunchCooperativeKernel((void *)kern, dim3(G), dim3(PANEL_NT), args, smem, st));
     wk.ep_base += (unsigned)w;
     return 0;
@@ -809,12 +598,6 @@ static int launch_panel_reg(cudaStream_t st, V Asub, int m, int w, int c0, int r
 template <class V> struct PanelRows;  // rows one CTA of the register-resident kernel can hold
 template <> struct PanelRows<ZView> { static constexpr int max_rpt = 1; };
 template <> struct PanelRows<CView> { static constexpr int max_rpt = 2; };
-
-template <class V> bool panel_applies_swaps(const LuWork<V> &wk, int m) {
-    int rpc = std::max(ceil_div(m, MAXG), PANEL_MINROWS);
-    rpc = (int)round_up(rpc, 2);
-    return wk.speculate && rpc <= PanelRows<V>::max_rpt * PANEL_NT;
-}
 
 template <class V>
 int panel_launch(cudaStream_t st, V Asub, int m, int w, int c0, int *ipiv, int *info_dev, LuWork<V> &wk, V dl, V du, int *perm) {
@@ -828,11 +611,8 @@ int panel_launch(cudaStream_t st, V Asub, int m, int w, int c0, int *ipiv, int *
     // taller than the register file allows: the shared-memory kernel with a counter barrier
     const size_t smem = ((size_t)IB * rpc + 2 * IB * IB) * sizeof(E);
     auto kern = panel_lu_kernel<V>;
-    static size_t configured = 0;
-    if (smem > configured) {
-        HP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    static SmemCfg cfg;
+    HP_TRY(configure_smem(cfg, kern, smem));
     unsigned base = wk.bar_base;
     void *args[] = {&Asub, &m, &w, &c0, &rpc, &ipiv, &info_dev, &wk.cand_val, &wk.cand_row, &wk.cand_data,
                     &wk.jrow, &wk.counter, &base, &dl, &du, &perm};
@@ -841,59 +621,6 @@ int panel_launch(cudaStream_t st, V Asub, int m, int w, int c0, int *ipiv, int *
     return 0;
 }
 
-// Measurement aid (hprmat_probe_panel): `reps` back-to-back factorisations of the same m x IB panel (the data are garbage
-// after the first one; only time is of interest) with the phase-timing variant of the register-resident kernel.
-int probe_panel(cudaStream_t st, int m, int reps, float *A_re, float *A_im, long lda, void *work, double *us_per_panel,
-                long long *phase_cycles_host) {
-    LuWork<CView> wk;
-    wk.carve(work, m);
-    CView A(A_re, A_im, lda);
-    int rpc = std::max(ceil_div(m, MAXG), PANEL_MINROWS);
-    rpc = (int)round_up(rpc, 2);
-    if (rpc > PANEL_NT) return -2;
-    const int G = ceil_div(m, rpc);
-    int *ipiv = nullptr, *info = nullptr;
-    long long *dbg = nullptr;
-    HP_CUDA(cudaMalloc((void **)&ipiv, sizeof(int) * (IB + 8)));
-    info = ipiv + IB;
-    HP_CUDA(cudaMalloc((void **)&dbg, sizeof(long long) * 8 * MAXG));
-    HP_CUDA(cudaMemsetAsync(ipiv, 0, sizeof(int) * (IB + 8), st));
-    HP_CUDA(cudaMemsetAsync(wk.slots, 0, sizeof(unsigned long long) * LL_WORDS, st));
-    auto kern = panel_reg_kernel<CView, 1, true>;
-    const size_t smem = 3 * (size_t)IB * IB * sizeof(float2);
-    HP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    cudaEvent_t e0, e1;
-    HP_CUDA(cudaEventCreate(&e0));
-    HP_CUDA(cudaEventCreate(&e1));
-    CView dl = wk.dinvL[0], du = wk.dinvU[0];
-    int w = IB, c0 = 0;
-    for (int it = 0; it <= reps; ++it) {
-        if (it == 1) HP_CUDA(cudaEventRecord(e0, st));
-        unsigned ep = wk.ep_base;
-        const int *spec_flag = nullptr;
-        int *swap_ready = nullptr;
-        int ncols_total = 0;
-        void *args[] = {&A, &m, &w, &c0, &rpc, &ipiv, &info, &wk.slots, &ep, &dl, &du, &wk.perm, &dbg, &spec_flag, &wk.backup,
-                        &swap_ready, &ncols_total};
-        HP_CUDA(cudaLaunchCooperativeKernel((void *)kern, dim3(G), dim3(PANEL_NT), args, smem, st));
-        HP_LAUNCHED();
-        wk.ep_base += IB;
-    }
-    HP_CUDA(cudaEventRecord(e1, st));
-    HP_CUDA(cudaEventSynchronize(e1));
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, e0, e1);
-    *us_per_panel = ms * 1e3 / reps;
-    if (phase_cycles_host) HP_CUDA(cudaMemcpy(phase_cycles_host, dbg, sizeof(long long) * 8 * MAXG, cudaMemcpyDeviceToHost));
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(ipiv);
-    cudaFree(dbg);
-    return 0;
-}
-
-template bool panel_applies_swaps<CView>(const LuWork<CView> &, int);
-template bool panel_applies_swaps<ZView>(const LuWork<ZView> &, int);
 template int panel_launch<CView>(cudaStream_t, CView, int, int, int, int *, int *, LuWork<CView> &, CView, CView, int *);
 template int panel_launch<ZView>(cudaStream_t, ZView, int, int, int, int *, int *, LuWork<ZView> &, ZView, ZView, int *);
 

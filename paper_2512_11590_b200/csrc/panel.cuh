@@ -19,8 +19,9 @@ constexpr size_t LL_WORDS = LL_SLOTS + LL_ROWS;
 template <class V>
 int panel_launch(cudaStream_t st, V Asub, int m, int w, int c0, int *ipiv, int *info_dev, LuWork<V> &wk, V dl, V du, int *perm);
 
-// true when the kernels enqueued by panel_launch apply the batch's row interchanges to the other columns themselves
-// (speculative mode: a verified panel has none, a re-done one applies them in its pivoting kernel)
-template <class V> bool panel_applies_swaps(const LuWork<V> &wk, int m);
+// Block panel of a factorisation with verified diagonal pivots (toplu.cu): factors the TW-wide (w <= TW) column block at
+// (c0,c0) of the n x n matrix A without interchanges -- top block in one CTA, L21 = A21 U11^-1 by one GEMM -- and counts
+// refuted multipliers (|l|_1 > 1/2, zero pivots) in *wk.refuted.  dl / du receive the inverses of the top block's triangles.
+template <class V> int block_panel(cudaStream_t st, int n, V A, int c0, int w, int *ipiv, int *info_dev, LuWork<V> &wk, V dl, V du);
 
 }  // namespace hp

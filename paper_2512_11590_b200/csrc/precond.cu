@@ -125,11 +125,8 @@ int precond_invert(cudaStream_t st, const StructTables &t, double energy, const 
     const size_t full = small + sizeof(double2) * (size_t)n * n;
     const int use_smem = full <= 200 * 1024;
     const size_t smem = use_smem ? full : small;
-    static size_t configured = 48 * 1024;
-    if (smem > configured) {
-        HP_CUDA(cudaFuncSetAttribute(kinv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    static SmemCfg cfg;
+    if (smem > 48 * 1024) HP_TRY(configure_smem(cfg, kinv_kernel, smem));
     kinv_kernel<<<t.nch, KI_NT, smem, st>>>(t.nch, n, t.hT, t.dg0, t.ethr, energy, V, W, ldw, Kinv, use_smem, info_dev);
     HP_LAUNCHED();
     return 0;
@@ -335,8 +332,9 @@ int demote(cudaStream_t st, long rows, int cols, const double2 *Z, long ldz, CVi
 // norms[0] = max|D|, norms[1] = max|X_new| (moduli; pre-zeroed here)
 __global__ void __launch_bounds__(256) promote_add_kernel(long rows, int cols, double2 *__restrict__ X, long ldx,
                                                           const float *__restrict__ re, const float *__restrict__ im, long ld,
-                                                          int accumulate, double *norms) {
+                                                          int accumulate, double *norms, const int *gate) {
     __shared__ double shred[32];
+    if (gate != nullptr && *gate != 0) return;  // the refinement has already stopped: this step must not touch X
     double md = 0.0, mx = 0.0;
     const long tot = rows * cols;
     for (long idx = (long)blockIdx.x * blockDim.x + threadIdx.x; idx < tot; idx += (long)gridDim.x * blockDim.x) {
@@ -365,12 +363,13 @@ __global__ void __launch_bounds__(256) promote_add_kernel(long rows, int cols, d
     }
 }
 
-int promote_add(cudaStream_t st, long rows, int cols, double2 *X, long ldx, CView D, bool accumulate, double *norms_dev) {
+int promote_add(cudaStream_t st, long rows, int cols, double2 *X, long ldx, CView D, bool accumulate, double *norms_dev,
+                const int *gate_dev) {
     HP_CUDA(cudaMemsetAsync(norms_dev, 0, 2 * sizeof(double), st));
     const long tot = rows * cols;
     if (tot <= 0) return 0;
     const int grid = (int)std::min<long>(ceil_div(tot, 256), 148L * 8);
-    promote_add_kernel<<<grid, 256, 0, st>>>(rows, cols, X, ldx, D.re, D.im, D.ld, accumulate ? 1 : 0, norms_dev);
+    promote_add_kernel<<<grid, 256, 0, st>>>(rows, cols, X, ldx, D.re, D.im, D.ld, accumulate ? 1 : 0, norms_dev, gate_dev);
     HP_LAUNCHED();
     return 0;
 }

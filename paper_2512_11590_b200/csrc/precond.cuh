@@ -21,7 +21,10 @@ int precond_rhs_z(cudaStream_t st, const StructTables &t, const double2 *Kinv, Z
 int precond_rhs(cudaStream_t st, const StructTables &t, const double2 *Kinv, CView B);
 // D <- (complex64) Z
 int demote(cudaStream_t st, long rows, int cols, const double2 *Z, long ldz, CView D);
-// X <- (accumulate ? X : 0) + D;  norms_dev[0] = max|D|, norms_dev[1] = max|X|
-int promote_add(cudaStream_t st, long rows, int cols, double2 *X, long ldx, CView D, bool accumulate, double *norms_dev);
+// X <- (accumulate ? X : 0) + D;  norms_dev[0] = max|D|, norms_dev[1] = max|X|.  gate_dev (device int, may be nullptr):
+// when it reads non-zero the kernel does nothing (norms stay zero) -- a refinement step enqueued after the device-side
+// stopping rule has fired
+int promote_add(cudaStream_t st, long rows, int cols, double2 *X, long ldx, CView D, bool accumulate, double *norms_dev,
+                const int *gate_dev = nullptr);
 
 }  // namespace hp

@@ -255,10 +255,8 @@ int zsolve_mixed(cudaStream_t st, int n, int nrhs, const double2 *A, long lda, d
         ZM_TRY(zgemm(st, n, nrhs, n, -1.0, A, lda, B, ldb, 1.0, w.R, n));
         ZM_TRY(maxabs(st, n, nrhs, w.R, n, w.scal + 3));
         ZM_TRY(maxabs(st, n, nrhs, w.B0, n, w.scal + 6));
+        ZM_TRY(backward_error(st, n, nrhs, w.R, n, B, ldb, w.scal + 4, w.scal + 6, w.scal + 5));
         ZM_CUDA(cudaMemcpyAsync(h, w.scal, sizeof(double) * 8, cudaMemcpyDeviceToHost, st));
-        ZM_CUDA(cudaStreamSynchronize(st));
-        ZM_TRY(backward_error(st, n, nrhs, w.R, n, B, ldb, h[4], h[6], w.scal + 5));
-        ZM_CUDA(cudaMemcpyAsync(h + 5, w.scal + 5, sizeof(double), cudaMemcpyDeviceToHost, st));
         ZM_CUDA(cudaStreamSynchronize(st));
         float ms = 0.f;
         info->status = status;

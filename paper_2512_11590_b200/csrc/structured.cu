@@ -319,11 +319,8 @@ int structured_residual(cudaStream_t st, const StructTables &t, double energy, c
     {
         dim3 grid(t.nch, ceil_div(nrhs, RES_QT));
         const size_t smem = sizeof(double2) * RES_QT * t.nb;
-        static size_t cfg1 = 48 * 1024;
-        if (smem > cfg1) {
-            HP_CUDA(cudaFuncSetAttribute(resid_channel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            cfg1 = smem;
-        }
+        static SmemCfg cfg1;
+        if (smem > 48 * 1024) HP_TRY(configure_smem(cfg1, resid_channel_kernel, smem));
         resid_channel_kernel<<<grid, RES_NT, smem, st>>>(t.nch, t.nb, nrhs, t.hT, t.dg0, t.ethr, energy, t.fa, V, Bx, ldb,
                                                          X, ldx, R, Rlo, ldr);
         HP_LAUNCHED();
@@ -331,11 +328,8 @@ int structured_residual(cudaStream_t st, const StructTables &t, double energy, c
     {
         dim3 grid(t.nb, ceil_div(nrhs, RES_QT));
         const size_t smem = sizeof(double2) * RES_QT * t.nch;
-        static size_t cfg2 = 48 * 1024;
-        if (smem > cfg2) {
-            HP_CUDA(cudaFuncSetAttribute(resid_coupling_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            cfg2 = smem;
-        }
+        static SmemCfg cfg2;
+        if (smem > 48 * 1024) HP_TRY(configure_smem(cfg2, resid_coupling_kernel, smem));
         resid_coupling_kernel<<<grid, RES_NT, smem, st>>>(t.nch, t.nb, nrhs, V, X, ldx, R, Rlo, ldr, rmax_dev);
         HP_LAUNCHED();
     }
@@ -345,8 +339,10 @@ int structured_residual(cudaStream_t st, const StructTables &t, double energy, c
 // ---------------------------------------------------------------------------------------------------- update + norms
 // X += D; norms[0] = max|D|, norms[1] = max|X_new|  (moduli; norms pre-zeroed by the caller)
 __global__ void __launch_bounds__(256) axpy_norm_kernel(long rows, int cols, double2 *__restrict__ X, long ldx,
-                                                        const double2 *__restrict__ D, long ldd, double *norms) {
+                                                        const double2 *__restrict__ D, long ldd, double *norms,
+                                                        const int *gate) {
     __shared__ double shred[32];
+    if (gate != nullptr && *gate != 0) return;  // the refinement has already stopped: this step must not touch X
     double md = 0.0, mx = 0.0;
     const long tot = rows * cols;
     for (long idx = (long)blockIdx.x * blockDim.x + threadIdx.x; idx < tot; idx += (long)gridDim.x * blockDim.x) {
@@ -367,12 +363,13 @@ __global__ void __launch_bounds__(256) axpy_norm_kernel(long rows, int cols, dou
     }
 }
 
-int axpy_norm(cudaStream_t st, long rows, int cols, double2 *X, long ldx, const double2 *D, long ldd, double *norms_dev) {
+int axpy_norm(cudaStream_t st, long rows, int cols, double2 *X, long ldx, const double2 *D, long ldd, double *norms_dev,
+              const int *gate_dev) {
     HP_CUDA(cudaMemsetAsync(norms_dev, 0, 2 * sizeof(double), st));
     const long tot = rows * cols;
     if (tot <= 0) return 0;
     const int grid = (int)std::min<long>(ceil_div(tot, 256), 148L * 8);
-    axpy_norm_kernel<<<grid, 256, 0, st>>>(rows, cols, X, ldx, D, ldd, norms_dev);
+    axpy_norm_kernel<<<grid, 256, 0, st>>>(rows, cols, X, ldx, D, ldd, norms_dev, gate_dev);
     HP_LAUNCHED();
     return 0;
 }
@@ -421,8 +418,9 @@ int maxabs_real(cudaStream_t st, long n, const double *x, double *out_dev) {
 // ---------------------------------------------------------------------------------------------------- backward error
 // out[0] = max_q  ||r_q||_inf / (anorm * ||x_q||_inf + ||b_q||_inf)   (one CTA per right-hand side; out pre-zeroed)
 __global__ void __launch_bounds__(256) backward_err_kernel(long rows, const double2 *__restrict__ R, long ldr,
-                                                           const double2 *__restrict__ X, long ldx, double anorm,
-                                                           double bnorm, double *out) {
+                                                           const double2 *__restrict__ X, long ldx,
+                                                           const double *__restrict__ anorm_p,
+                                                           const double *__restrict__ bnorm_p, double *out) {
     __shared__ double shred[32];
     const long q = blockIdx.x;
     double mr = 0.0, mx = 0.0;
@@ -434,16 +432,16 @@ __global__ void __launch_bounds__(256) backward_err_kernel(long rows, const doub
     mr = block_max(mr, shred);
     mx = block_max(mx, shred);
     if (threadIdx.x == 0) {
-        const double den = anorm * mx + bnorm;
+        const double den = *anorm_p * mx + *bnorm_p;
         atomic_max_nonneg(out, den > 0.0 ? mr / den : 0.0);
     }
 }
 
 int backward_error(cudaStream_t st, long rows, int nrhs, const double2 *R, long ldr, const double2 *X, long ldx,
-                   double anorm, double bnorm, double *out_dev) {
+                   const double *anorm_dev, const double *bnorm_dev, double *out_dev) {
     HP_CUDA(cudaMemsetAsync(out_dev, 0, sizeof(double), st));
     if (nrhs <= 0) return 0;
-    backward_err_kernel<<<nrhs, 256, 0, st>>>(rows, R, ldr, X, ldx, anorm, bnorm, out_dev);
+    backward_err_kernel<<<nrhs, 256, 0, st>>>(rows, R, ldr, X, ldx, anorm_dev, bnorm_dev, out_dev);
     HP_LAUNCHED();
     return 0;
 }

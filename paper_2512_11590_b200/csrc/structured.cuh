@@ -29,10 +29,14 @@ int build_rhs(cudaStream_t st, const StructTables &t, double2 *B, long ldb);
 int structured_residual(cudaStream_t st, const StructTables &t, double energy, const double2 *V, int nrhs,
                         const double2 *Bx, long ldb, const double2 *X, long ldx, double2 *R, double2 *Rlo, long ldr,
                         double *rmax_dev);
-int axpy_norm(cudaStream_t st, long rows, int cols, double2 *X, long ldx, const double2 *D, long ldd, double *norms_dev);
+// X += D; norms_dev[0] = max|D|, norms_dev[1] = max|X|.  gate_dev: as in promote_add (precond.cuh)
+int axpy_norm(cudaStream_t st, long rows, int cols, double2 *X, long ldx, const double2 *D, long ldd, double *norms_dev,
+              const int *gate_dev = nullptr);
 int maxabs(cudaStream_t st, long rows, int cols, const double2 *X, long ldx, double *out_dev);
+// out_dev <- max_q ||r_q||_inf / (anorm ||x_q||_inf + bnorm); anorm and bnorm are read from DEVICE memory, so that the whole
+// report can be enqueued without a host round trip
 int backward_error(cudaStream_t st, long rows, int nrhs, const double2 *R, long ldr, const double2 *X, long ldx,
-                   double anorm, double bnorm, double *out_dev);
+                   const double *anorm_dev, const double *bnorm_dev, double *out_dev);
 int structured_anorm(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double *out_dev);
 int contract(cudaStream_t st, const StructTables &t, const double2 *X, long ldx, double2 *R);
 

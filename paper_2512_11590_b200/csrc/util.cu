@@ -1,18 +1,20 @@
 // util.cu -- process-wide state behind the C ABI: error strings and the launch counter.
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
 #include <vector>
 
 #include "common.cuh"
 
 namespace hp {
 thread_local char g_cuda_err[256] = "";
-long long g_launches = 0;
+std::atomic<long long> g_launches{0};
 
 // ---- optional per-launch timing of the GEMM kernel (bench.py's roofline leg): one CUDA-event pair around every launch
 struct ProfRec { cudaEvent_t a, b; double flops; int cat; };
-static bool g_prof_on = false;
-int g_prof_cat = PROF_OTHER;
+static std::atomic<bool> g_prof_on{false};
+static std::mutex g_prof_mu;  // the record below is process-wide (a measurement aid)
+thread_local int g_prof_cat = PROF_OTHER;
 static double g_cat_ms[PROF_NCAT], g_cat_flops[PROF_NCAT];
 static long long g_cat_n[PROF_NCAT];
 static std::vector<ProfRec> g_prof;
@@ -25,11 +27,15 @@ static cudaEvent_t prof_event() {
 }
 bool prof_enabled() { return g_prof_on; }
 void prof_begin(cudaStream_t st, double flops) {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
     ProfRec r{prof_event(), prof_event(), flops, g_prof_cat};
     cudaEventRecord(r.a, st);
     g_prof.push_back(r);
 }
-void prof_end(cudaStream_t st) { cudaEventRecord(g_prof.back().b, st); }
+void prof_end(cudaStream_t st) {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    cudaEventRecord(g_prof.back().b, st);
+}
 }  // namespace hp
 
 extern "C" int hprmat_profile(int enable) {
@@ -39,21 +45,17 @@ extern "C" int hprmat_profile(int enable) {
 extern "C" int hprmat_profile_read(double *ms, double *flops, long long *launches) {
     double t = 0.0, f = 0.0;
     long long n = 0;
+    std::lock_guard<std::mutex> lk(hp::g_prof_mu);
     for (int c = 0; c < hp::PROF_NCAT; ++c) { hp::g_cat_ms[c] = hp::g_cat_flops[c] = 0.0; hp::g_cat_n[c] = 0; }
-    // HPRMAT_PROF_DUMP=<file>: append one "category flops milliseconds" line per recorded launch (measurement aid)
-    const char *dump = getenv("HPRMAT_PROF_DUMP");
-    FILE *df = dump && *dump ? fopen(dump, "a") : nullptr;
     for (auto &r : hp::g_prof) {
-        if (cudaEventSynchronize(r.b) != cudaSuccess) { if (df) fclose(df); return HPRMAT_ECUDA; }
+        if (cudaEventSynchronize(r.b) != cudaSuccess) return HPRMAT_ECUDA;
         float m = 0.f;
         cudaEventElapsedTime(&m, r.a, r.b);
-        if (df) fprintf(df, "%d %.6e %.6f\n", r.cat, r.flops, m);
         hp::g_cat_ms[r.cat] += m; hp::g_cat_flops[r.cat] += r.flops; ++hp::g_cat_n[r.cat];
         if (r.flops > 0.0) { t += m; f += r.flops; ++n; }
         hp::g_prof_pool.push_back(r.a);
         hp::g_prof_pool.push_back(r.b);
     }
-    if (df) fclose(df);
     hp::g_prof.clear();
     if (ms) *ms = t;
     if (flops) *flops = f;
@@ -76,8 +78,9 @@ extern "C" const char *hprmat_strerror(int code) {
         case HPRMAT_ENOTCONVERGED: return "iterative refinement did not converge";
         case HPRMAT_ENOMEM: return "out of device memory / workspace too small";
         case HPRMAT_ECUDA: return "CUDA error";
+        case HPRMAT_EUNVERIFIED: return "verified-diagonal factorisation refuted or unusable in an unsynchronised call";
         default: return code < 0 ? "invalid argument" : "unknown error";
     }
 }
 extern "C" const char *hprmat_last_cuda_error(void) { return hp::g_cuda_err; }
-extern "C" long long hprmat_launch_count(void) { return hp::g_launches; }
+extern "C" long long hprmat_launch_count(void) { return hp::g_launches.load(); }

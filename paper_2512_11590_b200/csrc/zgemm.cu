@@ -180,11 +180,8 @@ static int launch_zgemm(cudaStream_t st, int m, int n, int k, double alpha, cons
     constexpr int BM = WM * 32, BN = WN * 32;
     constexpr size_t smem = (size_t)STAGES * (KC * (BM + 2) + BN * (KC + 2)) * sizeof(double2);
     auto kern = zgemm_kernel<WM, WN, KC, STAGES, MINB>;
-    static bool configured = false;
-    if (!configured) {
-        HP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = true;
-    }
+    static SmemCfg cfg;
+    HP_TRY(configure_smem(cfg, kern, smem));
     dim3 grid(ceil_div(m, BM) * ceil_div(n, BN), 1, nbatch);
     kern<<<grid, WM * WN * 32, smem, st>>>(m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC);
     HP_LAUNCHED();
@@ -194,10 +191,16 @@ static int launch_zgemm(cudaStream_t st, int m, int n, int k, double alpha, cons
 // 3M variant (zgemm3m.cu) and the switch between the two decompositions (hprmat_zgemm_algo)
 int zgemm3m(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda, long strideA, const double2 *B,
             long ldb, long strideB, double beta, double2 *C, long ldc, long strideC, int nbatch);
-int g_zgemm_algo = 3;
+static std::atomic<int> g_zgemm_algo{3};       // process default (hprmat_zgemm_algo)
+static thread_local int tl_zgemm_algo = 0;     // a context's own setting while one of its calls runs on this thread
+int zgemm_algo_in_force() { return tl_zgemm_algo ? tl_zgemm_algo : g_zgemm_algo.load(std::memory_order_relaxed); }
+ScopedZgemmAlgo::ScopedZgemmAlgo(int algo) : prev(tl_zgemm_algo) {
+    if (algo == 3 || algo == 4) tl_zgemm_algo = algo;
+}
+ScopedZgemmAlgo::~ScopedZgemmAlgo() { tl_zgemm_algo = prev; }
 // the 3M kernel has several M tiles per column strip (C must not alias B) and 64-column tiles
 static inline bool use_3m(int n, int k, const double2 *B, const double2 *C) {
-    return g_zgemm_algo == 3 && n > 32 && k >= 16 && (const void *)B != (const void *)C;
+    return zgemm_algo_in_force() == 3 && n > 32 && k >= 16 && (const void *)B != (const void *)C;
 }
 
 // C <- beta*C + alpha*A*B  (device pointers, column-major)
@@ -230,8 +233,8 @@ int zgemm_batched(cudaStream_t st, int m, int n, int k, double alpha, const doub
 }  // namespace hp
 
 extern "C" int hprmat_zgemm_algo(int algo) {
-    if (algo == 3 || algo == 4) hp::g_zgemm_algo = algo;
-    return hp::g_zgemm_algo;
+    if (algo == 3 || algo == 4) hp::g_zgemm_algo.store(algo);
+    return hp::g_zgemm_algo.load();
 }
 
 extern "C" int hprmat_zgemm(void *cuda_stream, int m, int n, int k, double alpha, const void *A, int lda, const void *B,

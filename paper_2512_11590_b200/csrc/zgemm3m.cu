@@ -209,11 +209,8 @@ int zgemm3m(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A
     constexpr int LP = 6;
     static_assert(LP < KC / 4, "the issue point is a k-step of the slab");
     auto kern = zgemm3m_kernel<WM, WN, KC, STAGES, LP>;
-    static bool configured = false;
-    if (!configured) {
-        HP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = true;
-    }
+    static SmemCfg cfg;
+    HP_TRY(configure_smem(cfg, kern, smem));
     dim3 grid(ceil_div(m, BM) * ceil_div(n, BN), 1, nbatch);
     kern<<<grid, WM * WN * 32, smem, st>>>(m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, strideA, strideB, strideC);
     HP_LAUNCHED();

@@ -9,6 +9,7 @@ import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "hprmat.h")
+PROFILE_HEADER = os.path.join(ROOT, "include", "hprmat_profile.h")
 
 
 @pytest.fixture(scope="module")
@@ -18,8 +19,8 @@ def lib():
     return C.CDLL(path)
 
 
-def _declared_functions():
-    src = open(HEADER).read()
+def _declared_functions(header=HEADER):
+    src = open(header).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(hprmat_[a-z0-9_]+)\s*\(", src)))
 
@@ -35,6 +36,21 @@ def test_header_declares_the_boundary_calls():
 def test_library_exports_every_declared_symbol(lib):
     missing = [n for n in _declared_functions() if not hasattr(lib, n)]
     assert not missing, f"declared in hprmat.h but not exported: {missing}"
+
+
+def test_measurement_aids_live_outside_the_product_interface(lib):
+    """include/hprmat_profile.h: the timing record and the launch counter are exported by libhprmat.so, the FP64 peak probe
+    only by libhprmat_bench.so; hprmat.h declares none of them."""
+    product = set(_declared_functions())
+    aids = _declared_functions(PROFILE_HEADER)
+    assert aids and not (product & set(aids))
+    from paper_2512_11590_b200 import build
+    bench = C.CDLL(build.BENCH_LIB)
+    for n in aids:
+        if n.startswith("hprmat_bench_"):
+            assert hasattr(bench, n) and not hasattr(lib, n), n
+        else:
+            assert hasattr(lib, n), n
 
 
 def test_strerror_and_argument_validation(lib):

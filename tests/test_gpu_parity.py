@@ -233,7 +233,7 @@ def test_rmatrix_fp64_cfg3_headline_size_certificate(cfg):
     # the dropped second-order term O(||C^-1|| ||r||^2): bounded by the ORACLE's residual in the backward-error measure and
     # estimated explicitly (tests/certificate.py), neither taken from the library's own report
     assert c["backward_err"] <= 50 * w.n * 2.0 ** -53, c
-    assert c["second"] <= 1e-12 and c["contraction"] < 0.5, c
+    assert c["second"] <= 1e-12 and c["contraction"] < 1.0, c
     assert 0 <= info["backward_err"] <= 50 * w.n * 2.0 ** -53
     assert _relmax(Rg, Rg.T) <= 1e-10
     # sampled outputs the oracle can compute one by one: R_c1c2 = (h2m/a) sum_i fa_i X[(c1,i),c2] from the GPU's X
@@ -284,6 +284,14 @@ def test_preconditioned_fp64_falls_back_to_pivoting_when_the_diagonal_is_refuted
     R2, info2 = ctx.solve(E, V, hb.HPRMAT_FP64)
     R2 = _host(R2).copy()
     assert _relmax(R2, Ro) <= 1e-10 and info2["backward_err"] <= 50 * w.n * 2.0 ** -53
+    assert info2["reserved"] > 0, "the diagonal-pivot speculation was expected to be refuted (info.reserved counts the panels)"
+    # an unsynchronised call cannot fall back: it must say so through the device status word
+    ctx.solve(E, V, hb.HPRMAT_FP64, want_info=False)
+    assert ctx.last_status()[0] == hb.HPRMAT_EUNVERIFIED
+    # ... and with the configs' own couplings it reports success
+    w0 = make_workload(1, nch=12, nb=100)
+    ctx.solve(E, torch.from_numpy(w0.potential(r)).to(DEV), hb.HPRMAT_FP64, want_info=False)
+    assert ctx.last_status()[0] == hb.HPRMAT_OK
     try:
         hb.hprmat_fp64_algo(1)
         R1, _ = ctx.solve(E, V, hb.HPRMAT_FP64)
