@@ -48,11 +48,15 @@ def peaks():
 # DRAM traffic of the trailing-update kernels from the `ncu --set full` captures in profiles/r01_ncu_full.md (section 5,
 # final kernels of the round): dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the probe shape, next to
 # the algorithmic bytes of that launch (A and B once, C read + written).
+# These are NOT measured by this run (ncu cannot run inside a timed bench): each entry names the capture file and the commit
+# whose kernel it profiled.
 NCU_TRAFFIC = {
     "fp64": {"bytes": 5.575929e9 + 2.604247e9, "launch": "hprmat_zgemm (3M kernel) m=n=12800 k=1024",
-             "algorithmic_bytes": 16.0 * (2 * 12800 * 1024 + 2 * 12800 * 12800)},
+             "algorithmic_bytes": 16.0 * (2 * 12800 * 1024 + 2 * 12800 * 12800),
+             "capture": "profiles/r01_ncu_full.md section 5", "commit": "9ed5626 (round 1; kernel unchanged since)"},
     "tf32": {"bytes": 10.820277e9 + 1.285462e9, "launch": "hprmat_cgemm_tf32 m=n=12800 k=6400 (128 x 256 tiles)",
-             "algorithmic_bytes": 8.0 * (2 * 12800 * 6400 + 2 * 12800 * 12800)},
+             "algorithmic_bytes": 8.0 * (2 * 12800 * 6400 + 2 * 12800 * 12800),
+             "capture": "profiles/r01_ncu_full.md section 5", "commit": "9ed5626 (round 1; kernel unchanged since)"},
 }
 
 _DMMA_PEAK = None
@@ -87,6 +91,24 @@ def oracle_sample(cfg, steps, warmup):
     text = (f"configs[{cfg}] family reduced to Nc={w.nch}, Nb={w.nb} (N={w.n}); oracle long-double mode, factor + solves + 2 "
             f"long-double-residual refinement steps + contraction; mean of {steps} run(s)")
     return lu_flops(w.n) / t * 1e-12, t, oracle.num_threads(), text
+
+
+def cpu_full_size(cfg, w, sample_seconds):
+    """The oracle at the FULL size of the config: the stored once-only run (tests/golden/oracle_R_cfg<k>_E<E>.npz, written by
+    tests/golden/make_oracle_R.py from oracle/ only; its wall time was measured on the machine and thread count it names,
+    not on this box) when there is one, and in any case the N^3 extrapolation of this run's sample, LABELLED as such."""
+    out = {"extrapolated_from_sample": {"seconds": sample_seconds * (w.n / (CPU_SAMPLE_NCH * w.nb)) ** 3,
+                                        "label": "EXTRAPOLATED: this run's N=%d sample time x (N/%d)^3" % (
+                                            CPU_SAMPLE_NCH * w.nb, CPU_SAMPLE_NCH * w.nb)}}
+    path = os.path.join(ROOT, "tests", "golden", "oracle_R_cfg%d_E%g.npz" % (cfg, float(w.energies[0])))
+    if os.path.exists(path):
+        g = np.load(path)
+        out["stored_run"] = {"seconds": float(g["seconds"]), "threads": int(g["threads"]),
+                             "oracle_mode": "big-N (double accumulation in the O(N^3) part)" if int(g["mode"]) == 1
+                             else "long double", "n": int(g["n"]), "file": os.path.relpath(path, ROOT),
+                             "tflops_8n3_over_3": lu_flops(int(g["n"])) / float(g["seconds"]) * 1e-12,
+                             "label": "MEASURED ONCE on the build container's host cores, not in this run"}
+    return out
 
 
 def run_reference(args):
@@ -156,9 +178,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--mode", default="fp64", choices=["fp64", "mixed", "mixed_refine"])
     ap.add_argument("--cfg", type=int, default=3)
-    ap.add_argument("--zsolve", action="store_true",
-                    help="also time hprmat_zsolve alone on a dense random N x N system (raw solve, separately from assembly "
-                         "and contraction)")
+    ap.add_argument("--quick", action="store_true",
+                    help="only the headline step (and --also): skip the raw-solve, Type-1, other-config and matching legs")
     ap.add_argument("--nonlocal", dest="nonlocal_leg", action="store_true",
                     help="also time hprmat_solve_nonlocal (FP64, SURVEY 8(f) row 4) on the config with the synthetic Perey-Buck-type "
                          "non-local potential of workloads.nonlocal_matrix, built on the device")
@@ -183,6 +204,7 @@ def main():
         hb.hprmat_zgemm_algo(args.zgemm_algo)
     if args.fp64_algo:
         hb.hprmat_fp64_algo(args.fp64_algo)
+    full = not args.quick
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -205,16 +227,19 @@ def main():
     E = scan.bench_energy(w.energies, rank)   # rank k takes the k-th point of the config's energy scan (replicas)
     N = w.n
 
-    def measure(mode_name):
+    def measure(mode_name, w=w, E=E, steps=args.steps, warmup=args.warmup, fp64_algo=0, roofline=True, e2e=True):
+        N = w.n
         mode = hb.MODES[mode_name]
         ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
+        if fp64_algo:
+            ctx.set_option(hb.HPRMAT_OPT_FP64_ALGO, fp64_algo)
         r, _ = ctx.mesh()
         V_host = torch.from_numpy(w.potential(r)).pin_memory()
         V = V_host.to("cuda")
         R = torch.empty((w.nch, w.nch), dtype=torch.complex128, device="cuda")
         R_host = torch.empty((w.nch, w.nch), dtype=torch.complex128).pin_memory()
 
-        for _ in range(args.warmup):
+        for _ in range(warmup):
             ctx.solve(E, V, mode, R=R)
         # ---- timed region: K steps, device-resident inputs
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -223,7 +248,7 @@ def main():
         sampler = ClockSampler(local) if rank == 0 else None
         l0 = hb.hprmat_launch_count()
         e0.record()
-        for _ in range(args.steps):
+        for _ in range(steps):
             _, info = ctx.solve(E, V, mode, R=R)
             infos.append(info)
         e1.record()
@@ -232,22 +257,25 @@ def main():
         clocks = sampler.stop() if sampler else None
         t_dev = e0.elapsed_time(e1) * 1e-3
         t_max = scan.max_over_ranks(t_dev, device="cuda")
-        sec_per_step = t_max / args.steps
+        sec_per_step = t_max / steps
+        graphs = ctx.graphs()
 
         # ---- end to end: host V in, host R out, through hprmat_solve_host, copies inside the timed region
-        Vh_np, Rh_np = V_host.numpy(), R_host.numpy()
-        ctx.solve_host(E, Vh_np, mode, R_host=Rh_np)
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.steps):
+        e2e_sec = None
+        if e2e:
+            Vh_np, Rh_np = V_host.numpy(), R_host.numpy()
             ctx.solve_host(E, Vh_np, mode, R_host=Rh_np)
-        torch.cuda.synchronize()
-        te = time.perf_counter() - t0
-        e2e_sec = scan.max_over_ranks(te, device="cuda") / args.steps
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(steps):
+                ctx.solve_host(E, Vh_np, mode, R_host=Rh_np)
+            torch.cuda.synchronize()
+            te = time.perf_counter() - t0
+            e2e_sec = scan.max_over_ranks(te, device="cuda") / steps
 
         # ---- roofline leg: one more step with a CUDA-event pair around every GEMM launch (the trailing-update kernel)
         roof = None
-        if rank == 0:
+        if rank == 0 and roofline:
             hb.hprmat_profile(True)
             _, pinfo = ctx.solve(E, V, mode, R=R)
             hb.hprmat_profile(False)
@@ -287,9 +315,11 @@ def main():
                "time_to_rmatrix_s": sec_per_step, "lu_tflops": info["lu_tflops"],
                "stages_ms": {k: info[k] for k in ("ms_assemble", "ms_lu", "ms_solve", "ms_refine", "ms_contract", "ms_total")},
                "refine_steps": info["refine_steps"], "backward_err": info["backward_err"], "status": info["status"],
-               "e2e": {"value": world * lu_flops(N) / e2e_sec * 1e-12, "unit": UNIT, "seconds_per_step": e2e_sec,
-                       "h2d_bytes_per_step": int(V_host.numel() * 16), "d2h_bytes_per_step": int(R_host.numel() * 16)},
-               "gpu_launches": int(launches), "clocks": clocks, "roofline": roof}
+               "e2e": ({"value": world * lu_flops(N) / e2e_sec * 1e-12, "unit": UNIT, "seconds_per_step": e2e_sec,
+                        "h2d_bytes_per_step": int(V_host.numel() * 16), "d2h_bytes_per_step": int(R_host.numel() * 16)}
+                       if e2e else None),
+               "gpu_launches": int(launches), "cuda_graphs": {"captured": graphs[0], "eager": graphs[1]},
+               "steps": steps, "warmup": warmup, "clocks": clocks, "roofline": roof}
         res["_R"] = R.clone()
         ctx.destroy()
         del V, R, ctx
@@ -386,22 +416,42 @@ def main():
                                hb.hprmat_fp64_algo()],
                            "l2": "inputs_larger_than_L2 (matrix 16 N^2 B >> 126 MB)"}}
         for k in ("time_to_rmatrix_s", "lu_tflops", "stages_ms", "refine_steps", "backward_err", "e2e", "gpu_launches",
-                  "clocks", "roofline"):
+                  "cuda_graphs", "clocks", "roofline"):
             line[k] = m[k]
         # the metric names FP64 AND mixed: the other precision mode, measured the same way in the same run
         line["other_modes"] = others
-        if world == 1:
+        if full and world == 1:
             line["matching"] = matching_leg(R_last)
         if args.nonlocal_leg and world == 1:
             line["nonlocal"] = nonlocal_leg()
-        if args.zsolve and world == 1:
+        if full and world == 1:
+            # north_star: "raw dense complex solve timed separately from assembly and the R contraction"
             line["raw_zsolve"] = [raw_zsolve("fp64"), raw_zsolve("mixed_refine")]
+            # the paper's Type 1 (LU of C - E I itself, partial pivoting with row interchanges) next to the default
+            t1 = measure("fp64", steps=2, warmup=1, fp64_algo=1, roofline=True, e2e=False)
+            t1.pop("_R")
+            line["fp64_type1_lu_of_C_minus_EI"] = {k: t1[k] for k in ("ms_per_step", "lu_tflops", "stages_ms", "refine_steps",
+                                                                        "backward_err", "steps", "warmup")}
+            line["fp64_type1_lu_of_C_minus_EI"]["breakdown_ms"] = t1["roofline"]["breakdown_ms"]
+            # the other configs of BASELINE.json, every listed mode: time-to-R-matrix and LU TFLOP/s (fewer steps, stated)
+            cfgs = {}
+            for k in (1, 2, 4):
+                wk = make_workload(k)
+                cfgs[f"cfg{k}"] = {"N": wk.n, "energy": float(wk.energies[len(wk.energies) // 2])}
+                for mname in wk.modes:
+                    st, wu = (2, 1) if k == 4 else (3, 2)
+                    mm = measure(mname, w=wk, E=float(wk.energies[len(wk.energies) // 2]), steps=st, warmup=wu, roofline=False,
+                                 e2e=False)
+                    mm.pop("_R")
+                    cfgs[f"cfg{k}"][mname] = {kk: mm[kk] for kk in ("time_to_rmatrix_s", "value", "lu_tflops", "stages_ms",
+                                                                    "refine_steps", "backward_err", "status", "steps", "warmup")}
+            line["configs"] = cfgs
         line["paper_context"] = {"rtx3090_fp32_s": 3.554, "rtx3090_hybrid_s": 9.85, "xeon48_zgesv_s": 52.098,
                                  "legacy_inversion_s": 144.948, "note": "PAPER.md Tables 3-4, N=25600, other hardware"}
         if not args.no_cpu_baseline and world == 1:
             v, t, cores, text = oracle_sample(args.cfg, 1, 0)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text,
-                                    "seconds": t}
+                                    "seconds": t, "full_size": cpu_full_size(args.cfg, w, t)}
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -123,7 +123,9 @@ int hprmat_fp64_algo(int algo);
 /* Per-context settings.  value 0 = follow the process default again. */
 enum {
     HPRMAT_OPT_FP64_ALGO = 1,  /* 1 or 2, see hprmat_fp64_algo                                                           */
-    HPRMAT_OPT_ZGEMM_ALGO = 2  /* 3 or 4, see hprmat_zgemm_algo                                                          */
+    HPRMAT_OPT_ZGEMM_ALGO = 2, /* 3 or 4, see hprmat_zgemm_algo                                                          */
+    HPRMAT_OPT_GRAPHS = 3      /* 1 (default): the factorisation and every triangular solve of this context are captured    */
+                               /* into CUDA graphs on first use and replayed with one launch each; 0: plain stream launches */
 };
 int hprmat_set_option(hprmat_ctx *ctx, int option, int value);
 

@@ -27,6 +27,11 @@ int hprmat_profile_cat(int cat, double *ms, double *flops, long long *launches);
  * (bench.py's gpu_launches) */
 long long hprmat_launch_count(void);
 
+/* How many launch sequences (factorisations, triangular solves) of the context are replayed from CUDA graphs (captured) and
+ * how many had to stay plain stream launches (eager: capture refused).  captured / eager: host, may be NULL. */
+struct hprmat_ctx;
+int hprmat_profile_graphs(const struct hprmat_ctx *ctx, int *captured, int *eager);
+
 /* libhprmat_bench.so: FP64 tensor-core (DMMA, mma.sync.m8n8k4.f64) issue-rate ceiling of the device, measured with a
  * register-resident loop (no memory traffic) on 148*ctas_per_sm CTAs of 8 warps, `iters` x 8 MMAs per warp.
  * tflops (host, out): real TFLOP/s; ms (host, out, may be NULL): device time of the timed launch.  Synchronises. */

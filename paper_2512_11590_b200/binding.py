@@ -15,7 +15,7 @@ LIBPATH = os.path.join(HERE, "libhprmat.so")
 
 HPRMAT_FP64, HPRMAT_MIXED, HPRMAT_MIXED_REFINE = 1, 2, 3
 HPRMAT_OK, HPRMAT_ESINGULAR, HPRMAT_ENOTCONVERGED, HPRMAT_ENOMEM, HPRMAT_ECUDA, HPRMAT_EUNVERIFIED = 0, 1, 2, 3, 4, 5
-HPRMAT_OPT_FP64_ALGO, HPRMAT_OPT_ZGEMM_ALGO = 1, 2
+HPRMAT_OPT_FP64_ALGO, HPRMAT_OPT_ZGEMM_ALGO, HPRMAT_OPT_GRAPHS = 1, 2, 3
 MODES = {"fp64": HPRMAT_FP64, "mixed": HPRMAT_MIXED, "mixed_refine": HPRMAT_MIXED_REFINE}
 
 
@@ -187,6 +187,12 @@ class Context:
         if rc < 0:
             raise HprmatError(rc, "hprmat_last_status")
         return rc, steps.value, piv.value
+
+    def graphs(self):
+        """(captured, eager): launch sequences of this context replayed from CUDA graphs / left as plain launches."""
+        a, b = C.c_int(0), C.c_int(0)
+        _check(lib().hprmat_profile_graphs(self._h, C.byref(a), C.byref(b)), "hprmat_profile_graphs")
+        return a.value, b.value
 
     def get_x(self, device="cuda"):
         X = torch.empty((self.nch, self.n), dtype=torch.complex128, device=device)  # column-major N x nch

@@ -20,6 +20,7 @@
 #include "precond.cuh"
 #include "refine.cuh"
 #include "structured.cuh"
+#include "../../include/hprmat_profile.h"
 
 using namespace hp;
 
@@ -33,6 +34,7 @@ struct hprmat_ctx {
     double2 *d_C = nullptr;                                   // N x N complex128 (FP64 mode)
     double2 *d_X = nullptr, *d_Rr = nullptr, *d_Rlo = nullptr;  // N x nch each
     double2 *d_V = nullptr, *d_R = nullptr;                   // staging for hprmat_solve_host
+    double2 *d_Voff = nullptr, *d_Xp = nullptr, *d_Pp = nullptr;  // residual: V without its diagonal, point-major X, V X
     void *d_work = nullptr;                                   // LU workspace
     int *d_ipiv = nullptr, *d_info = nullptr;
     double *d_scal = nullptr;                                 // small device scalars (norms, maxima)
@@ -59,6 +61,18 @@ struct hprmat_ctx {
     // what the last solve was, for hprmat_last_status
     int last_fac = -1, last_mode = 0, last_max_refine = 0;
     bool last_valid = false;
+    // CUDA graphs of the factorisations and triangular solves (thousands of dependent launches that depend on nothing but
+    // this context's buffers): captured once on an internal stream, replayed on the caller's stream
+    struct GraphEntry {
+        int kind;              // 0 = getrf, 1 = getrs
+        int flags;             // factored matrix / pivoting variant / right-hand-side count
+        const void *key;       // right-hand-side buffer (getrs)
+        cudaGraphExec_t exec;  // nullptr: capture is not possible for this entry, run it eagerly
+        long long launches;    // kernel launches one replay stands for
+    };
+    std::vector<GraphEntry> graphs;
+    cudaStream_t cap = nullptr;  // capture stream
+    int use_graphs = 1;
 };
 
 namespace {
@@ -101,6 +115,7 @@ void shifted_legendre_zeros(int n, std::vector<ld> &x) {
 int free_ctx(hprmat_ctx *c) {
     if (!c) return 0;
     cudaFree(c->d_hT); cudaFree(c->d_dg0); cudaFree(c->d_ethr); cudaFree(c->d_fa);
+    cudaFree(c->d_Voff); cudaFree(c->d_Xp); cudaFree(c->d_Pp);
     cudaFree(c->d_C); cudaFree(c->d_X); cudaFree(c->d_Rr); cudaFree(c->d_Rlo); cudaFree(c->d_V); cudaFree(c->d_R);
     cudaFree(c->d_Sre); cudaFree(c->d_Sim); cudaFree(c->d_Bre); cudaFree(c->d_Bim); cudaFree(c->d_Kinv); cudaFree(c->d_workc);
     cudaFree(c->d_work); cudaFree(c->d_ipiv); cudaFree(c->d_info); cudaFree(c->d_scal);
@@ -111,6 +126,9 @@ int free_ctx(hprmat_ctx *c) {
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->side) cudaStreamDestroy(c->side);
+    for (auto &g : c->graphs)
+        if (g.exec) cudaGraphExecDestroy(g.exec);
+    if (c->cap) cudaStreamDestroy(c->cap);
     delete c;
     return 0;
 }
@@ -221,6 +239,9 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
     HP_ALLOC(c->d_Rr, sizeof(double2) * N * nch);
     HP_ALLOC(c->d_Rlo, sizeof(double2) * N * nch);
     HP_ALLOC(c->d_V, sizeof(double2) * (size_t)nb * nch * nch);
+    HP_ALLOC(c->d_Voff, sizeof(double2) * (size_t)nb * nch * nch);
+    HP_ALLOC(c->d_Xp, sizeof(double2) * N * nch);
+    HP_ALLOC(c->d_Pp, sizeof(double2) * N * nch);
     HP_ALLOC(c->d_R, sizeof(double2) * (size_t)nch * nch);
     HP_ALLOC(c->d_ipiv, sizeof(int) * N);
     HP_ALLOC(c->d_info, sizeof(int) * IN_NWORDS);
@@ -234,6 +255,7 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
     for (auto &e : c->ev)
         if (cudaEventCreate(&e) != cudaSuccess) { free_ctx(c); return HPRMAT_ECUDA; }
     if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&c->cap, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
         cudaGetLastError();
@@ -348,12 +370,53 @@ __global__ void __launch_bounds__(256) set_diag_blocks_identity_kernel(int nch, 
     }
 }
 
+// ---- CUDA-graph replay of a launch sequence that depends on the context's buffers only ---------------------------------
+// enqueue(stream) issues the sequence.  First use: it is captured on the context's capture stream (the side stream joins the
+// capture through its fork/join events) and instantiated; afterwards one cudaGraphLaunch on the caller's stream stands
+// for it.  Anything that cannot be captured (or the per-launch timing of hprmat_profile, which needs real launches) runs
+// eagerly on the caller's stream, as before.
+template <class F> int replay(hprmat_ctx *c, int kind, int flags, const void *key, F &&enqueue) {
+    if (!c->use_graphs || prof_enabled()) return enqueue(c->st);
+    flags |= zgemm_algo_in_force() << 16;  // the captured sequence holds the kernels of this decomposition
+    hprmat_ctx::GraphEntry *ent = nullptr;
+    for (auto &g : c->graphs)
+        if (g.kind == kind && g.flags == flags && g.key == key) ent = &g;
+    if (!ent) {
+        hprmat_ctx::GraphEntry ne{kind, flags, key, nullptr, 0};
+        const long long l0 = g_launches.load();
+        if (cudaStreamBeginCapture(c->cap, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            const int rc = enqueue(c->cap);
+            cudaGraph_t graph = nullptr;
+            const cudaError_t e = cudaStreamEndCapture(c->cap, &graph);
+            ne.launches = g_launches.load() - l0;
+            g_launches.fetch_sub(ne.launches);  // captured, not launched
+            if (rc == 0 && e == cudaSuccess && graph != nullptr) {
+                if (cudaGraphInstantiate(&ne.exec, graph, 0) != cudaSuccess) ne.exec = nullptr;
+            }
+            if (graph) cudaGraphDestroy(graph);
+        }
+        cudaGetLastError();  // a refused capture is not an error of the solve
+        c->graphs.push_back(ne);
+        ent = &c->graphs.back();
+    }
+    if (!ent->exec) return enqueue(c->st);
+    HP_CUDA(cudaGraphLaunch(ent->exec, c->st));
+    g_launches.fetch_add(ent->launches);
+    return 0;
+}
+
+template <class V> int getrs_replay(hprmat_ctx *c, int nrhs, V A, V B, LuWork<V> &wk, const void *key, int variant) {
+    const int n = c->n;
+    return replay(c, 1, nrhs * 4 + variant, key, [&](cudaStream_t s) { return getrs<V>(s, n, nrhs, A, B, wk); });
+}
+
 // ---- stages ---------------------------------------------------------------------------------------------------------------
 int assemble(hprmat_ctx *c, Fac fac, const Problem &p, double energy, bool want_anorm) {
     cudaStream_t st = c->st;
     const int N = c->n, nch = c->nch, nb = c->nb;
     HP_CUDA(cudaMemsetAsync(c->d_info, 0, sizeof(int) * IN_NWORDS, st));
     if (p.W) HP_CUDA(cudaMemsetAsync(c->d_V, 0, sizeof(double2) * (size_t)nb * nch * nch, st));  // "no local potential"
+    else HP_TRY(coupling_without_diagonal(st, c->tab, p.V, c->d_Voff));  // operand of the residual's tensor-core part
     if (fac == FAC_C_Z) {
         if (p.W) HP_TRY(assemble_nonlocal(st, c->tab, energy, p.W, p.ldw, c->d_C, N));
         else HP_TRY(assemble_z(st, c->tab, energy, p.V, c->d_C, N));
@@ -382,12 +445,16 @@ int factor(hprmat_ctx *c, Fac fac, bool pivoting_fallback) {
     cudaStream_t st = c->st;
     const int N = c->n;
     int *zp = c->d_info + IN_ZERO_PIVOT;
+    (void)st;
     if (fac == FAC_S_C) {
         c->wc.speculate = !pivoting_fallback;
-        return getrf<CView>(st, N, CView(c->d_Sre, c->d_Sim, c->ldS), c->d_ipiv, zp, c->wc);
+        return replay(c, 0, 4 + (pivoting_fallback ? 1 : 0), nullptr, [&](cudaStream_t s) {
+            return getrf<CView>(s, N, CView(c->d_Sre, c->d_Sim, c->ldS), c->d_ipiv, zp, c->wc);
+        });
     }
     c->wz.speculate = (fac == FAC_S_Z);
-    return getrf<ZView>(st, N, ZView(c->d_C, N), c->d_ipiv, zp, c->wz);
+    return replay(c, 0, fac == FAC_S_Z ? 2 : 0, nullptr,
+                  [&](cudaStream_t s) { return getrf<ZView>(s, N, ZView(c->d_C, N), c->d_ipiv, zp, c->wz); });
 }
 
 // X <- (factored matrix)^-1 (its right-hand sides); leaves max|X| in scal[SC_X0] (FP64) or scal[SC_XN] (complex64 factors)
@@ -397,7 +464,7 @@ int first_solve(hprmat_ctx *c, Fac fac, int *x0_word) {
     if (fac == FAC_S_C) {
         CView S(c->d_Sre, c->d_Sim, c->ldS), Bs(c->d_Bre, c->d_Bim, c->ldS);
         HP_TRY(precond_rhs(st, c->tab, c->d_Kinv, Bs));
-        HP_TRY(getrs<CView>(st, N, nch, S, Bs, c->wc));
+        HP_TRY(getrs_replay<CView>(c, nch, S, Bs, c->wc, Bs.re, 0));
         HP_TRY(promote_add(st, N, nch, c->d_X, N, Bs, false, c->d_scal + SC_DN));
         *x0_word = SC_XN;
         return 0;
@@ -405,7 +472,7 @@ int first_solve(hprmat_ctx *c, Fac fac, int *x0_word) {
     ZView A(c->d_C, N), X(c->d_X, N);
     if (fac == FAC_S_Z) HP_TRY(precond_rhs_z(st, c->tab, c->d_Kinv, X));
     else HP_TRY(build_rhs(st, c->tab, c->d_X, N));
-    HP_TRY(getrs<ZView>(st, N, nch, A, X, c->wz));
+    HP_TRY(getrs_replay<ZView>(c, nch, A, X, c->wz, X.p, fac));
     HP_TRY(maxabs(st, N, nch, c->d_X, N, c->d_scal + SC_X0));
     *x0_word = SC_X0;
     return 0;
@@ -417,8 +484,9 @@ int residual(hprmat_ctx *c, const Problem &p, double energy, double *rmax_dev) {
     cudaStream_t st = c->st;
     const int N = c->n, nch = c->nch;
     if (!p.W)
-        return structured_residual(st, c->tab, energy, p.V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, rmax_dev);
-    HP_TRY(structured_residual(st, c->tab, energy, c->d_V, nch, nullptr, 0, c->d_X, N, c->d_Rr, c->d_Rlo, N, nullptr));
+        return structured_residual_tc(st, c->tab, energy, p.V, c->d_Voff, c->d_X, N, c->d_Rr, c->d_Rlo, N, c->d_Xp, c->d_Pp,
+                                      rmax_dev);
+    HP_TRY(structured_residual_tc(st, c->tab, energy, c->d_V, nullptr, c->d_X, N, c->d_Rr, c->d_Rlo, N, nullptr, nullptr, nullptr));
     HP_TRY(gemm(st, N, nch, N, -1.0, ZView((double2 *)p.W, p.ldw), ZView(c->d_X, N), 1.0, ZView(c->d_Rr, N)));
     if (rmax_dev) HP_TRY(maxabs(st, N, nch, c->d_Rr, N, rmax_dev));
     return 0;
@@ -430,18 +498,18 @@ int correction(hprmat_ctx *c, Fac fac) {
     const int N = c->n, nch = c->nch, nb = c->nb;
     const int *gate = c->d_info + IN_VERDICT;
     if (fac == FAC_C_Z) {
-        HP_TRY(getrs<ZView>(st, N, nch, ZView(c->d_C, N), ZView(c->d_Rr, N), c->wz));
+        HP_TRY(getrs_replay<ZView>(c, nch, ZView(c->d_C, N), ZView(c->d_Rr, N), c->wz, c->d_Rr, fac));
         return axpy_norm(st, N, nch, c->d_X, N, c->d_Rr, N, c->d_scal + SC_DN, gate);
     }
     // z = K_d^-1 r: one nb x nb by nb x nch product per channel (FP64 tensor cores), into Rlo
     HP_TRY(zgemm_batched(st, nb, nch, nb, 1.0, c->d_Kinv, nb, (long)nb * nb, c->d_Rr, N, nb, 0.0, c->d_Rlo, N, nb, nch));
     if (fac == FAC_S_Z) {
-        HP_TRY(getrs<ZView>(st, N, nch, ZView(c->d_C, N), ZView(c->d_Rlo, N), c->wz));
+        HP_TRY(getrs_replay<ZView>(c, nch, ZView(c->d_C, N), ZView(c->d_Rlo, N), c->wz, c->d_Rlo, fac));
         return axpy_norm(st, N, nch, c->d_X, N, c->d_Rlo, N, c->d_scal + SC_DN, gate);
     }
     CView S(c->d_Sre, c->d_Sim, c->ldS), Bs(c->d_Bre, c->d_Bim, c->ldS);
     HP_TRY(demote(st, N, nch, c->d_Rlo, N, Bs));
-    HP_TRY(getrs<CView>(st, N, nch, S, Bs, c->wc));
+    HP_TRY(getrs_replay<CView>(c, nch, S, Bs, c->wc, Bs.re, 0));
     return promote_add(st, N, nch, c->d_X, N, Bs, true, c->d_scal + SC_DN, gate);
 }
 
@@ -632,6 +700,10 @@ extern "C" int hprmat_set_option(hprmat_ctx *ctx, int option, int value) {
             if (value != 0 && value != 3 && value != 4) return -3;
             ctx->zgemm_algo = value;
             return HPRMAT_OK;
+        case HPRMAT_OPT_GRAPHS:
+            if (value != 0 && value != 1) return -3;
+            ctx->use_graphs = value;
+            return HPRMAT_OK;
         default: return -2;
     }
 }
@@ -646,6 +718,17 @@ extern "C" int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int m
     Problem p;
     p.V = (const double2 *)V;
     return solve_any(ctx, p, energy, mode, max_refine, tol, (double2 *)R, info);
+}
+
+// measurement aid (include/hprmat_profile.h): how many launch sequences of this context are replayed from CUDA graphs and how
+// many had to stay plain launches
+extern "C" int hprmat_profile_graphs(const hprmat_ctx *ctx, int *captured, int *eager) {
+    if (!ctx) return -1;
+    int nc = 0, ne = 0;
+    for (const auto &g : ctx->graphs) (g.exec ? nc : ne)++;
+    if (captured) *captured = nc;
+    if (eager) *eager = ne;
+    return HPRMAT_OK;
 }
 
 // Status of the last solve of this context, for calls made with info == NULL: synchronises the stream, reads the device

@@ -336,6 +336,113 @@ int structured_residual(cudaStream_t st, const StructTables &t, double energy, c
     return 0;
 }
 
+// ---- the coupling part on the FP64 tensor cores ---------------------------------------------------------------------------
+// The within-channel part (entries up to ~1e9: the end-point kinetic diagonal) is where the residual cancels and needs the
+// double-double sum; the couplings are <= a few MeV, so sum_{c' != c} V_cc'(r_i) X[(c',i),q] in plain FP64 (DMMA) is exact
+// to ~Nc 2^-53 |V_cc'| |X| ~ 1e-14 |X|, eight orders below |C||X|.  Per mesh point i that is one Nc x Nc by Nc x nrhs
+// product: V_i (zero diagonal) times the point-major copy of X.  8 Nb Nc^3 flops at the DMMA rate instead of ~20x that many
+// FP64 CUDA-core operations of the double-double loop (4.2 ms -> 0.5 ms per residual at cfg 3).
+__global__ void __launch_bounds__(256) zero_diag_copy_kernel(int nch, long tot, const double2 *__restrict__ V,
+                                                             double2 *__restrict__ Voff) {
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < tot; idx += (long)gridDim.x * blockDim.x) {
+        const int c1 = (int)(idx % nch), c2 = (int)((idx / nch) % nch);
+        Voff[idx] = c1 == c2 ? make_double2(0.0, 0.0) : V[idx];
+    }
+}
+int coupling_without_diagonal(cudaStream_t st, const StructTables &t, const double2 *V, double2 *Voff) {
+    const long tot = (long)t.nb * t.nch * t.nch;
+    zero_diag_copy_kernel<<<(int)std::min<long>(ceil_div(tot, 256), 148L * 16), 256, 0, st>>>(t.nch, tot, V, Voff);
+    HP_LAUNCHED();
+    return 0;
+}
+
+// Xp[(i nrhs + q) nch + c] = X[q ldx + c nb + i]: 32 x 32 tiles over (c, i), one right-hand side per blockIdx.z
+__global__ void __launch_bounds__(256) to_point_major_kernel(int nch, int nb, int nrhs, const double2 *__restrict__ X, long ldx,
+                                                             double2 *__restrict__ Xp) {
+    __shared__ double2 tile[32][33];
+    const int q = blockIdx.z, c0 = blockIdx.y * 32, i0 = blockIdx.x * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int k = ty; k < 32; k += 8) {  // read: i fastest
+        const int c = c0 + k, i = i0 + tx;
+        if (c < nch && i < nb) tile[k][tx] = X[(long)q * ldx + (long)c * nb + i];
+    }
+    __syncthreads();
+    for (int k = ty; k < 32; k += 8) {  // write: c fastest
+        const int i = i0 + k, c = c0 + tx;
+        if (c < nch && i < nb) Xp[((long)i * nrhs + q) * nch + c] = tile[tx][k];
+    }
+}
+
+// R[(c,i),q] = (hi + lo)[(c,i),q] - P[(i nrhs + q) nch + c]  (P == nullptr: no coupling term); rmax as above
+__global__ void __launch_bounds__(256) resid_combine_kernel(int nch, int nb, int nrhs, double2 *__restrict__ R,
+                                                            const double2 *__restrict__ Rlo, long ldr,
+                                                            const double2 *__restrict__ P, double *rmax) {
+    __shared__ double2 tile[32][33];
+    __shared__ double shred[32];
+    const int q = blockIdx.z, c0 = blockIdx.y * 32, i0 = blockIdx.x * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    if (P) {
+        for (int k = ty; k < 32; k += 8) {  // read: c fastest
+            const int i = i0 + k, c = c0 + tx;
+            if (c < nch && i < nb) tile[tx][k] = P[((long)i * nrhs + q) * nch + c];
+        }
+        __syncthreads();
+    }
+    double lmax = 0.0;
+    for (int k = ty; k < 32; k += 8) {  // i fastest
+        const int c = c0 + k, i = i0 + tx;
+        if (c < nch && i < nb) {
+            const long at = (long)q * ldr + (long)c * nb + i;
+            double2 h = R[at];
+            const double2 l = Rlo[at];
+            if (P) {
+                const double2 p = tile[k][tx];
+                // TwoSum of hi - p, the error joins the low word
+                const double sr = __dsub_rn(h.x, p.x), br = __dsub_rn(sr, h.x);
+                const double er = __dadd_rn(__dsub_rn(h.x, __dsub_rn(sr, br)), __dsub_rn(-p.x, br));
+                const double si = __dsub_rn(h.y, p.y), bi = __dsub_rn(si, h.y);
+                const double ei = __dadd_rn(__dsub_rn(h.y, __dsub_rn(si, bi)), __dsub_rn(-p.y, bi));
+                h = make_double2(__dadd_rn(sr, __dadd_rn(l.x, er)), __dadd_rn(si, __dadd_rn(l.y, ei)));
+            } else {
+                h = make_double2(__dadd_rn(h.x, l.x), __dadd_rn(h.y, l.y));
+            }
+            R[at] = h;
+            lmax = fmax(lmax, sqrt(h.x * h.x + h.y * h.y));
+        }
+    }
+    lmax = block_max(lmax, shred);
+    if (threadIdx.x == 0 && rmax) atomic_max_nonneg(rmax, lmax);
+}
+
+int zgemm_batched(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda, long strideA,
+                  const double2 *B, long ldb, long strideB, double beta, double2 *C, long ldc, long strideC, int nbatch);
+
+int structured_residual_tc(cudaStream_t st, const StructTables &t, double energy, const double2 *V, const double2 *Voff,
+                           const double2 *X, long ldx, double2 *R, double2 *Rlo, long ldr, double2 *Xp, double2 *Pp,
+                           double *rmax_dev) {
+    const int nrhs = t.nch;
+    if (rmax_dev) HP_CUDA(cudaMemsetAsync(rmax_dev, 0, sizeof(double), st));
+    {
+        dim3 grid(t.nch, ceil_div(nrhs, RES_QT));
+        const size_t smem = sizeof(double2) * RES_QT * t.nb;
+        static SmemCfg cfg1;
+        if (smem > 48 * 1024) HP_TRY(configure_smem(cfg1, resid_channel_kernel, smem));
+        resid_channel_kernel<<<grid, RES_NT, smem, st>>>(t.nch, t.nb, nrhs, t.hT, t.dg0, t.ethr, energy, t.fa, V, nullptr, 0, X, ldx,
+                                                         R, Rlo, ldr);
+        HP_LAUNCHED();
+    }
+    const dim3 tgrid(ceil_div(t.nb, 32), ceil_div(t.nch, 32), nrhs);
+    if (Voff) {
+        to_point_major_kernel<<<tgrid, 256, 0, st>>>(t.nch, t.nb, nrhs, X, ldx, Xp);
+        HP_LAUNCHED();
+        HP_TRY(zgemm_batched(st, t.nch, nrhs, t.nch, 1.0, Voff, t.nch, (long)t.nch * t.nch, Xp, t.nch, (long)t.nch * nrhs, 0.0, Pp,
+                             t.nch, (long)t.nch * nrhs, t.nb));
+    }
+    resid_combine_kernel<<<tgrid, 256, 0, st>>>(t.nch, t.nb, nrhs, R, Rlo, ldr, Voff ? Pp : nullptr, rmax_dev);
+    HP_LAUNCHED();
+    return 0;
+}
+
 // ---------------------------------------------------------------------------------------------------- update + norms
 // X += D; norms[0] = max|D|, norms[1] = max|X_new|  (moduli; norms pre-zeroed by the caller)
 __global__ void __launch_bounds__(256) axpy_norm_kernel(long rows, int cols, double2 *__restrict__ X, long ldx,

@@ -30,6 +30,14 @@ int structured_residual(cudaStream_t st, const StructTables &t, double energy, c
                         const double2 *Bx, long ldb, const double2 *X, long ldx, double2 *R, double2 *Rlo, long ldr,
                         double *rmax_dev);
 // X += D; norms_dev[0] = max|D|, norms_dev[1] = max|X|.  gate_dev: as in promote_add (precond.cuh)
+// Voff <- V with the channel-diagonal entries V_cc(r_i) zeroed (they belong to the within-channel, double-double part)
+int coupling_without_diagonal(cudaStream_t st, const StructTables &t, const double2 *V, double2 *Voff);
+// Same residual for the nch surface right-hand sides, the coupling part as one batched DMMA product per mesh point on the
+// point-major copy of X (within-channel part still double-double).  Voff == nullptr: no coupling term (V = 0).
+// Xp, Pp: N x nch scratch each.
+int structured_residual_tc(cudaStream_t st, const StructTables &t, double energy, const double2 *V, const double2 *Voff,
+                           const double2 *X, long ldx, double2 *R, double2 *Rlo, long ldr, double2 *Xp, double2 *Pp,
+                           double *rmax_dev);
 int axpy_norm(cudaStream_t st, long rows, int cols, double2 *X, long ldx, const double2 *D, long ldd, double *norms_dev,
               const int *gate_dev = nullptr);
 int maxabs(cudaStream_t st, long rows, int cols, const double2 *X, long ldx, double *out_dev);

@@ -27,6 +27,7 @@ template <class E> struct TopLuSmem {
     E tile[TW * TW];         // column-major, ld = TW: the factored top block
     E rowb[2][2][TW];        // [which sweep][parity][col]: the row every thread needs in a step
     E colb[2][TW];           // [parity][row]: column j of the LU sweep
+    E invp[TW];              // 1 / u_jj (0 for a zero pivot), published by the owner of the diagonal element
 };
 
 template <class V>
@@ -63,15 +64,18 @@ __global__ void __launch_bounds__(TL_NT, 1)
             if (tj == jj) {
 #pragma unroll
                 for (int a = JB; a < TL_R; ++a) sm.colb[par][ti + 16 * a] = x[a][JB];
+                if (ti == jj) {  // the pivot's owner inverts it once for everybody (the long-latency part of the step)
+                    const E pv = x[JB][JB];
+                    const bool sing = (pv.x == (T)0 && pv.y == (T)0);
+                    sm.invp[j] = sing ? zero : crecip_fast(pv);
+                    if (sing) {
+                        atomicCAS(info, 0, c0 + j + 1);
+                        bad = 1;
+                    }
+                }
             }
             __syncthreads();
-            const E pv = sm.rowb[0][par][j];
-            const bool sing = (pv.x == (T)0 && pv.y == (T)0);
-            const E ip = sing ? zero : crecip_fast(pv);
-            if (sing && tid == 0 && j < w) {
-                atomicCAS(info, 0, c0 + j + 1);
-                bad = 1;
-            }
+            const E ip = sm.invp[j];
             E l[TL_R], u[TL_R];
 #pragma unroll
             for (int a = JB; a < TL_R; ++a) {
@@ -128,8 +132,7 @@ __global__ void __launch_bounds__(TL_NT, 1)
                 for (int b = 0; b <= JB; ++b) sm.rowb[0][par][tj + 16 * b] = xl[JB][b];
             }
             if (ti == 15 - jj) {  // row ju of XU, scaled by 1/u_jj: non-zero in columns >= ju
-                const E pu = sm.tile[ju * TW + ju];
-                const E ipu = (pu.x == (T)0 && pu.y == (T)0) ? zero : crecip_fast(pu);
+                const E ipu = sm.invp[ju];
 #pragma unroll
                 for (int b = UB; b < TL_R; ++b) {
                     xu[UB][b] = cmul(xu[UB][b], ipu);
@@ -185,15 +188,20 @@ __global__ void __launch_bounds__(TL_NT, 1)
         }
 }
 
-// counts the multipliers of L (m x w) that violate |l|_1 <= 1/2 (or are NaN): one CTA per 256 rows
+// counts the multipliers of L (m x w) that violate |l|_1 <= 1/2 (or are NaN): CTA = 256 rows x CHK_C columns
+constexpr int CHK_C = 8;
 template <class V> __global__ void __launch_bounds__(256) check_multipliers_kernel(V L, int m, int w, int *refuted) {
+    typedef typename V::elem_t E;
     typedef typename V::real_t T;
-    const int row = blockIdx.x * 256 + threadIdx.x;
+    const int row = blockIdx.x * 256 + threadIdx.x, c0 = blockIdx.y * CHK_C;
     int bad = 0;
     if (row < m) {
-#pragma unroll 8
-        for (int c = 0; c < w; ++c)
-            if (!(cabs1(L.get(row, c)) <= (T)0.5)) bad = 1;
+        E v[CHK_C];
+#pragma unroll
+        for (int c = 0; c < CHK_C; ++c) v[c] = c0 + c < w ? L.get(row, c0 + c) : mk((T)0, (T)0);
+#pragma unroll
+        for (int c = 0; c < CHK_C; ++c)
+            if (!(cabs1(v[c]) <= (T)0.5)) bad = 1;
     }
     if (__syncthreads_or(bad) && threadIdx.x == 0) atomicAdd(refuted, 1);
 }
@@ -226,7 +234,7 @@ template <class V> int block_panel(cudaStream_t st, int n, V A, int c0, int w, i
         HP_TRY(gemm(st, m2, w, w, 1.0, L21, du, 0.0, L21));
         const bool prof = prof_enabled();
         if (prof) prof_begin(st, 0.0);
-        check_multipliers_kernel<V><<<ceil_div(m2, 256), 256, 0, st>>>(L21, m2, w, wk.refuted);
+        check_multipliers_kernel<V><<<dim3(ceil_div(m2, 256), ceil_div(w, CHK_C)), 256, 0, st>>>(L21, m2, w, wk.refuted);
         if (prof) prof_end(st);
         HP_LAUNCHED();
     }

@@ -237,6 +237,29 @@ def test_mixed_refine_without_info_never_synchronises_and_reports_through_last_s
     ctx.destroy()
 
 
+@pytest.mark.parametrize("mode", [hb.HPRMAT_FP64, hb.HPRMAT_MIXED_REFINE])
+def test_graph_replay_equals_plain_launches(mode):
+    """The factorisation and the triangular solves are replayed from CUDA graphs captured on first use (HPRMAT_OPT_GRAPHS);
+    the same kernels in the same order: bit-identical R, and the replays are counted as launches."""
+    w = make_workload(2, nch=9, nb=100)
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    ctx.solve(16.25, V, mode)                                     # captures
+    l0 = hb.hprmat_launch_count()
+    R1, info1 = ctx.solve(16.25, V, mode)                         # replays
+    l1 = hb.hprmat_launch_count()
+    captured, eager = ctx.graphs()
+    assert captured >= 2 and eager == 0, (captured, eager)
+    R1 = R1.clone()
+    ctx.set_option(hb.HPRMAT_OPT_GRAPHS, 0)
+    R2, info2 = ctx.solve(16.25, V, mode)
+    l2 = hb.hprmat_launch_count()
+    assert np.array_equal(R1.cpu().numpy(), R2.cpu().numpy())
+    assert info1["refine_steps"] == info2["refine_steps"] and l1 - l0 == l2 - l1 > 100
+    ctx.destroy()
+
+
 def test_mixed_matches_fp64_mode_on_the_same_context():
     w = make_workload(2, nch=10, nb=100)
     ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=0)
