@@ -88,6 +88,11 @@ def hprmat_profile_read():
     return ms.value, fl.value, n.value
 
 
+def hprmat_profile_cgemm_variant(variant: int = -1) -> int:
+    """Select (0 auto, 1 one-tile-per-CTA, 2 persistent, 3 / 4 persistent CTA pairs with 256 x 128 / 256 x 256 tiles) or query the complex64 GEMM kernel."""
+    return int(lib().hprmat_profile_cgemm_variant(C.c_int(variant)))
+
+
 PROF_CATS = ("lu_gemm", "lu_trsm", "panel", "laswp", "solve", "other")
 
 

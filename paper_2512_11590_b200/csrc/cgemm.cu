@@ -22,6 +22,8 @@
 //
 // CTA = 6 warps: warp 0 TMA producer (one lane), warp 1 TMEM allocator + UMMA issuer (one lane), warps 2-5 epilogue
 // (each owns the TMEM lane quarter 32*(warp%4)): tcgen05.ld -> beta*C + alpha*acc -> coalesced global stores.
+#include <algorithm>
+
 #include "lu.cuh"
 #include "sm100.cuh"
 
@@ -39,7 +41,7 @@ template <int BN> struct CgCfg {
     static constexpr int A_PLANE = CG_BM * CG_KC * 4;               // bytes of one A plane per stage (16 KB)
     static constexpr int B_PLANE = BN * CG_KC * 4;                  // bytes of one B plane per stage
     static constexpr int STAGE = 2 * A_PLANE + 2 * B_PLANE;
-    static constexpr int STAGES = (BN <= 128) ? 3 : 2;
+    static constexpr int STAGES = BN <= 32 ? 5 : BN <= 64 ? 4 : BN <= 128 ? 3 : 2;
     static constexpr int SMEM = STAGES * STAGE + 1024 /* alignment slack */ + 256 /* barriers */;
     static constexpr int TMEM_COLS = 2 * BN;                        // Dr | Di
 };
@@ -201,7 +203,9 @@ EncodeTiledFn encode_fn() {
     return fn;
 }
 
-// plane: rows x cols floats, column-major with leading dimension ld; box = box_rows x box_cols
+}  // namespace
+
+// plane: rows x cols floats, column-major with leading dimension ld; box = box_rows x box_cols (shared with cgemm2.cu)
 int make_map(CUtensorMap *map, const float *plane, long rows, long cols, long ld, int box_rows, int box_cols,
              CUtensorMapSwizzle swz) {
     EncodeTiledFn fn = encode_fn();
@@ -223,6 +227,8 @@ int make_map(CUtensorMap *map, const float *plane, long rows, long cols, long ld
     }
     return 0;
 }
+
+namespace {
 
 template <int BN>
 int launch_cgemm(cudaStream_t st, int m, int n, int k, float alpha, CView A, CView B, float beta, CView C) {
@@ -246,13 +252,39 @@ int launch_cgemm(cudaStream_t st, int m, int n, int k, float alpha, CView A, CVi
 
 // C <- beta*C + alpha*A*B on split-complex float planes.  Requirements (met by every caller in lu.cu): plane base
 // addresses 16-byte aligned, leading dimensions multiples of 4 floats.
+// which kernel serves gemm(CView): 0 = automatic (the persistent kernel, CTA pairs when there is more than one M tile),
+// 1 = the one-tile-per-CTA kernel of this file, 2 = persistent single CTAs, 3 = persistent CTA pairs.  Measurement aid
+// (hprmat_profile_cgemm_variant, include/hprmat_profile.h); process-wide.
+static std::atomic<int> g_cgemm_variant{0};
+int cgemm_variant_in_force() { return g_cgemm_variant.load(std::memory_order_relaxed); }
+
 int cgemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C) {
     if (m <= 0 || n <= 0) return 0;
     if (k <= 0 && beta == 1.0) return 0;
     if (((uintptr_t)A.re | (uintptr_t)A.im | (uintptr_t)B.re | (uintptr_t)B.im) & 15) return -6;
     if ((A.ld | B.ld) & 3) return -7;
-    // 128 x 256 tiles when there are enough of them to fill the GPU: a 128 x 128 UMMA tile reads its operands from shared
-    // memory at exactly the tensor-core rate (128 B/clk), the wider tile at 3/4 of it (measured +15 % at K = 6400)
+    const int variant = cgemm_variant_in_force();
+    const long tiles128 = (long)ceil_div(m, CG_BM) * ceil_div(n, 128);
+    if (variant >= 2 || (variant == 0 && m > CG_BM && tiles128 >= 2L * kNumSMs)) {
+        // Two waves of work or more: the persistent kernel (cgemm2.cu).  Deep K and enough tiles -> pair tiles of 256 x 256
+        // (N = 256 MMAs keep the tensor pipe ~18 % busier than N = 128 ones; their un-overlapped epilogue is < 5 % of such a
+        // tile); otherwise pair tiles of 256 x 128 with double-buffered accumulators (epilogue under the next main loop).
+        // Crossover measured on B200 between k = 2048 and 3072 (profiles/r02_cgemm.md).
+        const bool deep = k >= 2560 && (long)ceil_div(m, 256) * ceil_div(n, 256) >= 4L * (kNumSMs / 2);
+        const int shape = variant == 0 ? (deep ? 2 : 1) : variant - 2;
+        return cgemm2(st, m, n, k, alpha, A, B, beta, C, shape);
+    }
+    // Less than two waves: one tile per CTA (no persistent-loop prologue, no cluster launch), with the tile NARROWED until the
+    // grid covers most of the GPU -- a 1024 x 1024 product is 8 x 8 tiles of 128 x 128 (16 % of the SMs) but 8 x 32 of
+    // 128 x 32.  C aliasing A (the in-place L21 product) needs all of n inside one tile.
+    const bool in_place_a = C.re == A.re;
+    const int natural = n <= 32 ? 32 : n <= 64 ? 64 : 128;  // narrowest tile that still holds all of n
+    int bn = natural;
+    if (variant == 0 && !in_place_a && tiles128 < 96) bn = std::min(natural, 2 * tiles128 >= 96 ? 64 : 32);
+    if (variant == 1) bn = 128;
+    if (bn == 32) return launch_cgemm<32>(st, m, n, k, (float)alpha, A, B, (float)beta, C);
+    if (bn == 64) return launch_cgemm<64>(st, m, n, k, (float)alpha, A, B, (float)beta, C);
+    // 128 x 256 tiles when there are enough of them to fill the GPU
     if (n >= 512 && (long)ceil_div(m, CG_BM) * ceil_div(n, 256) >= 2 * kNumSMs)
         return launch_cgemm<256>(st, m, n, k, (float)alpha, A, B, (float)beta, C);
     return launch_cgemm<128>(st, m, n, k, (float)alpha, A, B, (float)beta, C);
@@ -267,6 +299,11 @@ int gemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, d
 }
 
 }  // namespace hp
+
+extern "C" int hprmat_profile_cgemm_variant(int variant) {
+    if (variant >= 0 && variant <= 4) hp::g_cgemm_variant.store(variant);
+    return hp::g_cgemm_variant.load();
+}
 
 extern "C" int hprmat_cgemm_tf32(void *cuda_stream, int m, int n, int k, float alpha, const float *A_re, const float *A_im,
                                  int lda, const float *B_re, const float *B_im, int ldb, float beta, float *C_re, float *C_im,

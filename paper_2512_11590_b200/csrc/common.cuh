@@ -90,6 +90,8 @@ struct ScopedZgemmAlgo {
     ~ScopedZgemmAlgo();
 };
 
+int cgemm_variant_in_force();  // cgemm.cu (measurement aid: which tcgen05 kernel serves the planar complex64 GEMM)
+
 inline int ceil_div(long a, long b) { return (int)((a + b - 1) / b); }
 inline long round_up(long a, long b) { return (a + b - 1) / b * b; }
 

@@ -377,7 +377,8 @@ __global__ void __launch_bounds__(256) set_diag_blocks_identity_kernel(int nch, 
 // eagerly on the caller's stream, as before.
 template <class F> int replay(hprmat_ctx *c, int kind, int flags, const void *key, F &&enqueue) {
     if (!c->use_graphs || prof_enabled()) return enqueue(c->st);
-    flags |= zgemm_algo_in_force() << 16;  // the captured sequence holds the kernels of this decomposition
+    flags |= zgemm_algo_in_force() << 16;  // the captured sequence holds the kernels of this decomposition ...
+    flags |= cgemm_variant_in_force() << 20;  // ... and of this complex64 GEMM kernel
     hprmat_ctx::GraphEntry *ent = nullptr;
     for (auto &g : c->graphs)
         if (g.kind == kind && g.flags == flags && g.key == key) ent = &g;

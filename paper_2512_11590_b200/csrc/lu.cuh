@@ -19,6 +19,10 @@ constexpr int TW = 64;        // width of the block panel of a factorisation wit
 // leaf product B <- inv * B of the triangular solves (lu.cu).
 int gemm(cudaStream_t st, int m, int n, int k, double alpha, ZView A, ZView B, double beta, ZView C);
 int gemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
+// persistent tcgen05 kernel behind gemm(CView) (cgemm2.cu); shape: 0 = single CTAs (128 x 128 tiles), 1 / 2 = CTA pairs, cta_group::2 (256 x 128 / 256 x 256 tiles).  chk_count != nullptr: the
+// epilogue also counts results with |re| + |im| > chk_thr.  C may alias A when n <= 128, B when m <= 128 (pair == false).
+int cgemm2(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C, int shape, float chk_thr = 0.f,
+           int *chk_count = nullptr);
 // FP32-class accuracy variant for the planar complex64 type (3xTF32, cgemm3.cu); C may alias B when m <= 128, beta == 0
 int cgemm3(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
 int cgemm3_batched(cudaStream_t st, int m, int n, int k, double alpha, CView A, long strideA, CView B, long strideB, double beta,

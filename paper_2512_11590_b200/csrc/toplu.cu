@@ -208,6 +208,17 @@ template <class V> __global__ void __launch_bounds__(256) check_multipliers_kern
 
 }  // namespace
 
+// L21 <- L21 U11^-1 with the multiplier check fused into the GEMM's epilogue: the persistent tcgen05 kernel only
+static bool l21_checked(cudaStream_t, int, int, ZView, ZView, int *) { return false; }
+static bool l21_checked(cudaStream_t st, int m2, int w, CView L21, CView du, int *refuted) {
+    if (cgemm_variant_in_force() == 1) return false;
+    const bool prof = prof_enabled();
+    if (prof) prof_begin(st, 8.0 * m2 * w * w);
+    const int rc = cgemm2(st, m2, w, w, 1.0, L21, du, 0.0, L21, m2 > 128 ? 1 : 0, 0.5f, refuted);
+    if (prof) prof_end(st);
+    return rc == 0;
+}
+
 template <class V> int block_panel(cudaStream_t st, int n, V A, int c0, int w, int *ipiv, int *info_dev, LuWork<V> &wk, V dl, V du) {
     typedef typename V::elem_t E;
     const size_t smem = sizeof(TopLuSmem<E>);
@@ -231,6 +242,7 @@ template <class V> int block_panel(cudaStream_t st, int n, V A, int c0, int w, i
     V L21 = A.sub(c0 + w, c0);
     {
         ProfCat pc(PROF_PANEL);
+        if (l21_checked(st, m2, w, L21, du, wk.refuted)) return 0;  // complex64: the check rides in the GEMM's epilogue
         HP_TRY(gemm(st, m2, w, w, 1.0, L21, du, 0.0, L21));
         const bool prof = prof_enabled();
         if (prof) prof_begin(st, 0.0);

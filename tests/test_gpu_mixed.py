@@ -36,11 +36,20 @@ def _rup(x, q):
     return (x + q - 1) // q * q
 
 
+@pytest.fixture(params=[0, 1, 2, 3, 4], ids=["auto", "one_tile_per_cta", "persistent", "persistent_pairs", "persistent_pairs_n256"])
+def cgemm_variant(request):
+    """every tcgen05 kernel that can serve the planar complex64 GEMM (include/hprmat_profile.h)"""
+    prev = hb.hprmat_profile_cgemm_variant()
+    assert hb.hprmat_profile_cgemm_variant(request.param) == request.param
+    yield request.param
+    hb.hprmat_profile_cgemm_variant(prev)
+
+
 @pytest.mark.parametrize("m,n,k,alpha,beta", [
     (128, 128, 32, 1.0, 0.0), (128, 128, 64, -1.0, 1.0), (256, 384, 96, -1.0, 1.0), (100, 50, 37, 1.0, 0.0),
     (257, 129, 65, -1.0, 1.0), (32, 700, 32, 1.0, 0.0), (1000, 333, 200, -1.0, 1.0), (5, 3, 1, 2.0, -0.5),
-    (640, 512, 1024, -1.0, 1.0), (1, 1, 8, 1.0, 1.0)])
-def test_cgemm_tf32_matches_definition(m, n, k, alpha, beta):
+    (640, 512, 1024, -1.0, 1.0), (1, 1, 8, 1.0, 1.0), (3000, 2900, 160, -1.0, 1.0), (40000, 64, 64, 1.0, 0.0)])
+def test_cgemm_tf32_matches_definition(m, n, k, alpha, beta, cgemm_variant):
     rng = np.random.default_rng(m * 1000003 + n * 1009 + k)
     A = (rng.uniform(-1, 1, (m, k)) + 1j * rng.uniform(-1, 1, (m, k))).astype(np.complex64).astype(np.complex128)
     B = (rng.uniform(-1, 1, (k, n)) + 1j * rng.uniform(-1, 1, (k, n))).astype(np.complex64).astype(np.complex128)
@@ -62,7 +71,7 @@ def test_cgemm_tf32_matches_definition(m, n, k, alpha, beta):
     assert float(Cr[:, m:].abs().max()) == 0.0 and float(Ci[:, m:].abs().max()) == 0.0
 
 
-def test_cgemm_tf32_is_exact_on_tf32_representable_integers():
+def test_cgemm_tf32_is_exact_on_tf32_representable_integers(cgemm_variant):
     """Small integers are exact in TF32 and their dot products exact in FP32: the result must equal the definition
     bit for bit -- pins the operand layouts / descriptors (a transposed or mis-swizzled tile cannot pass)."""
     m, n, k = 384, 256, 160
