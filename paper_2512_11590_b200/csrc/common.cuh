@@ -164,6 +164,17 @@ template <class E> __device__ __forceinline__ E crecip(E a) {
 // 1/a by Smith's formula on the reciprocal intrinsics (two dependent reciprocals, no IEEE-division slow paths)
 __device__ __forceinline__ float rcp_rn(float x) { return __frcp_rn(x); }
 __device__ __forceinline__ double rcp_rn(double x) { return __drcp_rn(x); }
+// approximate reciprocal (to be refined by Newton steps)
+__device__ __forceinline__ float rcp_approx(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ double rcp_approx(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    return r;
+}
 template <class E> __device__ __forceinline__ E crecip_fast(E a) {
     typedef typename real_of<E>::type T;
     if (fabs(a.x) >= fabs(a.y)) {
@@ -174,6 +185,41 @@ template <class E> __device__ __forceinline__ E crecip_fast(E a) {
         return mk(r * id, -id);
     }
 }
+
+// Packed FP32 pairs (Blackwell FFMA2: one instruction, two lanes): complex64 arithmetic at half the FP32 issue count.
+// a - b*c  and  a*b  for float2, same rounding as the scalar forms up to the fused multiply-adds.
+__device__ __forceinline__ unsigned long long f2_pack(float lo, float hi) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ float2 f2_unpack(unsigned long long v) {
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+__device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsigned long long b, unsigned long long c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ unsigned long long f2_mul(unsigned long long a, unsigned long long b) {
+    unsigned long long d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ float2 cfnma_packed(float2 a, float2 b, float2 c) {
+    unsigned long long acc = f2_fma(f2_pack(-b.x, -b.x), f2_pack(c.x, c.y), f2_pack(a.x, a.y));
+    acc = f2_fma(f2_pack(b.y, -b.y), f2_pack(c.y, c.x), acc);
+    return f2_unpack(acc);
+}
+__device__ __forceinline__ double2 cfnma_packed(double2 a, double2 b, double2 c) { return cfnma(a, b, c); }
+__device__ __forceinline__ float2 cmul_packed(float2 a, float2 b) {
+    unsigned long long acc = f2_mul(f2_pack(a.x, a.x), f2_pack(b.x, b.y));
+    acc = f2_fma(f2_pack(-a.y, a.y), f2_pack(b.y, b.x), acc);
+    return f2_unpack(acc);
+}
+__device__ __forceinline__ double2 cmul_packed(double2 a, double2 b) { return cmul(a, b); }
 
 // compile-time loop: f(IntC<I>) for I = B .. E-1 (keeps register-resident tiles statically indexed)
 template <int I> struct IntC { static constexpr int value = I; };

@@ -20,172 +20,158 @@ namespace hp {
 
 namespace {
 
-constexpr int TL_NT = 256;   // 16 x 16 threads; thread (ti, tj) owns the elements (ti + 16 a, tj + 16 b), a, b = 0..3
+constexpr int TL_G = 256;         // threads of one role: 16 x 16, thread (ti, tj) owns the elements (ti + 16 a, tj + 16 b)
+constexpr int TL_NT = 2 * TL_G;   // two roles advance together, one barrier per column: the factorisation | both inversions
 constexpr int TL_R = TW / 16;
 
+// What crosses the roles, double-buffered by column parity
 template <class E> struct TopLuSmem {
-    E tile[TW * TW];         // column-major, ld = TW: the factored top block
-    E rowb[2][2][TW];        // [which sweep][parity][col]: the row every thread needs in a step
-    E colb[2][TW];           // [parity][row]: column j of the LU sweep
-    E invp[TW];              // 1 / u_jj (0 for a zero pivot), published by the owner of the diagonal element
+    E colb[2][TW];   // column j of the partly eliminated block, rows <= j zeroed  (LU role -> LU, XL)
+    E rowb[2][TW];   // row j of U, columns <= j zeroed                           (LU role -> LU, Y)
+    E xlrow[2][TW];  // row j of XL = inv(L)                                       (XL role -> XL)
+    E yrow[2][TW];   // row j of Y = inv(U)^T, not yet scaled by 1/u_jj            (Y role -> Y)
+    E invp[TW];      // the pivots u_jj, from the owner of the diagonal element
 };
 
+// One CTA factors the w x w block (w <= TW, padded to TW x TW by the identity) WITHOUT interchanges and inverts both
+// triangular factors, all out of registers: two groups of 256 threads run three rank-1 sweeps in lock step (the
+// factorisation in one group, both inversions in the other),
+//   LU:  step j: l_i = a_ij / u_jj (i > j),  a_ic -= l_i u_jc (i, c > j)
+//   XL = inv(L):     rows i > j:  XL[i,:] -= l_i XL[j,:]                (row j of XL is final when step j starts)
+//   Y  = inv(U)^T = inv(U^T), U^T lower triangular with diagonal u_jj:
+//                    Y[j,:] /= u_jj;  rows i > j:  Y[i,:] -= u_ji Y[j,:]   (u_ji = U[j,i]: row j of U, final at step j)
+// Column j of L and row j of U are exactly what the LU role publishes at step j, so the two inversions ride one step
+// behind the factorisation for free: TW barriers in all instead of 2 TW.
 template <class V>
 __global__ void __launch_bounds__(TL_NT, 1)
     top_lu_kernel(V A, int w, int c0, int *ipiv, int *info, int *refuted, V dinvL, V dinvU, int *perm, int nbatch) {
     typedef typename V::elem_t E;
     typedef typename V::real_t T;
-    extern __shared__ __align__(16) unsigned char smraw[];
-    TopLuSmem<E> &sm = *reinterpret_cast<TopLuSmem<E> *>(smraw);
-    const int tid = threadIdx.x, ti = tid & 15, tj = tid >> 4;
+    __shared__ TopLuSmem<E> sm;
+    const int role = threadIdx.x / TL_G, lt = threadIdx.x % TL_G, ti = lt & 15, tj = lt >> 4;
     const E zero = mk((T)0, (T)0), one = mk((T)1, (T)0);
 
-    // ---- the block, padded to TW x TW by the identity, in registers
-    E x[TL_R][TL_R];
+    // LU role: x = the block.  Inversion role: x = XL, y = Y, both start as the identity
+    E x[TL_R][TL_R], y[TL_R][TL_R];
 #pragma unroll
     for (int a = 0; a < TL_R; ++a)
 #pragma unroll
         for (int b = 0; b < TL_R; ++b) {
             const int row = ti + 16 * a, col = tj + 16 * b;
-            x[a][b] = (row < w && col < w) ? A.get(row, col) : (row == col ? one : zero);
+            x[a][b] = (role == 0 && row < w && col < w) ? A.get(row, col) : (row == col ? one : zero);
+            y[a][b] = row == col ? one : zero;
         }
     int bad = 0;
-    // ---- LU without interchanges, one rank-1 update per step; JB = j / 16 is compile-time so that the register tile is
-    //      statically indexed; rows / columns of tile index < JB are finished
+    // JB = j / 16 is compile-time so that the register tiles are statically indexed
     static_for<0, TL_R>([&](auto jbc) {
         constexpr int JB = decltype(jbc)::value;
 #pragma unroll 1
         for (int jj = 0; jj < 16; ++jj) {
             const int j = 16 * JB + jj, par = j & 1;
-            if (ti == jj) {
+            // ---- publish (owners only)
+            if (role == 0) {
+                if (ti == jj) {  // row j of U; finished columns read as zero
 #pragma unroll
-                for (int b = JB; b < TL_R; ++b) sm.rowb[0][par][tj + 16 * b] = x[JB][b];
-            }
-            if (tj == jj) {
+                    for (int b = JB; b < TL_R; ++b) sm.rowb[par][tj + 16 * b] = (tj + 16 * b > j) ? x[JB][b] : zero;
+                }
+                if (tj == jj) {  // column j, not yet divided by the pivot; finished rows read as zero
 #pragma unroll
-                for (int a = JB; a < TL_R; ++a) sm.colb[par][ti + 16 * a] = x[a][JB];
-                if (ti == jj) {  // the pivot's owner inverts it once for everybody (the long-latency part of the step)
-                    const E pv = x[JB][JB];
-                    const bool sing = (pv.x == (T)0 && pv.y == (T)0);
-                    sm.invp[j] = sing ? zero : crecip_fast(pv);
-                    if (sing) {
-                        atomicCAS(info, 0, c0 + j + 1);
-                        bad = 1;
+                    for (int a = JB; a < TL_R; ++a) sm.colb[par][ti + 16 * a] = (ti + 16 * a > j) ? x[a][JB] : zero;
+                    if (ti == jj) {  // the pivot itself: every thread inverts it on its own (no serial step behind one thread)
+                        const E pv = x[JB][JB];
+                        sm.invp[j] = pv;
+                        if (pv.x == (T)0 && pv.y == (T)0) {
+                            atomicCAS(info, 0, c0 + j + 1);
+                            bad = 1;
+                        }
                     }
                 }
-            }
-            __syncthreads();
-            const E ip = sm.invp[j];
-            E l[TL_R], u[TL_R];
+            } else if (ti == jj) {  // rows j of XL and of Y: non-zero in columns <= j only
 #pragma unroll
-            for (int a = JB; a < TL_R; ++a) {
-                const int row = ti + 16 * a;
-                l[a] = row > j ? cmul(sm.colb[par][row], ip) : zero;
-                if (!(cabs1(l[a]) <= (T)0.5)) bad = 1;  // also catches NaN
-            }
-#pragma unroll
-            for (int b = JB; b < TL_R; ++b) {
-                const int col = tj + 16 * b;
-                u[b] = col > j ? sm.rowb[0][par][col] : zero;
-            }
-#pragma unroll
-            for (int a = JB; a < TL_R; ++a)
-#pragma unroll
-                for (int b = JB; b < TL_R; ++b) x[a][b] = cfnma(x[a][b], l[a], u[b]);
-            if (tj == jj) {
-#pragma unroll
-                for (int a = JB; a < TL_R; ++a)
-                    if (ti + 16 * a > j) x[a][JB] = l[a];
-            }
-        }
-    });
-    // ---- factored block to shared memory (operand of the two inversion sweeps) and back to the matrix
-#pragma unroll
-    for (int a = 0; a < TL_R; ++a)
-#pragma unroll
-        for (int b = 0; b < TL_R; ++b) {
-            const int row = ti + 16 * a, col = tj + 16 * b;
-            sm.tile[col * TW + row] = x[a][b];
-            if (row < w && col < w) A.set(row, col, x[a][b]);
-        }
-    if (tid < w) ipiv[c0 + tid] = c0 + tid + 1;      // identity interchanges
-    if (tid < nbatch) perm[(size_t)tid * PERM_STRIDE] = 0;  // empty swap batches
-    if (__syncthreads_or(bad) && tid == 0) atomicAdd(refuted, 1);
-
-    // ---- inverses of the unit-lower triangle L and of the upper triangle U, both by rank-1 sweeps on the identity:
-    //        XL: for j ascending:   rows i > j:  XL[i,:] -= L[i,j] XL[j,:]      (row j is final when it is used)
-    //        XU: for j descending:  XU[j,:] /= u_jj;  rows i < j:  XU[i,:] -= U[i,j] XU[j,:]
-    //      Step s does column j = s of L and column j = TW-1-s of U, so that one barrier serves both.
-    E xl[TL_R][TL_R], xu[TL_R][TL_R];
-#pragma unroll
-    for (int a = 0; a < TL_R; ++a)
-#pragma unroll
-        for (int b = 0; b < TL_R; ++b) xl[a][b] = xu[a][b] = (ti + 16 * a == tj + 16 * b) ? one : zero;
-    static_for<0, TL_R>([&](auto jbc) {
-        constexpr int JB = decltype(jbc)::value;  // block of the L column; the U column is in block TL_R-1-JB
-        constexpr int UB = TL_R - 1 - JB;
-#pragma unroll 1
-        for (int jj = 0; jj < 16; ++jj) {
-            const int jl = 16 * JB + jj, ju = TW - 1 - jl, par = jj & 1;
-            if (ti == jj) {  // row jl of XL: non-zero in columns <= jl
-#pragma unroll
-                for (int b = 0; b <= JB; ++b) sm.rowb[0][par][tj + 16 * b] = xl[JB][b];
-            }
-            if (ti == 15 - jj) {  // row ju of XU, scaled by 1/u_jj: non-zero in columns >= ju
-                const E ipu = sm.invp[ju];
-#pragma unroll
-                for (int b = UB; b < TL_R; ++b) {
-                    xu[UB][b] = cmul(xu[UB][b], ipu);
-                    sm.rowb[1][par][tj + 16 * b] = xu[UB][b];
+                for (int b = 0; b <= JB; ++b) {
+                    sm.xlrow[par][tj + 16 * b] = x[JB][b];
+                    sm.yrow[par][tj + 16 * b] = y[JB][b];
                 }
             }
             __syncthreads();
+            // 1 / u_jj = conj(u_jj) / |u_jj|^2: the entries of these blocks are O(1) (S = I + coupling-sized terms), so the
+            // squared modulus cannot overflow; one reciprocal + one Newton step, identical in every thread
+            E ip;
             {
-                E l[TL_R], r[TL_R];
+                const E pv = sm.invp[j];
+                const T den = pv.x * pv.x + pv.y * pv.y;
+                T r = den > (T)0 ? rcp_approx(den) : (T)0;
+                r = r * ((T)2 - den * r);
+                r = r * ((T)2 - den * r);
+                ip = mk(pv.x * r, -pv.y * r);
+            }
+            if (role == 0) {
+                E l[TL_R], u[TL_R];
+#pragma unroll
+                for (int a = JB; a < TL_R; ++a) l[a] = cmul_packed(sm.colb[par][ti + 16 * a], ip);
+#pragma unroll
+                for (int b = JB; b < TL_R; ++b) u[b] = sm.rowb[par][tj + 16 * b];
+#pragma unroll
+                for (int a = JB; a < TL_R; ++a)
+#pragma unroll
+                    for (int b = JB; b < TL_R; ++b) x[a][b] = cfnma_packed(x[a][b], l[a], u[b]);
+                if (tj == jj) {  // keep the multipliers
+#pragma unroll
+                    for (int a = JB; a < TL_R; ++a)
+                        if (ti + 16 * a > j) x[a][JB] = l[a];
+                }
+            } else {
+                // rows i > j:  XL[i,:] -= l_i XL[j,:]  and  Y[i,:] -= u_ji (Y[j,:] / u_jj);  Y's row j takes its 1/u_jj
+                E la[TL_R], ua[TL_R], xr[TL_R], yr[TL_R];
 #pragma unroll
                 for (int a = JB; a < TL_R; ++a) {
-                    const int row = ti + 16 * a;
-                    l[a] = row > jl ? sm.tile[jl * TW + row] : zero;
+                    la[a] = cmul_packed(sm.colb[par][ti + 16 * a], ip);
+                    ua[a] = sm.rowb[par][ti + 16 * a];
                 }
 #pragma unroll
                 for (int b = 0; b <= JB; ++b) {
-                    const int col = tj + 16 * b;
-                    r[b] = col <= jl ? sm.rowb[0][par][col] : zero;
+                    xr[b] = sm.xlrow[par][tj + 16 * b];
+                    yr[b] = cmul_packed(sm.yrow[par][tj + 16 * b], ip);
                 }
 #pragma unroll
                 for (int a = JB; a < TL_R; ++a)
 #pragma unroll
-                    for (int b = 0; b <= JB; ++b) xl[a][b] = cfnma(xl[a][b], l[a], r[b]);
-            }
-            {
-                E uu[TL_R], r[TL_R];
+                    for (int b = 0; b <= JB; ++b) {
+                        x[a][b] = cfnma_packed(x[a][b], la[a], xr[b]);
+                        y[a][b] = cfnma_packed(y[a][b], ua[a], yr[b]);
+                    }
+                if (ti == jj) {
 #pragma unroll
-                for (int a = 0; a <= UB; ++a) {
-                    const int row = ti + 16 * a;
-                    uu[a] = row < ju ? sm.tile[ju * TW + row] : zero;
+                    for (int b = 0; b <= JB; ++b) y[JB][b] = yr[b];
                 }
-#pragma unroll
-                for (int b = UB; b < TL_R; ++b) {
-                    const int col = tj + 16 * b;
-                    r[b] = col >= ju ? sm.rowb[1][par][col] : zero;
-                }
-#pragma unroll
-                for (int a = 0; a <= UB; ++a)
-#pragma unroll
-                    for (int b = UB; b < TL_R; ++b) xu[a][b] = cfnma(xu[a][b], uu[a], r[b]);
             }
         }
     });
+    // ---- results
+    if (role == 0) {
 #pragma unroll
-    for (int a = 0; a < TL_R; ++a)
+        for (int a = 0; a < TL_R; ++a)
 #pragma unroll
-        for (int b = 0; b < TL_R; ++b) {
-            const int row = ti + 16 * a, col = tj + 16 * b;
-            if (row < w && col < w) {
-                dinvL.set(row, col, xl[a][b]);
-                dinvU.set(row, col, xu[a][b]);
+            for (int b = 0; b < TL_R; ++b) {
+                const int row = ti + 16 * a, col = tj + 16 * b;
+                if (row > col && !(cabs1(x[a][b]) <= (T)0.5)) bad = 1;  // every multiplier, once; also catches NaN
+                if (row < w && col < w) A.set(row, col, x[a][b]);
             }
-        }
+        if (lt < w) ipiv[c0 + lt] = c0 + lt + 1;              // identity interchanges
+        if (lt < nbatch) perm[(size_t)lt * PERM_STRIDE] = 0;  // empty swap batches
+    } else {
+#pragma unroll
+        for (int a = 0; a < TL_R; ++a)
+#pragma unroll
+            for (int b = 0; b < TL_R; ++b) {
+                const int row = ti + 16 * a, col = tj + 16 * b;
+                if (row < w && col < w) {
+                    dinvL.set(row, col, x[a][b]);
+                    dinvU.set(col, row, y[a][b]);  // inv(U) = Y^T
+                }
+            }
+    }
+    if (__syncthreads_or(bad) && threadIdx.x == 0) atomicAdd(refuted, 1);
 }
 
 // counts the multipliers of L (m x w) that violate |l|_1 <= 1/2 (or are NaN): CTA = 256 rows x CHK_C columns
@@ -221,16 +207,13 @@ static bool l21_checked(cudaStream_t st, int m2, int w, CView L21, CView du, int
 
 template <class V> int block_panel(cudaStream_t st, int n, V A, int c0, int w, int *ipiv, int *info_dev, LuWork<V> &wk, V dl, V du) {
     typedef typename V::elem_t E;
-    const size_t smem = sizeof(TopLuSmem<E>);
     auto kern = top_lu_kernel<V>;
-    static SmemCfg cfg;
-    HP_TRY(configure_smem(cfg, kern, smem));
     const int b0 = c0 / IB, nbatch = ceil_div(w, IB);
     {
         ProfCat pc(PROF_PANEL);
         const bool prof = prof_enabled();
         if (prof) prof_begin(st, 0.0);
-        kern<<<1, TL_NT, smem, st>>>(A.sub(c0, c0), w, c0, ipiv, info_dev, wk.refuted, dl, du, wk.perm + (size_t)b0 * PERM_STRIDE,
+        kern<<<1, TL_NT, 0, st>>>(A.sub(c0, c0), w, c0, ipiv, info_dev, wk.refuted, dl, du, wk.perm + (size_t)b0 * PERM_STRIDE,
                                      nbatch);
         if (prof) prof_end(st);
         HP_LAUNCHED();
