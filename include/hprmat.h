@@ -45,7 +45,12 @@ typedef struct hprmat_ctx hprmat_ctx; /* opaque */
 enum {
     HPRMAT_FP64 = 1,         /* FP64 LU of C - E*I on FP64 tensor cores (+ refinement with a compensated residual)     */
     HPRMAT_MIXED = 2,        /* low-precision (complex64 storage, TF32 tensor-core update) LU, NO refinement            */
-    HPRMAT_MIXED_REFINE = 3  /* low-precision LU + FP64 residual / iterative refinement to double accuracy            */
+    HPRMAT_MIXED_REFINE = 3, /* low-precision LU + FP64 residual / iterative refinement to double accuracy            */
+    HPRMAT_TYPE3 = 4         /* the paper's Type 3 as printed (Eqs. 7-9; local potentials only): the     */
+                             /* point-major Schur matrix I + K^-1 V with the REAL kinetic block K shared by all channels   */
+                             /* (its inverse and K^-1 q2 are energy-independent: computed once at hprmat_setup and reused   */
+                             /* across the scan), complex64 LU with partial pivoting and FP32-class (3xTF32) products, no   */
+                             /* refinement: ~1e-6 in R, the accuracy the paper quotes for Type 3             */
 };
 
 /* status codes */
@@ -79,7 +84,7 @@ typedef struct {
  *   a      channel radius, fm;  h2m = hbar^2/2mu, MeV fm^2 (equal reduced mass in all channels)
  *   lval   host, int[nch]: orbital momenta l_c;  ethr  host, double[nch]: thresholds E_c, MeV (enter as +E_c on the
  *          diagonal of Eq. 1)
- *   max_mode  bitwise OR of (1 << HPRMAT_FP64), (1 << HPRMAT_MIXED), (1 << HPRMAT_MIXED_REFINE): sizes the buffers
+ *   max_mode  bitwise OR of (1 << HPRMAT_FP64), (1 << HPRMAT_MIXED), (1 << HPRMAT_MIXED_REFINE), (1 << HPRMAT_TYPE3): sizes the buffers
  *          (FP64: 16 N^2 bytes; mixed: 8 N^2 bytes; plus O(N nch)).  0 means all modes.
  *   cuda_stream  a cudaStream_t (may be NULL = default stream)
  * Computes the mesh, f_i(a) and the kinetic + Bloch table on the host in long double and uploads them. */
@@ -92,7 +97,7 @@ int hprmat_mesh(const hprmat_ctx *ctx, double *r, double *fa);
 
 /* One energy point: assemble, factorise, solve, (refine), contract.
  *   V    dev, complex [nbasis][nch][nch]: V[(i*nch + c2)*nch + c1] = V_{c1 c2}(r_i), MeV (Eq. 4)
- *   mode one of HPRMAT_FP64 / HPRMAT_MIXED / HPRMAT_MIXED_REFINE (must be inside max_mode)
+ *   mode one of HPRMAT_FP64 / HPRMAT_MIXED / HPRMAT_MIXED_REFINE / HPRMAT_TYPE3 (must be inside max_mode)
  *   max_refine  maximum refinement steps; <0 = default (2 for FP64, 5 for MIXED_REFINE)
  *   tol  refinement stops when the estimated relative error left in X (correction norm x observed contraction, DESIGN.md
  *        reading R9) is <= tol; <=0 = default: 1e-13 in FP64 mode, 1e-12 in the mixed modes

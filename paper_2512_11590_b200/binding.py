@@ -13,10 +13,10 @@ import torch
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIBPATH = os.path.join(HERE, "libhprmat.so")
 
-HPRMAT_FP64, HPRMAT_MIXED, HPRMAT_MIXED_REFINE = 1, 2, 3
+HPRMAT_FP64, HPRMAT_MIXED, HPRMAT_MIXED_REFINE, HPRMAT_TYPE3 = 1, 2, 3, 4
 HPRMAT_OK, HPRMAT_ESINGULAR, HPRMAT_ENOTCONVERGED, HPRMAT_ENOMEM, HPRMAT_ECUDA, HPRMAT_EUNVERIFIED = 0, 1, 2, 3, 4, 5
 HPRMAT_OPT_FP64_ALGO, HPRMAT_OPT_ZGEMM_ALGO, HPRMAT_OPT_GRAPHS = 1, 2, 3
-MODES = {"fp64": HPRMAT_FP64, "mixed": HPRMAT_MIXED, "mixed_refine": HPRMAT_MIXED_REFINE}
+MODES = {"fp64": HPRMAT_FP64, "mixed": HPRMAT_MIXED, "mixed_refine": HPRMAT_MIXED_REFINE, "type3": HPRMAT_TYPE3}
 
 
 class hprmat_info(C.Structure):

@@ -31,6 +31,7 @@ struct hprmat_ctx {
     std::vector<double> r, fa;  // host copies for hprmat_mesh
     // device
     double *d_hT = nullptr, *d_dg0 = nullptr, *d_ethr = nullptr, *d_fa = nullptr;
+    double *d_KTinv = nullptr, *d_cf = nullptr, *d_g = nullptr;  // Type 3: (h2m T)^-1, centrifugal terms, (h2m T)^-1 q2
     double2 *d_C = nullptr;                                   // N x N complex128 (FP64 mode)
     double2 *d_X = nullptr, *d_Rr = nullptr, *d_Rlo = nullptr;  // N x nch each
     double2 *d_V = nullptr, *d_R = nullptr;                   // staging for hprmat_solve_host
@@ -57,7 +58,7 @@ struct hprmat_ctx {
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     // refinement steps the last solve in each mode took: that many are enqueued before the single read-back of the next
     // solve (index: HPRMAT_FP64 .. HPRMAT_MIXED_REFINE)
-    int plan_steps[4] = {0, 1, 0, 2};
+    int plan_steps[5] = {0, 1, 0, 2, 0};
     // what the last solve was, for hprmat_last_status
     int last_fac = -1, last_mode = 0, last_max_refine = 0;
     bool last_valid = false;
@@ -114,6 +115,7 @@ void shifted_legendre_zeros(int n, std::vector<ld> &x) {
 
 int free_ctx(hprmat_ctx *c) {
     if (!c) return 0;
+    cudaFree(c->d_KTinv); cudaFree(c->d_cf); cudaFree(c->d_g);
     cudaFree(c->d_hT); cudaFree(c->d_dg0); cudaFree(c->d_ethr); cudaFree(c->d_fa);
     cudaFree(c->d_Voff); cudaFree(c->d_Xp); cudaFree(c->d_Pp);
     cudaFree(c->d_C); cudaFree(c->d_X); cudaFree(c->d_Rr); cudaFree(c->d_Rlo); cudaFree(c->d_V); cudaFree(c->d_R);
@@ -159,7 +161,7 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
     if (!lval) return -6;
     if (!ethr) return -7;
     if ((long)nch * nbasis > 2000000000L / 16) return -2;
-    const int all = (1 << HPRMAT_FP64) | (1 << HPRMAT_MIXED) | (1 << HPRMAT_MIXED_REFINE);
+    const int all = (1 << HPRMAT_FP64) | (1 << HPRMAT_MIXED) | (1 << HPRMAT_MIXED_REFINE) | (1 << HPRMAT_TYPE3);
     if (max_mode == 0) max_mode = all;
     if (max_mode & ~all) return -8;
     int ndev = 0;
@@ -210,6 +212,51 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
             dg0[(size_t)ch * nb + i] = hT[(size_t)i * nb + i] + cf;
         }
 
+    // ---- Type 3: the kinetic block K = h2m T is real, shared by all channels and ENERGY-INDEPENDENT, so its
+    //      inverse (step 1 of the paper's algorithm; Gauss-Jordan with partial pivoting in long double here), the
+    //      transformed surface vector K^-1 q2 of Eq. (9) and the centrifugal terms are computed once per context
+    std::vector<double> KTinv, cfv, gv;
+    if (max_mode & (1 << HPRMAT_TYPE3)) {
+        std::vector<ld> aug((size_t)nb * 2 * nb);
+        for (int i = 0; i < nb; ++i)
+            for (int j = 0; j < nb; ++j) {
+                aug[(size_t)i * 2 * nb + j] = (ld)hT[(size_t)j * nb + i];
+                aug[(size_t)i * 2 * nb + nb + j] = i == j ? 1.0L : 0.0L;
+            }
+        for (int k = 0; k < nb; ++k) {
+            int piv = k;
+            for (int i = k + 1; i < nb; ++i)
+                if (fabsl(aug[(size_t)i * 2 * nb + k]) > fabsl(aug[(size_t)piv * 2 * nb + k])) piv = i;
+            if (piv != k)
+                for (int j = 0; j < 2 * nb; ++j) std::swap(aug[(size_t)k * 2 * nb + j], aug[(size_t)piv * 2 * nb + j]);
+            const ld d = aug[(size_t)k * 2 * nb + k];
+            if (d == 0.0L) { free_ctx(c); return -3; }  // cannot happen: T is positive definite
+            for (int j = 0; j < 2 * nb; ++j) aug[(size_t)k * 2 * nb + j] /= d;
+            for (int i = 0; i < nb; ++i) {
+                if (i == k) continue;
+                const ld f = aug[(size_t)i * 2 * nb + k];
+                if (f == 0.0L) continue;
+                for (int j = 0; j < 2 * nb; ++j) aug[(size_t)i * 2 * nb + j] -= f * aug[(size_t)k * 2 * nb + j];
+            }
+        }
+        KTinv.resize((size_t)nb * nb);
+        gv.assign(nb, 0.0);
+        for (int i = 0; i < nb; ++i) {
+            ld g = 0.0L;
+            for (int j = 0; j < nb; ++j) {
+                KTinv[(size_t)j * nb + i] = (double)aug[(size_t)i * 2 * nb + nb + j];
+                g += aug[(size_t)i * 2 * nb + nb + j] * (ld)c->fa[j];
+            }
+            gv[i] = (double)g;
+        }
+        cfv.resize((size_t)N);
+        for (int ch = 0; ch < nch; ++ch)
+            for (int i = 0; i < nb; ++i) {
+                const double l = lval[ch];
+                cfv[(size_t)ch * nb + i] = h2m * l * (l + 1) / (c->r[i] * c->r[i]);
+            }
+    }
+
     // ---- device buffers
     HP_ALLOC(c->d_hT, sizeof(double) * nb * nb);
     HP_ALLOC(c->d_dg0, sizeof(double) * N);
@@ -222,7 +269,7 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
         c->wz.carve(c->d_work, (int)N);
         HP_ALLOC(c->d_Kinv, sizeof(double2) * (size_t)nch * nb * nb);
     }
-    if (max_mode & ((1 << HPRMAT_MIXED) | (1 << HPRMAT_MIXED_REFINE))) {
+    if (max_mode & ((1 << HPRMAT_MIXED) | (1 << HPRMAT_MIXED_REFINE) | (1 << HPRMAT_TYPE3))) {
         c->ldS = round_up(N, 32);
         HP_ALLOC(c->d_Sre, sizeof(float) * c->ldS * N);
         HP_ALLOC(c->d_Sim, sizeof(float) * c->ldS * N);
@@ -278,6 +325,16 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
     cudaError_t e2 = cudaMemcpyAsync(c->d_dg0, dg0.data(), sizeof(double) * N, cudaMemcpyHostToDevice, c->st);
     cudaError_t e3 = cudaMemcpyAsync(c->d_ethr, ethr, sizeof(double) * nch, cudaMemcpyHostToDevice, c->st);
     cudaError_t e4 = cudaMemcpyAsync(c->d_fa, c->fa.data(), sizeof(double) * nb, cudaMemcpyHostToDevice, c->st);
+    if (max_mode & (1 << HPRMAT_TYPE3)) {
+        HP_ALLOC(c->d_KTinv, sizeof(double) * nb * nb);
+        HP_ALLOC(c->d_cf, sizeof(double) * N);
+        HP_ALLOC(c->d_g, sizeof(double) * nb);
+        cudaError_t t1 = cudaMemcpyAsync(c->d_KTinv, KTinv.data(), sizeof(double) * nb * nb, cudaMemcpyHostToDevice, c->st);
+        cudaError_t t2 = cudaMemcpyAsync(c->d_cf, cfv.data(), sizeof(double) * N, cudaMemcpyHostToDevice, c->st);
+        cudaError_t t3 = cudaMemcpyAsync(c->d_g, gv.data(), sizeof(double) * nb, cudaMemcpyHostToDevice, c->st);
+        for (cudaError_t e : {t1, t2, t3})
+            if (e != cudaSuccess) { free_ctx(c); return hp::cuda_fail(e, __FILE__, __LINE__); }
+    }
     cudaError_t e5 = cudaStreamSynchronize(c->st);  // the host vectors go out of scope
     for (cudaError_t e : {e1, e2, e3, e4, e5})
         if (e != cudaSuccess) { free_ctx(c); return hp::cuda_fail(e, __FILE__, __LINE__); }
@@ -324,12 +381,15 @@ extern "C" int hprmat_get_x(const hprmat_ctx *ctx, void *X) {
 //     FAC_C_Z   C - E I itself, FP64 LU with partial pivoting               (the paper's Type 1)
 //     FAC_S_Z   S = K_d^-1 (C - E I) in FP64, verified diagonal pivots      (the matrix of the paper's Type 3, Eqs. 7-9)
 //     FAC_S_C   S in planar complex64, TF32 tensor-core trailing update     (Types 2/4)
+//     FAC_T3    the paper's Type 3 LITERALLY (Eqs. 7-9): point-major Schur matrix I + K^-1 V with the real, shared,
+//               energy-independent kinetic block K; complex64 LU with partial pivoting and FP32-class (3xTF32) products
+//               (kappa(S) ~ 1e5: single-pass TF32 would cost 1e-3 ... 1e-2 in R); no refinement
 //   whether non-convergence of the refinement is an error (mixed+refine) or the rounding floor (FP64).
 // Residual, stopping rule and reported backward error always refer to the ORIGINAL system (C - E I) X = B.
 // ======================================================================================================================
 namespace {
 
-enum Fac { FAC_C_Z = 0, FAC_S_Z = 1, FAC_S_C = 2 };
+enum Fac { FAC_C_Z = 0, FAC_S_Z = 1, FAC_S_C = 2, FAC_T3 = 3 };
 constexpr int UNUSABLE = -1000;  // internal: the verified-diagonal factorisation cannot be trusted here (refuted pivots,
                                  // singular diagonal block, ill-conditioned preconditioner): factor with pivoting instead
 
@@ -418,7 +478,9 @@ int assemble(hprmat_ctx *c, Fac fac, const Problem &p, double energy, bool want_
     HP_CUDA(cudaMemsetAsync(c->d_info, 0, sizeof(int) * IN_NWORDS, st));
     if (p.W) HP_CUDA(cudaMemsetAsync(c->d_V, 0, sizeof(double2) * (size_t)nb * nch * nch, st));  // "no local potential"
     else HP_TRY(coupling_without_diagonal(st, c->tab, p.V, c->d_Voff));  // operand of the residual's tensor-core part
-    if (fac == FAC_C_Z) {
+    if (fac == FAC_T3) {
+        HP_TRY(type3_assemble(st, c->tab, c->d_KTinv, c->d_cf, energy, p.V, CView(c->d_Sre, c->d_Sim, c->ldS)));
+    } else if (fac == FAC_C_Z) {
         if (p.W) HP_TRY(assemble_nonlocal(st, c->tab, energy, p.W, p.ldw, c->d_C, N));
         else HP_TRY(assemble_z(st, c->tab, energy, p.V, c->d_C, N));
     } else {
@@ -447,6 +509,15 @@ int factor(hprmat_ctx *c, Fac fac, bool pivoting_fallback) {
     const int N = c->n;
     int *zp = c->d_info + IN_ZERO_PIVOT;
     (void)st;
+    if (fac == FAC_T3) {
+        c->wc.speculate = false;
+        c->wc.accurate = true;
+        const int rc = replay(c, 0, 8, nullptr, [&](cudaStream_t s) {
+            return getrf<CView>(s, N, CView(c->d_Sre, c->d_Sim, c->ldS), c->d_ipiv, zp, c->wc);
+        });
+        c->wc.accurate = false;
+        return rc;
+    }
     if (fac == FAC_S_C) {
         c->wc.speculate = !pivoting_fallback;
         return replay(c, 0, 4 + (pivoting_fallback ? 1 : 0), nullptr, [&](cudaStream_t s) {
@@ -462,6 +533,17 @@ int factor(hprmat_ctx *c, Fac fac, bool pivoting_fallback) {
 int first_solve(hprmat_ctx *c, Fac fac, int *x0_word) {
     cudaStream_t st = c->st;
     const int N = c->n, nch = c->nch;
+    if (fac == FAC_T3) {
+        CView S(c->d_Sre, c->d_Sim, c->ldS), Bs(c->d_Bre, c->d_Bim, c->ldS);
+        HP_TRY(type3_rhs(st, c->tab, c->d_g, Bs));
+        c->wc.accurate = true;
+        const int rc = getrs_replay<CView>(c, nch, S, Bs, c->wc, Bs.re, 2);
+        c->wc.accurate = false;
+        HP_TRY(rc);
+        HP_TRY(type3_promote(st, c->tab, Bs, c->d_X, N, c->d_scal + SC_DN));
+        *x0_word = SC_XN;
+        return 0;
+    }
     if (fac == FAC_S_C) {
         CView S(c->d_Sre, c->d_Sim, c->ldS), Bs(c->d_Bre, c->d_Bim, c->ldS);
         HP_TRY(precond_rhs(st, c->tab, c->d_Kinv, Bs));
@@ -546,7 +628,7 @@ int decode_status(const hprmat_ctx *c, Fac fac, bool must_converge, bool pivotin
     *pivot_index = 0;
     const bool verified_fac = (fac == FAC_S_Z) || (fac == FAC_S_C && !pivoting_fallback);
     if (verified_fac && hi[IN_REFUTED] != 0) return UNUSABLE;
-    if (hi[IN_ZERO_PIVOT] != 0 || (fac != FAC_C_Z && hi[IN_KBLOCK_SINGULAR] != 0)) {
+    if (hi[IN_ZERO_PIVOT] != 0 || ((fac == FAC_S_Z || fac == FAC_S_C) && hi[IN_KBLOCK_SINGULAR] != 0)) {
         if (fac == FAC_S_Z) return UNUSABLE;  // e.g. E on a pole of an uncoupled channel: C - E I itself may be regular
         *pivot_index = hi[IN_ZERO_PIVOT] ? hi[IN_ZERO_PIVOT] : hi[IN_KBLOCK_SINGULAR];
         return HPRMAT_ESINGULAR;
@@ -571,10 +653,10 @@ int run(hprmat_ctx *c, Fac fac, const Problem &p, double energy, int mode, int m
         hprmat_info *info, bool pivoting_fallback) {
     cudaStream_t st = c->st;
     const bool sync = info != nullptr;
-    const bool mixed = fac == FAC_S_C;
+    const bool mixed = fac == FAC_S_C || fac == FAC_T3;
     const bool must_converge = mode == HPRMAT_MIXED_REFINE;
     if (max_refine < 0) max_refine = mixed ? 5 : 2;
-    if (mode == HPRMAT_MIXED) max_refine = 0;
+    if (mode == HPRMAT_MIXED || mode == HPRMAT_TYPE3) max_refine = 0;
     if (!(tol > 0.0)) tol = mixed ? 1e-12 : 1e-13;  // estimated relative error left in X; the north-star asks 1e-10 of R
     ScopedZgemmAlgo algo_scope(c->zgemm_algo);
 
@@ -653,7 +735,7 @@ int solve_any(hprmat_ctx *c, const Problem &p, double energy, int mode, int max_
         info->backward_err = -1.0;
     }
     const int algo = c->fp64_algo ? c->fp64_algo : g_fp64_algo.load();
-    Fac fac = mode == HPRMAT_FP64 ? (algo == 2 ? FAC_S_Z : FAC_C_Z) : FAC_S_C;
+    Fac fac = mode == HPRMAT_FP64 ? (algo == 2 ? FAC_S_Z : FAC_C_Z) : mode == HPRMAT_TYPE3 ? FAC_T3 : FAC_S_C;
     int rc = run(c, fac, p, energy, mode, max_refine, tol, R, info, false);
     if (rc == UNUSABLE) {  // only reachable from a synchronised call: redo with pivoting
         *info = hprmat_info();
@@ -713,7 +795,7 @@ extern "C" int hprmat_solve(hprmat_ctx *ctx, double energy, const void *V, int m
                             hprmat_info *info) {
     if (!ctx) return -1;
     if (!V) return -3;
-    if (mode != HPRMAT_FP64 && mode != HPRMAT_MIXED && mode != HPRMAT_MIXED_REFINE) return -4;
+    if (mode != HPRMAT_FP64 && mode != HPRMAT_MIXED && mode != HPRMAT_MIXED_REFINE && mode != HPRMAT_TYPE3) return -4;
     if (!(ctx->max_mode & (1 << mode))) return -4;
     if (!R) return -7;
     Problem p;

@@ -326,6 +326,14 @@ static int diag_blocks_product(cudaStream_t st, const CView *dtab, int d0, int s
                       T.sub(nfull * LEAF, 0)));
     return 0;
 }
+// product inside the factorisation / the solves: FP32-class arithmetic when the workspace asks for it (complex64 only)
+static int lu_gemm(const LuWork<ZView> &, cudaStream_t st, int m, int n, int k, double alpha, ZView A, ZView B, double beta, ZView C) {
+    return gemm(st, m, n, k, alpha, A, B, beta, C);
+}
+static int lu_gemm(const LuWork<CView> &wk, cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta,
+                   CView C) {
+    return wk.accurate ? cgemm3(st, m, n, k, alpha, A, B, beta, C) : gemm(st, m, n, k, alpha, A, B, beta, C);
+}
 template <class V> struct IsPlanar { static constexpr bool value = false; };
 template <> struct IsPlanar<CView> { static constexpr bool value = true; };
 
@@ -339,9 +347,9 @@ static int big_leaf(cudaStream_t st, const V &binv, const V *dtab, int d0, int s
         V Bc = B.sub(0, c), T = wk.tmp;
         if (acc && IsPlanar<V>::value) {
             HP_TRY(diag_blocks_product(st, dtab, d0, s, Bc, nc, T));
-            HP_TRY(gemm(st, s, nc, s, 1.0, binv_of(binv, wk.sbld, d0), Bc, 1.0, T));
+            HP_TRY(lu_gemm(wk, st, s, nc, s, 1.0, binv_of(binv, wk.sbld, d0), Bc, 1.0, T));
         } else {
-            HP_TRY(gemm(st, s, nc, s, 1.0, binv_of(binv, wk.sbld, d0), Bc, 0.0, T));
+            HP_TRY(lu_gemm(wk, st, s, nc, s, 1.0, binv_of(binv, wk.sbld, d0), Bc, 0.0, T));
         }
         HP_TRY(copy_block(st, T, Bc, s, nc));
     }
@@ -371,8 +379,8 @@ static int leaf_product(bool acc, cudaStream_t st, int s, int ncols, ZView dinv,
     }
     return gemm_sel(acc, st, s, ncols, s, 1.0, dinv, B, 0.0, B);
 }
-static int leaf_product(bool acc, cudaStream_t st, int s, int ncols, CView dinv, CView B, LuWork<CView> &) {
-    return gemm_sel(acc, st, s, ncols, s, 1.0, dinv, B, 0.0, B);
+static int leaf_product(bool acc, cudaStream_t st, int s, int ncols, CView dinv, CView B, LuWork<CView> &wk) {
+    return gemm_sel(acc || wk.accurate, st, s, ncols, s, 1.0, dinv, B, 0.0, B);
 }
 
 // B <- L^-1 B, L = unit lower triangle of the s x s diagonal block of A at (d0,d0); B is s x ncols.  d0 is a multiple of
@@ -384,7 +392,7 @@ template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V 
         return big_leaf(st, wk.binvL, wk.dinvL, d0, s, B, ncols, wk, acc);
     const int h = split(s);
     HP_TRY(trsm_lower(st, A, d0, h, B, ncols, wk, acc));
-    HP_TRY(gemm(st, s - h, ncols, h, -1.0, A.sub(d0 + h, d0), B, 1.0, B.sub(h, 0)));
+    HP_TRY(lu_gemm(wk, st, s - h, ncols, h, -1.0, A.sub(d0 + h, d0), B, 1.0, B.sub(h, 0)));
     return trsm_lower(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk, acc);
 }
 
@@ -396,7 +404,7 @@ template <class V> static int trsm_upper(cudaStream_t st, V A, int d0, int s, V 
         return big_leaf(st, wk.binvU, wk.dinvU, d0, s, B, ncols, wk, acc);
     const int h = split(s);
     HP_TRY(trsm_upper(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk, acc));
-    HP_TRY(gemm(st, h, ncols, s - h, -1.0, A.sub(d0, d0 + h), B.sub(h, 0), 1.0, B));
+    HP_TRY(lu_gemm(wk, st, h, ncols, s - h, -1.0, A.sub(d0, d0 + h), B.sub(h, 0), 1.0, B));
     return trsm_upper(st, A, d0, h, B, ncols, wk, acc);
 }
 
@@ -481,7 +489,7 @@ template <class V> static int getrf_rec(cudaStream_t st, int n, V A, int c0, int
     }
     {
         ProfCat pc(PROF_LU_GEMM);
-        HP_TRY(gemm(st, n - mid, c1 - mid, h, -1.0, A.sub(mid, c0), A.sub(c0, mid), 1.0, A.sub(mid, mid)));
+        HP_TRY(lu_gemm(wk, st, n - mid, c1 - mid, h, -1.0, A.sub(mid, c0), A.sub(c0, mid), 1.0, A.sub(mid, mid)));
     }
     HP_TRY(getrf_rec(st, n, A, mid, c1, ipiv, info_dev, wk));
     // the node's diagonal block is final: keep its inverse for the triangular solves further up / in getrs

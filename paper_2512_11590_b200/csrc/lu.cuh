@@ -45,6 +45,9 @@ template <class V> struct LuWork {
     int *refuted = nullptr;    // device counter: multipliers that refuted the diagonal-pivot speculation (toplu.cu); zeroed by getrf
     bool speculate = false;    // host-side: the matrix is expected to pivot on its diagonal (S = K_d^-1 (C - E I)): factor
                                // without interchanges and VERIFY (toplu.cu); the caller checks *refuted afterwards
+    bool accurate = false;     // host-side, complex64 only: EVERY product of the factorisation and of the solves in FP32-class
+                               // arithmetic (3xTF32) instead of single-pass TF32 -- general matrices whose condition number
+                               // is beyond 2^11 (raw mixed solve after a failed refinement; the literal Type-3 Schur matrix)
     bool side_used = false; // host-side: something of this factorisation was enqueued on the side stream
     // host-side resources for the side stream (kept block inverses are built under the factorisation).  A context sets its
     // own (hprmat_setup); when null, a per-device pool serves the raw entries (lu.cu)

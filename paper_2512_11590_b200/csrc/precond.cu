@@ -374,4 +374,87 @@ int promote_add(cudaStream_t st, long rows, int cols, double2 *X, long ldx, CVie
     return 0;
 }
 
+// ---------------------------------------------------------------------------------------------------- Type 3 (literal)
+// M = K_diag (I + K^-1 V) with K the REAL kinetic (+ Bloch) block shared by all channels, V(r_j) the
+// Nc x Nc matrices of everything else on the mesh diagonal (potentials, centrifugal and threshold terms, -E), and the
+// point-major Schur matrix of Eq. (8):  S[(i,a),(j,a')] = delta_ij delta_aa' + Kinv_ij V_aa'(r_j),  index (i*nch + a).
+// Thread = (a, column (j,a')): loads V'_aa'(r_j) once and writes the nb entries of its column strip, each store of a warp
+// covering 128 contiguous bytes of a plane.
+__global__ void __launch_bounds__(128) assemble_type3_kernel(int nch, int nb, const double *__restrict__ KTinv,
+                                                             const double *__restrict__ cf, const double *__restrict__ ethr,
+                                                             double energy, const double2 *__restrict__ V,
+                                                             float *__restrict__ Sre, float *__restrict__ Sim, long ld) {
+    const int a = blockIdx.y * 128 + threadIdx.x;
+    const long q = blockIdx.x;            // column (j, a')
+    if (a >= nch) return;
+    const int j = (int)(q / nch), a2 = (int)(q - (long)j * nch);
+    double2 v = V[((long)j * nch + a2) * nch + a];  // V_{a a'}(r_j)
+    if (a == a2) v.x += cf[(long)a * nb + j] + (ethr[a] - energy);
+    float *re = Sre + q * ld + a, *im = Sim + q * ld + a;
+    for (int i = 0; i < nb; ++i) {
+        const double k = KTinv[(long)j * nb + i];
+        re[(long)i * nch] = (float)(k * v.x + ((i == j && a == a2) ? 1.0 : 0.0));
+        im[(long)i * nch] = (float)(k * v.y);
+    }
+}
+int type3_assemble(cudaStream_t st, const StructTables &t, const double *KTinv, const double *cf, double energy, const double2 *V,
+                   CView S) {
+    const long N = (long)t.nch * t.nb;
+    assemble_type3_kernel<<<dim3((unsigned)N, ceil_div(t.nch, 128)), 128, 0, st>>>(t.nch, t.nb, KTinv, cf, t.ethr, energy, V, S.re,
+                                                                                  S.im, S.ld);
+    HP_LAUNCHED();
+    return 0;
+}
+
+// Eq. (9): b~[(i,a), c'] = (Kinv q2)_i delta_{a c'}   (g = Kinv q2 is energy-independent, computed at setup)
+__global__ void __launch_bounds__(256) rhs_type3_kernel(int nch, int nb, const double *__restrict__ g, float *__restrict__ Bre,
+                                                        float *__restrict__ Bim, long ld) {
+    const long N = (long)nch * nb, tot = N * nch;
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < tot; idx += (long)gridDim.x * blockDim.x) {
+        const long c2 = idx / N, p = idx - c2 * N;
+        const int i = (int)(p / nch), a = (int)(p - (long)i * nch);
+        Bre[c2 * ld + p] = a == c2 ? (float)g[i] : 0.f;
+        Bim[c2 * ld + p] = 0.f;
+    }
+}
+int type3_rhs(cudaStream_t st, const StructTables &t, const double *g, CView B) {
+    const long tot = (long)t.nch * t.nb * t.nch;
+    rhs_type3_kernel<<<(int)std::min<long>(ceil_div(tot, 256), 148L * 8), 256, 0, st>>>(t.nch, t.nb, g, B.re, B.im, B.ld);
+    HP_LAUNCHED();
+    return 0;
+}
+
+// step 6 "transform solution back": X[(a,i), c'] <- x~[(i,a), c']  (point-major complex64 -> channel-major complex128);
+// norms[1] = max|X|
+__global__ void __launch_bounds__(256) promote_from_point_major_kernel(int nch, int nb, const float *__restrict__ re,
+                                                                       const float *__restrict__ im, long ld,
+                                                                       double2 *__restrict__ X, long ldx, double *norms) {
+    __shared__ double shred[32];
+    const long N = (long)nch * nb, tot = N * nch;
+    double mx = 0.0;
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < tot; idx += (long)gridDim.x * blockDim.x) {
+        const long c2 = idx / N, p = idx - c2 * N;
+        const int i = (int)(p / nch), a = (int)(p - (long)i * nch);
+        const double xr = (double)re[c2 * ld + p], xi = (double)im[c2 * ld + p];
+        X[c2 * ldx + (long)a * nb + i] = make_double2(xr, xi);
+        mx = fmax(mx, sqrt(xr * xr + xi * xi));
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, off));
+    if ((threadIdx.x & 31) == 0) shred[threadIdx.x >> 5] = mx;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) mx = fmax(mx, shred[w]);
+        atomicMax(reinterpret_cast<unsigned long long *>(norms + 1), (unsigned long long)__double_as_longlong(mx));
+    }
+}
+int type3_promote(cudaStream_t st, const StructTables &t, CView Xs, double2 *X, long ldx, double *norms_dev) {
+    HP_CUDA(cudaMemsetAsync(norms_dev, 0, 2 * sizeof(double), st));
+    const long tot = (long)t.nch * t.nb * t.nch;
+    promote_from_point_major_kernel<<<(int)std::min<long>(ceil_div(tot, 256), 148L * 8), 256, 0, st>>>(t.nch, t.nb, Xs.re, Xs.im,
+                                                                                                       Xs.ld, X, ldx, norms_dev);
+    HP_LAUNCHED();
+    return 0;
+}
+
 }  // namespace hp

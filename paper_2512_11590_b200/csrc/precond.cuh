@@ -27,4 +27,13 @@ int demote(cudaStream_t st, long rows, int cols, const double2 *Z, long ldz, CVi
 int promote_add(cudaStream_t st, long rows, int cols, double2 *X, long ldx, CView D, bool accumulate, double *norms_dev,
                 const int *gate_dev = nullptr);
 
+// The paper's Type 3 in its literal form (Eqs. 7-9): point-major Schur matrix S = I + K^-1 V with K the real
+// kinetic block shared by all channels.  KTinv: nb x nb column-major inverse of h2m*T; cf: [nch*nb] centrifugal terms
+// h2m l(l+1)/r_i^2; g = KTinv q2 (nb).  All three are energy-independent (computed once at setup).
+int type3_assemble(cudaStream_t st, const StructTables &t, const double *KTinv, const double *cf, double energy, const double2 *V,
+                   CView S);
+int type3_rhs(cudaStream_t st, const StructTables &t, const double *g, CView B);
+// X (channel-major complex128) <- point-major complex64 solution; norms_dev[1] = max|X|
+int type3_promote(cudaStream_t st, const StructTables &t, CView Xs, double2 *X, long ldx, double *norms_dev);
+
 }  // namespace hp

@@ -195,59 +195,70 @@ int zsolve_mixed(cudaStream_t st, int n, int nrhs, const double2 *A, long lda, d
     int hinfo = 0;
 #define ZM_TRY(x) do { int r__ = (x); if (r__ != 0) { cleanup(); return r__; } } while (0)
 #define ZM_CUDA(x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) { cleanup(); return hp::cuda_fail(e__, __FILE__, __LINE__); } } while (0)
-    ZM_CUDA(cudaMemsetAsync(w.info, 0, sizeof(int), st));
-    ZM_CUDA(cudaMemsetAsync(w.scal, 0, sizeof(double) * 16, st));
     ZM_CUDA(cudaEventRecord(ev[0], st));
-    // keep b for the residual; equilibrate and demote (PAPER.md:200-216 convert_z2c, fused with the scaling)
+    // keep b for the residual (PAPER.md:200-216 convert_z2c happens in equil_demote_kernel, fused with the scaling)
     ZM_CUDA(cudaMemcpy2DAsync(w.B0, sizeof(double2) * n, B, sizeof(double2) * ldb, sizeof(double2) * n, nrhs, cudaMemcpyDeviceToDevice, st));
     row_stats_kernel<<<ceil_div(n, 256), 256, 0, st>>>(n, A, lda, w.rs, w.rsum);
     HP_LAUNCHED();
     col_scale_kernel<<<n, 256, 0, st>>>(n, A, lda, w.rs, w.cs);
     HP_LAUNCHED();
-    equil_demote_kernel<<<dim3(ceil_div(n, 256), ceil_div(n, 8)), 256, 0, st>>>(n, A, lda, w.rs, w.cs, w.S.re, w.S.im, w.S.ld);
-    HP_LAUNCHED();
-    vecmax_kernel<<<std::min(ceil_div(n, 256), 148), 256, 0, st>>>(n, w.rsum, w.scal + 4);  // ||A||_inf
-    HP_LAUNCHED();
-    ZM_TRY(getrf<CView>(st, n, w.S, ipiv, w.info, w.wk));
-    ZM_CUDA(cudaEventRecord(ev[1], st));
     const int grid = (int)std::min<long>(ceil_div((long)n * nrhs, 256), 148L * 8);
-    scale_demote_kernel<<<grid, 256, 0, st>>>(n, nrhs, w.B0, n, w.rs, w.Bs.re, w.Bs.im, w.Bs.ld);
-    HP_LAUNCHED();
-    ZM_TRY(getrs<CView>(st, n, nrhs, w.S, w.Bs, w.wk));
-    promote_scale_add_kernel<<<grid, 256, 0, st>>>(n, nrhs, B, ldb, w.Bs.re, w.Bs.im, w.Bs.ld, w.cs, 0, w.scal);
-    HP_LAUNCHED();
-    ZM_CUDA(cudaEventRecord(ev[2], st));
-    ZM_CUDA(cudaMemcpyAsync(h, w.scal, sizeof(double) * 2, cudaMemcpyDeviceToHost, st));
-    ZM_CUDA(cudaMemcpyAsync(&hinfo, w.info, sizeof(int), cudaMemcpyDeviceToHost, st));
-    ZM_CUDA(cudaStreamSynchronize(st));
-    if (hinfo != 0) {
-        cleanup();
-        if (info) { info->status = HPRMAT_ESINGULAR; info->pivot_index = hinfo; }
-        return HPRMAT_ESINGULAR;
-    }
-    double dprev = h[1];
-    if (max_refine > 0) status = HPRMAT_ENOTCONVERGED;
-    for (int k = 0; k < max_refine; ++k) {
-        // r = b - A x in FP64 on the DMMA tensor cores
-        ZM_CUDA(cudaMemcpyAsync(w.R, w.B0, sizeof(double2) * (size_t)n * nrhs, cudaMemcpyDeviceToDevice, st));
-        ZM_TRY(zgemm(st, n, nrhs, n, -1.0, A, lda, B, ldb, 1.0, w.R, n));
-        scale_demote_kernel<<<grid, 256, 0, st>>>(n, nrhs, w.R, n, w.rs, w.Bs.re, w.Bs.im, w.Bs.ld);
+    int fp32_class = 0;
+    // Attempt 0: single-pass TF32 trailing update (contraction ~ sqrt(n) 2^-11 kappa per refinement step).  If the
+    // refinement does not converge with those factors, attempt 1 refactors with FP32-class products everywhere (3xTF32:
+    // contraction ~ sqrt(n) 2^-23 kappa), the paper's domain kappa u_FP32 < 1 (Fig. 5).
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        w.wk.accurate = attempt == 1;
+        fp32_class = attempt;
+        steps = 0;
+        ZM_CUDA(cudaMemsetAsync(w.info, 0, sizeof(int), st));
+        ZM_CUDA(cudaMemsetAsync(w.scal, 0, sizeof(double) * 16, st));
+        equil_demote_kernel<<<dim3(ceil_div(n, 256), ceil_div(n, 8)), 256, 0, st>>>(n, A, lda, w.rs, w.cs, w.S.re, w.S.im, w.S.ld);
+        HP_LAUNCHED();
+        vecmax_kernel<<<std::min(ceil_div(n, 256), 148), 256, 0, st>>>(n, w.rsum, w.scal + 4);  // ||A||_inf
+        HP_LAUNCHED();
+        ZM_TRY(getrf<CView>(st, n, w.S, ipiv, w.info, w.wk));
+        ZM_CUDA(cudaEventRecord(ev[1], st));
+        scale_demote_kernel<<<grid, 256, 0, st>>>(n, nrhs, w.B0, n, w.rs, w.Bs.re, w.Bs.im, w.Bs.ld);
         HP_LAUNCHED();
         ZM_TRY(getrs<CView>(st, n, nrhs, w.S, w.Bs, w.wk));
-        ZM_CUDA(cudaMemsetAsync(w.scal, 0, sizeof(double) * 2, st));
-        promote_scale_add_kernel<<<grid, 256, 0, st>>>(n, nrhs, B, ldb, w.Bs.re, w.Bs.im, w.Bs.ld, w.cs, 1, w.scal);
+        promote_scale_add_kernel<<<grid, 256, 0, st>>>(n, nrhs, B, ldb, w.Bs.re, w.Bs.im, w.Bs.ld, w.cs, 0, w.scal);
         HP_LAUNCHED();
-        ++steps;
+        ZM_CUDA(cudaEventRecord(ev[2], st));
         ZM_CUDA(cudaMemcpyAsync(h, w.scal, sizeof(double) * 2, cudaMemcpyDeviceToHost, st));
+        ZM_CUDA(cudaMemcpyAsync(&hinfo, w.info, sizeof(int), cudaMemcpyDeviceToHost, st));
         ZM_CUDA(cudaStreamSynchronize(st));
-        const int v = refine_verdict(h[0], h[1], dprev, tol);
-        dprev = h[0];
-        if (v == REF_CONVERGED) { status = HPRMAT_OK; break; }
-        if (v == REF_STAGNATED) {
-            status = (h[0] <= 64.0 * 2.220446049250313e-16 * h[1]) ? HPRMAT_OK : HPRMAT_ENOTCONVERGED;
-            break;
+        if (hinfo != 0) {
+            cleanup();
+            if (info) { info->status = HPRMAT_ESINGULAR; info->pivot_index = hinfo; }
+            return HPRMAT_ESINGULAR;
         }
+        double dprev = h[1];
+        status = max_refine > 0 ? HPRMAT_ENOTCONVERGED : HPRMAT_OK;
+        for (int k = 0; k < max_refine; ++k) {
+            // r = b - A x in FP64 on the DMMA tensor cores
+            ZM_CUDA(cudaMemcpyAsync(w.R, w.B0, sizeof(double2) * (size_t)n * nrhs, cudaMemcpyDeviceToDevice, st));
+            ZM_TRY(zgemm(st, n, nrhs, n, -1.0, A, lda, B, ldb, 1.0, w.R, n));
+            scale_demote_kernel<<<grid, 256, 0, st>>>(n, nrhs, w.R, n, w.rs, w.Bs.re, w.Bs.im, w.Bs.ld);
+            HP_LAUNCHED();
+            ZM_TRY(getrs<CView>(st, n, nrhs, w.S, w.Bs, w.wk));
+            ZM_CUDA(cudaMemsetAsync(w.scal, 0, sizeof(double) * 2, st));
+            promote_scale_add_kernel<<<grid, 256, 0, st>>>(n, nrhs, B, ldb, w.Bs.re, w.Bs.im, w.Bs.ld, w.cs, 1, w.scal);
+            HP_LAUNCHED();
+            ++steps;
+            ZM_CUDA(cudaMemcpyAsync(h, w.scal, sizeof(double) * 2, cudaMemcpyDeviceToHost, st));
+            ZM_CUDA(cudaStreamSynchronize(st));
+            const int v = refine_verdict(h[0], h[1], dprev, tol);
+            dprev = h[0];
+            if (v == REF_CONVERGED) { status = HPRMAT_OK; break; }
+            if (v == REF_STAGNATED) {
+                status = (h[0] <= 64.0 * 2.220446049250313e-16 * h[1]) ? HPRMAT_OK : HPRMAT_ENOTCONVERGED;
+                break;
+            }
+        }
+        if (status == HPRMAT_OK || max_refine == 0) break;
     }
+    w.wk.accurate = false;
     ZM_CUDA(cudaEventRecord(ev[3], st));
     if (info) {
         // backward error of the returned x: r = b - A x once more
@@ -261,6 +272,7 @@ int zsolve_mixed(cudaStream_t st, int n, int nrhs, const double2 *A, long lda, d
         float ms = 0.f;
         info->status = status;
         info->refine_steps = steps;
+        info->reserved = fp32_class;  // 1: the single-pass TF32 factors did not converge, FP32-class (3xTF32) factors were used
         info->resid_max = h[3];
         info->backward_err = h[5];
         cudaEventElapsedTime(&ms, ev[0], ev[1]);

@@ -225,7 +225,7 @@ template <class V> int block_panel(cudaStream_t st, int n, V A, int c0, int w, i
     V L21 = A.sub(c0 + w, c0);
     {
         ProfCat pc(PROF_PANEL);
-        if (l21_checked(st, m2, w, L21, du, wk.refuted)) return 0;  // complex64: the check rides in the GEMM's epilogue
+        if (!wk.accurate && l21_checked(st, m2, w, L21, du, wk.refuted)) return 0;  // complex64: the check rides in the epilogue
         HP_TRY(gemm(st, m2, w, w, 1.0, L21, du, 0.0, L21));
         const bool prof = prof_enabled();
         if (prof) prof_begin(st, 0.0);

@@ -188,6 +188,32 @@ def test_rmatrix_mixed_norefine_parity(cfg, nch, nb):
     ctx.destroy()
 
 
+@pytest.mark.parametrize("cfg,nch,nb", MIXED_CASES)
+def test_rmatrix_type3_literal_schur_form(cfg, nch, nb):
+    """HPRMAT_TYPE3: the paper's Type 3 as printed: point-major Schur matrix I + K^-1 V of Eq. (8) with
+    the real kinetic block K shared by all channels, transformed right-hand side of Eq. (9), complex64 LU with partial
+    pivoting, no refinement.  kappa(S) ~ 1e5 here, so the bar is the paper's own ~1e-6 class (asserted: 1e-4, far inside the
+    north-star's 1e-3 for unrefined results); it must agree with HPRMAT_MIXED (another factorisation of the same system) to
+    the same level, and K^-1 is reused across the energies of the scan."""
+    w = make_workload(cfg, nch=nch, nb=nb)
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=(1 << hb.HPRMAT_TYPE3) | (1 << hb.HPRMAT_MIXED))
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    for E in w.energies[:2]:
+        R3, info = ctx.solve(float(E), V, hb.HPRMAT_TYPE3)
+        R3 = _host(R3).copy()
+        X3 = _host(ctx.get_x()).copy()
+        Ro, Xo = _oracle_R(w, float(E))
+        assert info["status"] == 0 and info["refine_steps"] == 0, info
+        err = _relmax(R3, Ro)
+        assert err <= 1e-4, (err, info)
+        assert _relmax(X3, Xo) <= 1e-3
+        Rm, _ = ctx.solve(float(E), V, hb.HPRMAT_MIXED)
+        assert _relmax(_host(Rm), R3) <= 1e-4
+        print(f"type3 {w.name} E={E}: R error {err:.2e}")
+    ctx.destroy()
+
+
 def test_mixed_strong_coupling_needs_and_gets_more_refinement():
     """Couplings 100x stronger than the configs': the TF32 factors are poorer, refinement needs more steps than the
     configs' two and still reaches 1e-10 (observed: 4 steps) -- a regression that turns this into non-convergence fails."""
@@ -347,8 +373,11 @@ def test_zsolve_mixed_never_returns_a_silent_low_precision_result(kappa):
         assert err <= 100 * kappa * 2.0 ** -53 * n
     else:
         assert info["status"] == hb.HPRMAT_ENOTCONVERGED
-    if kappa <= 1e2:
-        assert info["status"] == hb.HPRMAT_OK                                  # well inside the convergence domain
+    if kappa <= 1e5:
+        # inside the paper's domain kappa * u_FP32 < 1 (Fig. 5): must converge.  Beyond kappa ~ 1e3 the
+        # single-pass TF32 factors do not contract and the solve refactors with FP32-class (3xTF32) products (info.reserved)
+        assert info["status"] == hb.HPRMAT_OK, info
+        assert info["reserved"] == (1 if kappa >= 1e5 else 0), info
 
 
 # ---------------------------------------------------------------------------------------------------- headline size, mixed
