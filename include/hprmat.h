@@ -161,6 +161,35 @@ int hprmat_solve_host(hprmat_ctx *ctx, double energy, const void *V_host, int mo
 int hprmat_solve_nonlocal(hprmat_ctx *ctx, double energy, const void *W, long ldw, int mode, int max_refine, double tol,
                           void *R, hprmat_info *info);
 
+/* ---- propagation over sub-intervals (hprmat_init(nr, ns, rmax, zrma)) ----
+ *
+ * PAPER.md names the propagation and the number of sub-intervals ns without printing formulas (they are in its ref. [2]);
+ * the reading taken is DESIGN.md section 3, R16.  The first sub-interval (0, a_1) is an ordinary context (hprmat_setup with
+ * a = a_1, hprmat_solve -> R at a_1).  Every further sub-interval (a_lo, a_hi), a_lo > 0, gets a SECTOR context: plain
+ * Lagrange-Legendre mesh on the interval, Bloch operators at both ends, the same matrix structure and the same hot path
+ * (assembly, LU, solves, refinement), with two sets of nch right-hand sides -- the surface vectors of the two ends -- on one
+ * factorisation.  hprmat_mesh returns the radii r_i = a_lo + (a_hi - a_lo) x_i and the RIGHT-end surface values. */
+int hprmat_setup_sector(hprmat_ctx **out, int nch, int nbasis, double a_lo, double a_hi, double h2m, const int *lval,
+                        const double *ethr, int max_mode, void *cuda_stream);
+
+/* Sector matrices of one energy point:  Rsec_ab = (hbar^2/2mu) B_a^T (C - E I)^-1 B_b,  a, b in {L (= a_lo), R (= a_hi)}.
+ *   V     dev, complex [nbasis][nch][nch] at the sector's mesh radii (layout as hprmat_solve)
+ *   mode  HPRMAT_FP64 / HPRMAT_MIXED / HPRMAT_MIXED_REFINE;  max_refine, tol as hprmat_solve
+ *   Rsec  dev, complex, four nch x nch column-major blocks in the order LL, LR, RL, RR (4 nch^2 elements)
+ *   info  host, REQUIRED (the two passes are synchronised); times are summed over both passes
+ * hprmat_get_x afterwards returns the solution block of the LEFT-end right-hand sides. */
+int hprmat_solve_sector(hprmat_ctx *ctx, double energy, const void *V, int mode, int max_refine, double tol, void *Rsec,
+                        hprmat_info *info);
+
+/* R-matrix at a_hi from the R-matrix at a_lo and the sector matrices of (a_lo, a_hi):
+ *     a_hi R_out = Rsec_RR - Rsec_RL (Rsec_LL + a_lo R_in)^-1 Rsec_LR
+ * (R in this library's convention u(a) = a R u'(a), i.e. with the prefactor hbar^2/(2 mu a)).  All matrices dev, complex
+ * nch x nch column-major; R_out may not alias R_in or Rsec.  info_dev: dev int[1], 0 or the 1-based zero pivot of the
+ * nch x nch LU.  workspace: dev, 256-byte aligned, >= hprmat_propagate_workspace_bytes(nch).  No synchronisation. */
+size_t hprmat_propagate_workspace_bytes(int nch);
+int hprmat_propagate(void *cuda_stream, int nch, double a_lo, double a_hi, const void *R_in, const void *Rsec, void *R_out,
+                     int *info_dev, void *workspace, size_t workspace_bytes);
+
 /* Solution block of the last hprmat_solve: X dev, complex N x nch column-major (copy out). */
 int hprmat_get_x(const hprmat_ctx *ctx, void *X);
 

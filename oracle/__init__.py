@@ -4,4 +4,4 @@ Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl refere
 It shares no code with paper_2512_11590_b200 (the CUDA path) and neither imports the other.
 """
 from .oracle import (mesh, kinetic, assemble, rhs, solve, structured_residual, contract, rmatrix,  # noqa: F401
-                     collision_matrix, rmatrix_nonlocal, num_threads)
+                     collision_matrix, rmatrix_nonlocal, num_threads, sector_tables, sector_matrices, propagate)

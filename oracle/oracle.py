@@ -242,3 +242,68 @@ def collision_matrix(R, lval, ethr, energy, h2m, a, zze2=None):
     ZF = ((np.diag(Fr) - R * dFr[None, :]) / np.sqrt(x)[None, :])[:, opn]
     Y = np.linalg.solve(ZO, ZF)
     return np.eye(len(opn)) - 2j * Y[opn, :], opn
+
+
+# ---- propagation over sub-intervals ("propagation", ns sub-intervals; reading R16) ----------
+def sector_tables(nb: int, a_lo: float, a_hi: float):
+    """Lagrange-Legendre mesh on the sub-interval (a_lo, a_hi), NOT regularised, with the definitions written out:
+    f_i(r) = l_i(x) / sqrt(h lam_i), x = (r - a_lo)/h, l_i(x) = prod_{m != i} (x - x_m)/(x_i - x_m).  Returns
+    (r, fa_left, fa_right, T) with T_ij = <f_i| -d2/dr2 + L(a_hi) - L(a_lo) |f_j> = int f_i' f_j' dr (Bloch operator at both
+    ends; units hbar^2/2mu = 1), the integral by the mesh's own Gauss quadrature, exact for this polynomial integrand.
+    l_i'(x_k) from the product rule: for k != i only the term without the factor (x - x_k) survives,
+    l_i'(x_k) = prod_{m != i,k} (x_k - x_m) / prod_{m != i} (x_i - x_m);  l_i'(x_i) = sum_{m != i} 1/(x_i - x_m).
+    long double throughout, rounded to double at the end."""
+    x, lam, _, _ = mesh(nb, 1.0)
+    xl = x.astype(np.longdouble)
+    ll = lam.astype(np.longdouble)
+    h = np.longdouble(a_hi) - np.longdouble(a_lo)
+    D = np.zeros((nb, nb), dtype=np.longdouble)          # D[k, i] = l_i'(x_k)
+    l0 = np.zeros(nb, dtype=np.longdouble)
+    l1 = np.zeros(nb, dtype=np.longdouble)
+    for i in range(nb):
+        others = [m for m in range(nb) if m != i]
+        den = np.prod(xl[i] - xl[others])
+        l0[i] = np.prod(0 - xl[others]) / den
+        l1[i] = np.prod(1 - xl[others]) / den
+        D[i, i] = np.sum(1 / (xl[i] - xl[others]))
+        for k in others:
+            rest = [m for m in others if m != k]
+            D[k, i] = np.prod(xl[k] - xl[rest]) / den
+    T = np.zeros((nb, nb), dtype=np.longdouble)
+    for i in range(nb):
+        for j in range(nb):
+            T[i, j] = np.sum(ll * D[:, i] * D[:, j]) / (h * h * np.sqrt(ll[i] * ll[j]))
+    r = (np.longdouble(a_lo) + h * xl).astype(np.float64)
+    return r, (l0 / np.sqrt(h * ll)).astype(np.float64), (l1 / np.sqrt(h * ll)).astype(np.float64), T.astype(np.float64)
+
+
+def sector_matrices(nch, nb, a_lo, a_hi, h2m, lval, ethr, energy, V):
+    """Rsec_ab = h2m B_a^T (C - E I)^-1 B_b for a, b in {L, R} on the sub-interval (a_lo, a_hi): returns the 2 x 2 nested list
+    [[LL, LR], [RL, RR]] of nch x nch matrices.  C - E I has the structure of Eqs. (3),(4) with the sector's T; dense
+    assembly, the oracle's LU (orc_solve) for the 2 nch right-hand sides."""
+    r, faL, faR, T = sector_tables(nb, a_lo, a_hi)
+    V = np.asarray(V, dtype=np.complex128)
+    assert V.shape == (nb, nch, nch)
+    N = nch * nb
+    Cm = np.zeros((N, N), dtype=np.complex128)
+    for c in range(nch):
+        blk = (h2m * T).astype(np.complex128)
+        blk[np.arange(nb), np.arange(nb)] += h2m * lval[c] * (lval[c] + 1) / r ** 2 + (ethr[c] - energy)
+        Cm[c * nb:(c + 1) * nb, c * nb:(c + 1) * nb] = blk
+    for i in range(nb):
+        idx = np.arange(nch) * nb + i
+        Cm[np.ix_(idx, idx)] += V[i].T                      # V[i, c2, c1] = V_{c1 c2}(r_i)
+    B = np.zeros((N, 2 * nch), dtype=np.complex128)
+    for c in range(nch):
+        B[c * nb:(c + 1) * nb, c] = faL
+        B[c * nb:(c + 1) * nb, nch + c] = faR
+    X = solve(Cm, B)
+    G = h2m * (B.T @ X)
+    return [[G[:nch, :nch], G[:nch, nch:]], [G[nch:, :nch], G[nch:, nch:]]]
+
+
+def propagate(a_lo, a_hi, R_in, Rsec):
+    """a_hi R_out = Rsec_RR - Rsec_RL (Rsec_LL + a_lo R_in)^-1 Rsec_LR  (reading R16: u(a_hi) = Rsec_RR u'(a_hi) - Rsec_RL u'(a_lo),
+    u(a_lo) = Rsec_LR u'(a_hi) - Rsec_LL u'(a_lo), u(a_lo) = a_lo R_in u'(a_lo); eliminate u'(a_lo))."""
+    (LL, LR), (RL, RR) = Rsec
+    return (RR - RL @ np.linalg.solve(LL + a_lo * np.asarray(R_in), LR)) / a_hi

@@ -54,6 +54,7 @@ def lib():
         L.hprmat_launch_count.restype = C.c_longlong
         L.hprmat_workspace_bytes.restype = C.c_size_t
         L.hprmat_collision_workspace_bytes.restype = C.c_size_t
+        L.hprmat_propagate_workspace_bytes.restype = C.c_size_t
         _lib = L
     return _lib
 
@@ -135,6 +136,32 @@ class Context:
                                 lv.ctypes.data_as(C.c_void_p), et.ctypes.data_as(C.c_void_p), C.c_int(max_mode),
                                 _stream(stream))
         _check(rc, "hprmat_setup")
+
+    @classmethod
+    def sector(cls, nch, nbasis, a_lo, a_hi, h2m, lval, ethr, max_mode=0, stream=None):
+        """hprmat_setup_sector: context of the sub-interval (a_lo, a_hi) of a propagation."""
+        self = cls.__new__(cls)
+        self.nch, self.nb, self.n = int(nch), int(nbasis), int(nch) * int(nbasis)
+        lv = np.ascontiguousarray(lval, dtype=np.int32)
+        et = np.ascontiguousarray(ethr, dtype=np.float64)
+        self._h = C.c_void_p()
+        self._stream = stream
+        rc = lib().hprmat_setup_sector(C.byref(self._h), C.c_int(nch), C.c_int(nbasis), C.c_double(a_lo), C.c_double(a_hi),
+                                       C.c_double(h2m), lv.ctypes.data_as(C.c_void_p), et.ctypes.data_as(C.c_void_p),
+                                       C.c_int(max_mode), _stream(stream))
+        _check(rc, "hprmat_setup_sector")
+        return self
+
+    def solve_sector(self, energy, V, mode=HPRMAT_FP64, max_refine=-1, tol=0.0, allow=(HPRMAT_OK,)):
+        """hprmat_solve_sector: returns (Rsec, info); Rsec torch complex128 [4, nch, nch], block b holds the column-major
+        matrix (use Rsec[b].T) in the order LL, LR, RL, RR."""
+        assert V.is_cuda and V.dtype == torch.complex128 and V.is_contiguous() and V.numel() == self.nb * self.nch ** 2
+        Rsec = torch.empty((4, self.nch, self.nch), dtype=torch.complex128, device=V.device)
+        info = hprmat_info()
+        rc = lib().hprmat_solve_sector(self._h, C.c_double(energy), _dev(V), C.c_int(mode), C.c_int(max_refine),
+                                       C.c_double(tol), _dev(Rsec), C.byref(info))
+        _check(rc, "hprmat_solve_sector", allow)
+        return Rsec, info.as_dict()
 
     def mesh(self):
         r = np.zeros(self.nb)
@@ -300,6 +327,21 @@ def hprmat_collision(lval, ethr, energy, h2m, a, R, zze2=None, info_dev=None, ws
                                 C.c_size_t(ws.numel() - 256))
     _check(rc, "hprmat_collision")
     return U[:nopen.value * nopen.value], nopen.value
+
+
+def hprmat_propagate(a_lo, a_hi, R_in, Rsec, info_dev=None, ws=None, stream=None):
+    """R-matrix at a_hi from the one at a_lo and the sector matrices (torch complex128 CUDA tensors, column-major)."""
+    nch = R_in.shape[0]
+    nbytes = int(lib().hprmat_propagate_workspace_bytes(C.c_int(nch)))
+    if ws is None:
+        ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=R_in.device)
+    if info_dev is None:
+        info_dev = torch.zeros(1, dtype=torch.int32, device=R_in.device)
+    R_out = torch.empty((nch, nch), dtype=torch.complex128, device=R_in.device)
+    rc = lib().hprmat_propagate(_stream(stream), C.c_int(nch), C.c_double(a_lo), C.c_double(a_hi), _dev(R_in), _dev(Rsec),
+                                _dev(R_out), _dev(info_dev), _aligned(ws), C.c_size_t(ws.numel() - 256))
+    _check(rc, "hprmat_propagate")
+    return R_out
 
 
 def hprmat_zgetrf(n, A, lda, ipiv, info_dev, ws=None, stream=None):

@@ -29,6 +29,12 @@ struct hprmat_ctx {
     double a = 0, h2m = 0;
     cudaStream_t st = nullptr;
     std::vector<double> r, fa;  // host copies for hprmat_mesh
+    // sub-interval contexts (hprmat_setup_sector): (a_lo, a), surface values at the LEFT end (fa holds the right end's)
+    bool sector = false;
+    double a_lo = 0;
+    std::vector<double> fa_left;
+    double *d_fa_left = nullptr;
+    double2 *d_Rsec = nullptr;  // scratch: one nch x nch block
     // device
     double *d_hT = nullptr, *d_dg0 = nullptr, *d_ethr = nullptr, *d_fa = nullptr;
     double *d_KTinv = nullptr, *d_cf = nullptr, *d_g = nullptr;  // Type 3: (h2m T)^-1, centrifugal terms, (h2m T)^-1 q2
@@ -61,7 +67,8 @@ struct hprmat_ctx {
     int plan_steps[5] = {0, 1, 0, 2, 0};
     // what the last solve was, for hprmat_last_status
     int last_fac = -1, last_mode = 0, last_max_refine = 0;
-    bool last_valid = false;
+    bool last_valid = false, last_fallback = false;
+    bool reuse_factor = false;  // the next run keeps the factors of the previous one (second right-hand-side set of a sector)
     // CUDA graphs of the factorisations and triangular solves (thousands of dependent launches that depend on nothing but
     // this context's buffers): captured once on an internal stream, replayed on the caller's stream
     struct GraphEntry {
@@ -115,7 +122,7 @@ void shifted_legendre_zeros(int n, std::vector<ld> &x) {
 
 int free_ctx(hprmat_ctx *c) {
     if (!c) return 0;
-    cudaFree(c->d_KTinv); cudaFree(c->d_cf); cudaFree(c->d_g);
+    cudaFree(c->d_KTinv); cudaFree(c->d_cf); cudaFree(c->d_g); cudaFree(c->d_fa_left); cudaFree(c->d_Rsec);
     cudaFree(c->d_hT); cudaFree(c->d_dg0); cudaFree(c->d_ethr); cudaFree(c->d_fa);
     cudaFree(c->d_Voff); cudaFree(c->d_Xp); cudaFree(c->d_Pp);
     cudaFree(c->d_C); cudaFree(c->d_X); cudaFree(c->d_Rr); cudaFree(c->d_Rlo); cudaFree(c->d_V); cudaFree(c->d_R);
@@ -150,13 +157,15 @@ float ev_ms(cudaEvent_t a, cudaEvent_t b) {
 
 }  // namespace
 
-extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, double h2m, const int *lval,
-                            const double *ethr, int max_mode, void *cuda_stream) {
+// a_lo == 0: the interval (0, a) with the mesh regularised by r (hprmat_setup).  a_lo > 0: the sub-interval (a_lo, a) of a
+// propagation (hprmat_setup_sector): plain Lagrange-Legendre mesh, Bloch operators at both ends.
+static int setup_impl(hprmat_ctx **out, int nch, int nbasis, double a_lo, double a, double h2m, const int *lval,
+                      const double *ethr, int max_mode, void *cuda_stream) {
     if (!out) return -1;
     *out = nullptr;
     if (nch < 1) return -2;
     if (nbasis < 2) return -3;
-    if (!(a > 0.0)) return -4;
+    if (!(a > 0.0) || !(a_lo >= 0.0) || !(a > a_lo)) return -4;
     if (!(h2m > 0.0)) return -5;
     if (!lval) return -6;
     if (!ethr) return -7;
@@ -182,14 +191,64 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
     std::vector<double> x(nb), hT((size_t)nb * nb), dg0((size_t)N);
     c->r.resize(nb);
     c->fa.resize(nb);
+    c->sector = a_lo > 0.0;
+    c->a_lo = a_lo;
+    if (c->sector) {
+        // Sub-interval (a_lo, a), h = a - a_lo (reading R16): Lagrange functions f_i(r) = l_i(x) / sqrt(h lam_i),
+        // x = (r - a_lo)/h, l_i the Lagrange polynomials of the nb Gauss-Legendre nodes, lam_i the weights on (0,1).  With
+        // the Bloch operator at BOTH ends,  <f_i| -d2/dr2 + L(a) - L(a_lo) |f_j> = int f_i' f_j' dr
+        //   = (1/h^2) sum_k lam_k l_i'(x_k) l_j'(x_k) / sqrt(lam_i lam_j)    (Gauss quadrature, exact: degree 2 nb - 4),
+        // l_i'(x_k) from the barycentric weights w_i = 1 / prod_{m != i} (x_i - x_m):
+        //   l_i'(x_k) = (w_i / w_k) / (x_k - x_i)  (k != i),   l_k'(x_k) = - sum_{i != k} l_i'(x_k).
+        const ld h = (ld)a - (ld)a_lo;
+        std::vector<ld> lam(nb), wb(nb), D((size_t)nb * nb);
+        for (int i = 0; i < nb; ++i) {
+            const ld t = 2.0L * xl[i] - 1.0L;
+            ld pn, pm;
+            legendre_pair(nb, t, pn, pm);
+            const ld dp = (ld)nb * (t * pn - pm) / (t * t - 1.0L);
+            lam[i] = 1.0L / ((1.0L - t * t) * dp * dp);
+            ld prod = 1.0L;
+            for (int m = 0; m < nb; ++m)
+                if (m != i) prod *= (xl[i] - xl[m]);
+            wb[i] = 1.0L / prod;
+        }
+        for (int k = 0; k < nb; ++k) {
+            ld sum = 0.0L;
+            for (int i = 0; i < nb; ++i)
+                if (i != k) {
+                    D[(size_t)k * nb + i] = (wb[i] / wb[k]) / (xl[k] - xl[i]);  // l_i'(x_k)
+                    sum += D[(size_t)k * nb + i];
+                }
+            D[(size_t)k * nb + k] = -sum;
+        }
+        c->fa_left.resize(nb);
+        for (int i = 0; i < nb; ++i) {
+            x[i] = (double)xl[i];
+            c->r[i] = (double)((ld)a_lo + h * xl[i]);
+            ld l0 = wb[i], l1 = wb[i];  // l_i(0), l_i(1)
+            for (int m = 0; m < nb; ++m)
+                if (m != i) { l0 *= (0.0L - xl[m]); l1 *= (1.0L - xl[m]); }
+            c->fa_left[i] = (double)(l0 / sqrtl(h * lam[i]));
+            c->fa[i] = (double)(l1 / sqrtl(h * lam[i]));  // right end: the surface the R-matrix is propagated to
+        }
+        for (int j = 0; j < nb; ++j)
+            for (int i = 0; i < nb; ++i) {
+                ld t = 0.0L;
+                for (int k = 0; k < nb; ++k) t += lam[k] * D[(size_t)k * nb + i] * D[(size_t)k * nb + j];
+                t /= (h * h * sqrtl(lam[i] * lam[j]));
+                hT[(size_t)j * nb + i] = h2m * (double)t;
+            }
+    } else {
     for (int i = 0; i < nb; ++i) {
         x[i] = (double)xl[i];
         c->r[i] = (double)((ld)a * xl[i]);
         const ld sgn = ((nb + i + 1) & 1) ? -1.0L : 1.0L;
         c->fa[i] = (double)(sgn / sqrtl((ld)a * xl[i] * (1.0L - xl[i])));
     }
+    }
     const ld n_ = nb, a2 = (ld)a * (ld)a;
-    for (int j = 0; j < nb; ++j)
+    for (int j = 0; j < nb && !c->sector; ++j)
         for (int i = 0; i < nb; ++i) {
             const ld xi = x[i], xj = x[j];
             ld t;
@@ -338,10 +397,31 @@ extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, dou
     cudaError_t e5 = cudaStreamSynchronize(c->st);  // the host vectors go out of scope
     for (cudaError_t e : {e1, e2, e3, e4, e5})
         if (e != cudaSuccess) { free_ctx(c); return hp::cuda_fail(e, __FILE__, __LINE__); }
-    c->tab.nch = nch; c->tab.nb = nb; c->tab.a = a; c->tab.h2m = h2m;
+    c->tab.nch = nch; c->tab.nb = nb; c->tab.a = c->sector ? 1.0 : a; c->tab.h2m = h2m;  // sector: no 1/a in the contraction
+    if (c->sector) {
+        HP_ALLOC(c->d_fa_left, sizeof(double) * nb);
+        HP_ALLOC(c->d_Rsec, sizeof(double2) * (size_t)nch * nch);
+        cudaError_t s1 = cudaMemcpy(c->d_fa_left, c->fa_left.data(), sizeof(double) * nb, cudaMemcpyHostToDevice);
+        if (s1 != cudaSuccess) { free_ctx(c); return hp::cuda_fail(s1, __FILE__, __LINE__); }
+    }
     c->tab.hT = c->d_hT; c->tab.dg0 = c->d_dg0; c->tab.ethr = c->d_ethr; c->tab.fa = c->d_fa;
     *out = c;
     return HPRMAT_OK;
+}
+
+extern "C" int hprmat_setup(hprmat_ctx **out, int nch, int nbasis, double a, double h2m, const int *lval,
+                            const double *ethr, int max_mode, void *cuda_stream) {
+    return setup_impl(out, nch, nbasis, 0.0, a, h2m, lval, ethr, max_mode, cuda_stream);
+}
+
+extern "C" int hprmat_setup_sector(hprmat_ctx **out, int nch, int nbasis, double a_lo, double a_hi, double h2m, const int *lval,
+                                   const double *ethr, int max_mode, void *cuda_stream) {
+    if (!(a_lo > 0.0)) return -4;
+    if (!(a_hi > a_lo)) return -5;
+    if (max_mode & (1 << HPRMAT_TYPE3)) return -9;  // Type 3 is printed for the single interval only
+    if (max_mode == 0) max_mode = (1 << HPRMAT_FP64) | (1 << HPRMAT_MIXED) | (1 << HPRMAT_MIXED_REFINE);
+    const int rc = setup_impl(out, nch, nbasis, a_lo, a_hi, h2m, lval, ethr, max_mode, cuda_stream);
+    return rc == -4 ? -5 : rc == -5 ? -6 : rc == -6 ? -7 : rc == -7 ? -8 : rc == -8 ? -9 : rc;
 }
 
 extern "C" int hprmat_mesh(const hprmat_ctx *ctx, double *r, double *fa) {
@@ -661,9 +741,9 @@ int run(hprmat_ctx *c, Fac fac, const Problem &p, double energy, int mode, int m
     ScopedZgemmAlgo algo_scope(c->zgemm_algo);
 
     HP_CUDA(cudaEventRecord(c->ev[0], st));
-    HP_TRY(assemble(c, fac, p, energy, sync));
+    if (!c->reuse_factor) HP_TRY(assemble(c, fac, p, energy, sync));
     HP_CUDA(cudaEventRecord(c->ev[1], st));
-    HP_TRY(factor(c, fac, pivoting_fallback));
+    if (!c->reuse_factor) HP_TRY(factor(c, fac, pivoting_fallback));
     HP_CUDA(cudaEventRecord(c->ev[2], st));
     int x0_word = SC_X0;
     HP_TRY(first_solve(c, fac, &x0_word));
@@ -684,6 +764,7 @@ int run(hprmat_ctx *c, Fac fac, const Problem &p, double energy, int mode, int m
     HP_CUDA(cudaEventRecord(c->ev[5], st));
     c->have_x = true;
     c->last_fac = fac;
+    c->last_fallback = pivoting_fallback;
     c->last_mode = mode;
     c->last_max_refine = max_refine;
     c->last_valid = true;
@@ -812,6 +893,53 @@ extern "C" int hprmat_profile_graphs(const hprmat_ctx *ctx, int *captured, int *
     if (captured) *captured = nc;
     if (eager) *eager = ne;
     return HPRMAT_OK;
+}
+
+// Sector matrices of a sub-interval context (propagate.cu; reading R16): one factorisation, two sets of nch
+// right-hand sides (surface vectors of the right and of the left end), four contractions.
+extern "C" int hprmat_solve_sector(hprmat_ctx *ctx, double energy, const void *V, int mode, int max_refine, double tol,
+                                   void *Rsec, hprmat_info *info) {
+    if (!ctx || !ctx->sector) return -1;
+    if (!V) return -3;
+    if (mode != HPRMAT_FP64 && mode != HPRMAT_MIXED && mode != HPRMAT_MIXED_REFINE) return -4;
+    if (!(ctx->max_mode & (1 << mode))) return -4;
+    if (!Rsec) return -7;
+    if (!info) return -8;  // two dependent passes: the call is synchronised
+    const long nn = (long)ctx->nch * ctx->nch;
+    double2 *LL = (double2 *)Rsec, *LR = LL + nn, *RL = LL + 2 * nn, *RR = LL + 3 * nn;
+    Problem p;
+    p.V = (const double2 *)V;
+    // pass 1: right-hand sides of the RIGHT end (tab.fa): X_R -> Rsec_RR, Rsec_LR
+    int rc = solve_any(ctx, p, energy, mode, max_refine, tol, RR, info);
+    if (rc != HPRMAT_OK && rc != HPRMAT_ENOTCONVERGED) return rc;
+    HP_TRY(contract_with(ctx->st, ctx->tab, ctx->d_fa_left, ctx->d_X, ctx->n, LR));
+    // pass 2: right-hand sides of the LEFT end, same factors: X_L -> Rsec_LL, Rsec_RL
+    hprmat_info i2 = hprmat_info();
+    double bn = 0.0;
+    for (double f : ctx->fa_left) bn = std::max(bn, fabs(f));
+    HP_CUDA(cudaMemcpyAsync(ctx->d_scal + SC_BNORM, &bn, sizeof(double), cudaMemcpyHostToDevice, ctx->st));
+    const double *fa_right = ctx->tab.fa;
+    ctx->tab.fa = ctx->d_fa_left;
+    ctx->reuse_factor = true;
+    int rc2 = run(ctx, (Fac)ctx->last_fac, p, energy, mode, max_refine, tol, LL, &i2, ctx->last_fallback);
+    ctx->reuse_factor = false;
+    ctx->tab.fa = fa_right;
+    bn = 0.0;
+    for (double f : ctx->fa) bn = std::max(bn, fabs(f));
+    cudaMemcpyAsync(ctx->d_scal + SC_BNORM, &bn, sizeof(double), cudaMemcpyHostToDevice, ctx->st);
+    if (rc2 == UNUSABLE) rc2 = HPRMAT_ENOTCONVERGED;  // the first pass accepted these factors; treat as not converged
+    if (rc2 != HPRMAT_OK && rc2 != HPRMAT_ENOTCONVERGED) return rc2;
+    HP_TRY(contract_with(ctx->st, ctx->tab, fa_right, ctx->d_X, ctx->n, RL));
+    info->refine_steps = std::max(info->refine_steps, i2.refine_steps);
+    info->resid_max = std::max(info->resid_max, i2.resid_max);
+    info->backward_err = std::max(info->backward_err, i2.backward_err);
+    info->ms_solve += i2.ms_solve;
+    info->ms_refine += i2.ms_refine;
+    info->ms_contract += i2.ms_contract;
+    info->ms_total += i2.ms_total;
+    rc = std::max(rc, rc2);
+    info->status = rc;
+    return rc;
 }
 
 // Status of the last solve of this context, for calls made with info == NULL: synchronises the stream, reads the device

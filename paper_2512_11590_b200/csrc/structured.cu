@@ -612,6 +612,13 @@ __global__ void __launch_bounds__(256) contract_kernel(int nch, int nb, double p
     if (lane == 0) R[(long)c2 * nch + c1] = make_double2(pref * sr, pref * si);
 }
 
+int contract_with(cudaStream_t st, const StructTables &t, const double *fa_dev, const double2 *X, long ldx, double2 *R) {
+    const long warps = (long)t.nch * t.nch;
+    contract_kernel<<<ceil_div(warps * 32, 256), 256, 0, st>>>(t.nch, t.nb, t.h2m / t.a, fa_dev, X, ldx, R);
+    HP_LAUNCHED();
+    return 0;
+}
+
 int contract(cudaStream_t st, const StructTables &t, const double2 *X, long ldx, double2 *R) {
     const long warps = (long)t.nch * t.nch;
     contract_kernel<<<ceil_div(warps * 32, 256), 256, 0, st>>>(t.nch, t.nb, t.h2m / t.a, t.fa, X, ldx, R);

@@ -47,5 +47,7 @@ int backward_error(cudaStream_t st, long rows, int nrhs, const double2 *R, long 
                    const double *anorm_dev, const double *bnorm_dev, double *out_dev);
 int structured_anorm(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double *out_dev);
 int contract(cudaStream_t st, const StructTables &t, const double2 *X, long ldx, double2 *R);
+// same with another surface vector (sector matrices of the propagation: left / right end)
+int contract_with(cudaStream_t st, const StructTables &t, const double *fa_dev, const double2 *X, long ldx, double2 *R);
 
 }  // namespace hp

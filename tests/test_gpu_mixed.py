@@ -383,7 +383,7 @@ def test_zsolve_mixed_never_returns_a_silent_low_precision_result(kappa):
 # ---------------------------------------------------------------------------------------------------- headline size, mixed
 @pytest.mark.slow
 @pytest.mark.parametrize("cfg,mode,tol", [(3, hb.HPRMAT_MIXED_REFINE, 1e-10), (3, hb.HPRMAT_MIXED, 1e-3),
-                                          (4, hb.HPRMAT_MIXED_REFINE, 1e-10)])
+                                          (4, hb.HPRMAT_MIXED_REFINE, 1e-10), (3, hb.HPRMAT_TYPE3, 1e-3)])
 def test_rmatrix_mixed_cfg3_headline_size_certificate(cfg, mode, tol):
     """BASELINE.json configs[3] (N = 25600) in the launch configuration bench.py times, mixed modes.  The full oracle
     needs ~10 core-hours here, so correctness is certified a posteriori: since C = C^T,
@@ -397,7 +397,7 @@ def test_rmatrix_mixed_cfg3_headline_size_certificate(cfg, mode, tol):
     assert info["status"] == 0
     X = _host(ctx.get_x())
     Rg = _host(R)
-    c = certificate(w, 30.0, X, Rg, jacobi_steps=2 if mode == hb.HPRMAT_MIXED else 1)
+    c = certificate(w, 30.0, X, Rg, jacobi_steps=1 if mode == hb.HPRMAT_MIXED_REFINE else 2)
     assert c["est"] <= tol, (c, info)
     # the dropped second-order term, estimated explicitly by the oracle-side block-Jacobi solve of tests/certificate.py
     assert c["second"] <= 1e-2 * tol and c["contraction"] < 1.0, c

@@ -643,3 +643,60 @@ def test_separable_potential_has_the_analytic_phase_shift(E):
     assert abs(abs(U[0, 0]) - 1.0) < 1e-12
     assert abs(tan_d) > 0.05
     assert abs(U[0, 0] - S_exact) < 1e-8
+
+
+# ----------------------------------------------------------------- propagation over sub-intervals (reading R16)
+def test_sector_matrices_of_free_motion_match_the_closed_form():
+    """V = 0, l = 0 on (a_lo, a_hi), h = a_hi - a_lo: u = A cos k(r - a_lo) + B sin k(r - a_lo) gives
+    u(a_hi) = -cot(kh)/k u'(a_hi) + 1/(k sin kh) u'(a_lo),  u(a_lo) = -1/(k sin kh) u'(a_hi) + cot(kh)/k u'(a_lo), i.e.
+    Rsec_RR = Rsec_LL = -cot(kh)/k, Rsec_RL = Rsec_LR = -1/(k sin kh).  Pins the sector mesh, the two-sided Bloch kinetic
+    matrix, both surface vectors and the sign convention of the four blocks."""
+    a_lo, a_hi, E, nb = 3.0, 7.5, 11.0, 30
+    k = np.sqrt(E / H2M)
+    h = a_hi - a_lo
+    (LL, LR), (RL, RR) = oracle.sector_matrices(1, nb, a_lo, a_hi, H2M, [0], [0.0], E, np.zeros((nb, 1, 1), dtype=complex))
+    d, o = -1 / (k * np.tan(k * h)), -1 / (k * np.sin(k * h))
+    assert abs(RR[0, 0] - d) < 1e-11 * abs(d) and abs(LL[0, 0] - d) < 1e-11 * abs(d)
+    assert abs(RL[0, 0] - o) < 1e-11 * abs(o) and abs(LR[0, 0] - o) < 1e-11 * abs(o)
+
+
+def test_sector_tables_lagrange_and_symmetry_properties():
+    nb, a_lo, a_hi = 12, 2.0, 5.0
+    r, faL, faR, T = oracle.sector_tables(nb, a_lo, a_hi)
+    x, lam, _, _ = oracle.mesh(nb, 1.0)
+    assert np.allclose(r, a_lo + (a_hi - a_lo) * x, rtol=1e-15)
+    assert np.allclose(T, T.T, rtol=0, atol=1e-12 * np.abs(T).max())
+    # sum_i sqrt(h lam_i) f_i(r) = 1 (the Lagrange polynomials sum to one): at both ends, and its derivative vanishes: T 1~ = 0
+    w = np.sqrt((a_hi - a_lo) * lam)
+    assert abs(np.dot(w, faL) - 1) < 1e-12 and abs(np.dot(w, faR) - 1) < 1e-12
+    assert np.abs(T @ w).max() < 1e-10 * np.abs(T).max()
+
+
+@pytest.mark.parametrize("lval,Vdepth", [([0], 0.0), ([2], 0.0), ([3], 30.0)])
+def test_propagated_rmatrix_matches_the_closed_form_of_a_constant_potential(lval, Vdepth):
+    """R at a_2 obtained from the single-interval R at a_1 and the sector (a_1, a_2) must be F_l(K a_2)/(K a_2 F_l'(K a_2)):
+    sees the centrifugal term on the shifted mesh and the propagation formula."""
+    a1, a2, E, nb = 4.0, 9.0, 13.0, 40
+    V1 = np.full((nb, 1, 1), -Vdepth, dtype=complex)
+    R1 = oracle.rmatrix(1, nb, a1, H2M, lval, [0.0], E, V1)
+    Rsec = oracle.sector_matrices(1, nb, a1, a2, H2M, lval, [0.0], E, V1)
+    R2 = oracle.propagate(a1, a2, R1, Rsec)
+    K = np.sqrt((E + Vdepth) / H2M)
+    assert abs(R2[0, 0] - R_constant_potential(lval[0], K, a2)) < 1e-9 * max(1.0, abs(R2[0, 0]))
+
+
+def test_propagation_over_two_sub_intervals_equals_the_single_interval_rmatrix():
+    """Coupled channels with a closed one and absorption: R(a) from (0, a/2) + (a/2, a) equals R(a) from (0, a) up to the
+    discretisation error of the two meshes (both converged here), and stays symmetric."""
+    w = make_workload(0)
+    a1, E, nb = 0.45 * w.a, 2.5, 50
+    r_full = oracle.mesh(nb, w.a)[2]
+    R_full = oracle.rmatrix(w.nch, nb, w.a, w.h2m, w.lval, w.ethr, E, make_workload(0, nb=nb).potential(r_full))
+    wl = make_workload(0, nb=nb)
+    R1 = oracle.rmatrix(w.nch, nb, a1, w.h2m, w.lval, w.ethr, E, wl.potential(oracle.mesh(nb, a1)[2]))
+    rs = oracle.sector_tables(nb, a1, w.a)[0]
+    Rsec = oracle.sector_matrices(w.nch, nb, a1, w.a, w.h2m, w.lval, w.ethr, E, wl.potential(rs))
+    R2 = oracle.propagate(a1, w.a, R1, Rsec)
+    assert np.abs(R2 - R_full).max() / np.abs(R_full).max() < 1e-8
+    assert np.abs(R2 - R2.T).max() < 1e-11 * np.abs(R2).max()
+    assert np.abs(Rsec[0][1] - Rsec[1][0].T).max() < 1e-11 * np.abs(Rsec[0][1]).max()
