@@ -6,8 +6,9 @@ What is compared:
     long-double residual r of the GPU solution, the oracle-evaluated backward error of that r against 50 N 2^-53 (FP64,
     mixed+refine), and an explicit estimate of the dropped second-order term;
   * configs[1], one energy per mode: the FULL long-double oracle (orc_rmatrix, ~17 s), R and X element by element;
-  * configs[2], E = 27.5 MeV: the stored oracle R (tests/golden/oracle_R_cfg2_E27.5.npz, written once by
-    tests/golden/make_oracle_R.py from oracle/ only, keyed by a hash of the inputs).
+  * configs[2], E = 27.5 MeV, and configs[3] (the headline size N = 25600), E = 30 MeV: the stored oracle R
+    (tests/golden/oracle_R_cfg2_E27.5.npz, oracle_R_cfg3_E30.npz: written once by tests/golden/make_oracle_R.py from oracle/
+    only -- 10 min / 57 min of the big-N oracle on 8 host threads --, keyed by a hash of the inputs).
 Tolerances (north_star): FP64 and mixed+refine <= 1e-10 in R, backward error <= 50 N 2^-53; mixed without refinement <= 1e-3.
 """
 import os
@@ -85,3 +86,25 @@ def test_cfg1_full_size_energy_sweep(mode_name, full_at):
 def test_cfg2_full_size_energy_sweep(mode_name):
     """configs[2]: Nc = 128, Nb = 100 (N = 12800), a = 15 fm, 5 energies, FP64 / mixed without refinement / mixed+refinement."""
     _sweep(2, mode_name, golden_at=27.5)
+
+
+@pytest.mark.parametrize("mode_name", ["fp64", "mixed_refine", "mixed", "type3"])
+def test_cfg3_headline_size_against_the_stored_oracle_run(mode_name):
+    """configs[3]: Nc = 256, Nb = 100 (N = 25600), E = 30 MeV, in the launch configuration bench.py times: the whole R-matrix
+    against the once-only oracle run (57 min of the big-N oracle), element by element; FP64 and mixed+refinement <= 1e-10,
+    the unrefined modes <= 1e-3."""
+    w = make_workload(3)
+    mode = {**MODE, "type3": hb.HPRMAT_TYPE3}[mode_name]
+    tol = 1e-10 if mode in (hb.HPRMAT_FP64, hb.HPRMAT_MIXED_REFINE) else 1e-3
+    path = golden_path(3, 30.0)
+    assert os.path.exists(path), f"{path} missing: run tests/golden/make_oracle_R.py --cfg 3 --energy 30"
+    g = np.load(path)
+    ro = oracle.mesh(w.nb, w.a)[2]
+    assert str(g["key"]) == input_key(w, 30.0, w.potential(ro)), "stored oracle R belongs to other inputs"
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
+    r, _ = ctx.mesh()
+    R, info = ctx.solve(30.0, torch.from_numpy(w.potential(r)).to(DEV), mode)
+    err = _relmax(_host(R), g["R"])
+    print(f"cfg3 {mode_name}: max|R - R_oracle|/max|R_oracle| = {err:.2e}, {info}")
+    assert info["status"] == hb.HPRMAT_OK and err <= tol, (err, info)
+    ctx.destroy()
