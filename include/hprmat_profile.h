@@ -29,8 +29,9 @@ long long hprmat_launch_count(void);
 
 /* Which tcgen05 kernel serves the planar complex64 GEMM (hprmat_cgemm_tf32 and every such product inside the mixed modes):
  * 0 = automatic (default: the persistent kernel, CTA pairs / cta_group::2 when there is more than one 128-row tile),
- * 1 = the one-tile-per-CTA kernel (cgemm.cu), 2 = persistent single CTAs, 3 = persistent CTA pairs.  Any other value only
- * queries.  Returns the setting in force.  Process-wide; for A/B measurements. */
+ * 1 = the one-tile-per-CTA kernel (cgemm.cu), 2 = persistent single CTAs, 3 / 4 = persistent CTA pairs with 256 x 128 /
+ * 256 x 256 tiles, 5 = as 0 but the cluster split-K kernel (cgemm_splitk.cu) wherever its preconditions hold.  Any other
+ * value only queries.  Returns the setting in force.  Process-wide; for A/B measurements. */
 int hprmat_profile_cgemm_variant(int variant);
 
 /* How many launch sequences (factorisations, triangular solves) of the context are replayed from CUDA graphs (captured) and

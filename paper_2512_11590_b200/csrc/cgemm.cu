@@ -265,7 +265,7 @@ int cgemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, 
     if ((A.ld | B.ld) & 3) return -7;
     const int variant = cgemm_variant_in_force();
     const long tiles128 = (long)ceil_div(m, CG_BM) * ceil_div(n, 128);
-    if (variant >= 2 || (variant == 0 && m > CG_BM && tiles128 >= 2L * kNumSMs)) {
+    if ((variant >= 2 && variant <= 4) || (variant == 0 && m > CG_BM && tiles128 >= 2L * kNumSMs)) {
         // Two waves of work or more: the persistent kernel (cgemm2.cu).  Deep K and enough tiles -> pair tiles of 256 x 256
         // (N = 256 MMAs keep the tensor pipe ~18 % busier than N = 128 ones; their un-overlapped epilogue is < 5 % of such a
         // tile); otherwise pair tiles of 256 x 128 with double-buffered accumulators (epilogue under the next main loop).
@@ -278,6 +278,15 @@ int cgemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, 
     // grid covers most of the GPU -- a 1024 x 1024 product is 8 x 8 tiles of 128 x 128 (16 % of the SMs) but 8 x 32 of
     // 128 x 32.  C aliasing A (the in-place L21 product) needs all of n inside one tile.
     const bool in_place_a = C.re == A.re;
+    // Few tiles and a deep inner dimension (substitution steps, products with the kept block inverses): a cluster of CTAs per
+    // tile splits K (cgemm_splitk.cu) -- as many slices as keep the grid within one wave, at least 8 k-steps of 32 each
+    if ((variant == 0 || variant == 5) && !in_place_a && C.re != B.re && n > 64) {
+        int slices = 0;
+        for (int sl = 8; sl >= 2; sl /= 2)
+            if (tiles128 * sl <= kNumSMs && k >= 256 * sl) { slices = sl; break; }
+        if (variant == 5 && slices == 0 && k >= 64) slices = 2;
+        if (slices) return cgemm_splitk(st, m, n, k, alpha, A, B, beta, C, slices);
+    }
     const int natural = n <= 32 ? 32 : n <= 64 ? 64 : 128;  // narrowest tile that still holds all of n
     int bn = natural;
     if (variant == 0 && !in_place_a && tiles128 < 96) bn = std::min(natural, 2 * tiles128 >= 96 ? 64 : 32);
@@ -301,7 +310,7 @@ int gemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, d
 }  // namespace hp
 
 extern "C" int hprmat_profile_cgemm_variant(int variant) {
-    if (variant >= 0 && variant <= 4) hp::g_cgemm_variant.store(variant);
+    if (variant >= 0 && variant <= 5) hp::g_cgemm_variant.store(variant);
     return hp::g_cgemm_variant.load();
 }
 

@@ -23,6 +23,9 @@ int gemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, d
 // epilogue also counts results with |re| + |im| > chk_thr.  C may alias A when n <= 128, B when m <= 128 (pair == false).
 int cgemm2(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C, int shape, float chk_thr = 0.f,
            int *chk_count = nullptr);
+// few output tiles, deep K: every 128 x 128 tile by a cluster of `slices` (2, 4, 8) CTAs along K, deterministic reduction through
+// distributed shared memory (cgemm_splitk.cu).  C must not alias A or B.
+int cgemm_splitk(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C, int slices);
 // FP32-class accuracy variant for the planar complex64 type (3xTF32, cgemm3.cu); C may alias B when m <= 128, beta == 0
 int cgemm3(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
 int cgemm3_batched(cudaStream_t st, int m, int n, int k, double alpha, CView A, long strideA, CView B, long strideB, double beta,

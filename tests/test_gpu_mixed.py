@@ -36,7 +36,8 @@ def _rup(x, q):
     return (x + q - 1) // q * q
 
 
-@pytest.fixture(params=[0, 1, 2, 3, 4], ids=["auto", "one_tile_per_cta", "persistent", "persistent_pairs", "persistent_pairs_n256"])
+@pytest.fixture(params=[0, 1, 2, 3, 4, 5], ids=["auto", "one_tile_per_cta", "persistent", "persistent_pairs", "persistent_pairs_n256",
+                                               "split_k_clusters"])
 def cgemm_variant(request):
     """every tcgen05 kernel that can serve the planar complex64 GEMM (include/hprmat_profile.h)"""
     prev = hb.hprmat_profile_cgemm_variant()
@@ -48,7 +49,8 @@ def cgemm_variant(request):
 @pytest.mark.parametrize("m,n,k,alpha,beta", [
     (128, 128, 32, 1.0, 0.0), (128, 128, 64, -1.0, 1.0), (256, 384, 96, -1.0, 1.0), (100, 50, 37, 1.0, 0.0),
     (257, 129, 65, -1.0, 1.0), (32, 700, 32, 1.0, 0.0), (1000, 333, 200, -1.0, 1.0), (5, 3, 1, 2.0, -0.5),
-    (640, 512, 1024, -1.0, 1.0), (1, 1, 8, 1.0, 1.0), (3000, 2900, 160, -1.0, 1.0), (40000, 64, 64, 1.0, 0.0)])
+    (640, 512, 1024, -1.0, 1.0), (1, 1, 8, 1.0, 1.0), (3000, 2900, 160, -1.0, 1.0), (40000, 64, 64, 1.0, 0.0),
+    (1024, 256, 2080, -1.0, 1.0), (1000, 130, 4100, 1.0, 0.0), (300, 200, 530, -1.0, 1.0)])
 def test_cgemm_tf32_matches_definition(m, n, k, alpha, beta, cgemm_variant):
     rng = np.random.default_rng(m * 1000003 + n * 1009 + k)
     A = (rng.uniform(-1, 1, (m, k)) + 1j * rng.uniform(-1, 1, (m, k))).astype(np.complex64).astype(np.complex128)
@@ -398,9 +400,11 @@ def test_rmatrix_mixed_cfg3_headline_size_certificate(cfg, mode, tol):
     X = _host(ctx.get_x())
     Rg = _host(R)
     c = certificate(w, 30.0, X, Rg, jacobi_steps=1 if mode == hb.HPRMAT_MIXED_REFINE else 2)
-    assert c["est"] <= tol, (c, info)
-    # the dropped second-order term, estimated explicitly by the oracle-side block-Jacobi solve of tests/certificate.py
-    assert c["second"] <= 1e-2 * tol and c["contraction"] < 1.0, c
+    # first-order term plus the dropped second-order one, the latter estimated explicitly by the oracle-side block-Jacobi solve of
+    # tests/certificate.py (doubled: the estimate is good to a factor); for the refined mode it must be negligible
+    assert c["est"] + 2.0 * c["second"] <= tol and c["contraction"] < 1.0, (c, info)
+    if mode == hb.HPRMAT_MIXED_REFINE:
+        assert c["second"] <= 1e-2 * tol, c
     if mode == hb.HPRMAT_MIXED_REFINE:
         assert c["backward_err"] <= 50 * w.n * 2.0 ** -53, c              # the ORACLE's residual of the GPU's X
     assert _relmax(Rg, Rg.T) <= 10 * tol
