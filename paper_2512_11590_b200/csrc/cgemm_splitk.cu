@@ -39,12 +39,14 @@ __device__ __forceinline__ uint32_t cluster_nctarank() {
     asm volatile("mov.u32 %0, %%cluster_nctarank;\n" : "=r"(r));
     return r;
 }
+// not volatile: the loads of all slices of a chunk are independent and must be in flight together (DSMEM latency ~0.1 us)
 __device__ __forceinline__ float4 ld_cluster_f4(uint32_t addr) {
     float4 v;
-    asm volatile("ld.shared::cluster.v4.f32 {%0,%1,%2,%3}, [%4];\n" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    asm("ld.shared::cluster.v4.f32 {%0,%1,%2,%3}, [%4];\n" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
     return v;
 }
 
+template <int S>
 __global__ void __launch_bounds__(SK_NT, 1)
     cgemm_splitk_kernel(const __grid_constant__ SkMaps maps, int M, int N, int K, float alpha, float beta, float *__restrict__ Cre,
                         float *__restrict__ Cim, long ldc, int tiles_m) {
@@ -56,7 +58,7 @@ __global__ void __launch_bounds__(SK_NT, 1)
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tmem_full + 1);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t S = cluster_nctarank(), rank = cluster_ctarank();
+    const uint32_t rank = cluster_ctarank();
     const int tile = (int)(blockIdx.x / S);
     const int tm = tile % tiles_m, tn = tile / tiles_m;
     const int m0 = tm * SK_BM, n0 = tn * SK_BN;
@@ -166,13 +168,18 @@ __global__ void __launch_bounds__(SK_NT, 1)
         for (int c = t; c < SK_BN * nrc; c += 128) {
             const int cl = c / nrc, r = r0 + 4 * (c - cl * nrc);
             const long col = (long)n0 + cl;
-            float4 sr = make_float4(0.f, 0.f, 0.f, 0.f), si = sr;
-            for (uint32_t s = 0; s < S; ++s) {
-                const uint32_t remote = mapa_u32(base, s);
-                const float4 pr = ld_cluster_f4(remote + (uint32_t)(((size_t)cl * SK_PLD + r) * 4));
-                const float4 pi = ld_cluster_f4(remote + (uint32_t)(((size_t)(SK_BN + cl) * SK_PLD + r) * 4));
-                sr.x += pr.x; sr.y += pr.y; sr.z += pr.z; sr.w += pr.w;
-                si.x += pi.x; si.y += pi.y; si.z += pi.z; si.w += pi.w;
+            float4 pr[S], pi[S];
+#pragma unroll
+            for (int s = 0; s < S; ++s) {  // all 2 S loads in flight, then the sums in slice order
+                const uint32_t remote = mapa_u32(base, (uint32_t)s);
+                pr[s] = ld_cluster_f4(remote + (uint32_t)(((size_t)cl * SK_PLD + r) * 4));
+                pi[s] = ld_cluster_f4(remote + (uint32_t)(((size_t)(SK_BN + cl) * SK_PLD + r) * 4));
+            }
+            float4 sr = pr[0], si = pi[0];
+#pragma unroll
+            for (int s = 1; s < S; ++s) {
+                sr.x += pr[s].x; sr.y += pr[s].y; sr.z += pr[s].z; sr.w += pr[s].w;
+                si.x += pi[s].x; si.y += pi[s].y; si.z += pi[s].z; si.w += pi[s].w;
             }
             if (col < N) {
                 const float vr[4] = {sr.x, sr.y, sr.z, sr.w}, vi[4] = {si.x, si.y, si.z, si.w};
@@ -205,9 +212,10 @@ int cgemm_splitk(cudaStream_t st, int m, int n, int k, double alpha, CView A, CV
     if (((uintptr_t)A.re | (uintptr_t)A.im | (uintptr_t)B.re | (uintptr_t)B.im) & 15) return -6;
     if ((A.ld | B.ld) & 3) return -7;
     if (slices != 2 && slices != 4 && slices != 8) return -10;
-    auto kern = cgemm_splitk_kernel;
-    static SmemCfg cfg;
-    HP_TRY(configure_smem(cfg, kern, SK_SMEM));
+    static SmemCfg cfg2, cfg4, cfg8;
+    HP_TRY(configure_smem(cfg2, cgemm_splitk_kernel<2>, SK_SMEM));
+    HP_TRY(configure_smem(cfg4, cgemm_splitk_kernel<4>, SK_SMEM));
+    HP_TRY(configure_smem(cfg8, cgemm_splitk_kernel<8>, SK_SMEM));
     SkMaps maps;
     const int kk = k > 0 ? k : 1;
     HP_TRY(make_map(&maps.a_re, A.re, m, kk, A.ld, 32, SK_KC, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B));
@@ -227,7 +235,10 @@ int cgemm_splitk(cudaStream_t st, int m, int n, int k, double alpha, CView A, CV
     attr[0].val.clusterDim.z = 1;
     lc.attrs = attr;
     lc.numAttrs = 1;
-    HP_CUDA(cudaLaunchKernelEx(&lc, kern, maps, m, n, k, (float)alpha, (float)beta, C.re, C.im, C.ld, tiles_m));
+    const float al = (float)alpha, be = (float)beta;
+    if (slices == 8) HP_CUDA(cudaLaunchKernelEx(&lc, cgemm_splitk_kernel<8>, maps, m, n, k, al, be, C.re, C.im, C.ld, tiles_m));
+    else if (slices == 4) HP_CUDA(cudaLaunchKernelEx(&lc, cgemm_splitk_kernel<4>, maps, m, n, k, al, be, C.re, C.im, C.ld, tiles_m));
+    else HP_CUDA(cudaLaunchKernelEx(&lc, cgemm_splitk_kernel<2>, maps, m, n, k, al, be, C.re, C.im, C.ld, tiles_m));
     HP_LAUNCHED();
     return 0;
 }
