@@ -190,6 +190,11 @@ def main():
     ap.add_argument("--fp64-algo", type=int, default=0, choices=[0, 1, 2],
                     help="what the FP64 LU factors: 1 = C - E I (the paper's Type 1), 2 = the block-preconditioned matrix with "
                          "verified diagonal pivots; 0 = the library default (2)")
+    ap.add_argument("--cgemm-variant", type=int, default=0, choices=[0, 1, 2, 3, 4, 5],
+                    help="which tcgen05 kernel serves the planar complex64 GEMM (include/hprmat_profile.h): 0 = the library's "
+                         "dispatch, 1 = round 1's one-tile-per-CTA kernel everywhere, 2-4 = persistent variants, 5 = split-K "
+                         "wherever possible; for A/B measurements")
+    ap.add_argument("--no-graphs", action="store_true", help="plain stream launches instead of CUDA-graph replay (A/B)")
     ap.add_argument("--zgemm-algo", type=int, default=0, choices=[0, 3, 4],
                     help="real decomposition of the complex128 GEMM (3M / 4M); 0 = the library default")
     args = ap.parse_args()
@@ -204,6 +209,8 @@ def main():
         hb.hprmat_zgemm_algo(args.zgemm_algo)
     if args.fp64_algo:
         hb.hprmat_fp64_algo(args.fp64_algo)
+    if args.cgemm_variant:
+        hb.hprmat_profile_cgemm_variant(args.cgemm_variant)
     full = not args.quick
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -233,6 +240,8 @@ def main():
         ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
         if fp64_algo:
             ctx.set_option(hb.HPRMAT_OPT_FP64_ALGO, fp64_algo)
+        if args.no_graphs:
+            ctx.set_option(hb.HPRMAT_OPT_GRAPHS, 0)
         r, _ = ctx.mesh()
         V_host = torch.from_numpy(w.potential(r)).pin_memory()
         V = V_host.to("cuda")
@@ -295,7 +304,9 @@ def main():
             hw_ratio = 0.75 if (mode == hb.HPRMAT_FP64 and hb.hprmat_zgemm_algo() == 3) else 1.0
             ach = ach_conv * hw_ratio
             tkey = "fp64" if mode == hb.HPRMAT_FP64 else "tf32"
-            kname = ("zgemm3m_kernel" if hw_ratio < 1 else "zgemm_kernel") if mode == hb.HPRMAT_FP64 else "cgemm_tf32_kernel"
+            kname = ("zgemm3m_kernel" if hw_ratio < 1 else "zgemm_kernel") if mode == hb.HPRMAT_FP64 else (
+                "cgemm2_kernel<2,256> / <2,128> (persistent CTA pairs)" if hb.hprmat_profile_cgemm_variant() == 0 else
+                f"complex64 GEMM variant {hb.hprmat_profile_cgemm_variant()}")
             roof = {"bound": "tensor", "kernel": kname + " (trailing update A22 -= L21 U12 of the LU)", "achieved": ach,
                     "peak": peak, "unit": "TFLOP/s", "achieved_8mnk_convention": ach_conv,
                     "hardware_flops_per_complex_mac": 8 * hw_ratio, "frac": ach / peak,

@@ -258,7 +258,18 @@ int launch_cgemm(cudaStream_t st, int m, int n, int k, float alpha, CView A, CVi
 static std::atomic<int> g_cgemm_variant{0};
 int cgemm_variant_in_force() { return g_cgemm_variant.load(std::memory_order_relaxed); }
 
+static int cgemm_impl(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C, unsigned *wave_ctr);
 int cgemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C) {
+    return cgemm_impl(st, m, n, k, alpha, A, B, beta, C, nullptr);
+}
+int cgemm_ws(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C, unsigned *wave_ctr) {
+    const bool prof = prof_enabled() && m > 0 && n > 0 && k > 0;
+    if (prof) prof_begin(st, 8.0 * m * n * k);
+    const int rc = cgemm_impl(st, m, n, k, alpha, A, B, beta, C, wave_ctr);
+    if (prof) prof_end(st);
+    return rc;
+}
+static int cgemm_impl(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C, unsigned *wave_ctr) {
     if (m <= 0 || n <= 0) return 0;
     if (k <= 0 && beta == 1.0) return 0;
     if (((uintptr_t)A.re | (uintptr_t)A.im | (uintptr_t)B.re | (uintptr_t)B.im) & 15) return -6;
@@ -272,7 +283,7 @@ int cgemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, 
         // Crossover measured on B200 between k = 2048 and 3072 (profiles/r02_cgemm.md).
         const bool deep = k >= 2560 && (long)ceil_div(m, 256) * ceil_div(n, 256) >= 4L * (kNumSMs / 2);
         const int shape = variant == 0 ? (deep ? 2 : 1) : variant - 2;
-        return cgemm2(st, m, n, k, alpha, A, B, beta, C, shape);
+        return cgemm2(st, m, n, k, alpha, A, B, beta, C, shape, 0.f, nullptr, wave_ctr);
     }
     // Less than two waves: one tile per CTA (no persistent-loop prologue, no cluster launch), with the tile NARROWED until the
     // grid covers most of the GPU -- a 1024 x 1024 product is 8 x 8 tiles of 128 x 128 (16 % of the SMs) but 8 x 32 of

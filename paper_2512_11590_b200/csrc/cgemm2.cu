@@ -32,6 +32,7 @@ namespace {
 constexpr int G2_BM = 128;   // rows of C per CTA (UMMA M = 128 * NCTA)
 constexpr int G2_KC = 32;    // floats of K per stage = one 128-byte swizzle row
 constexpr int G2_NT = 192;
+constexpr int G2_MAX_WAVES = 256;  // counters of the wave barrier (G2Args::wave_ctr)
 constexpr int G2_TMEM = 512; // BN = 128: two accumulator stages of (Dr | Di) = 2 x 2 x 128 columns; BN = 256: one stage
 
 template <int NCTA, int BN> struct G2Cfg {
@@ -57,6 +58,7 @@ struct G2Args {
     int group;              // rasterisation group (tile rows walked before stepping a tile column)
     float chk_thr;          // epilogue check: count |re| + |im| > chk_thr (or NaN) into *chk_count when non-null
     int *chk_count;
+    unsigned *wave_ctr;     // non-null: one zeroed counter per wave of tiles; the producers of all CTAs meet before each wave
 };
 
 template <int NCTA, int BN>
@@ -109,7 +111,18 @@ __global__ void __launch_bounds__(G2_NT, 1)
         if (lane == 0) {
             const uint32_t full0 = NCTA == 2 ? mapa_u32(smem_u32(&full[0]), 0) : smem_u32(&full[0]);
             long it = 0;
-            for (int t = cluster_id; t < ntiles; t += nclusters) {
+            int wave = 0;
+            for (int t = cluster_id; t < ntiles; t += nclusters, ++wave) {
+                if (p.wave_ctr != nullptr && wave > 0) {
+                    // Wave barrier: CTA pairs that finish a tile early would otherwise run ahead into the next wave alone and
+                    // stream its operands from HBM a second time when the others follow (L2 holds ~100 k-steps of a wave).
+                    // All CTAs that own a tile in this wave are resident (one CTA per SM, grid <= SM count), so this cannot
+                    // deadlock; it costs one L2 round trip per tile of >= 100 us.
+                    const unsigned parts = (unsigned)min(nclusters, ntiles - wave * nclusters) * NCTA;
+                    atomicAdd(&p.wave_ctr[wave], 1u);
+                    while (*(volatile unsigned *)&p.wave_ctr[wave] < parts) {
+                    }
+                }
                 int tm, tn;
                 raster(t, p.tiles_m, p.tiles_n, p.group, tm, tn);
                 const int m0 = tm * (G2_BM * NCTA) + (int)rank * G2_BM;
@@ -265,7 +278,7 @@ __global__ void __launch_bounds__(G2_NT, 1)
 
 template <int NCTA, int BN>
 int launch_cgemm2(cudaStream_t st, int m, int n, int k, float alpha, CView A, CView B, float beta, CView C, float chk_thr,
-                  int *chk_count) {
+                  int *chk_count, unsigned *wave_ctr) {
     typedef G2Cfg<NCTA, BN> Cfg;
     constexpr int G2_BN = BN;
     auto kern = cgemm2_kernel<NCTA, BN>;
@@ -289,6 +302,12 @@ int launch_cgemm2(cudaStream_t st, int m, int n, int k, float alpha, CView A, CV
     p.chk_count = chk_count;
     const long ntiles = (long)p.tiles_m * p.tiles_n;
     const int nclusters = (int)std::min<long>(ntiles, kNumSMs / NCTA);
+    const long waves = (ntiles + nclusters - 1) / nclusters;
+    p.wave_ctr = nullptr;
+    if (wave_ctr != nullptr && waves > 1 && waves <= G2_MAX_WAVES && k >= 1024) {  // long tiles only: the barrier is per tile
+        HP_CUDA(cudaMemsetAsync(wave_ctr, 0, sizeof(unsigned) * (size_t)waves, st));
+        p.wave_ctr = wave_ctr;
+    }
     cudaLaunchConfig_t lc = {};
     lc.gridDim = dim3(nclusters * NCTA);
     lc.blockDim = dim3(G2_NT);
@@ -314,14 +333,14 @@ int launch_cgemm2(cudaStream_t st, int m, int n, int k, float alpha, CView A, CV
 // n <= 128 and beta == 0.  chk_count != nullptr: *chk_count is incremented (by some positive amount) if any result has
 // |re| + |im| > chk_thr or is NaN.
 int cgemm2(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C, int shape, float chk_thr,
-           int *chk_count) {
+           int *chk_count, unsigned *wave_ctr) {
     if (m <= 0 || n <= 0) return 0;
     if (k <= 0 && beta == 1.0 && !chk_count) return 0;
     if (((uintptr_t)A.re | (uintptr_t)A.im | (uintptr_t)B.re | (uintptr_t)B.im) & 15) return -6;
     if ((A.ld | B.ld) & 3) return -7;
-    if (shape == 2) return launch_cgemm2<2, 256>(st, m, n, k, (float)alpha, A, B, (float)beta, C, chk_thr, chk_count);
-    if (shape == 1) return launch_cgemm2<2, 128>(st, m, n, k, (float)alpha, A, B, (float)beta, C, chk_thr, chk_count);
-    return launch_cgemm2<1, 128>(st, m, n, k, (float)alpha, A, B, (float)beta, C, chk_thr, chk_count);
+    if (shape == 2) return launch_cgemm2<2, 256>(st, m, n, k, (float)alpha, A, B, (float)beta, C, chk_thr, chk_count, wave_ctr);
+    if (shape == 1) return launch_cgemm2<2, 128>(st, m, n, k, (float)alpha, A, B, (float)beta, C, chk_thr, chk_count, wave_ctr);
+    return launch_cgemm2<1, 128>(st, m, n, k, (float)alpha, A, B, (float)beta, C, chk_thr, chk_count, wave_ctr);
 }
 
 }  // namespace hp

@@ -53,6 +53,7 @@ template <class V> size_t LuWork<V>::carve(void *base, int n_) {
         tmp = alloc_view<V>(p, sbld, std::max<long>(n, 256));
     }
     refuted = (int *)take(256);
+    wave_sync = (unsigned *)take(sizeof(unsigned) * 8 * 256);
     perm = (int *)take(sizeof(int) * (size_t)nblk * PERM_STRIDE);
     cand_val = (T *)take(sizeof(T) * 2 * MAXG);
     cand_row = (int *)take(sizeof(int) * 2 * MAXG);
@@ -332,7 +333,10 @@ static int lu_gemm(const LuWork<ZView> &, cudaStream_t st, int m, int n, int k, 
 }
 static int lu_gemm(const LuWork<CView> &wk, cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta,
                    CView C) {
-    return wk.accurate ? cgemm3(st, m, n, k, alpha, A, B, beta, C) : gemm(st, m, n, k, alpha, A, B, beta, C);
+    if (wk.accurate) return cgemm3(st, m, n, k, alpha, A, B, beta, C);
+    LuWork<CView> &w = const_cast<LuWork<CView> &>(wk);
+    unsigned *slot = w.wave_sync ? w.wave_sync + 256 * (w.wave_next++ & 7) : nullptr;
+    return cgemm_ws(st, m, n, k, alpha, A, B, beta, C, slot);
 }
 template <class V> struct IsPlanar { static constexpr bool value = false; };
 template <> struct IsPlanar<CView> { static constexpr bool value = true; };

