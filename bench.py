@@ -53,10 +53,12 @@ def peaks():
 NCU_TRAFFIC = {
     "fp64": {"bytes": 5.575929e9 + 2.604247e9, "launch": "hprmat_zgemm (3M kernel) m=n=12800 k=1024",
              "algorithmic_bytes": 16.0 * (2 * 12800 * 1024 + 2 * 12800 * 12800),
-             "capture": "profiles/r01_ncu_full.md section 5", "commit": "9ed5626 (round 1; kernel unchanged since)"},
-    "tf32": {"bytes": 10.820277e9 + 1.285462e9, "launch": "hprmat_cgemm_tf32 m=n=12800 k=6400 (128 x 256 tiles)",
-             "algorithmic_bytes": 8.0 * (2 * 12800 * 6400 + 2 * 12800 * 12800),
-             "capture": "profiles/r01_ncu_full.md section 5", "commit": "9ed5626 (round 1; kernel unchanged since)"},
+             "capture": "profiles/r01_ncu_full.md section 5", "commit": "9ed5626 (round 1; zgemm3m.cu unchanged since)"},
+    "tf32": {"bytes": 19.761905e9 + 1.207496e9,
+             "launch": "cgemm2_kernel<2,256> inside the cfg-3 mixed LU: the root trailing update m=n=k=12800",
+             "algorithmic_bytes": 8.0 * (12800 * 12800 + 12800 * 12800 + 2 * 12800 * 12800),
+             "capture": "profiles/r02_cgemm.md section 1 (ncu --set full)", "commit": "493995d",
+             "note": "4.0x algorithmic; the C-stationary minimum for waves of 74 pair tiles of 256 x 256 is 3.4x"},
 }
 
 _DMMA_PEAK = None
