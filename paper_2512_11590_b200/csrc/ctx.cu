@@ -548,7 +548,10 @@ template <class F> int replay(hprmat_ctx *c, int kind, int flags, const void *ke
 
 template <class V> int getrs_replay(hprmat_ctx *c, int nrhs, V A, V B, LuWork<V> &wk, const void *key, int variant) {
     const int n = c->n;
-    return replay(c, 1, nrhs * 4 + variant, key, [&](cudaStream_t s) { return getrs<V>(s, n, nrhs, A, B, wk); });
+    // the launch sequence depends on the right-hand-side count, the factored matrix and on whether the factorisation has
+    // interchanges (speculate) or FP32-class products (accurate)
+    const int flags = ((nrhs * 4 + variant) * 2 + (wk.speculate ? 1 : 0)) * 2 + (wk.accurate ? 1 : 0);
+    return replay(c, 1, flags, key, [&](cudaStream_t s) { return getrs<V>(s, n, nrhs, A, B, wk); });
 }
 
 // ---- stages ---------------------------------------------------------------------------------------------------------------

@@ -535,7 +535,9 @@ template <class V> int getrs(cudaStream_t st, int n, int nrhs, V A, V B, LuWork<
     if (n <= 0 || nrhs <= 0) return 0;
     ProfCat pc(PROF_SOLVE);
     wk.use_big = true;
-    HP_TRY(laswp(st, B, 0, nrhs, 0, 0, wk.perm, 0, wk.nblk));
+    // a factorisation with verified diagonal pivots has no interchanges (all swap batches are empty; a refuted one is never
+    // solved with: the caller refactors with pivoting)
+    if (!wk.speculate) HP_TRY(laswp(st, B, 0, nrhs, 0, 0, wk.perm, 0, wk.nblk));
     // the right-hand sides and the solution are O(1): FP32-class diagonal-block products (3xTF32 for the complex64 type)
     HP_TRY(trsm_lower(st, A, 0, n, B, nrhs, wk, true));
     return trsm_upper(st, A, 0, n, B, nrhs, wk, true);

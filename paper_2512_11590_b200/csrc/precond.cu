@@ -88,17 +88,23 @@ __global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const doub
         const double2 pv = rowk[k];
         const bool sing = (pv.x == 0.0 && pv.y == 0.0);
         const double2 ip = sing ? make_double2(0.0, 0.0) : crecip(pv);
-        // a[i][j] <- a[i][j] - colk[i] * (rowk[j] * ip)   for i != k;  row k <- rowk * ip;  column k <- -colk*ip, [k][k] = ip
-        for (int idx = tid; idx < n * n; idx += KI_NT) {
-            const int i = idx % n, j = idx / n;
-            double2 v;
-            if (j == k) {
-                v = (i == k) ? ip : cmul(make_double2(-colk[i].x, -colk[i].y), ip);
-            } else {
-                const double2 rj = cmul(rowk[j], ip);
-                v = (i == k) ? rj : cfnma(a[idx], colk[i], rj);
+        __syncthreads();  // everybody has read the pivot
+        for (int j = tid; j < n; j += KI_NT) rowk[j] = cmul(rowk[j], ip);  // the scaled pivot row, once per step
+        __syncthreads();
+        // a[i][j] <- a[i][j] - colk[i] * rowk[j]   for i != k;  row k <- rowk;  column k <- -colk*ip, [k][k] = ip.
+        // 32 rows x 16 columns of threads, each walking the matrix in strides: no division per element
+        {
+            const int ti = tid & 31, tj = tid >> 5;
+            for (int j = tj; j < n; j += KI_NT / 32) {
+                const double2 rj = rowk[j];
+                double2 *col = a + (size_t)j * n;
+                if (j == k) {
+                    for (int i = ti; i < n; i += 32)
+                        col[i] = (i == k) ? ip : cmul(make_double2(-colk[i].x, -colk[i].y), ip);
+                } else {
+                    for (int i = ti; i < n; i += 32) col[i] = (i == k) ? rj : cfnma(col[i], colk[i], rj);
+                }
             }
-            a[idx] = v;
         }
         __syncthreads();
     }
