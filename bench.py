@@ -324,7 +324,8 @@ def main():
 
         info = infos[-1]
         res = {"mode": mode_name, "value": world * lu_flops(N) / sec_per_step * 1e-12, "ms_per_step": sec_per_step * 1e3,
-               "dtype": "f64" if mode == hb.HPRMAT_FP64 else "tf32/f32 factors + f64 refinement",
+               "dtype": "f64" if mode == hb.HPRMAT_FP64 else "3xtf32 (fp32-class) factors" if mode == hb.HPRMAT_TYPE3
+               else "tf32/f32 factors + f64 refinement",
                "time_to_rmatrix_s": sec_per_step, "lu_tflops": info["lu_tflops"],
                "stages_ms": {k: info[k] for k in ("ms_assemble", "ms_lu", "ms_solve", "ms_refine", "ms_contract", "ms_total")},
                "refine_steps": info["refine_steps"], "backward_err": info["backward_err"], "status": info["status"],
@@ -380,6 +381,33 @@ def main():
                    "lu_tflops": info["lu_tflops"], "refine_steps": info["refine_steps"],
                    "max_abs_error_vs_x_exact": float((Bx - 1.0).abs().max().item())}
         del A, A0, B, Bx
+        torch.cuda.empty_cache()
+        return out
+
+    def raw_zsolve_graded(n=6400, kappa=1e5, nrhs=64):
+        """hprmat_zsolve (mixed+refine) on a Hermitian matrix of prescribed condition number -- Householder similarity of a graded
+        diagonal, the construction of the paper's Fig. 5 -- at kappa = 1e5, inside the paper's domain kappa u_FP32 < 1
+        but beyond what single-pass TF32 factors can refine: the solve escalates to FP32-class (3xTF32) factors by itself."""
+        g = torch.Generator(device="cuda").manual_seed(31)
+        v = torch.randn(n, dtype=torch.complex128, device="cuda", generator=g)
+        v = v / torch.linalg.vector_norm(v)
+        d = torch.pow(torch.tensor(kappa, dtype=torch.float64, device="cuda"), -torch.arange(n, device="cuda", dtype=torch.float64) / (n - 1.0))
+        dv = d * v
+        A = torch.diag(d).to(torch.complex128)
+        A -= 2.0 * torch.outer(v, torch.conj(dv))
+        A -= 2.0 * torch.outer(dv, torch.conj(v))
+        A += 4.0 * torch.sum(torch.conj(v) * dv) * torch.outer(v, torch.conj(v))     # (I - 2vv^H) D (I - 2vv^H), Hermitian
+        At = A.T.contiguous()                                                        # memory of At = column-major A
+        B = At.sum(dim=0, keepdim=True).expand(nrhs, n).contiguous()                 # column-major n x nrhs: B = A @ ones
+        out = None
+        for _ in range(2):
+            Bx = B.clone()
+            _, info = hb.hprmat_zsolve(n, nrhs, At, n, Bx, n, mode=hb.HPRMAT_MIXED_REFINE, max_refine=30,
+                                       allow=(hb.HPRMAT_OK, hb.HPRMAT_ENOTCONVERGED))
+            out = {"n": n, "nrhs": nrhs, "kappa": kappa, "status": info["status"], "fp32_class_factors": info["reserved"],
+                   "refine_steps": info["refine_steps"], "ms_total": info["ms_total"], "ms_lu_both_attempts": info["ms_lu"],
+                   "max_abs_error_vs_x_exact": float((Bx - 1.0).abs().max().item()), "backward_err": info["backward_err"]}
+        del A, At, B, Bx
         torch.cuda.empty_cache()
         return out
 
@@ -440,6 +468,12 @@ def main():
         if full and world == 1:
             # north_star: "raw dense complex solve timed separately from assembly and the R contraction"
             line["raw_zsolve"] = [raw_zsolve("fp64"), raw_zsolve("mixed_refine")]
+            line["raw_zsolve_kappa_1e5"] = raw_zsolve_graded()
+            # the paper's Type 3 as printed (point-major Schur form with the energy-independent kinetic inverse; R17)
+            t3 = measure("type3", steps=2, warmup=1, roofline=False, e2e=False)
+            t3.pop("_R")
+            line["type3_literal_schur"] = {k: t3[k] for k in ("ms_per_step", "lu_tflops", "stages_ms", "backward_err", "status",
+                                                                "steps", "warmup")}
             # the paper's Type 1 (LU of C - E I itself, partial pivoting with row interchanges) next to the default
             t1 = measure("fp64", steps=2, warmup=1, fp64_algo=1, roofline=True, e2e=False)
             t1.pop("_R")
