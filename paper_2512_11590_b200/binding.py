@@ -94,6 +94,11 @@ def hprmat_profile_cgemm_variant(variant: int = -1) -> int:
     return int(lib().hprmat_profile_cgemm_variant(C.c_int(variant)))
 
 
+def hprmat_profile_cgemm3_variant(variant: int) -> int:
+    """0 auto, 1 mma.sync, 2 tcgen05 (operand split in shared memory) for the FP32-class complex64 GEMM."""
+    return int(lib().hprmat_profile_cgemm3_variant(C.c_int(variant)))
+
+
 PROF_CATS = ("lu_gemm", "lu_trsm", "panel", "laswp", "solve", "other")
 
 

@@ -225,6 +225,6 @@ extern "C" int hprmat_cgemm_3xtf32(void *cuda_stream, int m, int n, int k, float
     if (ldb < (k > 1 ? k : 1) || (ldb & 3)) return -11;
     if (ldc < (m > 1 ? m : 1)) return -15;
     using namespace hp;
-    return cgemm3((cudaStream_t)cuda_stream, m, n, k, alpha, CView((float *)A_re, (float *)A_im, lda),
-                  CView((float *)B_re, (float *)B_im, ldb), beta, CView(C_re, C_im, ldc));
+    return cgemm3_any((cudaStream_t)cuda_stream, m, n, k, alpha, CView((float *)A_re, (float *)A_im, lda),
+                      CView((float *)B_re, (float *)B_im, ldb), beta, CView(C_re, C_im, ldc));
 }

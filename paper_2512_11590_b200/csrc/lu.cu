@@ -333,7 +333,7 @@ static int lu_gemm(const LuWork<ZView> &, cudaStream_t st, int m, int n, int k, 
 }
 static int lu_gemm(const LuWork<CView> &wk, cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta,
                    CView C) {
-    if (wk.accurate) return cgemm3(st, m, n, k, alpha, A, B, beta, C);
+    if (wk.accurate) return cgemm3_any(st, m, n, k, alpha, A, B, beta, C);
     LuWork<CView> &w = const_cast<LuWork<CView> &>(wk);
     unsigned *slot = w.wave_sync ? w.wave_sync + 256 * (w.wave_next++ & 7) : nullptr;
     return cgemm_ws(st, m, n, k, alpha, A, B, beta, C, slot);

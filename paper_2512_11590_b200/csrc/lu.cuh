@@ -31,6 +31,9 @@ int cgemm_ws(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView 
 int cgemm_splitk(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C, int slices);
 // FP32-class accuracy variant for the planar complex64 type (3xTF32, cgemm3.cu); C may alias B when m <= 128, beta == 0
 int cgemm3(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
+// tcgen05 version (cgemm3x.cu; C distinct from A and B) and the dispatcher between the two
+int cgemm3x(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
+int cgemm3_any(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B, double beta, CView C);
 int cgemm3_batched(cudaStream_t st, int m, int n, int k, double alpha, CView A, long strideA, CView B, long strideB, double beta,
                    CView C, long strideC, int nbatch);
 int zgemm_batched(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A, long lda, long strideA,

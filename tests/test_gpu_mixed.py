@@ -92,11 +92,13 @@ def test_cgemm_tf32_is_exact_on_tf32_representable_integers(cgemm_variant):
 @pytest.mark.parametrize("m,n,k,alpha,beta", [
     (128, 64, 32, 1.0, 0.0), (128, 256, 128, 1.0, 0.0), (256, 384, 96, -1.0, 1.0), (100, 50, 37, 1.0, 0.0),
     (257, 129, 65, -1.0, 1.0), (32, 700, 32, 1.0, 0.0), (1000, 333, 200, -1.0, 1.0), (5, 3, 1, 2.0, -0.5),
-    (640, 256, 1024, -1.0, 1.0), (1, 1, 8, 1.0, 1.0)])
-def test_cgemm_3xtf32_matches_definition_to_fp32_accuracy(m, n, k, alpha, beta):
+    (640, 256, 1024, -1.0, 1.0), (1, 1, 8, 1.0, 1.0), (2048, 1536, 520, -1.0, 1.0)])
+@pytest.mark.parametrize("c3_variant", [0, 1, 2])
+def test_cgemm_3xtf32_matches_definition_to_fp32_accuracy(m, n, k, alpha, beta, c3_variant):
     """hprmat_cgemm_3xtf32: operands split hi + lo in TF32 (dropped lo*lo term and the rounding of lo: <= 2^-21 relative
     per product, taken as 2^-20 here), FP32 accumulation:  |C - C_def| <= (2^-20 + (k + 4) 2^-23) (|alpha| |A||B| + |beta||C0|).
-    On the same data the single-pass kernel is ~2^-10: a kernel that silently fell back to one pass fails this bound."""
+    On the same data the single-pass kernel is ~2^-10: a kernel that silently fell back to one pass fails this bound.
+    c3_variant: 0 the dispatcher, 1 the mma.sync kernel, 2 the tcgen05 kernel that splits its operands in shared memory."""
     rng = np.random.default_rng(m * 1000003 + n * 1009 + k + 7)
     A = (rng.uniform(-1, 1, (m, k)) + 1j * rng.uniform(-1, 1, (m, k))).astype(np.complex64).astype(np.complex128)
     B = (rng.uniform(-1, 1, (k, n)) + 1j * rng.uniform(-1, 1, (k, n))).astype(np.complex64).astype(np.complex128)
@@ -105,8 +107,12 @@ def test_cgemm_3xtf32_matches_definition_to_fp32_accuracy(m, n, k, alpha, beta):
     Ar, Ai = _planes(A, lda)
     Br, Bi = _planes(B, ldb)
     Cr, Ci = _planes(C0, ldc)
-    hb.hprmat_cgemm_3xtf32(m, n, k, alpha, Ar, Ai, lda, Br, Bi, ldb, beta, Cr, Ci, ldc)
-    torch.cuda.synchronize()
+    hb.hprmat_profile_cgemm3_variant(c3_variant)
+    try:
+        hb.hprmat_cgemm_3xtf32(m, n, k, alpha, Ar, Ai, lda, Br, Bi, ldb, beta, Cr, Ci, ldc)
+        torch.cuda.synchronize()
+    finally:
+        hb.hprmat_profile_cgemm3_variant(0)
     got = _unplanes(Cr, Ci, m)
     ref = beta * C0 + alpha * (A @ B)
     absA = np.abs(A.real) + np.abs(A.imag)
