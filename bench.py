@@ -197,6 +197,8 @@ def main():
                          "dispatch, 1 = round 1's one-tile-per-CTA kernel everywhere, 2-4 = persistent variants, 5 = split-K "
                          "wherever possible; for A/B measurements")
     ap.add_argument("--no-graphs", action="store_true", help="plain stream launches instead of CUDA-graph replay (A/B)")
+    ap.add_argument("--no-pdl", action="store_true",
+                    help="launch the small LU kernels without programmatic dependent launch (A/B)")
     ap.add_argument("--zgemm-algo", type=int, default=0, choices=[0, 3, 4],
                     help="real decomposition of the complex128 GEMM (3M / 4M); 0 = the library default")
     args = ap.parse_args()
@@ -213,6 +215,8 @@ def main():
         hb.hprmat_fp64_algo(args.fp64_algo)
     if args.cgemm_variant:
         hb.hprmat_profile_cgemm_variant(args.cgemm_variant)
+    if args.no_pdl:
+        hb.hprmat_profile_pdl(0)
     full = not args.quick
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -40,6 +40,10 @@ int hprmat_profile_cgemm_variant(int variant);
  * 2 = tcgen05 whenever legal.  Returns 0, or -1 for another value.  Process-wide; for tests and A/B measurements. */
 int hprmat_profile_cgemm3_variant(int variant);
 
+/* Programmatic dependent launch of the small kernels of the complex64 LU (their prologues overlap the predecessor's tail):
+ * 1 = on (default), 0 = off, any other value only queries.  Returns the setting in force.  Process-wide; A/B measurements. */
+int hprmat_profile_pdl(int enable);
+
 /* How many launch sequences (factorisations, triangular solves) of the context are replayed from CUDA graphs (captured) and
  * how many had to stay plain stream launches (eager: capture refused).  captured / eager: host, may be NULL. */
 struct hprmat_ctx;

@@ -99,6 +99,11 @@ def hprmat_profile_cgemm3_variant(variant: int) -> int:
     return int(lib().hprmat_profile_cgemm3_variant(C.c_int(variant)))
 
 
+def hprmat_profile_pdl(enable: int = -1) -> int:
+    """Programmatic dependent launch of the small LU kernels: 1 on (default), 0 off, anything else queries."""
+    return int(lib().hprmat_profile_pdl(C.c_int(enable)))
+
+
 PROF_CATS = ("lu_gemm", "lu_trsm", "panel", "laswp", "solve", "other")
 
 

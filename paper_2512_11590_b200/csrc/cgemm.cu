@@ -85,6 +85,8 @@ __global__ void __launch_bounds__(CG_NT, 1)
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    pdl_wait();     // everything above overlapped the predecessor's tail; global memory only from here on
+    pdl_trigger();
 
     if (warp == 0) {
         if (lane == 0) {
@@ -243,7 +245,7 @@ int launch_cgemm(cudaStream_t st, int m, int n, int k, float alpha, CView A, CVi
     HP_TRY(make_map(&maps.b_re, B.re, kk, n, B.ld, CG_KC, BN, CU_TENSOR_MAP_SWIZZLE_128B));
     HP_TRY(make_map(&maps.b_im, B.im, kk, n, B.ld, CG_KC, BN, CU_TENSOR_MAP_SWIZZLE_128B));
     dim3 grid(ceil_div(m, CG_BM) * ceil_div(n, BN));
-    kern<<<grid, CG_NT, Cfg::SMEM, st>>>(maps, m, n, k, alpha, beta, C.re, C.im, C.ld);
+    HP_CUDA(launch_pdl(kern, grid, dim3(CG_NT), Cfg::SMEM, st, maps, m, n, k, alpha, beta, C.re, C.im, (long)C.ld));
     HP_LAUNCHED();
     return 0;
 }

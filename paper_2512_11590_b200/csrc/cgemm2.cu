@@ -105,6 +105,8 @@ __global__ void __launch_bounds__(G2_NT, 1)
     if constexpr (NCTA == 2) cluster_sync_all();  // the peer's barriers are initialised before anything arrives on them
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    pdl_wait();     // the prologue above may overlap the predecessor's tail (launch_pdl); global memory only from here on
+    pdl_trigger();
 
     if (warp == 0) {
         // ================================================================================ TMA producer
@@ -313,13 +315,15 @@ int launch_cgemm2(cudaStream_t st, int m, int n, int k, float alpha, CView A, CV
     lc.blockDim = dim3(G2_NT);
     lc.dynamicSmemBytes = Cfg::SMEM;
     lc.stream = st;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = NCTA;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
     lc.attrs = attr;
-    lc.numAttrs = 1;
+    lc.numAttrs = (pdl_enabled() && p.wave_ctr == nullptr) ? 2 : 1;  // behind the counters' memset: a plain dependency
     HP_CUDA(cudaLaunchKernelEx(&lc, kern, maps, p));
     HP_LAUNCHED();
     return 0;

@@ -75,6 +75,8 @@ __global__ void __launch_bounds__(C3_NT, 1)
     int tm, tn;
     raster((int)blockIdx.x, (M + C3_BM - 1) / C3_BM, (N + C3_BN - 1) / C3_BN, 8, tm, tn);
     const long m0 = (long)tm * C3_BM, n0 = (long)tn * C3_BN;
+    pdl_wait();
+    pdl_trigger();
 
     auto load_stage = [&](int slot, int k0) {
         float *ar = sm3 + (size_t)slot * C3_STAGE, *ai = ar + C3_A_PLANE, *br = ai + C3_A_PLANE, *bi = br + C3_B_PLANE;
@@ -206,8 +208,9 @@ int cgemm3_batched(cudaStream_t st, int m, int n, int k, double alpha, CView A, 
     HP_TRY(configure_smem(cfg, cgemm3_kernel, C3_SMEM));
     const bool prof = prof_enabled() && k > 0;
     if (prof) prof_begin(st, 8.0 * m * n * k * nbatch);
-    cgemm3_kernel<<<dim3(ceil_div(m, C3_BM) * ceil_div(n, C3_BN), nbatch), C3_NT, C3_SMEM, st>>>(
-        m, n, k, (float)alpha, A.re, A.im, A.ld, B.re, B.im, B.ld, (float)beta, C.re, C.im, C.ld, strideA, strideB, strideC);
+    HP_CUDA(launch_pdl(cgemm3_kernel, dim3(ceil_div(m, C3_BM) * ceil_div(n, C3_BN), nbatch), dim3(C3_NT), C3_SMEM, st, m, n, k,
+                       (float)alpha, A.re, A.im, (long)A.ld, B.re, B.im, (long)B.ld, (float)beta, C.re, C.im, (long)C.ld, strideA,
+                       strideB, strideC));
     if (prof) prof_end(st);
     HP_LAUNCHED();
     return 0;

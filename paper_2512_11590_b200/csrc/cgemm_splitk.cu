@@ -83,6 +83,8 @@ __global__ void __launch_bounds__(SK_NT, 1)
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    pdl_wait();     // the prologue above may overlap the predecessor's tail (launch_pdl); global memory only from here on
+    pdl_trigger();
 
     if (warp == 0) {
         if (lane == 0) {
@@ -228,13 +230,15 @@ int cgemm_splitk(cudaStream_t st, int m, int n, int k, double alpha, CView A, CV
     lc.blockDim = dim3(SK_NT);
     lc.dynamicSmemBytes = SK_SMEM;
     lc.stream = st;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = (unsigned)slices;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
     lc.attrs = attr;
-    lc.numAttrs = 1;
+    lc.numAttrs = pdl_enabled() ? 2 : 1;
     const float al = (float)alpha, be = (float)beta;
     if (slices == 8) HP_CUDA(cudaLaunchKernelEx(&lc, cgemm_splitk_kernel<8>, maps, m, n, k, al, be, C.re, C.im, C.ld, tiles_m));
     else if (slices == 4) HP_CUDA(cudaLaunchKernelEx(&lc, cgemm_splitk_kernel<4>, maps, m, n, k, al, be, C.re, C.im, C.ld, tiles_m));

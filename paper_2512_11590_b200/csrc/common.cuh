@@ -81,6 +81,31 @@ template <class K> inline int configure_smem(SmemCfg &c, K kern, size_t bytes) {
     return 0;
 }
 
+// Programmatic dependent launch (PDL): a kernel launched through launch_pdl may become resident while its predecessor on
+// the stream is still running, do its prologue (barrier init, TMEM allocation, descriptor prefetch) and then MUST execute
+// pdl_wait() -- in every CTA, before its first access to global memory -- which returns once the predecessor grid has
+// completed and its writes are visible.  pdl_trigger() lets the NEXT launch start that early.  The LU issues thousands of
+// small dependent kernels; this hides their launch latency and prologues behind the predecessor's tail.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\n" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory"); }
+#endif
+bool pdl_enabled();  // util.cu (hprmat_profile_pdl)
+template <class... KArgs, class... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = grid;
+    lc.blockDim = block;
+    lc.dynamicSmemBytes = smem;
+    lc.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    lc.attrs = at;
+    lc.numAttrs = pdl_enabled() ? 1 : 0;
+    return cudaLaunchKernelEx(&lc, kern, KArgs(args)...);
+}
+
 // Real decomposition of the complex128 GEMM (3 = 3M, 4 = 4M) in force on this host thread: the process default
 // (hprmat_zgemm_algo) unless a context's own setting is installed for the duration of one of its calls.
 int zgemm_algo_in_force();

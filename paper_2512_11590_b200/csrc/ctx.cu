@@ -519,6 +519,7 @@ template <class F> int replay(hprmat_ctx *c, int kind, int flags, const void *ke
     if (!c->use_graphs || prof_enabled()) return enqueue(c->st);
     flags |= zgemm_algo_in_force() << 16;  // the captured sequence holds the kernels of this decomposition ...
     flags |= cgemm_variant_in_force() << 20;  // ... and of this complex64 GEMM kernel
+    flags |= (pdl_enabled() ? 1 : 0) << 24;   // ... launched with or without programmatic dependent launch
     hprmat_ctx::GraphEntry *ent = nullptr;
     for (auto &g : c->graphs)
         if (g.kind == kind && g.flags == flags && g.key == key) ent = &g;

@@ -143,6 +143,8 @@ __global__ void __launch_bounds__(INV_NT) inv_double_kernel(V A, int h, int w, V
     const V Xa = isU ? Ua : La, Xb = isU ? Ub : Lb, O = isU ? Uout : Lout;
     const int hb = w - h;
     const bool top = i0 < h;
+    pdl_wait();
+    pdl_trigger();
     // rows that are plain copies / zeros
     if (top != isU) {
         // L top rows: [inv(La) | 0];  U bottom rows: [0 | inv(Ub)]
@@ -256,7 +258,8 @@ template <class V> static int inv_double(cudaStream_t st, V A, int c0, int h, in
     ProfCat pc(PROF_OTHER);
     const bool prof = prof_enabled();
     if (prof) prof_begin(st, 0.0);
-    inv_double_kernel<V><<<dim3(ceil_div(w, INV_RS), 2), INV_NT, smem, st>>>(A.sub(c0, c0), h, w, La, Lb, Lo, Ua, Ub, Uo);
+    HP_CUDA(launch_pdl(inv_double_kernel<V>, dim3(ceil_div(w, INV_RS), 2), dim3(INV_NT), smem, st, A.sub(c0, c0), h, w, La, Lb, Lo,
+                       Ua, Ub, Uo));
     if (prof) prof_end(st);
     HP_LAUNCHED();
     return 0;
@@ -291,6 +294,8 @@ template <class V> __global__ void __launch_bounds__(256) set_identity_kernel(V 
 }
 template <class V> __global__ void __launch_bounds__(256) copy_block_kernel(V Src, V Dst, int rows, long cols) {
     const long idx = (long)blockIdx.x * 256 + threadIdx.x;
+    pdl_wait();
+    pdl_trigger();
     if (idx >= (long)rows * cols) return;
     const int i = (int)(idx % rows);
     const long j = idx / rows;
@@ -307,7 +312,7 @@ template <class V> __global__ void __launch_bounds__(256) strip_diag_kernel(V X,
 }
 template <class V> static int copy_block(cudaStream_t st, V Src, V Dst, int rows, long cols) {
     if (rows <= 0 || cols <= 0) return 0;
-    copy_block_kernel<V><<<ceil_div((long)rows * cols, 256), 256, 0, st>>>(Src, Dst, rows, cols);
+    HP_CUDA(launch_pdl(copy_block_kernel<V>, dim3(ceil_div((long)rows * cols, 256)), dim3(256), 0, st, Src, Dst, rows, cols));
     HP_LAUNCHED();
     return 0;
 }

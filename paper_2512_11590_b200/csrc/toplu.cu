@@ -51,6 +51,8 @@ __global__ void __launch_bounds__(TL_NT, 1)
     const int role = threadIdx.x / TL_G, lt = threadIdx.x % TL_G, ti = lt & 15, tj = lt >> 4;
     const E zero = mk((T)0, (T)0), one = mk((T)1, (T)0);
 
+    pdl_wait();
+    pdl_trigger();
     // LU role: x = the block.  Inversion role: x = XL, y = Y, both start as the identity
     E x[TL_R][TL_R], y[TL_R][TL_R];
 #pragma unroll
@@ -181,6 +183,8 @@ template <class V> __global__ void __launch_bounds__(256) check_multipliers_kern
     typedef typename V::real_t T;
     const int row = blockIdx.x * 256 + threadIdx.x, c0 = blockIdx.y * CHK_C;
     int bad = 0;
+    pdl_wait();
+    pdl_trigger();
     if (row < m) {
         E v[CHK_C];
 #pragma unroll
@@ -207,14 +211,14 @@ static bool l21_checked(cudaStream_t st, int m2, int w, CView L21, CView du, int
 
 template <class V> int block_panel(cudaStream_t st, int n, V A, int c0, int w, int *ipiv, int *info_dev, LuWork<V> &wk, V dl, V du) {
     typedef typename V::elem_t E;
-    auto kern = top_lu_kernel<V>;
     const int b0 = c0 / IB, nbatch = ceil_div(w, IB);
     {
         ProfCat pc(PROF_PANEL);
         const bool prof = prof_enabled();
         if (prof) prof_begin(st, 0.0);
-        kern<<<1, TL_NT, 0, st>>>(A.sub(c0, c0), w, c0, ipiv, info_dev, wk.refuted, dl, du, wk.perm + (size_t)b0 * PERM_STRIDE,
-                                     nbatch);
+        auto kern = top_lu_kernel<V>;
+        HP_CUDA(launch_pdl(kern, dim3(1), dim3(TL_NT), 0, st, A.sub(c0, c0), w, c0, ipiv, info_dev, wk.refuted, dl, du,
+                           wk.perm + (size_t)b0 * PERM_STRIDE, nbatch));
         if (prof) prof_end(st);
         HP_LAUNCHED();
     }
@@ -229,7 +233,8 @@ template <class V> int block_panel(cudaStream_t st, int n, V A, int c0, int w, i
         HP_TRY(gemm(st, m2, w, w, 1.0, L21, du, 0.0, L21));
         const bool prof = prof_enabled();
         if (prof) prof_begin(st, 0.0);
-        check_multipliers_kernel<V><<<dim3(ceil_div(m2, 256), ceil_div(w, CHK_C)), 256, 0, st>>>(L21, m2, w, wk.refuted);
+        HP_CUDA(launch_pdl(check_multipliers_kernel<V>, dim3(ceil_div(m2, 256), ceil_div(w, CHK_C)), dim3(256), 0, st, L21, m2, w,
+                           wk.refuted));
         if (prof) prof_end(st);
         HP_LAUNCHED();
     }

@@ -61,6 +61,8 @@ __global__ void __launch_bounds__(WM *WN * 32, MINB)
     A += (long)blockIdx.z * strideA;
     B += (long)blockIdx.z * strideB;
     C += (long)blockIdx.z * strideC;
+    pdl_wait();
+    pdl_trigger();
 
     auto load_stage = [&](int slot, int k0) {
         double2 *a = sA + slot * A_STAGE;
@@ -183,7 +185,7 @@ static int launch_zgemm(cudaStream_t st, int m, int n, int k, double alpha, cons
     static SmemCfg cfg;
     HP_TRY(configure_smem(cfg, kern, smem));
     dim3 grid(ceil_div(m, BM) * ceil_div(n, BN), 1, nbatch);
-    kern<<<grid, WM * WN * 32, smem, st>>>(m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC);
+    HP_CUDA(launch_pdl(kern, grid, dim3(WM * WN * 32), smem, st, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, sA, sB, sC));
     HP_LAUNCHED();
     return 0;
 }

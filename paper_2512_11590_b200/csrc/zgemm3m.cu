@@ -105,6 +105,8 @@ __global__ void __launch_bounds__(WM *WN * 32, 1)
         fence_mbar_init();
     }
     __syncthreads();
+    pdl_wait();
+    pdl_trigger();
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
         if (s < nk) {
@@ -212,7 +214,8 @@ int zgemm3m(cudaStream_t st, int m, int n, int k, double alpha, const double2 *A
     static SmemCfg cfg;
     HP_TRY(configure_smem(cfg, kern, smem));
     dim3 grid(ceil_div(m, BM) * ceil_div(n, BN), 1, nbatch);
-    kern<<<grid, WM * WN * 32, smem, st>>>(m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, strideA, strideB, strideC);
+    HP_CUDA(launch_pdl(kern, grid, dim3(WM * WN * 32), smem, st, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, strideA, strideB,
+                       strideC));
     HP_LAUNCHED();
     return 0;
 }
