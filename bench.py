@@ -178,7 +178,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--mode", default="fp64", choices=["fp64", "mixed", "mixed_refine"])
+    ap.add_argument("--mode", default="fp64", choices=["fp64", "mixed", "mixed_refine", "type3"])
     ap.add_argument("--cfg", type=int, default=3)
     ap.add_argument("--quick", action="store_true",
                     help="only the headline step (and --also): skip the raw-solve, Type-1, other-config and matching legs")

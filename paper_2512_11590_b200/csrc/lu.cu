@@ -46,6 +46,7 @@ template <class V> size_t LuWork<V>::carve(void *base, int n_) {
         dinvL[lev] = alloc_view<V>(p, sz, (long)ceil_div(n, sz) * sz);
         dinvU[lev] = alloc_view<V>(p, sz, (long)ceil_div(n, sz) * sz);
     }
+    constexpr int SB = SolveBlock<V>::value;
     sbld = std::min<long>(SB, round_up(std::max(n, 1), 32));
     if (n > LEAF) {
         binvL = alloc_view<V>(p, sbld, (long)ceil_div(n, SB) * sbld);
@@ -227,7 +228,8 @@ __global__ void __launch_bounds__(INV_NT) inv_double_kernel(V A, int h, int w, V
 // Column split of a node of width w: below LEAF the tree is binary on power-of-two multiples of IB, so that every left
 // child is a full block of its size class (its inverse is kept, see LuWork); above, splits fall on multiples of LEAF, and
 // above SB on multiples of SB, so that every SB-aligned block is a node of the recursion (its full inverse is kept too).
-static inline int split(int w) {
+template <class V> static inline int split(int w) {
+    constexpr int SB = SolveBlock<V>::value;
     if (w > SB) return (int)round_up((w + 1) / 2, SB);
     if (w > LEAF) return (int)round_up((w + 1) / 2, LEAF);
     int h = IB;
@@ -317,8 +319,11 @@ template <class V> static int copy_block(cudaStream_t st, V Src, V Dst, int rows
     return 0;
 }
 // does the SB-aligned block starting at d0 have a kept full inverse, and is [d0, d0 + s) exactly that block?
-static inline bool is_big_block(int n, int d0, int s) { return d0 % SB == 0 && s > LEAF && s == std::min(SB, n - d0); }
-template <class V> static V binv_of(const V &tab, long sbld, int d0) { return tab.sub(0, (long)(d0 / SB) * sbld); }
+template <class V> static inline bool is_big_block(int n, int d0, int s) {
+    constexpr int SB = SolveBlock<V>::value;
+    return d0 % SB == 0 && s > LEAF && s == std::min(SB, n - d0);
+}
+template <class V> static V binv_of(const V &tab, long sbld, int d0) { return tab.sub(0, (long)(d0 / SolveBlock<V>::value) * sbld); }
 
 // the (batched) 3xTF32 product with the LEAF-diagonal blocks of an SB block, complex64 type only
 static int diag_blocks_product(cudaStream_t, const ZView *, int, int, ZView, int, ZView) { return 0; }
@@ -397,9 +402,9 @@ static int leaf_product(bool acc, cudaStream_t st, int s, int ncols, CView dinv,
 template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk, bool acc = false) {
     if (s <= 0 || ncols <= 0) return 0;
     if (s <= LEAF) return leaf_product(acc, st, s, ncols, dinv_of(wk.dinvL, d0, s), B, wk);
-    if (wk.use_big && (acc || IsPlanar<V>::value) && is_big_block(wk.n, d0, s))
+    if (wk.use_big && (acc || IsPlanar<V>::value) && is_big_block<V>(wk.n, d0, s))
         return big_leaf(st, wk.binvL, wk.dinvL, d0, s, B, ncols, wk, acc);
-    const int h = split(s);
+    const int h = split<V>(s);
     HP_TRY(trsm_lower(st, A, d0, h, B, ncols, wk, acc));
     HP_TRY(lu_gemm(wk, st, s - h, ncols, h, -1.0, A.sub(d0 + h, d0), B, 1.0, B.sub(h, 0)));
     return trsm_lower(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk, acc);
@@ -409,9 +414,9 @@ template <class V> static int trsm_lower(cudaStream_t st, V A, int d0, int s, V 
 template <class V> static int trsm_upper(cudaStream_t st, V A, int d0, int s, V B, int ncols, LuWork<V> &wk, bool acc = false) {
     if (s <= 0 || ncols <= 0) return 0;
     if (s <= LEAF) return leaf_product(acc, st, s, ncols, dinv_of(wk.dinvU, d0, s), B, wk);
-    if (wk.use_big && (acc || IsPlanar<V>::value) && is_big_block(wk.n, d0, s))
+    if (wk.use_big && (acc || IsPlanar<V>::value) && is_big_block<V>(wk.n, d0, s))
         return big_leaf(st, wk.binvU, wk.dinvU, d0, s, B, ncols, wk, acc);
-    const int h = split(s);
+    const int h = split<V>(s);
     HP_TRY(trsm_upper(st, A, d0 + h, s - h, B.sub(h, 0), ncols, wk, acc));
     HP_TRY(lu_gemm(wk, st, h, ncols, s - h, -1.0, A.sub(d0, d0 + h), B.sub(h, 0), 1.0, B));
     return trsm_upper(st, A, d0, h, B, ncols, wk, acc);
@@ -490,7 +495,7 @@ template <class V> static int getrf_rec(cudaStream_t st, int n, V A, int c0, int
         return block_panel<V>(st, n, A, c0, w, ipiv, info_dev, wk, dinv_of(wk.dinvL, c0, w), dinv_of(wk.dinvU, c0, w));
     }
     if (w <= IB) return panel(st, n, A, c0, w, ipiv, info_dev, wk);
-    const int h = split(w), mid = c0 + h;
+    const int h = split<V>(w), mid = c0 + h;
     HP_TRY(getrf_rec(st, n, A, c0, mid, ipiv, info_dev, wk));
     {
         ProfCat pc(PROF_LU_TRSM);
@@ -503,7 +508,7 @@ template <class V> static int getrf_rec(cudaStream_t st, int n, V A, int c0, int
     HP_TRY(getrf_rec(st, n, A, mid, c1, ipiv, info_dev, wk));
     // the node's diagonal block is final: keep its inverse for the triangular solves further up / in getrs
     if (w <= LEAF) HP_TRY(inv_double(st, A, c0, h, w, wk));
-    if (is_big_block(n, c0, w)) HP_TRY(build_binv(st, A, c0, w, wk));
+    if (is_big_block<V>(n, c0, w)) HP_TRY(build_binv(st, A, c0, w, wk));
     return 0;
 }
 
@@ -524,6 +529,7 @@ template <class V> int getrf(cudaStream_t st, int n, V A, int *ipiv, int *info_d
     if (IsPlanar<V>::value && n > LEAF) {
         // the solves apply the LEAF-diagonal blocks of the kept inverses separately, with FP32-class products
         ProfCat pc(PROF_OTHER);
+        constexpr int SB = SolveBlock<V>::value;
         for (int d0 = 0; d0 < n; d0 += SB) {
             const int sblk = std::min(SB, n - d0);
             if (sblk <= LEAF) continue;

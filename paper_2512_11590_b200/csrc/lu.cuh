@@ -8,8 +8,13 @@ constexpr int IB = 32;        // panel width = swap batch = smallest inverted di
 constexpr int LEAF = 128;     // largest inverted diagonal block = leaf of the triangular-solve recursion (one GEMM M tile,
                               // so that the leaf product B <- inv * B may run in place)
 constexpr int NLEV = 3;       // inverted diagonal blocks are kept at sizes IB << lev, lev = 0 .. NLEV-1
-constexpr int SB = 1024;      // "solve block": the full inverses of the SB x SB diagonal blocks of L and U are kept as well, so
-                              // that a triangular solve is N/SB dependent steps of large dense GEMMs instead of N/LEAF
+// "Solve block": the full inverses of the SB x SB diagonal blocks of L and U are kept as well, so that a triangular solve is
+// N/SB dependent steps of large dense GEMMs instead of N/LEAF.  Per type, by measurement at configs[3]: the complex64 solves
+// are a chain of latency-bound launches (2048: first solve 6.4 -> 4.2 ms, a refinement step 7.9 -> 6.0 ms, the factorisation
+// pays 2 ms for the larger inverses); the complex128 ones are flop bound and the larger inverses cost the LU more than the
+// solves gain (1024).
+template <class V> struct SolveBlock { static constexpr int value = 1024; };
+template <> struct SolveBlock<CView> { static constexpr int value = 2048; };
 constexpr int MAXG = kNumSMs; // CTAs of the cooperative panel kernel (one per SM)
 constexpr int TW = 64;        // width of the block panel of a factorisation with verified diagonal pivots (toplu.cu): its top
                               // block is factored and inverted by one CTA out of registers and shared memory
