@@ -35,7 +35,7 @@ long long hprmat_launch_count(void);
 int hprmat_profile_cgemm_variant(int variant);
 
 /* Which kernel serves the FP32-class ("3xTF32") planar complex64 GEMM (hprmat_cgemm_3xtf32 and the products of the
- * escalated factorisations): 0 = automatic (tcgen05 with the operand split done in shared memory, cgemm3x.cu, when C is
+ * escalated factorisations): 0 = automatic (tcgen05 with the lo parts computed in shared memory, cgemm3x.cu, when C is
  * distinct from A and B and the problem fills >= 32 tiles; else the mma.sync kernel, cgemm3.cu), 1 = mma.sync always,
  * 2 = tcgen05 whenever legal.  Returns 0, or -1 for another value.  Process-wide; for tests and A/B measurements. */
 int hprmat_profile_cgemm3_variant(int variant);

@@ -5,14 +5,19 @@
 //
 //   C <- beta*C + alpha*A*B,  operands and layouts as cgemm.cu.
 //
-// Every FP32 operand x is split as x = hi + lo, hi = x rounded to TF32 (10 mantissa bits), lo = x - hi (exact in FP32,
-// |lo| <= 2^-11 |x|), and every real product is three UMMAs: hi*hi + hi*lo + lo*hi (the dropped lo*lo and the rounding of lo
-// are <= 2^-21 relative).  The tensor core reads its operands from shared memory, so the split happens THERE: TMA lands the
-// FP32 tile, four "splitter" warps rewrite it in place as hi and write lo next to it (same swizzled layout: the transform
-// is elementwise), fence the async proxy and hand the stage to the MMA issuer.
+// Every FP32 operand x is split as x = hi + lo and every real product is three UMMAs: hi*hi + hi*lo + lo*hi.  The tensor core
+// reads its operands from shared memory and uses only the upper 19 bits of an FP32 word (kind::tf32 TRUNCATES), so
+//   hi = the word TMA landed, as it is (the hardware sees trunc(x)),
+//   lo = rne_tf32(x - trunc(x))  (x - trunc(x) is exact in FP32 and < 2^-10 |x|; rounded to 10 mantissa bits here so that the
+//        hardware's truncation of lo is exact),
+// which leaves the dropped lo*lo term and the rounding of lo: <= 2^-21 relative.  Four "splitter" warps compute lo from the
+// landed tile into a second tile of the same swizzled layout (the transform is elementwise), fence the async proxy and hand
+// the stage to the MMA issuer.  The accuracy test (tests/test_gpu_mixed.py, 2^-20 bound) fails if the hardware did anything
+// but truncate.
 //
 // CTA = 10 warps: warp 0 TMA producer, warp 1 TMEM allocator + UMMA issuer, warps 2-5 epilogue, warps 6-9 splitters.
-// Tile 128 x 64, K step 32, two stages of (A, B, A_lo, B_lo) = 2 x 96 KB.
+// Tile 128 x 128, K step 16, three stages of (A, B, A_lo, B_lo) = 3 x 64 KB.  (N = 128 halves the shared-memory reads per
+// flop of the 128 x 64 version, which was bound by them: 150 -> see DESIGN.md section 8.)
 #include <atomic>
 
 #include "lu.cuh"
@@ -27,18 +32,25 @@ int make_map(CUtensorMap *map, const float *plane, long rows, long cols, long ld
 
 namespace {
 
-constexpr int X3_BM = 128, X3_BN = 64, X3_KC = 32, X3_NT = 320;
-constexpr int X3_A_PLANE = X3_BM * X3_KC * 4;                 // 16 KB
+constexpr int X3_BM = 128, X3_BN = 128, X3_KC = 16, X3_NT = 320;
+constexpr int X3_A_PLANE = X3_BM * X3_KC * 4;                 // 8 KB
 constexpr int X3_B_PLANE = X3_BN * X3_KC * 4;                 // 8 KB
-constexpr int X3_HALF = 2 * X3_A_PLANE + 2 * X3_B_PLANE;      // 48 KB: the TMA-written (then hi) tiles of one stage
+constexpr int X3_HALF = 2 * X3_A_PLANE + 2 * X3_B_PLANE;      // 32 KB: the TMA-written tiles of one stage
 constexpr int X3_STAGE = 2 * X3_HALF;                         // + the lo tiles
-constexpr int X3_STAGES = 2;
+constexpr int X3_STAGES = 3;
 constexpr int X3_SMEM = X3_STAGES * X3_STAGE + 1024 + 256;
 constexpr int X3_TMEM = 2 * X3_BN;                            // Dr | Di
 
 struct X3Maps {
     CUtensorMap a_re, a_im, b_re, b_im;
 };
+
+// lo = rne_tf32(x - trunc_tf32(x)) as raw bits (round to nearest on the 13 dropped bits, ties away; an exponent carry is the
+// correct rounding)
+__device__ __forceinline__ uint32_t split_lo(uint32_t x) {
+    const float d = __uint_as_float(x) - __uint_as_float(x & 0xffffe000u);
+    return (__float_as_uint(d) + 0x1000u) & 0xffffe000u;
+}
 
 __global__ void __launch_bounds__(X3_NT, 1)
     cgemm3x_kernel(const __grid_constant__ X3Maps maps, int M, int N, int K, float alpha, float beta, float *__restrict__ Cre,
@@ -115,8 +127,8 @@ __global__ void __launch_bounds__(X3_NT, 1)
                         const uint32_t b_re = a_re + 2 * X3_A_PLANE, b_im = b_re + X3_B_PLANE;
                         dar[p] = smem_desc_sw128_base32(a_re + ks * 1024, X3_KC * 128, 512);
                         dai[p] = smem_desc_sw128_base32(a_im + ks * 1024, X3_KC * 128, 512);
-                        dbr[p] = smem_desc_sw128(b_re + ks * 32, 16, 1024);
-                        dbi[p] = smem_desc_sw128(b_im + ks * 32, 16, 1024);
+                        dbr[p] = smem_desc_sw64(b_re + ks * 32, 16, 512);
+                        dbi[p] = smem_desc_sw64(b_im + ks * 32, 16, 512);
                     }
                     // the two small terms first, then hi*hi: (a, b) part pairs (1,0), (0,1), (0,0)
 #pragma unroll
@@ -134,7 +146,7 @@ __global__ void __launch_bounds__(X3_NT, 1)
             umma_commit(tmem_full);
         }
     } else if (warp >= 6) {
-        // ---- splitters: x -> (hi in place, lo at +X3_HALF), 16 bytes at a time
+        // ---- splitters: lo at +X3_HALF from the landed words, 16 bytes at a time
         const int t = threadIdx.x - 192;  // 0 .. 127
         for (int kt = 0; kt < nk; ++kt) {
             const int s = kt % X3_STAGES;
@@ -145,16 +157,11 @@ __global__ void __launch_bounds__(X3_NT, 1)
 #pragma unroll 4
             for (int i = t; i < X3_HALF / 16; i += 128) {
                 const uint4 x = hi[i];
-                uint4 h, l;
-                h.x = (x.x + 0x1000u) & 0xffffe000u;  // round to nearest TF32 (ties away; exponent carry is the correct rounding)
-                h.y = (x.y + 0x1000u) & 0xffffe000u;
-                h.z = (x.z + 0x1000u) & 0xffffe000u;
-                h.w = (x.w + 0x1000u) & 0xffffe000u;
-                l.x = __float_as_uint(__uint_as_float(x.x) - __uint_as_float(h.x));
-                l.y = __float_as_uint(__uint_as_float(x.y) - __uint_as_float(h.y));
-                l.z = __float_as_uint(__uint_as_float(x.z) - __uint_as_float(h.z));
-                l.w = __float_as_uint(__uint_as_float(x.w) - __uint_as_float(h.w));
-                hi[i] = h;
+                uint4 l;
+                l.x = split_lo(x.x);
+                l.y = split_lo(x.y);
+                l.z = split_lo(x.z);
+                l.w = split_lo(x.w);
                 lo[i] = l;
             }
             fence_proxy_async();  // the UMMAs (async proxy) must see these generic-proxy writes
@@ -215,8 +222,8 @@ int cgemm3x(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B
     const int kk = k > 0 ? k : 1;
     HP_TRY(make_map(&maps.a_re, A.re, m, kk, A.ld, 32, X3_KC, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B));
     HP_TRY(make_map(&maps.a_im, A.im, m, kk, A.ld, 32, X3_KC, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B));
-    HP_TRY(make_map(&maps.b_re, B.re, kk, n, B.ld, X3_KC, X3_BN, CU_TENSOR_MAP_SWIZZLE_128B));
-    HP_TRY(make_map(&maps.b_im, B.im, kk, n, B.ld, X3_KC, X3_BN, CU_TENSOR_MAP_SWIZZLE_128B));
+    HP_TRY(make_map(&maps.b_re, B.re, kk, n, B.ld, X3_KC, X3_BN, CU_TENSOR_MAP_SWIZZLE_64B));
+    HP_TRY(make_map(&maps.b_im, B.im, kk, n, B.ld, X3_KC, X3_BN, CU_TENSOR_MAP_SWIZZLE_64B));
     const bool prof = prof_enabled() && k > 0;
     if (prof) prof_begin(st, 8.0 * m * n * k);
     kern<<<ceil_div(m, X3_BM) * ceil_div(n, X3_BN), X3_NT, X3_SMEM, st>>>(maps, m, n, k, (float)alpha, (float)beta, C.re, C.im, C.ld);

@@ -162,6 +162,16 @@ __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t addr, uint32_t lbo,
     d |= (uint64_t)2 << 61;                          // layout type: SWIZZLE_128B
     return d;
 }
+// Same, layout type SWIZZLE_64B (K-major tiles whose rows are 64 bytes: 16 tf32 of K; 8-row groups sbo = 512 bytes apart)
+__device__ __forceinline__ uint64_t smem_desc_sw64(uint32_t addr, uint32_t lbo, uint32_t sbo) {
+    uint64_t d = 0;
+    d |= (uint64_t)((addr & 0x3FFFF) >> 4);
+    d |= (uint64_t)((lbo >> 4) & 0x3FFF) << 16;
+    d |= (uint64_t)((sbo >> 4) & 0x3FFF) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)4 << 61;                          // layout type: SWIZZLE_64B
+    return d;
+}
 // Same, layout type SWIZZLE_128B_BASE32B (32-byte swizzle chunks inside the 128-byte span, atoms of 4 rows): the only
 // MN-major layout for 32-bit (tf32) operands.
 __device__ __forceinline__ uint64_t smem_desc_sw128_base32(uint32_t addr, uint32_t lbo, uint32_t sbo) {
