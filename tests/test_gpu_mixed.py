@@ -303,6 +303,34 @@ def test_graph_replay_equals_plain_launches(mode):
     ctx.destroy()
 
 
+@pytest.mark.parametrize("mode", [hb.HPRMAT_FP64, hb.HPRMAT_MIXED_REFINE, hb.HPRMAT_TYPE3])
+@pytest.mark.parametrize("graphs", [1, 0])
+def test_programmatic_dependent_launch_changes_nothing(mode, graphs):
+    """The small kernels of the LU and the solves are launched with programmatic stream serialisation (launch_pdl): each may
+    start its prologue while its predecessor drains and waits (griddepcontrol.wait) before its first global access.  Same
+    kernels, same order, same data: R must be bit-identical with the attribute on and off, replayed from graphs or launched
+    plainly, over repeated solves (a kernel that read its input before the predecessor's writes landed would differ)."""
+    w = make_workload(2, nch=12, nb=100)
+    r_ref = None
+    try:
+        for pdl in (0, 1, 1, 0, 1):
+            assert hb.hprmat_profile_pdl(pdl) == pdl
+            ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
+            ctx.set_option(hb.HPRMAT_OPT_GRAPHS, graphs)
+            r, _ = ctx.mesh()
+            V = torch.from_numpy(w.potential(r)).to(DEV)
+            for _ in range(3):
+                R, info = ctx.solve(16.25, V, mode)
+                assert info["status"] == 0
+                got = R.cpu().numpy().copy()
+                if r_ref is None:
+                    r_ref = got
+                assert np.array_equal(got, r_ref)
+            ctx.destroy()
+    finally:
+        hb.hprmat_profile_pdl(1)
+
+
 def test_mixed_matches_fp64_mode_on_the_same_context():
     w = make_workload(2, nch=10, nb=100)
     ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=0)
