@@ -20,9 +20,14 @@ namespace hp {
 
 namespace {
 
-constexpr int TL_G = 256;         // threads of one role: 16 x 16, thread (ti, tj) owns the elements (ti + 16 a, tj + 16 b)
-constexpr int TL_NT = 2 * TL_G;   // two roles advance together, one barrier per column: the factorisation | both inversions
-constexpr int TL_R = TW / 16;
+// Thread grid of one role: TGI x TGJ threads, thread (ti, tj) owns the elements (ti + TGI a, tj + TGJ b): an RA x RB register
+// tile.  8 x 16 threads with 8 x 4 tiles: half the warps of a 16 x 16 grid with 4 x 4 tiles, and the per-column bookkeeping
+// (publishing, barrier, operand loads, predicates) is paid per warp -- the kernel is bound by the issue rate of its one SM
+// (profiles/r02_toplu.md).
+// (profiles/r02_toplu.md).  The complex128 type keeps 16 x 16 threads: two 8 x 4 tiles of double2 do not fit the register file.
+constexpr int TGJ = 16;
+template <class V> struct TopGrid { static constexpr int TGI = 16; };
+template <> struct TopGrid<CView> { static constexpr int TGI = 8; };
 
 // What crosses the roles, double-buffered by column parity
 template <class E> struct TopLuSmem {
@@ -34,7 +39,7 @@ template <class E> struct TopLuSmem {
 };
 
 // One CTA factors the w x w block (w <= TW, padded to TW x TW by the identity) WITHOUT interchanges and inverts both
-// triangular factors, all out of registers: two groups of 256 threads run three rank-1 sweeps in lock step (the
+// triangular factors, all out of registers: two groups of threads run three rank-1 sweeps in lock step (the
 // factorisation in one group, both inversions in the other),
 //   LU:  step j: l_i = a_ij / u_jj (i > j),  a_ic -= l_i u_jc (i, c > j)
 //   XL = inv(L):     rows i > j:  XL[i,:] -= l_i XL[j,:]                (row j of XL is final when step j starts)
@@ -43,44 +48,52 @@ template <class E> struct TopLuSmem {
 // Column j of L and row j of U are exactly what the LU role publishes at step j, so the two inversions ride one step
 // behind the factorisation for free: TW barriers in all instead of 2 TW.
 template <class V>
-__global__ void __launch_bounds__(TL_NT, 1)
+__global__ void __launch_bounds__(2 * TopGrid<V>::TGI * TGJ, 1)
     top_lu_kernel(V A, int w, int c0, int *ipiv, int *info, int *refuted, V dinvL, V dinvU, int *perm, int nbatch) {
     typedef typename V::elem_t E;
     typedef typename V::real_t T;
+    constexpr int TGI = TopGrid<V>::TGI;
+    constexpr int TL_G = TGI * TGJ;   // threads of one role; two roles advance together, one barrier per column
+    constexpr int TL_RA = TW / TGI, TL_RB = TW / TGJ;
+    constexpr int TL_CG = TGI < TGJ ? TGI : TGJ;  // columns per compile-time group: j / TGI and j / TGJ are constant inside it
+    static_assert(TGJ % TGI == 0 || TGI % TGJ == 0, "one grid dimension divides the other");
+    static_assert(TL_G >= TW, "one thread per column writes the interchanges");
     __shared__ TopLuSmem<E> sm;
-    const int role = threadIdx.x / TL_G, lt = threadIdx.x % TL_G, ti = lt & 15, tj = lt >> 4;
+    const int role = threadIdx.x / TL_G, lt = threadIdx.x % TL_G, ti = lt % TGI, tj = lt / TGI;
     const E zero = mk((T)0, (T)0), one = mk((T)1, (T)0);
 
     pdl_wait();
     pdl_trigger();
     // LU role: x = the block.  Inversion role: x = XL, y = Y, both start as the identity
-    E x[TL_R][TL_R], y[TL_R][TL_R];
+    E x[TL_RA][TL_RB], y[TL_RA][TL_RB];
 #pragma unroll
-    for (int a = 0; a < TL_R; ++a)
+    for (int a = 0; a < TL_RA; ++a)
 #pragma unroll
-        for (int b = 0; b < TL_R; ++b) {
-            const int row = ti + 16 * a, col = tj + 16 * b;
+        for (int b = 0; b < TL_RB; ++b) {
+            const int row = ti + TGI * a, col = tj + TGJ * b;
             x[a][b] = (role == 0 && row < w && col < w) ? A.get(row, col) : (row == col ? one : zero);
             y[a][b] = row == col ? one : zero;
         }
     int bad = 0;
-    // JB = j / 16 is compile-time so that the register tiles are statically indexed
-    static_for<0, TL_R>([&](auto jbc) {
-        constexpr int JB = decltype(jbc)::value;
+    // the column group G is compile-time so that the register tiles are statically indexed: JA = j / TGI, JB = j / TGJ
+    static_for<0, TW / TL_CG>([&](auto gc) {
+        constexpr int G = decltype(gc)::value;
+        constexpr int JA = G * TL_CG / TGI, JB = G * TL_CG / TGJ;
 #pragma unroll 1
-        for (int jj = 0; jj < 16; ++jj) {
-            const int j = 16 * JB + jj, par = j & 1;
+        for (int jj = 0; jj < TL_CG; ++jj) {
+            const int j = TL_CG * G + jj, par = j & 1;
+            const int oi = j % TGI, oj = j % TGJ;  // thread coordinates of the owners of row j / column j
             // ---- publish (owners only)
             if (role == 0) {
-                if (ti == jj) {  // row j of U; finished columns read as zero
+                if (ti == oi) {  // row j of U; finished columns read as zero
 #pragma unroll
-                    for (int b = JB; b < TL_R; ++b) sm.rowb[par][tj + 16 * b] = (tj + 16 * b > j) ? x[JB][b] : zero;
+                    for (int b = JB; b < TL_RB; ++b) sm.rowb[par][tj + TGJ * b] = (tj + TGJ * b > j) ? x[JA][b] : zero;
                 }
-                if (tj == jj) {  // column j, not yet divided by the pivot; finished rows read as zero
+                if (tj == oj) {  // column j, not yet divided by the pivot; finished rows read as zero
 #pragma unroll
-                    for (int a = JB; a < TL_R; ++a) sm.colb[par][ti + 16 * a] = (ti + 16 * a > j) ? x[a][JB] : zero;
-                    if (ti == jj) {  // the pivot itself: every thread inverts it on its own (no serial step behind one thread)
-                        const E pv = x[JB][JB];
+                    for (int a = JA; a < TL_RA; ++a) sm.colb[par][ti + TGI * a] = (ti + TGI * a > j) ? x[a][JB] : zero;
+                    if (ti == oi) {  // the pivot itself: every thread inverts it on its own (no serial step behind one thread)
+                        const E pv = x[JA][JB];
                         sm.invp[j] = pv;
                         if (pv.x == (T)0 && pv.y == (T)0) {
                             atomicCAS(info, 0, c0 + j + 1);
@@ -88,16 +101,16 @@ __global__ void __launch_bounds__(TL_NT, 1)
                         }
                     }
                 }
-            } else if (ti == jj) {  // rows j of XL and of Y: non-zero in columns <= j only
+            } else if (ti == oi) {  // rows j of XL and of Y: non-zero in columns <= j only
 #pragma unroll
                 for (int b = 0; b <= JB; ++b) {
-                    sm.xlrow[par][tj + 16 * b] = x[JB][b];
-                    sm.yrow[par][tj + 16 * b] = y[JB][b];
+                    sm.xlrow[par][tj + TGJ * b] = x[JA][b];
+                    sm.yrow[par][tj + TGJ * b] = y[JA][b];
                 }
             }
             __syncthreads();
             // 1 / u_jj = conj(u_jj) / |u_jj|^2: the entries of these blocks are O(1) (S = I + coupling-sized terms), so the
-            // squared modulus cannot overflow; one reciprocal + one Newton step, identical in every thread
+            // squared modulus cannot overflow; one reciprocal + two Newton steps, identical in every thread
             E ip;
             {
                 const E pv = sm.invp[j];
@@ -108,43 +121,42 @@ __global__ void __launch_bounds__(TL_NT, 1)
                 ip = mk(pv.x * r, -pv.y * r);
             }
             if (role == 0) {
-                E l[TL_R], u[TL_R];
+                // a_ic -= a_ij (u_jc / u_jj): the row is scaled (TL_RB products per thread) rather than the column (TL_RA)
+                E cj[TL_RA], u[TL_RB];
 #pragma unroll
-                for (int a = JB; a < TL_R; ++a) l[a] = cmul_packed(sm.colb[par][ti + 16 * a], ip);
+                for (int a = JA; a < TL_RA; ++a) cj[a] = sm.colb[par][ti + TGI * a];
 #pragma unroll
-                for (int b = JB; b < TL_R; ++b) u[b] = sm.rowb[par][tj + 16 * b];
+                for (int b = JB; b < TL_RB; ++b) u[b] = cmul_packed(sm.rowb[par][tj + TGJ * b], ip);
 #pragma unroll
-                for (int a = JB; a < TL_R; ++a)
+                for (int a = JA; a < TL_RA; ++a)
 #pragma unroll
-                    for (int b = JB; b < TL_R; ++b) x[a][b] = cfnma_packed(x[a][b], l[a], u[b]);
-                if (tj == jj) {  // keep the multipliers
-#pragma unroll
-                    for (int a = JB; a < TL_R; ++a)
-                        if (ti + 16 * a > j) x[a][JB] = l[a];
-                }
+                    for (int b = JB; b < TL_RB; ++b) x[a][b] = cfnma_packed(x[a][b], cj[a], u[b]);
+                // (column j itself is left as a_ij^(j): its u[] entry is zero.  The multipliers l_i = a_ij / u_jj are formed
+                // once, after the sweep -- inside it they would be extra work for the one warp every column waits for.)
             } else {
                 // rows i > j:  XL[i,:] -= l_i XL[j,:]  and  Y[i,:] -= u_ji (Y[j,:] / u_jj);  Y's row j takes its 1/u_jj
-                E la[TL_R], ua[TL_R], xr[TL_R], yr[TL_R];
+                // (l_i = a_ij / u_jj: the 1 / u_jj goes onto row j of XL, JB + 1 products per thread instead of TL_RA)
+                E la[TL_RA], ua[TL_RA], xr[TL_RB], yr[TL_RB];
 #pragma unroll
-                for (int a = JB; a < TL_R; ++a) {
-                    la[a] = cmul_packed(sm.colb[par][ti + 16 * a], ip);
-                    ua[a] = sm.rowb[par][ti + 16 * a];
+                for (int a = JA; a < TL_RA; ++a) {
+                    la[a] = sm.colb[par][ti + TGI * a];
+                    ua[a] = sm.rowb[par][ti + TGI * a];
                 }
 #pragma unroll
                 for (int b = 0; b <= JB; ++b) {
-                    xr[b] = sm.xlrow[par][tj + 16 * b];
-                    yr[b] = cmul_packed(sm.yrow[par][tj + 16 * b], ip);
+                    xr[b] = cmul_packed(sm.xlrow[par][tj + TGJ * b], ip);
+                    yr[b] = cmul_packed(sm.yrow[par][tj + TGJ * b], ip);
                 }
 #pragma unroll
-                for (int a = JB; a < TL_R; ++a)
+                for (int a = JA; a < TL_RA; ++a)
 #pragma unroll
                     for (int b = 0; b <= JB; ++b) {
                         x[a][b] = cfnma_packed(x[a][b], la[a], xr[b]);
                         y[a][b] = cfnma_packed(y[a][b], ua[a], yr[b]);
                     }
-                if (ti == jj) {
+                if (ti == oi) {
 #pragma unroll
-                    for (int b = 0; b <= JB; ++b) y[JB][b] = yr[b];
+                    for (int b = 0; b <= JB; ++b) y[JA][b] = yr[b];
                 }
             }
         }
@@ -152,21 +164,35 @@ __global__ void __launch_bounds__(TL_NT, 1)
     // ---- results
     if (role == 0) {
 #pragma unroll
-        for (int a = 0; a < TL_R; ++a)
+        for (int b = 0; b < TL_RB; ++b) {
+            const int col = tj + TGJ * b;
+            E ipc;  // 1 / u_cc, as in the sweep (sm.invp is complete: the last column's barrier has passed)
+            {
+                const E pv = sm.invp[col];
+                const T den = pv.x * pv.x + pv.y * pv.y;
+                T r = den > (T)0 ? rcp_approx(den) : (T)0;
+                r = r * ((T)2 - den * r);
+                r = r * ((T)2 - den * r);
+                ipc = mk(pv.x * r, -pv.y * r);
+            }
 #pragma unroll
-            for (int b = 0; b < TL_R; ++b) {
-                const int row = ti + 16 * a, col = tj + 16 * b;
-                if (row > col && !(cabs1(x[a][b]) <= (T)0.5)) bad = 1;  // every multiplier, once; also catches NaN
+            for (int a = 0; a < TL_RA; ++a) {
+                const int row = ti + TGI * a;
+                if (row > col) {
+                    x[a][b] = cmul_packed(x[a][b], ipc);                   // the multiplier l_row,col
+                    if (!(cabs1(x[a][b]) <= (T)0.5)) bad = 1;              // every multiplier, once; also catches NaN
+                }
                 if (row < w && col < w) A.set(row, col, x[a][b]);
             }
+        }
         if (lt < w) ipiv[c0 + lt] = c0 + lt + 1;              // identity interchanges
         if (lt < nbatch) perm[(size_t)lt * PERM_STRIDE] = 0;  // empty swap batches
     } else {
 #pragma unroll
-        for (int a = 0; a < TL_R; ++a)
+        for (int a = 0; a < TL_RA; ++a)
 #pragma unroll
-            for (int b = 0; b < TL_R; ++b) {
-                const int row = ti + 16 * a, col = tj + 16 * b;
+            for (int b = 0; b < TL_RB; ++b) {
+                const int row = ti + TGI * a, col = tj + TGJ * b;
                 if (row < w && col < w) {
                     dinvL.set(row, col, x[a][b]);
                     dinvU.set(col, row, y[a][b]);  // inv(U) = Y^T
@@ -217,7 +243,7 @@ template <class V> int block_panel(cudaStream_t st, int n, V A, int c0, int w, i
         const bool prof = prof_enabled();
         if (prof) prof_begin(st, 0.0);
         auto kern = top_lu_kernel<V>;
-        HP_CUDA(launch_pdl(kern, dim3(1), dim3(TL_NT), 0, st, A.sub(c0, c0), w, c0, ipiv, info_dev, wk.refuted, dl, du,
+        HP_CUDA(launch_pdl(kern, dim3(1), dim3(2 * TopGrid<V>::TGI * TGJ), 0, st, A.sub(c0, c0), w, c0, ipiv, info_dev, wk.refuted, dl, du,
                            wk.perm + (size_t)b0 * PERM_STRIDE, nbatch));
         if (prof) prof_end(st);
         HP_LAUNCHED();
