@@ -35,8 +35,19 @@ template <class E> struct TopLuSmem {
     E rowb[2][TW];   // row j of U, columns <= j zeroed                           (LU role -> LU, Y)
     E xlrow[2][TW];  // row j of XL = inv(L)                                       (XL role -> XL)
     E yrow[2][TW];   // row j of Y = inv(U)^T, not yet scaled by 1/u_jj            (Y role -> Y)
-    E invp[TW];      // the pivots u_jj, from the owner of the diagonal element
+    E ipv[TW];       // 1 / u_jj, from the owner of the diagonal element (formed one column ahead, see the sweep)
 };
+
+// 1 / pv = conj(pv) / |pv|^2: the entries of these blocks are O(1) (S = I + coupling-sized terms), so the squared modulus
+// cannot overflow; one approximate reciprocal + two Newton steps.  A zero pivot gives zero (reported by the caller).
+template <class E> __device__ __forceinline__ E top_pivot_recip(E pv) {
+    typedef typename real_of<E>::type T;
+    const T den = pv.x * pv.x + pv.y * pv.y;
+    T r = den > (T)0 ? rcp_approx(den) : (T)0;
+    r = r * ((T)2 - den * r);
+    r = r * ((T)2 - den * r);
+    return mk(pv.x * r, -pv.y * r);
+}
 
 // One CTA factors the w x w block (w <= TW, padded to TW x TW by the identity) WITHOUT interchanges and inverts both
 // triangular factors, all out of registers: two groups of threads run three rank-1 sweeps in lock step (the
@@ -75,6 +86,13 @@ __global__ void __launch_bounds__(2 * TopGrid<V>::TGI * TGJ, 1)
             y[a][b] = row == col ? one : zero;
         }
     int bad = 0;
+    if (role == 0 && lt == 0) {  // the first pivot's reciprocal; every later one is formed at the end of the step before it
+        sm.ipv[0] = top_pivot_recip(x[0][0]);
+        if (x[0][0].x == (T)0 && x[0][0].y == (T)0) {
+            atomicCAS(info, 0, c0 + 1);
+            bad = 1;
+        }
+    }
     // the column group G is compile-time so that the register tiles are statically indexed: JA = j / TGI, JB = j / TGJ
     static_for<0, TW / TL_CG>([&](auto gc) {
         constexpr int G = decltype(gc)::value;
@@ -92,14 +110,6 @@ __global__ void __launch_bounds__(2 * TopGrid<V>::TGI * TGJ, 1)
                 if (tj == oj) {  // column j, not yet divided by the pivot; finished rows read as zero
 #pragma unroll
                     for (int a = JA; a < TL_RA; ++a) sm.colb[par][ti + TGI * a] = (ti + TGI * a > j) ? x[a][JB] : zero;
-                    if (ti == oi) {  // the pivot itself: every thread inverts it on its own (no serial step behind one thread)
-                        const E pv = x[JA][JB];
-                        sm.invp[j] = pv;
-                        if (pv.x == (T)0 && pv.y == (T)0) {
-                            atomicCAS(info, 0, c0 + j + 1);
-                            bad = 1;
-                        }
-                    }
                 }
             } else if (ti == oi) {  // rows j of XL and of Y: non-zero in columns <= j only
 #pragma unroll
@@ -109,17 +119,7 @@ __global__ void __launch_bounds__(2 * TopGrid<V>::TGI * TGJ, 1)
                 }
             }
             __syncthreads();
-            // 1 / u_jj = conj(u_jj) / |u_jj|^2: the entries of these blocks are O(1) (S = I + coupling-sized terms), so the
-            // squared modulus cannot overflow; one reciprocal + two Newton steps, identical in every thread
-            E ip;
-            {
-                const E pv = sm.invp[j];
-                const T den = pv.x * pv.x + pv.y * pv.y;
-                T r = den > (T)0 ? rcp_approx(den) : (T)0;
-                r = r * ((T)2 - den * r);
-                r = r * ((T)2 - den * r);
-                ip = mk(pv.x * r, -pv.y * r);
-            }
+            const E ip = sm.ipv[j];  // 1 / u_jj
             if (role == 0) {
                 // a_ic -= a_ij (u_jc / u_jj): the row is scaled (TL_RB products per thread) rather than the column (TL_RA)
                 E cj[TL_RA], u[TL_RB];
@@ -133,6 +133,22 @@ __global__ void __launch_bounds__(2 * TopGrid<V>::TGI * TGJ, 1)
                     for (int b = JB; b < TL_RB; ++b) x[a][b] = cfnma_packed(x[a][b], cj[a], u[b]);
                 // (column j itself is left as a_ij^(j): its u[] entry is zero.  The multipliers l_i = a_ij / u_jj are formed
                 // once, after the sweep -- inside it they would be extra work for the one warp every column waits for.)
+                // The next pivot u_{j+1,j+1} is final now.  Its reciprocal is formed here, branch-free on every thread's own
+                // candidate element so that the chain (reciprocal, two Newton steps) overlaps the update above instead of
+                // standing between the next barrier and everybody's first use; the owner publishes it.
+                if (j + 1 < TW) {
+                    constexpr int GN = G + 1 < TW / TL_CG ? G + 1 : G;
+                    constexpr int JAN = GN * TL_CG / TGI, JBN = GN * TL_CG / TGJ;
+                    const E pvn = (jj + 1 < TL_CG) ? x[JA][JB] : x[JAN][JBN];
+                    const E ipn = top_pivot_recip(pvn);
+                    if (ti == (j + 1) % TGI && tj == (j + 1) % TGJ) {
+                        sm.ipv[j + 1] = ipn;
+                        if (pvn.x == (T)0 && pvn.y == (T)0) {
+                            atomicCAS(info, 0, c0 + j + 2);
+                            bad = 1;
+                        }
+                    }
+                }
             } else {
                 // rows i > j:  XL[i,:] -= l_i XL[j,:]  and  Y[i,:] -= u_ji (Y[j,:] / u_jj);  Y's row j takes its 1/u_jj
                 // (l_i = a_ij / u_jj: the 1 / u_jj goes onto row j of XL, JB + 1 products per thread instead of TL_RA)
@@ -166,15 +182,7 @@ __global__ void __launch_bounds__(2 * TopGrid<V>::TGI * TGJ, 1)
 #pragma unroll
         for (int b = 0; b < TL_RB; ++b) {
             const int col = tj + TGJ * b;
-            E ipc;  // 1 / u_cc, as in the sweep (sm.invp is complete: the last column's barrier has passed)
-            {
-                const E pv = sm.invp[col];
-                const T den = pv.x * pv.x + pv.y * pv.y;
-                T r = den > (T)0 ? rcp_approx(den) : (T)0;
-                r = r * ((T)2 - den * r);
-                r = r * ((T)2 - den * r);
-                ipc = mk(pv.x * r, -pv.y * r);
-            }
+            const E ipc = sm.ipv[col];  // 1 / u_cc (complete: the last column's barrier has passed)
 #pragma unroll
             for (int a = 0; a < TL_RA; ++a) {
                 const int row = ti + TGI * a;
