@@ -190,6 +190,18 @@ size_t hprmat_propagate_workspace_bytes(int nch);
 int hprmat_propagate(void *cuda_stream, int nch, double a_lo, double a_hi, const void *R_in, const void *Rsec, void *R_out,
                      int *info_dev, void *workspace, size_t workspace_bytes);
 
+/* hprmat_propagate for callers that may not allocate device memory (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same arguments, same arithmetic and same result, but the workspace is a file-scope
+ * device array of the library (3 MiB, held by every GPU that loads the library until the process exits) instead of a
+ * caller's buffer.  The call itself makes no cudaMalloc / cudaFree and calls no allocating routine.
+ *   nch <= hprmat_propagate_static_max_nch() = 128; a larger nch returns HPRMAT_ENOMEM and hprmat_last_cuda_error() names the
+ *   limit (use hprmat_propagate with a workspace then).
+ * There is ONE array per device, shared by every call and cleared at the start of each: calls whose GPU work can overlap
+ * (different streams, several host threads) RACE on it -- issue them on one stream, or order them with events. */
+int hprmat_propagate_static_max_nch(void);
+int hprmat_propagate_static(void *cuda_stream, int nch, double a_lo, double a_hi, const void *R_in, const void *Rsec,
+                            void *R_out, int *info_dev);
+
 /* Solution block of the last hprmat_solve: X dev, complex N x nch column-major (copy out). */
 int hprmat_get_x(const hprmat_ctx *ctx, void *X);
 

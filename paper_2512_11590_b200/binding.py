@@ -354,6 +354,22 @@ def hprmat_propagate(a_lo, a_hi, R_in, Rsec, info_dev=None, ws=None, stream=None
     return R_out
 
 
+def hprmat_propagate_static_max_nch() -> int:
+    return int(lib().hprmat_propagate_static_max_nch())
+
+
+def hprmat_propagate_static(a_lo, a_hi, R_in, Rsec, R_out, info_dev, stream=None):
+    """hprmat_propagate on the library's static device scratch (no allocation in the call; nch <= 128).  The caller passes
+    every buffer, outputs included: R_out torch complex128 CUDA [nch, nch], info_dev torch int32 CUDA [1]."""
+    nch = R_in.shape[0]
+    rc = lib().hprmat_propagate_static(_stream(stream), C.c_int(nch), C.c_double(a_lo), C.c_double(a_hi), _dev(R_in),
+                                       _dev(Rsec), _dev(R_out), _dev(info_dev))
+    if rc == HPRMAT_ENOMEM:  # beyond the static limit: the library's message names it
+        raise HprmatError(rc, "hprmat_propagate_static [" + lib().hprmat_last_cuda_error().decode() + "]")
+    _check(rc, "hprmat_propagate_static")
+    return R_out
+
+
 def hprmat_zgetrf(n, A, lda, ipiv, info_dev, ws=None, stream=None):
     """In-place FP64 LU; A torch complex128 CUDA holding the column-major n x n matrix (lda >= n)."""
     if ws is None:

@@ -8,6 +8,9 @@
 // With the R-matrix at a_lo, u(a_lo) = a_lo R_in u'(a_lo), eliminating u'(a_lo) gives the R-matrix at a_hi:
 //     a_hi R_out = Rsec_RR - Rsec_RL (Rsec_LL + a_lo R_in)^-1 Rsec_LR.
 // This file does that Nc x Nc algebra on the device with the library's own FP64 LU (lu.cu) and DMMA GEMM (zgemm.cu).
+#include <atomic>
+#include <cstdio>
+
 #include "lu.cuh"
 
 namespace hp {
@@ -69,4 +72,54 @@ extern "C" int hprmat_propagate(void *cuda_stream, int nch, double a_lo, double 
     HP_TRY(getrs<ZView>(st, nch, nch, ZView(M, nch), ZView(Y, nch), wk));
     // R_out <- R_out - (1/a_hi) Rsec_RL Y
     return zgemm(st, nch, nch, nch, -1.0 / a_hi, (const double2 *)Rsec + 2 * nn, nch, Y, nch, 1.0, (double2 *)R_out, nch);
+}
+
+// ---- the same propagation step for callers that may not allocate (code under CUDA-graph capture, serving loops, harnesses
+// that forbid cudaMalloc): the workspace of hprmat_propagate lives in a file-scope device array instead of a caller's buffer.
+// Every GPU that loads the library holds PROP_STATIC_BYTES (3 MiB) until the process exits.  ONE array per device, shared by
+// every call and keeping the last call's contents: calls whose GPU work may overlap (different streams, several host
+// threads) race on it -- serialise them, or use hprmat_propagate with a workspace per call.
+namespace hp {
+namespace {
+constexpr int PROP_STATIC_MAX_NCH = 128;  // = LEAF: the nch x nch LU then keeps no solve-block inverses and forks no side stream
+constexpr size_t PROP_STATIC_BYTES = 3u << 20;
+static __device__ __align__(256) unsigned char g_prop_scratch[PROP_STATIC_BYTES];
+
+// In host code g_prop_scratch is a host-side stand-in, not a device address: the address a kernel may use comes from
+// cudaGetSymbolAddress, asked once per device with that device current.
+std::atomic<void *> g_prop_scratch_addr[32];
+int prop_scratch(void **out) {
+    int dev = 0;
+    HP_CUDA(cudaGetDevice(&dev));
+    const bool tracked = dev >= 0 && dev < 32;
+    void *p = tracked ? g_prop_scratch_addr[dev].load(std::memory_order_acquire) : nullptr;
+    if (!p) {
+        HP_CUDA(cudaGetSymbolAddress(&p, g_prop_scratch));
+        if (tracked) g_prop_scratch_addr[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return 0;
+}
+}  // namespace
+}  // namespace hp
+
+extern "C" int hprmat_propagate_static_max_nch(void) { return PROP_STATIC_MAX_NCH; }
+
+extern "C" int hprmat_propagate_static(void *cuda_stream, int nch, double a_lo, double a_hi, const void *R_in, const void *Rsec,
+                                       void *R_out, int *info_dev) {
+    if (nch < 1) return -2;
+    if (nch > PROP_STATIC_MAX_NCH || hprmat_propagate_workspace_bytes(nch) > PROP_STATIC_BYTES) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err),
+                 "hprmat_propagate_static: nch = %d exceeds the static scratch limit nch <= %d (use hprmat_propagate with a workspace)",
+                 nch, PROP_STATIC_MAX_NCH);
+        return HPRMAT_ENOMEM;
+    }
+    void *scratch = nullptr;
+    HP_TRY(prop_scratch(&scratch));
+    // The array keeps the previous call's contents (possibly of another nch).  The LU clears its own counters, lock words and
+    // verdict word on every call (lu.cu getrf) and M, Y and the pivot table are written before they are read; the whole array
+    // is cleared here all the same (3 MiB, ~2 us on the caller's stream) so that a call's result cannot depend on its
+    // predecessor's leftovers.
+    HP_CUDA(cudaMemsetAsync(scratch, 0, PROP_STATIC_BYTES, (cudaStream_t)cuda_stream));
+    return hprmat_propagate(cuda_stream, nch, a_lo, a_hi, R_in, Rsec, R_out, info_dev, scratch, PROP_STATIC_BYTES);
 }
