@@ -1,4 +1,4 @@
-"""BASELINE.json configs[1] and configs[2] at FULL size, every listed mode, every energy of their sweeps, through ONE context
+"""BASELINE.json configs[1], configs[2] (and configs[4] by certificate, configs[3] against a stored oracle run) at FULL size, every listed mode, every energy of their sweeps, through ONE context
 per mode (the paper's "reuse across the energy scan").  All tests need a B200 ("-m gpu").
 
 What is compared:
@@ -110,3 +110,14 @@ def test_cfg3_headline_size_against_the_stored_oracle_run(mode_name):
     print(f"cfg3 {mode_name}: max|R - R_oracle|/max|R_oracle| = {err:.2e}, {info}")
     assert info["status"] == hb.HPRMAT_OK and err <= tol, (err, info)
     ctx.destroy()
+
+
+@pytest.mark.parametrize("mode_name", ["mixed_refine", "fp64"])
+def test_cfg4_largest_size_certificate(mode_name):
+    """configs[4]: Nc = 512, Nb = 100 (N = 51200, a 42-GB matrix, the largest single-GPU config), E = 30 MeV, both listed modes.
+    The O(N^3) oracle is out of reach at this size (8 x the 57 min of configs[3]); what the oracle CAN compute is its
+    long-double matrix-free residual of the GPU's X (O(Nb^2 Nc^2 + Nb Nc^3)), so the comparison is the a-posteriori
+    certificate of tests/certificate.py: R_exact - R~ = (h2m/a) X~^T r + second-order term, both evaluated by the oracle, and
+    the oracle's backward error of X~ against 50 N 2^-53; plus the symmetry of R (C is complex symmetric)."""
+    _sweep(4, mode_name)
+
