@@ -20,7 +20,9 @@
 //                     swizzle atoms of 8 rows; one TMA box of 32 (K) x BN (N);  SBO = 1024 B between 8-column groups.
 // TMA zero-fills out-of-bounds elements, which takes care of ragged M, N and K edges.
 //
-// CTA = 6 warps: warp 0 TMA producer (one lane), warp 1 TMEM allocator + UMMA issuer (one lane), warps 2-5 epilogue
+// CTA = 10 warps: warp 0 TMA producer (one lane), warp 1 TMEM allocator + UMMA issuer (one lane), warps 2-9 epilogue (two per
+// TMEM lane quarter, half of the tile's columns each: 8 instead of 4 warps is +15-25 % on the k <= 512 updates, whose
+// epilogue loads are latency-bound; 16 is slower again)
 // (each owns the TMEM lane quarter 32*(warp%4)): tcgen05.ld -> beta*C + alpha*acc -> coalesced global stores.
 #include <algorithm>
 
@@ -35,7 +37,8 @@ namespace {
 
 constexpr int CG_BM = 128;   // UMMA M
 constexpr int CG_KC = 32;    // floats of K per stage = one 128-byte swizzle row
-constexpr int CG_NT = 192;
+constexpr int CG_EPI = 8;                 // epilogue warps: two per TMEM lane quarter, each takes half of the tile's columns
+constexpr int CG_NT = 64 + 32 * CG_EPI;
 
 template <int BN> struct CgCfg {
     static constexpr int A_PLANE = CG_BM * CG_KC * 4;               // bytes of one A plane per stage (16 KB)
@@ -140,6 +143,9 @@ __global__ void __launch_bounds__(CG_NT, 1)
     } else {
         const int q = warp & 3;  // TMEM lane quarter this warp may access
         const long row = (long)m0 + 32 * q + lane;
+        constexpr int EG = (CG_EPI / 4) < (BN / 16) ? (CG_EPI / 4) : (BN / 16);   // warps per quarter that have work
+        constexpr int EC = BN / EG;                    // columns per working epilogue warp
+        const int cbeg = ((warp - 2) >> 2) * EC;       // (>= BN for the idle ones: their loops are empty)
         if (nk > 0) {
             mbar_wait(tmem_full, 0);
             tc_fence_after();
@@ -147,7 +153,7 @@ __global__ void __launch_bounds__(CG_NT, 1)
         const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
         const bool row_ok = row < M;
 #pragma unroll 1
-        for (int c0 = 0; c0 < BN; c0 += 16) {
+        for (int c0 = cbeg; c0 < cbeg + EC && c0 < BN; c0 += 16) {
             if (n0 + c0 >= N) break;  // warp-uniform
             uint32_t ar[16], ai[16];
             if (nk > 0) {

@@ -14,8 +14,8 @@
 //     k-step reads 6 KB instead of 8 KB of shared memory per CTA (the 128 x 128 single-CTA tile sits exactly at the
 //     shared-memory operand bandwidth of the tensor core); only the leader CTA issues MMAs, completion is multicast to
 //     both CTAs' barriers.
-// Roles per CTA (6 warps): warp 0 TMA producer (one lane), warp 1 TMEM allocator + MMA issuer (one lane, leader CTA only),
-// warps 2-5 epilogue (each owns the TMEM lane quarter 32*(warp%4)).
+// Roles per CTA (10 warps): warp 0 TMA producer (one lane), warp 1 TMEM allocator + MMA issuer (one lane, leader CTA only),
+// warps 2-9 epilogue (two per TMEM lane quarter 32*(warp%4), half of the tile's columns each).
 // Optional in the epilogue: count the results with |re| + |im| > thr (the multiplier check of the block panel, toplu.cu).
 #include "lu.cuh"
 #include "sm100.cuh"
@@ -31,7 +31,8 @@ namespace {
 
 constexpr int G2_BM = 128;   // rows of C per CTA (UMMA M = 128 * NCTA)
 constexpr int G2_KC = 32;    // floats of K per stage = one 128-byte swizzle row
-constexpr int G2_NT = 192;
+constexpr int G2_EPI = 8;                 // epilogue warps: two per TMEM lane quarter, each takes half of the tile's columns
+constexpr int G2_NT = 64 + 32 * G2_EPI;   // (the epilogue's global loads are latency-bound: bytes in flight scale with its warps)
 constexpr int G2_MAX_WAVES = 256;  // counters of the wave barrier (G2Args::wave_ctr)
 constexpr int G2_TMEM = 512; // BN = 128: two accumulator stages of (Dr | Di) = 2 x 2 x 128 columns; BN = 256: one stage
 
@@ -92,7 +93,7 @@ __global__ void __launch_bounds__(G2_NT, 1)
         }
         for (int a = 0; a < Cfg::ACC; ++a) {
             mbar_init(&tmem_full[a], 1);
-            mbar_init(&tmem_empty[a], 4 * NCTA);  // one arrival per epilogue warp of every CTA of the pair
+            mbar_init(&tmem_empty[a], G2_EPI * NCTA);  // one arrival per epilogue warp of every CTA of the pair
         }
         fence_mbar_init();
     }
@@ -206,6 +207,8 @@ __global__ void __launch_bounds__(G2_NT, 1)
     } else {
         // ================================================================================ epilogue
         const int q = warp & 3;  // TMEM lane quarter this warp may access
+        constexpr int EC = G2_BN / (G2_EPI / 4);       // columns per epilogue warp
+        const int cbeg = ((warp - 2) >> 2) * EC;       // first column of this warp's share
         const uint32_t te0 = NCTA == 2 ? mapa_u32(smem_u32(&tmem_empty[0]), 0) : smem_u32(&tmem_empty[0]);
         int bad = 0;
         int ti = 0;
@@ -221,7 +224,7 @@ __global__ void __launch_bounds__(G2_NT, 1)
             tc_fence_after();
             const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16) + (uint32_t)(a * 2 * G2_BN);
 #pragma unroll 1
-            for (int c0 = 0; c0 < G2_BN; c0 += 16) {
+            for (int c0 = cbeg; c0 < cbeg + EC; c0 += 16) {
                 if (n0 + c0 >= p.N) break;  // warp-uniform
                 uint32_t ar[16], ai[16];
                 if (nk > 0) {
