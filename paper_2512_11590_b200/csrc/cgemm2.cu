@@ -223,24 +223,29 @@ __global__ void __launch_bounds__(G2_NT, 1)
             mbar_wait(&tmem_full[a], aph);
             tc_fence_after();
             const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16) + (uint32_t)(a * 2 * G2_BN);
-#pragma unroll 1
-            for (int c0 = cbeg; c0 < cbeg + EC; c0 += 16) {
+            // the old C values of chunk i + 1 are requested before chunk i is stored: twice the loads in flight per warp
+            float oldr[2][16], oldi[2][16];
+            auto load_old = [&](int c0, float (&orr)[16], float (&oii)[16]) {
+                if (p.beta == 0.f) return;
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const long col = (long)n0 + c0 + j;
+                    const bool ok = row_ok && col < p.N;
+                    orr[j] = ok ? p.Cre[col * p.ldc + row] : 0.f;
+                    oii[j] = ok ? p.Cim[col * p.ldc + row] : 0.f;
+                }
+            };
+            load_old(cbeg, oldr[0], oldi[0]);
+#pragma unroll
+            for (int ci = 0; ci < EC / 16; ++ci) {
+                const int c0 = cbeg + 16 * ci;
                 if (n0 + c0 >= p.N) break;  // warp-uniform
                 uint32_t ar[16], ai[16];
                 if (nk > 0) {
                     tmem_ld16(lane_base + c0, ar);
                     tmem_ld16(lane_base + G2_BN + c0, ai);
                 }
-                float oldr[16], oldi[16];
-                if (p.beta != 0.f) {  // issued before the TMEM wait: both latencies overlap
-#pragma unroll
-                    for (int j = 0; j < 16; ++j) {
-                        const long col = (long)n0 + c0 + j;
-                        const bool ok = row_ok && col < p.N;
-                        oldr[j] = ok ? p.Cre[col * p.ldc + row] : 0.f;
-                        oldi[j] = ok ? p.Cim[col * p.ldc + row] : 0.f;
-                    }
-                }
+                if (ci + 1 < EC / 16) load_old(c0 + 16, oldr[(ci + 1) & 1], oldi[(ci + 1) & 1]);
                 if (nk > 0) {
                     tmem_ld_wait();
                 } else {
@@ -253,8 +258,8 @@ __global__ void __launch_bounds__(G2_NT, 1)
                     if (row_ok && col < p.N) {
                         float vr = p.alpha * __uint_as_float(ar[j]), vi = p.alpha * __uint_as_float(ai[j]);
                         if (p.beta != 0.f) {
-                            vr = fmaf(p.beta, oldr[j], vr);
-                            vi = fmaf(p.beta, oldi[j], vi);
+                            vr = fmaf(p.beta, oldr[ci & 1][j], vr);
+                            vi = fmaf(p.beta, oldi[ci & 1][j], vi);
                         }
                         p.Cre[col * p.ldc + row] = vr;
                         p.Cim[col * p.ldc + row] = vi;
