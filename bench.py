@@ -54,11 +54,12 @@ NCU_TRAFFIC = {
     "fp64": {"bytes": 5.575929e9 + 2.604247e9, "launch": "hprmat_zgemm (3M kernel) m=n=12800 k=1024",
              "algorithmic_bytes": 16.0 * (2 * 12800 * 1024 + 2 * 12800 * 12800),
              "capture": "profiles/r01_ncu_full.md section 5", "commit": "9ed5626 (round 1; zgemm3m.cu unchanged since)"},
-    "tf32": {"bytes": 19.761905e9 + 1.207496e9,
-             "launch": "cgemm2_kernel<2,256> inside the cfg-3 mixed LU: the root trailing update m=n=k=12800",
-             "algorithmic_bytes": 8.0 * (12800 * 12800 + 12800 * 12800 + 2 * 12800 * 12800),
-             "capture": "profiles/r02_cgemm.md section 1 (ncu --set full)", "commit": "493995d",
-             "note": "4.0x algorithmic; the C-stationary minimum for waves of 74 pair tiles of 256 x 256 is 3.4x"},
+    "tf32": {"bytes": 16.272062e9 + 1.012782e9,
+             "launch": "cgemm2_kernel<2,256> inside the cfg-3 mixed LU: the root trailing update m=n=11264, k=14336 "
+                       "(the root splits at a multiple of the 2048 solve block)",
+             "algorithmic_bytes": 8.0 * (2 * 11264 * 14336 + 2 * 11264 * 11264),
+             "capture": "profiles/r02_cgemm.md section 1 (ncu --set full)", "commit": "5cf93af",
+             "note": "3.75x algorithmic; the C-stationary minimum for waves of 74 pair tiles of 256 x 256 is 3.4x"},
 }
 
 _DMMA_PEAK = None
