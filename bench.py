@@ -479,6 +479,18 @@ def main():
             t3.pop("_R")
             line["type3_literal_schur"] = {k: t3[k] for k in ("ms_per_step", "lu_tflops", "stages_ms", "backward_err", "status",
                                                                 "steps", "warmup")}
+            # the paper's use case is an energy scan: several contexts on one GPU, each on its own
+            # host thread and stream, interleave the latency-bound and the tensor-core phases of their factorisations
+            es = [float(w.energies[len(w.energies) // 2]) + 0.25 * k for k in range(8)]
+            sc = {}
+            for nctx in (1, 2, 3):
+                _, sinfos, secs = scan.interleaved_scan(w, es, hb.HPRMAT_MIXED_REFINE, nctx=nctx, warmup=2)
+                assert all(i["status"] == hb.HPRMAT_OK for i in sinfos)
+                sc[f"contexts_{nctx}"] = {"ms_per_energy_point": secs / len(es) * 1e3,
+                                          "tflops_8n3_over_3": lu_flops(N) * len(es) / secs * 1e-12}
+                torch.cuda.empty_cache()
+            line["energy_scan_interleaved"] = {"mode": "mixed_refine", "energies": len(es), "timing": "wall clock around the scan, "
+                                               "contexts set up and warmed before", **sc}
             # the FP64 path as the paper runs it: no refinement at all (the default step above spends one
             # residual + one more pair of triangular solves on verifying the result)
             if args.mode == "fp64":

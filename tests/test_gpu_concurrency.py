@@ -117,3 +117,18 @@ def test_raw_solves_from_two_host_threads():
     assert not errors, errors
     for k in range(2):
         assert np.array_equal(results[k], alone[k]), (k, np.abs(results[k] - alone[k]).max())
+
+
+@pytest.mark.parametrize("mode", [hb.HPRMAT_MIXED_REFINE, hb.HPRMAT_FP64])
+def test_interleaved_scan_equals_the_sequential_scan(mode):
+    """scan.interleaved_scan: the energies of a scan handed out to two contexts on two threads / streams; every R-matrix
+    bit-identical to the one-context scan (each solve is one hprmat_solve, whichever context takes it)."""
+    from paper_2512_11590_b200 import scan
+    w = make_workload(2, nch=14, nb=100)
+    energies = [float(e) for e in w.energies] + [float(e) + 0.37 for e in w.energies]
+    R1, infos1, _ = scan.interleaved_scan(w, energies, mode, nctx=1)
+    R2, infos2, _ = scan.interleaved_scan(w, energies, mode, nctx=2)
+    assert all(i["status"] == hb.HPRMAT_OK for i in infos1 + infos2)
+    assert np.array_equal(R1, R2)
+    assert np.abs(R1).max() > 0
+
