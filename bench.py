@@ -200,6 +200,8 @@ def main():
     ap.add_argument("--no-graphs", action="store_true", help="plain stream launches instead of CUDA-graph replay (A/B)")
     ap.add_argument("--no-pdl", action="store_true",
                     help="launch the small LU kernels without programmatic dependent launch (A/B)")
+    ap.add_argument("--no-lookahead", action="store_true",
+                    help="factor without look-ahead (the deferred part of every trailing update on the main stream; A/B)")
     ap.add_argument("--zgemm-algo", type=int, default=0, choices=[0, 3, 4],
                     help="real decomposition of the complex128 GEMM (3M / 4M); 0 = the library default")
     args = ap.parse_args()
@@ -218,6 +220,8 @@ def main():
         hb.hprmat_profile_cgemm_variant(args.cgemm_variant)
     if args.no_pdl:
         hb.hprmat_profile_pdl(0)
+    if args.no_lookahead:
+        hb.hprmat_profile_lookahead(0)
     full = not args.quick
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -44,6 +44,11 @@ int hprmat_profile_cgemm3_variant(int variant);
  * 1 = on (default), 0 = off, any other value only queries.  Returns the setting in force.  Process-wide; A/B measurements. */
 int hprmat_profile_pdl(int enable);
 
+/* Look-ahead inside the factorisations with verified diagonal pivots (the update of the columns the next panel does not need yet
+ * runs on another stream, under that panel's factorisation): 1 = on (default), 0 = off, any other value only queries.
+ * Returns the setting in force.  Process-wide; A/B measurements. */
+int hprmat_profile_lookahead(int enable);
+
 /* How many launch sequences (factorisations, triangular solves) of the context are replayed from CUDA graphs (captured) and
  * how many had to stay plain stream launches (eager: capture refused).  captured / eager: host, may be NULL. */
 struct hprmat_ctx;

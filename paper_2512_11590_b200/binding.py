@@ -104,6 +104,11 @@ def hprmat_profile_pdl(enable: int = -1) -> int:
     return int(lib().hprmat_profile_pdl(C.c_int(enable)))
 
 
+def hprmat_profile_lookahead(enable: int = -1) -> int:
+    """Look-ahead inside the verified-diagonal factorisations: 1 on (default), 0 off, anything else queries."""
+    return int(lib().hprmat_profile_lookahead(C.c_int(enable)))
+
+
 PROF_CATS = ("lu_gemm", "lu_trsm", "panel", "laswp", "solve", "other")
 
 

@@ -22,6 +22,13 @@
 
 namespace hp {
 
+// SMs a persistent launch leaves free (look-ahead: the deferred update runs beside the next panel's chain of small kernels,
+// which need an SM with free shared memory and TMEM to start at all).  Host-thread-local, set for the duration of the enqueue.
+static thread_local int g_sm_reserve = 0;
+int sm_reserve_in_force() { return g_sm_reserve; }
+ScopedSmReserve::ScopedSmReserve(int sms) : prev(g_sm_reserve) { g_sm_reserve = sms; }
+ScopedSmReserve::~ScopedSmReserve() { g_sm_reserve = prev; }
+
 using namespace sm100;
 
 int make_map(CUtensorMap *map, const float *plane, long rows, long cols, long ld, int box_rows, int box_cols,
@@ -119,11 +126,15 @@ __global__ void __launch_bounds__(G2_NT, 1)
                 if (p.wave_ctr != nullptr && wave > 0) {
                     // Wave barrier: CTA pairs that finish a tile early would otherwise run ahead into the next wave alone and
                     // stream its operands from HBM a second time when the others follow (L2 holds ~100 k-steps of a wave).
-                    // All CTAs that own a tile in this wave are resident (one CTA per SM, grid <= SM count), so this cannot
-                    // deadlock; it costs one L2 round trip per tile of >= 100 us.
+                    // Alone on the GPU all CTAs that own a tile in this wave are resident (one CTA per SM, grid <= SM count); it
+                    // costs one L2 round trip per tile of >= 100 us.
                     const unsigned parts = (unsigned)min(nclusters, ntiles - wave * nclusters) * NCTA;
+                    // The barrier is a traffic optimisation, not a correctness requirement, and it must not be able to hang: when
+                    // another stream's kernels hold SMs (several contexts, look-ahead), part of this grid may not be resident
+                    // yet -- so the wait is bounded (~150 us) and then simply gives up.
                     atomicAdd(&p.wave_ctr[wave], 1u);
-                    while (*(volatile unsigned *)&p.wave_ctr[wave] < parts) {
+                    const long long t_give_up = clock64() + 300000;
+                    while (*(volatile unsigned *)&p.wave_ctr[wave] < parts && clock64() < t_give_up) {
                     }
                 }
                 int tm, tn;
@@ -311,7 +322,7 @@ int launch_cgemm2(cudaStream_t st, int m, int n, int k, float alpha, CView A, CV
     p.chk_thr = chk_thr;
     p.chk_count = chk_count;
     const long ntiles = (long)p.tiles_m * p.tiles_n;
-    const int nclusters = (int)std::min<long>(ntiles, kNumSMs / NCTA);
+    const int nclusters = (int)std::min<long>(ntiles, (kNumSMs - sm_reserve_in_force()) / NCTA);
     const long waves = (ntiles + nclusters - 1) / nclusters;
     p.wave_ctr = nullptr;
     if (wave_ctr != nullptr && waves > 1 && waves <= G2_MAX_WAVES && k >= 1024) {  // long tiles only: the barrier is per tile

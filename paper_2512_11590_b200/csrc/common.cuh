@@ -91,6 +91,7 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory"); }
 #endif
 bool pdl_enabled();  // util.cu (hprmat_profile_pdl)
+bool lookahead_enabled();  // util.cu (hprmat_profile_lookahead)
 template <class... KArgs, class... Args>
 inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
     cudaLaunchConfig_t lc = {};
@@ -115,6 +116,12 @@ struct ScopedZgemmAlgo {
     ~ScopedZgemmAlgo();
 };
 
+int sm_reserve_in_force();  // cgemm2.cu
+struct ScopedSmReserve {
+    int prev;
+    explicit ScopedSmReserve(int sms);
+    ~ScopedSmReserve();
+};
 int cgemm_variant_in_force();  // cgemm.cu (measurement aid: which tcgen05 kernel serves the planar complex64 GEMM)
 
 inline int ceil_div(long a, long b) { return (int)((a + b - 1) / b); }

@@ -62,6 +62,8 @@ struct hprmat_ctx {
     // side stream of the factorisations of this context + its fork/join events
     cudaStream_t side = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    cudaStream_t la_stream[LuWork<ZView>::NLA] = {};   // look-ahead streams / events of the factorisations (lu.cuh)
+    cudaEvent_t la_fork[LuWork<ZView>::NLA] = {}, la_join[LuWork<ZView>::NLA] = {};
     // refinement steps the last solve in each mode took: that many are enqueued before the single read-back of the next
     // solve (index: HPRMAT_FP64 .. HPRMAT_MIXED_REFINE)
     int plan_steps[5] = {0, 1, 0, 2, 0};
@@ -135,6 +137,11 @@ int free_ctx(hprmat_ctx *c) {
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->side) cudaStreamDestroy(c->side);
+    for (int d = 0; d < LuWork<ZView>::NLA; ++d) {
+        if (c->la_fork[d]) cudaEventDestroy(c->la_fork[d]);
+        if (c->la_join[d]) cudaEventDestroy(c->la_join[d]);
+        if (c->la_stream[d]) cudaStreamDestroy(c->la_stream[d]);
+    }
     for (auto &g : c->graphs)
         if (g.exec) cudaGraphExecDestroy(g.exec);
     if (c->cap) cudaStreamDestroy(c->cap);
@@ -368,6 +375,18 @@ static int setup_impl(hprmat_ctx **out, int nch, int nbasis, double a_lo, double
         free_ctx(c);
         return HPRMAT_ECUDA;
     }
+    for (int d = 0; d < LuWork<ZView>::NLA; ++d) {
+        if (cudaStreamCreateWithFlags(&c->la_stream[d], cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->la_fork[d], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->la_join[d], cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
+            free_ctx(c);
+            return HPRMAT_ECUDA;
+        }
+        c->wz.la_stream[d] = c->wc.la_stream[d] = c->la_stream[d];
+        c->wz.la_fork[d] = c->wc.la_fork[d] = c->la_fork[d];
+        c->wz.la_join[d] = c->wc.la_join[d] = c->la_join[d];
+    }
     for (LuWork<ZView> *w : {&c->wz}) { w->side = c->side; w->ev_fork = c->ev_fork; w->ev_join = c->ev_join; w->refuted = c->d_info + IN_REFUTED; }
     for (LuWork<CView> *w : {&c->wc}) { w->side = c->side; w->ev_fork = c->ev_fork; w->ev_join = c->ev_join; w->refuted = c->d_info + IN_REFUTED; }
     {   // ||B||_inf of the surface right-hand sides, read by the backward-error kernel from device memory
@@ -520,6 +539,7 @@ template <class F> int replay(hprmat_ctx *c, int kind, int flags, const void *ke
     flags |= zgemm_algo_in_force() << 16;  // the captured sequence holds the kernels of this decomposition ...
     flags |= cgemm_variant_in_force() << 20;  // ... and of this complex64 GEMM kernel
     flags |= (pdl_enabled() ? 1 : 0) << 24;   // ... launched with or without programmatic dependent launch
+    flags |= (lookahead_enabled() ? 1 : 0) << 25;  // ... with or without look-ahead forks
     hprmat_ctx::GraphEntry *ent = nullptr;
     for (auto &g : c->graphs)
         if (g.kind == kind && g.flags == flags && g.key == key) ent = &g;

@@ -51,10 +51,16 @@ template <class V> size_t LuWork<V>::carve(void *base, int n_) {
     if (n > LEAF) {
         binvL = alloc_view<V>(p, sbld, (long)ceil_div(n, SB) * sbld);
         binvU = alloc_view<V>(p, sbld, (long)ceil_div(n, SB) * sbld);
-        tmp = alloc_view<V>(p, sbld, std::max<long>(n, 256));
+        tmp_cols = std::max<long>(n, 256);
+        tmp = alloc_view<V>(p, sbld, tmp_cols);
+    }
+    la_cols = 0;
+    if (n >= LA_MIN_N) {
+        la_cols = round_up(n / 2, 256);
+        for (int d = 0; d < NLA; ++d) la_tmp[d] = alloc_view<V>(p, sbld, la_cols);
     }
     refuted = (int *)take(256);
-    wave_sync = (unsigned *)take(sizeof(unsigned) * 8 * 256);
+    wave_sync = (unsigned *)take(sizeof(unsigned) * (8 + 4 * NLA) * 256);
     perm = (int *)take(sizeof(int) * (size_t)nblk * PERM_STRIDE);
     cand_val = (T *)take(sizeof(T) * 2 * MAXG);
     cand_row = (int *)take(sizeof(int) * 2 * MAXG);
@@ -345,7 +351,7 @@ static int lu_gemm(const LuWork<CView> &wk, cudaStream_t st, int m, int n, int k
                    CView C) {
     if (wk.accurate) return cgemm3_any(st, m, n, k, alpha, A, B, beta, C);
     LuWork<CView> &w = const_cast<LuWork<CView> &>(wk);
-    unsigned *slot = w.wave_sync ? w.wave_sync + 256 * (w.wave_next++ & 7) : nullptr;
+    unsigned *slot = w.wave_sync ? w.wave_sync + 256 * (w.wave_base + (w.wave_next++ & w.wave_mask)) : nullptr;
     return cgemm_ws(st, m, n, k, alpha, A, B, beta, C, slot);
 }
 template <class V> struct IsPlanar { static constexpr bool value = false; };
@@ -355,7 +361,7 @@ template <> struct IsPlanar<CView> { static constexpr bool value = true; };
 // has its LEAF-diagonal blocks zeroed; those are applied from the dinv table with the 3xTF32 kernel.
 template <class V>
 static int big_leaf(cudaStream_t st, const V &binv, const V *dtab, int d0, int s, V B, int ncols, LuWork<V> &wk, bool acc) {
-    const long cap = std::max<long>(wk.n, 256);
+    const long cap = wk.tmp_cols;
     for (long c = 0; c < ncols; c += cap) {
         const int nc = (int)std::min<long>(cap, ncols - c);
         V Bc = B.sub(0, c), T = wk.tmp;
@@ -387,7 +393,7 @@ static int gemm_sel(bool acc, cudaStream_t st, int m, int n, int k, double alpha
 // the side stream, concurrently with leaf products of the main stream that own the scratch.  cfg 1: 53.4 -> 50.5 ms per step,
 // cfg 3: 1318 -> 1306 ms.
 static int leaf_product(bool acc, cudaStream_t st, int s, int ncols, ZView dinv, ZView B, LuWork<ZView> &wk) {
-    if (wk.use_big && wk.tmp.p && s > 64 && ncols > 32 && ncols <= std::max<long>(wk.n, 256)) {
+    if (wk.use_big && wk.tmp.p && s > 64 && ncols > 32 && ncols <= wk.tmp_cols) {
         HP_TRY(gemm(st, s, ncols, s, 1.0, dinv, B, 0.0, wk.tmp));
         return copy_block(st, wk.tmp, B, s, ncols);
     }
@@ -488,24 +494,58 @@ template <class V> static int build_binv(cudaStream_t st, V A, int c0, int s, Lu
     return rc;
 }
 
-template <class V> static int getrf_rec(cudaStream_t st, int n, V A, int c0, int c1, int *ipiv, int *info_dev, LuWork<V> &wk) {
+// pending: an event the RIGHT part of this node (the columns right of its left child) has to wait for -- the parent's
+// look-ahead update of exactly those columns, running on another stream.  depth: look-ahead streams 0 .. depth - 1 may have
+// work in flight, so this node and its sub-tree fork on stream `depth` and deeper.
+template <class V>
+static int getrf_rec(cudaStream_t st, int n, V A, int c0, int c1, int *ipiv, int *info_dev, LuWork<V> &wk,
+                     cudaEvent_t pending = nullptr, int depth = 0) {
     const int w = c1 - c0;
-    if (wk.speculate && w <= TW) {
-        ProfCat pc(PROF_PANEL);
-        return block_panel<V>(st, n, A, c0, w, ipiv, info_dev, wk, dinv_of(wk.dinvL, c0, w), dinv_of(wk.dinvU, c0, w));
+    if ((wk.speculate && w <= TW) || w <= IB) {
+        if (pending) HP_CUDA(cudaStreamWaitEvent(st, pending, 0));  // (not reached: look-ahead needs a node to wait in)
+        if (wk.speculate) {
+            ProfCat pc(PROF_PANEL);
+            return block_panel<V>(st, n, A, c0, w, ipiv, info_dev, wk, dinv_of(wk.dinvL, c0, w), dinv_of(wk.dinvU, c0, w));
+        }
+        return panel(st, n, A, c0, w, ipiv, info_dev, wk);
     }
-    if (w <= IB) return panel(st, n, A, c0, w, ipiv, info_dev, wk);
     const int h = split<V>(w), mid = c0 + h;
-    HP_TRY(getrf_rec(st, n, A, c0, mid, ipiv, info_dev, wk));
+    HP_TRY(getrf_rec(st, n, A, c0, mid, ipiv, info_dev, wk, nullptr, pending ? depth + 1 : depth));
+    if (pending) HP_CUDA(cudaStreamWaitEvent(st, pending, 0));
+    // the right child's own left child spans [mid, mid + hr): only those columns are needed next
+    const int wr = c1 - mid;
+    const bool right_is_node = !((wk.speculate && wr <= TW) || wr <= IB);
+    const int hr = right_is_node ? split<V>(wr) : wr;
+    const bool ahead = IsPlanar<V>::value && wk.speculate && lookahead_enabled() && w <= LA_MAX_W && depth < LuWork<V>::NLA && wk.la_stream[depth] != nullptr &&
+                       wk.la_cols > 0 && right_is_node && wr - hr >= LA_MIN_COLS && wr - hr <= wk.la_cols && !prof_enabled();
+    const int now = ahead ? hr : wr;
     {
         ProfCat pc(PROF_LU_TRSM);
-        HP_TRY(trsm_lower(st, A, c0, h, A.sub(c0, mid), c1 - mid, wk));
+        HP_TRY(trsm_lower(st, A, c0, h, A.sub(c0, mid), now, wk));
     }
     {
         ProfCat pc(PROF_LU_GEMM);
-        HP_TRY(lu_gemm(wk, st, n - mid, c1 - mid, h, -1.0, A.sub(mid, c0), A.sub(c0, mid), 1.0, A.sub(mid, mid)));
+        HP_TRY(lu_gemm(wk, st, n - mid, now, h, -1.0, A.sub(mid, c0), A.sub(c0, mid), 1.0, A.sub(mid, mid)));
     }
-    HP_TRY(getrf_rec(st, n, A, mid, c1, ipiv, info_dev, wk));
+    cudaEvent_t join = nullptr;
+    if (ahead) {
+        // the rest of the update, under the factorisation of [mid, mid + hr): its own scratch, its own wave-barrier slots
+        cudaStream_t sl = wk.la_stream[depth];
+        HP_TRY(stream_follow(st, sl, wk.la_fork[depth]));
+        LuWork<V> ws = wk;
+        ws.tmp = wk.la_tmp[depth];
+        ws.tmp_cols = wk.la_cols;
+        ws.wave_base = 8 + 4 * depth;
+        ws.wave_mask = 3;
+        ws.wave_next = 0;
+        const int later = wr - hr;
+        ScopedSmReserve reserve(LA_SM_RESERVE);
+        HP_TRY(trsm_lower(sl, A, c0, h, A.sub(c0, mid + hr), later, ws));
+        HP_TRY(lu_gemm(ws, sl, n - mid, later, h, -1.0, A.sub(mid, c0), A.sub(c0, mid + hr), 1.0, A.sub(mid, mid + hr)));
+        join = wk.la_join[depth];
+        HP_CUDA(cudaEventRecord(join, sl));
+    }
+    HP_TRY(getrf_rec(st, n, A, mid, c1, ipiv, info_dev, wk, join, depth));
     // the node's diagonal block is final: keep its inverse for the triangular solves further up / in getrs
     if (w <= LEAF) HP_TRY(inv_double(st, A, c0, h, w, wk));
     if (is_big_block<V>(n, c0, w)) HP_TRY(build_binv(st, A, c0, w, wk));

@@ -16,6 +16,13 @@ constexpr int NLEV = 3;       // inverted diagonal blocks are kept at sizes IB <
 template <class V> struct SolveBlock { static constexpr int value = 1024; };
 template <> struct SolveBlock<CView> { static constexpr int value = 2048; };
 constexpr int MAXG = kNumSMs; // CTAs of the cooperative panel kernel (one per SM)
+constexpr int LA_MIN_N = 4096;  // smallest matrix whose factorisation looks ahead (LuWork::la_*)
+constexpr int LA_SM_RESERVE = 40;  // SMs the deferred update's persistent GEMMs leave to the panel chain (8 .. 64 measured:
+                                  // 117.8, 117.1, 116.1, 116.5, 114.4, 115.0, 116.5 ms per step at configs[3]; off: 120.3)
+constexpr int LA_MAX_W = 32768;   // widest node that looks ahead: beyond, the deferred GEMM is so long that running it on 108 SMs
+                                  // costs more than the overlap returns (configs[4] root, w = 51200: +17 ms; below: neutral there,
+                                  // -3.4 ms at configs[3]).  complex64 only: the FP64 GEMMs are not persistent and gain nothing.
+constexpr int LA_MIN_COLS = 512; // smallest deferred column range worth a fork / join
 constexpr int TW = 64;        // width of the block panel of a factorisation with verified diagonal pivots (toplu.cu): its top
                               // block is factored and inverted by one CTA out of registers and shared memory
 
@@ -54,9 +61,20 @@ template <class V> struct LuWork {
     V binvL, binvU;      // inverses of the SB-aligned diagonal blocks (of size min(SB, n - b SB) > LEAF), ld = sbld, block b at
                          // column offset b*sbld; for the complex64 type getrf leaves their LEAF-diagonal blocks zeroed
                          // (the solves apply those from dinvL/dinvU[NLEV-1] with the 3xTF32 kernel)
-    V tmp;               // sbld x max(n, 256) scratch: out-of-place leaf product
+    V tmp;               // sbld x tmp_cols scratch: out-of-place leaf product
+    long tmp_cols = 0;   // = max(n, 256) for the workspace's own scratch
     long sbld = 0;
-    unsigned *wave_sync = nullptr;  // 8 x 256 words: wave-barrier counters of the persistent complex64 GEMM (cgemm2.cu), one
+    // Look-ahead of the factorisations WITHOUT interchanges (speculate): at a node of the recursion the update of the columns the
+    // right child does not need yet (everything right of ITS left child) runs on another stream, under the factorisation of that
+    // left child, whose chains of small dependent kernels leave most SMs idle.  Nested NLA deep: one stream, one event pair and
+    // one scratch per level (device scratch: carve; host resources: set by the owner of the workspace, null = no look-ahead).
+    static constexpr int NLA = 3;
+    V la_tmp[NLA];       // sbld x la_cols each (n >= LA_MIN_N only)
+    long la_cols = 0;
+    cudaStream_t la_stream[NLA] = {nullptr, nullptr, nullptr};
+    cudaEvent_t la_fork[NLA] = {nullptr, nullptr, nullptr}, la_join[NLA] = {nullptr, nullptr, nullptr};
+    int wave_base = 0, wave_mask = 7;  // this (copy of the) workspace's share of the wave-barrier slots
+    unsigned *wave_sync = nullptr;  // (8 + 4 NLA) x 256 words: wave-barrier counters of the persistent complex64 GEMM (cgemm2.cu), one
     int wave_next = 0;              // slot per deep trailing update in flight (host-side round robin)
     int *refuted = nullptr;    // device counter: multipliers that refuted the diagonal-pivot speculation (toplu.cu); zeroed by getrf
     bool speculate = false;    // host-side: the matrix is expected to pivot on its diagonal (S = K_d^-1 (C - E I)): factor

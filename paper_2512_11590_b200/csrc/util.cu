@@ -11,6 +11,8 @@ thread_local char g_cuda_err[256] = "";
 std::atomic<long long> g_launches{0};
 static std::atomic<bool> g_pdl{true};
 bool pdl_enabled() { return g_pdl.load(std::memory_order_relaxed); }
+static std::atomic<bool> g_lookahead{true};
+bool lookahead_enabled() { return g_lookahead.load(std::memory_order_relaxed); }
 
 // ---- optional per-launch timing of the GEMM kernel (bench.py's roofline leg): one CUDA-event pair around every launch
 struct ProfRec { cudaEvent_t a, b; double flops; int cat; };
@@ -88,5 +90,9 @@ extern "C" const char *hprmat_last_cuda_error(void) { return hp::g_cuda_err; }
 extern "C" int hprmat_profile_pdl(int enable) {
     if (enable == 0 || enable == 1) hp::g_pdl.store(enable != 0, std::memory_order_relaxed);
     return hp::pdl_enabled() ? 1 : 0;
+}
+extern "C" int hprmat_profile_lookahead(int enable) {
+    if (enable == 0 || enable == 1) hp::g_lookahead.store(enable != 0, std::memory_order_relaxed);
+    return hp::lookahead_enabled() ? 1 : 0;
 }
 extern "C" long long hprmat_launch_count(void) { return hp::g_launches.load(); }

@@ -331,6 +331,40 @@ def test_programmatic_dependent_launch_changes_nothing(mode, graphs):
         hb.hprmat_profile_pdl(1)
 
 
+@pytest.mark.parametrize("graphs", [1, 0])
+def test_look_ahead_changes_the_schedule_not_the_result(graphs):
+    """Look-ahead (lu.cu getrf_rec): the update of the columns the next panel does not need yet runs on another stream, under that
+    panel's factorisation.  Engages from N = 4096 (configs[1], N = 6400, here).  Same arithmetic per element up to the GEMM
+    tiling of the split update: R agrees with the run without look-ahead to rounding, both meet the oracle-side bar through
+    the refinement, the split shows as extra launches, and repeated solves are bit-identical (no race between the streams)."""
+    w = make_workload(1)
+    mode = hb.HPRMAT_MIXED_REFINE
+    out = {}
+    try:
+        for la in (1, 0):
+            assert hb.hprmat_profile_lookahead(la) == la
+            ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
+            ctx.set_option(hb.HPRMAT_OPT_GRAPHS, graphs)
+            r, _ = ctx.mesh()
+            V = torch.from_numpy(w.potential(r)).to(DEV)
+            E = float(w.energies[3])
+            ctx.solve(E, V, mode)
+            l0 = hb.hprmat_launch_count()
+            Rs = []
+            for _ in range(4):
+                R, info = ctx.solve(E, V, mode)
+                assert info["status"] == 0 and 0 <= info["backward_err"] <= 50 * w.n * 2.0 ** -53
+                Rs.append(R.cpu().numpy().copy())
+            out[la] = (Rs[0], (hb.hprmat_launch_count() - l0) // 4)
+            for Rk in Rs[1:]:
+                assert np.array_equal(Rk, Rs[0])
+            ctx.destroy()
+    finally:
+        hb.hprmat_profile_lookahead(1)
+    assert out[1][1] > out[0][1], (out[1][1], out[0][1])          # the split updates are there
+    assert _relmax(out[1][0], out[0][0]) <= 1e-11
+
+
 def test_mixed_matches_fp64_mode_on_the_same_context():
     w = make_workload(2, nch=10, nb=100)
     ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=0)
