@@ -330,6 +330,10 @@ def main():
                                          "tf32_nominal_1125": ach / 1125.0}),
                     "breakdown_ms": {k: round(v["ms"], 3) for k, v in cats.items()},
                     "breakdown_launches": {k: v["launches"] for k, v in cats.items()}}
+            if roof["frac"] > 1.0:
+                roof["frac_note"] = ("above 1: the denominator is half of cuBLAS's SUSTAINED bf16 rate (power-limited, back to back "
+                                     "for seconds), which this TF32 kernel's launches inside the step exceed; it is not a hardware "
+                                     "ceiling -- see frac_of_other_peaks for the burst-derived and the nominal figure")
 
         info = infos[-1]
         res = {"mode": mode_name, "value": world * lu_flops(N) / sec_per_step * 1e-12, "ms_per_step": sec_per_step * 1e3,
