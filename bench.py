@@ -53,7 +53,7 @@ def peaks():
 NCU_TRAFFIC = {
     "fp64": {"bytes": 5.575929e9 + 2.604247e9, "launch": "hprmat_zgemm (3M kernel) m=n=12800 k=1024",
              "algorithmic_bytes": 16.0 * (2 * 12800 * 1024 + 2 * 12800 * 12800),
-             "capture": "profiles/r01_ncu_full.md section 5", "commit": "9ed5626 (round 1; zgemm3m.cu unchanged since)"},
+             "capture": "profiles/r01_ncu_full.md section 5", "commit": "9ed5626 (round 1; zgemm3m.cu has only gained the programmatic-dependent-launch prologue since)"},
     "tf32": {"bytes": 16.272062e9 + 1.012782e9,
              "launch": "cgemm2_kernel<2,256> inside the cfg-3 mixed LU: the root trailing update m=n=11264, k=14336 "
                        "(the root splits at a multiple of the 2048 solve block)",
