@@ -179,6 +179,24 @@ def test_rmatrix_mixed_refine_parity(cfg, nch, nb):
     ctx.destroy()
 
 
+@pytest.mark.parametrize("mode,tol", [(hb.HPRMAT_MIXED_REFINE, 1e-10), (hb.HPRMAT_FP64, 1e-10), (hb.HPRMAT_MIXED, 1e-3)])
+def test_ragged_size_above_the_look_ahead_threshold(mode, tol):
+    """Nc = 43, Nb = 97: N = 4171, just above the size from which the complex64 factorisation looks ahead (4096) and keeps
+    2048-column solve blocks, with every block ragged (97-row channels, a 75-column tail): R and X against the full oracle."""
+    w = make_workload(1, nch=43, nb=97)
+    assert w.n == 4171
+    ctx = hb.Context(w.nch, w.nb, w.a, w.h2m, w.lval, w.ethr, max_mode=1 << mode)
+    r, _ = ctx.mesh()
+    V = torch.from_numpy(w.potential(r)).to(DEV)
+    E = float(w.energies[1])
+    R, info = ctx.solve(E, V, mode)
+    Ro, Xo = _oracle_R(w, E)
+    assert info["status"] == 0, info
+    assert _relmax(_host(R), Ro) <= tol, (info, _relmax(_host(R), Ro))
+    assert _relmax(_host(ctx.get_x()), Xo) <= (1e-9 if mode != hb.HPRMAT_MIXED else 1e-2)
+    ctx.destroy()
+
+
 @pytest.mark.parametrize("cfg,nch,nb", MIXED_CASES)
 def test_rmatrix_mixed_norefine_parity(cfg, nch, nb):
     """north_star: mixed path without refinement <= 1e-3 in R-matrix elements (the paper's cross-section level)."""
