@@ -16,7 +16,8 @@
 // but truncate.
 //
 // CTA = 10 warps: warp 0 TMA producer, warp 1 TMEM allocator + UMMA issuer, warps 2-5 epilogue, warps 6-9 splitters.
-// Tile 128 x 128, K step 16, three stages of (A, B, A_lo, B_lo) = 3 x 64 KB.  (N = 128 halves the shared-memory reads per
+// PERSISTENT: one CTA per SM walks the rasterised tile sequence; two accumulator stages in TMEM, so the epilogue of a tile
+// overlaps the main loop of the next.  Tile 128 x 128, K step 16, three stages of (A, B, A_lo, B_lo) = 3 x 64 KB.  (N = 128 halves the shared-memory reads per
 // flop of the 128 x 64 version, which was bound by them: 150 -> see DESIGN.md section 8.)
 #include <atomic>
 
@@ -39,7 +40,8 @@ constexpr int X3_HALF = 2 * X3_A_PLANE + 2 * X3_B_PLANE;      // 32 KB: the TMA-
 constexpr int X3_STAGE = 2 * X3_HALF;                         // + the lo tiles
 constexpr int X3_STAGES = 3;
 constexpr int X3_SMEM = X3_STAGES * X3_STAGE + 1024 + 256;
-constexpr int X3_TMEM = 2 * X3_BN;                            // Dr | Di
+constexpr int X3_ACC = 2;                                     // accumulator stages (Dr | Di each) in TMEM
+constexpr int X3_TMEM = X3_ACC * 2 * X3_BN;                   // all 512 columns
 
 struct X3Maps {
     CUtensorMap a_re, a_im, b_re, b_im;
@@ -60,13 +62,13 @@ __global__ void __launch_bounds__(X3_NT, 1)
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + X3_STAGES * X3_STAGE);
     uint64_t *split = full + X3_STAGES;
     uint64_t *empty = split + X3_STAGES;
-    uint64_t *tmem_full = empty + X3_STAGES;
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tmem_full + 1);
+    uint64_t *tmem_full = empty + X3_STAGES;   // [X3_ACC]
+    uint64_t *tmem_empty = tmem_full + X3_ACC;  // [X3_ACC]
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tmem_empty + X3_ACC);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    int tm, tn;
-    raster((int)blockIdx.x, (M + X3_BM - 1) / X3_BM, (N + X3_BN - 1) / X3_BN, 12, tm, tn);
-    const int m0 = tm * X3_BM, n0 = tn * X3_BN;
+    const int tiles_m = (M + X3_BM - 1) / X3_BM, tiles_n = (N + X3_BN - 1) / X3_BN;
+    const int ntiles = tiles_m * tiles_n;
     const int nk = (K + X3_KC - 1) / X3_KC;
 
     if (warp == 0 && lane == 0) {
@@ -79,7 +81,10 @@ __global__ void __launch_bounds__(X3_NT, 1)
             mbar_init(&split[s], 4);   // one arrival per splitter warp
             mbar_init(&empty[s], 1);
         }
-        mbar_init(tmem_full, 1);
+        for (int a = 0; a < X3_ACC; ++a) {
+            mbar_init(&tmem_full[a], 1);
+            mbar_init(&tmem_empty[a], 4);  // one arrival per epilogue warp
+        }
         fence_mbar_init();
     }
     if (warp == 1) tmem_alloc<X3_TMEM>(tmem_slot);
@@ -87,119 +92,169 @@ __global__ void __launch_bounds__(X3_NT, 1)
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    pdl_wait();
+    pdl_trigger();
 
+    // Persistent: every CTA walks the rasterised tile sequence blockIdx.x, + gridDim.x, ...; the shared-memory ring runs on
+    // across tiles (iteration counter `it`), the accumulators alternate between the two halves of TMEM so that the epilogue
+    // of one tile overlaps the main loop of the next.
     if (warp == 0) {
         if (lane == 0) {
-            for (int kt = 0; kt < nk; ++kt) {
-                const int s = kt % X3_STAGES;
-                const uint32_t ph = (kt / X3_STAGES) & 1;
-                mbar_wait(&empty[s], ph ^ 1);
-                mbar_expect_tx(&full[s], X3_HALF);
-                unsigned char *st = smem + s * X3_STAGE;
-                const int k0 = kt * X3_KC;
+            long it = 0;
+            for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+                int tm, tn;
+                raster(t, tiles_m, tiles_n, 12, tm, tn);
+                const int m0 = tm * X3_BM, n0 = tn * X3_BN;
+                for (int kt = 0; kt < nk; ++kt, ++it) {
+                    const int s = (int)(it % X3_STAGES);
+                    const uint32_t ph = (uint32_t)(it / X3_STAGES) & 1;
+                    mbar_wait(&empty[s], ph ^ 1);
+                    mbar_expect_tx(&full[s], X3_HALF);
+                    unsigned char *st = smem + s * X3_STAGE;
+                    const int k0 = kt * X3_KC;
 #pragma unroll
-                for (int c = 0; c < X3_BM / 32; ++c) {
-                    tma_load_2d(st + c * (X3_KC * 128), &maps.a_re, &full[s], m0 + 32 * c, k0);
-                    tma_load_2d(st + X3_A_PLANE + c * (X3_KC * 128), &maps.a_im, &full[s], m0 + 32 * c, k0);
+                    for (int c = 0; c < X3_BM / 32; ++c) {
+                        tma_load_2d(st + c * (X3_KC * 128), &maps.a_re, &full[s], m0 + 32 * c, k0);
+                        tma_load_2d(st + X3_A_PLANE + c * (X3_KC * 128), &maps.a_im, &full[s], m0 + 32 * c, k0);
+                    }
+                    tma_load_2d(st + 2 * X3_A_PLANE, &maps.b_re, &full[s], k0, n0);
+                    tma_load_2d(st + 2 * X3_A_PLANE + X3_B_PLANE, &maps.b_im, &full[s], k0, n0);
                 }
-                tma_load_2d(st + 2 * X3_A_PLANE, &maps.b_re, &full[s], k0, n0);
-                tma_load_2d(st + 2 * X3_A_PLANE + X3_B_PLANE, &maps.b_im, &full[s], k0, n0);
             }
         }
     } else if (warp == 1) {
         if (lane == 0) {
             constexpr uint32_t ID = idesc_tf32(X3_BM, X3_BN, 1, 0, 0, 0);
             constexpr uint32_t ID_NEGA = idesc_tf32(X3_BM, X3_BN, 1, 0, 1, 0);
-            const uint32_t d_re = tmem, d_im = tmem + X3_BN;
-            for (int kt = 0; kt < nk; ++kt) {
-                const int s = kt % X3_STAGES;
-                const uint32_t ph = (kt / X3_STAGES) & 1;
-                mbar_wait(&split[s], ph);
+            long it = 0;
+            int ti = 0;
+            for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++ti) {
+                const int a = ti % X3_ACC;
+                const uint32_t aph = (uint32_t)(ti / X3_ACC) & 1;
+                mbar_wait(&tmem_empty[a], aph ^ 1);  // the epilogue of tile ti - X3_ACC has drained this accumulator
                 tc_fence_after();
-                const uint32_t base = smem_u32(smem + s * X3_STAGE);
+                const uint32_t d_re = tmem + (uint32_t)(a * 2 * X3_BN), d_im = d_re + X3_BN;
+                for (int kt = 0; kt < nk; ++kt, ++it) {
+                    const int s = (int)(it % X3_STAGES);
+                    const uint32_t ph = (uint32_t)(it / X3_STAGES) & 1;
+                    mbar_wait(&split[s], ph);
+                    tc_fence_after();
+                    const uint32_t base = smem_u32(smem + s * X3_STAGE);
 #pragma unroll
-                for (int ks = 0; ks < X3_KC / 8; ++ks) {
-                    // part p = 0: hi tiles, 1: lo tiles (same layout X3_HALF further on)
-                    uint64_t dar[2], dai[2], dbr[2], dbi[2];
+                    for (int ks = 0; ks < X3_KC / 8; ++ks) {
+                        // part p = 0: hi tiles, 1: lo tiles (same layout X3_HALF further on)
+                        uint64_t dar[2], dai[2], dbr[2], dbi[2];
 #pragma unroll
-                    for (int p = 0; p < 2; ++p) {
-                        const uint32_t a_re = base + p * X3_HALF, a_im = a_re + X3_A_PLANE;
-                        const uint32_t b_re = a_re + 2 * X3_A_PLANE, b_im = b_re + X3_B_PLANE;
-                        dar[p] = smem_desc_sw128_base32(a_re + ks * 1024, X3_KC * 128, 512);
-                        dai[p] = smem_desc_sw128_base32(a_im + ks * 1024, X3_KC * 128, 512);
-                        dbr[p] = smem_desc_sw64(b_re + ks * 32, 16, 512);
-                        dbi[p] = smem_desc_sw64(b_im + ks * 32, 16, 512);
+                        for (int p = 0; p < 2; ++p) {
+                            const uint32_t a_re = base + p * X3_HALF, a_im = a_re + X3_A_PLANE;
+                            const uint32_t b_re = a_re + 2 * X3_A_PLANE, b_im = b_re + X3_B_PLANE;
+                            dar[p] = smem_desc_sw128_base32(a_re + ks * 1024, X3_KC * 128, 512);
+                            dai[p] = smem_desc_sw128_base32(a_im + ks * 1024, X3_KC * 128, 512);
+                            dbr[p] = smem_desc_sw64(b_re + ks * 32, 16, 512);
+                            dbi[p] = smem_desc_sw64(b_im + ks * 32, 16, 512);
+                        }
+                        // the two small terms first, then hi*hi: (a, b) part pairs (1,0), (0,1), (0,0)
+#pragma unroll
+                        for (int tt = 0; tt < 3; ++tt) {
+                            const int pa = tt == 0 ? 1 : 0, pb = tt == 1 ? 1 : 0;
+                            const uint32_t acc = (kt | ks | tt) ? 1u : 0u;
+                            umma_tf32(d_re, dar[pa], dbr[pb], ID, acc);        // Dr += Ar Br
+                            umma_tf32(d_im, dar[pa], dbi[pb], ID, acc);        // Di += Ar Bi
+                            umma_tf32(d_re, dai[pa], dbi[pb], ID_NEGA, 1u);    // Dr -= Ai Bi
+                            umma_tf32(d_im, dai[pa], dbr[pb], ID, 1u);         // Di += Ai Br
+                        }
                     }
-                    // the two small terms first, then hi*hi: (a, b) part pairs (1,0), (0,1), (0,0)
-#pragma unroll
-                    for (int t = 0; t < 3; ++t) {
-                        const int pa = t == 0 ? 1 : 0, pb = t == 1 ? 1 : 0;
-                        const uint32_t acc = (kt | ks | t) ? 1u : 0u;
-                        umma_tf32(d_re, dar[pa], dbr[pb], ID, acc);        // Dr += Ar Br
-                        umma_tf32(d_im, dar[pa], dbi[pb], ID, acc);        // Di += Ar Bi
-                        umma_tf32(d_re, dai[pa], dbi[pb], ID_NEGA, 1u);    // Dr -= Ai Bi
-                        umma_tf32(d_im, dai[pa], dbr[pb], ID, 1u);         // Di += Ai Br
-                    }
+                    umma_commit(&empty[s]);
                 }
-                umma_commit(&empty[s]);
+                umma_commit(&tmem_full[a]);
             }
-            umma_commit(tmem_full);
         }
     } else if (warp >= 6) {
         // ---- splitters: lo at +X3_HALF from the landed words, 16 bytes at a time
-        const int t = threadIdx.x - 192;  // 0 .. 127
-        for (int kt = 0; kt < nk; ++kt) {
-            const int s = kt % X3_STAGES;
-            const uint32_t ph = (kt / X3_STAGES) & 1;
-            mbar_wait(&full[s], ph);
-            uint4 *hi = reinterpret_cast<uint4 *>(smem + s * X3_STAGE);
-            uint4 *lo = reinterpret_cast<uint4 *>(smem + s * X3_STAGE + X3_HALF);
+        const int tid = threadIdx.x - 192;  // 0 .. 127
+        long it = 0;
+        for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+            for (int kt = 0; kt < nk; ++kt, ++it) {
+                const int s = (int)(it % X3_STAGES);
+                const uint32_t ph = (uint32_t)(it / X3_STAGES) & 1;
+                mbar_wait(&full[s], ph);
+                uint4 *hi = reinterpret_cast<uint4 *>(smem + s * X3_STAGE);
+                uint4 *lo = reinterpret_cast<uint4 *>(smem + s * X3_STAGE + X3_HALF);
 #pragma unroll 4
-            for (int i = t; i < X3_HALF / 16; i += 128) {
-                const uint4 x = hi[i];
-                uint4 l;
-                l.x = split_lo(x.x);
-                l.y = split_lo(x.y);
-                l.z = split_lo(x.z);
-                l.w = split_lo(x.w);
-                lo[i] = l;
+                for (int i = tid; i < X3_HALF / 16; i += 128) {
+                    const uint4 x = hi[i];
+                    uint4 l;
+                    l.x = split_lo(x.x);
+                    l.y = split_lo(x.y);
+                    l.z = split_lo(x.z);
+                    l.w = split_lo(x.w);
+                    lo[i] = l;
+                }
+                fence_proxy_async();  // the UMMAs (async proxy) must see these generic-proxy writes
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&split[s]);
             }
-            fence_proxy_async();  // the UMMAs (async proxy) must see these generic-proxy writes
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&split[s]);
         }
     } else {
         const int q = warp & 3;
-        const long row = (long)m0 + 32 * q + lane;
-        mbar_wait(tmem_full, 0);
-        tc_fence_after();
-        const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
-        const bool row_ok = row < M;
-#pragma unroll 1
-        for (int c0 = 0; c0 < X3_BN; c0 += 16) {
-            if (n0 + c0 >= N) break;
-            uint32_t ar[16], ai[16];
-            if (nk > 0) {
-                tmem_ld16(lane_base + c0, ar);
-                tmem_ld16(lane_base + X3_BN + c0, ai);
-                tmem_ld_wait();
-            } else {
+        int ti = 0;
+        for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++ti) {
+            const int a = ti % X3_ACC;
+            const uint32_t aph = (uint32_t)(ti / X3_ACC) & 1;
+            int tm, tn;
+            raster(t, tiles_m, tiles_n, 12, tm, tn);
+            const int n0 = tn * X3_BN;
+            const long row = (long)tm * X3_BM + 32 * q + lane;
+            const bool row_ok = row < M;
+            mbar_wait(&tmem_full[a], aph);
+            tc_fence_after();
+            const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16) + (uint32_t)(a * 2 * X3_BN);
+            // the old C values of chunk i + 1 are requested before chunk i is stored
+            float oldr[2][16], oldi[2][16];
+            auto load_old = [&](int c0, float (&orr)[16], float (&oii)[16]) {
+                if (beta == 0.f) return;
 #pragma unroll
-                for (int j = 0; j < 16; ++j) ar[j] = ai[j] = 0u;
-            }
+                for (int j = 0; j < 16; ++j) {
+                    const long col = (long)n0 + c0 + j;
+                    const bool ok = row_ok && col < N;
+                    orr[j] = ok ? Cre[col * ldc + row] : 0.f;
+                    oii[j] = ok ? Cim[col * ldc + row] : 0.f;
+                }
+            };
+            load_old(0, oldr[0], oldi[0]);
 #pragma unroll
-            for (int j = 0; j < 16; ++j) {
-                const long col = (long)n0 + c0 + j;
-                if (row_ok && col < N) {
-                    float vr = alpha * __uint_as_float(ar[j]), vi = alpha * __uint_as_float(ai[j]);
-                    if (beta != 0.f) {
-                        vr = fmaf(beta, Cre[col * ldc + row], vr);
-                        vi = fmaf(beta, Cim[col * ldc + row], vi);
+            for (int ci = 0; ci < X3_BN / 16; ++ci) {
+                const int c0 = 16 * ci;
+                if (n0 + c0 >= N) break;  // warp-uniform
+                uint32_t ar[16], ai[16];
+                if (nk > 0) {
+                    tmem_ld16(lane_base + c0, ar);
+                    tmem_ld16(lane_base + X3_BN + c0, ai);
+                }
+                if (ci + 1 < X3_BN / 16) load_old(c0 + 16, oldr[(ci + 1) & 1], oldi[(ci + 1) & 1]);
+                if (nk > 0) {
+                    tmem_ld_wait();
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) ar[j] = ai[j] = 0u;
+                }
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const long col = (long)n0 + c0 + j;
+                    if (row_ok && col < N) {
+                        float vr = alpha * __uint_as_float(ar[j]), vi = alpha * __uint_as_float(ai[j]);
+                        if (beta != 0.f) {
+                            vr = fmaf(beta, oldr[ci & 1][j], vr);
+                            vi = fmaf(beta, oldi[ci & 1][j], vi);
+                        }
+                        Cre[col * ldc + row] = vr;
+                        Cim[col * ldc + row] = vi;
                     }
-                    Cre[col * ldc + row] = vr;
-                    Cim[col * ldc + row] = vi;
                 }
             }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&tmem_empty[a]);
         }
     }
     tc_fence_before();
@@ -226,7 +281,9 @@ int cgemm3x(cudaStream_t st, int m, int n, int k, double alpha, CView A, CView B
     HP_TRY(make_map(&maps.b_im, B.im, kk, n, B.ld, X3_KC, X3_BN, CU_TENSOR_MAP_SWIZZLE_64B));
     const bool prof = prof_enabled() && k > 0;
     if (prof) prof_begin(st, 8.0 * m * n * k);
-    kern<<<ceil_div(m, X3_BM) * ceil_div(n, X3_BN), X3_NT, X3_SMEM, st>>>(maps, m, n, k, (float)alpha, (float)beta, C.re, C.im, C.ld);
+    const long ntiles = (long)ceil_div(m, X3_BM) * ceil_div(n, X3_BN);
+    HP_CUDA(launch_pdl(kern, dim3((unsigned)std::min<long>(ntiles, kNumSMs)), dim3(X3_NT), X3_SMEM, st, maps, m, n, k, (float)alpha,
+                       (float)beta, C.re, C.im, (long)C.ld));
     if (prof) prof_end(st);
     HP_LAUNCHED();
     return 0;
