@@ -342,10 +342,10 @@ static int setup_impl(hprmat_ctx **out, int nch, int nbasis, double a_lo, double
         HP_ALLOC(c->d_Bre, sizeof(float) * c->ldS * nch);
         HP_ALLOC(c->d_Bim, sizeof(float) * c->ldS * nch);
         if (!c->d_Kinv) HP_ALLOC(c->d_Kinv, sizeof(double2) * (size_t)nch * nb * nb);
-        const size_t wb = LuWork<CView>::bytes((int)N);
+        const size_t wb = LuWork<CView>::bytes((int)N, true);
         HP_ALLOC(c->d_workc, wb);
         if (cudaMemsetAsync(c->d_workc, 0, wb, c->st) != cudaSuccess) { free_ctx(c); return HPRMAT_ECUDA; }
-        c->wc.carve(c->d_workc, (int)N);
+        c->wc.carve(c->d_workc, (int)N, true);
         c->wc.speculate = true;  // S = I + K_d^-1 V: the diagonal is the partial-pivoting choice; verified (toplu.cu)
     }
     HP_ALLOC(c->d_X, sizeof(double2) * N * nch);

@@ -32,7 +32,7 @@ template <> CView alloc_view<CView>(char *&p, long rows, long cols) {
     return CView(re, im, rows);
 }
 
-template <class V> size_t LuWork<V>::carve(void *base, int n_) {
+template <class V> size_t LuWork<V>::carve(void *base, int n_, bool look_ahead) {
     char *p = (char *)base;
     n = n_;
     nblk = ceil_div(n, IB);
@@ -55,7 +55,7 @@ template <class V> size_t LuWork<V>::carve(void *base, int n_) {
         tmp = alloc_view<V>(p, sbld, tmp_cols);
     }
     la_cols = 0;
-    if (n >= LA_MIN_N) {
+    if (look_ahead && n >= LA_MIN_N) {
         la_cols = round_up(n / 2, 256);
         for (int d = 0; d < NLA; ++d) la_tmp[d] = alloc_view<V>(p, sbld, la_cols);
     }
@@ -70,9 +70,9 @@ template <class V> size_t LuWork<V>::carve(void *base, int n_) {
     slots = (unsigned long long *)take(sizeof(unsigned long long) * LL_WORDS);
     return (size_t)(p - (char *)base);
 }
-template <class V> size_t LuWork<V>::bytes(int n) {
+template <class V> size_t LuWork<V>::bytes(int n, bool look_ahead) {
     LuWork<V> tmp;
-    return tmp.carve((void *)0, n);
+    return tmp.carve((void *)0, n, look_ahead);
 }
 
 // ------------------------------------------------------------------------------------------------- row interchanges

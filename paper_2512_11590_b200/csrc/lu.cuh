@@ -96,9 +96,10 @@ template <class V> struct LuWork {
     unsigned bar_base = 0; // host-side running value of the grid-barrier counter
     unsigned long long *slots = nullptr; // epoch-tagged exchange words of the register-resident panel kernel (lu.cu)
     unsigned ep_base = 0;  // host-side running column count (epoch base) of that kernel
-    static size_t bytes(int n);
+    // look_ahead: also carve the scratch of the look-ahead levels (la_tmp; contexts' complex64 workspace only)
+    static size_t bytes(int n, bool look_ahead = false);
     // carve from p (must be 256-byte aligned); returns bytes used
-    size_t carve(void *p, int n);
+    size_t carve(void *p, int n, bool look_ahead = false);
 };
 
 constexpr int PERM_STRIDE = 1 + 4 * IB;
