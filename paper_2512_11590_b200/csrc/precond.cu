@@ -27,11 +27,10 @@ __global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const doub
     double2 *out = Kinv + (size_t)c * n * n;
     double2 *rowk = reinterpret_cast<double2 *>(smraw);  // [n] pivot row
     double2 *colk = rowk + n;                            // [n] pivot column
-    int *piv = reinterpret_cast<int *>(colk + n);        // [n]
+    int *piv = reinterpret_cast<int *>(colk + 2 * n);    // [n]  (after rowp, see the sweep)
     double2 *a = use_smem ? reinterpret_cast<double2 *>(piv + ((n + 3) & ~3)) : out;
     __shared__ double red_v[KI_NT / 32];
     __shared__ int red_i[KI_NT / 32];
-    __shared__ int s_p;
 
     for (int idx = tid; idx < n * n; idx += KI_NT) {
         const int i = idx % n, j = idx / n;
@@ -51,8 +50,15 @@ __global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const doub
     }
     __syncthreads();
 
+    // Per step k (the kernel is bound by its instruction count, so the sweep over the matrix is kept branch-free):
+    //  (A) warp-level arg-max of column k, barrier, every thread finishes the reduction itself -> pivot row p;
+    //  (B1) stage old row k, old row p, column k; barrier;  (B2) exchange rows k and p in place and in the staged column; barrier;
+    //  (C) a_ij -= c_i r_j (r_j = pivot row / pv) for every i and every j != k, one multiply-add chain per element with no case
+    //       distinction; the owner of row k then overwrites it with r_j; column k is written separately: -c_i / pv, and 1 / pv
+    //       on the diagonal;  barrier.
+    double2 *rowp = rowk + 2 * n;  // [n] old row p (the pivot row before scaling); rowk: old row k; colk: column k
     for (int k = 0; k < n; ++k) {
-        // pivot search in column k, rows >= k
+        // (A)
         double bv = -1.0;
         int bi = -1;
         for (int i = k + tid; i < n; i += KI_NT) {
@@ -67,43 +73,62 @@ __global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const doub
         }
         if ((tid & 31) == 0) { red_v[tid >> 5] = bv; red_i[tid >> 5] = bi; }
         __syncthreads();
+        bv = red_v[0];
+        bi = red_i[0];
+#pragma unroll
+        for (int w = 1; w < KI_NT / 32; ++w) {
+            const double ov = red_v[w];
+            const int oi = red_i[w];
+            if (ov > bv || (ov == bv && oi >= 0 && (bi < 0 || oi < bi))) { bv = ov; bi = oi; }
+        }
+        const int p = bi < 0 ? k : bi;  // (bi < 0: NaN column; reported as singular below)
         if (tid == 0) {
-            for (int w = 1; w < KI_NT / 32; ++w)
-                if (red_v[w] > bv || (red_v[w] == bv && red_i[w] >= 0 && (bi < 0 || red_i[w] < bi))) { bv = red_v[w]; bi = red_i[w]; }
-            s_p = bi;
-            piv[k] = bi;
+            piv[k] = p;
             if (!(bv > 0.0)) atomicCAS(info, 0, c * n + k + 1);
         }
-        __syncthreads();
-        const int p = s_p;
-        // swap rows k and p, stage the (swapped) pivot row and pivot column
+        // (B1)
         for (int j = tid; j < n; j += KI_NT) {
-            const double2 vk = a[(size_t)j * n + k], vp = a[(size_t)j * n + p];
-            if (p != k) { a[(size_t)j * n + k] = vp; a[(size_t)j * n + p] = vk; }
-            rowk[j] = vp;
+            rowk[j] = a[(size_t)j * n + k];
+            rowp[j] = a[(size_t)j * n + p];
+            colk[j] = a[(size_t)k * n + j];
         }
         __syncthreads();
-        for (int i = tid; i < n; i += KI_NT) colk[i] = a[(size_t)k * n + i];
-        __syncthreads();
-        const double2 pv = rowk[k];
+        const double2 pv = rowp[k];
         const bool sing = (pv.x == 0.0 && pv.y == 0.0);
         const double2 ip = sing ? make_double2(0.0, 0.0) : crecip(pv);
-        __syncthreads();  // everybody has read the pivot
-        for (int j = tid; j < n; j += KI_NT) rowk[j] = cmul(rowk[j], ip);  // the scaled pivot row, once per step
+        // (B2)
+        if (p != k)
+            for (int j = tid; j < n; j += KI_NT) {
+                a[(size_t)j * n + k] = rowp[j];
+                a[(size_t)j * n + p] = rowk[j];
+            }
+        if (tid == 0 && p != k) {  // column k with its entries k and p exchanged
+            colk[p] = rowk[k];
+            colk[k] = rowp[k];
+        }
         __syncthreads();
-        // a[i][j] <- a[i][j] - colk[i] * rowk[j]   for i != k;  row k <- rowk;  column k <- -colk*ip, [k][k] = ip.
-        // 32 rows x 16 columns of threads, each walking the matrix in strides: no division per element
+        // (C) 32 rows x 16 columns of threads; the column-k values of a thread's rows sit in registers
         {
             const int ti = tid & 31, tj = tid >> 5;
+            constexpr int RC = 4;  // rows ti + 32 a, a < RC, cached (covers n <= 128)
+            double2 ck[RC];
+#pragma unroll
+            for (int r = 0; r < RC; ++r) ck[r] = (ti + 32 * r < n) ? colk[ti + 32 * r] : make_double2(0.0, 0.0);
             for (int j = tj; j < n; j += KI_NT / 32) {
-                const double2 rj = rowk[j];
                 double2 *col = a + (size_t)j * n;
-                if (j == k) {
-                    for (int i = ti; i < n; i += 32)
-                        col[i] = (i == k) ? ip : cmul(make_double2(-colk[i].x, -colk[i].y), ip);
-                } else {
-                    for (int i = ti; i < n; i += 32) col[i] = (i == k) ? rj : cfnma(col[i], colk[i], rj);
+                if (j == k) {  // warp-uniform
+                    for (int i = ti; i < n; i += 32) {
+                        const double2 ci = colk[i];
+                        col[i] = (i == k) ? ip : cmul(make_double2(-ci.x, -ci.y), ip);
+                    }
+                    continue;
                 }
+                const double2 rj = cmul(rowp[j], ip);
+#pragma unroll
+                for (int r = 0; r < RC; ++r)
+                    if (ti + 32 * r < n) col[ti + 32 * r] = cfnma(col[ti + 32 * r], ck[r], rj);
+                for (int i = ti + 32 * RC; i < n; i += 32) col[i] = cfnma(col[i], colk[i], rj);
+                if (ti == (k & 31)) col[k] = rj;  // row k, by the thread that has just swept over it: the scaled pivot row
             }
         }
         __syncthreads();
@@ -127,7 +152,7 @@ __global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const doub
 int precond_invert(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double2 *Kinv, int *info_dev,
                    const double2 *W, long ldw) {
     const int n = t.nb;
-    const size_t small = sizeof(double2) * 2 * n + sizeof(int) * ((n + 3) & ~3);
+    const size_t small = sizeof(double2) * 3 * n + sizeof(int) * ((n + 3) & ~3);
     const size_t full = small + sizeof(double2) * (size_t)n * n;
     const int use_smem = full <= 200 * 1024;
     const size_t smem = use_smem ? full : small;
