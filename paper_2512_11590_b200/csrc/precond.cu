@@ -17,18 +17,19 @@ namespace hp {
 // column-major n x n in shared memory when it fits (n <= 118), else in its global output buffer (L2-resident).
 constexpr int KI_NT = 512;
 
+template <bool SMEM>
 __global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const double *__restrict__ hT,
                                                      const double *__restrict__ dg0, const double *__restrict__ ethr,
                                                      double energy, const double2 *__restrict__ V,
                                                      const double2 *__restrict__ W, long ldw, double2 *__restrict__ Kinv,
-                                                     int use_smem, int *info) {
+                                                     int *info) {
     extern __shared__ __align__(16) unsigned char smraw[];
     const int c = blockIdx.x, n = nb, tid = threadIdx.x;
     double2 *out = Kinv + (size_t)c * n * n;
     double2 *rowk = reinterpret_cast<double2 *>(smraw);  // [n] pivot row
     double2 *colk = rowk + n;                            // [n] pivot column
     int *piv = reinterpret_cast<int *>(colk + 2 * n);    // [n]  (after rowp, see the sweep)
-    double2 *a = use_smem ? reinterpret_cast<double2 *>(piv + ((n + 3) & ~3)) : out;
+    double2 *a = SMEM ? reinterpret_cast<double2 *>(piv + ((n + 3) & ~3)) : out;  // compile-time: shared-space accesses
     __shared__ double red_v[KI_NT / 32];
     __shared__ int red_i[KI_NT / 32];
 
@@ -75,8 +76,8 @@ __global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const doub
         __syncthreads();
         bv = red_v[0];
         bi = red_i[0];
-#pragma unroll
-        for (int w = 1; w < KI_NT / 32; ++w) {
+        const int nw = min(KI_NT / 32, (n - k + 31) / 32);  // warps that had rows to look at
+        for (int w = 1; w < nw; ++w) {
             const double ov = red_v[w];
             const int oi = red_i[w];
             if (ov > bv || (ov == bv && oi >= 0 && (bi < 0 || oi < bi))) { bv = ov; bi = oi; }
@@ -95,7 +96,7 @@ __global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const doub
         __syncthreads();
         const double2 pv = rowp[k];
         const bool sing = (pv.x == 0.0 && pv.y == 0.0);
-        const double2 ip = sing ? make_double2(0.0, 0.0) : crecip(pv);
+        const double2 ip = sing ? make_double2(0.0, 0.0) : crecip_fast(pv);
         // (B2)
         if (p != k)
             for (int j = tid; j < n; j += KI_NT) {
@@ -133,20 +134,37 @@ __global__ void __launch_bounds__(KI_NT) kinv_kernel(int nch, int nb, const doub
         }
         __syncthreads();
     }
-    // undo the row interchanges: columns of the inverse, in reverse order
-    for (int k = n - 1; k >= 0; --k) {
-        const int p = piv[k];
-        if (p != k) {
-            for (int i = tid; i < n; i += KI_NT) {
-                const double2 t = a[(size_t)k * n + i];
-                a[(size_t)k * n + i] = a[(size_t)p * n + i];
-                a[(size_t)p * n + i] = t;
+    // undo the row interchanges: columns of the inverse, in reverse order.  In shared memory the exchanges are applied to an
+    // index array (one thread, n steps) and the columns are permuted on their way out; in place otherwise.
+    if (SMEM) {
+        __shared__ int cperm[128];              // the shared-memory path holds n <= 112
+        if (tid == 0) {
+            for (int j = 0; j < n; ++j) cperm[j] = j;
+            for (int k = n - 1; k >= 0; --k) {
+                const int p = piv[k];
+                const int t = cperm[k];
+                cperm[k] = cperm[p];
+                cperm[p] = t;
             }
         }
         __syncthreads();
+        for (int idx = tid; idx < n * n; idx += KI_NT) {
+            const int i = idx % n, j = idx / n;
+            out[idx] = a[(size_t)cperm[j] * n + i];
+        }
+    } else {
+        for (int k = n - 1; k >= 0; --k) {
+            const int p = piv[k];
+            if (p != k) {
+                for (int i = tid; i < n; i += KI_NT) {
+                    const double2 t = a[(size_t)k * n + i];
+                    a[(size_t)k * n + i] = a[(size_t)p * n + i];
+                    a[(size_t)p * n + i] = t;
+                }
+            }
+            __syncthreads();
+        }
     }
-    if (use_smem)
-        for (int idx = tid; idx < n * n; idx += KI_NT) out[idx] = a[idx];
 }
 
 int precond_invert(cudaStream_t st, const StructTables &t, double energy, const double2 *V, double2 *Kinv, int *info_dev,
@@ -154,11 +172,15 @@ int precond_invert(cudaStream_t st, const StructTables &t, double energy, const 
     const int n = t.nb;
     const size_t small = sizeof(double2) * 3 * n + sizeof(int) * ((n + 3) & ~3);
     const size_t full = small + sizeof(double2) * (size_t)n * n;
-    const int use_smem = full <= 200 * 1024;
+    const int use_smem = full <= 200 * 1024 && n <= 128;  // (n <= 128: the kernel's column-permutation table)
     const size_t smem = use_smem ? full : small;
-    static SmemCfg cfg;
-    if (smem > 48 * 1024) HP_TRY(configure_smem(cfg, kinv_kernel, smem));
-    kinv_kernel<<<t.nch, KI_NT, smem, st>>>(t.nch, n, t.hT, t.dg0, t.ethr, energy, V, W, ldw, Kinv, use_smem, info_dev);
+    if (use_smem) {
+        static SmemCfg cfg;
+        if (smem > 48 * 1024) HP_TRY(configure_smem(cfg, kinv_kernel<true>, smem));
+        kinv_kernel<true><<<t.nch, KI_NT, smem, st>>>(t.nch, n, t.hT, t.dg0, t.ethr, energy, V, W, ldw, Kinv, info_dev);
+    } else {
+        kinv_kernel<false><<<t.nch, KI_NT, smem, st>>>(t.nch, n, t.hT, t.dg0, t.ethr, energy, V, W, ldw, Kinv, info_dev);
+    }
     HP_LAUNCHED();
     return 0;
 }
